@@ -1,0 +1,797 @@
+/*
+ * c8ph_oracle.c — CPU ORACLE for the optical-photon hot path of
+ * arxiv/paper_2405_04229 (D. Baack, "Optical Photon Emission in Extended
+ * Airshowers").  P:n below = /root/reference/PAPER.md line n.
+ *
+ * THIS IS TEST INFRASTRUCTURE.  It is a plain, slow, fp64, step-by-step
+ * restatement of what the path computes, written from the paper.  Only
+ * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load it.  It shares no code, header, table or constant
+ * with the CUDA library (paper_2405_04229_b200/csrc); neither includes the
+ * other.  No blocking, fusion or reordering beyond what the cited passages
+ * state; OpenMP only distributes independent track segments over cores.
+ *
+ * Units: m, ns, nm, g/cm^2.  Frame: local Cartesian, origin at the array
+ * centre on the observation level, z up (plane normal parallel to z),
+ * observation plane z = 0 at altitude h_obs a.s.l.; Earth centre at
+ * (0,0,-(R+h_obs)).  Readings of silent / garbled passages are listed in
+ * DESIGN.md ("Readings"); each function cites the passage it follows.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"):
+ *   orc_philox4x32_10   published Random123 known-answer vectors
+ *   orc_cherenkov_yield Frank-Tamm closed form (Eq. 2.4), threshold beta = 1/n
+ *   orc_rodrigues       M D = P, M = M^T = M^-1
+ *   orc_cone_direction  u.P = cos(theta_c), |u| = 1, azimuth uniformity
+ *   orc_straight_line   constant-n ring radius Z tan(theta_c)
+ *   orc_trace           Snell / Bouguer invariants, constant-n limit, R->inf
+ *                       limit, corrected Eq. 3.23 closed form (linear n),
+ *                       brute-force fine-step ray integration
+ *   orc_table_lookup    node values, exactness on bilinear functions
+ *   orc_transmission    single-exponential closed form
+ *   orc_run             photon-count conservation, filter losslessness,
+ *                       ray-sphere analytic cases
+ *   fluorescence / camera (cfg3): isotropy moments, line frequencies,
+ *                       pixel-centre round trip.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_C_M_PER_NS 0.299792458
+#define ORC_ALPHA (1.0 / 137.035999)
+#define ORC_PI 3.14159265358979323846
+
+/* ------------------------------------------------------------------ types */
+typedef struct {
+    int32_t model;            /* 0 homogeneous, 1 planar, 2 spherical */
+    int32_t n_nodes;
+    double n_const_minus_1;   /* homogeneous refractivity */
+    double h0, dh;            /* uniform height grid (Listing 4.1) */
+    const float *refractivity;/* n-1 at the nodes (fp32 input bytes) */
+    const float *overburden;  /* vertical overburden X_v at the nodes [g/cm^2] or NULL */
+    double earth_radius, h_obs;
+    double rayleigh_X, rayleigh_lambda;            /* X_R [g/cm^2] at lambda_R [nm]; 0 = off */
+    double aer_L, aer_H, aer_lambda, aer_angstrom; /* aer_L = 0 => no aerosol */
+} orc_atmosphere;
+
+typedef struct {
+    int32_t n_h, n_zen, n_ch;      /* n_ch = 5: dd, ds, dt, X_slant, tau_aer */
+    int32_t pad;
+    double h_max, zen_max_rad;
+    const float *data;             /* [n_h][n_zen][n_ch], fp32 as stored */
+} orc_table;
+
+typedef struct {
+    const float *x, *y, *z, *dx, *dy, *dz, *len, *beta, *t0, *charge, *edep;
+} orc_segments;
+
+typedef struct {
+    int32_t hist_nx, hist_ny;
+    double hist_x0, hist_y0, hist_cell;
+    int32_t n_tel, cam_enabled;
+    const float *tel_xyzr;         /* [n_tel][4] */
+    double cam_az_deg, cam_el_deg, cam_pix_deg;
+    int32_t cam_rows, cam_cols, n_tbins, pad;
+    double t_ref_ns, t_bin_ns;
+} orc_detector;
+
+enum { ORC_EMIT_CHERENKOV = 0, ORC_EMIT_FLUOR = 1 };
+enum { ORC_TRACE_STRAIGHT = 0, ORC_TRACE_NUMERIC = 1, ORC_TRACE_TABLE = 2 };
+enum { ORC_TRANS_OFF = 0, ORC_TRANS_WEIGHT = 1, ORC_TRANS_ROULETTE = 2 };
+
+typedef struct {
+    int32_t emit, trace, trans;
+    int32_t lv1, lv2, substeps;
+    double lambda_min_nm, lambda_max_nm, bunch_weight;
+    double lv1_margin_rad, lv2_margin_m;
+    double fluor_yield_per_MeV, aim_factor;
+    int32_t n_lines, pad;
+    const float *line_nm, *line_cdf;
+} orc_params;
+
+/* photon status */
+enum { ORC_ST_LANDED = 0, ORC_ST_UPGOING = 1, ORC_ST_LV2 = 2, ORC_ST_TABLE_RANGE = 3,
+       ORC_ST_ROULETTE = 4 };
+
+typedef struct {
+    int64_t seg;                  /* index within the call */
+    int32_t j, status;
+    double x, y, ux, uy, uz, t, lambda_nm, T, weight;
+    double x_line, y_line;        /* straight-line point (before the correction) */
+    int32_t bin, tel, pix, tbin;
+} orc_photon;
+
+enum { ORC_CNT_SEGMENTS = 0, ORC_CNT_SEG_BELOW_THRESHOLD, ORC_CNT_SEG_LV1, ORC_CNT_SEG_EMITTING,
+       ORC_CNT_EMITTED, ORC_CNT_UPGOING, ORC_CNT_LV2, ORC_CNT_TABLE_RANGE, ORC_CNT_ROULETTE,
+       ORC_CNT_LANDED, ORC_CNT_IN_GRID, ORC_CNT_TEL_HIT, ORC_CNT_CAM_HIT, ORC_N_COUNTERS };
+
+/* ------------------------------------------------------------------ O0 RNG
+ * Philox4x32-10, Salmon et al. (the thesis' ref. [66], "counter
+ * based ... easily parallelized ... without losing the deterministic
+ * sequence").  Restated from the published algorithm: ten rounds of two
+ * 32x32->64 multiplications with the round key bumped by Weyl constants. */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* uniform in (0,1): (2m+1) 2^-24 with m the top 23 bits — exactly
+ * representable in fp32 and fp64, so oracle and device start from identical
+ * uniforms (reading R0). */
+double orc_uniform(uint32_t r) { return ((double)(r >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+/* counter = (j, id_lo, id_hi, stream); key = (seed_lo, seed_hi); id = global
+ * segment id; j = 0xFFFFFFFF is the per-segment draw. */
+static void orc_draw(uint64_t seed, uint64_t seg_id, uint32_t j, uint32_t stream, double u[4])
+{
+    uint32_t ctr[4] = { j, (uint32_t)seg_id, (uint32_t)(seg_id >> 32), stream };
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, r[4];
+    orc_philox4x32_10(ctr, key, r);
+    for (int k = 0; k < 4; ++k) u[k] = orc_uniform(r[k]);
+}
+
+/* ------------------------------------------------------------------ A3 n(h)
+ * Listing 4.1: idx = floor(h/step), linear between idx, idx+1.
+ * lookups must not leave the table -> h clamped to the table range. */
+static double table_lerp(const float *data, int32_t n_nodes, double h0, double dh, double h)
+{
+    double f = (h - h0) / dh;
+    if (f < 0.0) f = 0.0;
+    if (f > (double)(n_nodes - 1)) f = (double)(n_nodes - 1);
+    int idx = (int)floor(f);
+    if (idx > n_nodes - 2) idx = n_nodes - 2;
+    double frac = f - idx;
+    return (1.0 - frac) * (double)data[idx] + frac * (double)data[idx + 1];
+}
+
+double orc_refractivity(const orc_atmosphere *atm, double h)
+{
+    if (atm->model == 0) return atm->n_const_minus_1;
+    return table_lerp(atm->refractivity, atm->n_nodes, atm->h0, atm->dh, h);
+}
+
+double orc_overburden(const orc_atmosphere *atm, double h)
+{
+    if (!atm->overburden) return 0.0;
+    return table_lerp(atm->overburden, atm->n_nodes, atm->h0, atm->dh, h);
+}
+
+/* height a.s.l. of a local-frame point (planar h = h_obs + z;
+ * spherical h = |A - C| - R with C = (0,0,-(R+h_obs))). */
+double orc_height(const orc_atmosphere *atm, const double A[3])
+{
+    if (atm->model != 2) return atm->h_obs + A[2];
+    double Rg = atm->earth_radius + atm->h_obs;
+    double zz = A[2] + Rg;
+    return sqrt(A[0] * A[0] + A[1] * A[1] + zz * zz) - atm->earth_radius;
+}
+
+/* ------------------------------------------------------------------ A1 yield
+ * Eq. 2.2-2.4: d2N/dxdlambda = 2 pi alpha z^2 lambda^-2 sin^2(theta),
+ * cos(theta) = 1/(beta n), integrated over [lambda1, lambda2] for a
+ * non-dispersive n; Heaviside threshold of P:316-318 -> max(0, .). */
+double orc_cherenkov_yield(double charge, double len_m, double beta, double n,
+                           double lambda1_nm, double lambda2_nm)
+{
+    double sin2 = 1.0 - 1.0 / (beta * beta * n * n);
+    if (!(sin2 > 0.0)) return 0.0;
+    double inv_l = 1.0 / (lambda1_nm * 1e-9) - 1.0 / (lambda2_nm * 1e-9);
+    return 2.0 * ORC_PI * ORC_ALPHA * charge * charge * len_m * inv_l * sin2;
+}
+
+/* ------------------------------------------------------------------ A9 rotation
+ * 180 deg Euler-Rodrigues rotation about the bisector A = D + P of
+ * D = (0,0,-1) and P: M = 2 A A^T / |A|^2 - 1.  P -> (0,0,1)
+ * makes A -> 0: there M = diag(1,-1,-1) (reading R4). M row-major. */
+void orc_rodrigues(const double P[3], double M[9])
+{
+    double A[3] = { P[0], P[1], P[2] - 1.0 };
+    double a2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
+    if (P[2] > 1.0 - 1e-6 || a2 <= 0.0) {
+        double d[9] = { 1, 0, 0, 0, -1, 0, 0, 0, -1 };
+        memcpy(M, d, sizeof d);
+        return;
+    }
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c)
+            M[3 * r + c] = 2.0 * A[r] * A[c] / a2 - (r == c ? 1.0 : 0.0);
+}
+
+/* local cone vector p = (cos(phi) sin(th), sin(phi) sin(th), -cos(th))
+ * rotated into the particle direction, u = M p. */
+void orc_cone_direction(const double M[9], double cos_th, double sin_th, double phi, double u[3])
+{
+    double p[3] = { cos(phi) * sin_th, sin(phi) * sin_th, -cos_th };
+    for (int r = 0; r < 3; ++r) u[r] = M[3 * r] * p[0] + M[3 * r + 1] * p[1] + M[3 * r + 2] * p[2];
+}
+
+/* ------------------------------------------------------------------ A6 straight line
+ * Eq. 3.3 for the plane z = 0 with the sign fixed (reading R7):
+ * t* = -A_z/u_z, I = A + t* u.  Returns t* (the geometric distance D). */
+double orc_straight_line(const double A[3], const double u[3], double I[3])
+{
+    double t = -A[2] / u[2];
+    I[0] = A[0] + t * u[0];
+    I[1] = A[1] + t * u[1];
+    I[2] = 0.0;
+    return t;
+}
+
+/* ------------------------------------------------------------------ A7 numerical tracing
+ * Layered atmosphere, Snell's law in vector form, Eq. 3.15:
+ *   A2' = A1' + ( sqrt(n2^2 - n1^2 + n1^2 cos^2(a1)) - n1 cos(a1) ) N,
+ * A' = n * direction ("optical length" vector), N = unit normal of the
+ * layer boundary along the direction of travel.  Layers are the cells of the
+ * n(h) table split into `sub` equal sub-layers; each layer is homogeneous
+ * with n taken at its mid height from Listing 4.1 (reading R8).  Planar: the
+ * boundaries are horizontal planes, N = (0,-1).  Spherical: boundaries are
+ * spheres about the Earth centre, N = -r/|r| at the crossing point.
+ * Worked in the 2-D plane of the ray: coordinates (horizontal, up),
+ * spherical origin at the Earth centre.
+ *
+ * in : h_e [m a.s.l.], zenith angle of travel measured from the local
+ *      downward vertical (sin_z, cos_z > 0), target height h_g.
+ * out: [0] horizontal displacement (planar) or Earth-central angle psi (spherical)
+ *      [1] geometric path S  [2] optical path c*T = sum n s  [3] X_slant = int rho ds
+ *      [4] aerosol optical depth at aer_lambda  [5] sin of arrival zenith angle
+ * returns 0, or 1 if the ray never reaches h_g ("no-ground").
+ */
+int orc_trace(const orc_atmosphere *atm, int spherical, double h_e, double sin_z, double cos_z,
+              double h_g, int sub, double out[6])
+{
+    for (int k = 0; k < 6; ++k) out[k] = 0.0;
+    if (sub < 1) sub = 1;
+    const double R = atm->earth_radius;
+    double px = 0.0, py = spherical ? R + h_e : h_e;        /* position */
+    double n_prev = 1.0 + orc_refractivity(atm, h_e);
+    double Ax = n_prev * sin_z, Ay = -n_prev * cos_z;       /* A' = n * direction */
+    double h_cur = h_e;
+    double S = 0, cT = 0, X = 0, tau = 0;
+    const double step = atm->model == 0 ? 1.0e30 : atm->dh / sub;
+    while (h_cur > h_g) {
+        /* next boundary below h_cur on the sub-layer grid */
+        double h_next;
+        if (atm->model == 0) h_next = h_g;
+        else {
+            double g = floor((h_cur - atm->h0) / step);
+            h_next = atm->h0 + g * step;
+            if (!(h_next < h_cur - 1e-9 * step)) h_next = atm->h0 + (g - 1.0) * step;
+            if (h_next < h_g) h_next = h_g;
+        }
+        double n_l = 1.0 + orc_refractivity(atm, 0.5 * (h_cur + h_next));
+        /* boundary normal along the travel direction at the current point */
+        double Nx, Ny;
+        if (spherical) { double r = sqrt(px * px + py * py); Nx = -px / r; Ny = -py / r; }
+        else { Nx = 0.0; Ny = -1.0; }
+        double n1cos = Ax * Nx + Ay * Ny;                    /* n1 cos(a1) */
+        double rad = n_l * n_l - n_prev * n_prev + n1cos * n1cos;
+        if (!(rad > 0.0) || !(n1cos > 0.0)) return 1;        /* total reflection / turning ray */
+        double c = sqrt(rad) - n1cos;
+        Ax += c * Nx; Ay += c * Ny;                          /* Eq. 3.15 */
+        double dx = Ax / n_l, dy = Ay / n_l;                 /* unit direction in the layer */
+        double s;
+        if (spherical) {
+            /* |p + s d| = R + h_next, nearest root, cancellation-free form */
+            double rt = R + h_next;
+            double b = px * dx + py * dy;                    /* < 0 going down */
+            double cc = px * px + py * py - rt * rt;         /* >= 0 */
+            double disc = b * b - cc;
+            if (!(disc >= 0.0) || !(b < 0.0)) return 1;      /* misses the lower shell */
+            s = cc / (-b + sqrt(disc));
+        } else {
+            s = (h_cur - h_next) / (-dy);
+        }
+        double dhl = h_cur - h_next;
+        S += s;
+        cT += n_l * s;
+        X += (orc_overburden(atm, h_next) - orc_overburden(atm, h_cur)) * (s / dhl);
+        if (atm->aer_L > 0.0)
+            tau += (atm->aer_H / atm->aer_L) * (exp(-h_next / atm->aer_H) - exp(-h_cur / atm->aer_H)) * (s / dhl);
+        px += s * dx; py += s * dy;
+        n_prev = n_l;
+        h_cur = h_next;
+    }
+    /* leave the last layer into the medium at the target height */
+    {
+        double n_g = 1.0 + orc_refractivity(atm, h_g);
+        double Nx, Ny;
+        if (spherical) { double r = sqrt(px * px + py * py); Nx = -px / r; Ny = -py / r; }
+        else { Nx = 0.0; Ny = -1.0; }
+        double n1cos = Ax * Nx + Ay * Ny;
+        double rad = n_g * n_g - n_prev * n_prev + n1cos * n1cos;
+        if (!(rad > 0.0)) return 1;
+        double c = sqrt(rad) - n1cos;
+        Ax += c * Nx; Ay += c * Ny;
+        /* sine of the angle between the direction and the local downward vertical */
+        double tx = -Ny, ty = Nx;                            /* horizontal unit vector */
+        out[5] = fabs(Ax * tx + Ay * ty) / n_g;
+    }
+    out[0] = spherical ? atan2(px, py) : px;
+    out[1] = S; out[2] = cT; out[3] = X; out[4] = tau;
+    return 0;
+}
+
+/* ------------------------------------------------------------------ A15 interpolation tracing
+ * a correction table "calculated in advance from the difference
+ * between the swift linear propagation and the slower but more accurate
+ * iterative propagation".  Node (a,b): emission height h_a = a h_max/(n_h-1)
+ * a.s.l., local zenith theta_b = b theta_max/(n_zen-1); value = orc_trace to
+ * the sphere r_g = R + h_obs minus the straight line in the same direction to
+ * the same sphere (readings R9): ch0 dd = r_g (psi_true - psi_line) [m],
+ * ch1 ds = S - S_line [m], ch2 dt = (cT - S_line)/c [ns], ch3 X_slant,
+ * ch4 tau_aer.  h_a <= h_obs -> zeros.  No-ground nodes hold NaN.
+ * Planar model: psi -> horizontal displacement, sphere -> plane.  */
+void orc_build_table(const orc_atmosphere *atm, int n_h, int n_zen, double h_max, double zen_max_rad,
+                     int sub, float *out /* [n_h][n_zen][5] */)
+{
+    const int spherical = atm->model == 2;
+    const double rg = atm->earth_radius + atm->h_obs;
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int a = 0; a < n_h; ++a) {
+        double h = a * h_max / (n_h - 1);
+        for (int b = 0; b < n_zen; ++b) {
+            float *o = out + ((size_t)a * n_zen + b) * 5;
+            double th = b * zen_max_rad / (n_zen - 1);
+            if (h <= atm->h_obs) { for (int k = 0; k < 5; ++k) o[k] = 0.0f; continue; }
+            double r[6];
+            double sz = sin(th), cz = cos(th);
+            if (orc_trace(atm, spherical, h, sz, cz, atm->h_obs, sub, r)) {
+                for (int k = 0; k < 5; ++k) o[k] = NAN;
+                continue;
+            }
+            double S_line, d_line, d_true;
+            if (spherical) {
+                double re = atm->earth_radius + h;
+                double p = re * sz;
+                S_line = re * cz - sqrt(rg * rg - p * p);
+                d_line = rg * (asin(p / rg) - th);
+                d_true = rg * r[0];
+            } else {
+                S_line = (h - atm->h_obs) / cz;
+                d_line = (h - atm->h_obs) * sz / cz;
+                d_true = r[0];
+            }
+            o[0] = (float)(d_true - d_line);
+            o[1] = (float)(r[1] - S_line);
+            o[2] = (float)((r[2] - S_line) / ORC_C_M_PER_NS);
+            o[3] = (float)r[3];
+            o[4] = (float)r[4];
+        }
+    }
+}
+
+/* bilinear lookup, indices clamped to [0, n-2] (P:947 hardware-style linear
+ * interpolation between support points).  Returns 1 (TABLE_RANGE) if the
+ * point is outside the table or the 2x2 stencil touches a no-ground node. */
+int orc_table_lookup(const orc_table *t, double h, double zen, double out[5])
+{
+    if (!(h >= 0.0) || h > t->h_max || !(zen >= 0.0) || zen > t->zen_max_rad) return 1;
+    double f = h / (t->h_max / (t->n_h - 1)), g = zen / (t->zen_max_rad / (t->n_zen - 1));
+    int a = (int)floor(f), b = (int)floor(g);
+    if (a > t->n_h - 2) a = t->n_h - 2;
+    if (b > t->n_zen - 2) b = t->n_zen - 2;
+    double ff = f - a, gg = g - b;
+    int bad = 0;
+    for (int k = 0; k < t->n_ch; ++k) {
+        const float *d = t->data;
+        size_t s = (size_t)t->n_ch;
+        double v00 = d[((size_t)a * t->n_zen + b) * s + k], v01 = d[((size_t)a * t->n_zen + b + 1) * s + k];
+        double v10 = d[((size_t)(a + 1) * t->n_zen + b) * s + k], v11 = d[((size_t)(a + 1) * t->n_zen + b + 1) * s + k];
+        double v = (1 - ff) * ((1 - gg) * v00 + gg * v01) + ff * ((1 - gg) * v10 + gg * v11);
+        if (isnan(v)) bad = 1;
+        if (k < 5) out[k] = v;
+    }
+    return bad;
+}
+
+/* ------------------------------------------------------------------ A12 transmission
+ * P:360-366, P:772-796 with the analytic stand-in of DESIGN.md (R11):
+ * tau = X_slant (lambda_R/lambda)^4 / X_R + tau_aer(lambda_a) (lambda_a/lambda)^angstrom. */
+double orc_transmission(const orc_atmosphere *atm, double x_slant, double tau_aer, double lambda_nm)
+{
+    double tau = 0.0;
+    if (atm->rayleigh_X > 0.0) {
+        double q = atm->rayleigh_lambda / lambda_nm;
+        tau += x_slant * q * q * q * q / atm->rayleigh_X;
+    }
+    if (atm->aer_L > 0.0) tau += tau_aer * pow(atm->aer_lambda / lambda_nm, atm->aer_angstrom);
+    return exp(-tau);
+}
+
+/* ------------------------------------------------------------------ A14 ray / sphere
+ * P:1068 "hitting the bounding sphere": the line I + s u passes within r of c.
+ * Returns 1 and the entry parameter s_in if hit. */
+int orc_ray_sphere(const double I[3], const double u[3], const double c[3], double r, double *s_in)
+{
+    double d[3] = { c[0] - I[0], c[1] - I[1], c[2] - I[2] };
+    double du = d[0] * u[0] + d[1] * u[1] + d[2] * u[2];
+    double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    double m2 = d2 - du * du;
+    if (m2 > r * r) return 0;
+    *s_in = du - sqrt(r * r - m2);
+    return 1;
+}
+
+/* hex camera (cfg3, reading R12): pixel centres
+ * (a,e)_rc = ((c - (cols-1)/2 + (r mod 2)/2) p, (r - (rows-1)/2) p sqrt(3)/2);
+ * nearest centre wins (brute force), must lie within the hexagon's circumradius p/sqrt(3). */
+int orc_camera_pixel(const orc_detector *det, const double u_arr[3])
+{
+    const double d2r = ORC_PI / 180.0;
+    double az = det->cam_az_deg * d2r, el = det->cam_el_deg * d2r, p = det->cam_pix_deg * d2r;
+    /* camera frame: w = optical axis, right = horizontal, up completes it */
+    double w[3] = { cos(el) * cos(az), cos(el) * sin(az), sin(el) };
+    double rgt[3] = { -sin(az), cos(az), 0.0 };
+    double up[3] = { w[1] * rgt[2] - w[2] * rgt[1], w[2] * rgt[0] - w[0] * rgt[2], w[0] * rgt[1] - w[1] * rgt[0] };
+    double v[3] = { -u_arr[0], -u_arr[1], -u_arr[2] };       /* where the photon comes from */
+    double vw = v[0] * w[0] + v[1] * w[1] + v[2] * w[2];
+    if (!(vw > 0.0)) return -1;
+    double a = atan2(v[0] * rgt[0] + v[1] * rgt[1] + v[2] * rgt[2], vw);
+    double e = atan2(v[0] * up[0] + v[1] * up[1] + v[2] * up[2], vw);
+    int best = -1; double bd = 1e300;
+    for (int r = 0; r < det->cam_rows; ++r)
+        for (int c = 0; c < det->cam_cols; ++c) {
+            double ca = (c - 0.5 * (det->cam_cols - 1) + 0.5 * (r % 2)) * p;
+            double ce = (r - 0.5 * (det->cam_rows - 1)) * p * sqrt(3.0) / 2.0;
+            double dd = (a - ca) * (a - ca) + (e - ce) * (e - ce);
+            if (dd < bd) { bd = dd; best = r * det->cam_cols + c; }
+        }
+    if (bd > p * p / 3.0) return -1;
+    return best;
+}
+
+/* ------------------------------------------------------------------ per-segment quantities */
+typedef struct {
+    double A[3], P[3], L, beta, t0, M[9];
+    double n_exp; int64_t n_bunch; int lv1_dropped;
+    /* fluorescence */
+    double aim[3], cos_psi;
+} orc_segprep;
+
+static void norm3(double v[3]) { double n = sqrt(v[0]*v[0]+v[1]*v[1]+v[2]*v[2]); v[0]/=n; v[1]/=n; v[2]/=n; }
+
+/* bounding radius of telescopes and histogram about the array centre (origin) */
+static double array_radius(const orc_detector *det)
+{
+    double r = 0.0;
+    for (int k = 0; k < det->n_tel; ++k) {
+        const float *t = det->tel_xyzr + 4 * k;
+        double d = sqrt((double)t[0]*t[0] + (double)t[1]*t[1] + (double)t[2]*t[2]) + t[3];
+        if (d > r) r = d;
+    }
+    if (det->hist_nx > 0 && det->hist_ny > 0 && !det->cam_enabled) {
+        double xs[2] = { det->hist_x0, det->hist_x0 + det->hist_nx * det->hist_cell };
+        double ys[2] = { det->hist_y0, det->hist_y0 + det->hist_ny * det->hist_cell };
+        for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) {
+            double d = sqrt(xs[i]*xs[i] + ys[j]*ys[j]);
+            if (d > r) r = d;
+        }
+    }
+    return r;
+}
+
+/* a1-a4 for one segment: ingest, LV1, yield, bunch count, rotation. */
+static void prepare_segment(const orc_atmosphere *atm, const orc_detector *det, const orc_params *par,
+                            const orc_table *tab, const orc_segments *sg, int64_t i,
+                            uint64_t seed, uint64_t seg_id, double r_arr, orc_segprep *o)
+{
+    o->A[0] = sg->x[i]; o->A[1] = sg->y[i]; o->A[2] = sg->z[i];
+    o->P[0] = sg->dx[i]; o->P[1] = sg->dy[i]; o->P[2] = sg->dz[i];
+    norm3(o->P);
+    o->L = sg->len[i]; o->beta = sg->beta[i]; o->t0 = sg->t0[i];
+    o->lv1_dropped = 0; o->n_bunch = 0; o->n_exp = 0.0;
+    double mid[3] = { o->A[0] + 0.5*o->L*o->P[0], o->A[1] + 0.5*o->L*o->P[1], o->A[2] + 0.5*o->L*o->P[2] };
+    double h_mid = orc_height(atm, mid);
+    double u_seg[4];
+    orc_draw(seed, seg_id, 0xFFFFFFFFu, 0, u_seg);
+    if (par->emit == ORC_EMIT_CHERENKOV) {
+        double n_mid = 1.0 + orc_refractivity(atm, h_mid);
+        /* O1 (R1): midpoint rule for the height dependence of Eq. 2.2 */
+        o->n_exp = orc_cherenkov_yield(sg->charge[i], o->L, o->beta, n_mid,
+                                       par->lambda_min_nm, par->lambda_max_nm);
+        if (o->n_exp > 0.0 && par->lv1) {
+            /* O10 LV1: Eq. 4.3 with point of interest = array centre widened by the
+             * array's angular radius (options 1/2) and the Cherenkov angle */
+            double d[3] = { -mid[0], -mid[1], -mid[2] };
+            double dist = sqrt(d[0]*d[0] + d[1]*d[1] + d[2]*d[2]);
+            double cosa = (o->P[0]*d[0] + o->P[1]*d[1] + o->P[2]*d[2]) / dist;
+            if (cosa > 1.0) cosa = 1.0;
+            if (cosa < -1.0) cosa = -1.0;
+            double theta_c = acos(fmin(1.0, 1.0 / (o->beta * n_mid)));
+            double ratio = r_arr / dist; if (ratio > 1.0) ratio = 1.0;
+            if (acos(cosa) > theta_c + asin(ratio) + par->lv1_margin_rad) o->lv1_dropped = 1;
+        }
+        orc_rodrigues(o->P, o->M);
+    } else {
+        /* O5 fluorescence: N = Y E_dep Omega/4pi, forced cone about the line to the
+         * pre-corrected aim point ("favors the direction pointing to the experiment ...
+         * number of photons scaled accordingly") */
+        const float *t = det->tel_xyzr;                      /* aperture = telescope 0 */
+        double c[3] = { t[0], t[1], t[2] };
+        double d[3] = { c[0]-mid[0], c[1]-mid[1], c[2]-mid[2] };
+        double dist = sqrt(d[0]*d[0] + d[1]*d[1] + d[2]*d[2]);
+        o->aim[0] = c[0]; o->aim[1] = c[1]; o->aim[2] = c[2];
+        if (tab && par->trace == ORC_TRACE_TABLE) {
+            double dir[3] = { d[0]/dist, d[1]/dist, d[2]/dist };
+            double Rg = atm->earth_radius + atm->h_obs;
+            double rv[3] = { mid[0], mid[1], mid[2] + (atm->model == 2 ? Rg : 0.0) };
+            if (atm->model != 2) { rv[0] = 0; rv[1] = 0; rv[2] = 1; }
+            norm3(rv);
+            double cz = -(dir[0]*rv[0] + dir[1]*rv[1] + dir[2]*rv[2]);
+            double corr[5];
+            double hn = sqrt(dir[0]*dir[0] + dir[1]*dir[1]);
+            if (cz > 0 && hn > 1e-9 && !orc_table_lookup(tab, h_mid, acos(fmin(1.0, cz)), corr)) {
+                o->aim[0] -= corr[0] * dir[0] / hn;
+                o->aim[1] -= corr[0] * dir[1] / hn;
+            }
+        }
+        double rho_aim = par->aim_factor * t[3];
+        double sin_psi = rho_aim / dist; if (sin_psi > 1.0) sin_psi = 1.0;
+        o->cos_psi = sqrt(1.0 - sin_psi * sin_psi);
+        o->n_exp = par->fluor_yield_per_MeV * sg->edep[i] * 0.5 * (1.0 - o->cos_psi);
+    }
+    if (o->n_exp > 0.0 && !o->lv1_dropped)
+        o->n_bunch = (int64_t)floor(o->n_exp / par->bunch_weight + u_seg[0]);   /* R1(iv) */
+}
+
+/* number of bunches each segment emits (used to size the photon buffer) */
+int64_t orc_count(const orc_atmosphere *atm, const orc_detector *det, const orc_params *par,
+                  const orc_table *tab, const orc_segments *sg, int64_t n_seg, int64_t seg_id_base,
+                  uint64_t seed, int64_t *n_bunch /* [n_seg] or NULL */)
+{
+    double r_arr = array_radius(det);
+    int64_t total = 0;
+    #pragma omp parallel for schedule(static) reduction(+:total)
+    for (int64_t i = 0; i < n_seg; ++i) {
+        orc_segprep sp;
+        prepare_segment(atm, det, par, tab, sg, i, seed, (uint64_t)(seg_id_base + i), r_arr, &sp);
+        if (n_bunch) n_bunch[i] = sp.n_bunch;
+        total += sp.n_bunch;
+    }
+    return total;
+}
+
+/* ------------------------------------------------------------------ the whole path
+ * record_mode 0: histogram/counters only; 1: every emitted photon is written
+ * to `photons` at offset[segment] + j (offsets = exclusive prefix sum of
+ * orc_count's n_bunch), with its status. */
+int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params *par,
+            const orc_table *tab, const orc_segments *sg, int64_t n_seg, int64_t seg_id_base,
+            uint64_t seed, double *hist, double *tel_counts, uint64_t *counters,
+            int record_mode, const int64_t *offsets, orc_photon *photons)
+{
+    const double r_arr = array_radius(det);
+    const double Rg = atm->earth_radius + atm->h_obs;
+    const double n_ground = 1.0 + orc_refractivity(atm, atm->h_obs);
+    uint64_t cnt[ORC_N_COUNTERS];
+    memset(cnt, 0, sizeof cnt);
+    int err = 0;
+    if (par->trace == ORC_TRACE_TABLE && !tab) return -1;
+
+    #pragma omp parallel
+    {
+        uint64_t lc[ORC_N_COUNTERS];
+        memset(lc, 0, sizeof lc);
+        #pragma omp for schedule(dynamic, 16)
+        for (int64_t i = 0; i < n_seg; ++i) {
+            orc_segprep sp;
+            uint64_t seg_id = (uint64_t)(seg_id_base + i);
+            prepare_segment(atm, det, par, tab, sg, i, seed, seg_id, r_arr, &sp);
+            lc[ORC_CNT_SEGMENTS]++;
+            if (!(sp.n_exp > 0.0)) { lc[ORC_CNT_SEG_BELOW_THRESHOLD]++; continue; }
+            if (sp.lv1_dropped) { lc[ORC_CNT_SEG_LV1]++; continue; }
+            if (sp.n_bunch <= 0) continue;
+            lc[ORC_CNT_SEG_EMITTING]++;
+            for (int64_t j = 0; j < sp.n_bunch; ++j) {
+                orc_photon ph;
+                memset(&ph, 0, sizeof ph);
+                ph.seg = i; ph.j = (int32_t)j; ph.bin = ph.tel = ph.pix = ph.tbin = -1;
+                ph.weight = par->bunch_weight; ph.T = 1.0;
+                lc[ORC_CNT_EMITTED]++;
+                double u4[4];
+                orc_draw(seed, seg_id, (uint32_t)j, 0, u4);
+                /* O2: random position along the track, particle clock */
+                double s = u4[1] * sp.L;
+                double Ae[3] = { sp.A[0] + s*sp.P[0], sp.A[1] + s*sp.P[1], sp.A[2] + s*sp.P[2] };
+                double t_e = sp.t0 + s / (sp.beta * ORC_C_M_PER_NS);
+                double h_e = orc_height(atm, Ae);
+                double eta_e = orc_refractivity(atm, h_e);
+                double n_e = 1.0 + eta_e;
+                double u[3];
+                if (par->emit == ORC_EMIT_CHERENKOV) {
+                    /* O3: 1/lambda uniform (spectrum ~ 1/lambda^2, Eq. 2.4) */
+                    double il1 = 1.0 / par->lambda_min_nm, il2 = 1.0 / par->lambda_max_nm;
+                    ph.lambda_nm = 1.0 / (il1 - u4[2] * (il1 - il2));
+                    /* O4: Eq. 2.5 — the angle depends on the location */
+                    double cos_th = 1.0 / (sp.beta * n_e);
+                    double sin2 = 1.0 - cos_th * cos_th;
+                    if (sin2 < 0.0) { sin2 = 0.0; cos_th = 1.0; }
+                    orc_cone_direction(sp.M, cos_th, sqrt(sin2), 2.0 * ORC_PI * u4[0], u);
+                } else {
+                    /* O5: wavelength from the discrete line CDF, direction uniform in
+                     * the cone about (aim - A_e); cos(polar) uniform => isotropic density */
+                    int li = 0;
+                    while (li < par->n_lines - 1 && u4[2] >= (double)par->line_cdf[li]) ++li;
+                    ph.lambda_nm = par->line_nm[li];
+                    double ub[4];
+                    orc_draw(seed, seg_id, (uint32_t)j, 1, ub);
+                    double ax[3] = { sp.aim[0]-Ae[0], sp.aim[1]-Ae[1], sp.aim[2]-Ae[2] };
+                    norm3(ax);
+                    double cp = 1.0 - ub[0] * (1.0 - sp.cos_psi);
+                    double spn = sqrt(fmax(0.0, 1.0 - cp * cp));
+                    double phi = 2.0 * ORC_PI * u4[0];
+                    /* orthonormal basis about ax: e1 = normalised (ax x z), e2 = ax x e1 */
+                    double e1[3] = { ax[1], -ax[0], 0.0 };
+                    double e1n = sqrt(e1[0]*e1[0] + e1[1]*e1[1]);
+                    if (e1n < 1e-12) { e1[0] = 1; e1[1] = 0; e1n = 1; }
+                    e1[0] /= e1n; e1[1] /= e1n;
+                    double e2[3] = { ax[1]*e1[2]-ax[2]*e1[1], ax[2]*e1[0]-ax[0]*e1[2], ax[0]*e1[1]-ax[1]*e1[0] };
+                    for (int k = 0; k < 3; ++k) u[k] = cp*ax[k] + spn*(cos(phi)*e1[k] + sin(phi)*e2[k]);
+                }
+                /* O6: discard up-going / horizontal photons */
+                if (u[2] >= -1e-6) { ph.status = ORC_ST_UPGOING; lc[ORC_CNT_UPGOING]++; goto store; }
+                /* O7 straight line to the observation level */
+                double I[3];
+                double D = orc_straight_line(Ae, u, I);
+                ph.x_line = I[0]; ph.y_line = I[1];
+                double hn = sqrt(u[0]*u[0] + u[1]*u[1]);
+                double eh[2] = { 0.0, 0.0 };
+                if (hn >= 1e-9) { eh[0] = u[0]/hn; eh[1] = u[1]/hn; }
+                /* O10 LV2/LV3: on the straight-line point, before the correction */
+                if (par->lv2) {
+                    int keep = 0;
+                    double m = par->lv2_margin_m;
+                    if (det->hist_nx > 0 && !det->cam_enabled) {
+                        double x1 = det->hist_x0 + det->hist_nx*det->hist_cell, y1 = det->hist_y0 + det->hist_ny*det->hist_cell;
+                        if (I[0] >= det->hist_x0 - m && I[0] < x1 + m && I[1] >= det->hist_y0 - m && I[1] < y1 + m) keep = 1;
+                    }
+                    for (int k = 0; k < det->n_tel && !keep; ++k) {
+                        const float *t = det->tel_xyzr + 4*k;
+                        double ddx = I[0]-t[0], ddy = I[1]-t[1];
+                        double reach = t[3] / fabs(u[2]) + m;
+                        if (ddx*ddx + ddy*ddy <= reach*reach) keep = 1;
+                    }
+                    if (!keep) { ph.status = ORC_ST_LV2; lc[ORC_CNT_LV2]++; goto store; }
+                }
+                /* O8/O9 refraction */
+                double dd = 0, dt_ns = 0, x_slant = 0, tau_aer = 0, sin_arr, cos_zen, sin_zen;
+                double rv[3] = { 0, 0, 1 };                  /* local vertical at A_e */
+                if (atm->model == 2) { rv[0] = Ae[0]; rv[1] = Ae[1]; rv[2] = Ae[2] + Rg; norm3(rv); }
+                cos_zen = -(u[0]*rv[0] + u[1]*rv[1] + u[2]*rv[2]);
+                if (cos_zen > 1.0) cos_zen = 1.0;
+                sin_zen = sqrt(fmax(0.0, 1.0 - cos_zen*cos_zen));
+                sin_arr = sin_zen;
+                double delta = 0.0;                          /* rotation of the direction in the ray plane */
+                if (par->trace == ORC_TRACE_STRAIGHT) {
+                    dt_ns = eta_e * D / ORC_C_M_PER_NS;      /* homogeneous: t = t_e + n D / c */
+                    if (atm->model != 0) {
+                        /* straight line through a stratified medium: no delay model beyond n_e */
+                    }
+                } else if (par->trace == ORC_TRACE_NUMERIC) {
+                    double r[6];
+                    if (cos_zen <= 0.0 || orc_trace(atm, atm->model == 2, h_e, sin_zen, cos_zen, atm->h_obs, par->substeps, r)) {
+                        ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store;
+                    }
+                    double d_line, S_line;
+                    if (atm->model == 2) {
+                        double re = atm->earth_radius + h_e, p = re * sin_zen;
+                        S_line = re*cos_zen - sqrt(Rg*Rg - p*p);
+                        d_line = Rg * (asin(p/Rg) - acos(cos_zen));
+                        dd = Rg * r[0] - d_line;
+                    } else {
+                        S_line = (h_e - atm->h_obs) / cos_zen;
+                        d_line = (h_e - atm->h_obs) * sin_zen / cos_zen;
+                        dd = r[0] - d_line;
+                    }
+                    dt_ns = (r[2] - S_line) / ORC_C_M_PER_NS;
+                    x_slant = r[3]; tau_aer = r[4];
+                } else {
+                    double corr[5];
+                    if (cos_zen <= 0.0 || orc_table_lookup(tab, h_e, acos(cos_zen), corr)) {
+                        ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store;
+                    }
+                    dd = corr[0]; dt_ns = corr[2]; x_slant = corr[3]; tau_aer = corr[4];
+                }
+                if (par->trace != ORC_TRACE_STRAIGHT) {
+                    /* arrival direction from the Snell / Bouguer invariant: the direction
+                     * turns in the ray plane by delta = theta_arr - psi_true - theta_z  (R9) */
+                    if (atm->model == 2) {
+                        double re = atm->earth_radius + h_e;
+                        double a_line = re * sin_zen / Rg;
+                        double a_true = n_e * re * sin_zen / (n_ground * Rg);
+                        double psi_line = asin(a_line) - acos(cos_zen);
+                        delta = asin(a_true) - (psi_line + dd / Rg) - acos(cos_zen);
+                    } else {
+                        delta = asin(n_e * sin_zen / n_ground) - acos(cos_zen);
+                    }
+                }
+                /* O11 transmission */
+                if (par->trans != ORC_TRANS_OFF) {
+                    ph.T = orc_transmission(atm, x_slant, tau_aer, ph.lambda_nm);
+                    if (par->trans == ORC_TRANS_ROULETTE) {
+                        if (!(u4[3] < ph.T)) { ph.status = ORC_ST_ROULETTE; lc[ORC_CNT_ROULETTE]++; goto store; }
+                    } else ph.weight = par->bunch_weight * ph.T;
+                }
+                /* landed: corrected position, time, direction */
+                ph.x = I[0] + dd * eh[0];
+                ph.y = I[1] + dd * eh[1];
+                ph.t = t_e + D / ORC_C_M_PER_NS + dt_ns;
+                {
+                    double ua[3] = { u[0], u[1], u[2] };
+                    if (sin_zen > 1e-9 && delta != 0.0) {
+                        double ep[3];
+                        for (int k = 0; k < 3; ++k) ep[k] = (cos_zen*u[k] + rv[k]) / sin_zen;
+                        for (int k = 0; k < 3; ++k) ua[k] = cos(delta)*u[k] + sin(delta)*ep[k];
+                    }
+                    ph.ux = ua[0]; ph.uy = ua[1]; ph.uz = ua[2];
+                }
+                (void)sin_arr;
+                ph.status = ORC_ST_LANDED;
+                lc[ORC_CNT_LANDED]++;
+                /* O12 binning: ground grid */
+                if (det->hist_nx > 0 && !det->cam_enabled) {
+                    double fx = floor((ph.x - det->hist_x0) / det->hist_cell);
+                    double fy = floor((ph.y - det->hist_y0) / det->hist_cell);
+                    if (fx >= 0 && fx < det->hist_nx && fy >= 0 && fy < det->hist_ny) {
+                        ph.bin = (int32_t)fy * det->hist_nx + (int32_t)fx;
+                        lc[ORC_CNT_IN_GRID]++;
+                        if (hist) {
+                            #pragma omp atomic
+                            hist[ph.bin] += ph.weight;
+                        }
+                    }
+                }
+                /* O12 telescopes: brute force over all spheres; earliest entry, then lowest k */
+                {
+                    double Ip[3] = { ph.x, ph.y, 0.0 }, ua[3] = { ph.ux, ph.uy, ph.uz };
+                    double best = 1e300;
+                    for (int k = 0; k < det->n_tel; ++k) {
+                        const float *t = det->tel_xyzr + 4*k;
+                        double c[3] = { t[0], t[1], t[2] }, s_in;
+                        if (orc_ray_sphere(Ip, ua, c, t[3], &s_in) && s_in < best) { best = s_in; ph.tel = k; }
+                    }
+                    if (ph.tel >= 0) {
+                        lc[ORC_CNT_TEL_HIT]++;
+                        if (tel_counts) {
+                            #pragma omp atomic
+                            tel_counts[ph.tel] += ph.weight;
+                        }
+                        if (det->cam_enabled) {
+                            ph.pix = orc_camera_pixel(det, ua);
+                            double tb = floor((ph.t - det->t_ref_ns) / det->t_bin_ns);
+                            if (ph.pix >= 0 && tb >= 0 && tb < det->n_tbins) {
+                                ph.tbin = (int32_t)tb;
+                                lc[ORC_CNT_CAM_HIT]++;
+                                if (hist) {
+                                    #pragma omp atomic
+                                    hist[(size_t)ph.pix * det->n_tbins + ph.tbin] += ph.weight;
+                                }
+                            }
+                        }
+                    }
+                }
+            store:
+                if (record_mode == 1 && photons && offsets) photons[offsets[i] + j] = ph;
+            }
+        }
+        #pragma omp critical
+        for (int k = 0; k < ORC_N_COUNTERS; ++k) cnt[k] += lc[k];
+    }
+    if (counters) for (int k = 0; k < ORC_N_COUNTERS; ++k) counters[k] += cnt[k];
+    return err;
+}
+
+int orc_sizeof_photon(void) { return (int)sizeof(orc_photon); }
+int orc_n_counters(void) { return ORC_N_COUNTERS; }

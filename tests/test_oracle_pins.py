@@ -1,0 +1,515 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (-m "not gpu").
+
+Each pin is something other than the oracle itself: values the thesis prints
+(tests/golden), closed forms, invariants, limits that reduce to textbook
+results, brute force on tiny inputs.  P:n = PAPER.md line n.
+"""
+import copy
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.constants as sc
+from scipy import stats
+
+from oracle import c8ph_oracle as O
+from paper_2405_04229_b200 import workloads as W
+
+C_LIGHT = sc.c * 1e-9  # m/ns
+
+
+# ------------------------------------------------------------------ O0 RNG
+def test_philox_known_answers(golden_dir):
+    n = 0
+    for line in open(os.path.join(golden_dir, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(t, 16) for t in line.split()]
+        assert O.philox4x32_10(w[0:4], w[4:6]) == w[6:10]
+        n += 1
+    assert n == 3
+
+
+def test_philox_bijective_and_uniform():
+    outs = set()
+    words = []
+    for j in range(1 << 12):
+        r = O.philox4x32_10([j, 7, 0, 0], [1, 0])
+        outs.add(tuple(r))
+        words.append(r)
+    assert len(outs) == 1 << 12                       # a bijection never collides
+    words = np.array(words, dtype=np.uint64)
+    for k in range(4):                                # equidistribution of the top byte
+        cnt = np.bincount((words[:, k] >> 24).astype(int), minlength=256)
+        assert stats.chisquare(cnt).pvalue > 1e-4
+
+
+def test_uniform_is_exact_in_fp32_and_open_interval():
+    for r in (0, 1, 511, 512, 0x7FFFFFFF, 0xFFFFFFFF, 123456789):
+        u = O.uniform(r)
+        assert 0.0 < u < 1.0
+        assert float(np.float32(u)) == u              # (2m+1) 2^-24 is an fp32 number
+        assert u == ((r >> 9) * 2 + 1) / 2.0 ** 24
+
+
+# ------------------------------------------------------------------ O1 yield
+def test_frank_tamm_closed_form():
+    # Eq. 2.3: alpha = e^2 / (2 h eps0 c) from CODATA, not from the oracle's constant
+    alpha = sc.e ** 2 / (2 * sc.h * sc.epsilon_0 * sc.c)
+    n = 1.000293
+    for beta in (1.0, 0.9999):
+        want = 2 * math.pi * alpha * (1 / 300e-9 - 1 / 600e-9) * (1 - 1 / (beta * n) ** 2)
+        got = O.cherenkov_yield(1.0, 1.0, beta, n, 300.0, 600.0)
+        assert got == pytest.approx(want, rel=2e-8)
+    assert O.cherenkov_yield(1.0, 1.0, 1.0, n, 300.0, 600.0) == pytest.approx(44.761, abs=2e-3)
+    assert O.cherenkov_yield(-2.0, 3.0, 1.0, n, 300.0, 600.0) == pytest.approx(4 * 3 * 44.7611, rel=1e-5)
+
+
+def test_cherenkov_threshold():
+    n = 1.000293
+    beta_th = 1.0 / n
+    assert O.cherenkov_yield(1, 1, beta_th * (1 - 1e-9), n, 300, 600) == 0.0
+    assert O.cherenkov_yield(1, 1, beta_th * (1 + 1e-9), n, 300, 600) > 0.0
+    gamma_th = 1 / math.sqrt(1 - beta_th ** 2)
+    assert gamma_th == pytest.approx(41.32, abs=0.01)  # sea-level electron threshold gamma
+
+
+# ------------------------------------------------------------------ O4 rotation / cone
+def test_rodrigues_properties():
+    rng = np.random.default_rng(5)
+    D = np.array([0.0, 0.0, -1.0])
+    for _ in range(50):
+        P = rng.normal(size=3)
+        P /= np.linalg.norm(P)
+        M = O.rodrigues(P)
+        assert np.allclose(M @ D, P, atol=1e-14)       # maps the cone axis onto the particle
+        assert np.allclose(M, M.T, atol=1e-15)
+        assert np.allclose(M @ M, np.eye(3), atol=1e-14)
+        assert np.linalg.det(M) == pytest.approx(1.0, abs=1e-13)
+    M = O.rodrigues([0.0, 0.0, 1.0])                   # degenerate bisector
+    assert np.allclose(M @ D, [0, 0, 1])
+    # P = D: a half turn about the axis itself (M = 1 + 2 R^2 of P:706 with A = D)
+    assert np.allclose(O.rodrigues([0.0, 0.0, -1.0]), np.diag([-1.0, -1.0, 1.0]))
+
+
+def test_cone_direction_angle_norm_azimuth(golden_dir):
+    facts = dict(l.split(None, 1) for l in open(os.path.join(golden_dir, "paper_facts.txt")) if not l.startswith("#"))
+    rng = np.random.default_rng(6)
+    P = np.array([0.3, -0.2, -0.9])
+    P /= np.linalg.norm(P)
+    M = O.rodrigues(P)
+    cos_th = 1 / 1.000293
+    sin_th = math.sqrt(1 - cos_th ** 2)
+    # the thesis: opening angle in air "less than 1.4 deg"
+    assert math.degrees(math.acos(cos_th)) < float(facts["cherenkov_angle_max_deg"])
+    assert math.degrees(math.acos(cos_th)) == pytest.approx(1.3868, abs=1e-4)
+    e1, e2 = M[:, 0], M[:, 1]
+    az = []
+    for phi in rng.uniform(0, 2 * math.pi, 4000):
+        u = O.cone_direction(M, cos_th, sin_th, phi)
+        assert abs(np.dot(u, P) - cos_th) < 1e-13
+        assert abs(np.linalg.norm(u) - 1) < 1e-13
+        az.append(math.atan2(np.dot(u, e2), np.dot(u, e1)))
+    cnt = np.histogram(az, bins=16, range=(-math.pi, math.pi))[0]
+    assert stats.chisquare(cnt).pvalue > 1e-4
+    # local vector of P:680 for the un-rotated axis
+    u = O.cone_direction(np.eye(3).ravel(), cos_th, sin_th, 0.25)
+    assert np.allclose(u, [math.cos(0.25) * sin_th, math.sin(0.25) * sin_th, -cos_th])
+
+
+# ------------------------------------------------------------------ O7 straight line, O2/O13 time
+def _one_segment_cfg(z=10000.0, L=10.0, beta=1.0, d=(0.0, 0.0, -1.0), x=0.0, y=0.0):
+    cfg = W.make_config(0, n_segments=1)
+    s = cfg["segments"]
+    s["x"][:], s["y"][:], s["z"][:] = x, y, z
+    s["dx"][:], s["dy"][:], s["dz"][:] = d
+    s["len"][:], s["beta"][:], s["t0"][:], s["charge"][:] = L, beta, 100.0, 1.0
+    cfg["detector"].update(hist_nx=0, hist_ny=0)
+    return cfg
+
+
+def test_straight_line_plane_hit():
+    I, t = O.straight_line([1.0, 2.0, 50.0], [0.6, 0.0, -0.8])
+    assert np.allclose(I, [1 + 62.5 * 0.6, 2.0, 0.0]) and t == pytest.approx(62.5)
+
+
+def test_constant_n_ring_and_arrival_time():
+    """Exact constant-n limit: a vertical beta=1 particle lights the ring r = (Z-s) tan(theta_c)."""
+    cfg = _one_segment_cfg()
+    ph = O.run(cfg)["photons"]
+    assert len(ph) > 300 and np.all(ph["status"] == O.ST_LANDED)
+    n = float(np.float32(0.000293)) + 1.0
+    tan_c = math.sqrt(n * n - 1.0)
+    r = np.hypot(ph["x"], ph["y"])
+    assert r.max() <= 10000.0 * tan_c + 1e-9 and r.min() >= 9990.0 * tan_c - 1e-9
+    assert r.max() == pytest.approx(242.1, abs=0.3)    # 10 km * tan(1.3868 deg)
+    # t = t0 + s/(beta c) + n D / c with D = (Z - s)/cos(theta_c)
+    zs = r / tan_c
+    s = 10000.0 - zs
+    t = 100.0 + s / C_LIGHT + n * (zs * n) / C_LIGHT
+    assert np.allclose(ph["t"], t, atol=1e-9, rtol=0)
+    # direction keeps the cone angle
+    assert np.allclose(-ph["uz"], 1 / n, atol=1e-13)
+    assert abs(np.mean(s) - 5.0) < 5 * 10 / math.sqrt(12 * len(s))           # O2: uniform on the track
+
+
+def test_wavelength_law():
+    cfg = _one_segment_cfg(L=200.0)
+    ph = O.run(cfg)["photons"]
+    lam = ph["lambda_nm"]
+    assert lam.min() >= 300.0 and lam.max() <= 600.0
+    # CDF of a 1/lambda^2 spectrum: F = (1/l1 - 1/l)/(1/l1 - 1/l2)
+    cdf = lambda l: (1 / 300.0 - 1 / l) / (1 / 300.0 - 1 / 600.0)
+    assert stats.kstest(lam, cdf).pvalue > 1e-3
+    sig = (1 / 300 - 1 / 600) / math.sqrt(12 * len(lam))
+    assert abs(np.mean(1 / lam) - 0.5 * (1 / 300 + 1 / 600)) < 5 * sig
+
+
+# ------------------------------------------------------------------ O8 refraction
+def _linear_atm(model="planar", n_g=1.5, n_top=1.0, h_top=100000.0):
+    atm = W.make_atmosphere("planar_exp")
+    h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
+    atm["refractivity"] = ((n_g - 1.0) + (n_top - n_g) * h / h_top).astype(np.float32)
+    atm["model"] = model
+    return atm
+
+
+def test_trace_linear_profile_closed_form(golden_dir):
+    """Thesis' test medium n = 1.5 -> 1.0 over 100 km; closed forms of the differential
+    Snell law (Eq. 3.20, Eq. 3.23 with the integration constant's sign fixed)."""
+    atm = _linear_atm()
+    eta = atm["refractivity"].astype(np.float64)
+    n_of = lambda h: 1.0 + np.interp(h, atm["dh"] * np.arange(len(eta)), eta)
+    h_e, th = 50000.0, math.radians(45.0)
+    n_e, n_g = n_of(h_e), n_of(0.0)
+    b = abs((1.0 - 1.5) / 100000.0)
+    K = n_e * math.sin(th)
+    X = K / b * (math.acosh(n_g / K) - math.acosh(n_e / K))
+    S = (math.sqrt(n_g ** 2 - K ** 2) - math.sqrt(n_e ** 2 - K ** 2)) / b
+    F = lambda x: 0.5 * (x * math.sqrt(x * x - K * K) + K * K * math.acosh(x / K))
+    cT = (F(n_g) - F(n_e)) / b
+    assert X == pytest.approx(42375.7267, abs=0.05) and S == pytest.approx(65607.2976, abs=0.05)
+    r1 = O.trace(atm, False, h_e, th, 0.0, sub=1)
+    r4 = O.trace(atm, False, h_e, th, 0.0, sub=4)
+    for key, want in (("disp", X), ("S", S), ("cT", cT)):
+        e1, e4 = abs(r1[key] - want), abs(r4[key] - want)
+        assert e1 / want < 1e-3                        # the thesis' own bound: <= 0.1 %
+        assert e1 < 2e-3 and e4 < 2e-4, (key, e1, e4)  # second-order convergence to the closed form
+    # Eq. 3.20: sin(nu) = c sin(alpha) / (c - y) -> arrival angle
+    assert r1["sin_arr"] == pytest.approx(K / n_g, abs=1e-13)
+
+
+def test_trace_invariants_and_limits():
+    atm = W.make_atmosphere("spherical_5layer")
+    R = atm["earth_radius"]
+    for h_e, zen in ((10000.0, 20.0), (25000.0, 60.0), (5000.0, 75.0), (60000.0, 80.0)):
+        th = math.radians(zen)
+        n_e = 1 + O.refractivity(atm, h_e)
+        n_g = 1 + O.refractivity(atm, 0.0)
+        rp = O.trace(atm, False, h_e, th, 0.0)
+        assert n_g * rp["sin_arr"] == pytest.approx(n_e * math.sin(th), rel=1e-13)          # Snell
+        rs = O.trace(atm, True, h_e, th, 0.0)
+        assert n_g * R * rs["sin_arr"] == pytest.approx(n_e * (R + h_e) * math.sin(th), rel=1e-12)  # Bouguer
+        assert rs["S"] > rp["S"] * 0.999 and rs["cT"] > rs["S"]
+    # constant n: the trace is the straight line
+    hom = W.make_atmosphere("homogeneous")
+    hom["model"] = "planar"
+    r = O.trace(hom, False, 10000.0, math.radians(40), 0.0)
+    assert r["disp"] == pytest.approx(10000 * math.tan(math.radians(40)), rel=1e-13)
+    assert r["S"] == pytest.approx(10000 / math.cos(math.radians(40)), rel=1e-13)
+    assert r["cT"] == pytest.approx(r["S"] * (1 + float(np.float32(0.000293))), rel=1e-13)
+    hom["model"] = "spherical"
+    r = O.trace(hom, True, 10000.0, math.radians(40), 0.0)
+    re, rg, th = R + 10000.0, R, math.radians(40)
+    assert r["disp"] == pytest.approx(math.asin(re * math.sin(th) / rg) - th, rel=1e-9)
+    assert r["S"] == pytest.approx(re * math.cos(th) - math.sqrt(rg ** 2 - (re * math.sin(th)) ** 2), rel=1e-10)
+    # R -> infinity: spherical -> planar
+    big = copy.deepcopy(atm)
+    big["earth_radius"] = 1e10
+    rp = O.trace(atm, False, 12000.0, math.radians(50), 0.0)
+    rs = O.trace(big, True, 12000.0, math.radians(50), 0.0)
+    assert rs["disp"] * 1e10 == pytest.approx(rp["disp"], rel=2e-5)
+    assert rs["S"] == pytest.approx(rp["S"], rel=2e-5) and rs["X"] == pytest.approx(rp["X"], rel=2e-5)
+    # beyond the horizon: no ground
+    assert O.trace(atm, True, 5000.0, math.radians(88.5), 0.0) is None
+    assert O.trace(atm, True, 5000.0, math.radians(85.0), 0.0) is not None
+
+
+def _brute_force_ray(atm, spherical, h_e, zen, h_g, ds=0.5):
+    """Fine-step RK4 integration of the ray equation d/ds(n u) = grad n in the medium defined by
+    the linearly interpolated table (independent numpy code)."""
+    eta = atm["refractivity"].astype(np.float64)
+    dh = atm["dh"]
+    R = atm["earth_radius"]
+
+    def n_and_grad(p):
+        if spherical:
+            r = math.hypot(p[0], p[1])
+            h = r - R
+            up = np.array([p[0] / r, p[1] / r])
+        else:
+            h = p[1]
+            up = np.array([0.0, 1.0])
+        f = min(max(h / dh, 0.0), len(eta) - 1.000001)
+        i = int(f)
+        return 1 + eta[i] + (f - i) * (eta[i + 1] - eta[i]), (eta[i + 1] - eta[i]) / dh * up, h
+
+    def rhs(y):
+        p, T = y[:2], y[2:4]
+        n, g, _ = n_and_grad(p)
+        return np.array([T[0] / n, T[1] / n, g[0], g[1], n])
+
+    p0 = np.array([0.0, (R if spherical else 0.0) + h_e])
+    n0, _, _ = n_and_grad(p0)
+    y = np.array([p0[0], p0[1], n0 * math.sin(zen), -n0 * math.cos(zen), 0.0])
+    S = 0.0
+    while True:
+        k1 = rhs(y); k2 = rhs(y + 0.5 * ds * k1); k3 = rhs(y + 0.5 * ds * k2); k4 = rhs(y + ds * k3)
+        yn = y + ds / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+        h_new = n_and_grad(yn[:2])[2]
+        if h_new <= h_g:
+            h_old = n_and_grad(y[:2])[2]
+            f = (h_old - h_g) / (h_old - h_new)
+            y = y + f * (yn - y)
+            S += f * ds
+            break
+        y, S = yn, S + ds
+    disp = math.atan2(y[0], y[1]) if spherical else y[0]
+    return dict(disp=disp, S=S, cT=y[4])
+
+
+@pytest.mark.parametrize("spherical", [False, True])
+def test_trace_against_brute_force_integration(spherical):
+    atm = W.make_atmosphere("spherical_5layer")
+    scale = atm["earth_radius"] if spherical else 1.0
+    for h_e, zen in ((3000.0, 30.0), (8000.0, 65.0)):
+        th = math.radians(zen)
+        want = _brute_force_ray(atm, spherical, h_e, th, 0.0, ds=1.0)
+        got = O.trace(atm, spherical, h_e, th, 0.0, sub=1)
+        assert abs(got["disp"] - want["disp"]) * scale < 2e-4
+        assert abs(got["S"] - want["S"]) < 2e-4
+        assert abs(got["cT"] - want["cT"]) < 2e-4
+
+
+def test_trace_converged_at_table_spacing():
+    """Reading R8: the integrator is converged to <= 0.1 mm / 0.3 ps at sub = 1."""
+    atm = W.make_atmosphere("spherical_5layer")
+    for h_e, zen in ((10000.0, 60.0), (30000.0, 75.0)):
+        a = O.trace(atm, True, h_e, math.radians(zen), 0.0, sub=1)
+        b = O.trace(atm, True, h_e, math.radians(zen), 0.0, sub=8)
+        assert abs(a["disp"] - b["disp"]) * atm["earth_radius"] < 1e-4
+        assert abs(a["cT"] - b["cT"]) / C_LIGHT < 3e-4
+
+
+def test_refraction_magnitudes_sane():
+    """The ray bends towards the vertical and lands short of the straight line (Fig. 3.3)."""
+    cfg = W.make_config(2, n_segments=4)
+    tab = O.table_for(cfg)
+    v20 = O.table_lookup(cfg["table"], tab, 10000.0, math.radians(20))
+    v60 = O.table_lookup(cfg["table"], tab, 10000.0, math.radians(60))
+    assert v60[0] < v20[0] < 0 and -10.0 < v60[0] < -3.0
+    assert 600 < v20[3] < 900 and 1200 < v60[3] < 1700            # slant depth g/cm^2 from 10 km
+    assert 3.0 < v20[2] < 8.0                                       # ~ int (n-1) ds / c  [ns]
+
+
+# ------------------------------------------------------------------ O9 table
+def test_table_lookup_nodes_bilinear_and_sentinels():
+    table = dict(n_h=9, n_zen=7, h_max=8000.0, zen_max_deg=60.0)
+    hh = np.linspace(0, 8000.0, 9)[:, None]
+    zz = np.linspace(0, math.radians(float(np.float32(60.0))), 7)[None, :]
+    data = np.zeros((9, 7, 5), dtype=np.float32)
+    coef = [(1.0, 2e-3, 3.0, 5e-4), (0.5, -1e-3, 1.0, 1e-4), (2, 0, 0, 0), (0, 1e-3, 0, 0), (0, 0, 1, 0)]
+    for k, (a, b, c, d) in enumerate(coef):
+        data[:, :, k] = a + b * hh + c * zz + d * hh * zz
+    assert np.allclose(O.table_lookup(table, data, 3000.0, float(zz[0, 4])), data[3, 4], rtol=1e-6)   # node
+    h, z = 3456.7, 0.61
+    want = [a + b * h + c * z + d * h * z for a, b, c, d in coef]
+    assert np.allclose(O.table_lookup(table, data, h, z), want, rtol=2e-6)                             # bilinear exact
+    assert np.allclose(O.table_lookup(table, data, 8000.0, z)[0], want[0] + (8000 - h) * (2e-3 + 5e-4 * z), rtol=2e-6)
+    assert O.table_lookup(table, data, 8000.1, z) is None and O.table_lookup(table, data, 100.0, 1.06) is None
+    data[4, 5, :] = np.nan
+    assert O.table_lookup(table, data, 3500.0, float(zz[0, 4]) + 0.01) is None                         # stencil touches NaN
+    assert O.table_lookup(table, data, 2500.0, float(zz[0, 4]) + 0.01) is not None
+
+
+def test_table_nodes_are_trace_minus_straight_line():
+    cfg = W.make_config(2, n_segments=4)
+    atm, table = cfg["atmosphere"], dict(n_h=17, n_zen=9, h_max=40000.0, zen_max_deg=80.0)
+    tab = O.build_table(atm, table)
+    assert np.all(tab[0] == 0)                                   # h_a <= h_obs
+    assert np.all(tab[:, 0, 0] == 0)                             # vertical ray: no displacement
+    R = atm["earth_radius"]
+    a, b = 5, 6
+    h, th = a * 40000.0 / 16, b * math.radians(float(np.float32(80.0))) / 8
+    r = O.trace(atm, True, h, th, 0.0)
+    p = (R + h) * math.sin(th)
+    s_line = (R + h) * math.cos(th) - math.sqrt(R * R - p * p)
+    psi_line = math.asin(p / R) - th
+    assert tab[a, b, 0] == pytest.approx(R * (r["disp"] - psi_line), rel=1e-5)
+    assert tab[a, b, 1] == pytest.approx(r["S"] - s_line, rel=1e-5)
+    assert tab[a, b, 2] == pytest.approx((r["cT"] - s_line) / C_LIGHT, rel=1e-5)
+    assert tab[a, b, 3] == pytest.approx(r["X"], rel=1e-6)
+
+
+# ------------------------------------------------------------------ O11 transmission
+def test_transmission_single_exponential_closed_form():
+    atm = W.make_atmosphere("planar_exp", h_obs=2000.0, rayleigh=True)
+    atm["refractivity"] = np.zeros_like(atm["refractivity"])          # straight ray
+    th = math.radians(35.0)
+    r = O.trace(atm, False, 9000.0, th, 2000.0)
+    x_want = 1030.0 * (math.exp(-2000 / 8400.0) - math.exp(-9000 / 8400.0)) / math.cos(th)
+    assert r["X"] == pytest.approx(x_want, rel=1e-6)
+    lam = 350.0
+    assert O.transmission(atm, r["X"], 0.0, lam) == pytest.approx(math.exp(-(400 / lam) ** 4 * x_want / 2970.0), rel=1e-6)
+    atm["rayleigh_X"] = 0.0
+    assert O.transmission(atm, r["X"], 0.3, lam) == 1.0               # alpha -> 0  =>  T = 1
+    atm["aer_L"] = 15000.0
+    ra = O.trace(atm, False, 9000.0, th, 2000.0)
+    tau = 1200.0 / 15000.0 * (math.exp(-2000 / 1200.0) - math.exp(-9000 / 1200.0)) / math.cos(th)
+    assert ra["tau_aer"] == pytest.approx(tau, rel=1e-12)
+    assert O.transmission(atm, 0.0, ra["tau_aer"], 700.0) == pytest.approx(math.exp(-tau * 350.0 / 700.0), rel=1e-6)
+
+
+# ------------------------------------------------------------------ O12 intersection
+def test_ray_sphere_analytic_cases():
+    u = np.array([0.0, 0.6, -0.8])
+    hit, s = O.ray_sphere([0, 0, 0], u, [0, 0, 0], 6.0)
+    assert hit and s == pytest.approx(-6.0)
+    assert O.ray_sphere([7.5 - 1e-9, 0, 0], [0, 0, -1.0], [0, 0, 0], 7.5)[0]
+    assert not O.ray_sphere([7.5 + 1e-9, 0, 0], [0, 0, -1.0], [0, 0, 0], 7.5)[0]
+    # inclined ray: footprint stretches to r/|u_z| along the ray azimuth, stays r across it
+    assert O.ray_sphere([0, 7.4, 0], u, [0, 0, 0], 6.0)[0] and not O.ray_sphere([0, 7.6, 0], u, [0, 0, 0], 6.0)[0]
+    assert O.ray_sphere([5.9, 0, 0], u, [0, 0, 0], 6.0)[0] and not O.ray_sphere([6.1, 0, 0], u, [0, 0, 0], 6.0)[0]
+
+
+def test_camera_pixel_centres_round_trip():
+    det = W.make_config(3, n_segments=4)["detector"]
+    az, el, p = math.radians(det["cam_az_deg"]), math.radians(det["cam_el_deg"]), math.radians(det["cam_pix_deg"])
+    w = np.array([math.cos(el) * math.cos(az), math.cos(el) * math.sin(az), math.sin(el)])
+    right = np.array([-math.sin(az), math.cos(az), 0.0])
+    up = np.cross(w, right)
+    for r, c in ((0, 0), (10, 7), (21, 19), (5, 0)):
+        a = (c - 0.5 * (det["cam_cols"] - 1) + 0.5 * (r % 2)) * p
+        e = (r - 0.5 * (det["cam_rows"] - 1)) * p * math.sqrt(3) / 2
+        v = w + math.tan(a) * right + math.tan(e) * up
+        v /= np.linalg.norm(v)
+        assert O.camera_pixel(det, -v) == r * det["cam_cols"] + c
+    assert O.camera_pixel(det, w) == -1                              # photon travelling along +axis: from behind
+    v = w + math.tan(math.radians(25.0)) * right
+    assert O.camera_pixel(det, -v / np.linalg.norm(v)) == -1         # outside the field of view
+
+
+# ------------------------------------------------------------------ whole path: conservation, filters
+def _check_conservation(res, w):
+    c = res["counters"]
+    assert c["emitted"] == res["total_bunches"] == int(res["n_bunch"].sum())
+    assert c["emitted"] == c["upgoing"] + c["lv2"] + c["table_range"] + c["roulette"] + c["landed"]
+    ph = res["photons"]
+    assert len(ph) == c["emitted"] and int((ph["status"] == O.ST_LANDED).sum()) == c["landed"]
+    assert c["segments"] == len(res["n_bunch"])
+    assert c["in_grid"] == int((ph["bin"] >= 0).sum()) and c["tel_hit"] == int((ph["tel"] >= 0).sum())
+
+
+def test_photon_count_conservation_cfg0():
+    cfg = W.make_config(0)
+    res = O.run(cfg)
+    _check_conservation(res, 1.0)
+    c = res["counters"]
+    assert res["hist"].sum() == c["in_grid"] and c["landed"] == c["emitted"]
+    # stochastic rounding is unbiased: sum N_i vs sum N_exp  (sigma^2 <= n_seg / 4)
+    seg = cfg["segments"]
+    n_exp = sum(O.cherenkov_yield(1.0, 10.0, float(b), 1 + float(np.float32(0.000293)), 300, 600) for b in seg["beta"])
+    assert abs(c["emitted"] - n_exp) < 5 * math.sqrt(len(seg["beta"]) / 4)
+    assert 3.5e5 < c["emitted"] < 3.9e5
+
+
+def test_segment_order_and_batching_independence():
+    cfg = W.make_config(0, n_segments=64)
+    full = O.run(cfg)
+    part = copy.deepcopy(cfg)
+    part["segments"] = W.slice_segments(cfg["segments"], 40, 64)
+    part["seg_id_base"] = 40
+    sub = O.run(part)
+    a = full["photons"][full["photons"]["seg"] >= 40]
+    b = sub["photons"]
+    assert len(a) == len(b)
+    for f in ("x", "y", "t", "lambda_nm", "ux"):
+        assert np.array_equal(a[f], b[f])
+
+
+def test_filters_are_lossless_and_roulette_unbiased():
+    cfg = W.make_config(2, n_segments=3000)
+    on = O.run(cfg)
+    _check_conservation(on, 5.0)
+    off_cfg = copy.deepcopy(cfg)
+    off_cfg["params"].update(lv1=False, lv2=False)
+    off = O.run(off_cfg)
+    _check_conservation(off, 5.0)
+    assert on["counters"]["seg_lv1"] > 0 and on["counters"]["lv2"] > 0
+    assert on["counters"]["tel_hit"] == off["counters"]["tel_hit"] > 50
+    assert np.array_equal(on["tel_counts"], off["tel_counts"])
+    hit_on = on["photons"][on["photons"]["tel"] >= 0]
+    hit_off = off["photons"][off["photons"]["tel"] >= 0]
+    key = lambda p: p["seg"] * (1 << 20) + p["j"]
+    assert np.array_equal(np.sort(key(hit_on)), np.sort(key(hit_off)))
+    # roulette: sum over survivors of w vs sum of w T over all that reached the roulette
+    w_cfg = copy.deepcopy(off_cfg)
+    w_cfg["params"]["trans"] = "weight"
+    wres = O.run(w_cfg)
+    ph = wres["photons"][wres["photons"]["status"] == O.ST_LANDED]
+    exp, var = ph["T"].sum(), (ph["T"] * (1 - ph["T"])).sum()
+    assert abs(off["counters"]["landed"] - exp) < 5 * math.sqrt(var)
+    assert 0.2 < exp / len(ph) < 0.95
+
+
+def test_planar_numeric_path_cfg1_small():
+    cfg = W.make_config(1, n_segments=300)
+    res = O.run(cfg)
+    _check_conservation(res, 1.0)
+    ph = res["photons"][res["photons"]["status"] == O.ST_LANDED]
+    assert len(ph) > 1000
+    assert res["hist"].sum() == pytest.approx(ph["weight"][ph["bin"] >= 0].sum(), rel=1e-12)
+    assert np.all(ph["T"] < 1.0) and np.all(ph["T"] > 0.3)
+    # refraction pulls the photon towards the vertical: it lands short of the straight line
+    seg = cfg["segments"]
+    ax = seg["x"][ph["seg"]] - seg["z"][ph["seg"]] * seg["dx"][ph["seg"]] / seg["dz"][ph["seg"]]
+    assert np.all(np.hypot(ph["x"] - ph["x_line"], ph["y"] - ph["y_line"]) < 2.0)
+    assert np.all(np.abs(np.hypot(ph["ux"], ph["uy"]) ** 2 + ph["uz"] ** 2 - 1) < 1e-12)
+
+
+def test_fluorescence_sampling_isotropy_and_lines():
+    cfg = W.make_config(3, n_segments=1)
+    s = cfg["segments"]
+    s["x"][:], s["y"][:], s["z"][:] = 0.0, 0.0, 10000.0
+    s["dx"][:], s["dy"][:], s["dz"][:] = 0.0, 0.0, -1.0
+    s["edep"][:] = 5000.0
+    cfg["detector"]["tel_xyzr"] = np.array([[0.0, 0.0, 0.0, 1.9]], dtype=np.float32)
+    cfg["params"].update(trace="straight", trans="off", lv2=False, aim_factor=1e9)   # psi -> 90 deg: half sphere
+    res = O.run(cfg)
+    ph = res["photons"]
+    assert len(ph) == pytest.approx(4.0 * 5000.0 * 0.5, abs=1)                      # Y E Omega/4pi
+    ph = ph[ph["status"] == O.ST_LANDED]
+    mu = -ph["uz"]                                                                  # cos to the aim axis (-z)
+    assert np.mean(mu) == pytest.approx(0.5, abs=5 * math.sqrt(1 / 12 / len(mu)))
+    assert np.mean(mu ** 2) == pytest.approx(1 / 3, abs=0.02)
+    assert abs(np.mean(ph["ux"])) < 0.03 and abs(np.mean(ph["uy"])) < 0.03
+    lines, cdf = cfg["params"]["line_nm"], cfg["params"]["line_cdf"].astype(np.float64)
+    prob = np.diff(np.concatenate([[0.0], cdf]))
+    idx = np.searchsorted(lines, ph["lambda_nm"].astype(np.float32))
+    cnt = np.bincount(idx, minlength=len(lines))
+    keep = prob * len(ph) > 5
+    assert stats.chisquare(cnt[keep], prob[keep] / prob[keep].sum() * cnt[keep].sum()).pvalue > 1e-4
+
+
+def test_forced_cone_is_unbiased_in_margin():
+    """hits/Omega independent of the aim factor (photon number scaled with the solid angle)."""
+    hits = []
+    for fac in (1.5, 3.0):
+        cfg = W.make_config(3, n_segments=2000)
+        cfg["segments"]["edep"][:] = 2.0e10
+        cfg["params"].update(aim_factor=fac, trans="off")
+        res = O.run(cfg, record=False)
+        hits.append(res["counters"]["tel_hit"])
+    assert hits[0] > 200
+    assert abs(hits[0] - hits[1]) < 5 * math.sqrt(hits[0] + hits[1])
