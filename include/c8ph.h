@@ -1,0 +1,185 @@
+/*
+ * c8ph.h — C-ABI of libc8ph: B200-native optical-photon emission and propagation
+ * for air-shower track segments (arxiv/paper_2405_04229, D. Baack).
+ * P:n = PAPER.md line n of the thesis text.
+ *
+ * The library computes, per charged-particle track segment:
+ *   Cherenkov yield (Frank-Tamm, Eq. 2.2-2.4, height dependent n(h) from
+ *   Listing 4.1) or fluorescence yield (Eq. 2.6, constant photons/MeV)
+ *   -> photons on the cone cos(theta) = 1/(beta n) (Eq. 2.5), Philox4x32-10
+ *      keyed on (seed; segment id, photon index)
+ *   -> straight line to the observation level (Eq. 3.3)
+ *   -> refraction: none | per-photon layered Snell sum (Eq. 3.15) | interpolation
+ *      tracing with a pre-computed correction table
+ *   -> atmospheric transmission
+ *   -> photon cuts: LV1 segment filter (Eq. 4.3), LV2/LV3 photon filter
+ *   -> ground grid / telescope spheres / camera pixels x time bins, photon list.
+ *
+ * Conventions: units m, ns, nm, g/cm^2, MeV.  Local right-handed frame, origin at the array
+ * centre on the observation level, z up; observation level is the plane z = 0 at
+ * altitude h_obs a.s.l.; in the spherical model the Earth centre is (0,0,-(R+h_obs)).
+ *
+ * All functions return C8PH_OK (0) or a negative error code; no exceptions cross the
+ * boundary.  Pointers are marked HOST or DEVICE.  No torch types appear here.
+ */
+#ifndef C8PH_H
+#define C8PH_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define C8PH_VERSION 100
+
+enum {
+    C8PH_OK = 0,
+    C8PH_E_ARG = -1,      /* NULL / out-of-range / inconsistent argument                      */
+    C8PH_E_STATE = -2,    /* atmosphere, detector or trace table not set up for this request   */
+    C8PH_E_CUDA = -3,     /* a CUDA runtime call failed; text in c8ph_last_error()              */
+    C8PH_E_NOMEM = -4
+};
+
+typedef struct c8ph_ctx c8ph_ctx;   /* opaque; owns only what it creates (tables, detector grids) */
+
+/* Create / destroy a context bound to one CUDA device.  Not thread-safe per context. */
+int c8ph_create(c8ph_ctx **out, int cuda_device);
+int c8ph_destroy(c8ph_ctx *ctx);
+/* Text of the last error of this context (or of create, if ctx == NULL); never NULL. */
+const char *c8ph_last_error(const c8ph_ctx *ctx);
+int c8ph_version(void);
+
+/* ---- atmosphere (thesis sec. 3.3, sec. 4.1) ------------------------------ */
+enum { C8PH_ATM_HOMOGENEOUS = 0, C8PH_ATM_PLANAR = 1, C8PH_ATM_SPHERICAL = 2 };
+typedef struct {
+    uint32_t size;                   /* sizeof(c8ph_atmosphere_desc), for versioning              */
+    int32_t model;                   /* C8PH_ATM_*                                                 */
+    float n_const_minus_1;           /* homogeneous model: refractivity n-1                        */
+    float h0_m, dh_m;                /* uniform height grid of the tables, node k at h0 + k dh     */
+    int32_t n_nodes;                 /* >= 2 (ignored for the homogeneous model)                   */
+    const float *refractivity;       /* HOST [n_nodes]: n-1 at the nodes (Listing 4.1)             */
+    const float *overburden_gcm2;    /* HOST [n_nodes] or NULL: vertical overburden X_v(h)         */
+    float earth_radius_m, h_obs_m;   /* R and the altitude of the observation level                */
+    float rayleigh_X_gcm2, rayleigh_lambda_nm; /* tau_R = X_slant (lambda_R/lambda)^4 / X_R; X_R = 0: off */
+    float aer_L_m, aer_H_m, aer_lambda_nm, aer_angstrom; /* aerosol: alpha = exp(-h/H)/L (lambda_a/lambda)^a; L = 0: off */
+} c8ph_atmosphere_desc;
+/* Copies the tables to the device (synchronous).  Invalidates a previously built trace table. */
+int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *desc);
+
+/* ---- interpolation-tracing correction table (thesis sec. 4.4.1) -------------------- */
+#define C8PH_TABLE_CHANNELS 5        /* dd [m], ds [m], dt [ns], X_slant [g/cm^2], tau_aer        */
+typedef struct {
+    uint32_t size;
+    int32_t n_h, n_zen;              /* nodes: h_a = a h_max/(n_h-1) a.s.l., theta_b = b zen_max/(n_zen-1) */
+    float h_max_m, zen_max_deg;
+    int32_t substeps;                /* sub-layers per n(h) table cell in the builder (>= 1)       */
+} c8ph_table_desc;
+/* One kernel, one thread per node: the exact layered-Snell ray (fp64) from (h_a, theta_b) to the
+ * observation sphere/plane minus the straight line (asynchronous on `stream`, a cudaStream_t).   */
+int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *desc, void *stream);
+/* Copy the table out / in (HOST, layout [n_h][n_zen][C8PH_TABLE_CHANNELS]); synchronous.
+ * set_ lets a caller inject a table computed elsewhere.  No-ground nodes hold NaN.              */
+int c8ph_get_trace_table(c8ph_ctx *ctx, float *host_out, int64_t n_floats);
+int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *desc, const float *host_in);
+
+/* ---- detector (thesis sec. 6.2; camera: BASELINE cfg3) ---------------------------- */
+typedef struct {
+    uint32_t size;
+    int32_t hist_nx, hist_ny;        /* ground grid, bin (ix,iy) -> iy*hist_nx + ix; 0: no grid    */
+    float hist_x0, hist_y0, hist_cell;
+    int32_t n_tel;                   /* telescope bounding spheres                        */
+    const float *tel_xyzr;           /* HOST [n_tel][4] = centre x,y,z and radius; copied          */
+    int32_t cam_enabled;             /* camera on telescope 0: pixel x time-bin histogram          */
+    float cam_axis_az_deg, cam_axis_el_deg, cam_pix_deg;
+    int32_t cam_rows, cam_cols, n_tbins;
+    double t_ref_ns;                 /* photon times are reported relative to t_ref               */
+    float t_bin_ns;
+} c8ph_detector;
+/* Copies the telescope list and builds the uniform-grid accelerators (synchronous). */
+int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *det);
+
+/* ---- run parameters --------------------------------------------------------------------------- */
+enum {
+    C8PH_EMIT_CHERENKOV = 0, C8PH_EMIT_FLUORESCENCE = 1
+};
+enum { C8PH_TRACE_STRAIGHT = 0, C8PH_TRACE_NUMERIC = 1, C8PH_TRACE_TABLE = 2 };
+enum { C8PH_TRANS_OFF = 0, C8PH_TRANS_WEIGHT = 1, C8PH_TRANS_ROULETTE = 2 };
+enum { C8PH_WRITE_NONE = 0, C8PH_WRITE_ALL = 1, C8PH_WRITE_TEL = 2 };
+typedef struct {
+    uint32_t size;
+    int32_t emit, trace, trans, write;      /* the enums above                                    */
+    int32_t filter_lv1, filter_lv2;         /* booleans                                           */
+    float lambda_min_nm, lambda_max_nm;     /* Cherenkov band                                     */
+    float bunch_weight;                     /* photons per generated bunch (> 0)                  */
+    float lv1_margin_rad, lv2_margin_m;
+    float fluor_yield_per_MeV, aim_factor;  /* fluorescence: photons/MeV; forced-cone radius = aim_factor * r_tel */
+    int32_t n_lines;                        /* fluorescence line spectrum                         */
+    const float *line_nm, *line_cdf;        /* HOST [n_lines]; copied at every call               */
+} c8ph_params;
+
+/* ---- segments, outputs ------------------------------------------------------------------------- */
+typedef struct {                            /* SoA, fp32, n_segments each, caller-owned            */
+    uint32_t size;
+    const float *x, *y, *z;                 /* start point A                                       */
+    const float *dx, *dy, *dz;              /* direction P (renormalised on the device)            */
+    const float *len, *beta, *t0, *charge;  /* length, v/c, time at A, charge number               */
+    const float *edep;                      /* MeV deposited (fluorescence) or NULL                */
+} c8ph_segments;
+
+typedef struct {                            /* 32 B photon record                                  */
+    float x, y;                             /* position on the observation plane                   */
+    float ux, uy;                           /* arrival direction (uz = -sqrt(1-ux^2-uy^2))         */
+    float t_ns;                             /* arrival time - t_ref                                */
+    float lambda_nm;
+    uint32_t seg;                           /* segment index within the call                       */
+    uint32_t j_tel;                         /* (photon index j << 14) | telescope, 0x3FFF = none   */
+} c8ph_photon;
+#define C8PH_TEL_NONE 0x3FFFu
+#define C8PH_MAX_BUNCHES_PER_SEGMENT (1 << 18)
+
+enum {
+    C8PH_CNT_SEGMENTS = 0, C8PH_CNT_SEG_BELOW_THRESHOLD, C8PH_CNT_SEG_LV1, C8PH_CNT_SEG_EMITTING,
+    C8PH_CNT_EMITTED, C8PH_CNT_UPGOING, C8PH_CNT_LV2, C8PH_CNT_TABLE_RANGE, C8PH_CNT_ROULETTE,
+    C8PH_CNT_LANDED, C8PH_CNT_IN_GRID, C8PH_CNT_TEL_HIT, C8PH_CNT_CAM_HIT,
+    C8PH_CNT_WRITTEN, C8PH_CNT_OVERFLOW, C8PH_CNT_CLIPPED,
+    C8PH_N_COUNTERS
+};
+
+typedef struct {
+    uint32_t size;
+    float *hist;               /* [hist_ny*hist_nx] or camera [n_pix*n_tbins]; += weight; or NULL   */
+    float *tel_counts;         /* [n_tel]; += weight per telescope hit; or NULL                     */
+    c8ph_photon *photons;      /* [photon_capacity] or NULL                                         */
+    float *photon_weight;      /* [photon_capacity] or NULL: bunch weight x transmission per record */
+    int64_t photon_capacity;
+    uint64_t *counters;        /* [C8PH_N_COUNTERS], accumulated; counters[WRITTEN] is the photon-list cursor */
+} c8ph_outputs;
+
+/* The hot call.  All segment and output pointers are DEVICE pointers; every buffer is borrowed for
+ * the duration of the enqueued work only.  Asynchronous on `stream`; no allocation, no host sync
+ * and no host<->device copy of bulk data.  Outputs are ACCUMULATED (caller zeroes them).  Results
+ * depend only on (seed, seg_id_base + i, j): not on grid size, segment order or batching.
+ * Photons that do not fit photon_capacity are still binned and counted in OVERFLOW.             */
+int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *segments, int64_t n_segments,
+                        int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
+                        const c8ph_outputs *out, void *stream);
+
+/* Same path with HOST buffers (pinned or pageable): copies the segments in, zeroes device
+ * outputs, runs, copies hist / tel_counts / counters / the first min(written, capacity) photons
+ * back into the HOST buffers of `out` (which are overwritten, not accumulated); synchronous.    */
+int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, int64_t n_segments,
+                             int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
+                             const c8ph_outputs *host_out);
+
+/* Device time of the last c8ph_emit_propagate kernel of this context in ms (CUDA events on the
+ * launch stream; synchronises on the end event).  Returns < 0 if nothing was launched.          */
+float c8ph_last_kernel_ms(c8ph_ctx *ctx);
+/* Number of kernels the library has launched in this context so far. */
+int64_t c8ph_launch_count(const c8ph_ctx *ctx);
+const char *c8ph_counter_name(int index);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* C8PH_H */

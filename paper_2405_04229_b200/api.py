@@ -1,0 +1,406 @@
+"""Thin Python binding over the C-ABI of ``libc8ph.so`` (include/c8ph.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of the library.
+PyTorch is used for device memory and streams.  There is no CPU fallback: if the shared library
+is missing or cannot be loaded, importing a symbol raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libc8ph.so")
+
+OK, E_ARG, E_STATE, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4
+ATM = {"homogeneous": 0, "planar": 1, "spherical": 2}
+EMIT = {"cherenkov": 0, "fluorescence": 1}
+TRACE = {"straight": 0, "numeric": 1, "table": 2}
+TRANS = {"off": 0, "weight": 1, "roulette": 2}
+WRITE = {"none": 0, "all": 1, "tel": 2}
+TABLE_CHANNELS = 5
+TEL_NONE = 0x3FFF
+COUNTER_NAMES = ("segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "emitted", "upgoing", "lv2",
+                 "table_range", "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "written", "overflow",
+                 "clipped")
+N_COUNTERS = len(COUNTER_NAMES)
+
+EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8ph_init_atmosphere",
+           "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
+           "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
+           "c8ph_counter_name")
+
+PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
+                         ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
+assert PHOTON_DTYPE.itemsize == 32
+
+_fp = C.POINTER(C.c_float)
+
+
+class AtmosphereDesc(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("model", C.c_int32), ("n_const_minus_1", C.c_float),
+                ("h0_m", C.c_float), ("dh_m", C.c_float), ("n_nodes", C.c_int32),
+                ("refractivity", _fp), ("overburden_gcm2", _fp),
+                ("earth_radius_m", C.c_float), ("h_obs_m", C.c_float),
+                ("rayleigh_X_gcm2", C.c_float), ("rayleigh_lambda_nm", C.c_float),
+                ("aer_L_m", C.c_float), ("aer_H_m", C.c_float), ("aer_lambda_nm", C.c_float),
+                ("aer_angstrom", C.c_float)]
+
+
+class TableDesc(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("n_h", C.c_int32), ("n_zen", C.c_int32),
+                ("h_max_m", C.c_float), ("zen_max_deg", C.c_float), ("substeps", C.c_int32)]
+
+
+class Detector(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("hist_nx", C.c_int32), ("hist_ny", C.c_int32),
+                ("hist_x0", C.c_float), ("hist_y0", C.c_float), ("hist_cell", C.c_float),
+                ("n_tel", C.c_int32), ("tel_xyzr", _fp), ("cam_enabled", C.c_int32),
+                ("cam_axis_az_deg", C.c_float), ("cam_axis_el_deg", C.c_float), ("cam_pix_deg", C.c_float),
+                ("cam_rows", C.c_int32), ("cam_cols", C.c_int32), ("n_tbins", C.c_int32),
+                ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_float)]
+
+
+class Params(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("emit", C.c_int32), ("trace", C.c_int32), ("trans", C.c_int32),
+                ("write", C.c_int32), ("filter_lv1", C.c_int32), ("filter_lv2", C.c_int32),
+                ("lambda_min_nm", C.c_float), ("lambda_max_nm", C.c_float), ("bunch_weight", C.c_float),
+                ("lv1_margin_rad", C.c_float), ("lv2_margin_m", C.c_float),
+                ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float), ("n_lines", C.c_int32),
+                ("line_nm", _fp), ("line_cdf", _fp)]
+
+
+class Segments(C.Structure):
+    _fields_ = [("size", C.c_uint32)] + [(k, C.c_void_p) for k in
+                                          ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
+
+
+class Outputs(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("hist", C.c_void_p), ("tel_counts", C.c_void_p), ("photons", C.c_void_p),
+                ("photon_weight", C.c_void_p), ("photon_capacity", C.c_int64), ("counters", C.c_void_p)]
+
+
+SEG_FIELDS = ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")
+
+_lib = None
+
+
+def load_library():
+    """dlopen libc8ph.so; raises if it is missing (there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2405_04229_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.c8ph_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
+        L.c8ph_destroy.argtypes = [C.c_void_p]
+        L.c8ph_last_error.argtypes = [C.c_void_p]
+        L.c8ph_last_error.restype = C.c_char_p
+        L.c8ph_init_atmosphere.argtypes = [C.c_void_p, C.POINTER(AtmosphereDesc)]
+        L.c8ph_build_trace_table.argtypes = [C.c_void_p, C.POINTER(TableDesc), C.c_void_p]
+        L.c8ph_get_trace_table.argtypes = [C.c_void_p, _fp, C.c_int64]
+        L.c8ph_set_trace_table.argtypes = [C.c_void_p, C.POINTER(TableDesc), _fp]
+        L.c8ph_set_detector.argtypes = [C.c_void_p, C.POINTER(Detector)]
+        L.c8ph_emit_propagate.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_int64, C.c_int64,
+                                          C.POINTER(Params), C.c_uint64, C.POINTER(Outputs), C.c_void_p]
+        L.c8ph_emit_propagate_host.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_int64, C.c_int64,
+                                               C.POINTER(Params), C.c_uint64, C.POINTER(Outputs)]
+        L.c8ph_last_kernel_ms.argtypes = [C.c_void_p]
+        L.c8ph_last_kernel_ms.restype = C.c_float
+        L.c8ph_launch_count.argtypes = [C.c_void_p]
+        L.c8ph_launch_count.restype = C.c_int64
+        L.c8ph_counter_name.argtypes = [C.c_int]
+        L.c8ph_counter_name.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+class C8phError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libc8ph error {code}: {msg}")
+        self.code = code
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+class Context:
+    """One libc8ph context on one CUDA device.  Method names follow the C entry points."""
+
+    def __init__(self, device: int = 0):
+        self.lib = load_library()
+        self._h = C.c_void_p()
+        rc = self.lib.c8ph_create(C.byref(self._h), int(device))
+        if rc:
+            raise C8phError(rc, self.lib.c8ph_last_error(None).decode())
+        self.device = int(device)
+        self._det = None
+        self._keep = []
+
+    def close(self):
+        if self._h:
+            self.lib.c8ph_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc:
+            raise C8phError(rc, self.lib.c8ph_last_error(self._h).decode())
+
+    # ---- setup ---------------------------------------------------------------------------------
+    def init_atmosphere(self, atm: dict):
+        d = AtmosphereDesc()
+        d.size = C.sizeof(AtmosphereDesc)
+        d.model = ATM[atm["model"]]
+        d.n_const_minus_1 = float(atm["n_const_minus_1"])
+        d.h0_m, d.dh_m, d.n_nodes = float(atm["h0"]), float(atm["dh"]), int(atm["n_nodes"])
+        eta = _f32(atm["refractivity"])
+        d.refractivity = eta.ctypes.data_as(_fp)
+        xv = None
+        if atm.get("overburden") is not None:
+            xv = _f32(atm["overburden"])
+            d.overburden_gcm2 = xv.ctypes.data_as(_fp)
+        d.earth_radius_m, d.h_obs_m = float(atm["earth_radius"]), float(atm["h_obs"])
+        d.rayleigh_X_gcm2, d.rayleigh_lambda_nm = float(atm["rayleigh_X"]), float(atm["rayleigh_lambda"])
+        d.aer_L_m, d.aer_H_m = float(atm["aer_L"]), float(atm["aer_H"])
+        d.aer_lambda_nm, d.aer_angstrom = float(atm["aer_lambda"]), float(atm["aer_angstrom"])
+        self._check(self.lib.c8ph_init_atmosphere(self._h, C.byref(d)))
+
+    @staticmethod
+    def _table_desc(table: dict) -> TableDesc:
+        t = TableDesc()
+        t.size = C.sizeof(TableDesc)
+        t.n_h, t.n_zen = int(table["n_h"]), int(table["n_zen"])
+        t.h_max_m, t.zen_max_deg = float(table["h_max"]), float(table["zen_max_deg"])
+        t.substeps = int(table.get("substeps", 1))
+        return t
+
+    def build_trace_table(self, table: dict, stream=None):
+        self._table = dict(table)
+        self._check(self.lib.c8ph_build_trace_table(self._h, C.byref(self._table_desc(table)), _stream_ptr(stream)))
+
+    def get_trace_table(self) -> np.ndarray:
+        t = self._table
+        out = np.empty((t["n_h"], t["n_zen"], TABLE_CHANNELS), dtype=np.float32)
+        self._check(self.lib.c8ph_get_trace_table(self._h, out.ctypes.data_as(_fp), out.size))
+        return out
+
+    def set_trace_table(self, table: dict, data: np.ndarray):
+        self._table = dict(table)
+        data = _f32(data)
+        assert data.shape == (table["n_h"], table["n_zen"], TABLE_CHANNELS)
+        self._check(self.lib.c8ph_set_trace_table(self._h, C.byref(self._table_desc(table)), data.ctypes.data_as(_fp)))
+
+    def set_detector(self, det: dict):
+        d = Detector()
+        d.size = C.sizeof(Detector)
+        d.hist_nx, d.hist_ny = int(det["hist_nx"]), int(det["hist_ny"])
+        d.hist_x0, d.hist_y0, d.hist_cell = float(det["hist_x0"]), float(det["hist_y0"]), float(det["hist_cell"])
+        tel = _f32(det["tel_xyzr"]).reshape(-1, 4)
+        d.n_tel = tel.shape[0]
+        d.tel_xyzr = tel.ctypes.data_as(_fp) if tel.shape[0] else None
+        d.cam_enabled = int(bool(det["cam_enabled"]))
+        d.cam_axis_az_deg, d.cam_axis_el_deg = float(det["cam_az_deg"]), float(det["cam_el_deg"])
+        d.cam_pix_deg = float(det["cam_pix_deg"])
+        d.cam_rows, d.cam_cols, d.n_tbins = int(det["cam_rows"]), int(det["cam_cols"]), int(det["n_tbins"])
+        d.t_ref_ns, d.t_bin_ns = float(det["t_ref_ns"]), float(det["t_bin_ns"])
+        self._check(self.lib.c8ph_set_detector(self._h, C.byref(d)))
+        self._det = dict(det)
+        self._n_tel = tel.shape[0]
+
+    def n_hist(self) -> int:
+        d = self._det
+        if d["cam_enabled"]:
+            return d["cam_rows"] * d["cam_cols"] * d["n_tbins"]
+        return d["hist_nx"] * d["hist_ny"]
+
+    def _params(self, par: dict):
+        p = Params()
+        p.size = C.sizeof(Params)
+        p.emit, p.trace, p.trans = EMIT[par["emit"]], TRACE[par["trace"]], TRANS[par["trans"]]
+        p.write = WRITE[par["write"]]
+        p.filter_lv1, p.filter_lv2 = int(bool(par["lv1"])), int(bool(par["lv2"]))
+        p.lambda_min_nm, p.lambda_max_nm = float(par["lambda_min_nm"]), float(par["lambda_max_nm"])
+        p.bunch_weight = float(par["bunch_weight"])
+        p.lv1_margin_rad, p.lv2_margin_m = float(par["lv1_margin_rad"]), float(par["lv2_margin_m"])
+        p.fluor_yield_per_MeV, p.aim_factor = float(par["fluor_yield_per_MeV"]), float(par["aim_factor"])
+        ln, lc = _f32(par["line_nm"]), _f32(par["line_cdf"])
+        p.n_lines = len(ln)
+        if len(ln):
+            p.line_nm, p.line_cdf = ln.ctypes.data_as(_fp), lc.ctypes.data_as(_fp)
+        return p, (ln, lc)
+
+    # ---- the hot call, DEVICE buffers ------------------------------------------------------------
+    def emit_propagate(self, seg_dev: dict, n_segments: int, seg_id_base: int, par: dict, seed: int,
+                       out: dict, stream=None):
+        """seg_dev: dict of torch CUDA float32 tensors (SoA); out: dict with torch CUDA tensors
+        'hist' (f32), 'tel_counts' (f32), 'photons' (uint8, 32 B/record), 'photon_weight' (f32),
+        'counters' (int64[N_COUNTERS]); any but 'counters' may be None.  Asynchronous."""
+        s = Segments()
+        s.size = C.sizeof(Segments)
+        for k in SEG_FIELDS:
+            t = seg_dev.get(k)
+            setattr(s, k, _dev_ptr(t, "float32", n_segments) if t is not None else None)
+        o = Outputs()
+        o.size = C.sizeof(Outputs)
+        o.hist = _dev_ptr(out.get("hist"), "float32", self.n_hist())
+        o.tel_counts = _dev_ptr(out.get("tel_counts"), "float32", self._n_tel)
+        ph = out.get("photons")
+        cap = 0
+        if ph is not None:
+            cap = ph.numel() * ph.element_size() // 32
+            o.photons = _dev_ptr(ph, None, 0)
+        pw = out.get("photon_weight")
+        o.photon_weight = _dev_ptr(pw, "float32", cap) if pw is not None else None
+        o.photon_capacity = cap
+        o.counters = _dev_ptr(out["counters"], "int64", N_COUNTERS)
+        p, keep = self._params(par)
+        self._check(self.lib.c8ph_emit_propagate(self._h, C.byref(s), int(n_segments), int(seg_id_base),
+                                                 C.byref(p), C.c_uint64(int(seed)), C.byref(o), _stream_ptr(stream)))
+        del keep
+
+    # ---- the same call with HOST buffers (end-to-end path) ---------------------------------------
+    def emit_propagate_host(self, seg_host: dict, n_segments: int, seg_id_base: int, par: dict, seed: int,
+                            photon_capacity: int = 0, want_weight: bool = False, out: Optional[dict] = None) -> dict:
+        """seg_host: dict of numpy float32 arrays (or pinned torch CPU tensors).  Returns a dict of
+        numpy arrays: hist, tel_counts, counters{name: int}, photons (structured), photon_weight."""
+        s = Segments()
+        s.size = C.sizeof(Segments)
+        keep = []
+        for k in SEG_FIELDS:
+            a = seg_host.get(k)
+            if a is None:
+                continue
+            if hasattr(a, "data_ptr"):
+                assert str(a.dtype) == "torch.float32" and a.is_contiguous() and a.numel() >= n_segments
+                setattr(s, k, a.data_ptr())
+                keep.append(a)
+            else:
+                a = _f32(a)
+                assert a.size >= n_segments
+                keep.append(a)
+                setattr(s, k, a.ctypes.data)
+        if out is None:
+            out = self.alloc_host_outputs(photon_capacity, want_weight)
+        o = Outputs()
+        o.size = C.sizeof(Outputs)
+        o.hist = out["hist"].ctypes.data if out["hist"].size else None
+        o.tel_counts = out["tel_counts"].ctypes.data if out["tel_counts"].size else None
+        o.photons = out["photons"].ctypes.data if len(out["photons"]) else None
+        o.photon_weight = out["photon_weight"].ctypes.data if out.get("photon_weight") is not None and len(out["photon_weight"]) else None
+        o.photon_capacity = len(out["photons"])
+        o.counters = out["counters_raw"].ctypes.data
+        p, keep2 = self._params(par)
+        self._check(self.lib.c8ph_emit_propagate_host(self._h, C.byref(s), int(n_segments), int(seg_id_base),
+                                                      C.byref(p), C.c_uint64(int(seed)), C.byref(o)))
+        del keep, keep2
+        cnt = out["counters_raw"]
+        res = dict(out)
+        res["counters"] = {k: int(v) for k, v in zip(COUNTER_NAMES, cnt)}
+        n = min(res["counters"]["written"], len(out["photons"]))
+        res["photons"] = out["photons"][:n]
+        if res.get("photon_weight") is not None:
+            res["photon_weight"] = out["photon_weight"][:n]
+        return res
+
+    def alloc_host_outputs(self, photon_capacity: int = 0, want_weight: bool = False) -> dict:
+        return dict(hist=np.zeros(self.n_hist(), dtype=np.float32),
+                    tel_counts=np.zeros(self._n_tel, dtype=np.float32),
+                    photons=np.zeros(int(photon_capacity), dtype=PHOTON_DTYPE),
+                    photon_weight=np.zeros(int(photon_capacity), dtype=np.float32) if want_weight else None,
+                    counters_raw=np.zeros(N_COUNTERS, dtype=np.uint64))
+
+    def last_kernel_ms(self) -> float:
+        return float(self.lib.c8ph_last_kernel_ms(self._h))
+
+    def launch_count(self) -> int:
+        return int(self.lib.c8ph_launch_count(self._h))
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if hasattr(stream, "cuda_stream"):
+        return C.c_void_p(stream.cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+def _dev_ptr(t, dtype, min_elems):
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    if dtype is not None:
+        assert str(t.dtype) == "torch." + dtype, (t.dtype, dtype)
+        assert t.numel() >= min_elems, (t.numel(), min_elems)
+    return t.data_ptr()
+
+
+# ---- convenience: run a whole workload dict on the device -----------------------------------------
+def setup_context(cfg: dict, device: int = 0, ctx: Optional[Context] = None) -> Context:
+    """create -> init_atmosphere -> set_detector -> build_trace_table for a workloads.make_config dict."""
+    ctx = ctx or Context(device)
+    ctx.init_atmosphere(cfg["atmosphere"])
+    ctx.set_detector(cfg["detector"])
+    if cfg.get("table") is not None:
+        ctx.build_trace_table(cfg["table"])
+    return ctx
+
+
+def segments_to_device(seg: dict, device: int = 0) -> dict:
+    import torch
+    return {k: torch.from_numpy(_f32(v)).to(f"cuda:{device}") for k, v in seg.items()}
+
+
+def alloc_device_outputs(ctx: Context, photon_capacity: int, want_weight: bool = False, device: int = 0) -> dict:
+    import torch
+    dev = f"cuda:{device}"
+    return dict(hist=torch.zeros(max(ctx.n_hist(), 1), dtype=torch.float32, device=dev),
+                tel_counts=torch.zeros(max(ctx._n_tel, 1), dtype=torch.float32, device=dev),
+                photons=torch.zeros((max(int(photon_capacity), 1), 32), dtype=torch.uint8, device=dev) if photon_capacity else None,
+                photon_weight=torch.zeros(max(int(photon_capacity), 1), dtype=torch.float32, device=dev) if (want_weight and photon_capacity) else None,
+                counters=torch.zeros(N_COUNTERS, dtype=torch.int64, device=dev))
+
+
+def outputs_to_host(ctx: Context, out: dict) -> dict:
+    """Synchronising copy of device outputs into numpy (tests / examples)."""
+    cnt = out["counters"].cpu().numpy().astype(np.uint64)
+    res = dict(counters={k: int(v) for k, v in zip(COUNTER_NAMES, cnt)})
+    res["hist"] = out["hist"].cpu().numpy()[:ctx.n_hist()]
+    res["tel_counts"] = out["tel_counts"].cpu().numpy()[:ctx._n_tel]
+    if out.get("photons") is not None:
+        n = min(res["counters"]["written"], out["photons"].shape[0])
+        res["photons"] = out["photons"][:n].cpu().numpy().view(PHOTON_DTYPE).reshape(-1)
+        if out.get("photon_weight") is not None:
+            res["photon_weight"] = out["photon_weight"][:n].cpu().numpy()
+    else:
+        res["photons"] = np.zeros(0, dtype=PHOTON_DTYPE)
+    return res
+
+
+def run_config(cfg: dict, ctx: Optional[Context] = None, photon_capacity: Optional[int] = None,
+               want_weight: bool = True, device: int = 0) -> dict:
+    """One pass of the whole path over cfg['segments'] with device-resident inputs (tests / smoke)."""
+    import torch
+    ctx = ctx or setup_context(cfg, device)
+    seg = segments_to_device(cfg["segments"], device)
+    n = len(cfg["segments"]["x"])
+    if photon_capacity is None:
+        photon_capacity = 1 << 22
+    out = alloc_device_outputs(ctx, photon_capacity, want_weight, device)
+    ctx.emit_propagate(seg, n, cfg["seg_id_base"], cfg["params"], cfg["seed"], out)
+    torch.cuda.synchronize()
+    res = outputs_to_host(ctx, out)
+    res["kernel_ms"] = ctx.last_kernel_ms()
+    return res

@@ -1,0 +1,95 @@
+// c8ph_device.cuh — launch-argument structs shared by the host API and the kernels of libc8ph.
+// (Internal to the CUDA library; the CPU oracle under oracle/ shares nothing with this.)
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/c8ph.h"
+
+namespace c8ph {
+
+struct DevAtm {
+    int model;              // C8PH_ATM_*
+    int n_nodes;            // nodes of the n(h) grid (>= 2; homogeneous: 2 identical nodes)
+    int n_pad;              // floats per table array, multiple of 4 (16 B, bulk-copy granule)
+    float h0, dh, inv_dh, h_top;
+    const float *eta;       // DEVICE [n_pad] refractivity n-1 at the nodes
+    const float *xv;        // DEVICE [n_pad] vertical overburden at the nodes (zeros if none)
+    const float *eta_mid;   // DEVICE [n_pad] refractivity at the cell mid height (layer k = nodes k..k+1)
+    const float *dxv;       // DEVICE [n_pad] X_v(node k) - X_v(node k+1)
+    double R, h_obs, Rg;    // Earth radius, observation altitude, R + h_obs
+    float eta_g;            // refractivity at the observation level
+    float ray_inv_X;        // 1 / X_R, 0 = Rayleigh off
+    float ray_lambda;       // lambda_R [nm]
+    float aer_L, aer_H, aer_lambda, aer_angstrom;
+};
+
+struct DevTable {
+    int n_h, n_zen;
+    float h_max, zen_max;           // [m], [rad]
+    float inv_dh, inv_dz;           // (n_h-1)/h_max, (n_zen-1)/zen_max
+    const float4 *hot;              // DEVICE [n_h][n_zen] = (dd, dt, X_slant, tau_aer)
+    const float *full;              // DEVICE [n_h][n_zen][5]
+};
+
+struct DevGrid {                    // uniform grid over telescopes; cell lists of candidate indices
+    float x0, y0, inv_cs;
+    int nx, ny;
+    const int *start;               // DEVICE [nx*ny+1]
+    const int *items;               // DEVICE
+};
+
+struct DevDet {
+    int hist_nx, hist_ny;
+    float hist_x0, hist_y0, hist_cell, hist_inv_cell;
+    int n_tel;
+    const float4 *tel;              // DEVICE [n_tel]
+    int use_grid;                   // 0: brute force over all telescopes
+    float grid_min_cos;             // the grids are valid for |u_z| >= grid_min_cos
+    DevGrid lv2, hit;
+    double r_array;                 // bounding radius of telescopes + histogram about the origin
+    int cam_enabled, cam_rows, cam_cols, n_tbins;
+    float cam_w[3], cam_r[3], cam_u[3];   // camera frame: axis, right, up
+    float cam_pitch, cam_inv_pitch;       // [rad]
+    double t_ref;
+    float t_bin, inv_t_bin;
+};
+
+struct DevRun {
+    int emit, trace, trans, write, lv1, lv2;
+    float il1, il2;                 // 1/lambda_min, 1/lambda_max  [1/nm]
+    float w;                        // bunch weight
+    double yield_k;                 // Cherenkov: 2 pi alpha (1/l1 - 1/l2) [1/m]
+    double lv1_margin;
+    float lv2_margin;
+    double fluor_yield, aim_factor;
+    int n_lines;
+    const float *line_nm, *line_cdf;      // DEVICE
+    uint32_t key0[10], key1[10];    // Philox round keys
+    int64_t n_seg, seg_id_base;
+    c8ph_segments seg;              // DEVICE pointers
+    c8ph_outputs out;               // DEVICE pointers
+    unsigned long long *cursor;     // DEVICE work cursor (segments)
+    int segs_per_grab;              // segments one warp prepares per grab (1..32)
+};
+
+struct KArgs {
+    DevAtm atm;
+    DevTable tab;
+    DevDet det;
+    DevRun run;
+};
+
+struct TableBuildArgs {
+    DevAtm atm;
+    int n_h, n_zen, substeps;
+    double h_max, zen_max;
+    float *full;                    // [n_h][n_zen][5]
+    float4 *hot;                    // [n_h][n_zen]
+};
+
+// kernels / launchers (c8ph_kernels.cu)
+cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st);
+cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st);
+size_t emit_smem_bytes(const KArgs &a);
+
+}  // namespace c8ph

@@ -1,0 +1,559 @@
+// c8ph_host.cu — host side of libc8ph: context, argument validation, table / detector setup and
+// kernel launches behind the C-ABI of include/c8ph.h.  No torch types, no exceptions across the ABI.
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include "c8ph_device.cuh"
+
+using namespace c8ph;
+
+struct c8ph_ctx {
+    int device = 0;
+    int n_sm = 0;
+    std::string err;
+    // atmosphere
+    bool have_atm = false;
+    DevAtm atm{};
+    float *d_eta = nullptr, *d_xv = nullptr, *d_mid = nullptr, *d_dxv = nullptr;
+    // table
+    bool have_table = false;
+    DevTable tab{};
+    c8ph_table_desc tab_desc{};
+    float *d_full = nullptr;
+    float4 *d_hot = nullptr;
+    // detector
+    bool have_det = false;
+    DevDet det{};
+    float4 *d_tel = nullptr;
+    int *d_g_start[2] = {nullptr, nullptr}, *d_g_items[2] = {nullptr, nullptr};
+    // run scratch
+    unsigned long long *d_cursor = nullptr;
+    float *d_lines = nullptr;          // [2][max_lines]
+    int lines_cap = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool timed = false;
+    int64_t launches = 0;
+    // host-path scratch
+    float *d_seg = nullptr; size_t seg_cap = 0;
+    void *d_out = nullptr; size_t out_cap = 0;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(c8ph_ctx *ctx, int code, const std::string &msg)
+{
+    if (ctx) ctx->err = msg; else g_create_err = msg;
+    return code;
+}
+static int cuda_fail(c8ph_ctx *ctx, cudaError_t e, const char *what)
+{
+    return fail(ctx, C8PH_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                                        \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);        \
+    } while (0)
+
+template <typename T>
+static void dfree(T *&p)
+{
+    if (p) cudaFree(p);
+    p = nullptr;
+}
+
+extern "C" int c8ph_version(void) { return C8PH_VERSION; }
+
+extern "C" const char *c8ph_last_error(const c8ph_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
+{
+    if (!out) return fail(nullptr, C8PH_E_ARG, "c8ph_create: out is NULL");
+    *out = nullptr;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n <= 0)
+        return fail(nullptr, C8PH_E_CUDA, std::string("c8ph_create: no CUDA device: ") + cudaGetErrorString(e));
+    if (cuda_device < 0 || cuda_device >= n) return fail(nullptr, C8PH_E_ARG, "c8ph_create: bad device index");
+    c8ph_ctx *ctx = new (std::nothrow) c8ph_ctx();
+    if (!ctx) return fail(nullptr, C8PH_E_NOMEM, "c8ph_create: out of host memory");
+    ctx->device = cuda_device;
+    if ((e = cudaSetDevice(cuda_device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
+        (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess) {
+        g_create_err = std::string("c8ph_create: ") + cudaGetErrorString(e);
+        delete ctx;
+        return C8PH_E_CUDA;
+    }
+    *out = ctx;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_destroy(c8ph_ctx *ctx)
+{
+    if (!ctx) return C8PH_E_ARG;
+    cudaSetDevice(ctx->device);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
+    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
+    for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); }
+    dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_seg);
+    if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    delete ctx;
+    return C8PH_OK;
+}
+
+// ------------------------------------------------------------------------------------ atmosphere
+static double lerp_table(const std::vector<float> &t, double h0, double dh, double h)
+{
+    double f = (h - h0) / dh;
+    f = std::min(std::max(f, 0.0), (double)(t.size() - 1));
+    int k = std::min((int)f, (int)t.size() - 2);
+    double fr = f - k;
+    return (1.0 - fr) * t[k] + fr * t[k + 1];
+}
+
+extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!d || d->size != sizeof(c8ph_atmosphere_desc)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: bad desc/size");
+    if (d->model < C8PH_ATM_HOMOGENEOUS || d->model > C8PH_ATM_SPHERICAL) return fail(ctx, C8PH_E_ARG, "init_atmosphere: bad model");
+    CU(cudaSetDevice(ctx->device));
+    std::vector<float> eta, xv;
+    double h0 = d->h0_m, dh = d->dh_m;
+    if (d->model == C8PH_ATM_HOMOGENEOUS) {
+        eta.assign(2, d->n_const_minus_1);
+        xv.assign(2, 0.f);
+        h0 = 0.0; dh = 1.0e6;
+    } else {
+        if (d->n_nodes < 2 || !d->refractivity || !(d->dh_m > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: need n_nodes >= 2, refractivity, dh > 0");
+        if (d->n_nodes > 16000) return fail(ctx, C8PH_E_ARG, "init_atmosphere: n_nodes > 16000 does not fit the shared-memory staging");
+        eta.assign(d->refractivity, d->refractivity + d->n_nodes);
+        if (d->overburden_gcm2) xv.assign(d->overburden_gcm2, d->overburden_gcm2 + d->n_nodes);
+        else xv.assign(d->n_nodes, 0.f);
+    }
+    for (float v : eta) if (!(v > -1.f) || !std::isfinite(v)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: non-finite refractivity");
+    if (d->model == C8PH_ATM_SPHERICAL && !(d->earth_radius_m > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: earth_radius");
+    const int n = (int)eta.size();
+    const int n_pad = (n + 3) & ~3;
+    std::vector<float> mid(n_pad, 0.f), dxv(n_pad, 0.f), eta_p(n_pad, eta.back()), xv_p(n_pad, xv.back());
+    for (int k = 0; k < n; ++k) { eta_p[k] = eta[k]; xv_p[k] = xv[k]; }
+    for (int k = 0; k + 1 < n; ++k) {
+        mid[k] = (float)(0.5 * ((double)eta[k] + (double)eta[k + 1]));   // Listing 4.1 at the cell mid height
+        dxv[k] = (float)((double)xv[k] - (double)xv[k + 1]);
+    }
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
+    const size_t bytes = (size_t)n_pad * sizeof(float);
+    CU(cudaMalloc(&ctx->d_eta, bytes)); CU(cudaMalloc(&ctx->d_xv, bytes));
+    CU(cudaMalloc(&ctx->d_mid, bytes)); CU(cudaMalloc(&ctx->d_dxv, bytes));
+    CU(cudaMemcpy(ctx->d_eta, eta_p.data(), bytes, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_xv, xv_p.data(), bytes, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_mid, mid.data(), bytes, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_dxv, dxv.data(), bytes, cudaMemcpyHostToDevice));
+    DevAtm &a = ctx->atm;
+    a.model = d->model; a.n_nodes = n; a.n_pad = n_pad;
+    a.h0 = (float)h0; a.dh = (float)dh; a.inv_dh = (float)(1.0 / dh); a.h_top = (float)(h0 + dh * (n - 1));
+    a.eta = ctx->d_eta; a.xv = ctx->d_xv; a.eta_mid = ctx->d_mid; a.dxv = ctx->d_dxv;
+    a.R = d->earth_radius_m; a.h_obs = d->h_obs_m; a.Rg = (double)d->earth_radius_m + (double)d->h_obs_m;
+    a.eta_g = (float)lerp_table(eta, h0, dh, d->h_obs_m);
+    a.ray_inv_X = d->rayleigh_X_gcm2 > 0.f ? 1.0f / d->rayleigh_X_gcm2 : 0.f;
+    a.ray_lambda = d->rayleigh_lambda_nm;
+    a.aer_L = d->aer_L_m; a.aer_H = d->aer_H_m; a.aer_lambda = d->aer_lambda_nm; a.aer_angstrom = d->aer_angstrom;
+    if (a.aer_L > 0.f && !(a.aer_H > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: aerosol scale height");
+    ctx->have_atm = true;
+    ctx->have_table = false;
+    return C8PH_OK;
+}
+
+// ------------------------------------------------------------------------------------ trace table
+static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
+{
+    if (!t || t->size != sizeof(c8ph_table_desc)) return fail(ctx, C8PH_E_ARG, "trace_table: bad desc/size");
+    if (t->n_h < 2 || t->n_zen < 2 || (int64_t)t->n_h * t->n_zen > (1 << 26) || !(t->h_max_m > 0.f) ||
+        !(t->zen_max_deg > 0.f) || !(t->zen_max_deg < 90.f))
+        return fail(ctx, C8PH_E_ARG, "trace_table: need n_h,n_zen >= 2, h_max > 0, 0 < zen_max < 90");
+    if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "trace_table: atmosphere not initialised");
+    CU(cudaSetDevice(ctx->device));
+    dfree(ctx->d_full); dfree(ctx->d_hot);
+    const size_t n = (size_t)t->n_h * t->n_zen;
+    CU(cudaMalloc(&ctx->d_full, n * C8PH_TABLE_CHANNELS * sizeof(float)));
+    CU(cudaMalloc(&ctx->d_hot, n * sizeof(float4)));
+    ctx->tab_desc = *t;
+    DevTable &d = ctx->tab;
+    d.n_h = t->n_h; d.n_zen = t->n_zen; d.h_max = t->h_max_m;
+    const double zmax = (double)t->zen_max_deg * (3.14159265358979323846 / 180.0);
+    d.zen_max = (float)zmax;
+    d.inv_dh = (float)((t->n_h - 1) / (double)t->h_max_m);
+    d.inv_dz = (float)((t->n_zen - 1) / zmax);
+    d.hot = ctx->d_hot; d.full = ctx->d_full;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, void *stream)
+{
+    if (!ctx) return C8PH_E_ARG;
+    int rc = alloc_table(ctx, t);
+    if (rc) return rc;
+    TableBuildArgs a{};
+    a.atm = ctx->atm;
+    a.n_h = t->n_h; a.n_zen = t->n_zen; a.substeps = std::max(1, t->substeps);
+    a.h_max = t->h_max_m;
+    a.zen_max = (double)t->zen_max_deg * (3.14159265358979323846 / 180.0);
+    a.full = ctx->d_full; a.hot = ctx->d_hot;
+    cudaError_t e = launch_build_table(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "build_trace_table launch");
+    ctx->launches++;
+    ctx->have_table = true;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_get_trace_table(c8ph_ctx *ctx, float *host_out, int64_t n_floats)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!ctx->have_table) return fail(ctx, C8PH_E_STATE, "get_trace_table: no table");
+    const int64_t need = (int64_t)ctx->tab.n_h * ctx->tab.n_zen * C8PH_TABLE_CHANNELS;
+    if (!host_out || n_floats < need) return fail(ctx, C8PH_E_ARG, "get_trace_table: buffer too small");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(host_out, ctx->d_full, need * sizeof(float), cudaMemcpyDeviceToHost));
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, const float *host_in)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!host_in) return fail(ctx, C8PH_E_ARG, "set_trace_table: host_in is NULL");
+    int rc = alloc_table(ctx, t);
+    if (rc) return rc;
+    const size_t n = (size_t)t->n_h * t->n_zen;
+    std::vector<float4> hot(n);
+    for (size_t i = 0; i < n; ++i) {
+        const float *v = host_in + i * C8PH_TABLE_CHANNELS;
+        hot[i] = make_float4(v[0], v[2], v[3], v[4]);
+    }
+    CU(cudaMemcpy(ctx->d_full, host_in, n * C8PH_TABLE_CHANNELS * sizeof(float), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_hot, hot.data(), n * sizeof(float4), cudaMemcpyHostToDevice));
+    ctx->have_table = true;
+    return C8PH_OK;
+}
+
+// ------------------------------------------------------------------------------------ detector
+// Uniform grid over the telescope footprints: cell -> telescopes whose disc of radius `reach_k`
+// about the centre overlaps the cell.  Item lists are ascending in k.
+static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, const std::vector<double> &reach, DevGrid &g)
+{
+    const int n = (int)reach.size();
+    double x0 = 1e300, y0 = 1e300, x1 = -1e300, y1 = -1e300, rmax = 0.0;
+    for (int k = 0; k < n; ++k) {
+        x0 = std::min(x0, tel[4 * k] - reach[k]); x1 = std::max(x1, tel[4 * k] + reach[k]);
+        y0 = std::min(y0, tel[4 * k + 1] - reach[k]); y1 = std::max(y1, tel[4 * k + 1] + reach[k]);
+        rmax = std::max(rmax, reach[k]);
+    }
+    double cs = std::max(rmax, std::max(x1 - x0, y1 - y0) / 2048.0);
+    if (!(cs > 0.0)) cs = 1.0;
+    const int nx = std::max(1, (int)std::ceil((x1 - x0) / cs)), ny = std::max(1, (int)std::ceil((y1 - y0) / cs));
+    std::vector<int> count((size_t)nx * ny + 1, 0);
+    auto cells = [&](int k, int &cx0, int &cx1, int &cy0, int &cy1) {
+        cx0 = std::max(0, (int)std::floor((tel[4 * k] - reach[k] - x0) / cs) - 1);
+        cx1 = std::min(nx - 1, (int)std::floor((tel[4 * k] + reach[k] - x0) / cs) + 1);
+        cy0 = std::max(0, (int)std::floor((tel[4 * k + 1] - reach[k] - y0) / cs) - 1);
+        cy1 = std::min(ny - 1, (int)std::floor((tel[4 * k + 1] + reach[k] - y0) / cs) + 1);
+    };
+    // a telescope is listed in a cell iff its disc overlaps the cell rectangle (padded by 1e-3 cell)
+    auto overlaps = [&](int k, int cx, int cy) {
+        const double pad = 1e-3 * cs;
+        const double bx0 = x0 + cx * cs - pad, bx1 = x0 + (cx + 1) * cs + pad, by0 = y0 + cy * cs - pad, by1 = y0 + (cy + 1) * cs + pad;
+        const double px = std::min(std::max((double)tel[4 * k], bx0), bx1), py = std::min(std::max((double)tel[4 * k + 1], by0), by1);
+        const double dx = px - tel[4 * k], dy = py - tel[4 * k + 1];
+        return dx * dx + dy * dy <= reach[k] * reach[k];
+    };
+    for (int k = 0; k < n; ++k) {
+        int a, b, c, d; cells(k, a, b, c, d);
+        for (int cy = c; cy <= d; ++cy) for (int cx = a; cx <= b; ++cx) if (overlaps(k, cx, cy)) count[(size_t)cy * nx + cx + 1]++;
+    }
+    for (size_t i = 1; i < count.size(); ++i) count[i] += count[i - 1];
+    std::vector<int> items(std::max<size_t>(1, (size_t)count.back())), fill(count.begin(), count.end() - 1);
+    for (int k = 0; k < n; ++k) {
+        int a, b, c, d; cells(k, a, b, c, d);
+        for (int cy = c; cy <= d; ++cy) for (int cx = a; cx <= b; ++cx) if (overlaps(k, cx, cy)) items[fill[(size_t)cy * nx + cx]++] = k;
+    }
+    dfree(ctx->d_g_start[which]); dfree(ctx->d_g_items[which]);
+    CU(cudaMalloc(&ctx->d_g_start[which], count.size() * sizeof(int)));
+    CU(cudaMalloc(&ctx->d_g_items[which], items.size() * sizeof(int)));
+    CU(cudaMemcpy(ctx->d_g_start[which], count.data(), count.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_g_items[which], items.data(), items.size() * sizeof(int), cudaMemcpyHostToDevice));
+    g.x0 = (float)x0; g.y0 = (float)y0; g.inv_cs = (float)(1.0 / cs); g.nx = nx; g.ny = ny;
+    g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
+    return C8PH_OK;
+}
+
+static int setup_detector(c8ph_ctx *ctx, const c8ph_detector *d, float lv2_margin_for_grid)
+{
+    DevDet &o = ctx->det;
+    const int n = d->n_tel;
+    std::vector<float> tel(d->tel_xyzr ? d->tel_xyzr : nullptr, d->tel_xyzr ? d->tel_xyzr + 4 * (size_t)n : nullptr);
+    if (n > 0) {
+        const double min_cos = 0.2588190451;                       // grids valid up to 75 deg zenith
+        o.grid_min_cos = (float)(min_cos * (1.0 + 1e-6));
+        o.use_grid = n > 8 ? 1 : 0;
+        if (o.use_grid) {
+            std::vector<double> r_hit(n), r_lv2(n);
+            for (int k = 0; k < n; ++k) {
+                const double tant = std::sqrt(1.0 - min_cos * min_cos) / min_cos;
+                // footprint of the sphere on z = 0 for zenith <= 75 deg, inflated for fp32 rounding
+                r_hit[k] = (tel[4 * k + 3] / min_cos + std::fabs(tel[4 * k + 2]) * tant) * 1.001 + 1e-3;
+                r_lv2[k] = (tel[4 * k + 3] / min_cos + lv2_margin_for_grid) * 1.001 + 1e-3;
+            }
+            int rc = build_grid(ctx, 0, tel, r_hit, o.hit);
+            if (rc) return rc;
+            rc = build_grid(ctx, 1, tel, r_lv2, o.lv2);
+            if (rc) return rc;
+        }
+    }
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!d || d->size != sizeof(c8ph_detector)) return fail(ctx, C8PH_E_ARG, "set_detector: bad desc/size");
+    if (d->hist_nx < 0 || d->hist_ny < 0 || (int64_t)d->hist_nx * d->hist_ny > (1ll << 30)) return fail(ctx, C8PH_E_ARG, "set_detector: hist size");
+    if ((d->hist_nx > 0) != (d->hist_ny > 0) || (d->hist_nx > 0 && !(d->hist_cell > 0.f))) return fail(ctx, C8PH_E_ARG, "set_detector: hist grid");
+    if (d->n_tel < 0 || d->n_tel >= (int)C8PH_TEL_NONE || (d->n_tel > 0 && !d->tel_xyzr)) return fail(ctx, C8PH_E_ARG, "set_detector: telescopes");
+    if (d->cam_enabled && (d->n_tel < 1 || d->cam_rows < 1 || d->cam_cols < 1 || d->n_tbins < 1 || !(d->cam_pix_deg > 0.f) || !(d->t_bin_ns > 0.f)))
+        return fail(ctx, C8PH_E_ARG, "set_detector: camera needs a telescope, rows, cols, time bins");
+    CU(cudaSetDevice(ctx->device));
+    DevDet o{};
+    o.hist_nx = d->hist_nx; o.hist_ny = d->hist_ny;
+    o.hist_x0 = d->hist_x0; o.hist_y0 = d->hist_y0; o.hist_cell = d->hist_nx > 0 ? d->hist_cell : 1.f;
+    o.hist_inv_cell = 1.0f / o.hist_cell;
+    o.n_tel = d->n_tel;
+    double r_arr = 0.0;
+    for (int k = 0; k < d->n_tel; ++k) {
+        const float *t = d->tel_xyzr + 4 * k;
+        if (!(t[3] > 0.f)) return fail(ctx, C8PH_E_ARG, "set_detector: telescope radius <= 0");
+        r_arr = std::max(r_arr, std::sqrt((double)t[0] * t[0] + (double)t[1] * t[1] + (double)t[2] * t[2]) + t[3]);
+    }
+    if (d->hist_nx > 0 && !d->cam_enabled) {
+        const double xs[2] = {d->hist_x0, (double)d->hist_x0 + d->hist_nx * (double)d->hist_cell};
+        const double ys[2] = {d->hist_y0, (double)d->hist_y0 + d->hist_ny * (double)d->hist_cell};
+        for (double x : xs) for (double y : ys) r_arr = std::max(r_arr, std::sqrt(x * x + y * y));
+    }
+    o.r_array = r_arr;
+    o.cam_enabled = d->cam_enabled ? 1 : 0;
+    o.cam_rows = d->cam_rows; o.cam_cols = d->cam_cols; o.n_tbins = d->n_tbins;
+    {
+        const double d2r = 3.14159265358979323846 / 180.0;
+        const double az = d->cam_axis_az_deg * d2r, el = d->cam_axis_el_deg * d2r;
+        const double w[3] = {std::cos(el) * std::cos(az), std::cos(el) * std::sin(az), std::sin(el)};
+        const double r[3] = {-std::sin(az), std::cos(az), 0.0};
+        const double u[3] = {w[1] * r[2] - w[2] * r[1], w[2] * r[0] - w[0] * r[2], w[0] * r[1] - w[1] * r[0]};
+        for (int k = 0; k < 3; ++k) { o.cam_w[k] = (float)w[k]; o.cam_r[k] = (float)r[k]; o.cam_u[k] = (float)u[k]; }
+        o.cam_pitch = (float)(d->cam_pix_deg * d2r);
+        o.cam_inv_pitch = d->cam_pix_deg > 0.f ? (float)(1.0 / (d->cam_pix_deg * d2r)) : 0.f;
+    }
+    o.t_ref = d->t_ref_ns; o.t_bin = d->t_bin_ns; o.inv_t_bin = d->t_bin_ns > 0.f ? 1.0f / d->t_bin_ns : 0.f;
+    dfree(ctx->d_tel);
+    if (d->n_tel > 0) {
+        CU(cudaMalloc(&ctx->d_tel, (size_t)d->n_tel * sizeof(float4)));
+        CU(cudaMemcpy(ctx->d_tel, d->tel_xyzr, (size_t)d->n_tel * sizeof(float4), cudaMemcpyHostToDevice));
+    }
+    o.tel = ctx->d_tel;
+    ctx->det = o;
+    // the LV2 grid is built for margins up to 64 m; larger margins fall back to brute force (see emit)
+    int rc = setup_detector(ctx, d, 64.0f);
+    if (rc) return rc;
+    ctx->have_det = true;
+    return C8PH_OK;
+}
+
+// ------------------------------------------------------------------------------------ the hot call
+static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64_t base, const c8ph_params *p,
+                     uint64_t seed, const c8ph_outputs *o, KArgs &a, cudaStream_t st)
+{
+    if (!s || s->size != sizeof(c8ph_segments) || !p || p->size != sizeof(c8ph_params) || !o || o->size != sizeof(c8ph_outputs))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: NULL struct or size mismatch");
+    if (n_seg < 0 || base < 0) return fail(ctx, C8PH_E_ARG, "emit_propagate: negative n_segments / seg_id_base");
+    if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "emit_propagate: atmosphere not initialised");
+    if (!ctx->have_det) return fail(ctx, C8PH_E_STATE, "emit_propagate: detector not set");
+    if (n_seg > 0 && (!s->x || !s->y || !s->z || !s->dx || !s->dy || !s->dz || !s->len || !s->beta || !s->t0 || !s->charge))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: NULL segment array");
+    if (p->emit != C8PH_EMIT_CHERENKOV && p->emit != C8PH_EMIT_FLUORESCENCE) return fail(ctx, C8PH_E_ARG, "emit_propagate: emit");
+    if (p->trace < C8PH_TRACE_STRAIGHT || p->trace > C8PH_TRACE_TABLE) return fail(ctx, C8PH_E_ARG, "emit_propagate: trace");
+    if (p->trans < C8PH_TRANS_OFF || p->trans > C8PH_TRANS_ROULETTE) return fail(ctx, C8PH_E_ARG, "emit_propagate: trans");
+    if (p->write < C8PH_WRITE_NONE || p->write > C8PH_WRITE_TEL) return fail(ctx, C8PH_E_ARG, "emit_propagate: write");
+    if (!(p->bunch_weight > 0.f)) return fail(ctx, C8PH_E_ARG, "emit_propagate: bunch_weight <= 0");
+    if (!o->counters) return fail(ctx, C8PH_E_ARG, "emit_propagate: counters is NULL");
+    if (o->photons && o->photon_capacity < 0) return fail(ctx, C8PH_E_ARG, "emit_propagate: photon_capacity");
+    if (p->trace == C8PH_TRACE_TABLE && !ctx->have_table) return fail(ctx, C8PH_E_STATE, "emit_propagate: trace table not built");
+    if (p->trace == C8PH_TRACE_NUMERIC && ctx->atm.model == C8PH_ATM_SPHERICAL)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: per-photon numeric tracing is planar only; use the table in the spherical model");
+    if (p->trace == C8PH_TRACE_NUMERIC && p->emit == C8PH_EMIT_FLUORESCENCE) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence + numeric tracing");
+    if (p->emit == C8PH_EMIT_CHERENKOV && !(p->lambda_min_nm > 0.f && p->lambda_max_nm > p->lambda_min_nm))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: wavelength band");
+    if (p->emit == C8PH_EMIT_FLUORESCENCE) {
+        if (ctx->det.n_tel < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: fluorescence needs a telescope to aim at");
+        if (p->n_lines < 1 || !p->line_nm || !p->line_cdf) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence line spectrum");
+        if (n_seg > 0 && !s->edep) return fail(ctx, C8PH_E_ARG, "emit_propagate: edep is NULL");
+    }
+    if (p->filter_lv2 && p->lv2_margin_m > 64.0f && ctx->det.use_grid)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: lv2_margin_m > 64 m is not covered by the LV2 grid");
+    a.atm = ctx->atm;
+    a.tab = ctx->tab;
+    a.det = ctx->det;
+    DevRun &r = a.run;
+    r.emit = p->emit; r.trace = p->trace; r.trans = p->trans; r.write = p->write;
+    r.lv1 = p->filter_lv1 ? 1 : 0; r.lv2 = p->filter_lv2 ? 1 : 0;
+    r.il1 = p->emit == C8PH_EMIT_CHERENKOV ? 1.0f / p->lambda_min_nm : 0.f;
+    r.il2 = p->emit == C8PH_EMIT_CHERENKOV ? 1.0f / p->lambda_max_nm : 0.f;
+    r.w = p->bunch_weight;
+    r.yield_k = p->emit == C8PH_EMIT_CHERENKOV
+                    ? 2.0 * 3.14159265358979323846 / 137.035999 * (1.0 / ((double)p->lambda_min_nm * 1e-9) - 1.0 / ((double)p->lambda_max_nm * 1e-9))
+                    : 0.0;
+    r.lv1_margin = p->lv1_margin_rad; r.lv2_margin = p->lv2_margin_m;
+    r.fluor_yield = p->fluor_yield_per_MeV; r.aim_factor = p->aim_factor;
+    r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
+    if (p->emit == C8PH_EMIT_FLUORESCENCE) {
+        if (p->n_lines > ctx->lines_cap) {
+            dfree(ctx->d_lines);
+            CU(cudaMalloc(&ctx->d_lines, 2 * (size_t)p->n_lines * sizeof(float)));
+            ctx->lines_cap = p->n_lines;
+        }
+        CU(cudaMemcpyAsync(ctx->d_lines, p->line_nm, p->n_lines * sizeof(float), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(ctx->d_lines + ctx->lines_cap, p->line_cdf, p->n_lines * sizeof(float), cudaMemcpyHostToDevice, st));
+        r.n_lines = p->n_lines; r.line_nm = ctx->d_lines; r.line_cdf = ctx->d_lines + ctx->lines_cap;
+    }
+    for (int k = 0; k < 10; ++k) {
+        r.key0[k] = (uint32_t)seed + (uint32_t)k * 0x9E3779B9u;
+        r.key1[k] = (uint32_t)(seed >> 32) + (uint32_t)k * 0xBB67AE85u;
+    }
+    r.n_seg = n_seg; r.seg_id_base = base;
+    r.seg = *s; r.out = *o;
+    r.cursor = ctx->d_cursor;
+    const long long warps = (long long)ctx->n_sm * 2 * 8;
+    long long g = n_seg / (warps * 4);
+    r.segs_per_grab = (int)std::min<long long>(32, std::max<long long>(1, g));
+    if (emit_smem_bytes(a) > 200 * 1024) return fail(ctx, C8PH_E_ARG, "emit_propagate: atmosphere table too large for shared memory");
+    return C8PH_OK;
+}
+
+static int launch(c8ph_ctx *ctx, const KArgs &a, cudaStream_t st)
+{
+    CU(cudaMemsetAsync(ctx->d_cursor, 0, sizeof(unsigned long long), st));
+    CU(cudaEventRecord(ctx->ev0, st));
+    cudaError_t e = launch_emit_propagate(a, ctx->n_sm, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "emit_propagate launch");
+    CU(cudaEventRecord(ctx->ev1, st));
+    ctx->timed = true;
+    ctx->launches++;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64_t base,
+                                   const c8ph_params *p, uint64_t seed, const c8ph_outputs *o, void *stream)
+{
+    if (!ctx) return C8PH_E_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaSetDevice(ctx->device));
+    KArgs a{};
+    int rc = make_args(ctx, s, n_seg, base, p, seed, o, a, st);
+    if (rc) return rc;
+    if (n_seg == 0) return C8PH_OK;
+    return launch(ctx, a, st);
+}
+
+extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, int64_t n_seg, int64_t base,
+                                        const c8ph_params *p, uint64_t seed, const c8ph_outputs *ho)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!hs || hs->size != sizeof(c8ph_segments) || !ho || ho->size != sizeof(c8ph_outputs) || n_seg < 0)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate_host: NULL struct or size mismatch");
+    if (!ctx->have_det) return fail(ctx, C8PH_E_STATE, "emit_propagate_host: detector not set");
+    CU(cudaSetDevice(ctx->device));
+    cudaStream_t st = nullptr;
+    const float *src[11] = {hs->x, hs->y, hs->z, hs->dx, hs->dy, hs->dz, hs->len, hs->beta, hs->t0, hs->charge, hs->edep};
+    const size_t n = (size_t)n_seg, npad = (n + 63) & ~(size_t)63;
+    if (11 * npad > ctx->seg_cap) {
+        dfree(ctx->d_seg);
+        CU(cudaMalloc(&ctx->d_seg, std::max<size_t>(1, 11 * npad) * sizeof(float)));
+        ctx->seg_cap = 11 * npad;
+    }
+    const float *dp[11];
+    for (int k = 0; k < 11; ++k) {
+        dp[k] = src[k] ? ctx->d_seg + k * npad : nullptr;
+        if (src[k] && n) CU(cudaMemcpyAsync(ctx->d_seg + k * npad, src[k], n * sizeof(float), cudaMemcpyHostToDevice, st));
+    }
+    c8ph_segments ds{};
+    ds.size = sizeof(ds);
+    ds.x = dp[0]; ds.y = dp[1]; ds.z = dp[2]; ds.dx = dp[3]; ds.dy = dp[4]; ds.dz = dp[5];
+    ds.len = dp[6]; ds.beta = dp[7]; ds.t0 = dp[8]; ds.charge = dp[9]; ds.edep = dp[10];
+    // device outputs in one arena: counters | hist | tel_counts | photon_weight | photons
+    const DevDet &det = ctx->det;
+    const size_t n_hist = ho->hist ? (det.cam_enabled ? (size_t)det.cam_rows * det.cam_cols * det.n_tbins : (size_t)det.hist_nx * det.hist_ny) : 0;
+    const size_t n_tel = ho->tel_counts ? (size_t)det.n_tel : 0;
+    const size_t cap = ho->photons ? (size_t)std::max<int64_t>(0, ho->photon_capacity) : 0;
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t off_hist = up(C8PH_N_COUNTERS * sizeof(uint64_t));
+    const size_t off_tel = off_hist + up(n_hist * sizeof(float));
+    const size_t off_w = off_tel + up(n_tel * sizeof(float));
+    const size_t off_ph = off_w + up((ho->photon_weight ? cap : 0) * sizeof(float));
+    const size_t total = off_ph + up(cap * sizeof(c8ph_photon));
+    if (total > ctx->out_cap) {
+        if (ctx->d_out) cudaFree(ctx->d_out);
+        ctx->d_out = nullptr;
+        CU(cudaMalloc(&ctx->d_out, total));
+        ctx->out_cap = total;
+    }
+    char *b = (char *)ctx->d_out;
+    CU(cudaMemsetAsync(b, 0, off_w, st));                   // counters, hist, tel_counts
+    c8ph_outputs dout{};
+    dout.size = sizeof(dout);
+    dout.counters = (uint64_t *)b;
+    dout.hist = n_hist ? (float *)(b + off_hist) : nullptr;
+    dout.tel_counts = n_tel ? (float *)(b + off_tel) : nullptr;
+    dout.photon_weight = (ho->photon_weight && cap) ? (float *)(b + off_w) : nullptr;
+    dout.photons = cap ? (c8ph_photon *)(b + off_ph) : nullptr;
+    dout.photon_capacity = (int64_t)cap;
+    KArgs a{};
+    int rc = make_args(ctx, &ds, n_seg, base, p, seed, &dout, a, st);
+    if (rc) return rc;
+    if (n_seg > 0) { rc = launch(ctx, a, st); if (rc) return rc; }
+    uint64_t cnt[C8PH_N_COUNTERS];
+    CU(cudaMemcpyAsync(cnt, dout.counters, sizeof cnt, cudaMemcpyDeviceToHost, st));
+    if (n_hist) CU(cudaMemcpyAsync(ho->hist, dout.hist, n_hist * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (n_tel) CU(cudaMemcpyAsync(ho->tel_counts, dout.tel_counts, n_tel * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const size_t written = (size_t)std::min<uint64_t>(cnt[C8PH_CNT_WRITTEN], cap);
+    if (written) {
+        CU(cudaMemcpyAsync(ho->photons, dout.photons, written * sizeof(c8ph_photon), cudaMemcpyDeviceToHost, st));
+        if (dout.photon_weight) CU(cudaMemcpyAsync(ho->photon_weight, dout.photon_weight, written * sizeof(float), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    if (ho->counters) memcpy(ho->counters, cnt, sizeof cnt);
+    return C8PH_OK;
+}
+
+extern "C" float c8ph_last_kernel_ms(c8ph_ctx *ctx)
+{
+    if (!ctx || !ctx->timed) return -1.f;
+    if (cudaEventSynchronize(ctx->ev1) != cudaSuccess) return -1.f;
+    float ms = -1.f;
+    if (cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1) != cudaSuccess) return -1.f;
+    return ms;
+}
+
+extern "C" int64_t c8ph_launch_count(const c8ph_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" const char *c8ph_counter_name(int i)
+{
+    static const char *names[C8PH_N_COUNTERS] = {
+        "segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "emitted", "upgoing", "lv2", "table_range",
+        "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "written", "overflow", "clipped"};
+    return (i >= 0 && i < C8PH_N_COUNTERS) ? names[i] : "";
+}

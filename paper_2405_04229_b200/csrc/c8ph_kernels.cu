@@ -1,0 +1,926 @@
+// c8ph_kernels.cu — sm_100a kernels of libc8ph.
+//
+//  * k_emit_propagate: the fused hot path  segment -> yield -> photons -> straight line -> cuts ->
+//    refraction (none | layered Snell sum | interpolation-tracing table) -> transmission ->
+//    ground grid / telescope spheres / camera -> compacted photon list.   (thesis sec. 5.3)
+//  * k_build_table: the interpolation-tracing correction table (thesis sec. 4.4.1).
+//
+// Design (DESIGN.md has the long version):
+//  - persistent grid, one warp owns a group of segments taken from a global cursor; the 32 lanes
+//    first PREPARE up to 32 segments in parallel, one per lane, in fp64 (yield, bunch count, LV1,
+//    Rodrigues basis, axis-landing anchor), then the warp walks the emitting segments and the
+//    lanes stride over the photons of one segment (photon state lives in registers only; the
+//    thesis' shared-memory photon buffer, is not needed);
+//  - per-photon arithmetic is fp32 in cancellation-free "anchor + offset" form: the landing point
+//    of the particle axis and its clock are computed once per segment in fp64, the photon only
+//    adds small offsets, which keeps bin flips against the fp64 oracle below 1e-4;
+//  - Philox4x32-10 keyed on (seed; segment id, photon index): results are independent of grid
+//    size, segment order and batching;
+//  - n(h) (and for the layered sum the mid-layer n and overburden steps) are staged once per CTA
+//    in shared memory with one TMA bulk copy each (cp.async.bulk + mbarrier): lanes of a warp emit
+//    from the same short segment, so their n(h) reads fall in 1-3 adjacent words (broadcast);
+//  - the correction table (float4 texels dd, dt, X_slant, tau_aer) is read with 4 x LDG.128
+//    through L1: the lanes of a warp share (height, zenith) to within the Cherenkov angle, so they
+//    hit a handful of cache lines;
+//  - survivors are compacted by warp ballot into a per-warp shared-memory stage and flushed 32
+//    records (1 KiB) at a time with one cursor atomic per flush; the ground histogram takes one
+//    RED.ADD.F32 per landed photon into the L2-resident grid.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <cstdint>
+#include "c8ph_device.cuh"
+
+namespace c8ph {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kStage = 64;                       // photon records staged per warp
+constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
+constexpr double kC = 0.299792458;               // m / ns
+constexpr double kAlpha = 1.0 / 137.035999;
+constexpr float kUpCut = -1.0e-6f;               // drop photons with u_z >= kUpCut
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+// ---- TMA bulk copy global -> shared, completion on an mbarrier ---------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// ---- Philox4x32-10 (Salmon et al.; thesis ref. [66]), round keys precomputed ---------
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const uint32_t (&k0)[10], const uint32_t (&k1)[10])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0[r];
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1[r];
+        c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// (2m+1) 2^-24, m = top 23 bits: exact in fp32; built from the mantissa bits without an I2F
+__device__ __forceinline__ float u01(uint32_t r)
+{
+    return __uint_as_float(0x3F800000u | (r >> 9)) - 0.99999994f;
+}
+
+__device__ __forceinline__ double u01d(uint32_t r)
+{
+    return (static_cast<double>(r >> 9) + 0.5) * (1.0 / 8388608.0);
+}
+
+// ---- per-segment state (prepared by one lane in fp64, broadcast to the warp) --------------------
+struct Seg {
+    float Px, Py, Pz, e1x, e1y, e1z, e2x, e2y, e2z;   // direction and the two Rodrigues columns
+    float Ax, Ay, Az, L, beta, delta;                 // start point, length, beta, 1 - beta
+    float Gx, Gy;                                      // axis landing point (anchor) or unused
+    float fbx, fby;                                    // fractional grid coordinate of the anchor
+    int ibx, iby;                                      // integer grid coordinate of the anchor
+    float Tg;                                          // anchor clock - t_ref  (or t0 - t_ref)
+    float AzP;                                         // A_z / P_z (anchor form)
+    float hA, cA, k2;                                  // height of A, dh/ds, second-order term
+    float rx, ry, rz, inv_rA, a1, a2;                  // local vertical at A; e1.r, e2.r
+    // fluorescence
+    float aimx, aimy, aimz, omc;                       // aim point, 1 - cos(psi)
+    int N;                                             // bunches to emit
+    int anchor;                                        // 1: anchor form valid
+    uint32_t id_lo, id_hi, local;
+};
+
+__device__ __forceinline__ Seg shfl_seg(const Seg &s, int src)
+{
+    Seg o;
+    const unsigned m = 0xFFFFFFFFu;
+#define C8_SH(f) o.f = __shfl_sync(m, s.f, src)
+    C8_SH(Px); C8_SH(Py); C8_SH(Pz); C8_SH(e1x); C8_SH(e1y); C8_SH(e1z); C8_SH(e2x); C8_SH(e2y); C8_SH(e2z);
+    C8_SH(Ax); C8_SH(Ay); C8_SH(Az); C8_SH(L); C8_SH(beta); C8_SH(delta);
+    C8_SH(Gx); C8_SH(Gy); C8_SH(fbx); C8_SH(fby); C8_SH(ibx); C8_SH(iby); C8_SH(Tg); C8_SH(AzP);
+    C8_SH(hA); C8_SH(cA); C8_SH(k2); C8_SH(rx); C8_SH(ry); C8_SH(rz); C8_SH(inv_rA); C8_SH(a1); C8_SH(a2);
+    C8_SH(aimx); C8_SH(aimy); C8_SH(aimz); C8_SH(omc);
+    C8_SH(N); C8_SH(anchor); C8_SH(id_lo); C8_SH(id_hi); C8_SH(local);
+#undef C8_SH
+    return o;
+}
+
+// n-1 at height h from the global table in fp64 (Listing 4.1), clamped to the table
+__device__ __forceinline__ double eta_lookup_d(const DevAtm &atm, double h)
+{
+    double f = (h - (double)atm.h0) / (double)atm.dh;
+    f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
+    int k = min((int)f, atm.n_nodes - 2);
+    double fr = f - k;
+    return (1.0 - fr) * (double)__ldg(atm.eta + k) + fr * (double)__ldg(atm.eta + k + 1);
+}
+
+struct TabVal { float dd, dt, X, ta; bool bad; };
+
+__device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float thz)
+{
+    TabVal o;
+    o.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f);
+    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), (float)(t.n_h - 1));
+    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), (float)(t.n_zen - 1));
+    const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
+    const float ff = f - (float)ia, gg = g - (float)ib;
+    const float4 *p = t.hot + (size_t)ia * t.n_zen + ib;
+    const float4 v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + t.n_zen), v11 = __ldg(p + t.n_zen + 1);
+    const float w00 = (1.f - ff) * (1.f - gg), w01 = (1.f - ff) * gg, w10 = ff * (1.f - gg), w11 = ff * gg;
+    o.dd = w00 * v00.x + w01 * v01.x + w10 * v10.x + w11 * v11.x;
+    o.dt = w00 * v00.y + w01 * v01.y + w10 * v10.y + w11 * v11.y;
+    o.X = w00 * v00.z + w01 * v01.z + w10 * v10.z + w11 * v11.z;
+    o.ta = w00 * v00.w + w01 * v01.w + w10 * v10.w + w11 * v11.w;
+    o.bad = o.bad || (o.dd != o.dd);
+    return o;
+}
+
+// telescope candidates around (x,y): nearest entry along the arrival ray, lowest index on ties
+__device__ __forceinline__ int tel_hit_cell(const DevDet &det, const DevGrid &g, float x, float y,
+                                            float ux, float uy, float uz, bool brute)
+{
+    int best_k = -1;
+    float best_s = CUDART_INF_F;
+    int lo = 0, hi = det.n_tel;
+    const int *items = nullptr;
+    if (!brute) {
+        const int cx = (int)floorf((x - g.x0) * g.inv_cs), cy = (int)floorf((y - g.y0) * g.inv_cs);
+        if (cx < 0 || cy < 0 || cx >= g.nx || cy >= g.ny) return -1;
+        const int c = cy * g.nx + cx;
+        lo = __ldg(g.start + c);
+        hi = __ldg(g.start + c + 1);
+        items = g.items;
+    }
+    for (int i = lo; i < hi; ++i) {
+        const int k = items ? __ldg(items + i) : i;
+        const float4 t = __ldg(det.tel + k);
+        const float dx = t.x - x, dy = t.y - y, dz = t.z;
+        const float du = dx * ux + dy * uy + dz * uz;
+        const float m2 = dx * dx + dy * dy + dz * dz - du * du;
+        const float r2 = t.w * t.w;
+        if (m2 <= r2) {
+            const float s_in = du - sqrtf(r2 - m2);
+            if (s_in < best_s) { best_s = s_in; best_k = k; }
+        }
+    }
+    return best_k;
+}
+
+// LV2/LV3 proximity: is the straight-line point within r/|u_z| + margin of any telescope centre?
+__device__ __forceinline__ bool tel_near(const DevDet &det, float x, float y, float inv_abs_uz, float margin, bool brute)
+{
+    int lo = 0, hi = det.n_tel;
+    const int *items = nullptr;
+    if (!brute) {
+        const DevGrid &g = det.lv2;
+        const int cx = (int)floorf((x - g.x0) * g.inv_cs), cy = (int)floorf((y - g.y0) * g.inv_cs);
+        if (cx < 0 || cy < 0 || cx >= g.nx || cy >= g.ny) return false;
+        const int c = cy * g.nx + cx;
+        lo = __ldg(g.start + c);
+        hi = __ldg(g.start + c + 1);
+        items = g.items;
+    }
+    for (int i = lo; i < hi; ++i) {
+        const int k = items ? __ldg(items + i) : i;
+        const float4 t = __ldg(det.tel + k);
+        const float dx = x - t.x, dy = y - t.y;
+        const float reach = fmaf(t.w, inv_abs_uz, margin);
+        if (dx * dx + dy * dy <= reach * reach) return true;
+    }
+    return false;
+}
+
+// hexagonal camera pixel of an arrival direction (cfg3); -1 outside.  Nearest centre among the
+// rows/columns adjacent to the point (equivalent to the brute-force nearest centre).
+__device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float uy, float uz)
+{
+    const float vx = -ux, vy = -uy, vz = -uz;
+    const float vw = vx * det.cam_w[0] + vy * det.cam_w[1] + vz * det.cam_w[2];
+    if (!(vw > 0.f)) return -1;
+    const float a = atan2f(vx * det.cam_r[0] + vy * det.cam_r[1] + vz * det.cam_r[2], vw);
+    const float e = atan2f(vx * det.cam_u[0] + vy * det.cam_u[1] + vz * det.cam_u[2], vw);
+    const float p = det.cam_pitch, rp = p * 0.8660254037844386f;
+    const float fr = e / rp + 0.5f * (float)(det.cam_rows - 1);
+    const int r0 = (int)floorf(fr);
+    int best = -1;
+    float bd = CUDART_INF_F;
+#pragma unroll
+    for (int dr = 0; dr < 2; ++dr) {
+        const int r = r0 + dr;
+        if (r < 0 || r >= det.cam_rows) continue;
+        const float ce = ((float)r - 0.5f * (float)(det.cam_rows - 1)) * rp;
+        const float fc = a * det.cam_inv_pitch + 0.5f * (float)(det.cam_cols - 1) - 0.5f * (float)(r & 1);
+        const int c0 = (int)floorf(fc);
+#pragma unroll
+        for (int dc = 0; dc < 2; ++dc) {
+            const int c = c0 + dc;
+            if (c < 0 || c >= det.cam_cols) continue;
+            const float ca = ((float)c - 0.5f * (float)(det.cam_cols - 1) + 0.5f * (float)(r & 1)) * p;
+            const float d2 = (a - ca) * (a - ca) + (e - ce) * (e - ce);
+            const int idx = r * det.cam_cols + c;
+            if (d2 < bd || (d2 == bd && idx < best)) { bd = d2; best = idx; }
+        }
+    }
+    if (bd > p * p * (1.0f / 3.0f)) return -1;
+    return best;
+}
+
+struct Counters {
+    uint32_t up, lv2, tr, roul, grid, tel, cam;
+};
+
+// ================================================================================================
+template <int EMIT, int TRACE, bool SPH>
+__global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_constant__ KArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t s_bar;
+
+    const DevAtm &atm = a.atm;
+    const DevDet &det = a.det;
+    const DevRun &run = a.run;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned FULL = 0xFFFFFFFFu;
+    unsigned long long *cntp = reinterpret_cast<unsigned long long *>(run.out.counters);
+
+    // ---- shared memory carve-up: n(h) tables, then the per-warp photon stage
+    float *s_eta = reinterpret_cast<float *>(smem_raw);
+    float *s_mid = s_eta + atm.n_pad;
+    float *s_dxv = s_mid + (TRACE == C8PH_TRACE_NUMERIC ? atm.n_pad : 0);
+    float *s_end = s_dxv + (TRACE == C8PH_TRACE_NUMERIC ? atm.n_pad : 0);
+    c8ph_photon *s_rec = reinterpret_cast<c8ph_photon *>(s_end) + warp * kStage;
+    float *s_wgt = reinterpret_cast<float *>(reinterpret_cast<c8ph_photon *>(s_end) + kWarps * kStage) + warp * kStage;
+
+    // ---- stage the atmosphere tables: one TMA bulk copy per array, completion on an mbarrier
+    if (threadIdx.x == 0) {
+        mbar_init(&s_bar, 1);
+        const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
+        mbar_expect_tx(&s_bar, bytes * (TRACE == C8PH_TRACE_NUMERIC ? 3u : 1u));
+        bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
+        if (TRACE == C8PH_TRACE_NUMERIC) {
+            bulk_g2s(s_mid, atm.eta_mid, bytes, &s_bar);
+            bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
+        }
+    }
+    __syncthreads();
+    mbar_wait(&s_bar, 0);
+
+    Counters cnt = {0, 0, 0, 0, 0, 0, 0};
+    uint32_t c_below = 0, c_lv1 = 0, c_emitting = 0, c_clipped = 0, c_written = 0, c_overflow = 0;
+    unsigned long long c_emitted = 0;
+    int stage_fill = 0;                                   // records waiting in this warp's stage (warp-uniform)
+
+    const bool has_hist = det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr;
+    const bool has_grid_geom = det.hist_nx > 0 && !det.cam_enabled;
+    const float hx1 = det.hist_x0 + det.hist_nx * det.hist_cell, hy1 = det.hist_y0 + det.hist_ny * det.hist_cell;
+    const float inv_ng = 1.0f / (1.0f + atm.eta_g);
+
+    // flush `n` staged records (n <= 32) starting at stage slot `first`
+    auto flush = [&](int first, int n) {
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(&cntp[C8PH_CNT_WRITTEN], (unsigned long long)n);
+        base = __shfl_sync(FULL, base, 0);
+        const long long room = run.out.photon_capacity - (long long)base;
+        const int fit = room >= n ? n : (room > 0 ? (int)room : 0);
+        __syncwarp();
+        if (lane < fit) {
+            const int slot = (first + lane) & (kStage - 1);
+            const uint4 *src = reinterpret_cast<const uint4 *>(s_rec + slot);
+            uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + base + lane);
+            dst[0] = src[0];
+            dst[1] = src[1];
+            if (run.out.photon_weight) run.out.photon_weight[base + lane] = s_wgt[slot];
+        }
+        __syncwarp();
+        if (lane == 0) { c_written += fit; c_overflow += n - fit; }
+    };
+    int stage_head = 0;
+
+    for (;;) {
+        // ---- grab a group of segments for this warp
+        unsigned long long g0 = 0;
+        if (lane == 0) g0 = atomicAdd(run.cursor, (unsigned long long)run.segs_per_grab);
+        g0 = __shfl_sync(FULL, g0, 0);
+        if ((long long)g0 >= run.n_seg) break;
+
+        // ---- a1-a4: one lane prepares one segment (fp64)
+        Seg me;
+        me.N = 0;
+        {
+            const long long i = (long long)g0 + lane;
+            if (lane < run.segs_per_grab && i < run.n_seg) {
+                const double Ax = run.seg.x[i], Ay = run.seg.y[i], Az = run.seg.z[i];
+                double Px = run.seg.dx[i], Py = run.seg.dy[i], Pz = run.seg.dz[i];
+                const double L = run.seg.len[i], beta = run.seg.beta[i], t0 = run.seg.t0[i];
+                const double pn = 1.0 / sqrt(Px * Px + Py * Py + Pz * Pz);
+                Px *= pn; Py *= pn; Pz *= pn;
+                const unsigned long long gid = (unsigned long long)(run.seg_id_base + i);
+                me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); me.local = (uint32_t)i;
+                // local vertical and height at A and at the midpoint
+                double rx = 0.0, ry = 0.0, rz = 1.0, rA = 1.0, hA, h_mid;
+                const double mx = Ax + 0.5 * L * Px, my = Ay + 0.5 * L * Py, mz = Az + 0.5 * L * Pz;
+                if (SPH) {
+                    const double zz = Az + atm.Rg;
+                    rA = sqrt(Ax * Ax + Ay * Ay + zz * zz);
+                    rx = Ax / rA; ry = Ay / rA; rz = zz / rA;
+                    hA = rA - atm.R;
+                    const double zm = mz + atm.Rg;
+                    h_mid = sqrt(mx * mx + my * my + zm * zm) - atm.R;
+                } else {
+                    hA = atm.h_obs + Az;
+                    h_mid = atm.h_obs + mz;
+                }
+                const double cA = Px * rx + Py * ry + Pz * rz;
+                double n_exp = 0.0;
+                bool lv1_drop = false;
+                const uint4 rs = philox4x32_10(0xFFFFFFFFu, me.id_lo, me.id_hi, 0u, run.key0, run.key1);
+                if (EMIT == C8PH_EMIT_CHERENKOV) {
+                    // Frank-Tamm, Eq. 2.2-2.4, n at the segment mid height
+                    const double n_mid = 1.0 + eta_lookup_d(atm, h_mid);
+                    const double bn = beta * n_mid;
+                    const double sin2 = 1.0 - 1.0 / (bn * bn);
+                    const double zq = run.seg.charge[i];
+                    if (sin2 > 0.0) n_exp = run.yield_k * zq * zq * L * sin2;
+                    if (n_exp > 0.0 && run.lv1) {
+                        // LV1, Eq. 4.3: angle between P and the direction to the array centre
+                        const double dist = sqrt(mx * mx + my * my + mz * mz);
+                        double cosa = -(Px * mx + Py * my + Pz * mz) / dist;
+                        cosa = fmin(1.0, fmax(-1.0, cosa));
+                        const double theta_c = acos(fmin(1.0, 1.0 / bn));
+                        const double ratio = fmin(1.0, det.r_array / dist);
+                        lv1_drop = acos(cosa) > theta_c + asin(ratio) + run.lv1_margin;
+                    }
+                    // Rodrigues half-turn about the bisector of D = (0,0,-1) and P
+                    const double Bx = Px, By = Py, Bz = Pz - 1.0;
+                    const double b2 = Bx * Bx + By * By + Bz * Bz;
+                    if (Pz > 1.0 - 1e-6 || b2 <= 0.0) {
+                        me.e1x = 1.f; me.e1y = 0.f; me.e1z = 0.f; me.e2x = 0.f; me.e2y = -1.f; me.e2z = 0.f;
+                    } else {
+                        const double k = 2.0 / b2;
+                        me.e1x = (float)(k * Bx * Bx - 1.0); me.e1y = (float)(k * Bx * By); me.e1z = (float)(k * Bx * Bz);
+                        me.e2x = (float)(k * By * Bx); me.e2y = (float)(k * By * By - 1.0); me.e2z = (float)(k * By * Bz);
+                    }
+                    me.aimx = me.aimy = me.aimz = me.omc = 0.f;
+                } else {
+                    // fluorescence: N = Y E_dep Omega/4pi, forced cone towards the pre-corrected aim point
+                    const float4 t0v = __ldg(det.tel);
+                    const double dx = t0v.x - mx, dy = t0v.y - my, dz = t0v.z - mz;
+                    const double dist = sqrt(dx * dx + dy * dy + dz * dz);
+                    double aimx = t0v.x, aimy = t0v.y;
+                    if (TRACE == C8PH_TRACE_TABLE) {
+                        const double ux = dx / dist, uy = dy / dist, uz = dz / dist;
+                        double vx = 0, vy = 0, vz = 1;
+                        if (SPH) {
+                            const double zm = mz + atm.Rg, rm = sqrt(mx * mx + my * my + zm * zm);
+                            vx = mx / rm; vy = my / rm; vz = zm / rm;
+                        }
+                        const double cz = -(ux * vx + uy * vy + uz * vz);
+                        const double hn = sqrt(ux * ux + uy * uy);
+                        if (cz > 0.0 && hn > 1e-9) {
+                            // same bilinear rule as the per-photon lookup, in fp64 on the stored fp32 nodes
+                            const DevTable &t = a.tab;
+                            const double thz = acos(fmin(1.0, cz));
+                            if (h_mid >= 0.0 && h_mid <= (double)t.h_max && thz <= (double)t.zen_max) {
+                                const double f = h_mid / ((double)t.h_max / (t.n_h - 1)), g = thz / ((double)t.zen_max / (t.n_zen - 1));
+                                const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
+                                const double ff = f - ia, gg = g - ib;
+                                const float4 *p = t.hot + (size_t)ia * t.n_zen + ib;
+                                const double v = (1 - ff) * ((1 - gg) * (double)__ldg(p).x + gg * (double)__ldg(p + 1).x)
+                                               + ff * ((1 - gg) * (double)__ldg(p + t.n_zen).x + gg * (double)__ldg(p + t.n_zen + 1).x);
+                                if (v == v) { aimx -= v * ux / hn; aimy -= v * uy / hn; }
+                            }
+                        }
+                    }
+                    me.aimx = (float)aimx; me.aimy = (float)aimy; me.aimz = t0v.z;
+                    const double rho = run.aim_factor * (double)t0v.w;
+                    const double sp = fmin(1.0, rho / dist);
+                    const double cps = sqrt(1.0 - sp * sp);
+                    const double omc = sp * sp / (1.0 + cps);                 // 1 - cos(psi), cancellation-free
+                    me.omc = (float)omc;
+                    const float *ed = run.seg.edep;
+                    n_exp = run.fluor_yield * (ed ? (double)ed[i] : 0.0) * 0.5 * omc;
+                    me.e1x = me.e1y = me.e1z = me.e2x = me.e2y = me.e2z = 0.f;
+                }
+                long long N = 0;
+                if (!(n_exp > 0.0)) c_below++;
+                else if (lv1_drop) c_lv1++;
+                else {
+                    N = (long long)floor(n_exp / (double)run.w + u01d(rs.x));
+                    if (N >= C8PH_MAX_BUNCHES_PER_SEGMENT) { c_clipped += 1; N = C8PH_MAX_BUNCHES_PER_SEGMENT - 1; }
+                    if (N > 0) c_emitting++;
+                }
+                me.N = (int)N;
+                me.Px = (float)Px; me.Py = (float)Py; me.Pz = (float)Pz;
+                me.Ax = (float)Ax; me.Ay = (float)Ay; me.Az = (float)Az;
+                me.L = (float)L; me.beta = (float)beta; me.delta = 1.0f - (float)beta;
+                me.hA = (float)hA; me.cA = (float)cA; me.k2 = SPH ? (float)((1.0 - cA * cA) / (2.0 * rA)) : 0.f;
+                me.rx = (float)rx; me.ry = (float)ry; me.rz = (float)rz; me.inv_rA = SPH ? (float)(1.0 / rA) : 0.f;
+                me.a1 = me.e1x * me.rx + me.e1y * me.ry + me.e1z * me.rz;
+                me.a2 = me.e2x * me.rx + me.e2y * me.ry + me.e2z * me.rz;
+                // axis landing anchor (fp64): G = A - A_z P / P_z, its clock, its grid coordinate
+                me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
+                me.Gx = me.Gy = me.fbx = me.fby = me.AzP = 0.f; me.ibx = me.iby = 0;
+                if (me.anchor) {
+                    const double azp = Az / Pz;
+                    const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
+                    me.Gx = (float)Gx; me.Gy = (float)Gy; me.AzP = (float)azp;
+                    me.Tg = (float)(t0 - azp / kC - det.t_ref);
+                    if (has_grid_geom) {
+                        const double bx = (Gx - (double)det.hist_x0) / (double)det.hist_cell;
+                        const double by = (Gy - (double)det.hist_y0) / (double)det.hist_cell;
+                        const double fx = fmin(fmax(floor(bx), -1.0e9), 1.0e9), fy = fmin(fmax(floor(by), -1.0e9), 1.0e9);
+                        me.ibx = (int)fx; me.iby = (int)fy;
+                        me.fbx = (float)(bx - fx); me.fby = (float)(by - fy);
+                    }
+                } else {
+                    me.Tg = (float)(t0 - det.t_ref);
+                }
+            }
+        }
+        unsigned emask = __ballot_sync(FULL, me.N > 0);
+
+        // ---- a5-a16: the warp walks the emitting segments; lanes stride over the photons
+        while (emask) {
+            const int src = __ffs(emask) - 1;
+            emask &= emask - 1;
+            const Seg sg = shfl_seg(me, src);
+            if (lane == 0) c_emitted += (unsigned long long)sg.N;
+            const int n_iter = (sg.N + 31) >> 5;
+            for (int it = 0; it < n_iter; ++it) {
+                const int j = it * 32 + lane;
+                bool alive = j < sg.N;
+                bool write = false;
+                c8ph_photon rec;
+                float rec_w = 0.f;
+                if (alive) {
+                    const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, run.key0, run.key1);
+                    const float u0 = u01(rn.x), u1 = u01(rn.y), u2 = u01(rn.z), u3 = u01(rn.w);
+                    // a6: emission point on the track, its height and n(h_e) (Listing 4.1)
+                    const float s = u1 * sg.L;
+                    const float h_e = fmaf(s, fmaf(s, sg.k2, sg.cA), sg.hA);
+                    float eta_e;
+                    {
+                        float f = (h_e - atm.h0) * atm.inv_dh;
+                        f = fminf(fmaxf(f, 0.f), (float)(atm.n_nodes - 1));
+                        const int k = min((int)f, atm.n_nodes - 2);
+                        const float e0 = s_eta[k], e1 = s_eta[k + 1];
+                        eta_e = fmaf(f - (float)k, e1 - e0, e0);
+                    }
+                    float ux, uy, uz, lam_inv, cth = 1.f, q = 0.f, pqz = 0.f, wx = 0.f, wy = 0.f, wz = 0.f;
+                    float sphi, cphi;
+                    sincospif(2.0f * u0, &sphi, &cphi);
+                    if (EMIT == C8PH_EMIT_CHERENKOV) {
+                        // a6/a7: cos(theta_c) = 1/(beta n(h_e)) (Eq. 2.5), beta n - 1 without cancellation
+                        const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
+                        q = sqrtf(bn1 * (2.f + bn1));                   // tan(theta_c)
+                        cth = __frcp_rn(1.f + bn1);                     // cos(theta_c)
+                        wx = cphi * sg.e1x + sphi * sg.e2x;
+                        wy = cphi * sg.e1y + sphi * sg.e2y;
+                        wz = cphi * sg.e1z + sphi * sg.e2z;
+                        pqz = fmaf(q, wz, sg.Pz);
+                        ux = cth * fmaf(q, wx, sg.Px);
+                        uy = cth * fmaf(q, wy, sg.Py);
+                        uz = cth * pqz;
+                        lam_inv = fmaf(-u2, run.il1 - run.il2, run.il1);  // 1/lambda uniform
+                    } else {
+                        // fluorescence: uniform in the cone about (aim - A_e)
+                        int li = 0;
+                        while (li < run.n_lines - 1 && u2 >= __ldg(run.line_cdf + li)) ++li;
+                        lam_inv = 1.0f / __ldg(run.line_nm + li);
+                        const uint4 rb = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 1u, run.key0, run.key1);
+                        const float xe = fmaf(s, sg.Px, sg.Ax), ye = fmaf(s, sg.Py, sg.Ay), ze = fmaf(s, sg.Pz, sg.Az);
+                        float ax = sg.aimx - xe, ay = sg.aimy - ye, az = sg.aimz - ze;
+                        const float an = rsqrtf(ax * ax + ay * ay + az * az);
+                        ax *= an; ay *= an; az *= an;
+                        const float tt = u01(rb.x) * sg.omc;             // 1 - cos(polar)
+                        const float cp = 1.f - tt, sp = sqrtf(tt * (2.f - tt));
+                        float e1x = ay, e1y = -ax;
+                        float e1n = e1x * e1x + e1y * e1y;
+                        if (e1n < 1e-24f) { e1x = 1.f; e1y = 0.f; e1n = 1.f; }
+                        const float ie = rsqrtf(e1n);
+                        e1x *= ie; e1y *= ie;
+                        const float e2x = -az * e1y, e2y = az * e1x, e2z = ax * e1y - ay * e1x;
+                        ux = cp * ax + sp * (cphi * e1x + sphi * e2x);
+                        uy = cp * ay + sp * (cphi * e1y + sphi * e2y);
+                        uz = cp * az + sp * (sphi * e2z);
+                    }
+                    // a8: up-going / horizontal photons are discarded
+                    if (uz >= kUpCut) { alive = false; cnt.up++; }
+                    float xl = 0.f, yl = 0.f, ox = 0.f, oy = 0.f, D = 0.f, inv_uz = 0.f, tx_l = 0.f, ty_l = 0.f;
+                    if (alive) {
+                        // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
+                        inv_uz = __frcp_rn(uz);
+                        const float Z = fmaf(s, sg.Pz, sg.Az);
+                        D = -Z * inv_uz;
+                        if (sg.anchor) {
+                            const float zq = -Z * q * __frcp_rn(sg.Pz * pqz);
+                            ox = zq * (wx * sg.Pz - sg.Px * wz);
+                            oy = zq * (wy * sg.Pz - sg.Py * wz);
+                            xl = sg.Gx + ox;
+                            yl = sg.Gy + oy;
+                        } else {
+                            xl = fmaf(D, ux, fmaf(s, sg.Px, sg.Ax));
+                            yl = fmaf(D, uy, fmaf(s, sg.Py, sg.Ay));
+                        }
+                        // a10: LV2/LV3 on the straight-line point, before the correction
+                        if (run.lv2) {
+                            const float m = run.lv2_margin;
+                            bool keep = has_grid_geom && xl >= det.hist_x0 - m && xl < hx1 + m && yl >= det.hist_y0 - m && yl < hy1 + m;
+                            if (!keep && det.n_tel > 0)
+                                keep = tel_near(det, xl, yl, -inv_uz, m, !det.use_grid || -uz < det.grid_min_cos);
+                            if (!keep) { alive = false; cnt.lv2++; }
+                        }
+                    }
+                    float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz = 1.f, sinz = 0.f, delta_arr = 0.f;
+                    if (alive) {
+                        // local zenith angle of the photon at the emission point
+                        if (SPH) {
+                            float ur;
+                            if (EMIT == C8PH_EMIT_CHERENKOV) ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
+                            else ur = ux * sg.rx + uy * sg.ry + uz * sg.rz;
+                            const float sr = s * sg.inv_rA;
+                            const float uP = (EMIT == C8PH_EMIT_CHERENKOV) ? cth : (ux * sg.Px + uy * sg.Py + uz * sg.Pz);
+                            cz = -(fmaf(-sr * sg.cA, ur, ur) + sr * uP);
+                        } else {
+                            cz = -uz;
+                        }
+                        cz = fminf(cz, 1.f);
+                        sinz = sqrtf(fmaxf(1.f - cz * cz, 0.f));
+                        // a11: refraction
+                        if (TRACE == C8PH_TRACE_STRAIGHT) {
+                            dt = eta_e * D * kInvC;                      // homogeneous: t = t_e + n D / c
+                        } else if (TRACE == C8PH_TRACE_TABLE) {
+                            const TabVal v = table_lookup(a.tab, h_e, acosf(cz));
+                            if (v.bad || !(cz > 0.f)) { alive = false; cnt.tr++; }
+                            dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
+                        } else {
+                            // layered Snell sum (Eq. 3.15 in its invariant form K = n sin(theta)),
+                            // accumulated as the difference to the straight line
+                            const float n_e = 1.f + eta_e;
+                            const float K = n_e * sinz;
+                            const float r_e = __frcp_rn(n_e * cz);
+                            const float fe = fminf(fmaxf((h_e - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
+                            const float fg = fminf(fmaxf(((float)atm.h_obs - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
+                            const int ke = min((int)fe, atm.n_nodes - 2), kg = min((int)fg, atm.n_nodes - 2);
+                            const float fre = fe - (float)ke, frg = fg - (float)kg;
+                            float aX = 0.f, aT = 0.f, aS = 0.f;
+                            bool ok = cz > 0.f;
+                            auto layer = [&](float eta_l, float thick, float dxv_l) {
+                                const float n_l = 1.f + eta_l;
+                                const float ql = fmaf(n_l, n_l, -K * K);
+                                ok = ok && (ql > 0.f);
+                                const float r_l = rsqrtf(ql);
+                                const float dq = (eta_e - eta_l) * (2.f + eta_e + eta_l);       // q_e - q_l
+                                const float dr = dq * r_l * r_l * r_e * r_e * __frcp_rn(r_l + r_e); // r_l - r_e
+                                aX = fmaf(thick * K, dr, aX);
+                                aT = fmaf(thick, fmaf(n_l * n_l, dr, r_e * (fmaf(eta_l, eta_l, 2.f * eta_l) - eta_e)), aT);
+                                aS = fmaf(dxv_l * n_l, r_l, aS);
+                            };
+                            if (ke == kg) {
+                                const float fm = 0.5f * (fre + frg);
+                                layer(fmaf(fm, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), (fre - frg) * atm.dh, (fre - frg) * s_dxv[ke]);
+                            } else {
+                                if (fre > 0.f)
+                                    layer(fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke]);
+                                for (int k = ke - 1; k > kg; --k) layer(s_mid[k], atm.dh, s_dxv[k]);
+                                layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
+                            }
+                            if (!ok) { alive = false; cnt.tr++; }
+                            dd = aX; dt = aT * kInvC; Xs = aS;
+                        }
+                    }
+                    float T = 1.f, wgt = run.w;
+                    if (alive && run.trans != C8PH_TRANS_OFF) {
+                        // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
+                        float tau = 0.f;
+                        if (atm.ray_inv_X > 0.f) {
+                            float qq = atm.ray_lambda * lam_inv;
+                            qq *= qq; qq *= qq;
+                            tau = Xs * qq * atm.ray_inv_X;
+                        }
+                        if (atm.aer_L > 0.f) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
+                        T = __expf(-tau);
+                        if (run.trans == C8PH_TRANS_ROULETTE) {
+                            if (!(u3 < T)) { alive = false; cnt.roul++; }
+                        } else wgt = run.w * T;
+                    }
+                    if (alive) {
+                        // landed: corrected position (dd along the horizontal direction of flight)
+                        const float hn2 = ux * ux + uy * uy;
+                        float ehx = 0.f, ehy = 0.f;
+                        if (hn2 >= 1e-18f) { const float ih = rsqrtf(hn2); ehx = ux * ih; ehy = uy * ih; }
+                        const float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);     // offset from the anchor
+                        float xg, yg;
+                        if (sg.anchor) { xg = sg.Gx + cx; yg = sg.Gy + cy; }
+                        else { xg = fmaf(dd, ehx, xl); yg = fmaf(dd, ehy, yl); }
+                        // a13: arrival time relative to t_ref
+                        float t_arr;
+                        if (sg.anchor) {
+                            // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
+                            const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
+                            const float num = fmaf(q, wz, -bn1 * sg.Pz);
+                            const float geo = (s + sg.AzP) * num * __frcp_rn(pqz);
+                            t_arr = sg.Tg + fmaf(fmaf(s, sg.delta / sg.beta, geo), kInvC, dt);
+                        } else {
+                            t_arr = sg.Tg + fmaf(s / sg.beta + D, kInvC, dt);
+                        }
+                        // a15: ground grid
+                        int bin = -1;
+                        if (has_grid_geom) {
+                            int ix, iy;
+                            if (sg.anchor) {
+                                ix = sg.ibx + (int)floorf(fmaf(cx, det.hist_inv_cell, sg.fbx));
+                                iy = sg.iby + (int)floorf(fmaf(cy, det.hist_inv_cell, sg.fby));
+                            } else {
+                                ix = (int)floorf((xg - det.hist_x0) * det.hist_inv_cell);
+                                iy = (int)floorf((yg - det.hist_y0) * det.hist_inv_cell);
+                            }
+                            if (ix >= 0 && ix < det.hist_nx && iy >= 0 && iy < det.hist_ny) {
+                                bin = iy * det.hist_nx + ix;
+                                cnt.grid++;
+                                if (has_hist) atomicAdd(run.out.hist + bin, wgt);
+                            }
+                        }
+                        // arrival direction: rotation by delta in the ray plane (Snell / Bouguer invariant)
+                        float uax = ux, uay = uy, uaz = uz;
+                        auto arrival_direction = [&]() {
+                            if (TRACE == C8PH_TRACE_STRAIGHT || sinz < 1e-6f) return;
+                            const float eps = (eta_e - atm.eta_g) * inv_ng;
+                            const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * (float)(1.0 / atm.Rg) : 1.f;
+                            const float al = sinz * scale;
+                            const float cyy = sqrtf(fmaxf(1.f - al * al, 0.f));
+                            const float at = al * (1.f + eps);
+                            const float cxx = sqrtf(fmaxf(1.f - at * at, 0.f));
+                            float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * __frcp_rn(cyy + cxx));
+                            if (SPH) dl -= dd * (float)(1.0 / atm.Rg);
+                            delta_arr = dl;
+                            const float k1 = 1.f - 0.5f * dl * dl + dl * cz / sinz, k2 = dl / sinz;
+                            uax = fmaf(k1, ux, k2 * sg.rx);
+                            uay = fmaf(k1, uy, k2 * sg.ry);
+                            uaz = fmaf(k1, uz, k2 * sg.rz);
+                        };
+                        // a14: telescope spheres, only if a candidate list is non-empty
+                        int tel = -1;
+                        bool dir_done = false;
+                        if (det.n_tel > 0) {
+                            arrival_direction();
+                            dir_done = true;
+                            const bool brute = !det.use_grid || -uaz < det.grid_min_cos;
+                            tel = tel_hit_cell(det, det.hit, xg, yg, uax, uay, uaz, brute);
+                            if (tel >= 0) {
+                                cnt.tel++;
+                                if (run.out.tel_counts) atomicAdd(run.out.tel_counts + tel, wgt);
+                                if (det.cam_enabled) {
+                                    const int pix = camera_pixel(det, uax, uay, uaz);
+                                    const float tb = floorf(t_arr * det.inv_t_bin);
+                                    if (pix >= 0 && tb >= 0.f && tb < (float)det.n_tbins) {
+                                        cnt.cam++;
+                                        if (run.out.hist) atomicAdd(run.out.hist + (size_t)pix * det.n_tbins + (int)tb, wgt);
+                                    }
+                                }
+                            }
+                        }
+                        write = run.write == C8PH_WRITE_ALL || (run.write == C8PH_WRITE_TEL && tel >= 0);
+                        if (write) {
+                            if (!dir_done) arrival_direction();
+                            rec.x = xg; rec.y = yg; rec.ux = uax; rec.uy = uay;
+                            rec.t_ns = t_arr;
+                            rec.lambda_nm = __frcp_rn(lam_inv);
+                            rec.seg = sg.local;
+                            rec.j_tel = ((uint32_t)j << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE);
+                            rec_w = wgt;
+                        }
+                        (void)delta_arr; (void)tx_l; (void)ty_l; (void)T;
+                    }
+                }
+                // a16: warp-ballot compaction into the per-warp stage, flushed 32 records at a time
+                if (run.out.photons) {
+                    const unsigned wm = __ballot_sync(FULL, write);
+                    if (wm) {
+                        if (write) {
+                            const int slot = (stage_head + stage_fill + __popc(wm & ((1u << lane) - 1u))) & (kStage - 1);
+                            s_rec[slot] = rec;
+                            s_wgt[slot] = rec_w;
+                        }
+                        stage_fill += __popc(wm);
+                        __syncwarp();
+                        if (stage_fill >= 32) {
+                            flush(stage_head, 32);
+                            stage_head = (stage_head + 32) & (kStage - 1);
+                            stage_fill -= 32;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (run.out.photons && stage_fill > 0) flush(stage_head, stage_fill);
+
+    // ---- counters: warp reduction, one atomic per warp and counter
+    auto add = [&](int idx, uint32_t v) {
+        v = __reduce_add_sync(FULL, v);
+        if (lane == 0 && v) atomicAdd(&cntp[idx], (unsigned long long)v);
+    };
+    if (run.out.counters) {
+        if (blockIdx.x == 0 && threadIdx.x == 0)
+            atomicAdd(&cntp[C8PH_CNT_SEGMENTS], (unsigned long long)run.n_seg);
+        add(C8PH_CNT_SEG_BELOW_THRESHOLD, c_below);
+        add(C8PH_CNT_SEG_LV1, c_lv1);
+        add(C8PH_CNT_SEG_EMITTING, c_emitting);
+        add(C8PH_CNT_CLIPPED, c_clipped);
+        add(C8PH_CNT_UPGOING, cnt.up);
+        add(C8PH_CNT_LV2, cnt.lv2);
+        add(C8PH_CNT_TABLE_RANGE, cnt.tr);
+        add(C8PH_CNT_ROULETTE, cnt.roul);
+        add(C8PH_CNT_IN_GRID, cnt.grid);
+        add(C8PH_CNT_TEL_HIT, cnt.tel);
+        add(C8PH_CNT_CAM_HIT, cnt.cam);
+        add(C8PH_CNT_OVERFLOW, c_overflow);
+        const uint32_t drops = __reduce_add_sync(FULL, cnt.up + cnt.lv2 + cnt.tr + cnt.roul);
+        if (lane == 0) {
+            if (c_emitted) atomicAdd(&cntp[C8PH_CNT_EMITTED], c_emitted);
+            // landed = emitted - drops, accumulated as two's-complement u64 pieces
+            atomicAdd(&cntp[C8PH_CNT_LANDED], c_emitted - (unsigned long long)drops);
+        }
+    }
+    (void)c_written;
+}
+
+// ================================================================================================
+// Correction table: one thread per node, exact layered ray in fp64 by the Snell (planar) or
+// Bouguer (spherical) invariant, layer by layer on the n(h) grid (layers = table cells split in
+// `substeps`, n at the layer mid height), minus the straight line to the same sphere / plane.
+__global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ TableBuildArgs a)
+{
+    const int node = blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= a.n_h * a.n_zen) return;
+    const int ia = node / a.n_zen, ib = node % a.n_zen;
+    const DevAtm &atm = a.atm;
+    const double h_e = ia * a.h_max / (a.n_h - 1);
+    const double th = ib * a.zen_max / (a.n_zen - 1);
+    float out[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+    const bool sph = atm.model == C8PH_ATM_SPHERICAL;
+    const double h_g = atm.h_obs;
+    if (h_e > h_g) {
+        const double sz = sin(th), cz = cos(th);
+        const double n_e = 1.0 + eta_lookup_d(atm, h_e);
+        const double K = sph ? n_e * (atm.R + h_e) * sz : n_e * sz;     // Bouguer / Snell invariant
+        const double step = atm.model == C8PH_ATM_HOMOGENEOUS ? 1.0e30 : (double)atm.dh / a.substeps;
+        double h_cur = h_e, psi = 0.0, S = 0.0, cT = 0.0, X = 0.0, tau = 0.0;
+        bool ground = true;
+        auto xv_at = [&](double h) {
+            double f = (h - (double)atm.h0) / (double)atm.dh;
+            f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
+            const int k = min((int)f, atm.n_nodes - 2);
+            const double fr = f - k;
+            return (1.0 - fr) * (double)__ldg(atm.xv + k) + fr * (double)__ldg(atm.xv + k + 1);
+        };
+        double xv_cur = xv_at(h_cur);
+        double ea_cur = atm.aer_L > 0.f ? exp(-h_cur / (double)atm.aer_H) : 0.0;
+        while (h_cur > h_g) {
+            double h_next;
+            if (atm.model == C8PH_ATM_HOMOGENEOUS) h_next = h_g;
+            else {
+                const double g = floor((h_cur - (double)atm.h0) / step);
+                h_next = (double)atm.h0 + g * step;
+                if (!(h_next < h_cur - 1e-9 * step)) h_next = (double)atm.h0 + (g - 1.0) * step;
+                if (h_next < h_g) h_next = h_g;
+            }
+            const double n_l = 1.0 + eta_lookup_d(atm, 0.5 * (h_cur + h_next));
+            const double dhl = h_cur - h_next;
+            double s;
+            if (sph) {
+                const double p = K / n_l;                                // impact parameter of the chord
+                const double rt = atm.R + h_cur, rb = atm.R + h_next;
+                if (!(rb > p)) { ground = false; break; }
+                const double at = sqrt(rt * rt - p * p), ab = sqrt(rb * rb - p * p);
+                s = dhl * (rt + rb) / (at + ab);                         // at - ab, cancellation-free
+                const double x = p * s / (rt * rb);                      // sin of the central-angle step
+                psi += x * (1.0 + x * x * (1.0 / 6.0 + x * x * (3.0 / 40.0)));
+            } else {
+                const double q2 = n_l * n_l - K * K;
+                if (!(q2 > 0.0)) { ground = false; break; }
+                const double iq = 1.0 / sqrt(q2);
+                s = dhl * n_l * iq;
+                psi += dhl * K * iq;                                     // horizontal displacement
+            }
+            S += s;
+            cT += n_l * s;
+            const double xv_next = xv_at(h_next);
+            X += (xv_next - xv_cur) * (s / dhl);
+            xv_cur = xv_next;
+            if (atm.aer_L > 0.f) {
+                const double ea_next = exp(-h_next / (double)atm.aer_H);
+                tau += ((double)atm.aer_H / (double)atm.aer_L) * (ea_next - ea_cur) * (s / dhl);
+                ea_cur = ea_next;
+            }
+            h_cur = h_next;
+        }
+        if (ground) {
+            double S_line, d_line, d_true;
+            if (sph) {
+                const double re = atm.R + h_e, rg = atm.Rg, p = re * sz;
+                S_line = re * cz - sqrt(rg * rg - p * p);
+                d_line = rg * (asin(p / rg) - th);
+                d_true = rg * psi;
+            } else {
+                S_line = (h_e - h_g) / cz;
+                d_line = (h_e - h_g) * sz / cz;
+                d_true = psi;
+            }
+            out[0] = (float)(d_true - d_line);
+            out[1] = (float)(S - S_line);
+            out[2] = (float)((cT - S_line) / kC);
+            out[3] = (float)X;
+            out[4] = (float)tau;
+        } else {
+            const float nanv = __int_as_float(0x7FC00000);
+            for (int k = 0; k < 5; ++k) out[k] = nanv;
+        }
+    }
+    for (int k = 0; k < 5; ++k) a.full[(size_t)node * 5 + k] = out[k];
+    a.hot[node] = make_float4(out[0], out[2], out[3], out[4]);
+}
+
+template <int EMIT, int TRACE, bool SPH>
+cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
+{
+    auto kern = k_emit_propagate<EMIT, TRACE, SPH>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long warps_needed = (a.run.n_seg + a.run.segs_per_grab - 1) / a.run.segs_per_grab;
+    long long blocks = (warps_needed + kWarps - 1) / kWarps;
+    const long long max_blocks = (long long)n_sm * per_sm;          // persistent: one resident wave
+    if (blocks > max_blocks) blocks = max_blocks;
+    if (blocks < 1) blocks = 1;
+    kern<<<(unsigned)blocks, kThreads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t emit_smem_bytes(const KArgs &a)
+{
+    const size_t tables = (size_t)a.atm.n_pad * 4u * (a.run.trace == C8PH_TRACE_NUMERIC ? 3u : 1u);
+    return tables + (size_t)kWarps * kStage * (sizeof(c8ph_photon) + sizeof(float));
+}
+
+cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
+{
+    const size_t smem = emit_smem_bytes(a);
+    const bool sph = a.atm.model == C8PH_ATM_SPHERICAL;
+#define C8_CASE(E, T)                                                             \
+    if (a.run.emit == E && a.run.trace == T)                                      \
+        return sph ? launch_one<E, T, true>(a, n_sm, smem, st) : launch_one<E, T, false>(a, n_sm, smem, st);
+    C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_STRAIGHT)
+    C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_NUMERIC)
+    C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE)
+    C8_CASE(C8PH_EMIT_FLUORESCENCE, C8PH_TRACE_STRAIGHT)
+    C8_CASE(C8PH_EMIT_FLUORESCENCE, C8PH_TRACE_TABLE)
+#undef C8_CASE
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st)
+{
+    const int n = a.n_h * a.n_zen;
+    k_build_table<<<(n + 127) / 128, 128, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace c8ph
