@@ -22,8 +22,13 @@ def _key(seg, j):
     return seg.astype(np.int64) * (1 << 18) + j.astype(np.int64)
 
 
-def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True) -> dict:
-    """Returns a report dict and raises AssertionError on any violated tolerance."""
+def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_range_m: float = None) -> dict:
+    """Returns a report dict and raises AssertionError on any violated tolerance.
+
+    max_range_m: if given, the per-photon position / time / direction tolerances are applied to the
+    photons the oracle lands within that distance of the array centre; photons beyond it (grazing
+    rays of stress inputs, |u_z| -> 1e-6, whose landing point is ill-conditioned in any fp32
+    evaluation: d(x)/d(u_z) = D/u_z) are matched by key only.  The BASELINE configs never need it."""
     par, det = cfg["params"], cfg["detector"]
     rep = {}
     oc, gc = ora["counters"], gpu["counters"]
@@ -84,6 +89,10 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True) -> dict
     assert unmatched <= budget, (unmatched, budget)
     g = gph[gi][ia]
     o = want[oi][ib]
+    if max_range_m is not None:
+        near = np.hypot(o["x"], o["y"]) <= max_range_m
+        rep["beyond_range"] = int((~near).sum())
+        g, o = g[near], o[near]
     dx, dy = g["x"].astype(np.float64) - o["x"], g["y"].astype(np.float64) - o["y"]
     dt = g["t_ns"].astype(np.float64) - (o["t"] - float(det["t_ref_ns"]))
     guz = -np.sqrt(np.maximum(0.0, 1.0 - g["ux"].astype(np.float64) ** 2 - g["uy"].astype(np.float64) ** 2))
