@@ -89,6 +89,7 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
     assert unmatched <= budget, (unmatched, budget)
     g = gph[gi][ia]
     o = want[oi][ib]
+    near = np.ones(len(o), dtype=bool)
     if max_range_m is not None:
         near = np.hypot(o["x"], o["y"]) <= max_range_m
         rep["beyond_range"] = int((~near).sum())
@@ -113,7 +114,7 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
     rep["tel_flips"] = tel_flips
     assert tel_flips <= budget
     if gpu.get("photon_weight") is not None and len(gph):
-        w = gpu["photon_weight"][gi][ia]
+        w = gpu["photon_weight"][gi][ia][near]
         assert np.allclose(w, o["weight"], rtol=2e-5, atol=0), "photon weight"
     # per-photon bin agreement recomputed from the device positions (hist grid only)
     if det["hist_nx"] > 0 and not det["cam_enabled"] and len(g):
