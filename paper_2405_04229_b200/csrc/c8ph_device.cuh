@@ -7,6 +7,8 @@
 
 namespace c8ph {
 
+#define C8PH_MAX_BLOCKS_PER_SM 8
+
 struct DevAtm {
     int model;              // C8PH_ATM_*
     int n_nodes;            // nodes of the n(h) grid (>= 2; homogeneous: 2 identical nodes)
@@ -31,11 +33,20 @@ struct DevTable {
     const float *full;              // DEVICE [n_h][n_zen][5]
 };
 
-struct DevGrid {                    // uniform grid over telescopes; cell lists of candidate indices
+// Uniform grid over the telescope array.  Every cell lists the telescopes that a point of the cell
+// can reach, SORTED by a lower-bound key, together with the smallest key of the cell, so that the
+// common "nothing near" case exits after one 4-byte load and a search stops at the first key
+// above the photon's threshold.
+//   hit grid: key = dist(cell rectangle, centre_xy) / (r + |z|);  a photon with direction u at a
+//             point of the cell can hit the sphere only if key <= 1/|u_z|
+//   LV2 grid: key = dist(cell rectangle, centre_xy) [m];  the point can be within r/|u_z| + margin
+//             of the centre only if key <= r_max/|u_z| + margin
+struct DevGrid {
     float x0, y0, inv_cs;
     int nx, ny;
-    const int *start;               // DEVICE [nx*ny+1]
-    const int *items;               // DEVICE
+    const float *kmin;              // DEVICE [nx*ny]   smallest key of the cell (+inf: empty)
+    const int *start;               // DEVICE [nx*ny+1] CSR offsets into items
+    const float2 *items;            // DEVICE (key, telescope index as int bits), ascending key per cell
 };
 
 struct DevDet {
@@ -45,6 +56,7 @@ struct DevDet {
     const float4 *tel;              // DEVICE [n_tel]
     int use_grid;                   // 0: brute force over all telescopes
     float grid_min_cos;             // the grids are valid for |u_z| >= grid_min_cos
+    float r_max;                    // largest telescope radius (LV2 threshold)
     DevGrid lv2, hit;
     double r_array;                 // bounding radius of telescopes + histogram about the origin
     int cam_enabled, cam_rows, cam_cols, n_tbins;
@@ -61,6 +73,10 @@ struct DevRun {
     double yield_k;                 // Cherenkov: 2 pi alpha (1/l1 - 1/l2) [1/m]
     double lv1_margin;
     float lv2_margin;
+    float box_x0, box_x1, box_y0, box_y1;   // LV2: histogram extent widened by the margin (empty if no grid)
+    float inv_Rg;                   // 1 / (R + h_obs)
+    float hit_infl;                 // telescope pre-test: 1/|u_z| inflated to cover the refraction rotation
+    int hit_brute;                  // 1: the rotation can exceed what the hit grid lists cover -> search all
     double fluor_yield, aim_factor;
     int n_lines;
     const float *line_nm, *line_cdf;      // DEVICE
@@ -69,6 +85,7 @@ struct DevRun {
     c8ph_segments seg;              // DEVICE pointers
     c8ph_outputs out;               // DEVICE pointers
     unsigned long long *cursor;     // DEVICE work cursor (segments)
+    void *slots_hot, *slots_cold;   // DEVICE scratch: 32 prepared-segment slots (hot / cold part) per resident warp
     int segs_per_grab;              // segments one warp prepares per grab (1..32)
 };
 
@@ -91,5 +108,7 @@ struct TableBuildArgs {
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st);
 cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st);
 size_t emit_smem_bytes(const KArgs &a);
+size_t segment_slot_bytes(int n_sm);
+void segment_slot_pointers(void *base, int n_sm, DevRun &run);
 
 }  // namespace c8ph

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -18,6 +19,8 @@ struct c8ph_ctx {
     // atmosphere
     bool have_atm = false;
     DevAtm atm{};
+    bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
+    double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
     float *d_eta = nullptr, *d_xv = nullptr, *d_mid = nullptr, *d_dxv = nullptr;
     // table
     bool have_table = false;
@@ -29,9 +32,12 @@ struct c8ph_ctx {
     bool have_det = false;
     DevDet det{};
     float4 *d_tel = nullptr;
-    int *d_g_start[2] = {nullptr, nullptr}, *d_g_items[2] = {nullptr, nullptr};
+    int *d_g_start[2] = {nullptr, nullptr};
+    float2 *d_g_items[2] = {nullptr, nullptr};
+    float *d_g_kmin[2] = {nullptr, nullptr};
     // run scratch
     unsigned long long *d_cursor = nullptr;
+    void *d_slots = nullptr;           // prepared-segment slots of the resident warps
     float *d_lines = nullptr;          // [2][max_lines]
     int lines_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -82,9 +88,11 @@ extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
     c8ph_ctx *ctx = new (std::nothrow) c8ph_ctx();
     if (!ctx) return fail(nullptr, C8PH_E_NOMEM, "c8ph_create: out of host memory");
     ctx->device = cuda_device;
+    { const char *e = getenv("C8PH_FORCE_BRUTE"); ctx->force_brute = e && e[0] == '1'; }
     if ((e = cudaSetDevice(cuda_device)) != cudaSuccess ||
         (e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_slots, segment_slot_bytes(ctx->n_sm))) != cudaSuccess ||
         (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess) {
         g_create_err = std::string("c8ph_create: ") + cudaGetErrorString(e);
         delete ctx;
@@ -100,8 +108,9 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     cudaSetDevice(ctx->device);
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
-    for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); }
+    for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_seg);
+    if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
@@ -162,6 +171,8 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
     a.eta = ctx->d_eta; a.xv = ctx->d_xv; a.eta_mid = ctx->d_mid; a.dxv = ctx->d_dxv;
     a.R = d->earth_radius_m; a.h_obs = d->h_obs_m; a.Rg = (double)d->earth_radius_m + (double)d->h_obs_m;
     a.eta_g = (float)lerp_table(eta, h0, dh, d->h_obs_m);
+    ctx->eta_span = 0.0;
+    for (float v : eta) ctx->eta_span = std::max(ctx->eta_span, std::fabs((double)v - (double)a.eta_g));
     a.ray_inv_X = d->rayleigh_X_gcm2 > 0.f ? 1.0f / d->rayleigh_X_gcm2 : 0.f;
     a.ray_lambda = d->rayleigh_lambda_nm;
     a.aer_L = d->aer_L_m; a.aer_H = d->aer_H_m; a.aer_lambda = d->aer_lambda_nm; a.aer_angstrom = d->aer_angstrom;
@@ -244,75 +255,113 @@ extern "C" int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, con
 }
 
 // ------------------------------------------------------------------------------------ detector
-// Uniform grid over the telescope footprints: cell -> telescopes whose disc of radius `reach_k`
-// about the centre overlaps the cell.  Item lists are ascending in k.
-static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, const std::vector<double> &reach, DevGrid &g)
+// Uniform grid over the telescope footprints (see DevGrid).  mode 0 (hit): key = dist(cell, centre)
+// / (r + |z|), listed while key <= key_max = 1/min_cos.  mode 1 (LV2): key = dist(cell, centre) in
+// metres, listed while key <= r_max/min_cos + margin_max.  Cell rectangles are padded so that the
+// fp32 cell index of a point can be off by rounding without losing a candidate; keys are rounded
+// DOWN to fp32 so a device-side "key > threshold" never rejects a reachable telescope.
+static const double kLv2MarginMax = 64.0;   // the LV2 grid lists telescopes up to this margin
+static const double kGridMinCos = 0.2588190451;   // grids valid up to 75 deg zenith
+static const double kHitListSlack = 0.02;    // hit lists reach 2 % beyond 1/min_cos (refraction rotation)
+
+static float f32_down(double v)
 {
-    const int n = (int)reach.size();
-    double x0 = 1e300, y0 = 1e300, x1 = -1e300, y1 = -1e300, rmax = 0.0;
+    float f = (float)v;
+    if ((double)f > v) f = std::nextafterf(f, -INFINITY);
+    return f;
+}
+
+static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, int mode, double min_cos,
+                      double margin_max, DevGrid &g)
+{
+    const int n = (int)tel.size() / 4;
+    double r_max = 0.0, rz_min = 1e300, coord_max = 0.0;
     for (int k = 0; k < n; ++k) {
-        x0 = std::min(x0, tel[4 * k] - reach[k]); x1 = std::max(x1, tel[4 * k] + reach[k]);
-        y0 = std::min(y0, tel[4 * k + 1] - reach[k]); y1 = std::max(y1, tel[4 * k + 1] + reach[k]);
-        rmax = std::max(rmax, reach[k]);
+        r_max = std::max(r_max, (double)tel[4 * k + 3]);
+        rz_min = std::min(rz_min, (double)tel[4 * k + 3] + std::fabs((double)tel[4 * k + 2]));
+        coord_max = std::max(coord_max, std::max(std::fabs((double)tel[4 * k]), std::fabs((double)tel[4 * k + 1])));
     }
-    double cs = std::max(rmax, std::max(x1 - x0, y1 - y0) / 2048.0);
+    auto reach = [&](int k) {            // horizontal distance up to which telescope k is listed
+        const double rz = (double)tel[4 * k + 3] + std::fabs((double)tel[4 * k + 2]);
+        return mode == 0 ? rz / min_cos * (1.0 + kHitListSlack) : r_max / min_cos + margin_max;
+    };
+    double x0 = 1e300, y0 = 1e300, x1 = -1e300, y1 = -1e300;
+    for (int k = 0; k < n; ++k) {
+        const double rc = reach(k) * 1.001 + 1e-2;
+        x0 = std::min(x0, tel[4 * k] - rc); x1 = std::max(x1, tel[4 * k] + rc);
+        y0 = std::min(y0, tel[4 * k + 1] - rc); y1 = std::max(y1, tel[4 * k + 1] + rc);
+    }
+    const double ext = std::max(x1 - x0, y1 - y0);
+    double cs = mode == 0 ? rz_min : 2.0 * r_max;
+    cs = std::max(cs, ext / 1536.0);
     if (!(cs > 0.0)) cs = 1.0;
     const int nx = std::max(1, (int)std::ceil((x1 - x0) / cs)), ny = std::max(1, (int)std::ceil((y1 - y0) / cs));
-    std::vector<int> count((size_t)nx * ny + 1, 0);
-    auto cells = [&](int k, int &cx0, int &cx1, int &cy0, int &cy1) {
-        cx0 = std::max(0, (int)std::floor((tel[4 * k] - reach[k] - x0) / cs) - 1);
-        cx1 = std::min(nx - 1, (int)std::floor((tel[4 * k] + reach[k] - x0) / cs) + 1);
-        cy0 = std::max(0, (int)std::floor((tel[4 * k + 1] - reach[k] - y0) / cs) - 1);
-        cy1 = std::min(ny - 1, (int)std::floor((tel[4 * k + 1] + reach[k] - y0) / cs) + 1);
-    };
-    // a telescope is listed in a cell iff its disc overlaps the cell rectangle (padded by 1e-3 cell)
-    auto overlaps = [&](int k, int cx, int cy) {
-        const double pad = 1e-3 * cs;
-        const double bx0 = x0 + cx * cs - pad, bx1 = x0 + (cx + 1) * cs + pad, by0 = y0 + cy * cs - pad, by1 = y0 + (cy + 1) * cs + pad;
-        const double px = std::min(std::max((double)tel[4 * k], bx0), bx1), py = std::min(std::max((double)tel[4 * k + 1], by0), by1);
-        const double dx = px - tel[4 * k], dy = py - tel[4 * k + 1];
-        return dx * dx + dy * dy <= reach[k] * reach[k];
-    };
+    const size_t ncell = (size_t)nx * ny;
+    // fp32 rounding of (x - x0) * inv_cs on the device: a few ulp of the largest coordinate
+    const double pad = 1e-3 * cs + 8.0 * (coord_max + ext) * 1.2e-7 + 1e-4;
+    struct Entry { uint32_t cell; float key; int k; };
+    std::vector<Entry> ent;
+    ent.reserve((size_t)n * 64);
     for (int k = 0; k < n; ++k) {
-        int a, b, c, d; cells(k, a, b, c, d);
-        for (int cy = c; cy <= d; ++cy) for (int cx = a; cx <= b; ++cx) if (overlaps(k, cx, cy)) count[(size_t)cy * nx + cx + 1]++;
+        const double cx_ = tel[4 * k], cy_ = tel[4 * k + 1], rc = reach(k);
+        const double rz = (double)tel[4 * k + 3] + std::fabs((double)tel[4 * k + 2]);
+        const int a = std::max(0, (int)std::floor((cx_ - rc - pad - x0) / cs)), b = std::min(nx - 1, (int)std::floor((cx_ + rc + pad - x0) / cs));
+        const int c = std::max(0, (int)std::floor((cy_ - rc - pad - y0) / cs)), d = std::min(ny - 1, (int)std::floor((cy_ + rc + pad - y0) / cs));
+        for (int iy = c; iy <= d; ++iy)
+            for (int ix = a; ix <= b; ++ix) {
+                const double bx0 = x0 + ix * cs - pad, bx1 = x0 + (ix + 1) * cs + pad;
+                const double by0 = y0 + iy * cs - pad, by1 = y0 + (iy + 1) * cs + pad;
+                const double px = std::min(std::max(cx_, bx0), bx1), py = std::min(std::max(cy_, by0), by1);
+                const double dist = std::sqrt((px - cx_) * (px - cx_) + (py - cy_) * (py - cy_));
+                if (dist > rc) continue;
+                const double key = mode == 0 ? dist / rz : dist;
+                ent.push_back({(uint32_t)((size_t)iy * nx + ix), f32_down(key * (1.0 - 1e-6)), k});
+            }
     }
-    for (size_t i = 1; i < count.size(); ++i) count[i] += count[i - 1];
-    std::vector<int> items(std::max<size_t>(1, (size_t)count.back())), fill(count.begin(), count.end() - 1);
-    for (int k = 0; k < n; ++k) {
-        int a, b, c, d; cells(k, a, b, c, d);
-        for (int cy = c; cy <= d; ++cy) for (int cx = a; cx <= b; ++cx) if (overlaps(k, cx, cy)) items[fill[(size_t)cy * nx + cx]++] = k;
+    std::sort(ent.begin(), ent.end(), [](const Entry &l, const Entry &r) {
+        if (l.cell != r.cell) return l.cell < r.cell;
+        if (l.key != r.key) return l.key < r.key;
+        return l.k < r.k;
+    });
+    std::vector<int> start(ncell + 1, 0);
+    std::vector<float> kmin(ncell, INFINITY);
+    std::vector<float2> items(std::max<size_t>(1, ent.size()));
+    for (const Entry &e : ent) start[e.cell + 1]++;
+    for (size_t i = 1; i <= ncell; ++i) start[i] += start[i - 1];
+    for (size_t i = 0; i < ent.size(); ++i) {
+        float kb;
+        memcpy(&kb, &ent[i].k, sizeof kb);
+        items[i] = make_float2(ent[i].key, kb);
+        if (ent[i].key < kmin[ent[i].cell]) kmin[ent[i].cell] = ent[i].key;
     }
-    dfree(ctx->d_g_start[which]); dfree(ctx->d_g_items[which]);
-    CU(cudaMalloc(&ctx->d_g_start[which], count.size() * sizeof(int)));
-    CU(cudaMalloc(&ctx->d_g_items[which], items.size() * sizeof(int)));
-    CU(cudaMemcpy(ctx->d_g_start[which], count.data(), count.size() * sizeof(int), cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(ctx->d_g_items[which], items.data(), items.size() * sizeof(int), cudaMemcpyHostToDevice));
+    dfree(ctx->d_g_start[which]); dfree(ctx->d_g_items[which]); dfree(ctx->d_g_kmin[which]);
+    CU(cudaMalloc(&ctx->d_g_start[which], start.size() * sizeof(int)));
+    CU(cudaMalloc(&ctx->d_g_items[which], items.size() * sizeof(float2)));
+    CU(cudaMalloc(&ctx->d_g_kmin[which], kmin.size() * sizeof(float)));
+    CU(cudaMemcpy(ctx->d_g_start[which], start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_g_items[which], items.data(), items.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_g_kmin[which], kmin.data(), kmin.size() * sizeof(float), cudaMemcpyHostToDevice));
     g.x0 = (float)x0; g.y0 = (float)y0; g.inv_cs = (float)(1.0 / cs); g.nx = nx; g.ny = ny;
-    g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
+    g.kmin = ctx->d_g_kmin[which]; g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
     return C8PH_OK;
 }
 
-static int setup_detector(c8ph_ctx *ctx, const c8ph_detector *d, float lv2_margin_for_grid)
+
+static int setup_detector(c8ph_ctx *ctx, const c8ph_detector *d)
 {
     DevDet &o = ctx->det;
     const int n = d->n_tel;
     std::vector<float> tel(d->tel_xyzr ? d->tel_xyzr : nullptr, d->tel_xyzr ? d->tel_xyzr + 4 * (size_t)n : nullptr);
+    o.r_max = 0.f;
+    for (int k = 0; k < n; ++k) o.r_max = std::max(o.r_max, tel[4 * k + 3]);
     if (n > 0) {
-        const double min_cos = 0.2588190451;                       // grids valid up to 75 deg zenith
-        o.grid_min_cos = (float)(min_cos * (1.0 + 1e-6));
+        const double min_cos = kGridMinCos;
+        o.grid_min_cos = (float)(min_cos * (1.0 + 1e-4));
         o.use_grid = n > 8 ? 1 : 0;
         if (o.use_grid) {
-            std::vector<double> r_hit(n), r_lv2(n);
-            for (int k = 0; k < n; ++k) {
-                const double tant = std::sqrt(1.0 - min_cos * min_cos) / min_cos;
-                // footprint of the sphere on z = 0 for zenith <= 75 deg, inflated for fp32 rounding
-                r_hit[k] = (tel[4 * k + 3] / min_cos + std::fabs(tel[4 * k + 2]) * tant) * 1.001 + 1e-3;
-                r_lv2[k] = (tel[4 * k + 3] / min_cos + lv2_margin_for_grid) * 1.001 + 1e-3;
-            }
-            int rc = build_grid(ctx, 0, tel, r_hit, o.hit);
+            int rc = build_grid(ctx, 0, tel, 0, min_cos, 0.0, o.hit);
             if (rc) return rc;
-            rc = build_grid(ctx, 1, tel, r_lv2, o.lv2);
+            rc = build_grid(ctx, 1, tel, 1, min_cos, kLv2MarginMax, o.lv2);
             if (rc) return rc;
         }
     }
@@ -366,8 +415,8 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
     }
     o.tel = ctx->d_tel;
     ctx->det = o;
-    // the LV2 grid is built for margins up to 64 m; larger margins fall back to brute force (see emit)
-    int rc = setup_detector(ctx, d, 64.0f);
+    // the LV2 grid lists telescopes for margins up to kLv2MarginMax (checked in emit_propagate)
+    int rc = setup_detector(ctx, d);
     if (rc) return rc;
     ctx->have_det = true;
     return C8PH_OK;
@@ -402,11 +451,12 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         if (p->n_lines < 1 || !p->line_nm || !p->line_cdf) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence line spectrum");
         if (n_seg > 0 && !s->edep) return fail(ctx, C8PH_E_ARG, "emit_propagate: edep is NULL");
     }
-    if (p->filter_lv2 && p->lv2_margin_m > 64.0f && ctx->det.use_grid)
-        return fail(ctx, C8PH_E_ARG, "emit_propagate: lv2_margin_m > 64 m is not covered by the LV2 grid");
+    if (p->filter_lv2 && (!(p->lv2_margin_m >= 0.f) || (p->lv2_margin_m > (float)kLv2MarginMax && ctx->det.use_grid)))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: lv2_margin_m must be in [0, 64] m (range covered by the LV2 grid)");
     a.atm = ctx->atm;
     a.tab = ctx->tab;
     a.det = ctx->det;
+    if (ctx->force_brute) a.det.use_grid = 0;
     DevRun &r = a.run;
     r.emit = p->emit; r.trace = p->trace; r.trans = p->trans; r.write = p->write;
     r.lv1 = p->filter_lv1 ? 1 : 0; r.lv2 = p->filter_lv2 ? 1 : 0;
@@ -417,7 +467,26 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
                     ? 2.0 * 3.14159265358979323846 / 137.035999 * (1.0 / ((double)p->lambda_min_nm * 1e-9) - 1.0 / ((double)p->lambda_max_nm * 1e-9))
                     : 0.0;
     r.lv1_margin = p->lv1_margin_rad; r.lv2_margin = p->lv2_margin_m;
+    {
+        // LV2 keep-box: the histogram extent widened by the margin, in the fp32 arithmetic of the test
+        const DevDet &dd = ctx->det;
+        const bool geom = dd.hist_nx > 0 && !dd.cam_enabled;
+        const float m = p->lv2_margin_m;
+        const float hx1 = dd.hist_x0 + (float)dd.hist_nx * dd.hist_cell, hy1 = dd.hist_y0 + (float)dd.hist_ny * dd.hist_cell;
+        r.box_x0 = geom ? dd.hist_x0 - m : INFINITY; r.box_x1 = geom ? hx1 + m : -INFINITY;
+        r.box_y0 = geom ? dd.hist_y0 - m : INFINITY; r.box_y1 = geom ? hy1 + m : -INFINITY;
+    }
     r.fluor_yield = p->fluor_yield_per_MeV; r.aim_factor = p->aim_factor;
+    r.inv_Rg = (float)(1.0 / ctx->atm.Rg);
+    {
+        // relative change of 1/|u_z| by the refraction rotation: <= (n_e - n_g)/n_g tan^2(zenith) plus
+        // the spherical term, at the grid's zenith limit; the hit lists are built for 2 % (kHitListSlack)
+        const double tan2 = 1.0 / (kGridMinCos * kGridMinCos) - 1.0;
+        const double infl = 1.0 + 2.0 * ctx->eta_span * tan2 + 1e-3;
+        r.hit_infl = (float)infl;
+        r.hit_brute = (p->trace != C8PH_TRACE_STRAIGHT && infl > 1.0 + 0.9 * kHitListSlack) ? 1 : 0;
+        if (p->trace == C8PH_TRACE_STRAIGHT) r.hit_infl = 1.0f + 1e-5f;
+    }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
     if (p->emit == C8PH_EMIT_FLUORESCENCE) {
         if (p->n_lines > ctx->lines_cap) {
@@ -436,6 +505,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     r.n_seg = n_seg; r.seg_id_base = base;
     r.seg = *s; r.out = *o;
     r.cursor = ctx->d_cursor;
+    segment_slot_pointers(ctx->d_slots, ctx->n_sm, r);
     const long long warps = (long long)ctx->n_sm * 2 * 8;
     long long g = n_seg / (warps * 4);
     r.segs_per_grab = (int)std::min<long long>(32, std::max<long long>(1, g));

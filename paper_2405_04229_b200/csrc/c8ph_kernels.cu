@@ -36,7 +36,8 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kStage = 64;                       // photon records staged per warp
+constexpr int kMaxBlocksPerSM = C8PH_MAX_BLOCKS_PER_SM;
+constexpr int kMinBlocks = 3;                    // resident CTAs per SM the register budget is set for
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
 constexpr double kAlpha = 1.0 / 137.035999;
@@ -102,37 +103,44 @@ __device__ __forceinline__ double u01d(uint32_t r)
     return (static_cast<double>(r >> 9) + 0.5) * (1.0 / 8388608.0);
 }
 
-// ---- per-segment state (prepared by one lane in fp64, broadcast to the warp) --------------------
-struct Seg {
+// ---- per-segment state: prepared by one lane in fp64, parked in the warp's slot of a global
+// scratch array (L2-resident), then read back by all lanes (uniform address).  HOT = used by every
+// photon, kept in registers while the warp walks the segment; COLD = used by landed photons /
+// rare branches, re-read through L1 where it is needed (keeps the register count down).
+struct alignas(16) SegHot {                       // 28 words = 7 x 16 B
     float Px, Py, Pz, e1x, e1y, e1z, e2x, e2y, e2z;   // direction and the two Rodrigues columns
-    float Ax, Ay, Az, L, beta, delta;                 // start point, length, beta, 1 - beta
-    float Gx, Gy;                                      // axis landing point (anchor) or unused
-    float fbx, fby;                                    // fractional grid coordinate of the anchor
-    int ibx, iby;                                      // integer grid coordinate of the anchor
-    float Tg;                                          // anchor clock - t_ref  (or t0 - t_ref)
-    float AzP;                                         // A_z / P_z (anchor form)
-    float hA, cA, k2;                                  // height of A, dh/ds, second-order term
-    float rx, ry, rz, inv_rA, a1, a2;                  // local vertical at A; e1.r, e2.r
-    // fluorescence
-    float aimx, aimy, aimz, omc;                       // aim point, 1 - cos(psi)
-    int N;                                             // bunches to emit
-    int anchor;                                        // 1: anchor form valid
-    uint32_t id_lo, id_hi, local;
+    float L, beta, delta;                             // length, beta, 1 - beta
+    float hA, cA, k2;                                 // height of A, dh/ds, second-order term
+    float Az, AzP;                                    // A_z, A_z / P_z (anchor form)
+    float Gx, Gy;                                     // axis landing point (anchor) or unused
+    float a1, a2, inv_rA;                             // e1.r, e2.r, 1/|A - C|
+    uint32_t id_lo, id_hi;                            // global segment id (Philox counter words)
+    int N, anchor;                                    // bunches to emit; 1: anchor form valid
+    float pad0, pad1;
 };
+struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
+    float fbx, fby;                                   // fractional grid coordinate of the anchor
+    int ibx, iby;                                     // integer grid coordinate of the anchor
+    float rx, ry, rz;                                 // local vertical at A
+    float Ax, Ay;                                     // start point (non-anchor form)
+    float aimx, aimy, aimz, omc;                      // fluorescence: aim point, 1 - cos(psi)
+    float Tg;                                         // anchor clock - t_ref  (or t0 - t_ref)
+    uint32_t local;                                   // segment index within the call
+    float pad0;
+};
+static_assert(sizeof(SegHot) == 112 && sizeof(SegCold) == 64, "segment slot layout");
 
-__device__ __forceinline__ Seg shfl_seg(const Seg &s, int src)
+// candidate queue entry (SoA in shared memory): what finish() needs of a photon
+enum { Q_X = 0, Q_Y, Q_UX, Q_UY, Q_UZ, Q_T, Q_LAMINV, Q_WGT, Q_ETA, Q_H, Q_DD, Q_CZ, Q_CELL, Q_JSLOT, Q_WORDS };
+constexpr int kQueue = 64;                       // ring entries per warp (a drain leaves < 32)
+
+template <typename T>
+__device__ __forceinline__ void copy16(T *dst, const T *src)
 {
-    Seg o;
-    const unsigned m = 0xFFFFFFFFu;
-#define C8_SH(f) o.f = __shfl_sync(m, s.f, src)
-    C8_SH(Px); C8_SH(Py); C8_SH(Pz); C8_SH(e1x); C8_SH(e1y); C8_SH(e1z); C8_SH(e2x); C8_SH(e2y); C8_SH(e2z);
-    C8_SH(Ax); C8_SH(Ay); C8_SH(Az); C8_SH(L); C8_SH(beta); C8_SH(delta);
-    C8_SH(Gx); C8_SH(Gy); C8_SH(fbx); C8_SH(fby); C8_SH(ibx); C8_SH(iby); C8_SH(Tg); C8_SH(AzP);
-    C8_SH(hA); C8_SH(cA); C8_SH(k2); C8_SH(rx); C8_SH(ry); C8_SH(rz); C8_SH(inv_rA); C8_SH(a1); C8_SH(a2);
-    C8_SH(aimx); C8_SH(aimy); C8_SH(aimz); C8_SH(omc);
-    C8_SH(N); C8_SH(anchor); C8_SH(id_lo); C8_SH(id_hi); C8_SH(local);
-#undef C8_SH
-    return o;
+    const float4 *s = reinterpret_cast<const float4 *>(src);
+    float4 *d = reinterpret_cast<float4 *>(dst);
+#pragma unroll
+    for (int i = 0; i < (int)(sizeof(T) / 16); ++i) d[i] = s[i];
 }
 
 // n-1 at height h from the global table in fp64 (Listing 4.1), clamped to the table
@@ -166,56 +174,70 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
     return o;
 }
 
-// telescope candidates around (x,y): nearest entry along the arrival ray, lowest index on ties
-__device__ __forceinline__ int tel_hit_cell(const DevDet &det, const DevGrid &g, float x, float y,
-                                            float ux, float uy, float uz, bool brute)
+// ---- telescope search (DevGrid: sorted candidate lists with a per-cell smallest key) -----------
+// cell of (x,y), or -1 outside the grid (outside => no telescope within reach)
+__device__ __forceinline__ int grid_cell(const DevGrid &g, float x, float y)
+{
+    const int cx = __float2int_rd((x - g.x0) * g.inv_cs), cy = __float2int_rd((y - g.y0) * g.inv_cs);
+    if ((unsigned)cx >= (unsigned)g.nx || (unsigned)cy >= (unsigned)g.ny) return -1;
+    return cy * g.nx + cx;
+}
+
+// exact ray / bounding-sphere test of one telescope; updates the nearest entry
+__device__ __forceinline__ void sphere_test(const DevDet &det, int k, float x, float y, float ux, float uy, float uz,
+                                            float &best_s, int &best_k)
+{
+    const float4 t = __ldg(det.tel + k);
+    const float dx = t.x - x, dy = t.y - y, dz = t.z;
+    const float du = dx * ux + dy * uy + dz * uz;
+    const float m2 = dx * dx + dy * dy + dz * dz - du * du;
+    const float r2 = t.w * t.w;
+    if (m2 <= r2) {
+        const float s_in = du - sqrtf(r2 - m2);
+        if (s_in < best_s || (s_in == best_s && k < best_k)) { best_s = s_in; best_k = k; }
+    }
+}
+
+// nearest entry along the arrival ray, lowest index on ties.  `cell` < -1: brute force over all
+// telescopes; otherwise the sorted candidates of the cell while key <= thr (thr >= 1/|u_z|).
+__device__ __forceinline__ int tel_hit_search(const DevDet &det, int cell, float thr, float x, float y,
+                                           float ux, float uy, float uz)
 {
     int best_k = -1;
     float best_s = CUDART_INF_F;
-    int lo = 0, hi = det.n_tel;
-    const int *items = nullptr;
-    if (!brute) {
-        const int cx = (int)floorf((x - g.x0) * g.inv_cs), cy = (int)floorf((y - g.y0) * g.inv_cs);
-        if (cx < 0 || cy < 0 || cx >= g.nx || cy >= g.ny) return -1;
-        const int c = cy * g.nx + cx;
-        lo = __ldg(g.start + c);
-        hi = __ldg(g.start + c + 1);
-        items = g.items;
+    if (cell < -1) {
+        for (int k = 0; k < det.n_tel; ++k) sphere_test(det, k, x, y, ux, uy, uz, best_s, best_k);
+        return best_k;
     }
-    for (int i = lo; i < hi; ++i) {
-        const int k = items ? __ldg(items + i) : i;
-        const float4 t = __ldg(det.tel + k);
-        const float dx = t.x - x, dy = t.y - y, dz = t.z;
-        const float du = dx * ux + dy * uy + dz * uz;
-        const float m2 = dx * dx + dy * dy + dz * dz - du * du;
-        const float r2 = t.w * t.w;
-        if (m2 <= r2) {
-            const float s_in = du - sqrtf(r2 - m2);
-            if (s_in < best_s) { best_s = s_in; best_k = k; }
-        }
+    if (cell < 0) return -1;
+    const int hi = __ldg(det.hit.start + cell + 1);
+    for (int i = __ldg(det.hit.start + cell); i < hi; ++i) {
+        const float2 e = __ldg(det.hit.items + i);
+        if (e.x > thr) break;
+        sphere_test(det, __float_as_int(e.y), x, y, ux, uy, uz, best_s, best_k);
     }
     return best_k;
 }
 
-// LV2/LV3 proximity: is the straight-line point within r/|u_z| + margin of any telescope centre?
-__device__ __forceinline__ bool tel_near(const DevDet &det, float x, float y, float inv_abs_uz, float margin, bool brute)
+// LV2/LV3 proximity: is (x,y) within r_k/|u_z| + margin of any telescope centre?
+__device__ __forceinline__ bool tel_near_search(const DevDet &det, int cell, float thr, float x, float y,
+                                             float inv_abs_uz, float margin)
 {
-    int lo = 0, hi = det.n_tel;
-    const int *items = nullptr;
-    if (!brute) {
-        const DevGrid &g = det.lv2;
-        const int cx = (int)floorf((x - g.x0) * g.inv_cs), cy = (int)floorf((y - g.y0) * g.inv_cs);
-        if (cx < 0 || cy < 0 || cx >= g.nx || cy >= g.ny) return false;
-        const int c = cy * g.nx + cx;
-        lo = __ldg(g.start + c);
-        hi = __ldg(g.start + c + 1);
-        items = g.items;
+    if (cell < -1) {
+        for (int k = 0; k < det.n_tel; ++k) {
+            const float4 t = __ldg(det.tel + k);
+            const float dx = x - t.x, dy = y - t.y, reach = fmaf(t.w, inv_abs_uz, margin);
+            if (dx * dx + dy * dy <= reach * reach) return true;
+        }
+        return false;
     }
-    for (int i = lo; i < hi; ++i) {
-        const int k = items ? __ldg(items + i) : i;
-        const float4 t = __ldg(det.tel + k);
-        const float dx = x - t.x, dy = y - t.y;
-        const float reach = fmaf(t.w, inv_abs_uz, margin);
+    if (cell < 0) return false;
+    const int hi = __ldg(det.lv2.start + cell + 1);
+    for (int i = __ldg(det.lv2.start + cell); i < hi; ++i) {
+        const float2 e = __ldg(det.lv2.items + i);
+        if (e.x > thr) break;
+        const float4 t = __ldg(det.tel + __float_as_int(e.y));
+        const float dx = x - t.x, dy = y - t.y, reach = fmaf(t.w, inv_abs_uz, margin);
         if (dx * dx + dy * dy <= reach * reach) return true;
     }
     return false;
@@ -256,16 +278,18 @@ __device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float u
     return best;
 }
 
-struct Counters {
-    uint32_t up, lv2, tr, roul, grid, tel, cam;
-};
+// per-warp event counters kept in shared memory (u64), flushed to the global counters at the end
+enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2, WC_TR, WC_ROUL, WC_GRID, WC_TEL,
+       WC_CAM, WC_WRITTEN, WC_OVERFLOW, WC_N };
 
 // ================================================================================================
 template <int EMIT, int TRACE, bool SPH>
-__global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_constant__ KArgs a)
+__global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 1 : kMinBlocks)
+k_emit_propagate(const __grid_constant__ KArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
+    __shared__ unsigned long long s_cnt[kWarps][WC_N];
 
     const DevAtm &atm = a.atm;
     const DevDet &det = a.det;
@@ -273,59 +297,147 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned FULL = 0xFFFFFFFFu;
     unsigned long long *cntp = reinterpret_cast<unsigned long long *>(run.out.counters);
+    constexpr bool STAGED = TRACE == C8PH_TRACE_NUMERIC;     // n(h) tables in shared memory
 
-    // ---- shared memory carve-up: n(h) tables, then the per-warp photon stage
+    // ---- shared memory carve-up: [n(h) tables] | per-warp candidate queue (SoA, kQueue entries)
     float *s_eta = reinterpret_cast<float *>(smem_raw);
-    float *s_mid = s_eta + atm.n_pad;
-    float *s_dxv = s_mid + (TRACE == C8PH_TRACE_NUMERIC ? atm.n_pad : 0);
-    float *s_end = s_dxv + (TRACE == C8PH_TRACE_NUMERIC ? atm.n_pad : 0);
-    c8ph_photon *s_rec = reinterpret_cast<c8ph_photon *>(s_end) + warp * kStage;
-    float *s_wgt = reinterpret_cast<float *>(reinterpret_cast<c8ph_photon *>(s_end) + kWarps * kStage) + warp * kStage;
+    float *s_mid = s_eta + (STAGED ? atm.n_pad : 0);
+    float *s_dxv = s_mid + (STAGED ? atm.n_pad : 0);
+    float *s_end = s_dxv + (STAGED ? atm.n_pad : 0);
+    float *s_q = s_end + warp * (kQueue * Q_WORDS);           // s_q[field * kQueue + slot]
+    __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
+    // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
+    SegHot *g_hot = static_cast<SegHot *>(run.slots_hot) + ((size_t)blockIdx.x * kWarps + warp) * 32;
+    SegCold *g_cold = static_cast<SegCold *>(run.slots_cold) + ((size_t)blockIdx.x * kWarps + warp) * 32;
 
-    // ---- stage the atmosphere tables: one TMA bulk copy per array, completion on an mbarrier
-    if (threadIdx.x == 0) {
-        mbar_init(&s_bar, 1);
-        const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
-        mbar_expect_tx(&s_bar, bytes * (TRACE == C8PH_TRACE_NUMERIC ? 3u : 1u));
-        bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
-        if (TRACE == C8PH_TRACE_NUMERIC) {
+    if (lane < WC_N) s_cnt[warp][lane] = 0ull;
+    if (lane == 0) s_qn[warp] = 0;
+    // ---- layered-sum variant: stage the atmosphere tables with one TMA bulk copy per array
+    if (STAGED) {
+        if (threadIdx.x == 0) {
+            mbar_init(&s_bar, 1);
+            const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
+            mbar_expect_tx(&s_bar, bytes * 3u);
+            bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
             bulk_g2s(s_mid, atm.eta_mid, bytes, &s_bar);
             bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
         }
+        __syncthreads();
+        mbar_wait(&s_bar, 0);
     }
-    __syncthreads();
-    mbar_wait(&s_bar, 0);
+    __syncwarp();
+    // n(h) node: shared memory when staged, otherwise through L1 (the lanes of a warp emit from one
+    // short segment: 1-3 adjacent words, one cache line)
+    auto eta_node = [&](int k) -> float { return STAGED ? s_eta[k] : __ldg(atm.eta + k); };
 
-    Counters cnt = {0, 0, 0, 0, 0, 0, 0};
-    uint32_t c_below = 0, c_lv1 = 0, c_emitting = 0, c_clipped = 0, c_written = 0, c_overflow = 0;
-    unsigned long long c_emitted = 0;
-    int stage_fill = 0;                                   // records waiting in this warp's stage (warp-uniform)
+    // per-lane event counters of the photon loop, two 16-bit fields per register, flushed to
+    // s_cnt before a field can overflow
+    uint32_t pkA = 0, pkB = 0, pkC = 0;          // up | lv2<<16 ; tr | roul<<16 ; grid | tel<<16
+    int iters_pending = 0;
+    auto flush_counts = [&]() {
+        const uint32_t v0 = __reduce_add_sync(FULL, pkA & 0xFFFFu), v1 = __reduce_add_sync(FULL, pkA >> 16);
+        const uint32_t v2 = __reduce_add_sync(FULL, pkB & 0xFFFFu), v3 = __reduce_add_sync(FULL, pkB >> 16);
+        const uint32_t v4 = __reduce_add_sync(FULL, pkC & 0xFFFFu), v5 = __reduce_add_sync(FULL, pkC >> 16);
+        if (lane == 0) {
+            s_cnt[warp][WC_UP] += v0; s_cnt[warp][WC_LV2] += v1; s_cnt[warp][WC_TR] += v2;
+            s_cnt[warp][WC_ROUL] += v3; s_cnt[warp][WC_GRID] += v4; s_cnt[warp][WC_TEL] += v5;
+        }
+        pkA = pkB = pkC = 0;
+        iters_pending = 0;
+    };
 
     const bool has_hist = det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr;
     const bool has_grid_geom = det.hist_nx > 0 && !det.cam_enabled;
-    const float hx1 = det.hist_x0 + det.hist_nx * det.hist_cell, hy1 = det.hist_y0 + det.hist_ny * det.hist_cell;
     const float inv_ng = 1.0f / (1.0f + atm.eta_g);
+    int q_head = 0;                                           // ring position of the oldest queue entry
 
-    // flush `n` staged records (n <= 32) starting at stage slot `first`
-    auto flush = [&](int first, int n) {
-        unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(&cntp[C8PH_CNT_WRITTEN], (unsigned long long)n);
-        base = __shfl_sync(FULL, base, 0);
-        const long long room = run.out.photon_capacity - (long long)base;
-        const int fit = room >= n ? n : (room > 0 ? (int)room : 0);
-        __syncwarp();
-        if (lane < fit) {
-            const int slot = (first + lane) & (kStage - 1);
-            const uint4 *src = reinterpret_cast<const uint4 *>(s_rec + slot);
-            uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + base + lane);
-            dst[0] = src[0];
-            dst[1] = src[1];
-            if (run.out.photon_weight) run.out.photon_weight[base + lane] = s_wgt[slot];
+    // ---- a13/a14/a16 for photons that may hit a telescope or are written anyway: arrival direction
+    // (rotation in the ray plane by the Snell / Bouguer invariant), exact sphere search, counters,
+    // ballot-compacted record store.  Called warp-converged; `act` marks the lanes that carry a photon.
+    auto finish = [&](bool act, float xg, float yg, float ux, float uy, float uz, float t_arr, float lam_inv,
+                      float wgt, float eta_e, float h_e, float dd, float cz, int cell, uint32_t jslot) {
+        int tel = -1;
+        float uax = ux, uay = uy, uaz = uz;
+        const SegCold *sc = g_cold + (jslot & 31u);
+        if (act) {
+            const float sinz = sqrtf(fmaxf(1.f - cz * cz, 0.f));
+            if (TRACE != C8PH_TRACE_STRAIGHT && sinz >= 1e-6f) {
+                const float eps = (eta_e - atm.eta_g) * inv_ng;
+                const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * run.inv_Rg : 1.f;
+                const float al = sinz * scale;
+                const float cyy = sqrtf(fmaxf(1.f - al * al, 0.f));
+                const float at = al * (1.f + eps);
+                const float cxx = sqrtf(fmaxf(1.f - at * at, 0.f));
+                float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * __frcp_rn(cyy + cxx));
+                if (SPH) dl -= dd * run.inv_Rg;
+                const float k1 = 1.f - 0.5f * dl * dl + dl * cz / sinz, k2 = dl / sinz;
+                uax = fmaf(k1, ux, k2 * sc->rx);
+                uay = fmaf(k1, uy, k2 * sc->ry);
+                uaz = fmaf(k1, uz, k2 * sc->rz);
+            }
+            if (det.n_tel > 0 && cell != -1) {
+                // the pre-test threshold must cover the rotated direction; if it does not (never in
+                // air), search all telescopes
+                const float thr = -__frcp_rn(uz) * run.hit_infl;
+                if (cell >= 0 && !(-uaz * thr >= 1.f)) cell = -2;
+                tel = tel_hit_search(det, cell, thr, xg, yg, uax, uay, uaz);
+            }
+            if (tel >= 0) {
+                pkC += 0x10000u;
+                if (run.out.tel_counts) atomicAdd(run.out.tel_counts + tel, wgt);
+                if (det.cam_enabled) {
+                    const int pix = camera_pixel(det, uax, uay, uaz);
+                    const float tb = floorf(t_arr * det.inv_t_bin);
+                    if (pix >= 0 && tb >= 0.f && tb < (float)det.n_tbins) {
+                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                        if (run.out.hist) atomicAdd(run.out.hist + (size_t)pix * det.n_tbins + (int)tb, wgt);
+                    }
+                }
+            }
         }
-        __syncwarp();
-        if (lane == 0) { c_written += fit; c_overflow += n - fit; }
+        // a16: survivors are ranked by warp ballot and stored straight from registers: one cursor
+        // atomic per call, consecutive 32 B records
+        const bool write = act && (run.write == C8PH_WRITE_ALL || (run.write == C8PH_WRITE_TEL && tel >= 0));
+        if (run.out.photons) {
+            const unsigned wm = __ballot_sync(FULL, write);
+            if (wm) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(&cntp[C8PH_CNT_WRITTEN], (unsigned long long)__popc(wm));
+                base = __shfl_sync(FULL, base, 0);
+                if (write) {
+                    const long long idx = (long long)base + __popc(wm & ((1u << lane) - 1u));
+                    if (idx < run.out.photon_capacity) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + idx);
+                        dst[0] = make_uint4(__float_as_uint(xg), __float_as_uint(yg), __float_as_uint(uax), __float_as_uint(uay));
+                        dst[1] = make_uint4(__float_as_uint(t_arr), __float_as_uint(__frcp_rn(lam_inv)), sc->local,
+                                            ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE));
+                        if (run.out.photon_weight) run.out.photon_weight[idx] = wgt;
+                    } else {
+                        atomicAdd(&s_cnt[warp][WC_OVERFLOW], 1ull);
+                    }
+                }
+            }
+        }
     };
-    int stage_head = 0;
+
+    // take up to 32 queued candidates (all of them if `all`) through finish()
+    auto drain = [&](bool all) {
+        __syncwarp();
+        int n = s_qn[warp];
+        while (n >= 32 || (all && n > 0)) {
+            const int take = n < 32 ? n : 32;
+            const float *e = s_q + ((q_head + lane) & (kQueue - 1));
+            const bool act = lane < take;
+            finish(act, e[Q_X * kQueue], e[Q_Y * kQueue], e[Q_UX * kQueue], e[Q_UY * kQueue], e[Q_UZ * kQueue],
+                   e[Q_T * kQueue], e[Q_LAMINV * kQueue], e[Q_WGT * kQueue], e[Q_ETA * kQueue], e[Q_H * kQueue],
+                   e[Q_DD * kQueue], e[Q_CZ * kQueue], __float_as_int(e[Q_CELL * kQueue]), __float_as_uint(e[Q_JSLOT * kQueue]));
+            q_head = (q_head + take) & (kQueue - 1);
+            n -= take;
+            __syncwarp();
+            if (lane == 0) s_qn[warp] = n;
+            __syncwarp();
+        }
+    };
 
     for (;;) {
         // ---- grab a group of segments for this warp
@@ -334,19 +446,21 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
         g0 = __shfl_sync(FULL, g0, 0);
         if ((long long)g0 >= run.n_seg) break;
 
-        // ---- a1-a4: one lane prepares one segment (fp64)
-        Seg me;
-        me.N = 0;
+        // ---- a1-a4: one lane prepares one segment (fp64) and parks it in its shared-memory slot
+        int myN = 0;
         {
             const long long i = (long long)g0 + lane;
+            bool below = false, lv1_drop = false, clipped = false;
             if (lane < run.segs_per_grab && i < run.n_seg) {
+                SegHot me;
+                SegCold mc;
                 const double Ax = run.seg.x[i], Ay = run.seg.y[i], Az = run.seg.z[i];
                 double Px = run.seg.dx[i], Py = run.seg.dy[i], Pz = run.seg.dz[i];
                 const double L = run.seg.len[i], beta = run.seg.beta[i], t0 = run.seg.t0[i];
                 const double pn = 1.0 / sqrt(Px * Px + Py * Py + Pz * Pz);
                 Px *= pn; Py *= pn; Pz *= pn;
                 const unsigned long long gid = (unsigned long long)(run.seg_id_base + i);
-                me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); me.local = (uint32_t)i;
+                me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); mc.local = (uint32_t)i;
                 // local vertical and height at A and at the midpoint
                 double rx = 0.0, ry = 0.0, rz = 1.0, rA = 1.0, hA, h_mid;
                 const double mx = Ax + 0.5 * L * Px, my = Ay + 0.5 * L * Py, mz = Az + 0.5 * L * Pz;
@@ -363,8 +477,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                 }
                 const double cA = Px * rx + Py * ry + Pz * rz;
                 double n_exp = 0.0;
-                bool lv1_drop = false;
                 const uint4 rs = philox4x32_10(0xFFFFFFFFu, me.id_lo, me.id_hi, 0u, run.key0, run.key1);
+                float e1x, e1y, e1z, e2x, e2y, e2z;
+                mc.aimx = mc.aimy = mc.aimz = mc.omc = 0.f;
                 if (EMIT == C8PH_EMIT_CHERENKOV) {
                     // Frank-Tamm, Eq. 2.2-2.4, n at the segment mid height
                     const double n_mid = 1.0 + eta_lookup_d(atm, h_mid);
@@ -385,13 +500,12 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                     const double Bx = Px, By = Py, Bz = Pz - 1.0;
                     const double b2 = Bx * Bx + By * By + Bz * Bz;
                     if (Pz > 1.0 - 1e-6 || b2 <= 0.0) {
-                        me.e1x = 1.f; me.e1y = 0.f; me.e1z = 0.f; me.e2x = 0.f; me.e2y = -1.f; me.e2z = 0.f;
+                        e1x = 1.f; e1y = 0.f; e1z = 0.f; e2x = 0.f; e2y = -1.f; e2z = 0.f;
                     } else {
                         const double k = 2.0 / b2;
-                        me.e1x = (float)(k * Bx * Bx - 1.0); me.e1y = (float)(k * Bx * By); me.e1z = (float)(k * Bx * Bz);
-                        me.e2x = (float)(k * By * Bx); me.e2y = (float)(k * By * By - 1.0); me.e2z = (float)(k * By * Bz);
+                        e1x = (float)(k * Bx * Bx - 1.0); e1y = (float)(k * Bx * By); e1z = (float)(k * Bx * Bz);
+                        e2x = (float)(k * By * Bx); e2y = (float)(k * By * By - 1.0); e2z = (float)(k * By * Bz);
                     }
-                    me.aimx = me.aimy = me.aimz = me.omc = 0.f;
                 } else {
                     // fluorescence: N = Y E_dep Omega/4pi, forced cone towards the pre-corrected aim point
                     const float4 t0v = __ldg(det.tel);
@@ -422,67 +536,83 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                             }
                         }
                     }
-                    me.aimx = (float)aimx; me.aimy = (float)aimy; me.aimz = t0v.z;
+                    mc.aimx = (float)aimx; mc.aimy = (float)aimy; mc.aimz = t0v.z;
                     const double rho = run.aim_factor * (double)t0v.w;
                     const double sp = fmin(1.0, rho / dist);
                     const double cps = sqrt(1.0 - sp * sp);
                     const double omc = sp * sp / (1.0 + cps);                 // 1 - cos(psi), cancellation-free
-                    me.omc = (float)omc;
+                    mc.omc = (float)omc;
                     const float *ed = run.seg.edep;
                     n_exp = run.fluor_yield * (ed ? (double)ed[i] : 0.0) * 0.5 * omc;
-                    me.e1x = me.e1y = me.e1z = me.e2x = me.e2y = me.e2z = 0.f;
+                    e1x = e1y = e1z = e2x = e2y = e2z = 0.f;
                 }
                 long long N = 0;
-                if (!(n_exp > 0.0)) c_below++;
-                else if (lv1_drop) c_lv1++;
-                else {
+                if (!(n_exp > 0.0)) below = true;
+                else if (!lv1_drop) {
                     N = (long long)floor(n_exp / (double)run.w + u01d(rs.x));
-                    if (N >= C8PH_MAX_BUNCHES_PER_SEGMENT) { c_clipped += 1; N = C8PH_MAX_BUNCHES_PER_SEGMENT - 1; }
-                    if (N > 0) c_emitting++;
+                    if (N >= C8PH_MAX_BUNCHES_PER_SEGMENT) { clipped = true; N = C8PH_MAX_BUNCHES_PER_SEGMENT - 1; }
                 }
-                me.N = (int)N;
-                me.Px = (float)Px; me.Py = (float)Py; me.Pz = (float)Pz;
-                me.Ax = (float)Ax; me.Ay = (float)Ay; me.Az = (float)Az;
-                me.L = (float)L; me.beta = (float)beta; me.delta = 1.0f - (float)beta;
-                me.hA = (float)hA; me.cA = (float)cA; me.k2 = SPH ? (float)((1.0 - cA * cA) / (2.0 * rA)) : 0.f;
-                me.rx = (float)rx; me.ry = (float)ry; me.rz = (float)rz; me.inv_rA = SPH ? (float)(1.0 / rA) : 0.f;
-                me.a1 = me.e1x * me.rx + me.e1y * me.ry + me.e1z * me.rz;
-                me.a2 = me.e2x * me.rx + me.e2y * me.ry + me.e2z * me.rz;
-                // axis landing anchor (fp64): G = A - A_z P / P_z, its clock, its grid coordinate
-                me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
-                me.Gx = me.Gy = me.fbx = me.fby = me.AzP = 0.f; me.ibx = me.iby = 0;
-                if (me.anchor) {
-                    const double azp = Az / Pz;
-                    const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
-                    me.Gx = (float)Gx; me.Gy = (float)Gy; me.AzP = (float)azp;
-                    me.Tg = (float)(t0 - azp / kC - det.t_ref);
-                    if (has_grid_geom) {
-                        const double bx = (Gx - (double)det.hist_x0) / (double)det.hist_cell;
-                        const double by = (Gy - (double)det.hist_y0) / (double)det.hist_cell;
-                        const double fx = fmin(fmax(floor(bx), -1.0e9), 1.0e9), fy = fmin(fmax(floor(by), -1.0e9), 1.0e9);
-                        me.ibx = (int)fx; me.iby = (int)fy;
-                        me.fbx = (float)(bx - fx); me.fby = (float)(by - fy);
+                myN = (int)N;
+                if (myN > 0) {
+                    me.N = myN;
+                    me.Px = (float)Px; me.Py = (float)Py; me.Pz = (float)Pz;
+                    me.e1x = e1x; me.e1y = e1y; me.e1z = e1z; me.e2x = e2x; me.e2y = e2y; me.e2z = e2z;
+                    mc.Ax = (float)Ax; mc.Ay = (float)Ay; me.Az = (float)Az;
+                    me.L = (float)L; me.beta = (float)beta; me.delta = 1.0f - (float)beta;
+                    me.hA = (float)hA; me.cA = (float)cA; me.k2 = SPH ? (float)((1.0 - cA * cA) / (2.0 * rA)) : 0.f;
+                    mc.rx = (float)rx; mc.ry = (float)ry; mc.rz = (float)rz; me.inv_rA = SPH ? (float)(1.0 / rA) : 0.f;
+                    me.a1 = e1x * mc.rx + e1y * mc.ry + e1z * mc.rz;
+                    me.a2 = e2x * mc.rx + e2y * mc.ry + e2z * mc.rz;
+                    // axis landing anchor (fp64): G = A - A_z P / P_z, its clock, its grid coordinate
+                    me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
+                    me.Gx = me.Gy = me.AzP = 0.f;
+                    mc.fbx = mc.fby = 0.f; mc.ibx = mc.iby = 0;
+                    mc.pad0 = me.pad0 = me.pad1 = 0.f;
+                    if (me.anchor) {
+                        const double azp = Az / Pz;
+                        const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
+                        me.Gx = (float)Gx; me.Gy = (float)Gy; me.AzP = (float)azp;
+                        mc.Tg = (float)(t0 - azp / kC - det.t_ref);
+                        if (has_grid_geom) {
+                            const double bx = (Gx - (double)det.hist_x0) / (double)det.hist_cell;
+                            const double by = (Gy - (double)det.hist_y0) / (double)det.hist_cell;
+                            const double fx = fmin(fmax(floor(bx), -1.0e9), 1.0e9), fy = fmin(fmax(floor(by), -1.0e9), 1.0e9);
+                            mc.ibx = (int)fx; mc.iby = (int)fy;
+                            mc.fbx = (float)(bx - fx); mc.fby = (float)(by - fy);
+                        }
+                    } else {
+                        mc.Tg = (float)(t0 - det.t_ref);
                     }
-                } else {
-                    me.Tg = (float)(t0 - det.t_ref);
+                    copy16(g_hot + lane, &me);
+                    copy16(g_cold + lane, &mc);
                 }
             }
+            // segment-level counters of the group: one ballot each, lane 0 books them
+            const unsigned mb = __ballot_sync(FULL, below), ml = __ballot_sync(FULL, lv1_drop), mcl = __ballot_sync(FULL, clipped);
+            const unsigned me_ = __ballot_sync(FULL, myN > 0);
+            const uint32_t nsum = __reduce_add_sync(FULL, (uint32_t)myN);
+            if (lane == 0) {
+                s_cnt[warp][WC_BELOW] += __popc(mb); s_cnt[warp][WC_LV1] += __popc(ml);
+                s_cnt[warp][WC_CLIPPED] += __popc(mcl); s_cnt[warp][WC_EMITTING] += __popc(me_);
+                s_cnt[warp][WC_EMITTED] += nsum;
+            }
         }
-        unsigned emask = __ballot_sync(FULL, me.N > 0);
+        unsigned emask = __ballot_sync(FULL, myN > 0);
+        __syncwarp();
 
         // ---- a5-a16: the warp walks the emitting segments; lanes stride over the photons
         while (emask) {
             const int src = __ffs(emask) - 1;
             emask &= emask - 1;
-            const Seg sg = shfl_seg(me, src);
-            if (lane == 0) c_emitted += (unsigned long long)sg.N;
+            SegHot sg;
+            copy16(&sg, g_hot + src);                                 // uniform address: one sector per LDG.128
+            const SegCold *sc = g_cold + src;                         // cold fields are re-read (L1) where used
             const int n_iter = (sg.N + 31) >> 5;
+            if (iters_pending + n_iter > 60000) flush_counts();
+            iters_pending += n_iter;
             for (int it = 0; it < n_iter; ++it) {
                 const int j = it * 32 + lane;
                 bool alive = j < sg.N;
-                bool write = false;
-                c8ph_photon rec;
-                float rec_w = 0.f;
                 if (alive) {
                     const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, run.key0, run.key1);
                     const float u0 = u01(rn.x), u1 = u01(rn.y), u2 = u01(rn.z), u3 = u01(rn.w);
@@ -494,7 +624,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                         float f = (h_e - atm.h0) * atm.inv_dh;
                         f = fminf(fmaxf(f, 0.f), (float)(atm.n_nodes - 1));
                         const int k = min((int)f, atm.n_nodes - 2);
-                        const float e0 = s_eta[k], e1 = s_eta[k + 1];
+                        const float e0 = eta_node(k), e1 = eta_node(k + 1);
                         eta_e = fmaf(f - (float)k, e1 - e0, e0);
                     }
                     float ux, uy, uz, lam_inv, cth = 1.f, q = 0.f, pqz = 0.f, wx = 0.f, wy = 0.f, wz = 0.f;
@@ -519,25 +649,25 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                         while (li < run.n_lines - 1 && u2 >= __ldg(run.line_cdf + li)) ++li;
                         lam_inv = 1.0f / __ldg(run.line_nm + li);
                         const uint4 rb = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 1u, run.key0, run.key1);
-                        const float xe = fmaf(s, sg.Px, sg.Ax), ye = fmaf(s, sg.Py, sg.Ay), ze = fmaf(s, sg.Pz, sg.Az);
-                        float ax = sg.aimx - xe, ay = sg.aimy - ye, az = sg.aimz - ze;
+                        const float xe = fmaf(s, sg.Px, sc->Ax), ye = fmaf(s, sg.Py, sc->Ay), ze = fmaf(s, sg.Pz, sg.Az);
+                        float ax = sc->aimx - xe, ay = sc->aimy - ye, az = sc->aimz - ze;
                         const float an = rsqrtf(ax * ax + ay * ay + az * az);
                         ax *= an; ay *= an; az *= an;
-                        const float tt = u01(rb.x) * sg.omc;             // 1 - cos(polar)
-                        const float cp = 1.f - tt, sp = sqrtf(tt * (2.f - tt));
+                        const float tt = u01(rb.x) * sc->omc;            // 1 - cos(polar)
+                        const float cp = 1.f - tt, sp2 = sqrtf(tt * (2.f - tt));
                         float e1x = ay, e1y = -ax;
                         float e1n = e1x * e1x + e1y * e1y;
                         if (e1n < 1e-24f) { e1x = 1.f; e1y = 0.f; e1n = 1.f; }
                         const float ie = rsqrtf(e1n);
                         e1x *= ie; e1y *= ie;
                         const float e2x = -az * e1y, e2y = az * e1x, e2z = ax * e1y - ay * e1x;
-                        ux = cp * ax + sp * (cphi * e1x + sphi * e2x);
-                        uy = cp * ay + sp * (cphi * e1y + sphi * e2y);
-                        uz = cp * az + sp * (sphi * e2z);
+                        ux = cp * ax + sp2 * (cphi * e1x + sphi * e2x);
+                        uy = cp * ay + sp2 * (cphi * e1y + sphi * e2y);
+                        uz = cp * az + sp2 * (sphi * e2z);
                     }
                     // a8: up-going / horizontal photons are discarded
-                    if (uz >= kUpCut) { alive = false; cnt.up++; }
-                    float xl = 0.f, yl = 0.f, ox = 0.f, oy = 0.f, D = 0.f, inv_uz = 0.f, tx_l = 0.f, ty_l = 0.f;
+                    if (uz >= kUpCut) { alive = false; pkA += 1u; }
+                    float xl = 0.f, yl = 0.f, ox = 0.f, oy = 0.f, D = 0.f, inv_uz = 0.f;
                     if (alive) {
                         // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
                         inv_uz = __frcp_rn(uz);
@@ -550,25 +680,30 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                             xl = sg.Gx + ox;
                             yl = sg.Gy + oy;
                         } else {
-                            xl = fmaf(D, ux, fmaf(s, sg.Px, sg.Ax));
-                            yl = fmaf(D, uy, fmaf(s, sg.Py, sg.Ay));
+                            xl = fmaf(D, ux, fmaf(s, sg.Px, sc->Ax));
+                            yl = fmaf(D, uy, fmaf(s, sg.Py, sc->Ay));
                         }
-                        // a10: LV2/LV3 on the straight-line point, before the correction
+                        // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
+                        // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
                         if (run.lv2) {
-                            const float m = run.lv2_margin;
-                            bool keep = has_grid_geom && xl >= det.hist_x0 - m && xl < hx1 + m && yl >= det.hist_y0 - m && yl < hy1 + m;
-                            if (!keep && det.n_tel > 0)
-                                keep = tel_near(det, xl, yl, -inv_uz, m, !det.use_grid || -uz < det.grid_min_cos);
-                            if (!keep) { alive = false; cnt.lv2++; }
+                            bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
+                            if (!keep && det.n_tel > 0) {
+                                const bool brute = !det.use_grid || -uz < det.grid_min_cos;
+                                const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
+                                const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
+                                if (cell < -1 || (cell >= 0 && __ldg(det.lv2.kmin + cell) <= thr))
+                                    keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
+                            }
+                            if (!keep) { alive = false; pkA += 0x10000u; }
                         }
                     }
-                    float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz = 1.f, sinz = 0.f, delta_arr = 0.f;
+                    float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz = 1.f, sinz = 0.f;
                     if (alive) {
                         // local zenith angle of the photon at the emission point
                         if (SPH) {
                             float ur;
                             if (EMIT == C8PH_EMIT_CHERENKOV) ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
-                            else ur = ux * sg.rx + uy * sg.ry + uz * sg.rz;
+                            else ur = ux * sc->rx + uy * sc->ry + uz * sc->rz;
                             const float sr = s * sg.inv_rA;
                             const float uP = (EMIT == C8PH_EMIT_CHERENKOV) ? cth : (ux * sg.Px + uy * sg.Py + uz * sg.Pz);
                             cz = -(fmaf(-sr * sg.cA, ur, ur) + sr * uP);
@@ -582,7 +717,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                             dt = eta_e * D * kInvC;                      // homogeneous: t = t_e + n D / c
                         } else if (TRACE == C8PH_TRACE_TABLE) {
                             const TabVal v = table_lookup(a.tab, h_e, acosf(cz));
-                            if (v.bad || !(cz > 0.f)) { alive = false; cnt.tr++; }
+                            if (v.bad || !(cz > 0.f)) { alive = false; pkB += 1u; }
                             dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
                         } else {
                             // layered Snell sum (Eq. 3.15 in its invariant form K = n sin(theta)),
@@ -616,11 +751,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                                 for (int k = ke - 1; k > kg; --k) layer(s_mid[k], atm.dh, s_dxv[k]);
                                 layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
                             }
-                            if (!ok) { alive = false; cnt.tr++; }
+                            if (!ok) { alive = false; pkB += 1u; }
                             dd = aX; dt = aT * kInvC; Xs = aS;
                         }
                     }
-                    float T = 1.f, wgt = run.w;
+                    float wgt = run.w;
                     if (alive && run.trans != C8PH_TRANS_OFF) {
                         // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
                         float tau = 0.f;
@@ -630,9 +765,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                             tau = Xs * qq * atm.ray_inv_X;
                         }
                         if (atm.aer_L > 0.f) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
-                        T = __expf(-tau);
+                        const float T = __expf(-tau);
                         if (run.trans == C8PH_TRANS_ROULETTE) {
-                            if (!(u3 < T)) { alive = false; cnt.roul++; }
+                            if (!(u3 < T)) { alive = false; pkB += 0x10000u; }
                         } else wgt = run.w * T;
                     }
                     if (alive) {
@@ -644,137 +779,91 @@ __global__ void __launch_bounds__(kThreads, 2) k_emit_propagate(const __grid_con
                         float xg, yg;
                         if (sg.anchor) { xg = sg.Gx + cx; yg = sg.Gy + cy; }
                         else { xg = fmaf(dd, ehx, xl); yg = fmaf(dd, ehy, yl); }
-                        // a13: arrival time relative to t_ref
-                        float t_arr;
-                        if (sg.anchor) {
-                            // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
-                            const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
-                            const float num = fmaf(q, wz, -bn1 * sg.Pz);
-                            const float geo = (s + sg.AzP) * num * __frcp_rn(pqz);
-                            t_arr = sg.Tg + fmaf(fmaf(s, sg.delta / sg.beta, geo), kInvC, dt);
-                        } else {
-                            t_arr = sg.Tg + fmaf(s / sg.beta + D, kInvC, dt);
-                        }
                         // a15: ground grid
-                        int bin = -1;
                         if (has_grid_geom) {
                             int ix, iy;
                             if (sg.anchor) {
-                                ix = sg.ibx + (int)floorf(fmaf(cx, det.hist_inv_cell, sg.fbx));
-                                iy = sg.iby + (int)floorf(fmaf(cy, det.hist_inv_cell, sg.fby));
+                                ix = sc->ibx + __float2int_rd(fmaf(cx, det.hist_inv_cell, sc->fbx));
+                                iy = sc->iby + __float2int_rd(fmaf(cy, det.hist_inv_cell, sc->fby));
                             } else {
-                                ix = (int)floorf((xg - det.hist_x0) * det.hist_inv_cell);
-                                iy = (int)floorf((yg - det.hist_y0) * det.hist_inv_cell);
+                                ix = __float2int_rd((xg - det.hist_x0) * det.hist_inv_cell);
+                                iy = __float2int_rd((yg - det.hist_y0) * det.hist_inv_cell);
                             }
-                            if (ix >= 0 && ix < det.hist_nx && iy >= 0 && iy < det.hist_ny) {
-                                bin = iy * det.hist_nx + ix;
-                                cnt.grid++;
-                                if (has_hist) atomicAdd(run.out.hist + bin, wgt);
+                            if ((unsigned)ix < (unsigned)det.hist_nx && (unsigned)iy < (unsigned)det.hist_ny) {
+                                pkC += 1u;
+                                if (has_hist) atomicAdd(run.out.hist + (iy * det.hist_nx + ix), wgt);
                             }
                         }
-                        // arrival direction: rotation by delta in the ray plane (Snell / Bouguer invariant)
-                        float uax = ux, uay = uy, uaz = uz;
-                        auto arrival_direction = [&]() {
-                            if (TRACE == C8PH_TRACE_STRAIGHT || sinz < 1e-6f) return;
-                            const float eps = (eta_e - atm.eta_g) * inv_ng;
-                            const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * (float)(1.0 / atm.Rg) : 1.f;
-                            const float al = sinz * scale;
-                            const float cyy = sqrtf(fmaxf(1.f - al * al, 0.f));
-                            const float at = al * (1.f + eps);
-                            const float cxx = sqrtf(fmaxf(1.f - at * at, 0.f));
-                            float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * __frcp_rn(cyy + cxx));
-                            if (SPH) dl -= dd * (float)(1.0 / atm.Rg);
-                            delta_arr = dl;
-                            const float k1 = 1.f - 0.5f * dl * dl + dl * cz / sinz, k2 = dl / sinz;
-                            uax = fmaf(k1, ux, k2 * sg.rx);
-                            uay = fmaf(k1, uy, k2 * sg.ry);
-                            uaz = fmaf(k1, uz, k2 * sg.rz);
-                        };
-                        // a14: telescope spheres, only if a candidate list is non-empty
-                        int tel = -1;
-                        bool dir_done = false;
+                        // a14: telescope spheres.  Pre-test on the sorted grid: the photon can
+                        // hit a sphere of its cell only if the cell's smallest key <= 1/|u_z| (inflated
+                        // for the refraction rotation of the direction); everything else skips the
+                        // arrival-direction arithmetic unless the record is written anyway.
+                        int cell = -1;
+                        bool cand = false;
                         if (det.n_tel > 0) {
-                            arrival_direction();
-                            dir_done = true;
-                            const bool brute = !det.use_grid || -uaz < det.grid_min_cos;
-                            tel = tel_hit_cell(det, det.hit, xg, yg, uax, uay, uaz, brute);
-                            if (tel >= 0) {
-                                cnt.tel++;
-                                if (run.out.tel_counts) atomicAdd(run.out.tel_counts + tel, wgt);
-                                if (det.cam_enabled) {
-                                    const int pix = camera_pixel(det, uax, uay, uaz);
-                                    const float tb = floorf(t_arr * det.inv_t_bin);
-                                    if (pix >= 0 && tb >= 0.f && tb < (float)det.n_tbins) {
-                                        cnt.cam++;
-                                        if (run.out.hist) atomicAdd(run.out.hist + (size_t)pix * det.n_tbins + (int)tb, wgt);
-                                    }
-                                }
+                            const bool brute = run.hit_brute || !det.use_grid || -uz < det.grid_min_cos;
+                            cell = brute ? -2 : grid_cell(det.hit, xg, yg);
+                            cand = cell < -1 || (cell >= 0 && __ldg(det.hit.kmin + cell) <= -inv_uz * run.hit_infl);
+                            if (!cand) cell = -1;
+                        }
+                        if (cand || run.write == C8PH_WRITE_ALL) {
+                            // a13: arrival time relative to t_ref
+                            float t_arr;
+                            if (sg.anchor) {
+                                // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
+                                const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
+                                const float num = fmaf(q, wz, -bn1 * sg.Pz);
+                                const float geo = (s + sg.AzP) * num * __frcp_rn(pqz);
+                                t_arr = sc->Tg + fmaf(fmaf(s, sg.delta / sg.beta, geo), kInvC, dt);
+                            } else {
+                                t_arr = sc->Tg + fmaf(s / sg.beta + D, kInvC, dt);
                             }
-                        }
-                        write = run.write == C8PH_WRITE_ALL || (run.write == C8PH_WRITE_TEL && tel >= 0);
-                        if (write) {
-                            if (!dir_done) arrival_direction();
-                            rec.x = xg; rec.y = yg; rec.ux = uax; rec.uy = uay;
-                            rec.t_ns = t_arr;
-                            rec.lambda_nm = __frcp_rn(lam_inv);
-                            rec.seg = sg.local;
-                            rec.j_tel = ((uint32_t)j << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE);
-                            rec_w = wgt;
-                        }
-                        (void)delta_arr; (void)tx_l; (void)ty_l; (void)T;
-                    }
-                }
-                // a16: warp-ballot compaction into the per-warp stage, flushed 32 records at a time
-                if (run.out.photons) {
-                    const unsigned wm = __ballot_sync(FULL, write);
-                    if (wm) {
-                        if (write) {
-                            const int slot = (stage_head + stage_fill + __popc(wm & ((1u << lane) - 1u))) & (kStage - 1);
-                            s_rec[slot] = rec;
-                            s_wgt[slot] = rec_w;
-                        }
-                        stage_fill += __popc(wm);
-                        __syncwarp();
-                        if (stage_fill >= 32) {
-                            flush(stage_head, 32);
-                            stage_head = (stage_head + 32) & (kStage - 1);
-                            stage_fill -= 32;
+                            // queue the photon for finish(): slots are handed out per group of lanes
+                            // that arrive here together (one shared-memory atomic per group)
+                            const unsigned am = __activemask();
+                            const int leader = __ffs(am) - 1;
+                            int qb = 0;
+                            if (lane == leader) qb = atomicAdd(&s_qn[warp], __popc(am));
+                            qb = __shfl_sync(am, qb, leader);
+                            float *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1));
+                            e[Q_X * kQueue] = xg; e[Q_Y * kQueue] = yg;
+                            e[Q_UX * kQueue] = ux; e[Q_UY * kQueue] = uy; e[Q_UZ * kQueue] = uz;
+                            e[Q_T * kQueue] = t_arr; e[Q_LAMINV * kQueue] = lam_inv; e[Q_WGT * kQueue] = wgt;
+                            e[Q_ETA * kQueue] = eta_e; e[Q_H * kQueue] = h_e; e[Q_DD * kQueue] = dd; e[Q_CZ * kQueue] = cz;
+                            e[Q_CELL * kQueue] = __int_as_float(cell);
+                            e[Q_JSLOT * kQueue] = __uint_as_float(((uint32_t)j << 5) | (uint32_t)src);
                         }
                     }
                 }
+                // a14/a16: once 32 candidates wait, a full warp takes them through finish()
+                drain(false);
             }
         }
+        drain(true);                                                  // slots are rewritten by the next group
     }
-    if (run.out.photons && stage_fill > 0) flush(stage_head, stage_fill);
+    flush_counts();
+    __syncwarp();
 
-    // ---- counters: warp reduction, one atomic per warp and counter
-    auto add = [&](int idx, uint32_t v) {
-        v = __reduce_add_sync(FULL, v);
-        if (lane == 0 && v) atomicAdd(&cntp[idx], (unsigned long long)v);
-    };
-    if (run.out.counters) {
-        if (blockIdx.x == 0 && threadIdx.x == 0)
-            atomicAdd(&cntp[C8PH_CNT_SEGMENTS], (unsigned long long)run.n_seg);
-        add(C8PH_CNT_SEG_BELOW_THRESHOLD, c_below);
-        add(C8PH_CNT_SEG_LV1, c_lv1);
-        add(C8PH_CNT_SEG_EMITTING, c_emitting);
-        add(C8PH_CNT_CLIPPED, c_clipped);
-        add(C8PH_CNT_UPGOING, cnt.up);
-        add(C8PH_CNT_LV2, cnt.lv2);
-        add(C8PH_CNT_TABLE_RANGE, cnt.tr);
-        add(C8PH_CNT_ROULETTE, cnt.roul);
-        add(C8PH_CNT_IN_GRID, cnt.grid);
-        add(C8PH_CNT_TEL_HIT, cnt.tel);
-        add(C8PH_CNT_CAM_HIT, cnt.cam);
-        add(C8PH_CNT_OVERFLOW, c_overflow);
-        const uint32_t drops = __reduce_add_sync(FULL, cnt.up + cnt.lv2 + cnt.tr + cnt.roul);
-        if (lane == 0) {
-            if (c_emitted) atomicAdd(&cntp[C8PH_CNT_EMITTED], c_emitted);
-            // landed = emitted - drops, accumulated as two's-complement u64 pieces
-            atomicAdd(&cntp[C8PH_CNT_LANDED], c_emitted - (unsigned long long)drops);
-        }
+    // ---- counters: one global atomic per warp and non-zero counter
+    if (run.out.counters && lane == 0) {
+        const unsigned long long *c = s_cnt[warp];
+        auto add = [&](int idx, unsigned long long v) { if (v) atomicAdd(&cntp[idx], v); };
+        if (blockIdx.x == 0 && warp == 0) add(C8PH_CNT_SEGMENTS, (unsigned long long)run.n_seg);
+        add(C8PH_CNT_SEG_BELOW_THRESHOLD, c[WC_BELOW]);
+        add(C8PH_CNT_SEG_LV1, c[WC_LV1]);
+        add(C8PH_CNT_SEG_EMITTING, c[WC_EMITTING]);
+        add(C8PH_CNT_CLIPPED, c[WC_CLIPPED]);
+        add(C8PH_CNT_EMITTED, c[WC_EMITTED]);
+        add(C8PH_CNT_UPGOING, c[WC_UP]);
+        add(C8PH_CNT_LV2, c[WC_LV2]);
+        add(C8PH_CNT_TABLE_RANGE, c[WC_TR]);
+        add(C8PH_CNT_ROULETTE, c[WC_ROUL]);
+        add(C8PH_CNT_IN_GRID, c[WC_GRID]);
+        add(C8PH_CNT_TEL_HIT, c[WC_TEL]);
+        add(C8PH_CNT_CAM_HIT, c[WC_CAM]);
+        add(C8PH_CNT_OVERFLOW, c[WC_OVERFLOW]);
+        add(C8PH_CNT_LANDED, c[WC_EMITTED] - c[WC_UP] - c[WC_LV2] - c[WC_TR] - c[WC_ROUL]);
     }
-    (void)c_written;
 }
 
 // ================================================================================================
@@ -885,6 +974,7 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
     if (per_sm < 1) per_sm = 1;
     long long warps_needed = (a.run.n_seg + a.run.segs_per_grab - 1) / a.run.segs_per_grab;
     long long blocks = (warps_needed + kWarps - 1) / kWarps;
+    if (per_sm > kMaxBlocksPerSM) per_sm = kMaxBlocksPerSM;         // the segment-slot scratch is sized for this
     const long long max_blocks = (long long)n_sm * per_sm;          // persistent: one resident wave
     if (blocks > max_blocks) blocks = max_blocks;
     if (blocks < 1) blocks = 1;
@@ -894,10 +984,21 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
 
 }  // namespace
 
+size_t segment_slot_bytes(int n_sm)
+{
+    return (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32 * (sizeof(SegHot) + sizeof(SegCold));
+}
+
+void segment_slot_pointers(void *base, int n_sm, DevRun &run)
+{
+    run.slots_hot = base;
+    run.slots_cold = static_cast<SegHot *>(base) + (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32;
+}
+
 size_t emit_smem_bytes(const KArgs &a)
 {
-    const size_t tables = (size_t)a.atm.n_pad * 4u * (a.run.trace == C8PH_TRACE_NUMERIC ? 3u : 1u);
-    return tables + (size_t)kWarps * kStage * (sizeof(c8ph_photon) + sizeof(float));
+    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * 3u : 0u;
+    return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
