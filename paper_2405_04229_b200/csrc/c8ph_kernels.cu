@@ -116,7 +116,7 @@ struct alignas(16) SegHot {                       // 28 words = 7 x 16 B
     float a1, a2, inv_rA;                             // e1.r, e2.r, 1/|A - C|
     uint32_t id_lo, id_hi;                            // global segment id (Philox counter words)
     int N, anchor;                                    // bunches to emit; 1: anchor form valid
-    float pad0, pad1;
+    float dob, inv_beta;                              // (1 - beta)/beta, 1/beta (read from the slot, not kept in registers)
 };
 struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
     float fbx, fby;                                   // fractional grid coordinate of the anchor
@@ -153,8 +153,72 @@ __device__ __forceinline__ double eta_lookup_d(const DevAtm &atm, double h)
     return (1.0 - fr) * (double)__ldg(atm.eta + k) + fr * (double)__ldg(atm.eta + k + 1);
 }
 
+// ---- single-instruction special functions (MUFU, max relative error 2^-23; PTX ISA "rcp.approx",
+// "sqrt.approx", "rsqrt.approx").  The IEEE versions add a range check, a branch and a Newton step
+// per call; one ulp more on these quantities is far inside the parity budget.
+__device__ __forceinline__ float rcp_fast(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float sqrt_fast(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rsqrt_fast(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// acos(x) for x in [0,1]: sqrt(1-x) * p6(x) (least-squares fit on Chebyshev nodes, max error
+// 3.3e-7 rad in fp32 = 5e-5 of a zenith cell of the correction table)
+__device__ __forceinline__ float acos01(float x)
+{
+    float p = 0.002251368248835206f;
+    p = fmaf(p, x, -0.011012386530637741f);
+    p = fmaf(p, x, 0.02674933150410652f);
+    p = fmaf(p, x, -0.048724401742219925f);
+    p = fmaf(p, x, 0.08873733133077621f);
+    p = fmaf(p, x, -0.21458369493484497f);
+    p = fmaf(p, x, 1.5707961320877075f);
+    return sqrt_fast(1.f - x) * p;
+}
+
+// sin and cos of phi = 2 pi u, u = (2m+1) 2^-24 with m = r >> 9 the uniform's 23 mantissa bits
+// (a6: azimuth on the cone).  Octant from the top three bits of m, the remaining 20 bits give the
+// angle a in (0, pi/4) exactly (odd octants reflected), degree-7/8 polynomials in a (max error
+// 7e-8), then swap / sign by octant.
+__device__ __forceinline__ void sincos_2pi_u(uint32_t r, float &sphi, float &cphi)
+{
+    const uint32_t m = r >> 9, o = m >> 20;
+    uint32_t ml = m & 0xFFFFFu;
+    if (o & 1u) ml ^= 0xFFFFFu;
+    const float a = (float)(int)(2u * ml + 1u) * 3.7450702829e-07f;        // pi / 2^23
+    const float z = a * a;
+    float sp = -0.0001958794891834259f;
+    sp = fmaf(sp, z, 0.008332748897373676f);
+    sp = fmaf(sp, z, -0.166666641831398f);
+    const float sv = fmaf(a * z, sp, a);
+    float cp = 2.4463915906380862e-05f;
+    cp = fmaf(cp, z, -0.001388759003020823f);
+    cp = fmaf(cp, z, 0.04166664928197861f);
+    cp = fmaf(cp, z, -0.5f);
+    const float cv = fmaf(z, cp, 1.f);
+    const bool swap = ((o + 1u) & 2u) != 0u;
+    const float s0 = swap ? cv : sv, c0 = swap ? sv : cv;
+    sphi = __uint_as_float(__float_as_uint(s0) ^ ((o & 4u) << 29));
+    cphi = __uint_as_float(__float_as_uint(c0) ^ (((o + 2u) & 4u) << 29));
+}
+
 struct TabVal { float dd, dt, X, ta; bool bad; };
 
+// bilinear lookup in the correction table (linear interpolation between support points):
+// four LDG.128 texels (dd, dt, X_slant, tau_aer); indices clamped; out of range / no-ground -> bad
 __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float thz)
 {
     TabVal o;
@@ -163,13 +227,14 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
     const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), (float)(t.n_zen - 1));
     const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
     const float ff = f - (float)ia, gg = g - (float)ib;
-    const float4 *p = t.hot + (size_t)ia * t.n_zen + ib;
-    const float4 v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + t.n_zen), v11 = __ldg(p + t.n_zen + 1);
-    const float w00 = (1.f - ff) * (1.f - gg), w01 = (1.f - ff) * gg, w10 = ff * (1.f - gg), w11 = ff * gg;
-    o.dd = w00 * v00.x + w01 * v01.x + w10 * v10.x + w11 * v11.x;
-    o.dt = w00 * v00.y + w01 * v01.y + w10 * v10.y + w11 * v11.y;
-    o.X = w00 * v00.z + w01 * v01.z + w10 * v10.z + w11 * v11.z;
-    o.ta = w00 * v00.w + w01 * v01.w + w10 * v10.w + w11 * v11.w;
+    const float4 *p = t.hot + (unsigned)(ia * t.n_zen + ib);
+    const float4 *p1 = p + (unsigned)t.n_zen;
+    const float4 v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p1), v11 = __ldg(p1 + 1);
+    const float w11 = ff * gg, w10 = ff - w11, w01 = gg - w11, w00 = (1.f - ff) - w01;
+    o.dd = fmaf(w11, v11.x, fmaf(w10, v10.x, fmaf(w01, v01.x, w00 * v00.x)));
+    o.dt = fmaf(w11, v11.y, fmaf(w10, v10.y, fmaf(w01, v01.y, w00 * v00.y)));
+    o.X = fmaf(w11, v11.z, fmaf(w10, v10.z, fmaf(w01, v01.z, w00 * v00.z)));
+    o.ta = fmaf(w11, v11.w, fmaf(w10, v10.w, fmaf(w01, v01.w, w00 * v00.w)));
     o.bad = o.bad || (o.dd != o.dd);
     return o;
 }
@@ -360,17 +425,17 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         float uax = ux, uay = uy, uaz = uz;
         const SegCold *sc = g_cold + (jslot & 31u);
         if (act) {
-            const float sinz = sqrtf(fmaxf(1.f - cz * cz, 0.f));
+            const float sinz = sqrt_fast(fmaxf(1.f - cz * cz, 0.f));
             if (TRACE != C8PH_TRACE_STRAIGHT && sinz >= 1e-6f) {
                 const float eps = (eta_e - atm.eta_g) * inv_ng;
                 const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * run.inv_Rg : 1.f;
                 const float al = sinz * scale;
-                const float cyy = sqrtf(fmaxf(1.f - al * al, 0.f));
+                const float cyy = sqrt_fast(fmaxf(1.f - al * al, 0.f));
                 const float at = al * (1.f + eps);
-                const float cxx = sqrtf(fmaxf(1.f - at * at, 0.f));
-                float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * __frcp_rn(cyy + cxx));
+                const float cxx = sqrt_fast(fmaxf(1.f - at * at, 0.f));
+                float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * rcp_fast(cyy + cxx));
                 if (SPH) dl -= dd * run.inv_Rg;
-                const float k1 = 1.f - 0.5f * dl * dl + dl * cz / sinz, k2 = dl / sinz;
+                const float k2 = dl * rcp_fast(sinz), k1 = fmaf(k2, cz, fmaf(-0.5f * dl, dl, 1.f));
                 uax = fmaf(k1, ux, k2 * sc->rx);
                 uay = fmaf(k1, uy, k2 * sc->ry);
                 uaz = fmaf(k1, uz, k2 * sc->rz);
@@ -378,7 +443,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             if (det.n_tel > 0 && cell != -1) {
                 // the pre-test threshold must cover the rotated direction; if it does not (never in
                 // air), search all telescopes
-                const float thr = -__frcp_rn(uz) * run.hit_infl;
+                const float thr = -rcp_fast(uz) * run.hit_infl;
                 if (cell >= 0 && !(-uaz * thr >= 1.f)) cell = -2;
                 tel = tel_hit_search(det, cell, thr, xg, yg, uax, uay, uaz);
             }
@@ -409,7 +474,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (idx < run.out.photon_capacity) {
                         uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + idx);
                         dst[0] = make_uint4(__float_as_uint(xg), __float_as_uint(yg), __float_as_uint(uax), __float_as_uint(uay));
-                        dst[1] = make_uint4(__float_as_uint(t_arr), __float_as_uint(__frcp_rn(lam_inv)), sc->local,
+                        dst[1] = make_uint4(__float_as_uint(t_arr), __float_as_uint(rcp_fast(lam_inv)), sc->local,
                                             ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE));
                         if (run.out.photon_weight) run.out.photon_weight[idx] = wgt;
                     } else {
@@ -567,7 +632,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
                     me.Gx = me.Gy = me.AzP = 0.f;
                     mc.fbx = mc.fby = 0.f; mc.ibx = mc.iby = 0;
-                    mc.pad0 = me.pad0 = me.pad1 = 0.f;
+                    mc.pad0 = 0.f;
+                    me.dob = (float)((double)me.delta / beta); me.inv_beta = (float)(1.0 / beta);
                     if (me.anchor) {
                         const double azp = Az / Pz;
                         const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
@@ -612,10 +678,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             iters_pending += n_iter;
             for (int it = 0; it < n_iter; ++it) {
                 const int j = it * 32 + lane;
-                bool alive = j < sg.N;
-                if (alive) {
+                // one photon per lane; every cut leaves through the same exit (one reconvergence point)
+                if (j < sg.N) do {
                     const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, run.key0, run.key1);
-                    const float u0 = u01(rn.x), u1 = u01(rn.y), u2 = u01(rn.z), u3 = u01(rn.w);
+                    const float u1 = u01(rn.y), u2 = u01(rn.z);
                     // a6: emission point on the track, its height and n(h_e) (Listing 4.1)
                     const float s = u1 * sg.L;
                     const float h_e = fmaf(s, fmaf(s, sg.k2, sg.cA), sg.hA);
@@ -629,12 +695,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     }
                     float ux, uy, uz, lam_inv, cth = 1.f, q = 0.f, pqz = 0.f, wx = 0.f, wy = 0.f, wz = 0.f;
                     float sphi, cphi;
-                    sincospif(2.0f * u0, &sphi, &cphi);
+                    sincos_2pi_u(rn.x, sphi, cphi);                       // phi = 2 pi u0
                     if (EMIT == C8PH_EMIT_CHERENKOV) {
                         // a6/a7: cos(theta_c) = 1/(beta n(h_e)) (Eq. 2.5), beta n - 1 without cancellation
                         const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
-                        q = sqrtf(bn1 * (2.f + bn1));                   // tan(theta_c)
-                        cth = __frcp_rn(1.f + bn1);                     // cos(theta_c)
+                        q = sqrt_fast(bn1 * (2.f + bn1));               // tan(theta_c)
+                        cth = rcp_fast(1.f + bn1);                      // cos(theta_c)
                         wx = cphi * sg.e1x + sphi * sg.e2x;
                         wy = cphi * sg.e1y + sphi * sg.e2y;
                         wz = cphi * sg.e1z + sphi * sg.e2z;
@@ -666,97 +732,93 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         uz = cp * az + sp2 * (sphi * e2z);
                     }
                     // a8: up-going / horizontal photons are discarded
-                    if (uz >= kUpCut) { alive = false; pkA += 1u; }
-                    float xl = 0.f, yl = 0.f, ox = 0.f, oy = 0.f, D = 0.f, inv_uz = 0.f;
-                    if (alive) {
-                        // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
-                        inv_uz = __frcp_rn(uz);
-                        const float Z = fmaf(s, sg.Pz, sg.Az);
-                        D = -Z * inv_uz;
-                        if (sg.anchor) {
-                            const float zq = -Z * q * __frcp_rn(sg.Pz * pqz);
-                            ox = zq * (wx * sg.Pz - sg.Px * wz);
-                            oy = zq * (wy * sg.Pz - sg.Py * wz);
-                            xl = sg.Gx + ox;
-                            yl = sg.Gy + oy;
-                        } else {
-                            xl = fmaf(D, ux, fmaf(s, sg.Px, sc->Ax));
-                            yl = fmaf(D, uy, fmaf(s, sg.Py, sc->Ay));
-                        }
-                        // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
-                        // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
-                        if (run.lv2) {
-                            bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
-                            if (!keep && det.n_tel > 0) {
-                                const bool brute = !det.use_grid || -uz < det.grid_min_cos;
-                                const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
-                                const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
-                                if (cell < -1 || (cell >= 0 && __ldg(det.lv2.kmin + cell) <= thr))
-                                    keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
-                            }
-                            if (!keep) { alive = false; pkA += 0x10000u; }
-                        }
+                    if (uz >= kUpCut) { pkA += 1u; break; }
+                    // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
+                    float xl, yl, ox = 0.f, oy = 0.f;
+                    const float inv_uz = rcp_fast(uz);
+                    const float Z = fmaf(s, sg.Pz, sg.Az);
+                    const float D = -Z * inv_uz;
+                    if (sg.anchor) {
+                        const float zq = -Z * q * rcp_fast(sg.Pz * pqz);
+                        ox = zq * (wx * sg.Pz - sg.Px * wz);
+                        oy = zq * (wy * sg.Pz - sg.Py * wz);
+                        xl = sg.Gx + ox;
+                        yl = sg.Gy + oy;
+                    } else {
+                        xl = fmaf(D, ux, fmaf(s, sg.Px, sc->Ax));
+                        yl = fmaf(D, uy, fmaf(s, sg.Py, sc->Ay));
                     }
-                    float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz = 1.f, sinz = 0.f;
-                    if (alive) {
-                        // local zenith angle of the photon at the emission point
-                        if (SPH) {
-                            float ur;
-                            if (EMIT == C8PH_EMIT_CHERENKOV) ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
-                            else ur = ux * sc->rx + uy * sc->ry + uz * sc->rz;
-                            const float sr = s * sg.inv_rA;
-                            const float uP = (EMIT == C8PH_EMIT_CHERENKOV) ? cth : (ux * sg.Px + uy * sg.Py + uz * sg.Pz);
-                            cz = -(fmaf(-sr * sg.cA, ur, ur) + sr * uP);
-                        } else {
-                            cz = -uz;
+                    // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
+                    // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
+                    if (run.lv2) {
+                        bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
+                        if (!keep && det.n_tel > 0) {
+                            const bool brute = !det.use_grid || -uz < det.grid_min_cos;
+                            const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
+                            const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
+                            if (cell < -1 || (cell >= 0 && __ldg(det.lv2.kmin + cell) <= thr))
+                                keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
                         }
-                        cz = fminf(cz, 1.f);
-                        sinz = sqrtf(fmaxf(1.f - cz * cz, 0.f));
-                        // a11: refraction
-                        if (TRACE == C8PH_TRACE_STRAIGHT) {
-                            dt = eta_e * D * kInvC;                      // homogeneous: t = t_e + n D / c
-                        } else if (TRACE == C8PH_TRACE_TABLE) {
-                            const TabVal v = table_lookup(a.tab, h_e, acosf(cz));
-                            if (v.bad || !(cz > 0.f)) { alive = false; pkB += 1u; }
-                            dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
+                        if (!keep) { pkA += 0x10000u; break; }
+                    }
+                    // local zenith angle of the photon at the emission point
+                    float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz;
+                    if (SPH) {
+                        float ur;
+                        if (EMIT == C8PH_EMIT_CHERENKOV) ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
+                        else ur = ux * sc->rx + uy * sc->ry + uz * sc->rz;
+                        const float sr = s * sg.inv_rA;
+                        const float uP = (EMIT == C8PH_EMIT_CHERENKOV) ? cth : (ux * sg.Px + uy * sg.Py + uz * sg.Pz);
+                        cz = -(fmaf(-sr * sg.cA, ur, ur) + sr * uP);
+                    } else {
+                        cz = -uz;
+                    }
+                    cz = fminf(cz, 1.f);
+                    // a11: refraction
+                    if (TRACE == C8PH_TRACE_STRAIGHT) {
+                        dt = eta_e * D * kInvC;                          // homogeneous: t = t_e + n D / c
+                    } else if (TRACE == C8PH_TRACE_TABLE) {
+                        const TabVal v = table_lookup(a.tab, h_e, acos01(fmaxf(cz, 0.f)));
+                        if (v.bad || !(cz > 0.f)) { pkB += 1u; break; }
+                        dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
+                    } else {
+                        // layered Snell sum (Eq. 3.15 in its invariant form K = n sin(theta)),
+                        // accumulated as the difference to the straight line
+                        const float sinz = sqrtf(fmaxf(1.f - cz * cz, 0.f));
+                        const float n_e = 1.f + eta_e;
+                        const float K = n_e * sinz;
+                        const float r_e = __frcp_rn(n_e * cz);
+                        const float fe = fminf(fmaxf((h_e - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
+                        const float fg = fminf(fmaxf(((float)atm.h_obs - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
+                        const int ke = min((int)fe, atm.n_nodes - 2), kg = min((int)fg, atm.n_nodes - 2);
+                        const float fre = fe - (float)ke, frg = fg - (float)kg;
+                        float aX = 0.f, aT = 0.f, aS = 0.f;
+                        bool ok = cz > 0.f;
+                        auto layer = [&](float eta_l, float thick, float dxv_l) {
+                            const float n_l = 1.f + eta_l;
+                            const float ql = fmaf(n_l, n_l, -K * K);
+                            ok = ok && (ql > 0.f);
+                            const float r_l = rsqrtf(ql);
+                            const float dq = (eta_e - eta_l) * (2.f + eta_e + eta_l);       // q_e - q_l
+                            const float dr = dq * r_l * r_l * r_e * r_e * __frcp_rn(r_l + r_e); // r_l - r_e
+                            aX = fmaf(thick * K, dr, aX);
+                            aT = fmaf(thick, fmaf(n_l * n_l, dr, r_e * (fmaf(eta_l, eta_l, 2.f * eta_l) - eta_e)), aT);
+                            aS = fmaf(dxv_l * n_l, r_l, aS);
+                        };
+                        if (ke == kg) {
+                            const float fm = 0.5f * (fre + frg);
+                            layer(fmaf(fm, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), (fre - frg) * atm.dh, (fre - frg) * s_dxv[ke]);
                         } else {
-                            // layered Snell sum (Eq. 3.15 in its invariant form K = n sin(theta)),
-                            // accumulated as the difference to the straight line
-                            const float n_e = 1.f + eta_e;
-                            const float K = n_e * sinz;
-                            const float r_e = __frcp_rn(n_e * cz);
-                            const float fe = fminf(fmaxf((h_e - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
-                            const float fg = fminf(fmaxf(((float)atm.h_obs - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
-                            const int ke = min((int)fe, atm.n_nodes - 2), kg = min((int)fg, atm.n_nodes - 2);
-                            const float fre = fe - (float)ke, frg = fg - (float)kg;
-                            float aX = 0.f, aT = 0.f, aS = 0.f;
-                            bool ok = cz > 0.f;
-                            auto layer = [&](float eta_l, float thick, float dxv_l) {
-                                const float n_l = 1.f + eta_l;
-                                const float ql = fmaf(n_l, n_l, -K * K);
-                                ok = ok && (ql > 0.f);
-                                const float r_l = rsqrtf(ql);
-                                const float dq = (eta_e - eta_l) * (2.f + eta_e + eta_l);       // q_e - q_l
-                                const float dr = dq * r_l * r_l * r_e * r_e * __frcp_rn(r_l + r_e); // r_l - r_e
-                                aX = fmaf(thick * K, dr, aX);
-                                aT = fmaf(thick, fmaf(n_l * n_l, dr, r_e * (fmaf(eta_l, eta_l, 2.f * eta_l) - eta_e)), aT);
-                                aS = fmaf(dxv_l * n_l, r_l, aS);
-                            };
-                            if (ke == kg) {
-                                const float fm = 0.5f * (fre + frg);
-                                layer(fmaf(fm, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), (fre - frg) * atm.dh, (fre - frg) * s_dxv[ke]);
-                            } else {
-                                if (fre > 0.f)
-                                    layer(fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke]);
-                                for (int k = ke - 1; k > kg; --k) layer(s_mid[k], atm.dh, s_dxv[k]);
-                                layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
-                            }
-                            if (!ok) { alive = false; pkB += 1u; }
-                            dd = aX; dt = aT * kInvC; Xs = aS;
+                            if (fre > 0.f)
+                                layer(fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke]);
+                            for (int k = ke - 1; k > kg; --k) layer(s_mid[k], atm.dh, s_dxv[k]);
+                            layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
                         }
+                        if (!ok) { pkB += 1u; break; }
+                        dd = aX; dt = aT * kInvC; Xs = aS;
                     }
                     float wgt = run.w;
-                    if (alive && run.trans != C8PH_TRANS_OFF) {
+                    if (run.trans != C8PH_TRANS_OFF) {
                         // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
                         float tau = 0.f;
                         if (atm.ray_inv_X > 0.f) {
@@ -767,74 +829,73 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         if (atm.aer_L > 0.f) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
                         const float T = __expf(-tau);
                         if (run.trans == C8PH_TRANS_ROULETTE) {
-                            if (!(u3 < T)) { alive = false; pkB += 0x10000u; }
+                            if (!(u01(rn.w) < T)) { pkB += 0x10000u; break; }
                         } else wgt = run.w * T;
                     }
-                    if (alive) {
-                        // landed: corrected position (dd along the horizontal direction of flight)
-                        const float hn2 = ux * ux + uy * uy;
-                        float ehx = 0.f, ehy = 0.f;
-                        if (hn2 >= 1e-18f) { const float ih = rsqrtf(hn2); ehx = ux * ih; ehy = uy * ih; }
-                        const float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);     // offset from the anchor
-                        float xg, yg;
-                        if (sg.anchor) { xg = sg.Gx + cx; yg = sg.Gy + cy; }
-                        else { xg = fmaf(dd, ehx, xl); yg = fmaf(dd, ehy, yl); }
-                        // a15: ground grid
-                        if (has_grid_geom) {
-                            int ix, iy;
-                            if (sg.anchor) {
-                                ix = sc->ibx + __float2int_rd(fmaf(cx, det.hist_inv_cell, sc->fbx));
-                                iy = sc->iby + __float2int_rd(fmaf(cy, det.hist_inv_cell, sc->fby));
-                            } else {
-                                ix = __float2int_rd((xg - det.hist_x0) * det.hist_inv_cell);
-                                iy = __float2int_rd((yg - det.hist_y0) * det.hist_inv_cell);
-                            }
-                            if ((unsigned)ix < (unsigned)det.hist_nx && (unsigned)iy < (unsigned)det.hist_ny) {
-                                pkC += 1u;
-                                if (has_hist) atomicAdd(run.out.hist + (iy * det.hist_nx + ix), wgt);
-                            }
+                    // landed: corrected position (dd along the horizontal direction of flight)
+                    const float hn2 = ux * ux + uy * uy;
+                    float ehx = 0.f, ehy = 0.f;
+                    if (hn2 >= 1e-18f) { const float ih = rsqrt_fast(hn2); ehx = ux * ih; ehy = uy * ih; }
+                    const float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);         // offset from the anchor
+                    float xg, yg;
+                    if (sg.anchor) { xg = sg.Gx + cx; yg = sg.Gy + cy; }
+                    else { xg = fmaf(dd, ehx, xl); yg = fmaf(dd, ehy, yl); }
+                    // a14 pre-test: the photon can hit a sphere of its grid cell only if the cell's
+                    // smallest key <= 1/|u_z| (inflated for the refraction rotation of the direction); the
+                    // load is issued before the binning arithmetic so its latency overlaps
+                    int cell = -1;
+                    float kmin = CUDART_INF_F;
+                    if (det.n_tel > 0) {
+                        const bool brute = run.hit_brute || !det.use_grid || -uz < det.grid_min_cos;
+                        cell = brute ? -2 : grid_cell(det.hit, xg, yg);
+                        if (cell >= 0) kmin = __ldg(det.hit.kmin + cell);
+                    }
+                    // a15: ground grid
+                    if (has_grid_geom) {
+                        int ix, iy;
+                        if (sg.anchor) {
+                            ix = sc->ibx + __float2int_rd(fmaf(cx, det.hist_inv_cell, sc->fbx));
+                            iy = sc->iby + __float2int_rd(fmaf(cy, det.hist_inv_cell, sc->fby));
+                        } else {
+                            ix = __float2int_rd((xg - det.hist_x0) * det.hist_inv_cell);
+                            iy = __float2int_rd((yg - det.hist_y0) * det.hist_inv_cell);
                         }
-                        // a14: telescope spheres.  Pre-test on the sorted grid: the photon can
-                        // hit a sphere of its cell only if the cell's smallest key <= 1/|u_z| (inflated
-                        // for the refraction rotation of the direction); everything else skips the
-                        // arrival-direction arithmetic unless the record is written anyway.
-                        int cell = -1;
-                        bool cand = false;
-                        if (det.n_tel > 0) {
-                            const bool brute = run.hit_brute || !det.use_grid || -uz < det.grid_min_cos;
-                            cell = brute ? -2 : grid_cell(det.hit, xg, yg);
-                            cand = cell < -1 || (cell >= 0 && __ldg(det.hit.kmin + cell) <= -inv_uz * run.hit_infl);
-                            if (!cand) cell = -1;
-                        }
-                        if (cand || run.write == C8PH_WRITE_ALL) {
-                            // a13: arrival time relative to t_ref
-                            float t_arr;
-                            if (sg.anchor) {
-                                // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
-                                const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
-                                const float num = fmaf(q, wz, -bn1 * sg.Pz);
-                                const float geo = (s + sg.AzP) * num * __frcp_rn(pqz);
-                                t_arr = sc->Tg + fmaf(fmaf(s, sg.delta / sg.beta, geo), kInvC, dt);
-                            } else {
-                                t_arr = sc->Tg + fmaf(s / sg.beta + D, kInvC, dt);
-                            }
-                            // queue the photon for finish(): slots are handed out per group of lanes
-                            // that arrive here together (one shared-memory atomic per group)
-                            const unsigned am = __activemask();
-                            const int leader = __ffs(am) - 1;
-                            int qb = 0;
-                            if (lane == leader) qb = atomicAdd(&s_qn[warp], __popc(am));
-                            qb = __shfl_sync(am, qb, leader);
-                            float *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1));
-                            e[Q_X * kQueue] = xg; e[Q_Y * kQueue] = yg;
-                            e[Q_UX * kQueue] = ux; e[Q_UY * kQueue] = uy; e[Q_UZ * kQueue] = uz;
-                            e[Q_T * kQueue] = t_arr; e[Q_LAMINV * kQueue] = lam_inv; e[Q_WGT * kQueue] = wgt;
-                            e[Q_ETA * kQueue] = eta_e; e[Q_H * kQueue] = h_e; e[Q_DD * kQueue] = dd; e[Q_CZ * kQueue] = cz;
-                            e[Q_CELL * kQueue] = __int_as_float(cell);
-                            e[Q_JSLOT * kQueue] = __uint_as_float(((uint32_t)j << 5) | (uint32_t)src);
+                        if ((unsigned)ix < (unsigned)det.hist_nx && (unsigned)iy < (unsigned)det.hist_ny) {
+                            pkC += 1u;
+                            if (has_hist) atomicAdd(run.out.hist + (iy * det.hist_nx + ix), wgt);
                         }
                     }
-                }
+                    const bool cand = cell < -1 || kmin <= -inv_uz * run.hit_infl;
+                    if (!cand) {
+                        if (run.write != C8PH_WRITE_ALL) break;
+                        cell = -1;
+                    }
+                    // a13: arrival time relative to t_ref
+                    float t_arr;
+                    if (sg.anchor) {
+                        // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
+                        const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
+                        const float num = fmaf(q, wz, -bn1 * sg.Pz);
+                        const float geo = (s + sg.AzP) * num * rcp_fast(pqz);
+                        t_arr = sc->Tg + fmaf(fmaf(s, (g_hot + src)->dob, geo), kInvC, dt);
+                    } else {
+                        t_arr = sc->Tg + fmaf(fmaf(s, (g_hot + src)->inv_beta, D), kInvC, dt);
+                    }
+                    // queue the photon for finish(): slots are handed out per group of lanes that arrive
+                    // here together (one shared-memory atomic per group)
+                    const unsigned am = __activemask();
+                    const int leader = __ffs(am) - 1;
+                    int qb = 0;
+                    if (lane == leader) qb = atomicAdd(&s_qn[warp], __popc(am));
+                    qb = __shfl_sync(am, qb, leader);
+                    float *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1));
+                    e[Q_X * kQueue] = xg; e[Q_Y * kQueue] = yg;
+                    e[Q_UX * kQueue] = ux; e[Q_UY * kQueue] = uy; e[Q_UZ * kQueue] = uz;
+                    e[Q_T * kQueue] = t_arr; e[Q_LAMINV * kQueue] = lam_inv; e[Q_WGT * kQueue] = wgt;
+                    e[Q_ETA * kQueue] = eta_e; e[Q_H * kQueue] = h_e; e[Q_DD * kQueue] = dd; e[Q_CZ * kQueue] = cz;
+                    e[Q_CELL * kQueue] = __int_as_float(cell);
+                    e[Q_JSLOT * kQueue] = __uint_as_float(((uint32_t)j << 5) | (uint32_t)src);
+                } while (false);
                 // a14/a16: once 32 candidates wait, a full warp takes them through finish()
                 drain(false);
             }
