@@ -34,10 +34,16 @@ namespace c8ph {
 
 namespace {
 
-constexpr int kThreads = 256;
+#ifndef C8PH_THREADS
+#define C8PH_THREADS 256
+#endif
+#ifndef C8PH_MIN_BLOCKS
+#define C8PH_MIN_BLOCKS 3
+#endif
+constexpr int kThreads = C8PH_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kMaxBlocksPerSM = C8PH_MAX_BLOCKS_PER_SM;
-constexpr int kMinBlocks = 3;                    // resident CTAs per SM the register budget is set for
+constexpr int kMinBlocks = C8PH_MIN_BLOCKS;                    // resident CTAs per SM the register budget is set for
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
 constexpr double kAlpha = 1.0 / 137.035999;
@@ -348,7 +354,10 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2,
        WC_CAM, WC_WRITTEN, WC_OVERFLOW, WC_N };
 
 // ================================================================================================
-template <int EMIT, int TRACE, bool SPH>
+// SPEC = 1 fixes the run-time switches to the array-detector production setting (LV2 on, Rayleigh
+// roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present):
+// the host picks it when the call matches (launch_emit_propagate); SPEC = 0 reads the switches.
+template <int EMIT, int TRACE, bool SPH, int SPEC>
 __global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 1 : kMinBlocks)
 k_emit_propagate(const __grid_constant__ KArgs a)
 {
@@ -411,8 +420,19 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         iters_pending = 0;
     };
 
-    const bool has_hist = det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr;
-    const bool has_grid_geom = det.hist_nx > 0 && !det.cam_enabled;
+    const bool has_hist = SPEC ? true : (det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr);
+    const bool has_grid_geom = SPEC ? true : (det.hist_nx > 0 && !det.cam_enabled);
+    const bool f_lv2 = SPEC ? true : run.lv2 != 0;
+    const bool f_tel = SPEC ? true : det.n_tel > 0;
+    const bool f_grid = SPEC ? true : det.use_grid != 0;
+    const bool f_hit_brute = SPEC ? false : run.hit_brute != 0;
+    const int f_trans = SPEC ? (int)C8PH_TRANS_ROULETTE : run.trans;
+    const bool f_ray = SPEC ? true : atm.ray_inv_X > 0.f;
+    const bool f_aer = SPEC ? false : atm.aer_L > 0.f;
+    const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
+    const bool f_cam = SPEC ? false : det.cam_enabled != 0;
+    const bool f_photons = SPEC ? true : run.out.photons != nullptr;
+    const bool f_telc = SPEC ? true : run.out.tel_counts != nullptr;
     const float inv_ng = 1.0f / (1.0f + atm.eta_g);
     int q_head = 0;                                           // ring position of the oldest queue entry
 
@@ -440,7 +460,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 uay = fmaf(k1, uy, k2 * sc->ry);
                 uaz = fmaf(k1, uz, k2 * sc->rz);
             }
-            if (det.n_tel > 0 && cell != -1) {
+            if (f_tel && cell != -1) {
                 // the pre-test threshold must cover the rotated direction; if it does not (never in
                 // air), search all telescopes
                 const float thr = -rcp_fast(uz) * run.hit_infl;
@@ -449,8 +469,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             }
             if (tel >= 0) {
                 pkC += 0x10000u;
-                if (run.out.tel_counts) atomicAdd(run.out.tel_counts + tel, wgt);
-                if (det.cam_enabled) {
+                if (f_telc) atomicAdd(run.out.tel_counts + tel, wgt);
+                if (f_cam) {
                     const int pix = camera_pixel(det, uax, uay, uaz);
                     const float tb = floorf(t_arr * det.inv_t_bin);
                     if (pix >= 0 && tb >= 0.f && tb < (float)det.n_tbins) {
@@ -462,8 +482,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         }
         // a16: survivors are ranked by warp ballot and stored straight from registers: one cursor
         // atomic per call, consecutive 32 B records
-        const bool write = act && (run.write == C8PH_WRITE_ALL || (run.write == C8PH_WRITE_TEL && tel >= 0));
-        if (run.out.photons) {
+        const bool write = act && (f_write == C8PH_WRITE_ALL || (f_write == C8PH_WRITE_TEL && tel >= 0));
+        if (f_photons) {
             const unsigned wm = __ballot_sync(FULL, write);
             if (wm) {
                 unsigned long long base = 0;
@@ -750,10 +770,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     }
                     // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
                     // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
-                    if (run.lv2) {
+                    if (f_lv2) {
                         bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
-                        if (!keep && det.n_tel > 0) {
-                            const bool brute = !det.use_grid || -uz < det.grid_min_cos;
+                        if (!keep && f_tel) {
+                            const bool brute = !f_grid || -uz < det.grid_min_cos;
                             const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
                             const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
                             if (cell < -1 || (cell >= 0 && __ldg(det.lv2.kmin + cell) <= thr))
@@ -818,17 +838,17 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         dd = aX; dt = aT * kInvC; Xs = aS;
                     }
                     float wgt = run.w;
-                    if (run.trans != C8PH_TRANS_OFF) {
+                    if (f_trans != C8PH_TRANS_OFF) {
                         // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
                         float tau = 0.f;
-                        if (atm.ray_inv_X > 0.f) {
+                        if (f_ray) {
                             float qq = atm.ray_lambda * lam_inv;
                             qq *= qq; qq *= qq;
                             tau = Xs * qq * atm.ray_inv_X;
                         }
-                        if (atm.aer_L > 0.f) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
+                        if (f_aer) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
                         const float T = __expf(-tau);
-                        if (run.trans == C8PH_TRANS_ROULETTE) {
+                        if (f_trans == C8PH_TRANS_ROULETTE) {
                             if (!(u01(rn.w) < T)) { pkB += 0x10000u; break; }
                         } else wgt = run.w * T;
                     }
@@ -845,8 +865,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // load is issued before the binning arithmetic so its latency overlaps
                     int cell = -1;
                     float kmin = CUDART_INF_F;
-                    if (det.n_tel > 0) {
-                        const bool brute = run.hit_brute || !det.use_grid || -uz < det.grid_min_cos;
+                    if (f_tel) {
+                        const bool brute = f_hit_brute || !f_grid || -uz < det.grid_min_cos;
                         cell = brute ? -2 : grid_cell(det.hit, xg, yg);
                         if (cell >= 0) kmin = __ldg(det.hit.kmin + cell);
                     }
@@ -867,7 +887,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     }
                     const bool cand = cell < -1 || kmin <= -inv_uz * run.hit_infl;
                     if (!cand) {
-                        if (run.write != C8PH_WRITE_ALL) break;
+                        if (f_write != C8PH_WRITE_ALL) break;
                         cell = -1;
                     }
                     // a13: arrival time relative to t_ref
@@ -1023,19 +1043,19 @@ __global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ Tab
     a.hot[node] = make_float4(out[0], out[2], out[3], out[4]);
 }
 
-template <int EMIT, int TRACE, bool SPH>
+template <int EMIT, int TRACE, bool SPH, int SPEC>
 cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
 {
-    auto kern = k_emit_propagate<EMIT, TRACE, SPH>;
+    auto kern = k_emit_propagate<EMIT, TRACE, SPH, SPEC>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
+    if (per_sm > kMaxBlocksPerSM) per_sm = kMaxBlocksPerSM;         // the segment-slot scratch is sized for this
     long long warps_needed = (a.run.n_seg + a.run.segs_per_grab - 1) / a.run.segs_per_grab;
     long long blocks = (warps_needed + kWarps - 1) / kWarps;
-    if (per_sm > kMaxBlocksPerSM) per_sm = kMaxBlocksPerSM;         // the segment-slot scratch is sized for this
     const long long max_blocks = (long long)n_sm * per_sm;          // persistent: one resident wave
     if (blocks > max_blocks) blocks = max_blocks;
     if (blocks < 1) blocks = 1;
@@ -1062,13 +1082,27 @@ size_t emit_smem_bytes(const KArgs &a)
     return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
 }
 
+// true iff the call matches the switches k_emit_propagate<.., SPEC = 1> is compiled for
+static bool array_production_setting(const KArgs &a)
+{
+    const DevRun &r = a.run;
+    const DevDet &d = a.det;
+    return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
+           a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
+           d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
+           r.out.tel_counts != nullptr;
+}
+
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 {
     const size_t smem = emit_smem_bytes(a);
     const bool sph = a.atm.model == C8PH_ATM_SPHERICAL;
+    if (array_production_setting(a))
+        return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, 1>(a, n_sm, smem, st)
+                   : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, 1>(a, n_sm, smem, st);
 #define C8_CASE(E, T)                                                             \
     if (a.run.emit == E && a.run.trace == T)                                      \
-        return sph ? launch_one<E, T, true>(a, n_sm, smem, st) : launch_one<E, T, false>(a, n_sm, smem, st);
+        return sph ? launch_one<E, T, true, 0>(a, n_sm, smem, st) : launch_one<E, T, false, 0>(a, n_sm, smem, st);
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_STRAIGHT)
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_NUMERIC)
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE)
