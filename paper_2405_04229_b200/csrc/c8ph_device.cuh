@@ -45,6 +45,8 @@ struct DevGrid {
     float x0, y0, inv_cs;
     int nx, ny;
     const float *kmin;              // DEVICE [nx*ny]   smallest key of the cell (+inf: empty)
+    const float2 *kacc;             // LV2 grid only, DEVICE [nx*ny]: (kmin, acc) with acc = min_k(max dist(cell, centre_k) - r_k):
+                                    // every point of the cell is within r_k/|u_z| + margin of a centre if acc <= margin
     const int *start;               // DEVICE [nx*ny+1] CSR offsets into items
     const float2 *items;            // DEVICE (key, telescope index as int bits), ascending key per cell
 };

@@ -35,6 +35,7 @@ struct c8ph_ctx {
     int *d_g_start[2] = {nullptr, nullptr};
     float2 *d_g_items[2] = {nullptr, nullptr};
     float *d_g_kmin[2] = {nullptr, nullptr};
+    float2 *d_g_kacc = nullptr;
     // run scratch
     unsigned long long *d_cursor = nullptr;
     void *d_slots = nullptr;           // prepared-segment slots of the resident warps
@@ -109,6 +110,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
+    dfree(ctx->d_g_kacc);
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
@@ -292,7 +294,13 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
         y0 = std::min(y0, tel[4 * k + 1] - rc); y1 = std::max(y1, tel[4 * k + 1] + rc);
     }
     const double ext = std::max(x1 - x0, y1 - y0);
-    double cs = mode == 0 ? rz_min : 2.0 * r_max;
+    // cell size: about one telescope radius, but no more than ~4e6 list entries and 1536^2 cells
+    double cs = mode == 0 ? rz_min : r_max;
+    {
+        double area = 0.0;
+        for (int k = 0; k < n; ++k) area += 3.14159265358979 * reach(k) * reach(k);
+        cs = std::max(cs, std::sqrt(area / 4.0e6));
+    }
     cs = std::max(cs, ext / 1536.0);
     if (!(cs > 0.0)) cs = 1.0;
     const int nx = std::max(1, (int)std::ceil((x1 - x0) / cs)), ny = std::max(1, (int)std::ceil((y1 - y0) / cs));
@@ -301,6 +309,7 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     const double pad = 1e-3 * cs + 8.0 * (coord_max + ext) * 1.2e-7 + 1e-4;
     struct Entry { uint32_t cell; float key; int k; };
     std::vector<Entry> ent;
+    std::vector<float> acc(mode == 1 ? ncell : 0, INFINITY);
     ent.reserve((size_t)n * 64);
     for (int k = 0; k < n; ++k) {
         const double cx_ = tel[4 * k], cy_ = tel[4 * k + 1], rc = reach(k);
@@ -314,6 +323,15 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
                 const double px = std::min(std::max(cx_, bx0), bx1), py = std::min(std::max(cy_, by0), by1);
                 const double dist = std::sqrt((px - cx_) * (px - cx_) + (py - cy_) * (py - cy_));
                 if (dist > rc) continue;
+                if (mode == 1) {
+                    // farthest point of the padded cell from the centre, minus the radius, rounded up
+                    const double fx = std::max(std::fabs(bx0 - cx_), std::fabs(bx1 - cx_)), fy = std::max(std::fabs(by0 - cy_), std::fabs(by1 - cy_));
+                    const double av = (std::sqrt(fx * fx + fy * fy) - (double)tel[4 * k + 3]) * (1.0 + 1e-6) + 1e-4;
+                    float af = (float)av;
+                    if ((double)af < av) af = std::nextafterf(af, INFINITY);
+                    float &slot = acc[(size_t)iy * nx + ix];
+                    if (af < slot) slot = af;
+                }
                 const double key = mode == 0 ? dist / rz : dist;
                 ent.push_back({(uint32_t)((size_t)iy * nx + ix), f32_down(key * (1.0 - 1e-6)), k});
             }
@@ -343,6 +361,15 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     CU(cudaMemcpy(ctx->d_g_kmin[which], kmin.data(), kmin.size() * sizeof(float), cudaMemcpyHostToDevice));
     g.x0 = (float)x0; g.y0 = (float)y0; g.inv_cs = (float)(1.0 / cs); g.nx = nx; g.ny = ny;
     g.kmin = ctx->d_g_kmin[which]; g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
+    g.kacc = nullptr;
+    if (mode == 1) {
+        std::vector<float2> ka(ncell);
+        for (size_t i = 0; i < ncell; ++i) ka[i] = make_float2(kmin[i], acc[i]);
+        dfree(ctx->d_g_kacc);
+        CU(cudaMalloc(&ctx->d_g_kacc, ncell * sizeof(float2)));
+        CU(cudaMemcpy(ctx->d_g_kacc, ka.data(), ncell * sizeof(float2), cudaMemcpyHostToDevice));
+        g.kacc = ctx->d_g_kacc;
+    }
     return C8PH_OK;
 }
 

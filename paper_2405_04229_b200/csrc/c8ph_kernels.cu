@@ -290,28 +290,28 @@ __device__ __forceinline__ int tel_hit_search(const DevDet &det, int cell, float
     return best_k;
 }
 
-// LV2/LV3 proximity: is (x,y) within r_k/|u_z| + margin of any telescope centre?
+// LV2/LV3 proximity: is (x,y) within r_k/|u_z| + margin of any telescope centre?  (single exit)
 __device__ __forceinline__ bool tel_near_search(const DevDet &det, int cell, float thr, float x, float y,
-                                             float inv_abs_uz, float margin)
+                                                float inv_abs_uz, float margin)
 {
+    bool found = false;
     if (cell < -1) {
-        for (int k = 0; k < det.n_tel; ++k) {
+        for (int k = 0; k < det.n_tel && !found; ++k) {
             const float4 t = __ldg(det.tel + k);
             const float dx = x - t.x, dy = y - t.y, reach = fmaf(t.w, inv_abs_uz, margin);
-            if (dx * dx + dy * dy <= reach * reach) return true;
+            found = dx * dx + dy * dy <= reach * reach;
         }
-        return false;
+    } else if (cell >= 0) {
+        const int hi = __ldg(det.lv2.start + cell + 1);
+        for (int i = __ldg(det.lv2.start + cell); i < hi && !found; ++i) {
+            const float2 e = __ldg(det.lv2.items + i);
+            if (e.x > thr) break;
+            const float4 t = __ldg(det.tel + __float_as_int(e.y));
+            const float dx = x - t.x, dy = y - t.y, reach = fmaf(t.w, inv_abs_uz, margin);
+            found = dx * dx + dy * dy <= reach * reach;
+        }
     }
-    if (cell < 0) return false;
-    const int hi = __ldg(det.lv2.start + cell + 1);
-    for (int i = __ldg(det.lv2.start + cell); i < hi; ++i) {
-        const float2 e = __ldg(det.lv2.items + i);
-        if (e.x > thr) break;
-        const float4 t = __ldg(det.tel + __float_as_int(e.y));
-        const float dx = x - t.x, dy = y - t.y, reach = fmaf(t.w, inv_abs_uz, margin);
-        if (dx * dx + dy * dy <= reach * reach) return true;
-    }
-    return false;
+    return found;
 }
 
 // hexagonal camera pixel of an arrival direction (cfg3); -1 outside.  Nearest centre among the
@@ -776,7 +776,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             const bool brute = !f_grid || -uz < det.grid_min_cos;
                             const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
                             const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
-                            if (cell < -1 || (cell >= 0 && __ldg(det.lv2.kmin + cell) <= thr))
+                            // per cell: (smallest key, acc); acc <= margin: every point of the cell is near
+                            // a telescope; smallest key > thr: none is; otherwise walk the sorted list
+                            float2 ka = make_float2(CUDART_INF_F, CUDART_INF_F);
+                            if (cell >= 0) ka = __ldg(det.lv2.kacc + cell);
+                            keep = ka.y <= run.lv2_margin;
+                            if (!keep && (cell < -1 || ka.x <= thr))
                                 keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
                         }
                         if (!keep) { pkA += 0x10000u; break; }
