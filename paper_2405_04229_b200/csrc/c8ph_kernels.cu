@@ -771,6 +771,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
                     // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
                     if (f_lv2) {
+                        const unsigned conv = __activemask();            // lanes that reach the filter together
                         bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
                         if (!keep && f_tel) {
                             const bool brute = !f_grid || -uz < det.grid_min_cos;
@@ -784,6 +785,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             if (!keep && (cell < -1 || ka.x <= thr))
                                 keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
                         }
+                        __syncwarp(conv);                                // rejoin the lanes that searched a list
                         if (!keep) { pkA += 0x10000u; break; }
                     }
                     // local zenith angle of the photon at the emission point
