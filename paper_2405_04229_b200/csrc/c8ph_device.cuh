@@ -87,7 +87,7 @@ struct DevRun {
     c8ph_segments seg;              // DEVICE pointers
     c8ph_outputs out;               // DEVICE pointers
     unsigned long long *cursor;     // DEVICE work cursor (segments)
-    void *slots_hot, *slots_cold;   // DEVICE scratch: 32 prepared-segment slots (hot / cold part) per resident warp
+    void *slots;                    // DEVICE scratch: 32 prepared-segment slots per resident warp
     int segs_per_grab;              // segments one warp prepares per grab (1..32)
 };
 

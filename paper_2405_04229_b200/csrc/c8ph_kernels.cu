@@ -134,10 +134,13 @@ struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
     uint32_t local;                                   // segment index within the call
     float pad0;
 };
-static_assert(sizeof(SegHot) == 112 && sizeof(SegCold) == 64, "segment slot layout");
+struct alignas(16) SegSlot { SegHot h; SegCold c; };
+static_assert(sizeof(SegHot) == 112 && sizeof(SegCold) == 64 && sizeof(SegSlot) == 176, "segment slot layout");
 
-// candidate queue entry (SoA in shared memory): what finish() needs of a photon
-enum { Q_X = 0, Q_Y, Q_UX, Q_UY, Q_UZ, Q_T, Q_LAMINV, Q_WGT, Q_ETA, Q_H, Q_DD, Q_CZ, Q_CELL, Q_JSLOT, Q_WORDS };
+// candidate queue entry (64 B in shared memory, written / read with four 16 B accesses): what finish()
+// needs of a photon
+// entry = 4 x float4: (x, y, ux, uy) (uz, s, q w_z, dt) (1/lambda, weight, eta_e, h_e) (dd, cos zenith, cell, j<<5|slot)
+constexpr int Q_WORDS = 16;
 constexpr int kQueue = 64;                       // ring entries per warp (a drain leaves < 32)
 
 template <typename T>
@@ -378,11 +381,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     float *s_mid = s_eta + (STAGED ? atm.n_pad : 0);
     float *s_dxv = s_mid + (STAGED ? atm.n_pad : 0);
     float *s_end = s_dxv + (STAGED ? atm.n_pad : 0);
-    float *s_q = s_end + warp * (kQueue * Q_WORDS);           // s_q[field * kQueue + slot]
+    float4 *s_q = reinterpret_cast<float4 *>(s_end) + warp * (kQueue * 4);   // s_q[slot * 4 + part]
     __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
-    SegHot *g_hot = static_cast<SegHot *>(run.slots_hot) + ((size_t)blockIdx.x * kWarps + warp) * 32;
-    SegCold *g_cold = static_cast<SegCold *>(run.slots_cold) + ((size_t)blockIdx.x * kWarps + warp) * 32;
+    SegSlot *g_slot = static_cast<SegSlot *>(run.slots) + ((size_t)blockIdx.x * kWarps + warp) * 32;
 
     if (lane < WC_N) s_cnt[warp][lane] = 0ull;
     if (lane == 0) s_qn[warp] = 0;
@@ -439,12 +441,29 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // ---- a13/a14/a16 for photons that may hit a telescope or are written anyway: arrival direction
     // (rotation in the ray plane by the Snell / Bouguer invariant), exact sphere search, counters,
     // ballot-compacted record store.  Called warp-converged; `act` marks the lanes that carry a photon.
-    auto finish = [&](bool act, float xg, float yg, float ux, float uy, float uz, float t_arr, float lam_inv,
-                      float wgt, float eta_e, float h_e, float dd, float cz, int cell, uint32_t jslot) {
+    auto finish = [&](bool act, float4 q0, float4 q1, float4 q2, float4 q3) {
+        const float xg = q0.x, yg = q0.y, ux = q0.z, uy = q0.w, uz = q1.x, s = q1.y, qw = q1.z, dt = q1.w;
+        const float lam_inv = q2.x, wgt = q2.y, eta_e = q2.z, h_e = q2.w, dd = q3.x, cz = q3.y;
+        int cell = __float_as_int(q3.z);
+        const uint32_t jslot = __float_as_uint(q3.w);
         int tel = -1;
-        float uax = ux, uay = uy, uaz = uz;
-        const SegCold *sc = g_cold + (jslot & 31u);
+        float uax = ux, uay = uy, uaz = uz, t_arr = 0.f;
+        const SegSlot *sl = g_slot + (jslot & 31u);
+        const SegHot *sh = &sl->h;
+        const SegCold *sc = &sl->c;
         if (act) {
+            // a13: arrival time relative to t_ref
+            if (sh->anchor) {
+                // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
+                const float Pz = sh->Pz;
+                const float bn1 = fmaxf(fmaf(sh->beta, eta_e, -sh->delta), 0.f);
+                const float num = fmaf(-bn1, Pz, qw);
+                const float geo = (s + sh->AzP) * num * rcp_fast(Pz + qw);
+                t_arr = sc->Tg + fmaf(fmaf(s, sh->dob, geo), kInvC, dt);
+            } else {
+                const float D = -fmaf(s, sh->Pz, sh->Az) * rcp_fast(uz);
+                t_arr = sc->Tg + fmaf(fmaf(s, sh->inv_beta, D), kInvC, dt);
+            }
             const float sinz = sqrt_fast(fmaxf(1.f - cz * cz, 0.f));
             if (TRACE != C8PH_TRACE_STRAIGHT && sinz >= 1e-6f) {
                 const float eps = (eta_e - atm.eta_g) * inv_ng;
@@ -511,11 +530,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         int n = s_qn[warp];
         while (n >= 32 || (all && n > 0)) {
             const int take = n < 32 ? n : 32;
-            const float *e = s_q + ((q_head + lane) & (kQueue - 1));
+            const float4 *e = s_q + ((q_head + lane) & (kQueue - 1)) * 4;
             const bool act = lane < take;
-            finish(act, e[Q_X * kQueue], e[Q_Y * kQueue], e[Q_UX * kQueue], e[Q_UY * kQueue], e[Q_UZ * kQueue],
-                   e[Q_T * kQueue], e[Q_LAMINV * kQueue], e[Q_WGT * kQueue], e[Q_ETA * kQueue], e[Q_H * kQueue],
-                   e[Q_DD * kQueue], e[Q_CZ * kQueue], __float_as_int(e[Q_CELL * kQueue]), __float_as_uint(e[Q_JSLOT * kQueue]));
+            finish(act, e[0], e[1], e[2], e[3]);
             q_head = (q_head + take) & (kQueue - 1);
             n -= take;
             __syncwarp();
@@ -669,8 +686,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     } else {
                         mc.Tg = (float)(t0 - det.t_ref);
                     }
-                    copy16(g_hot + lane, &me);
-                    copy16(g_cold + lane, &mc);
+                    copy16(&g_slot[lane].h, &me);
+                    copy16(&g_slot[lane].c, &mc);
                 }
             }
             // segment-level counters of the group: one ballot each, lane 0 books them
@@ -690,9 +707,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         while (emask) {
             const int src = __ffs(emask) - 1;
             emask &= emask - 1;
+            const SegSlot *sl = g_slot + src;
+            asm volatile("" : "+l"(sl));                              // keep the slot address in registers
             SegHot sg;
-            copy16(&sg, g_hot + src);                                 // uniform address: one sector per LDG.128
-            const SegCold *sc = g_cold + src;                         // cold fields are re-read (L1) where used
+            copy16(&sg, &sl->h);                                      // uniform address: one sector per LDG.128
+            const SegCold *sc = &sl->c;                               // cold fields are re-read (L1) where used
             const int n_iter = (sg.N + 31) >> 5;
             if (iters_pending + n_iter > 60000) flush_counts();
             iters_pending += n_iter;
@@ -881,8 +900,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (has_grid_geom) {
                         int ix, iy;
                         if (sg.anchor) {
-                            ix = sc->ibx + __float2int_rd(fmaf(cx, det.hist_inv_cell, sc->fbx));
-                            iy = sc->iby + __float2int_rd(fmaf(cy, det.hist_inv_cell, sc->fby));
+                            const float4 fb = *reinterpret_cast<const float4 *>(sc);     // fbx, fby, ibx, iby
+                            ix = __float_as_int(fb.z) + __float2int_rd(fmaf(cx, det.hist_inv_cell, fb.x));
+                            iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, det.hist_inv_cell, fb.y));
                         } else {
                             ix = __float2int_rd((xg - det.hist_x0) * det.hist_inv_cell);
                             iy = __float2int_rd((yg - det.hist_y0) * det.hist_inv_cell);
@@ -897,31 +917,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         if (f_write != C8PH_WRITE_ALL) break;
                         cell = -1;
                     }
-                    // a13: arrival time relative to t_ref
-                    float t_arr;
-                    if (sg.anchor) {
-                        // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
-                        const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
-                        const float num = fmaf(q, wz, -bn1 * sg.Pz);
-                        const float geo = (s + sg.AzP) * num * rcp_fast(pqz);
-                        t_arr = sc->Tg + fmaf(fmaf(s, (g_hot + src)->dob, geo), kInvC, dt);
-                    } else {
-                        t_arr = sc->Tg + fmaf(fmaf(s, (g_hot + src)->inv_beta, D), kInvC, dt);
-                    }
-                    // queue the photon for finish(): slots are handed out per group of lanes that arrive
-                    // here together (one shared-memory atomic per group)
+                    // queue the photon for finish() (a13/a14/a16): slots are handed out per group of lanes
+                    // that arrive here together (one shared-memory atomic per group), four 16 B stores
                     const unsigned am = __activemask();
                     const int leader = __ffs(am) - 1;
                     int qb = 0;
                     if (lane == leader) qb = atomicAdd(&s_qn[warp], __popc(am));
                     qb = __shfl_sync(am, qb, leader);
-                    float *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1));
-                    e[Q_X * kQueue] = xg; e[Q_Y * kQueue] = yg;
-                    e[Q_UX * kQueue] = ux; e[Q_UY * kQueue] = uy; e[Q_UZ * kQueue] = uz;
-                    e[Q_T * kQueue] = t_arr; e[Q_LAMINV * kQueue] = lam_inv; e[Q_WGT * kQueue] = wgt;
-                    e[Q_ETA * kQueue] = eta_e; e[Q_H * kQueue] = h_e; e[Q_DD * kQueue] = dd; e[Q_CZ * kQueue] = cz;
-                    e[Q_CELL * kQueue] = __int_as_float(cell);
-                    e[Q_JSLOT * kQueue] = __uint_as_float(((uint32_t)j << 5) | (uint32_t)src);
+                    float4 *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
+                    e[0] = make_float4(xg, yg, ux, uy);
+                    e[1] = make_float4(uz, s, q * wz, dt);
+                    e[2] = make_float4(lam_inv, wgt, eta_e, h_e);
+                    e[3] = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
                 } while (false);
                 // a14/a16: once 32 candidates wait, a full warp takes them through finish()
                 drain(false);
@@ -1074,13 +1081,13 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
 
 size_t segment_slot_bytes(int n_sm)
 {
-    return (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32 * (sizeof(SegHot) + sizeof(SegCold));
+    return (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32 * sizeof(SegSlot);
 }
 
 void segment_slot_pointers(void *base, int n_sm, DevRun &run)
 {
-    run.slots_hot = base;
-    run.slots_cold = static_cast<SegHot *>(base) + (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32;
+    (void)n_sm;
+    run.slots = base;
 }
 
 size_t emit_smem_bytes(const KArgs &a)
