@@ -14,6 +14,7 @@ struct DevAtm {
     int n_nodes;            // nodes of the n(h) grid (>= 2; homogeneous: 2 identical nodes)
     int n_pad;              // floats per table array, multiple of 4 (16 B, bulk-copy granule)
     float h0, dh, inv_dh, h_top;
+    float f_max;            // (float)(n_nodes - 1)
     const float *eta;       // DEVICE [n_pad] refractivity n-1 at the nodes
     const float *xv;        // DEVICE [n_pad] vertical overburden at the nodes (zeros if none)
     const float *eta_mid;   // DEVICE [n_pad] refractivity at the cell mid height (layer k = nodes k..k+1)
@@ -29,6 +30,7 @@ struct DevTable {
     int n_h, n_zen;
     float h_max, zen_max;           // [m], [rad]
     float inv_dh, inv_dz;           // (n_h-1)/h_max, (n_zen-1)/zen_max
+    float f_max, g_max;             // (float)(n_h-1), (float)(n_zen-1)
     const float4 *hot;              // DEVICE [n_h][n_zen] = (dd, dt, X_slant, tau_aer)
     const float *full;              // DEVICE [n_h][n_zen][5]
 };

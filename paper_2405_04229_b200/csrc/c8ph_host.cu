@@ -169,7 +169,7 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
     CU(cudaMemcpy(ctx->d_dxv, dxv.data(), bytes, cudaMemcpyHostToDevice));
     DevAtm &a = ctx->atm;
     a.model = d->model; a.n_nodes = n; a.n_pad = n_pad;
-    a.h0 = (float)h0; a.dh = (float)dh; a.inv_dh = (float)(1.0 / dh); a.h_top = (float)(h0 + dh * (n - 1));
+    a.h0 = (float)h0; a.dh = (float)dh; a.inv_dh = (float)(1.0 / dh); a.h_top = (float)(h0 + dh * (n - 1)); a.f_max = (float)(n - 1);
     a.eta = ctx->d_eta; a.xv = ctx->d_xv; a.eta_mid = ctx->d_mid; a.dxv = ctx->d_dxv;
     a.R = d->earth_radius_m; a.h_obs = d->h_obs_m; a.Rg = (double)d->earth_radius_m + (double)d->h_obs_m;
     a.eta_g = (float)lerp_table(eta, h0, dh, d->h_obs_m);
@@ -204,6 +204,7 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
     d.zen_max = (float)zmax;
     d.inv_dh = (float)((t->n_h - 1) / (double)t->h_max_m);
     d.inv_dz = (float)((t->n_zen - 1) / zmax);
+    d.f_max = (float)(t->n_h - 1); d.g_max = (float)(t->n_zen - 1);
     d.hot = ctx->d_hot; d.full = ctx->d_full;
     return C8PH_OK;
 }

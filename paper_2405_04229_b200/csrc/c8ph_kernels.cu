@@ -232,8 +232,8 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
 {
     TabVal o;
     o.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f);
-    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), (float)(t.n_h - 1));
-    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), (float)(t.n_zen - 1));
+    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
+    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
     const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
     const float ff = f - (float)ia, gg = g - (float)ib;
     const float4 *p = t.hot + (unsigned)(ia * t.n_zen + ib);
@@ -727,7 +727,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     float eta_e;
                     {
                         float f = (h_e - atm.h0) * atm.inv_dh;
-                        f = fminf(fmaxf(f, 0.f), (float)(atm.n_nodes - 1));
+                        f = fminf(fmaxf(f, 0.f), atm.f_max);
                         const int k = min((int)f, atm.n_nodes - 2);
                         const float e0 = eta_node(k), e1 = eta_node(k + 1);
                         eta_e = fmaf(f - (float)k, e1 - e0, e0);
@@ -922,7 +922,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const unsigned am = __activemask();
                     const int leader = __ffs(am) - 1;
                     int qb = 0;
-                    if (lane == leader) qb = atomicAdd(&s_qn[warp], __popc(am));
+                    if (lane == leader)                                  // plain ATOMS: the group is already aggregated
+                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])), "r"(__popc(am)) : "memory");
                     qb = __shfl_sync(am, qb, leader);
                     float4 *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
                     e[0] = make_float4(xg, yg, ux, uy);
