@@ -38,22 +38,24 @@ import numpy as np
 METRIC = "propagated photons/sec"
 UNIT = "photons/s"
 
-# Algorithmic thread-instructions per unit of each stage of the fused kernel (DESIGN.md section
-# "Roofline": audited from the SASS of k_emit_propagate<CHERENKOV,TABLE,SPH>, minimal path through
-# each stage, loop overhead and predication included once).
+# Algorithmic thread-instructions per unit of each stage of the fused kernel, audited from the SASS
+# of k_emit_propagate<CHERENKOV,TABLE,SPH,SPEC=1> with ncu's per-instruction execution counts
+# (DESIGN.md section 5 "Roofline"; profiles/r1_cfg4_sass_classes.md): the instructions every unit of a
+# stage executes exactly once on its way through.  What is NOT counted: telescope candidates that turn
+# out to miss, LV2 list searches, queue drains of partly filled warps, idle lanes.
 I_ALG = {
-    "segment": 620.0,     # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor (per segment)
-    "emitted": 151.0,     # a5-a10: Philox4x32-10, uniforms, emission point, n(h), cone, straight line, LV2
-    "traced": 74.0,       # a11-a12: zenith, acos, bilinear float4 lookup, transmission, roulette
-    "landed": 83.0,       # a13-a15: position, time, bin + RED, arrival direction, telescope lattice test
-    "written": 22.0,      # a16: record assembly, ballot compaction, staged store
+    "segment": 1000.0,    # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor, slot store (per segment)
+    "emitted": 265.0,     # a5-a12: loop slot 16 + Philox4x32-10, uniforms, emission point, n(h), cone, sincos,
+                          #         straight line, LV2 box, zenith, acos, bilinear float4 lookup, transmission, roulette: 249
+    "landed": 68.0,       # a15 + a14 pre-test: corrected position, telescope-grid cell + smallest key, bin index
+    "in_grid": 6.0,       # a15: bin address + RED.ADD.F32
+    "tel_hit": 193.0,     # a13/a14/a16: queue push 29 + finish 164 (time, arrival direction, sphere search, record)
 }
 
 
 def _stage_population(cnt: dict) -> dict:
-    traced = cnt["emitted"] - cnt["upgoing"] - cnt["lv2"]
-    return {"segment": cnt["segments"], "emitted": cnt["emitted"], "traced": traced,
-            "landed": cnt["landed"], "written": cnt["written"]}
+    return {"segment": cnt["segments"], "emitted": cnt["emitted"], "landed": cnt["landed"],
+            "in_grid": cnt["in_grid"], "tel_hit": cnt["tel_hit"]}
 
 
 def algorithmic_instructions(cnt: dict) -> float:
