@@ -86,6 +86,7 @@ struct DevRun {
     const float *line_nm, *line_cdf;      // DEVICE
     uint32_t key0[10], key1[10];    // Philox round keys
     int64_t n_seg, seg_id_base;
+    uint32_t local_base;            // added to the call-local segment index written into photon records
     c8ph_segments seg;              // DEVICE pointers
     c8ph_outputs out;               // DEVICE pointers
     unsigned long long *cursor;     // DEVICE work cursor (segments)

@@ -12,6 +12,8 @@
 
 using namespace c8ph;
 
+static const int kMaxChunks = 16;           // host path: pipeline depth (chunks of segments per call)
+
 struct c8ph_ctx {
     int device = 0;
     int n_sm = 0;
@@ -47,6 +49,9 @@ struct c8ph_ctx {
     // host-path scratch
     float *d_seg = nullptr; size_t seg_cap = 0;
     void *d_out = nullptr; size_t out_cap = 0;
+    cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
+    unsigned long long *h_written = nullptr;    // pinned: photon-list cursor after each chunk
+    cudaEvent_t ev_in[kMaxChunks] = {}, ev_run[kMaxChunks] = {};
 };
 
 static thread_local std::string g_create_err;
@@ -114,6 +119,11 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
+    if (ctx->st_h2d) {
+        cudaStreamDestroy(ctx->st_h2d); cudaStreamDestroy(ctx->st_run); cudaStreamDestroy(ctx->st_d2h);
+        if (ctx->h_written) cudaFreeHost(ctx->h_written);
+        for (int c = 0; c < kMaxChunks; ++c) { if (ctx->ev_in[c]) cudaEventDestroy(ctx->ev_in[c]); if (ctx->ev_run[c]) cudaEventDestroy(ctx->ev_run[c]); }
+    }
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
@@ -530,7 +540,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         r.key0[k] = (uint32_t)seed + (uint32_t)k * 0x9E3779B9u;
         r.key1[k] = (uint32_t)(seed >> 32) + (uint32_t)k * 0xBB67AE85u;
     }
-    r.n_seg = n_seg; r.seg_id_base = base;
+    r.n_seg = n_seg; r.seg_id_base = base; r.local_base = 0;
     r.seg = *s; r.out = *o;
     r.cursor = ctx->d_cursor;
     segment_slot_pointers(ctx->d_slots, ctx->n_sm, r);
@@ -566,6 +576,10 @@ extern "C" int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *s, int64_
     return launch(ctx, a, st);
 }
 
+// HOST-buffer path.  The call is split into chunks of segments and pipelined over three streams:
+// H2D of chunk c+1 | kernel of chunk c | D2H of the photons chunk c-1 wrote, so the PCIe transfer of
+// the photon list (the dominant cost) overlaps the kernel.  Chunks run in order on one
+// stream, each with seg_id_base = base + offset: the photons are those of a single call.
 extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, int64_t n_seg, int64_t base,
                                         const c8ph_params *p, uint64_t seed, const c8ph_outputs *ho)
 {
@@ -574,7 +588,16 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         return fail(ctx, C8PH_E_ARG, "emit_propagate_host: NULL struct or size mismatch");
     if (!ctx->have_det) return fail(ctx, C8PH_E_STATE, "emit_propagate_host: detector not set");
     CU(cudaSetDevice(ctx->device));
-    cudaStream_t st = nullptr;
+    if (!ctx->st_h2d) {
+        CU(cudaStreamCreateWithFlags(&ctx->st_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->st_run, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->st_d2h, cudaStreamNonBlocking));
+        CU(cudaHostAlloc(&ctx->h_written, (kMaxChunks + C8PH_N_COUNTERS) * sizeof(unsigned long long), cudaHostAllocDefault));
+        for (int c = 0; c < kMaxChunks; ++c) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_in[c], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_run[c], cudaEventDisableTiming));
+        }
+    }
     const float *src[11] = {hs->x, hs->y, hs->z, hs->dx, hs->dy, hs->dz, hs->len, hs->beta, hs->t0, hs->charge, hs->edep};
     const size_t n = (size_t)n_seg, npad = (n + 63) & ~(size_t)63;
     if (11 * npad > ctx->seg_cap) {
@@ -582,15 +605,6 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         CU(cudaMalloc(&ctx->d_seg, std::max<size_t>(1, 11 * npad) * sizeof(float)));
         ctx->seg_cap = 11 * npad;
     }
-    const float *dp[11];
-    for (int k = 0; k < 11; ++k) {
-        dp[k] = src[k] ? ctx->d_seg + k * npad : nullptr;
-        if (src[k] && n) CU(cudaMemcpyAsync(ctx->d_seg + k * npad, src[k], n * sizeof(float), cudaMemcpyHostToDevice, st));
-    }
-    c8ph_segments ds{};
-    ds.size = sizeof(ds);
-    ds.x = dp[0]; ds.y = dp[1]; ds.z = dp[2]; ds.dx = dp[3]; ds.dy = dp[4]; ds.dz = dp[5];
-    ds.len = dp[6]; ds.beta = dp[7]; ds.t0 = dp[8]; ds.charge = dp[9]; ds.edep = dp[10];
     // device outputs in one arena: counters | hist | tel_counts | photon_weight | photons
     const DevDet &det = ctx->det;
     const size_t n_hist = ho->hist ? (det.cam_enabled ? (size_t)det.cam_rows * det.cam_cols * det.n_tbins : (size_t)det.hist_nx * det.hist_ny) : 0;
@@ -609,7 +623,8 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         ctx->out_cap = total;
     }
     char *b = (char *)ctx->d_out;
-    CU(cudaMemsetAsync(b, 0, off_w, st));                   // counters, hist, tel_counts
+    cudaStream_t s_in = ctx->st_h2d, s_run = ctx->st_run, s_out = ctx->st_d2h;
+    CU(cudaMemsetAsync(b, 0, off_w, s_run));                // counters, hist, tel_counts
     c8ph_outputs dout{};
     dout.size = sizeof(dout);
     dout.counters = (uint64_t *)b;
@@ -618,22 +633,58 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
     dout.photon_weight = (ho->photon_weight && cap) ? (float *)(b + off_w) : nullptr;
     dout.photons = cap ? (c8ph_photon *)(b + off_ph) : nullptr;
     dout.photon_capacity = (int64_t)cap;
-    KArgs a{};
-    int rc = make_args(ctx, &ds, n_seg, base, p, seed, &dout, a, st);
-    if (rc) return rc;
-    if (n_seg > 0) { rc = launch(ctx, a, st); if (rc) return rc; }
-    uint64_t cnt[C8PH_N_COUNTERS];
-    CU(cudaMemcpyAsync(cnt, dout.counters, sizeof cnt, cudaMemcpyDeviceToHost, st));
-    if (n_hist) CU(cudaMemcpyAsync(ho->hist, dout.hist, n_hist * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (n_tel) CU(cudaMemcpyAsync(ho->tel_counts, dout.tel_counts, n_tel * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    const size_t written = (size_t)std::min<uint64_t>(cnt[C8PH_CNT_WRITTEN], cap);
-    if (written) {
-        CU(cudaMemcpyAsync(ho->photons, dout.photons, written * sizeof(c8ph_photon), cudaMemcpyDeviceToHost, st));
-        if (dout.photon_weight) CU(cudaMemcpyAsync(ho->photon_weight, dout.photon_weight, written * sizeof(float), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+
+    // chunk plan: at most kMaxChunks, at least 2^18 segments each (keeps the persistent grid busy)
+    int n_chunks = (int)std::min<size_t>(kMaxChunks, std::max<size_t>(1, n / (1u << 18)));
+    if (!cap) n_chunks = 1;                                 // nothing to overlap without a photon list
+    const size_t chunk = ((n + n_chunks - 1) / n_chunks + 63) & ~(size_t)63;
+    bool first = true;
+    for (int c = 0; c < n_chunks; ++c) {
+        const size_t lo = std::min(n, (size_t)c * chunk), hi = std::min(n, lo + chunk);
+        for (int k = 0; k < 11; ++k)
+            if (src[k] && hi > lo)
+                CU(cudaMemcpyAsync(ctx->d_seg + k * npad + lo, src[k] + lo, (hi - lo) * sizeof(float), cudaMemcpyHostToDevice, s_in));
+        CU(cudaEventRecord(ctx->ev_in[c], s_in));
+        CU(cudaStreamWaitEvent(s_run, ctx->ev_in[c], 0));
+        c8ph_segments ds{};
+        ds.size = sizeof(ds);
+        const float **dp[11] = {&ds.x, &ds.y, &ds.z, &ds.dx, &ds.dy, &ds.dz, &ds.len, &ds.beta, &ds.t0, &ds.charge, &ds.edep};
+        for (int k = 0; k < 11; ++k) *dp[k] = src[k] ? ctx->d_seg + k * npad + lo : nullptr;
+        KArgs a{};
+        int rc = make_args(ctx, &ds, (int64_t)(hi - lo), base + (int64_t)lo, p, seed, &dout, a, s_run);
+        if (rc) { cudaDeviceSynchronize(); return rc; }
+        a.run.local_base = (uint32_t)lo;
+        if (hi > lo) {
+            CU(cudaMemsetAsync(ctx->d_cursor, 0, sizeof(unsigned long long), s_run));
+            if (first) CU(cudaEventRecord(ctx->ev0, s_run));
+            first = false;
+            cudaError_t e = launch_emit_propagate(a, ctx->n_sm, s_run);
+            if (e != cudaSuccess) { cudaDeviceSynchronize(); return cuda_fail(ctx, e, "emit_propagate launch"); }
+            ctx->launches++;
+        }
+        CU(cudaMemcpyAsync(&ctx->h_written[c], &dout.counters[C8PH_CNT_WRITTEN], sizeof(unsigned long long), cudaMemcpyDeviceToHost, s_run));
+        CU(cudaEventRecord(ctx->ev_run[c], s_run));
     }
-    if (ho->counters) memcpy(ho->counters, cnt, sizeof cnt);
+    if (!first) { CU(cudaEventRecord(ctx->ev1, s_run)); ctx->timed = true; }
+    // photons: as soon as a chunk's kernel is done its records [written before, written after) go home
+    size_t done = 0;
+    for (int c = 0; c < n_chunks && cap; ++c) {
+        CU(cudaEventSynchronize(ctx->ev_run[c]));
+        const size_t w = (size_t)std::min<unsigned long long>(ctx->h_written[c], cap);
+        if (w > done) {
+            CU(cudaMemcpyAsync(ho->photons + done, dout.photons + done, (w - done) * sizeof(c8ph_photon), cudaMemcpyDeviceToHost, s_out));
+            if (dout.photon_weight) CU(cudaMemcpyAsync(ho->photon_weight + done, dout.photon_weight + done, (w - done) * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+            done = w;
+        }
+    }
+    // the small results follow the last kernel on the run stream (counters through pinned memory)
+    uint64_t *cnt = reinterpret_cast<uint64_t *>(ctx->h_written + kMaxChunks);
+    CU(cudaMemcpyAsync(cnt, dout.counters, C8PH_N_COUNTERS * sizeof(uint64_t), cudaMemcpyDeviceToHost, s_run));
+    if (n_hist) CU(cudaMemcpyAsync(ho->hist, dout.hist, n_hist * sizeof(float), cudaMemcpyDeviceToHost, s_run));
+    if (n_tel) CU(cudaMemcpyAsync(ho->tel_counts, dout.tel_counts, n_tel * sizeof(float), cudaMemcpyDeviceToHost, s_run));
+    CU(cudaStreamSynchronize(s_run));
+    CU(cudaStreamSynchronize(s_out));
+    if (ho->counters) memcpy(ho->counters, cnt, C8PH_N_COUNTERS * sizeof(uint64_t));
     return C8PH_OK;
 }
 

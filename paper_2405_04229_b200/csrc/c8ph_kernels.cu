@@ -562,7 +562,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 const double pn = 1.0 / sqrt(Px * Px + Py * Py + Pz * Pz);
                 Px *= pn; Py *= pn; Pz *= pn;
                 const unsigned long long gid = (unsigned long long)(run.seg_id_base + i);
-                me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); mc.local = (uint32_t)i;
+                me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); mc.local = run.local_base + (uint32_t)i;
                 // local vertical and height at A and at the midpoint
                 double rx = 0.0, ry = 0.0, rz = 1.0, rA = 1.0, hA, h_mid;
                 const double mx = Ax + 0.5 * L * Px, my = Ay + 0.5 * L * Py, mz = Az + 0.5 * L * Pz;
