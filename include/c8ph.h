@@ -43,7 +43,9 @@ enum {
 
 typedef struct c8ph_ctx c8ph_ctx;   /* opaque; owns only what it creates (tables, detector grids) */
 
-/* Create / destroy a context bound to one CUDA device.  Not thread-safe per context. */
+/* Create / destroy a context bound to one CUDA device.  Not thread-safe per context.
+ * Validation switch: with C8PH_FORCE_BRUTE=1 in the environment at create time every telescope
+ * search of the context walks all telescopes instead of the uniform grids (same results, slow). */
 int c8ph_create(c8ph_ctx **out, int cuda_device);
 int c8ph_destroy(c8ph_ctx *ctx);
 /* Text of the last error of this context (or of create, if ctx == NULL); never NULL. */
@@ -96,7 +98,9 @@ typedef struct {
     double t_ref_ns;                 /* photon times are reported relative to t_ref               */
     float t_bin_ns;
 } c8ph_detector;
-/* Copies the telescope list and builds the uniform-grid accelerators (synchronous). */
+/* Copies the telescope list and builds the two uniform-grid accelerators on the host (per cell: the
+ * candidate telescopes sorted by a lower-bound key, the smallest key, an accept bound); synchronous.
+ * LV2 margins up to 64 m are covered by the grid.                                                */
 int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *det);
 
 /* ---- run parameters --------------------------------------------------------------------------- */
@@ -165,9 +169,13 @@ int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *segments, int64_t n_
                         int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
                         const c8ph_outputs *out, void *stream);
 
-/* Same path with HOST buffers (pinned or pageable): copies the segments in, zeroes device
- * outputs, runs, copies hist / tel_counts / counters / the first min(written, capacity) photons
- * back into the HOST buffers of `out` (which are overwritten, not accumulated); synchronous.    */
+/* Same path with HOST buffers (pinned or pageable; pinned for full overlap): the segments are split
+ * into up to 16 chunks that are pipelined over three internal streams (H2D of chunk c+1 | kernel of
+ * chunk c | D2H of the photons chunk c-1 wrote), each chunk with seg_id_base + its offset, so the
+ * result is that of one call.  hist / tel_counts / counters / the first min(written, capacity)
+ * photons are copied into the HOST buffers of `out` (overwritten, not accumulated); photon.seg is
+ * the segment index within the whole call.  Synchronous; device scratch is owned by the context
+ * and grown on demand.                                                                          */
 int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, int64_t n_segments,
                              int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
                              const c8ph_outputs *host_out);
