@@ -40,7 +40,7 @@ UNIT = "photons/s"
 
 # Algorithmic thread-instructions per unit of each stage of the fused kernel, audited from the SASS
 # of k_emit_propagate<CHERENKOV,TABLE,SPH,SPEC=1> with ncu's per-instruction execution counts
-# (DESIGN.md section 5 "Roofline"; profiles/r1_cfg4_sass_classes.md): the instructions every unit of a
+# (DESIGN.md section 5 "Roofline"; profiles/r1_cfg4_final.md): the instructions every unit of a
 # stage executes exactly once on its way through.  What is NOT counted: telescope candidates that turn
 # out to miss, LV2 list searches, queue drains of partly filled warps, idle lanes.
 I_ALG = {
@@ -51,6 +51,12 @@ I_ALG = {
     "in_grid": 6.0,       # a15: bin address + RED.ADD.F32
     "tel_hit": 193.0,     # a13/a14/a16: queue push 29 + finish 164 (time, arrival direction, sphere search, record)
 }
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_emit_propagate launch on the N=1 workload, from the
+# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.586 GB + 5.995 GB).  Reported as
+# `roofline.traffic` only when the run is that workload (cfg4, 1e7 segments); otherwise null.
+NCU_TRAFFIC_BYTES_CFG4 = 0.586090240e9 + 5.995012e9
 
 
 def _stage_population(cnt: dict) -> dict:
@@ -285,7 +291,9 @@ def run_ours(args):
             pass
     alg_bytes = algorithmic_bytes(cnt, ctx.n_hist(), ctx._n_tel)
     roofline = {"bound": "alu", "kernel": "k_emit_propagate", "achieved": achieved, "peak": peak,
-                "unit": "Ginst/s", "frac": achieved / peak, "traffic": None,
+                "unit": "Ginst/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES_CFG4 if (k == 4 and n == W.FULL_SEGMENTS[4]) else None,
+                "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic bytes = %.4g" % alg_bytes,
                 "peak_def": f"{n_sm} SMs x 4 schedulers x 32 lanes x clocks.max.sm {sm_max:.0f} MHz (issue slots)",
                 "frac_at_measured_clock": (achieved / (n_sm * 128 * clocks["sm_mhz"] * 1e-3)) if clocks.get("sm_mhz") else None,
                 "alg_inst_per_photon": i_alg / max(cnt["emitted"], 1),
