@@ -5,26 +5,27 @@
 //    ground grid / telescope spheres / camera -> compacted photon list.   (thesis sec. 5.3)
 //  * k_build_table: the interpolation-tracing correction table (thesis sec. 4.4.1).
 //
-// Design (DESIGN.md has the long version):
+// Design (DESIGN.md section 5 has the long version and the measurements behind each choice):
 //  - persistent grid, one warp owns a group of segments taken from a global cursor; the 32 lanes
 //    first PREPARE up to 32 segments in parallel, one per lane, in fp64 (yield, bunch count, LV1,
-//    Rodrigues basis, axis-landing anchor), then the warp walks the emitting segments and the
-//    lanes stride over the photons of one segment (photon state lives in registers only; the
-//    thesis' shared-memory photon buffer, is not needed);
+//    Rodrigues basis, axis-landing anchor) and park them in the warp's slots of a global scratch
+//    array; then the warp walks the emitting segments and the lanes stride over the photons of one
+//    segment, photon state in registers only;
 //  - per-photon arithmetic is fp32 in cancellation-free "anchor + offset" form: the landing point
 //    of the particle axis and its clock are computed once per segment in fp64, the photon only
 //    adds small offsets, which keeps bin flips against the fp64 oracle below 1e-4;
 //  - Philox4x32-10 keyed on (seed; segment id, photon index): results are independent of grid
 //    size, segment order and batching;
-//  - n(h) (and for the layered sum the mid-layer n and overburden steps) are staged once per CTA
-//    in shared memory with one TMA bulk copy each (cp.async.bulk + mbarrier): lanes of a warp emit
-//    from the same short segment, so their n(h) reads fall in 1-3 adjacent words (broadcast);
+//  - n(h) through L1 (lanes of a warp emit from one short segment: one cache line); only the
+//    layered-sum variant stages n(h) and the overburden steps per CTA in shared memory with one
+//    TMA bulk copy each (cp.async.bulk + mbarrier);
 //  - the correction table (float4 texels dd, dt, X_slant, tau_aer) is read with 4 x LDG.128
-//    through L1: the lanes of a warp share (height, zenith) to within the Cherenkov angle, so they
-//    hit a handful of cache lines;
-//  - survivors are compacted by warp ballot into a per-warp shared-memory stage and flushed 32
-//    records (1 KiB) at a time with one cursor atomic per flush; the ground histogram takes one
-//    RED.ADD.F32 per landed photon into the L2-resident grid.
+//    through L1: the lanes of a warp share (height, zenith) to within the Cherenkov angle;
+//  - telescope searches on uniform grids whose cells list candidates sorted by a lower-bound key
+//    (one 4 B load decides "nothing in reach"); the few photons that pass the pre-test are queued
+//    in a per-warp shared-memory ring and a full warp finishes 32 of them at a time (arrival time
+//    and direction, exact sphere test, ballot-ranked record store);
+//  - the ground histogram takes one RED.ADD.F32 per binned photon into the L2-resident grid.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <cstdint>
@@ -361,7 +362,7 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2,
 // roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present):
 // the host picks it when the call matches (launch_emit_propagate); SPEC = 0 reads the switches.
 template <int EMIT, int TRACE, bool SPH, int SPEC>
-__global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 1 : kMinBlocks)
+__global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 2 : kMinBlocks)
 k_emit_propagate(const __grid_constant__ KArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -378,8 +379,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 
     // ---- shared memory carve-up: [n(h) tables] | per-warp candidate queue (SoA, kQueue entries)
     float *s_eta = reinterpret_cast<float *>(smem_raw);
-    float *s_mid = s_eta + (STAGED ? atm.n_pad : 0);
-    float *s_dxv = s_mid + (STAGED ? atm.n_pad : 0);
+    float *s_dxv = s_eta + (STAGED ? atm.n_pad : 0);
     float *s_end = s_dxv + (STAGED ? atm.n_pad : 0);
     float4 *s_q = reinterpret_cast<float4 *>(s_end) + warp * (kQueue * 4);   // s_q[slot * 4 + part]
     __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
@@ -393,9 +393,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         if (threadIdx.x == 0) {
             mbar_init(&s_bar, 1);
             const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
-            mbar_expect_tx(&s_bar, bytes * 3u);
+            mbar_expect_tx(&s_bar, bytes * 2u);
             bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
-            bulk_g2s(s_mid, atm.eta_mid, bytes, &s_bar);
             bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
         }
         __syncthreads();
@@ -844,9 +843,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             const float n_l = 1.f + eta_l;
                             const float ql = fmaf(n_l, n_l, -K * K);
                             ok = ok && (ql > 0.f);
-                            const float r_l = rsqrtf(ql);
+                            const float r_l = rsqrt_fast(ql);
                             const float dq = (eta_e - eta_l) * (2.f + eta_e + eta_l);       // q_e - q_l
-                            const float dr = dq * r_l * r_l * r_e * r_e * __frcp_rn(r_l + r_e); // r_l - r_e
+                            const float dr = dq * r_l * r_l * r_e * r_e * rcp_fast(r_l + r_e);  // r_l - r_e
                             aX = fmaf(thick * K, dr, aX);
                             aT = fmaf(thick, fmaf(n_l * n_l, dr, r_e * (fmaf(eta_l, eta_l, 2.f * eta_l) - eta_e)), aT);
                             aS = fmaf(dxv_l * n_l, r_l, aS);
@@ -857,7 +856,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         } else {
                             if (fre > 0.f)
                                 layer(fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke]);
-                            for (int k = ke - 1; k > kg; --k) layer(s_mid[k], atm.dh, s_dxv[k]);
+                            for (int k = ke - 1; k > kg; --k) layer(0.5f * (s_eta[k] + s_eta[k + 1]), atm.dh, s_dxv[k]);   // n at the layer mid height
                             layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
                         }
                         if (!ok) { pkB += 1u; break; }
@@ -1093,7 +1092,7 @@ void segment_slot_pointers(void *base, int n_sm, DevRun &run)
 
 size_t emit_smem_bytes(const KArgs &a)
 {
-    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * 3u : 0u;
+    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * 2u : 0u;
     return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
 }
 
