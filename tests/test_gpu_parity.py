@@ -118,6 +118,27 @@ def test_telescope_grids_equal_brute_force_search(monkeypatch):
 
 
 
+def test_irregular_array_varied_radii_and_heights(monkeypatch):
+    """Row f1 (non-lattice arrays): 300 telescopes at random positions with radii 2-12 m and centres up
+    to 15 m above / below the observation level, the 1 PeV shower of cfg4 at 2 000 segments and the
+    inclined one of cfg2 at 20 000.  Against the oracle's brute force, and grid == search-all."""
+    rng = np.random.default_rng(4242)
+    tel = np.zeros((300, 4), dtype=np.float32)
+    tel[:, 0], tel[:, 1] = rng.uniform(-450.0, 450.0, 300), rng.uniform(-450.0, 450.0, 300)
+    tel[:, 2], tel[:, 3] = rng.uniform(-15.0, 15.0, 300), rng.uniform(2.0, 12.0, 300)
+    for k, n in ((4, 2000), (2, 20000)):
+        cfg = W.make_config(k, n_segments=n)
+        cfg["detector"]["tel_xyzr"] = tel.copy()
+        ora, gpu, rep = _both(cfg)
+        assert gpu["counters"]["tel_hit"] > 2000 and gpu["counters"]["lv2"] >= 0
+        monkeypatch.setenv("C8PH_FORCE_BRUTE", "1")
+        ctx = api.setup_context(cfg)
+        brute = api.run_config(cfg, ctx=ctx)
+        ctx.close()
+        monkeypatch.setenv("C8PH_FORCE_BRUTE", "0")
+        assert brute["counters"] == gpu["counters"] and np.array_equal(brute["tel_counts"], gpu["tel_counts"])
+
+
 # ---------------------------------------------------------------------------------- edge cases
 def test_empty_and_tiny_inputs():
     cfg = W.make_config(0, n_segments=1)
