@@ -178,6 +178,12 @@ __device__ __forceinline__ float sqrt_fast(float x)
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float exp2_fast(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float rsqrt_fast(float x)
 {
     float y;
@@ -351,6 +357,15 @@ __device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float u
     }
     if (bd > p * p * (1.0f / 3.0f)) return -1;
     return best;
+}
+
+// a9 for a segment without a valid axis anchor (P_z >= -0.05: near-horizontal or up-going particle):
+// plain Eq. 3.3 from the emission point.  Rare; kept out of line so the common path does not pay.
+__device__ __noinline__ void line_general(const SegCold *sc, float s, float D, float Px, float Py, float ux, float uy,
+                                          float &ox, float &oy)
+{
+    ox = fmaf(D, ux, fmaf(s, Px, sc->Ax));
+    oy = fmaf(D, uy, fmaf(s, Py, sc->Ay));
 }
 
 // per-warp event counters kept in shared memory (u64), flushed to the global counters at the end
@@ -684,6 +699,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         }
                     } else {
                         mc.Tg = (float)(t0 - det.t_ref);
+                        if (has_grid_geom) {                         // bin = floor(x / cell + fb) with G = 0
+                            mc.fbx = (float)(-(double)det.hist_x0 / (double)det.hist_cell);
+                            mc.fby = (float)(-(double)det.hist_y0 / (double)det.hist_cell);
+                        }
                     }
                     copy16(&g_slot[lane].h, &me);
                     copy16(&g_slot[lane].c, &mc);
@@ -739,9 +758,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
                         q = sqrt_fast(bn1 * (2.f + bn1));               // tan(theta_c)
                         cth = rcp_fast(1.f + bn1);                      // cos(theta_c)
-                        wx = cphi * sg.e1x + sphi * sg.e2x;
+                        // M = 2 A A^T - 1 is symmetric with third column -P: e2x = e1y, e1z = -P_x, e2z = -P_y
+                        wx = cphi * sg.e1x + sphi * sg.e1y;
                         wy = cphi * sg.e1y + sphi * sg.e2y;
-                        wz = cphi * sg.e1z + sphi * sg.e2z;
+                        wz = -(cphi * sg.Px + sphi * sg.Py);
                         pqz = fmaf(q, wz, sg.Pz);
                         ux = cth * fmaf(q, wx, sg.Px);
                         uy = cth * fmaf(q, wy, sg.Py);
@@ -772,7 +792,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // a8: up-going / horizontal photons are discarded
                     if (uz >= kUpCut) { pkA += 1u; break; }
                     // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
-                    float xl, yl, ox = 0.f, oy = 0.f;
+                    // (segments without a valid anchor carry G = 0 and the offset is the whole position)
+                    float ox, oy;
                     const float inv_uz = rcp_fast(uz);
                     const float Z = fmaf(s, sg.Pz, sg.Az);
                     const float D = -Z * inv_uz;
@@ -780,12 +801,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         const float zq = -Z * q * rcp_fast(sg.Pz * pqz);
                         ox = zq * (wx * sg.Pz - sg.Px * wz);
                         oy = zq * (wy * sg.Pz - sg.Py * wz);
-                        xl = sg.Gx + ox;
-                        yl = sg.Gy + oy;
                     } else {
-                        xl = fmaf(D, ux, fmaf(s, sg.Px, sc->Ax));
-                        yl = fmaf(D, uy, fmaf(s, sg.Py, sc->Ay));
+                        line_general(sc, s, D, sg.Px, sg.Py, ux, uy, ox, oy);
                     }
+                    const float xl = sg.Gx + ox, yl = sg.Gy + oy;
                     // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
                     // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
                     if (f_lv2) {
@@ -872,19 +891,17 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             tau = Xs * qq * atm.ray_inv_X;
                         }
                         if (f_aer) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
-                        const float T = __expf(-tau);
+                        const float T = exp2_fast(-1.4426950408889634f * tau);
                         if (f_trans == C8PH_TRANS_ROULETTE) {
                             if (!(u01(rn.w) < T)) { pkB += 0x10000u; break; }
                         } else wgt = run.w * T;
                     }
                     // landed: corrected position (dd along the horizontal direction of flight)
                     const float hn2 = ux * ux + uy * uy;
-                    float ehx = 0.f, ehy = 0.f;
-                    if (hn2 >= 1e-18f) { const float ih = rsqrt_fast(hn2); ehx = ux * ih; ehy = uy * ih; }
+                    const float ih = hn2 >= 1e-18f ? rsqrt_fast(hn2) : 0.f;            // vertical photon: no correction
+                    const float ehx = ux * ih, ehy = uy * ih;
                     const float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);         // offset from the anchor
-                    float xg, yg;
-                    if (sg.anchor) { xg = sg.Gx + cx; yg = sg.Gy + cy; }
-                    else { xg = fmaf(dd, ehx, xl); yg = fmaf(dd, ehy, yl); }
+                    const float xg = sg.Gx + cx, yg = sg.Gy + cy;
                     // a14 pre-test: the photon can hit a sphere of its grid cell only if the cell's
                     // smallest key <= 1/|u_z| (inflated for the refraction rotation of the direction); the
                     // load is issued before the binning arithmetic so its latency overlaps
@@ -892,20 +909,16 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     float kmin = CUDART_INF_F;
                     if (f_tel) {
                         const bool brute = f_hit_brute || !f_grid || -uz < det.grid_min_cos;
-                        cell = brute ? -2 : grid_cell(det.hit, xg, yg);
-                        if (cell >= 0) kmin = __ldg(det.hit.kmin + cell);
+                        cell = grid_cell(det.hit, xg, yg);
+                        kmin = __ldg(det.hit.kmin + max(cell, 0));          // cell -1 (outside): never a candidate
+                        if (cell < 0) kmin = CUDART_INF_F;
+                        if (brute) cell = -2;
                     }
                     // a15: ground grid
                     if (has_grid_geom) {
-                        int ix, iy;
-                        if (sg.anchor) {
-                            const float4 fb = *reinterpret_cast<const float4 *>(sc);     // fbx, fby, ibx, iby
-                            ix = __float_as_int(fb.z) + __float2int_rd(fmaf(cx, det.hist_inv_cell, fb.x));
-                            iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, det.hist_inv_cell, fb.y));
-                        } else {
-                            ix = __float2int_rd((xg - det.hist_x0) * det.hist_inv_cell);
-                            iy = __float2int_rd((yg - det.hist_y0) * det.hist_inv_cell);
-                        }
+                        const float4 fb = *reinterpret_cast<const float4 *>(sc);         // fbx, fby, ibx, iby
+                        const int ix = __float_as_int(fb.z) + __float2int_rd(fmaf(cx, det.hist_inv_cell, fb.x));
+                        const int iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, det.hist_inv_cell, fb.y));
                         if ((unsigned)ix < (unsigned)det.hist_nx && (unsigned)iy < (unsigned)det.hist_ny) {
                             pkC += 1u;
                             if (has_hist) atomicAdd(run.out.hist + (iy * det.hist_nx + ix), wgt);
