@@ -909,9 +909,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     float kmin = CUDART_INF_F;
                     if (f_tel) {
                         const bool brute = f_hit_brute || !f_grid || -uz < det.grid_min_cos;
-                        cell = grid_cell(det.hit, xg, yg);
-                        kmin = __ldg(det.hit.kmin + max(cell, 0));          // cell -1 (outside): never a candidate
-                        if (cell < 0) kmin = CUDART_INF_F;
+                        if (f_grid) {
+                            cell = grid_cell(det.hit, xg, yg);
+                            kmin = __ldg(det.hit.kmin + max(cell, 0));      // cell -1 (outside): never a candidate
+                            if (cell < 0) kmin = CUDART_INF_F;
+                        }
                         if (brute) cell = -2;
                     }
                     // a15: ground grid
