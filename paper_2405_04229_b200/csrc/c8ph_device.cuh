@@ -17,7 +17,6 @@ struct DevAtm {
     float f_max;            // (float)(n_nodes - 1)
     const float *eta;       // DEVICE [n_pad] refractivity n-1 at the nodes
     const float *xv;        // DEVICE [n_pad] vertical overburden at the nodes (zeros if none)
-    const float *eta_mid;   // DEVICE [n_pad] refractivity at the cell mid height (layer k = nodes k..k+1)
     const float *dxv;       // DEVICE [n_pad] X_v(node k) - X_v(node k+1)
     double R, h_obs, Rg;    // Earth radius, observation altitude, R + h_obs
     float eta_g;            // refractivity at the observation level

@@ -23,7 +23,7 @@ struct c8ph_ctx {
     DevAtm atm{};
     bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
     double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
-    float *d_eta = nullptr, *d_xv = nullptr, *d_mid = nullptr, *d_dxv = nullptr;
+    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr;
     // table
     bool have_table = false;
     DevTable tab{};
@@ -112,7 +112,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
 {
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
-    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_g_kacc);
@@ -163,24 +163,22 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
     if (d->model == C8PH_ATM_SPHERICAL && !(d->earth_radius_m > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: earth_radius");
     const int n = (int)eta.size();
     const int n_pad = (n + 3) & ~3;
-    std::vector<float> mid(n_pad, 0.f), dxv(n_pad, 0.f), eta_p(n_pad, eta.back()), xv_p(n_pad, xv.back());
+    std::vector<float> dxv(n_pad, 0.f), eta_p(n_pad, eta.back()), xv_p(n_pad, xv.back());
     for (int k = 0; k < n; ++k) { eta_p[k] = eta[k]; xv_p[k] = xv[k]; }
     for (int k = 0; k + 1 < n; ++k) {
-        mid[k] = (float)(0.5 * ((double)eta[k] + (double)eta[k + 1]));   // Listing 4.1 at the cell mid height
         dxv[k] = (float)((double)xv[k] - (double)xv[k + 1]);
     }
-    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_mid); dfree(ctx->d_dxv);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv);
     const size_t bytes = (size_t)n_pad * sizeof(float);
     CU(cudaMalloc(&ctx->d_eta, bytes)); CU(cudaMalloc(&ctx->d_xv, bytes));
-    CU(cudaMalloc(&ctx->d_mid, bytes)); CU(cudaMalloc(&ctx->d_dxv, bytes));
+    CU(cudaMalloc(&ctx->d_dxv, bytes));
     CU(cudaMemcpy(ctx->d_eta, eta_p.data(), bytes, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_xv, xv_p.data(), bytes, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(ctx->d_mid, mid.data(), bytes, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_dxv, dxv.data(), bytes, cudaMemcpyHostToDevice));
     DevAtm &a = ctx->atm;
     a.model = d->model; a.n_nodes = n; a.n_pad = n_pad;
     a.h0 = (float)h0; a.dh = (float)dh; a.inv_dh = (float)(1.0 / dh); a.h_top = (float)(h0 + dh * (n - 1)); a.f_max = (float)(n - 1);
-    a.eta = ctx->d_eta; a.xv = ctx->d_xv; a.eta_mid = ctx->d_mid; a.dxv = ctx->d_dxv;
+    a.eta = ctx->d_eta; a.xv = ctx->d_xv; a.dxv = ctx->d_dxv;
     a.R = d->earth_radius_m; a.h_obs = d->h_obs_m; a.Rg = (double)d->earth_radius_m + (double)d->h_obs_m;
     a.eta_g = (float)lerp_table(eta, h0, dh, d->h_obs_m);
     ctx->eta_span = 0.0;

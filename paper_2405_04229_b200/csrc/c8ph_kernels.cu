@@ -47,7 +47,6 @@ constexpr int kMaxBlocksPerSM = C8PH_MAX_BLOCKS_PER_SM;
 constexpr int kMinBlocks = C8PH_MIN_BLOCKS;                    // resident CTAs per SM the register budget is set for
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
-constexpr double kAlpha = 1.0 / 137.035999;
 constexpr float kUpCut = -1.0e-6f;               // drop photons with u_z >= kUpCut
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
