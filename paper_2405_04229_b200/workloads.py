@@ -284,8 +284,13 @@ def make_config(k: int, n_segments: Optional[int] = None, rng_seed: Optional[int
         table = dict(_TABLE)
         par.update(emit="fluorescence", trace="table", trans="roulette", write="tel",
                    line_nm=lines, line_cdf=cdf.astype(np.float32), lv2=True, lv2_margin_m=25.0)
-        # time window: first light from the top of the shower reaches the camera
-        det["t_ref_ns"] = float(np.floor(seg["t0"].min() / 100.0) * 100.0)
+        # time window (1000 x 100 ns): opens 2 us before the light of the earliest 5 % of the segments
+        # can reach the aperture (segment clock + straight distance / c), so the bulk of the shower
+        # falls inside it at any segment count
+        tel0 = det["tel_xyzr"][0].astype(np.float64)
+        dist = np.sqrt((seg["x"] - tel0[0]) ** 2 + (seg["y"] - tel0[1]) ** 2 + (seg["z"] - tel0[2]) ** 2)
+        first = np.percentile(seg["t0"].astype(np.float64) + dist / _C, 5.0)
+        det["t_ref_ns"] = float(np.floor((first - 2000.0) / 100.0) * 100.0)
     elif k == 4:
         atm = make_atmosphere("spherical_5layer", h_obs=0.0, rayleigh=True)
         seg = _shower_segments(rng, n, atm, 20.0, 0.0, 580.0, 70.0, 80.0, 4.0, 1.0, 20.0, 1.0, 6.0)

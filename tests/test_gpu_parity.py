@@ -302,3 +302,47 @@ def test_cfg4_full_size_sampled_windows_and_invariants():
         k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
         k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
+
+
+def test_cfg3_full_size_against_the_whole_oracle():
+    """BASELINE configs[3] at its full 1e6 segments (forced-cone fluorescence: ~1.7e5 photons, which
+    the oracle runs completely): counters, camera histogram and every photon record."""
+    cfg = W.make_config(3)
+    assert len(cfg["segments"]["x"]) == W.FULL_SEGMENTS[3]
+    ora, gpu, rep = _both(cfg, capacity=1 << 20)
+    assert gpu["counters"]["segments"] == 1_000_000 and gpu["counters"]["emitted"] > 1e5
+    assert gpu["counters"]["cam_hit"] > 1000
+
+
+def test_cfg2_full_size_sampled_windows_and_invariants():
+    """BASELINE configs[2] at its full 1e6 segments (1.4e8 bunches of weight 5 after LV1): whole-run
+    identities plus photon-by-photon comparison with the oracle on sampled segment windows."""
+    n = W.FULL_SEGMENTS[2]
+    cfg = W.make_config(2)
+    ctx = api.setup_context(cfg)
+    seg = api.segments_to_device(cfg["segments"])
+    out = api.alloc_device_outputs(ctx, 4_000_000, False)
+    ctx.emit_propagate(seg, n, 0, cfg["params"], cfg["seed"], out)
+    torch.cuda.synchronize()
+    cnt = {k: int(v) for k, v in zip(api.COUNTER_NAMES, out["counters"].cpu().numpy())}
+    assert cnt["segments"] == n and cnt["overflow"] == 0 and cnt["clipped"] == 0
+    assert cnt["segments"] >= cnt["seg_below_threshold"] + cnt["seg_lv1"] + cnt["seg_emitting"]
+    assert cnt["emitted"] == cnt["upgoing"] + cnt["lv2"] + cnt["table_range"] + cnt["roulette"] + cnt["landed"]
+    assert cnt["seg_lv1"] > 0.2 * n and cnt["lv2"] > 0.5 * cnt["emitted"] and cnt["emitted"] > 1e8
+    w = float(cfg["params"]["bunch_weight"])
+    assert int(round(out["tel_counts"].double().sum().item() / w)) == cnt["tel_hit"] == cnt["written"]
+    rec_all = out["photons"][:cnt["written"]]
+    ph_seg = rec_all.view(torch.int32)[:, 6]
+    for lo, hi in ((0, 3000), (500_123, 504_000), (n - 2500, n)):
+        m = (ph_seg >= lo) & (ph_seg < hi)
+        rec = rec_all[m].cpu().numpy().view(api.PHOTON_DTYPE).reshape(-1).copy()
+        rec["seg"] -= lo
+        sub = copy.deepcopy(cfg)
+        sub["segments"] = W.slice_segments(cfg["segments"], lo, hi)
+        sub["seg_id_base"] = lo
+        ora = O.run(sub)
+        win = api.run_config(sub, ctx=ctx)
+        parity.compare(sub, ora, win)
+        k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
+        k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
+        assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
