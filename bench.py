@@ -158,7 +158,7 @@ def _oracle_setup(cfg):
     return cores
 
 
-def cpu_baseline(cfg, target_s: float = 12.0) -> dict:
+def cpu_baseline(cfg, target_s: float = 20.0) -> dict:
     cores = _oracle_setup(cfg)
     n_total = len(cfg["segments"]["x"])
     n0 = min(n_total, 400)

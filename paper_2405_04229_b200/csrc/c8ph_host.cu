@@ -465,6 +465,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     if (!s || s->size != sizeof(c8ph_segments) || !p || p->size != sizeof(c8ph_params) || !o || o->size != sizeof(c8ph_outputs))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: NULL struct or size mismatch");
     if (n_seg < 0 || base < 0) return fail(ctx, C8PH_E_ARG, "emit_propagate: negative n_segments / seg_id_base");
+    if (n_seg > 0x7FFFFFFFll) return fail(ctx, C8PH_E_ARG, "emit_propagate: more than 2^31-1 segments per call (photon records carry a 32-bit segment index); split the call");
     if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "emit_propagate: atmosphere not initialised");
     if (!ctx->have_det) return fail(ctx, C8PH_E_STATE, "emit_propagate: detector not set");
     if (n_seg > 0 && (!s->x || !s->y || !s->z || !s->dx || !s->dy || !s->dz || !s->len || !s->beta || !s->t0 || !s->charge))
