@@ -7,6 +7,7 @@ the benchmark configuration is checked on sampled segment windows plus size-inde
 properties.
 """
 import copy
+import os
 import math
 
 import numpy as np
@@ -346,3 +347,28 @@ def test_cfg2_full_size_sampled_windows_and_invariants():
         k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
         k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
+
+
+def _thesis_array(golden_dir, name):
+    return np.loadtxt(os.path.join(golden_dir, name), comments="#", dtype=np.float32).reshape(-1, 4)
+
+
+@pytest.mark.parametrize("name,n_tel", [("telescope_array_1.txt", 13), ("telescope_array_2.txt", 180)])
+def test_thesis_model_arrays(golden_dir, monkeypatch, name, n_tel):
+    """Row f1: the thesis' own model arrays (Appendix B.3; fixtures parsed from PAPER.md by
+    tests/golden/make_telescope_arrays.py): 13 telescopes of radius 12 / 23 m and 180 of radius
+    2.1 / 5.8 / 11.1 m, centres 5-75 m above the observation level, non-lattice.  cfg4's shower
+    (vertical-ish) and cfg2's (60 deg zenith) against the oracle's brute force, and grid == search-all."""
+    tel = _thesis_array(golden_dir, name)
+    assert tel.shape == (n_tel, 4)
+    for k, n in ((4, 3000), (2, 30000)):
+        cfg = W.make_config(k, n_segments=n)
+        cfg["detector"]["tel_xyzr"] = tel.copy()
+        ora, gpu, rep = _both(cfg)
+        assert gpu["counters"]["tel_hit"] > 500
+        monkeypatch.setenv("C8PH_FORCE_BRUTE", "1")
+        ctx = api.setup_context(cfg)
+        brute = api.run_config(cfg, ctx=ctx)
+        ctx.close()
+        monkeypatch.setenv("C8PH_FORCE_BRUTE", "0")
+        assert brute["counters"] == gpu["counters"] and np.array_equal(brute["tel_counts"], gpu["tel_counts"])

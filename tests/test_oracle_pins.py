@@ -513,3 +513,24 @@ def test_forced_cone_is_unbiased_in_margin():
         hits.append(res["counters"]["tel_hit"])
     assert hits[0] > 200
     assert abs(hits[0] - hits[1]) < 5 * math.sqrt(hits[0] + hits[1])
+
+
+def test_thesis_model_array_fixtures(golden_dir):
+    """Appendix B.3 layouts as parsed into tests/golden: counts, radii classes, and an
+    oracle run of cfg4's shower on Array 1 whose telescope hits obey the bounding-sphere definition."""
+    a1 = np.loadtxt(os.path.join(golden_dir, "telescope_array_1.txt"), comments="#").reshape(-1, 4)
+    a2 = np.loadtxt(os.path.join(golden_dir, "telescope_array_2.txt"), comments="#").reshape(-1, 4)
+    assert a1.shape == (13, 4) and sorted(set(a1[:, 3])) == [12.0, 23.0] and (a1[:, 3] == 23.0).sum() == 4
+    assert a2.shape == (180, 4) and sorted(set(a2[:, 3])) == [2.1, 5.8, 11.1]
+    assert [(a2[:, 3] == r).sum() for r in (11.1, 5.8, 2.1)] == [4, 56, 120]
+    cfg = W.make_config(4, n_segments=300)
+    cfg["detector"]["tel_xyzr"] = a1.astype(np.float32)
+    res = O.run(cfg, record=True)
+    ph = res["photons"]
+    hit = ph[(ph["status"] == O.ST_LANDED) & (ph["tel"] >= 0)]
+    assert len(hit) > 100 and res["counters"]["tel_hit"] == len(hit)
+    c = a1[hit["tel"]]
+    d = np.stack([c[:, 0] - hit["x"], c[:, 1] - hit["y"], c[:, 2]], axis=1)
+    u = np.stack([hit["ux"], hit["uy"], hit["uz"]], axis=1)
+    m2 = (d ** 2).sum(1) - ((d * u).sum(1)) ** 2
+    assert np.all(m2 <= c[:, 3] ** 2 * (1 + 1e-9))
