@@ -93,7 +93,22 @@ struct DevRun {
     int segs_per_grab;              // segments one warp prepares per grab (1..32)
 };
 
+// Constants every photon reads, copied by the host from the structs below into 16-byte groups in
+// the order of use, so the kernel fetches them with few wide constant loads.
+struct alignas(16) HotConst {
+    uint2 key[10];                                      // Philox round keys (k0, k1) per round
+    float eta_h0, eta_inv_dh, eta_fmax; int eta_kmax;   // n(h) lookup: origin, 1/dh, n_nodes-1, n_nodes-2
+    const float *eta; float il1, dil;                   // n(h) nodes; 1/lambda_min, 1/lambda_min - 1/lambda_max
+    float box_x0, box_x1, box_y0, box_y1;               // LV2 keep-box
+    float lv2_margin, r_max, grid_min_cos, hit_infl;
+    float ray_lambda, ray_k, w, pad0;                   // ray_k = log2(e) / X_R
+    float hit_x0, hit_y0, hit_inv_cs; int hit_nx;       // hit grid
+    int hit_ny; float hist_inv_cell; int hist_nx, hist_ny;
+    const float *hit_kmin; float *hist;
+};
+
 struct KArgs {
+    HotConst hc;
     DevAtm atm;
     DevTable tab;
     DevDet det;

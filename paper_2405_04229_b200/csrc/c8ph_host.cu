@@ -546,6 +546,18 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     const long long warps = (long long)ctx->n_sm * 2 * 8;
     long long g = n_seg / (warps * 4);
     r.segs_per_grab = (int)std::min<long long>(32, std::max<long long>(1, g));
+    {
+        HotConst &h = a.hc;
+        for (int k = 0; k < 10; ++k) h.key[k] = make_uint2(r.key0[k], r.key1[k]);
+        h.eta_h0 = a.atm.h0; h.eta_inv_dh = a.atm.inv_dh; h.eta_fmax = a.atm.f_max; h.eta_kmax = a.atm.n_nodes - 2;
+        h.eta = a.atm.eta; h.il1 = r.il1; h.dil = r.il1 - r.il2;
+        h.box_x0 = r.box_x0; h.box_x1 = r.box_x1; h.box_y0 = r.box_y0; h.box_y1 = r.box_y1;
+        h.lv2_margin = r.lv2_margin; h.r_max = a.det.r_max; h.grid_min_cos = a.det.grid_min_cos; h.hit_infl = r.hit_infl;
+        h.ray_lambda = a.atm.ray_lambda; h.ray_k = (float)(1.4426950408889634 * (double)a.atm.ray_inv_X); h.w = r.w; h.pad0 = 0.f;
+        h.hit_x0 = a.det.hit.x0; h.hit_y0 = a.det.hit.y0; h.hit_inv_cs = a.det.hit.inv_cs; h.hit_nx = a.det.hit.nx;
+        h.hit_ny = a.det.hit.ny; h.hist_inv_cell = a.det.hist_inv_cell; h.hist_nx = a.det.hist_nx; h.hist_ny = a.det.hist_ny;
+        h.hit_kmin = a.det.hit.kmin; h.hist = r.out.hist;
+    }
     if (emit_smem_bytes(a) > 200 * 1024) return fail(ctx, C8PH_E_ARG, "emit_propagate: atmosphere table too large for shared memory");
     return C8PH_OK;
 }

@@ -84,15 +84,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 
 // ---- Philox4x32-10 (Salmon et al.; thesis ref. [66]), round keys precomputed ---------
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               const uint32_t (&k0)[10], const uint32_t (&k1)[10])
+                                               const uint2 (&key)[10])
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
         const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        c0 = hi1 ^ c1 ^ k0[r];
+        c0 = hi1 ^ c1 ^ key[r].x;
         c1 = lo1;
-        c2 = hi0 ^ c3 ^ k1[r];
+        c2 = hi0 ^ c3 ^ key[r].y;
         c3 = lo0;
     }
     return make_uint4(c0, c1, c2, c3);
@@ -383,6 +383,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     __shared__ __align__(8) uint64_t s_bar;
     __shared__ unsigned long long s_cnt[kWarps][WC_N];
 
+    const HotConst &hc = a.hc;
     const DevAtm &atm = a.atm;
     const DevDet &det = a.det;
     const DevRun &run = a.run;
@@ -417,7 +418,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     __syncwarp();
     // n(h) node: shared memory when staged, otherwise through L1 (the lanes of a warp emit from one
     // short segment: 1-3 adjacent words, one cache line)
-    auto eta_node = [&](int k) -> float { return STAGED ? s_eta[k] : __ldg(atm.eta + k); };
+    auto eta_node = [&](int k) -> float { return STAGED ? s_eta[k] : __ldg(hc.eta + k); };
 
     // per-lane event counters of the photon loop, two 16-bit fields per register, flushed to
     // s_cnt before a field can overflow
@@ -592,7 +593,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 }
                 const double cA = Px * rx + Py * ry + Pz * rz;
                 double n_exp = 0.0;
-                const uint4 rs = philox4x32_10(0xFFFFFFFFu, me.id_lo, me.id_hi, 0u, run.key0, run.key1);
+                const uint4 rs = philox4x32_10(0xFFFFFFFFu, me.id_lo, me.id_hi, 0u, hc.key);
                 float e1x, e1y, e1z, e2x, e2y, e2z;
                 mc.aimx = mc.aimy = mc.aimz = mc.omc = 0.f;
                 if (EMIT == C8PH_EMIT_CHERENKOV) {
@@ -736,16 +737,16 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 const int j = it * 32 + lane;
                 // one photon per lane; every cut leaves through the same exit (one reconvergence point)
                 if (j < sg.N) do {
-                    const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, run.key0, run.key1);
+                    const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, hc.key);
                     const float u1 = u01(rn.y), u2 = u01(rn.z);
                     // a6: emission point on the track, its height and n(h_e) (Listing 4.1)
                     const float s = u1 * sg.L;
                     const float h_e = fmaf(s, fmaf(s, sg.k2, sg.cA), sg.hA);
                     float eta_e;
                     {
-                        float f = (h_e - atm.h0) * atm.inv_dh;
-                        f = fminf(fmaxf(f, 0.f), atm.f_max);
-                        const int k = min((int)f, atm.n_nodes - 2);
+                        float f = (h_e - hc.eta_h0) * hc.eta_inv_dh;
+                        f = fminf(fmaxf(f, 0.f), hc.eta_fmax);
+                        const int k = min((int)f, hc.eta_kmax);
                         const float e0 = eta_node(k), e1 = eta_node(k + 1);
                         eta_e = fmaf(f - (float)k, e1 - e0, e0);
                     }
@@ -765,13 +766,13 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         ux = cth * fmaf(q, wx, sg.Px);
                         uy = cth * fmaf(q, wy, sg.Py);
                         uz = cth * pqz;
-                        lam_inv = fmaf(-u2, run.il1 - run.il2, run.il1);  // 1/lambda uniform
+                        lam_inv = fmaf(-u2, hc.dil, hc.il1);  // 1/lambda uniform
                     } else {
                         // fluorescence: uniform in the cone about (aim - A_e)
                         int li = 0;
                         while (li < run.n_lines - 1 && u2 >= __ldg(run.line_cdf + li)) ++li;
                         lam_inv = 1.0f / __ldg(run.line_nm + li);
-                        const uint4 rb = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 1u, run.key0, run.key1);
+                        const uint4 rb = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 1u, hc.key);
                         const float xe = fmaf(s, sg.Px, sc->Ax), ye = fmaf(s, sg.Py, sc->Ay), ze = fmaf(s, sg.Pz, sg.Az);
                         float ax = sc->aimx - xe, ay = sc->aimy - ye, az = sc->aimz - ze;
                         const float an = rsqrtf(ax * ax + ay * ay + az * az);
@@ -808,18 +809,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // inside the histogram extent + margin or within r/|u_z| + margin of a telescope
                     if (f_lv2) {
                         const unsigned conv = __activemask();            // lanes that reach the filter together
-                        bool keep = xl >= run.box_x0 && xl < run.box_x1 && yl >= run.box_y0 && yl < run.box_y1;
+                        bool keep = xl >= hc.box_x0 && xl < hc.box_x1 && yl >= hc.box_y0 && yl < hc.box_y1;
                         if (!keep && f_tel) {
-                            const bool brute = !f_grid || -uz < det.grid_min_cos;
-                            const float thr = fmaf(det.r_max, -inv_uz, run.lv2_margin);
+                            const bool brute = !f_grid || -uz < hc.grid_min_cos;
+                            const float thr = fmaf(hc.r_max, -inv_uz, hc.lv2_margin);
                             const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
                             // per cell: (smallest key, acc); acc <= margin: every point of the cell is near
                             // a telescope; smallest key > thr: none is; otherwise walk the sorted list
                             float2 ka = make_float2(CUDART_INF_F, CUDART_INF_F);
                             if (cell >= 0) ka = __ldg(det.lv2.kacc + cell);
-                            keep = ka.y <= run.lv2_margin;
+                            keep = ka.y <= hc.lv2_margin;
                             if (!keep && (cell < -1 || ka.x <= thr))
-                                keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, run.lv2_margin);
+                                keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, hc.lv2_margin);
                         }
                         __syncwarp(conv);                                // rejoin the lanes that searched a list
                         if (!keep) { pkA += 0x10000u; break; }
@@ -880,20 +881,20 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         if (!ok) { pkB += 1u; break; }
                         dd = aX; dt = aT * kInvC; Xs = aS;
                     }
-                    float wgt = run.w;
+                    float wgt = hc.w;
                     if (f_trans != C8PH_TRANS_OFF) {
                         // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
                         float tau = 0.f;
                         if (f_ray) {
-                            float qq = atm.ray_lambda * lam_inv;
+                            float qq = hc.ray_lambda * lam_inv;
                             qq *= qq; qq *= qq;
-                            tau = Xs * qq * atm.ray_inv_X;
+                            tau = Xs * qq * hc.ray_k;                        // optical depth in units of ln 2
                         }
-                        if (f_aer) tau = fmaf(ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
-                        const float T = exp2_fast(-1.4426950408889634f * tau);
+                        if (f_aer) tau = fmaf(1.4426950408889634f * ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
+                        const float T = exp2_fast(-tau);
                         if (f_trans == C8PH_TRANS_ROULETTE) {
                             if (!(u01(rn.w) < T)) { pkB += 0x10000u; break; }
-                        } else wgt = run.w * T;
+                        } else wgt = hc.w * T;
                     }
                     // landed: corrected position (dd along the horizontal direction of flight)
                     const float hn2 = ux * ux + uy * uy;
@@ -907,10 +908,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     int cell = -1;
                     float kmin = CUDART_INF_F;
                     if (f_tel) {
-                        const bool brute = f_hit_brute || !f_grid || -uz < det.grid_min_cos;
+                        const bool brute = f_hit_brute || !f_grid || -uz < hc.grid_min_cos;
                         if (f_grid) {
-                            cell = grid_cell(det.hit, xg, yg);
-                            kmin = __ldg(det.hit.kmin + max(cell, 0));      // cell -1 (outside): never a candidate
+                            const int gx = __float2int_rd((xg - hc.hit_x0) * hc.hit_inv_cs), gy = __float2int_rd((yg - hc.hit_y0) * hc.hit_inv_cs);
+                            cell = ((unsigned)gx < (unsigned)hc.hit_nx && (unsigned)gy < (unsigned)hc.hit_ny) ? gy * hc.hit_nx + gx : -1;
+                            kmin = __ldg(hc.hit_kmin + max(cell, 0));       // cell -1 (outside): never a candidate
                             if (cell < 0) kmin = CUDART_INF_F;
                         }
                         if (brute) cell = -2;
@@ -918,14 +920,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // a15: ground grid
                     if (has_grid_geom) {
                         const float4 fb = *reinterpret_cast<const float4 *>(sc);         // fbx, fby, ibx, iby
-                        const int ix = __float_as_int(fb.z) + __float2int_rd(fmaf(cx, det.hist_inv_cell, fb.x));
-                        const int iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, det.hist_inv_cell, fb.y));
-                        if ((unsigned)ix < (unsigned)det.hist_nx && (unsigned)iy < (unsigned)det.hist_ny) {
+                        const int ix = __float_as_int(fb.z) + __float2int_rd(fmaf(cx, hc.hist_inv_cell, fb.x));
+                        const int iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, hc.hist_inv_cell, fb.y));
+                        if ((unsigned)ix < (unsigned)hc.hist_nx && (unsigned)iy < (unsigned)hc.hist_ny) {
                             pkC += 1u;
-                            if (has_hist) atomicAdd(run.out.hist + (iy * det.hist_nx + ix), wgt);
+                            if (has_hist) atomicAdd(hc.hist + (iy * hc.hist_nx + ix), wgt);
                         }
                     }
-                    const bool cand = cell < -1 || kmin <= -inv_uz * run.hit_infl;
+                    const bool cand = cell < -1 || kmin <= -inv_uz * hc.hit_infl;
                     if (!cand) {
                         if (f_write != C8PH_WRITE_ALL) break;
                         cell = -1;
