@@ -372,3 +372,33 @@ def test_thesis_model_arrays(golden_dir, monkeypatch, name, n_tel):
         ctx.close()
         monkeypatch.setenv("C8PH_FORCE_BRUTE", "0")
         assert brute["counters"] == gpu["counters"] and np.array_equal(brute["tel_counts"], gpu["tel_counts"])
+
+
+def test_emit_propagate_is_stream_ordered_and_graph_capturable():
+    """The hot call enqueues only (no allocation, no host sync, no bulk copy): it can run on a side
+    stream and be captured into a CUDA graph; replays give the bits of the eager call."""
+    cfg = W.make_config(4, n_segments=1200)
+    ctx = api.setup_context(cfg)
+    eager = api.run_config(cfg, ctx=ctx)
+    seg = api.segments_to_device(cfg["segments"])
+    out = api.alloc_device_outputs(ctx, 1 << 20, True)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        ctx.emit_propagate(seg, 1200, 0, cfg["params"], cfg["seed"], out, stream=side)     # warm-up on the side stream
+    side.synchronize()
+    first = api.outputs_to_host(ctx, out)
+    assert first["counters"] == eager["counters"] and np.array_equal(first["hist"], eager["hist"])
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        for k in ("hist", "tel_counts", "counters"):
+            out[k].zero_()
+        ctx.emit_propagate(seg, 1200, 0, cfg["params"], cfg["seed"], out, stream=torch.cuda.current_stream())
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    rep = api.outputs_to_host(ctx, out)
+    assert rep["counters"] == eager["counters"]
+    assert np.array_equal(rep["hist"], eager["hist"]) and np.array_equal(rep["tel_counts"], eager["tel_counts"])
+    key = lambda p: np.argsort(p["seg"].astype(np.int64) << 32 | p["j_tel"])
+    assert np.array_equal(rep["photons"][key(rep["photons"])], eager["photons"][key(eager["photons"])])
