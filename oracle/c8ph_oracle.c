@@ -32,6 +32,8 @@
  *                       ray-sphere analytic cases
  *   fluorescence / camera (cfg3): isotropy moments, line frequencies,
  *                       pixel-centre round trip.
+ *   dispersion (R13)    b -> 0 limit, closed form of the yield integral incl. threshold
+ *                       inside the band, u.P = 1/(beta n(lambda)), KS test of the spectrum.
  */
 #include <math.h>
 #include <stdint.h>
@@ -88,6 +90,7 @@ typedef struct {
     double fluor_yield_per_MeV, aim_factor;
     int32_t n_lines, pad;
     const float *line_nm, *line_cdf;
+    double disp_b_nm2, disp_lambda0_nm;   /* dispersion n-1 = eta(h) D(lambda); b = 0: off (reading R13) */
 } orc_params;
 
 /* photon status */
@@ -189,6 +192,39 @@ double orc_cherenkov_yield(double charge, double len_m, double beta, double n,
     if (!(sin2 > 0.0)) return 0.0;
     double inv_l = 1.0 / (lambda1_nm * 1e-9) - 1.0 / (lambda2_nm * 1e-9);
     return 2.0 * ORC_PI * ORC_ALPHA * charge * charge * len_m * inv_l * sin2;
+}
+
+/* ------------------------------------------------------------------ dispersion (row f4, reading R13)
+ * "wavelength dependence of the refractive index, called dispersion ... only for a part
+ * of the light spectrum the condition beta > 1/n(lambda) may be fulfilled"; the yield integral with
+ * the Heaviside function (unnumbered equation before Eq. 2.5) and theta = arccos(1/(beta n(lambda,l))).
+ * The thesis gives no dispersion law (Sellmeier / Edlen are only named); reading: a
+ * Cauchy-type law on the refractivity, n(lambda,h) - 1 = eta(h) D(lambda),
+ * D(lambda) = 1 + b (1/lambda^2 - 1/lambda0^2), eta tabulated at lambda0. */
+double orc_dispersion_factor(double b_nm2, double lambda0_nm, double lambda_nm)
+{
+    return 1.0 + b_nm2 * (1.0 / (lambda_nm * lambda_nm) - 1.0 / (lambda0_nm * lambda0_nm));
+}
+
+/* sin^2(theta) = max(0, 1 - 1/(beta n)^2) at wave number k = 1/lambda [1/nm] */
+static double disp_sin2(double beta, double eta, double b, double lambda0, double k)
+{
+    double n = 1.0 + eta * (1.0 + b * (k * k - 1.0 / (lambda0 * lambda0)));
+    double s = 1.0 - 1.0 / (beta * beta * n * n);
+    return s > 0.0 ? s : 0.0;
+}
+
+/* N = 2 pi alpha z^2 L int_{1/l2}^{1/l1} Theta(beta n(k) - 1) (1 - 1/(beta n(k))^2) dk,
+ * plain composite Simpson rule, 8192 panels. */
+double orc_cherenkov_yield_dispersive(double charge, double len_m, double beta, double eta,
+                                      double lambda1_nm, double lambda2_nm, double b_nm2, double lambda0_nm)
+{
+    const int n = 8192;
+    double k_lo = 1.0 / lambda2_nm, k_hi = 1.0 / lambda1_nm, h = (k_hi - k_lo) / n;
+    double acc = disp_sin2(beta, eta, b_nm2, lambda0_nm, k_lo) + disp_sin2(beta, eta, b_nm2, lambda0_nm, k_hi);
+    for (int i = 1; i < n; ++i)
+        acc += (i & 1 ? 4.0 : 2.0) * disp_sin2(beta, eta, b_nm2, lambda0_nm, k_lo + i * h);
+    return 2.0 * ORC_PI * ORC_ALPHA * charge * charge * len_m * (acc * h / 3.0) * 1e9;
 }
 
 /* ------------------------------------------------------------------ A9 rotation
@@ -456,6 +492,7 @@ int orc_camera_pixel(const orc_detector *det, const double u_arr[3])
 typedef struct {
     double A[3], P[3], L, beta, t0, M[9];
     double n_exp; int64_t n_bunch; int lv1_dropped;
+    double eta_mid;               /* refractivity at the segment mid height (dispersive sampling) */
     /* fluorescence */
     double aim[3], cos_psi;
 } orc_segprep;
@@ -498,7 +535,18 @@ static void prepare_segment(const orc_atmosphere *atm, const orc_detector *det, 
     orc_draw(seed, seg_id, 0xFFFFFFFFu, 0, u_seg);
     if (par->emit == ORC_EMIT_CHERENKOV) {
         double n_mid = 1.0 + orc_refractivity(atm, h_mid);
+        o->eta_mid = n_mid - 1.0;
         /* O1 (R1): midpoint rule for the height dependence of Eq. 2.2 */
+        if (par->disp_b_nm2 != 0.0) {
+            o->eta_mid = orc_refractivity(atm, h_mid);
+            o->n_exp = orc_cherenkov_yield_dispersive(sg->charge[i], o->L, o->beta, o->eta_mid,
+                                                      par->lambda_min_nm, par->lambda_max_nm,
+                                                      par->disp_b_nm2, par->disp_lambda0_nm);
+            /* LV1 and the threshold use the largest n of the band (blue end for b > 0) */
+            double Dmax = fmax(orc_dispersion_factor(par->disp_b_nm2, par->disp_lambda0_nm, par->lambda_min_nm),
+                               orc_dispersion_factor(par->disp_b_nm2, par->disp_lambda0_nm, par->lambda_max_nm));
+            n_mid = 1.0 + o->eta_mid * Dmax;
+        } else
         o->n_exp = orc_cherenkov_yield(sg->charge[i], o->L, o->beta, n_mid,
                                        par->lambda_min_nm, par->lambda_max_nm);
         if (o->n_exp > 0.0 && par->lv1) {
@@ -614,7 +662,23 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                     /* O3: 1/lambda uniform (spectrum ~ 1/lambda^2, Eq. 2.4) */
                     double il1 = 1.0 / par->lambda_min_nm, il2 = 1.0 / par->lambda_max_nm;
                     ph.lambda_nm = 1.0 / (il1 - u4[2] * (il1 - il2));
-                    /* O4: Eq. 2.5 — the angle depends on the location */
+                    if (par->disp_b_nm2 != 0.0) {
+                        /* R13: the spectrum is 1/lambda^2 sin^2 theta(lambda): rejection from the
+                         * 1/lambda-uniform law with the envelope max sin^2, n at the segment mid height;
+                         * trial t takes the uniforms (2 (t&1), 2 (t&1) + 1) of draw stream 2 + t/2 */
+                        double b = par->disp_b_nm2, l0 = par->disp_lambda0_nm;
+                        double smax = fmax(disp_sin2(sp.beta, sp.eta_mid, b, l0, il1), disp_sin2(sp.beta, sp.eta_mid, b, l0, il2));
+                        double k = il1;
+                        for (int t = 0; t < 32; ++t) {
+                            double ut[4];
+                            orc_draw(seed, seg_id, (uint32_t)j, 2u + (uint32_t)(t >> 1), ut);
+                            k = il1 - ut[2 * (t & 1)] * (il1 - il2);
+                            if (ut[2 * (t & 1) + 1] * smax < disp_sin2(sp.beta, sp.eta_mid, b, l0, k)) break;
+                        }
+                        ph.lambda_nm = 1.0 / k;
+                        n_e = 1.0 + eta_e * orc_dispersion_factor(b, l0, ph.lambda_nm);
+                    }
+                    /* O4: Eq. 2.5 — the angle depends on the location (and, with dispersion, on lambda) */
                     double cos_th = 1.0 / (sp.beta * n_e);
                     double sin2 = 1.0 - cos_th * cos_th;
                     if (sin2 < 0.0) { sin2 = 0.0; cos_th = 1.0; }

@@ -69,7 +69,8 @@ class Params(C.Structure):
                 ("lv1_margin_rad", C.c_double), ("lv2_margin_m", C.c_double),
                 ("fluor_yield_per_MeV", C.c_double), ("aim_factor", C.c_double),
                 ("n_lines", C.c_int32), ("pad", C.c_int32),
-                ("line_nm", C.POINTER(C.c_float)), ("line_cdf", C.POINTER(C.c_float))]
+                ("line_nm", C.POINTER(C.c_float)), ("line_cdf", C.POINTER(C.c_float)),
+                ("disp_b_nm2", C.c_double), ("disp_lambda0_nm", C.c_double)]
 
 
 PHOTON_DTYPE = np.dtype([("seg", "<i8"), ("j", "<i4"), ("status", "<i4"),
@@ -107,6 +108,10 @@ def lib():
             L.orc_height.restype = C.c_double
             L.orc_cherenkov_yield.restype = C.c_double
             L.orc_cherenkov_yield.argtypes = [C.c_double] * 6
+            L.orc_cherenkov_yield_dispersive.restype = C.c_double
+            L.orc_cherenkov_yield_dispersive.argtypes = [C.c_double] * 8
+            L.orc_dispersion_factor.restype = C.c_double
+            L.orc_dispersion_factor.argtypes = [C.c_double] * 3
             L.orc_straight_line.restype = C.c_double
             L.orc_trace.restype = C.c_int
             L.orc_trace.argtypes = [C.POINTER(Atmosphere), C.c_int, C.c_double, C.c_double, C.c_double,
@@ -179,6 +184,8 @@ def params_struct(par: dict, keep: _Keep) -> Params:
     s.n_lines = len(par["line_nm"])
     s.line_nm = keep.f32(par["line_nm"]) if s.n_lines else None
     s.line_cdf = keep.f32(par["line_cdf"]) if s.n_lines else None
+    s.disp_b_nm2 = float(np.float32(par.get("disp_b_nm2", 0.0)))
+    s.disp_lambda0_nm = float(np.float32(par.get("disp_lambda0_nm", 400.0)))
     return s
 
 

@@ -234,7 +234,8 @@ def _default_params() -> dict:
                 lambda_min_nm=300.0, lambda_max_nm=600.0, bunch_weight=1.0,
                 lv1_margin_rad=0.0, lv2_margin_m=0.0, substeps=1,
                 fluor_yield_per_MeV=4.0, line_nm=np.zeros(0, np.float32),
-                line_cdf=np.zeros(0, np.float32), aim_factor=1.5)
+                line_cdf=np.zeros(0, np.float32), aim_factor=1.5,
+                disp_b_nm2=0.0, disp_lambda0_nm=400.0)      # dispersion off (R13)
 
 
 _TABLE = dict(n_h=512, n_zen=256, h_max=100000.0, zen_max_deg=89.0)

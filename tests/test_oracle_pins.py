@@ -534,3 +534,76 @@ def test_thesis_model_array_fixtures(golden_dir):
     u = np.stack([hit["ux"], hit["uy"], hit["uz"]], axis=1)
     m2 = (d ** 2).sum(1) - ((d * u).sum(1)) ** 2
     assert np.all(m2 <= c[:, 3] ** 2 * (1 + 1e-9))
+
+
+# ---------------------------------------------------------------------------------- dispersion (R13, row f4)
+def _disp_integrand(k, beta, eta, b, l0):
+    n = 1.0 + eta * (1.0 + b * (k * k - 1.0 / l0 ** 2))
+    return np.maximum(0.0, 1.0 - 1.0 / (beta * n) ** 2)
+
+
+def test_dispersive_yield_limits_closed_form_and_threshold():
+    """P:318 yield integral with n(lambda): b -> 0 is Frank-Tamm's closed form; for b > 0 the integral has
+    the closed form  k - [k/(2A(A+Bk^2)) + atan(k sqrt(B/A))/(2A sqrt(AB))]/beta^2  (A + B k^2 = n(k));
+    with the Cherenkov threshold inside the band only the blue side of it contributes."""
+    from scipy import integrate
+    L = O.lib()
+    a2pi = 2.0 * math.pi / 137.035999
+    y0 = L.orc_cherenkov_yield(1.0, 7.0, 0.99995, 1.000293, 300.0, 600.0)
+    assert abs(L.orc_cherenkov_yield_dispersive(1.0, 7.0, 0.99995, 0.000293, 300.0, 600.0, 0.0, 400.0) / y0 - 1) < 1e-12
+    eta, b, l0, l1, l2 = 2.5e-4, 5700.0, 400.0, 250.0, 700.0
+    A, B = 1.0 + eta * (1.0 - b / l0 ** 2), eta * b
+    F = lambda k: k / (2 * A * (A + B * k * k)) + math.atan(k * math.sqrt(B / A)) / (2 * A * math.sqrt(A * B))
+    for beta in (1.0, 0.99990):                                           # far above threshold
+        want = a2pi * 3.0 * ((1 / l1 - 1 / l2) - (F(1 / l1) - F(1 / l2)) / beta ** 2) * 1e9
+        got = L.orc_cherenkov_yield_dispersive(1.0, 3.0, beta, eta, l1, l2, b, l0)
+        assert abs(got / want - 1) < 1e-9, (beta, got, want)
+    # threshold inside the band: beta n(k_th) = 1
+    k_th = 1.0 / 400.0
+    beta = 1.0 / (1.0 + eta * (1.0 + b * (k_th ** 2 - 1 / l0 ** 2)))
+    got = L.orc_cherenkov_yield_dispersive(1.0, 3.0, beta, eta, l1, l2, b, l0)
+    want = a2pi * 3.0 * ((1 / l1 - k_th) - (F(1 / l1) - F(k_th)) / beta ** 2) * 1e9
+    quad = a2pi * 3.0 * integrate.quad(_disp_integrand, 1 / l2, 1 / l1, args=(beta, eta, b, l0), points=[k_th], epsabs=0, epsrel=1e-12)[0] * 1e9
+    assert 0 < got < 0.2 * L.orc_cherenkov_yield_dispersive(1.0, 3.0, 1.0, eta, l1, l2, b, l0)
+    assert abs(got / want - 1) < 1e-6 and abs(quad / want - 1) < 1e-8
+    # below threshold over the whole band
+    assert L.orc_cherenkov_yield_dispersive(1.0, 3.0, 0.9997, eta, l1, l2, b, l0) == 0.0
+    assert abs(L.orc_dispersion_factor(b, l0, l0) - 1.0) < 1e-15 and L.orc_dispersion_factor(b, l0, 300.0) > 1.0
+
+
+def test_dispersive_photons_spectrum_and_cone_angle():
+    """Photon level (cfg0: homogeneous n, straight line, so the record keeps the emission direction):
+    u.P = 1/(beta n(lambda)) for every photon, and the wavelengths follow the density
+    lambda^-2 sin^2 theta(lambda) (KS test) for particles just above threshold, where it is far from
+    the non-dispersive 1/lambda-uniform law."""
+    cfg = W.make_config(0, n_segments=400)
+    eta, b, l0 = 0.000293, 5700.0, 400.0
+    cfg["params"].update(disp_b_nm2=b, disp_lambda0_nm=l0, lambda_min_nm=300.0, lambda_max_nm=600.0)
+    s = cfg["segments"]
+    k_th = 1.0 / 520.0                                                    # threshold at 520 nm: only 300-520 nm emits
+    s["beta"][:] = np.float32(1.0 / (1.0 + eta * (1.0 + b * (k_th ** 2 - 1 / l0 ** 2))))
+    s["len"][:] = 400.0
+    res = O.run(cfg, record=True)
+    ph = res["photons"]
+    assert len(ph) > 5000 and ph["lambda_nm"].max() < 520.5 and ph["lambda_nm"].min() >= 300.0
+    P = np.stack([s["dx"], s["dy"], s["dz"]], axis=1).astype(np.float64)
+    P /= np.linalg.norm(P, axis=1, keepdims=True)
+    beta = s["beta"].astype(np.float64)[ph["seg"]]
+    n_lam = 1.0 + float(np.float32(eta)) * (1.0 + float(np.float32(b)) * (1.0 / ph["lambda_nm"] ** 2 - 1.0 / l0 ** 2))
+    cos_c = np.minimum(1.0, 1.0 / (beta * n_lam))
+    up = ph["ux"] * P[ph["seg"], 0] + ph["uy"] * P[ph["seg"], 1] + ph["uz"] * P[ph["seg"], 2]
+    assert np.abs(up - cos_c).max() < 1e-12
+    # analytic CDF in k = 1/lambda of the density sin^2 theta(k)
+    b0 = float(beta[0])
+    ks = np.linspace(1 / 600.0, 1 / 300.0, 20001)
+    dens = _disp_integrand(ks, b0, float(np.float32(eta)), float(np.float32(b)), l0)
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(ks))])
+    cdf /= cdf[-1]
+    ks_stat = stats.kstest(1.0 / ph["lambda_nm"], lambda x: np.interp(x, ks, cdf))
+    assert ks_stat.pvalue > 1e-3, ks_stat
+    flat = stats.kstest(1.0 / ph["lambda_nm"], lambda x: np.clip((x - 1 / 600.0) / (1 / 300.0 - 1 / 600.0), 0, 1))
+    assert flat.pvalue < 1e-12                                            # and clearly not the non-dispersive law
+    # expected count: sum of the stochastic roundings reproduces the integral within 5 sigma
+    want = sum(O.lib().orc_cherenkov_yield_dispersive(float(q), 400.0, float(bb), float(np.float32(eta)), 300.0, 600.0, float(np.float32(b)), l0)
+               for q, bb in zip(s["charge"], s["beta"]))
+    assert abs(len(ph) - want) < 5 * math.sqrt(len(s["beta"]) / 4.0) + 1
