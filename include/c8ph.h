@@ -120,6 +120,11 @@ typedef struct {
     float fluor_yield_per_MeV, aim_factor;  /* fluorescence: photons/MeV; forced-cone radius = aim_factor * r_tel */
     int32_t n_lines;                        /* fluorescence line spectrum                         */
     const float *line_nm, *line_cdf;        /* HOST [n_lines]; copied at every call               */
+    /* Dispersion (thesis P:314-322, Eq. 2.5): n(lambda,h) - 1 = (n(h) - 1) D(lambda),
+     * D = 1 + b (1/lambda^2 - 1/lambda0^2), the n(h) table being valid at lambda0.  The yield is the
+     * integral over the band with the Heaviside threshold beta n(lambda) > 1, wavelengths follow
+     * lambda^-2 sin^2 theta(lambda), the cone angle uses n(lambda, h_e).  b = 0: off; b >= 0.    */
+    float disp_b_nm2, disp_lambda0_nm;
 } c8ph_params;
 
 /* ---- segments, outputs ------------------------------------------------------------------------- */

@@ -71,7 +71,7 @@ class Params(C.Structure):
                 ("lambda_min_nm", C.c_float), ("lambda_max_nm", C.c_float), ("bunch_weight", C.c_float),
                 ("lv1_margin_rad", C.c_float), ("lv2_margin_m", C.c_float),
                 ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float), ("n_lines", C.c_int32),
-                ("line_nm", _fp), ("line_cdf", _fp)]
+                ("line_nm", _fp), ("line_cdf", _fp), ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float)]
 
 
 class Segments(C.Structure):
@@ -235,6 +235,7 @@ class Context:
         p.bunch_weight = float(par["bunch_weight"])
         p.lv1_margin_rad, p.lv2_margin_m = float(par["lv1_margin_rad"]), float(par["lv2_margin_m"])
         p.fluor_yield_per_MeV, p.aim_factor = float(par["fluor_yield_per_MeV"]), float(par["aim_factor"])
+        p.disp_b_nm2, p.disp_lambda0_nm = float(par.get("disp_b_nm2", 0.0)), float(par.get("disp_lambda0_nm", 400.0))
         ln, lc = _f32(par["line_nm"]), _f32(par["line_cdf"])
         p.n_lines = len(ln)
         if len(ln):

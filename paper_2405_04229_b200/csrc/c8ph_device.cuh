@@ -83,6 +83,9 @@ struct DevRun {
     double fluor_yield, aim_factor;
     int n_lines;
     const float *line_nm, *line_cdf;      // DEVICE
+    float disp_b, disp_c0;          // dispersion D(k) = disp_c0 + disp_b k^2, k = 1/lambda [1/nm]; disp_b = 0: off
+    double disp_k0sq;               // 1/lambda0^2
+    double il1_d, il2_d;            // 1/lambda_min, 1/lambda_max in fp64 (dispersive yield integral)
     uint32_t key0[10], key1[10];    // Philox round keys
     int64_t n_seg, seg_id_base;
     uint32_t local_base;            // added to the call-local segment index written into photon records

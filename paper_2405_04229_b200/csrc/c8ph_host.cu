@@ -483,6 +483,8 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     if (p->trace == C8PH_TRACE_NUMERIC && p->emit == C8PH_EMIT_FLUORESCENCE) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence + numeric tracing");
     if (p->emit == C8PH_EMIT_CHERENKOV && !(p->lambda_min_nm > 0.f && p->lambda_max_nm > p->lambda_min_nm))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: wavelength band");
+    if (!(p->disp_b_nm2 >= 0.f) || (p->disp_b_nm2 > 0.f && !(p->disp_lambda0_nm > 0.f)))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: dispersion needs disp_b_nm2 >= 0 and disp_lambda0_nm > 0");
     if (p->emit == C8PH_EMIT_FLUORESCENCE) {
         if (ctx->det.n_tel < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: fluorescence needs a telescope to aim at");
         if (p->n_lines < 1 || !p->line_nm || !p->line_cdf) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence line spectrum");
@@ -525,6 +527,11 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         if (p->trace == C8PH_TRACE_STRAIGHT) r.hit_infl = 1.0f + 1e-5f;
     }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
+    r.disp_b = p->emit == C8PH_EMIT_CHERENKOV ? p->disp_b_nm2 : 0.f;
+    r.disp_k0sq = r.disp_b > 0.f ? 1.0 / ((double)p->disp_lambda0_nm * (double)p->disp_lambda0_nm) : 0.0;
+    r.disp_c0 = (float)(1.0 - (double)r.disp_b * r.disp_k0sq);
+    r.il1_d = p->emit == C8PH_EMIT_CHERENKOV ? 1.0 / (double)p->lambda_min_nm : 0.0;
+    r.il2_d = p->emit == C8PH_EMIT_CHERENKOV ? 1.0 / (double)p->lambda_max_nm : 0.0;
     if (p->emit == C8PH_EMIT_FLUORESCENCE) {
         if (p->n_lines > ctx->lines_cap) {
             dfree(ctx->d_lines);

@@ -47,6 +47,7 @@ constexpr int kMaxBlocksPerSM = C8PH_MAX_BLOCKS_PER_SM;
 constexpr int kMinBlocks = C8PH_MIN_BLOCKS;                    // resident CTAs per SM the register budget is set for
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
+constexpr double kAlphaFS = 1.0 / 137.035999;    // fine-structure constant (Eq. 2.3)
 constexpr float kUpCut = -1.0e-6f;               // drop photons with u_z >= kUpCut
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
@@ -132,7 +133,7 @@ struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
     float aimx, aimy, aimz, omc;                      // fluorescence: aim point, 1 - cos(psi)
     float Tg;                                         // anchor clock - t_ref  (or t0 - t_ref)
     uint32_t local;                                   // segment index within the call
-    float pad0;
+    float eta_mid;                                    // refractivity at the segment mid height (dispersion)
 };
 struct alignas(16) SegSlot { SegHot h; SegCold c; };
 static_assert(sizeof(SegHot) == 112 && sizeof(SegCold) == 64 && sizeof(SegSlot) == 176, "segment slot layout");
@@ -228,6 +229,33 @@ __device__ __forceinline__ void sincos_2pi_u(uint32_t r, float &sphi, float &cph
     const float s0 = swap ? cv : sv, c0 = swap ? sv : cv;
     sphi = __uint_as_float(__float_as_uint(s0) ^ ((o & 4u) << 29));
     cphi = __uint_as_float(__float_as_uint(c0) ^ (((o + 2u) & 4u) << 29));
+}
+
+// Dispersive Cherenkov yield integral (thesis P:318, unnumbered equation before Eq. 2.5):
+//   int_{k_lo}^{k_hi} Theta(beta n(k) - 1) (1 - 1/(beta n(k))^2) dk,  n(k) = 1 + eta (c0 + b k^2),  k = 1/lambda,
+// b >= 0 so n grows towards the blue: the threshold k_th (beta n = 1) is a lower limit.  8-point
+// Gauss-Legendre on the smooth part; sin^2 in the cancellation-free form x(2+x)/(1+x)^2, x = beta n - 1.
+__device__ __forceinline__ double disp_yield_integral(double beta, double eta, double b, double k0sq,
+                                                      double k_lo, double k_hi)
+{
+    const double delta = 1.0 - beta;
+    auto D = [&](double k) { return 1.0 + b * (k * k - k0sq); };
+    if (!(beta * eta * D(k_hi) > delta)) return 0.0;                  // below threshold over the whole band
+    double ka = k_lo;
+    if (!(beta * eta * D(k_lo) > delta)) ka = sqrt(k0sq + (delta / (beta * eta) - 1.0) / b);
+    const double xs[4] = {0.1834346424956498, 0.5255324099163290, 0.7966664774136267, 0.9602898564975363};
+    const double ws[4] = {0.3626837833783620, 0.3137066458778873, 0.2223810344533745, 0.1012285362903763};
+    const double c = 0.5 * (k_hi + ka), hw = 0.5 * (k_hi - ka);
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+        for (int sgn = -1; sgn <= 1; sgn += 2) {
+            const double x = fmax(beta * eta * D(c + sgn * hw * xs[i]) - delta, 0.0);
+            acc += ws[i] * x * (2.0 + x) / ((1.0 + x) * (1.0 + x));
+        }
+    }
+    return acc * hw;
 }
 
 struct TabVal { float dd, dt, X, ta; bool bad; };
@@ -445,6 +473,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const int f_trans = SPEC ? (int)C8PH_TRANS_ROULETTE : run.trans;
     const bool f_ray = SPEC ? true : atm.ray_inv_X > 0.f;
     const bool f_aer = SPEC ? false : atm.aer_L > 0.f;
+    const bool f_disp = SPEC ? false : run.disp_b != 0.f;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -470,7 +499,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             if (sh->anchor) {
                 // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
                 const float Pz = sh->Pz;
-                const float bn1 = fmaxf(fmaf(sh->beta, eta_e, -sh->delta), 0.f);
+                const float eta_c = f_disp ? eta_e * fmaf(run.disp_b, lam_inv * lam_inv, run.disp_c0) : eta_e;
+                const float bn1 = fmaxf(fmaf(sh->beta, eta_c, -sh->delta), 0.f);
                 const float num = fmaf(-bn1, Pz, qw);
                 const float geo = (s + sh->AzP) * num * rcp_fast(Pz + qw);
                 t_arr = sc->Tg + fmaf(fmaf(s, sh->dob, geo), kInvC, dt);
@@ -598,11 +628,21 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 mc.aimx = mc.aimy = mc.aimz = mc.omc = 0.f;
                 if (EMIT == C8PH_EMIT_CHERENKOV) {
                     // Frank-Tamm, Eq. 2.2-2.4, n at the segment mid height
-                    const double n_mid = 1.0 + eta_lookup_d(atm, h_mid);
+                    const double eta_mid = eta_lookup_d(atm, h_mid);
+                    double n_mid = 1.0 + eta_mid;
+                    const double zq = run.seg.charge[i];
+                    mc.eta_mid = (float)eta_mid;                      // eta at the mid height (dispersive sampling)
+                    if (run.disp_b != 0.f) {
+                        // dispersion: yield integral over the band with the threshold;
+                        // LV1 below uses the largest n of the band (blue end)
+                        const double k1 = run.il1_d, k2 = run.il2_d, b = run.disp_b;
+                        n_exp = (2.0 * 3.14159265358979323846 * kAlphaFS * 1.0e9) * zq * zq * L *
+                                disp_yield_integral(beta, eta_mid, b, run.disp_k0sq, k2, k1);
+                        n_mid = 1.0 + eta_mid * (1.0 + b * (k1 * k1 - run.disp_k0sq));
+                    }
                     const double bn = beta * n_mid;
                     const double sin2 = 1.0 - 1.0 / (bn * bn);
-                    const double zq = run.seg.charge[i];
-                    if (sin2 > 0.0) n_exp = run.yield_k * zq * zq * L * sin2;
+                    if (run.disp_b == 0.f && sin2 > 0.0) n_exp = run.yield_k * zq * zq * L * sin2;
                     if (n_exp > 0.0 && run.lv1) {
                         // LV1, Eq. 4.3: angle between P and the direction to the array centre
                         const double dist = sqrt(mx * mx + my * my + mz * mz);
@@ -661,6 +701,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float *ed = run.seg.edep;
                     n_exp = run.fluor_yield * (ed ? (double)ed[i] : 0.0) * 0.5 * omc;
                     e1x = e1y = e1z = e2x = e2y = e2z = 0.f;
+                    mc.eta_mid = 0.f;
                 }
                 long long N = 0;
                 if (!(n_exp > 0.0)) below = true;
@@ -683,7 +724,6 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
                     me.Gx = me.Gy = me.AzP = 0.f;
                     mc.fbx = mc.fby = 0.f; mc.ibx = mc.iby = 0;
-                    mc.pad0 = 0.f;
                     me.dob = (float)((double)me.delta / beta); me.inv_beta = (float)(1.0 / beta);
                     if (me.anchor) {
                         const double azp = Az / Pz;
@@ -755,7 +795,27 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     sincos_2pi_u(rn.x, sphi, cphi);                       // phi = 2 pi u0
                     if (EMIT == C8PH_EMIT_CHERENKOV) {
                         // a6/a7: cos(theta_c) = 1/(beta n(h_e)) (Eq. 2.5), beta n - 1 without cancellation
-                        const float bn1 = fmaxf(fmaf(sg.beta, eta_e, -sg.delta), 0.f);
+                        lam_inv = fmaf(-u2, hc.dil, hc.il1);            // 1/lambda uniform
+                        float eta_c = eta_e;                            // refractivity that sets the cone angle
+                        if (f_disp) {
+                            // dispersion (Eq. 2.5): spectrum lambda^-2 sin^2 theta(lambda) by rejection from
+                            // the 1/lambda-uniform law (n at the segment mid height); trial t takes uniforms
+                            // (2 (t&1), 2 (t&1) + 1) of Philox stream 2 + t/2; then n(lambda, h_e) for the angle
+                            const float em = sc->eta_mid * sg.beta;
+                            auto sin2 = [&](float k) {
+                                const float x = fmaxf(fmaf(em, fmaf(run.disp_b, k * k, run.disp_c0), -sg.delta), 0.f);
+                                return x * (2.f + x) * rcp_fast((1.f + x) * (1.f + x));
+                            };
+                            const float smax = fmaxf(sin2(hc.il1), sin2(hc.il1 - hc.dil));
+                            uint4 rt = make_uint4(0u, 0u, 0u, 0u);
+                            for (int t = 0; t < 32; ++t) {
+                                if (!(t & 1)) rt = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 2u + (uint32_t)(t >> 1), hc.key);
+                                lam_inv = fmaf(-u01((t & 1) ? rt.z : rt.x), hc.dil, hc.il1);
+                                if (u01((t & 1) ? rt.w : rt.y) * smax < sin2(lam_inv)) break;
+                            }
+                            eta_c = eta_e * fmaf(run.disp_b, lam_inv * lam_inv, run.disp_c0);
+                        }
+                        const float bn1 = fmaxf(fmaf(sg.beta, eta_c, -sg.delta), 0.f);
                         q = sqrt_fast(bn1 * (2.f + bn1));               // tan(theta_c)
                         cth = rcp_fast(1.f + bn1);                      // cos(theta_c)
                         // M = 2 A A^T - 1 is symmetric with third column -P: e2x = e1y, e1z = -P_x, e2z = -P_y
@@ -766,7 +826,6 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         ux = cth * fmaf(q, wx, sg.Px);
                         uy = cth * fmaf(q, wy, sg.Py);
                         uz = cth * pqz;
-                        lam_inv = fmaf(-u2, hc.dil, hc.il1);  // 1/lambda uniform
                     } else {
                         // fluorescence: uniform in the cone about (aim - A_e)
                         int li = 0;
@@ -1120,7 +1179,7 @@ static bool array_production_setting(const KArgs &a)
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr;
+           r.out.tel_counts != nullptr && r.disp_b == 0.f;
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)

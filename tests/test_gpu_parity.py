@@ -402,3 +402,33 @@ def test_emit_propagate_is_stream_ordered_and_graph_capturable():
     assert np.array_equal(rep["hist"], eager["hist"]) and np.array_equal(rep["tel_counts"], eager["tel_counts"])
     key = lambda p: np.argsort(p["seg"].astype(np.int64) << 32 | p["j_tel"])
     assert np.array_equal(rep["photons"][key(rep["photons"])], eager["photons"][key(eager["photons"])])
+
+
+def test_dispersion_yield_spectrum_and_cone():
+    """Row f4: n(lambda, h) = 1 + eta(h) D(lambda) (thesis P:314-322).  Device against oracle, photon
+    by photon: (a) cfg0 with particles whose Cherenkov threshold lies inside the band (only the blue
+    part emits, strongly non-uniform spectrum, rejection sampling takes several trials); (b) cfg4's
+    full feature set with dispersion on (generic kernel variant); (c) the layered-sum variant."""
+    eta, b, l0 = 0.000293, 5700.0, 400.0
+    cfg = W.make_config(0, n_segments=600)
+    cfg["params"].update(disp_b_nm2=b, disp_lambda0_nm=l0)
+    k_th = 1.0 / np.linspace(280.0, 640.0, 600)                        # threshold wavelength: below, inside, beyond the band
+    cfg["segments"]["beta"][:] = (1.0 / (1.0 + eta * (1.0 + b * (k_th ** 2 - 1 / l0 ** 2)))).astype(np.float32)
+    cfg["segments"]["len"][:] = 60.0
+    ora, gpu, rep = _both(cfg)
+    assert gpu["counters"]["emitted"] > 1e4 and gpu["counters"]["seg_below_threshold"] > 10
+    lam = gpu["photons"]["lambda_nm"]
+    assert lam.min() >= 300.0 and lam.max() <= 600.0 and np.median(lam) < 400.0
+    plain = api.run_config(W.make_config(0, n_segments=600))
+    assert plain["counters"]["emitted"] != gpu["counters"]["emitted"]
+    for k, n in ((4, 2500), (1, 600)):
+        cfg = W.make_config(k, n_segments=n)
+        cfg["params"].update(disp_b_nm2=b, disp_lambda0_nm=l0)
+        ora, gpu, rep = _both(cfg)
+        off = api.run_config(W.make_config(k, n_segments=n))
+        assert gpu["counters"]["emitted"] > off["counters"]["emitted"]      # blue end sees a larger n
+    bad = dict(cfg["params"], disp_b_nm2=-1.0)
+    ctx = api.setup_context(cfg)
+    with pytest.raises(api.C8phError) as e:
+        api.run_config(dict(cfg, params=bad), ctx=ctx)
+    assert e.value.code == api.E_ARG
