@@ -125,6 +125,13 @@ typedef struct {
      * integral over the band with the Heaviside threshold beta n(lambda) > 1, wavelengths follow
      * lambda^-2 sin^2 theta(lambda), the cone angle uses n(lambda, h_e).  b = 0: off; b >= 0.    */
     float disp_b_nm2, disp_lambda0_nm;
+    /* Detector efficiency eps(lambda) (mirror x sensor, thesis P:360-366) folded into the
+     * survival probability / weight together with the atmospheric transmission: n_eff values in [0,1]
+     * on the uniform grid eff_lambda0_nm + i eff_dlambda_nm, linear between nodes, end values held
+     * outside.  n_eff = 0: off.  Needs trans != C8PH_TRANS_OFF.                                    */
+    int32_t n_eff;
+    float eff_lambda0_nm, eff_dlambda_nm;
+    const float *eff;                       /* HOST [n_eff]; copied at every call                  */
 } c8ph_params;
 
 /* ---- segments, outputs ------------------------------------------------------------------------- */

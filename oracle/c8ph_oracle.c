@@ -32,6 +32,7 @@
  *                       ray-sphere analytic cases
  *   fluorescence / camera (cfg3): isotropy moments, line frequencies,
  *                       pixel-centre round trip.
+ *   efficiency (R14)    lookup values, eps = 1 identity, constant eps scaling, step curve.
  *   dispersion (R13)    b -> 0 limit, closed form of the yield integral incl. threshold
  *                       inside the band, u.P = 1/(beta n(lambda)), KS test of the spectrum.
  */
@@ -91,6 +92,9 @@ typedef struct {
     int32_t n_lines, pad;
     const float *line_nm, *line_cdf;
     double disp_b_nm2, disp_lambda0_nm;   /* dispersion n-1 = eta(h) D(lambda); b = 0: off (reading R13) */
+    int32_t n_eff, pad2;                  /* detector efficiency eps(lambda) folded into the transmission (R14) */
+    double eff_lambda0_nm, eff_dlambda_nm;
+    const float *eff;                     /* [n_eff] on the uniform grid lambda0 + i dlambda, in [0,1] */
 } orc_params;
 
 /* photon status */
@@ -446,6 +450,23 @@ double orc_transmission(const orc_atmosphere *atm, double x_slant, double tau_ae
     return exp(-tau);
 }
 
+/* detector efficiency eps(lambda) ("reduce the number of photons by one to two orders of
+ * magnitude ... atmosphere and detector efficiencies", Fig. 4.7b: mirror reflectivity x
+ * sensor efficiency): user table on a uniform wavelength grid, linear between nodes, end values
+ * held outside (reading R14).  Folded into the survival probability: p = T_atm eps. */
+double orc_efficiency(const orc_params *par, double lambda_nm)
+{
+    if (par->n_eff <= 0 || !par->eff) return 1.0;
+    if (par->n_eff == 1) return (double)par->eff[0];
+    double f = (lambda_nm - par->eff_lambda0_nm) / par->eff_dlambda_nm;
+    if (f < 0.0) f = 0.0;
+    if (f > (double)(par->n_eff - 1)) f = (double)(par->n_eff - 1);
+    int i = (int)floor(f);
+    if (i > par->n_eff - 2) i = par->n_eff - 2;
+    double fr = f - i;
+    return (1.0 - fr) * (double)par->eff[i] + fr * (double)par->eff[i + 1];
+}
+
 /* ------------------------------------------------------------------ A14 ray / sphere
  * P:1068 "hitting the bounding sphere": the line I + s u passes within r of c.
  * Returns 1 and the entry parameter s_in if hit. */
@@ -783,7 +804,7 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 }
                 /* O11 transmission */
                 if (par->trans != ORC_TRANS_OFF) {
-                    ph.T = orc_transmission(atm, x_slant, tau_aer, ph.lambda_nm);
+                    ph.T = orc_transmission(atm, x_slant, tau_aer, ph.lambda_nm) * orc_efficiency(par, ph.lambda_nm);
                     if (par->trans == ORC_TRANS_ROULETTE) {
                         if (!(u4[3] < ph.T)) { ph.status = ORC_ST_ROULETTE; lc[ORC_CNT_ROULETTE]++; goto store; }
                     } else ph.weight = par->bunch_weight * ph.T;

@@ -70,7 +70,9 @@ class Params(C.Structure):
                 ("fluor_yield_per_MeV", C.c_double), ("aim_factor", C.c_double),
                 ("n_lines", C.c_int32), ("pad", C.c_int32),
                 ("line_nm", C.POINTER(C.c_float)), ("line_cdf", C.POINTER(C.c_float)),
-                ("disp_b_nm2", C.c_double), ("disp_lambda0_nm", C.c_double)]
+                ("disp_b_nm2", C.c_double), ("disp_lambda0_nm", C.c_double),
+                ("n_eff", C.c_int32), ("pad2", C.c_int32),
+                ("eff_lambda0_nm", C.c_double), ("eff_dlambda_nm", C.c_double), ("eff", C.POINTER(C.c_float))]
 
 
 PHOTON_DTYPE = np.dtype([("seg", "<i8"), ("j", "<i4"), ("status", "<i4"),
@@ -112,6 +114,8 @@ def lib():
             L.orc_cherenkov_yield_dispersive.argtypes = [C.c_double] * 8
             L.orc_dispersion_factor.restype = C.c_double
             L.orc_dispersion_factor.argtypes = [C.c_double] * 3
+            L.orc_efficiency.restype = C.c_double
+            L.orc_efficiency.argtypes = [C.POINTER(Params), C.c_double]
             L.orc_straight_line.restype = C.c_double
             L.orc_trace.restype = C.c_int
             L.orc_trace.argtypes = [C.POINTER(Atmosphere), C.c_int, C.c_double, C.c_double, C.c_double,
@@ -186,6 +190,11 @@ def params_struct(par: dict, keep: _Keep) -> Params:
     s.line_cdf = keep.f32(par["line_cdf"]) if s.n_lines else None
     s.disp_b_nm2 = float(np.float32(par.get("disp_b_nm2", 0.0)))
     s.disp_lambda0_nm = float(np.float32(par.get("disp_lambda0_nm", 400.0)))
+    eff = par.get("eff")
+    s.n_eff = 0 if eff is None else len(eff)
+    s.eff = keep.f32(eff) if s.n_eff else None
+    s.eff_lambda0_nm = float(np.float32(par.get("eff_lambda0_nm", 0.0)))
+    s.eff_dlambda_nm = float(np.float32(par.get("eff_dlambda_nm", 1.0)))
     return s
 
 

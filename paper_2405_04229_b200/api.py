@@ -71,7 +71,8 @@ class Params(C.Structure):
                 ("lambda_min_nm", C.c_float), ("lambda_max_nm", C.c_float), ("bunch_weight", C.c_float),
                 ("lv1_margin_rad", C.c_float), ("lv2_margin_m", C.c_float),
                 ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float), ("n_lines", C.c_int32),
-                ("line_nm", _fp), ("line_cdf", _fp), ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float)]
+                ("line_nm", _fp), ("line_cdf", _fp), ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float),
+                ("n_eff", C.c_int32), ("eff_lambda0_nm", C.c_float), ("eff_dlambda_nm", C.c_float), ("eff", _fp)]
 
 
 class Segments(C.Structure):
@@ -240,7 +241,13 @@ class Context:
         p.n_lines = len(ln)
         if len(ln):
             p.line_nm, p.line_cdf = ln.ctypes.data_as(_fp), lc.ctypes.data_as(_fp)
-        return p, (ln, lc)
+        eff = par.get("eff")
+        ef = _f32(eff) if eff is not None and len(eff) else None
+        p.n_eff = 0 if ef is None else len(ef)
+        if ef is not None:
+            p.eff = ef.ctypes.data_as(_fp)
+        p.eff_lambda0_nm, p.eff_dlambda_nm = float(par.get("eff_lambda0_nm", 0.0)), float(par.get("eff_dlambda_nm", 1.0))
+        return p, (ln, lc, ef)
 
     # ---- the hot call, DEVICE buffers ------------------------------------------------------------
     def emit_propagate(self, seg_dev: dict, n_segments: int, seg_id_base: int, par: dict, seed: int,

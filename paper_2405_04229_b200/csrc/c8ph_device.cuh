@@ -86,6 +86,9 @@ struct DevRun {
     float disp_b, disp_c0;          // dispersion D(k) = disp_c0 + disp_b k^2, k = 1/lambda [1/nm]; disp_b = 0: off
     double disp_k0sq;               // 1/lambda0^2
     double il1_d, il2_d;            // 1/lambda_min, 1/lambda_max in fp64 (dispersive yield integral)
+    int n_eff;                      // detector efficiency table (0: off)
+    float eff_l0, eff_inv_dl;       // grid origin [nm], 1 / spacing
+    const float *eff;               // DEVICE [n_eff]
     uint32_t key0[10], key1[10];    // Philox round keys
     int64_t n_seg, seg_id_base;
     uint32_t local_base;            // added to the call-local segment index written into photon records

@@ -43,6 +43,8 @@ struct c8ph_ctx {
     void *d_slots = nullptr;           // prepared-segment slots of the resident warps
     float *d_lines = nullptr;          // [2][max_lines]
     int lines_cap = 0;
+    float *d_eff = nullptr;            // detector efficiency table
+    int eff_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool timed = false;
     int64_t launches = 0;
@@ -116,7 +118,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_g_kacc);
-    dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_seg);
+    dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
     if (ctx->st_h2d) {
@@ -485,6 +487,10 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         return fail(ctx, C8PH_E_ARG, "emit_propagate: wavelength band");
     if (!(p->disp_b_nm2 >= 0.f) || (p->disp_b_nm2 > 0.f && !(p->disp_lambda0_nm > 0.f)))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: dispersion needs disp_b_nm2 >= 0 and disp_lambda0_nm > 0");
+    if (p->n_eff < 0 || (p->n_eff > 0 && (!p->eff || p->trans == C8PH_TRANS_OFF || (p->n_eff > 1 && !(p->eff_dlambda_nm > 0.f)))))
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: efficiency table needs eff, eff_dlambda_nm > 0 and a transmission mode");
+    for (int k = 0; k < p->n_eff; ++k)
+        if (!(p->eff[k] >= 0.f && p->eff[k] <= 1.f)) return fail(ctx, C8PH_E_ARG, "emit_propagate: efficiency outside [0,1]");
     if (p->emit == C8PH_EMIT_FLUORESCENCE) {
         if (ctx->det.n_tel < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: fluorescence needs a telescope to aim at");
         if (p->n_lines < 1 || !p->line_nm || !p->line_cdf) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence line spectrum");
@@ -527,6 +533,17 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         if (p->trace == C8PH_TRACE_STRAIGHT) r.hit_infl = 1.0f + 1e-5f;
     }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
+    r.n_eff = p->n_eff; r.eff = nullptr;
+    r.eff_l0 = p->eff_lambda0_nm; r.eff_inv_dl = p->n_eff > 1 ? 1.0f / p->eff_dlambda_nm : 0.f;
+    if (p->n_eff > 0) {
+        if (p->n_eff > ctx->eff_cap) {
+            dfree(ctx->d_eff);
+            CU(cudaMalloc(&ctx->d_eff, (size_t)p->n_eff * sizeof(float)));
+            ctx->eff_cap = p->n_eff;
+        }
+        CU(cudaMemcpyAsync(ctx->d_eff, p->eff, (size_t)p->n_eff * sizeof(float), cudaMemcpyHostToDevice, st));
+        r.eff = ctx->d_eff;
+    }
     r.disp_b = p->emit == C8PH_EMIT_CHERENKOV ? p->disp_b_nm2 : 0.f;
     r.disp_k0sq = r.disp_b > 0.f ? 1.0 / ((double)p->disp_lambda0_nm * (double)p->disp_lambda0_nm) : 0.0;
     r.disp_c0 = (float)(1.0 - (double)r.disp_b * r.disp_k0sq);

@@ -474,6 +474,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_ray = SPEC ? true : atm.ray_inv_X > 0.f;
     const bool f_aer = SPEC ? false : atm.aer_L > 0.f;
     const bool f_disp = SPEC ? false : run.disp_b != 0.f;
+    const bool f_eff = SPEC ? false : run.n_eff > 0;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -950,7 +951,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             tau = Xs * qq * hc.ray_k;                        // optical depth in units of ln 2
                         }
                         if (f_aer) tau = fmaf(1.4426950408889634f * ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
-                        const float T = exp2_fast(-tau);
+                        float T = exp2_fast(-tau);
+                        if (f_eff) {
+                            // detector efficiency eps(lambda): linear on a uniform grid, ends held
+                            const float fl = fminf(fmaxf((rcp_fast(lam_inv) - run.eff_l0) * run.eff_inv_dl, 0.f), (float)(run.n_eff - 1));
+                            const int ie = min((int)fl, max(run.n_eff - 2, 0));
+                            const float e0 = __ldg(run.eff + ie), e1 = __ldg(run.eff + min(ie + 1, run.n_eff - 1));
+                            T *= fmaf(fl - (float)ie, e1 - e0, e0);
+                        }
                         if (f_trans == C8PH_TRANS_ROULETTE) {
                             if (!(u01(rn.w) < T)) { pkB += 0x10000u; break; }
                         } else wgt = hc.w * T;
@@ -1179,7 +1187,7 @@ static bool array_production_setting(const KArgs &a)
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr && r.disp_b == 0.f;
+           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0;
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)

@@ -432,3 +432,24 @@ def test_dispersion_yield_spectrum_and_cone():
     with pytest.raises(api.C8phError) as e:
         api.run_config(dict(cfg, params=bad), ctx=ctx)
     assert e.value.code == api.E_ARG
+
+
+def test_detector_efficiency_folding():
+    """Row f4: eps(lambda) folded into the survival probability (roulette: cfg2, cfg4) or the weight
+    (cfg1), device against oracle photon by photon; a bell-shaped curve on a 10 nm grid."""
+    lam = np.arange(200.0, 801.0, 10.0)
+    eff = (0.85 * np.exp(-0.5 * ((lam - 420.0) / 90.0) ** 2)).astype(np.float32)
+    for k, n in ((2, 20000), (4, 2500), (1, 600)):
+        cfg = W.make_config(k, n_segments=n)
+        cfg["params"].update(eff=eff, eff_lambda0_nm=200.0, eff_dlambda_nm=10.0)
+        ora, gpu, rep = _both(cfg)
+        off = api.run_config(W.make_config(k, n_segments=n))
+        if k == 1:
+            assert gpu["counters"]["landed"] == off["counters"]["landed"] and gpu["hist"].sum() < 0.8 * off["hist"].sum()
+        else:
+            assert 0.2 * off["counters"]["landed"] < gpu["counters"]["landed"] < 0.8 * off["counters"]["landed"]
+    cfg = W.make_config(0, n_segments=50)                                  # transmission off: the table is refused
+    cfg["params"].update(eff=eff, eff_lambda0_nm=200.0, eff_dlambda_nm=10.0)
+    with pytest.raises(api.C8phError) as e:
+        api.run_config(cfg)
+    assert e.value.code == api.E_ARG

@@ -5,6 +5,7 @@ Each pin is something other than the oracle itself: values the thesis prints
 results, brute force on tiny inputs.  P:n = PAPER.md line n.
 """
 import copy
+import ctypes as C
 import math
 import os
 
@@ -607,3 +608,44 @@ def test_dispersive_photons_spectrum_and_cone_angle():
     want = sum(O.lib().orc_cherenkov_yield_dispersive(float(q), 400.0, float(bb), float(np.float32(eta)), 300.0, 600.0, float(np.float32(b)), l0)
                for q, bb in zip(s["charge"], s["beta"]))
     assert abs(len(ph) - want) < 5 * math.sqrt(len(s["beta"]) / 4.0) + 1
+
+
+# ---------------------------------------------------------------------------------- detector efficiency (R14, row f4)
+def test_detector_efficiency_folding():
+    """eps(lambda) table folded into the survival probability: lookup is linear
+    between nodes and held outside; eps = 1 changes nothing; a constant eps scales the roulette
+    survivors by eps (binomial 5 sigma) and the weight-mode histogram exactly; a step eps(lambda)
+    removes exactly the photons of the dark band."""
+    keep = O._Keep()
+    par = dict(W.make_config(4, n_segments=1)["params"])
+    par.update(eff=np.array([0.0, 0.5, 1.0, 0.25], np.float32), eff_lambda0_nm=300.0, eff_dlambda_nm=100.0)
+    ps = O.params_struct(par, keep)
+    eff = lambda lam: O.lib().orc_efficiency(C.byref(ps), float(lam))
+    assert eff(300.0) == 0.0 and eff(400.0) == 0.5 and eff(350.0) == 0.25 and abs(eff(575.0) - 0.4375) < 1e-12
+    assert eff(100.0) == 0.0 and eff(900.0) == 0.25                     # end values held
+    cfg = W.make_config(2, n_segments=6000)
+    base = O.run(cfg, record=False)
+    one = copy.deepcopy(cfg)
+    one["params"].update(eff=np.ones(5, np.float32), eff_lambda0_nm=200.0, eff_dlambda_nm=150.0)
+    r1 = O.run(one, record=False)
+    assert r1["counters"] == base["counters"] and np.array_equal(r1["tel_counts"], base["tel_counts"])
+    half = copy.deepcopy(cfg)
+    half["params"].update(eff=np.full(2, 0.5, np.float32), eff_lambda0_nm=200.0, eff_dlambda_nm=600.0)
+    rh = O.run(half, record=False)
+    n0 = base["counters"]["landed"]
+    assert n0 > 20000 and abs(rh["counters"]["landed"] - 0.5 * n0) < 5 * math.sqrt(0.25 * n0)
+    assert rh["counters"]["roulette"] + rh["counters"]["landed"] == base["counters"]["roulette"] + n0
+    # weight mode: hist scales exactly
+    wcfg = W.make_config(1, n_segments=60)
+    wb = O.run(wcfg, record=False)
+    wh = copy.deepcopy(wcfg)
+    wh["params"].update(eff=np.full(3, 0.25, np.float32), eff_lambda0_nm=100.0, eff_dlambda_nm=400.0)
+    wr = O.run(wh, record=False)
+    assert np.allclose(wr["hist"], 0.25 * wb["hist"], rtol=1e-12, atol=0) and wr["counters"] == wb["counters"]
+    # step: dark below 450 nm (nodes at 449.9 / 450.1)
+    st = copy.deepcopy(cfg)
+    st["params"].update(eff=np.array([0, 0, 1, 1], np.float32), eff_lambda0_nm=449.7, eff_dlambda_nm=0.2)
+    rs = O.run(st, record=True)
+    ph = rs["photons"]
+    landed = ph[ph["status"] == O.ST_LANDED]
+    assert len(landed) > 1000 and landed["lambda_nm"].min() >= 449.9
