@@ -32,6 +32,8 @@
  *                       ray-sphere analytic cases
  *   fluorescence / camera (cfg3): isotropy moments, line frequencies,
  *                       pixel-centre round trip.
+ *   orc_last_mile (R15) focus and constant path of axis-parallel rays, camera shadow fraction,
+ *                       vertex-ray shadow rule, independent numerical intersection of skew rays.
  *   efficiency (R14)    lookup values, eps = 1 identity, constant eps scaling, step curve.
  *   dispersion (R13)    b -> 0 limit, closed form of the yield integral incl. threshold
  *                       inside the band, u.P = 1/(beta n(lambda)), KS test of the spectrum.
@@ -77,6 +79,10 @@ typedef struct {
     double cam_az_deg, cam_el_deg, cam_pix_deg;
     int32_t cam_rows, cam_cols, n_tbins, pad;
     double t_ref_ns, t_bin_ns;
+    /* last-mile optics (thesis sec. 6.4, reading R15): one parabolic mirror + camera disc per telescope */
+    int32_t opt_enabled, pad3;
+    double opt_az_deg, opt_el_deg;         /* pointing direction of every telescope */
+    double opt_focal_m, opt_mirror_radius_m, opt_camera_radius_m;
 } orc_detector;
 
 enum { ORC_EMIT_CHERENKOV = 0, ORC_EMIT_FLUOR = 1 };
@@ -509,6 +515,69 @@ int orc_camera_pixel(const orc_detector *det, const double u_arr[3])
     return best;
 }
 
+/* ------------------------------------------------------------------ last mile (row f3, reading R15)
+ * Thesis sec. 6.4: "a raytracer can replace the photon propagator in a defined area
+ * around the experiment": reflection on a (first-surface) mirror and absorption by objects, shown
+ * for "a MAGIC like telescope with 17 m diameter parabola and focal point distance of 17 m" and a
+ * camera of 1.47 m diameter, angular acceptance not considered.  Reading: inside the bounding
+ * sphere of a telescope (centre c) the photon's arrival ray I + s u meets
+ *   the camera disc  (radius R_c, centre c + (f/2) w, normal w)   from behind: absorbed (shadow),
+ *   the paraboloid   z = rho^2/(4f) about the axis w with vertex V = c - (f/2) w, rho <= R_m:
+ *                    mirror reflection  u' = u - 2 (u.n) n,
+ *   the camera disc  again, now from the mirror side: a camera hit at (x_c, y_c) in the plane
+ *                    coordinates (right, up) = (e_r, e_u), e_r = (-sin az, cos az, 0), e_u = w x e_r.
+ * w = (cos el cos az, cos el sin az, sin el) is the common pointing direction.
+ * in : I (point on the arrival ray, any), u (unit direction), c (sphere centre)
+ * out: res[0..1] camera-plane coordinates, res[2..4] reflected direction (e_r, e_u, w components),
+ *      res[5] path length from I to the camera along the ray (may start before I: s < 0 allowed)
+ * returns 1 camera hit, 0 missed mirror / camera, -1 shadowed by the camera. */
+int orc_last_mile(const orc_detector *det, const double I[3], const double u[3], const double c[3], double res[6])
+{
+    const double d2r = ORC_PI / 180.0;
+    const double az = det->opt_az_deg * d2r, el = det->opt_el_deg * d2r;
+    const double f = det->opt_focal_m, Rm = det->opt_mirror_radius_m, Rc = det->opt_camera_radius_m;
+    const double w[3] = { cos(el) * cos(az), cos(el) * sin(az), sin(el) };
+    const double er[3] = { -sin(az), cos(az), 0.0 };
+    const double eu[3] = { w[1]*er[2] - w[2]*er[1], w[2]*er[0] - w[0]*er[2], w[0]*er[1] - w[1]*er[0] };
+    double p0[3], a, b, z0, dr, du, dw;
+    for (int k = 0; k < 3; ++k) p0[k] = I[k] - (c[k] - 0.5 * f * w[k]);       /* relative to the vertex */
+    a = p0[0]*er[0] + p0[1]*er[1] + p0[2]*er[2];
+    b = p0[0]*eu[0] + p0[1]*eu[1] + p0[2]*eu[2];
+    z0 = p0[0]*w[0] + p0[1]*w[1] + p0[2]*w[2];
+    dr = u[0]*er[0] + u[1]*er[1] + u[2]*er[2];
+    du = u[0]*eu[0] + u[1]*eu[1] + u[2]*eu[2];
+    dw = u[0]*w[0] + u[1]*w[1] + u[2]*w[2];
+    if (!(dw < 0.0)) return 0;                                  /* not travelling towards the mirror */
+    /* camera disc from behind */
+    double sc = (f - z0) / dw, xs = a + sc * dr, ys = b + sc * du;
+    if (xs * xs + ys * ys <= Rc * Rc) return -1;
+    /* paraboloid: (a + s dr)^2 + (b + s du)^2 = 4 f (z0 + s dw); the ray leaves the bowl at the larger root */
+    double A = dr * dr + du * du, B = 2.0 * (a * dr + b * du) - 4.0 * f * dw, C = a * a + b * b - 4.0 * f * z0;
+    double sh;
+    if (A < 1e-18) sh = -C / B;
+    else {
+        double disc = B * B - 4.0 * A * C;
+        if (disc < 0.0) return 0;
+        double q = -0.5 * (B + (B >= 0.0 ? sqrt(disc) : -sqrt(disc)));
+        double s1 = q / A, s2 = (q != 0.0) ? C / q : s1;
+        sh = s1 > s2 ? s1 : s2;
+    }
+    double x = a + sh * dr, y = b + sh * du, z = z0 + sh * dw;
+    if (x * x + y * y > Rm * Rm) return 0;
+    /* mirror normal (towards the focus) and reflection */
+    double n[3] = { -x / (2.0 * f), -y / (2.0 * f), 1.0 };
+    double nn = sqrt(n[0]*n[0] + n[1]*n[1] + 1.0);
+    n[0] /= nn; n[1] /= nn; n[2] /= nn;
+    double dn = dr * n[0] + du * n[1] + dw * n[2];
+    double r[3] = { dr - 2.0 * dn * n[0], du - 2.0 * dn * n[1], dw - 2.0 * dn * n[2] };
+    if (!(r[2] > 0.0)) return 0;
+    double s2c = (f - z) / r[2];
+    double xc = x + s2c * r[0], yc = y + s2c * r[1];
+    if (xc * xc + yc * yc > Rc * Rc) return 0;
+    res[0] = xc; res[1] = yc; res[2] = r[0]; res[3] = r[1]; res[4] = r[2]; res[5] = sh + s2c;
+    return 1;
+}
+
 /* ------------------------------------------------------------------ per-segment quantities */
 typedef struct {
     double A[3], P[3], L, beta, t0, M[9];
@@ -852,6 +921,20 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                         if (tel_counts) {
                             #pragma omp atomic
                             tel_counts[ph.tel] += ph.weight;
+                        }
+                        if (det->opt_enabled) {
+                            /* R15 last mile: the record becomes the camera-plane hit (x_c, y_c), the
+                             * reflected direction in the telescope frame (stored as (r, u, -w) so that the
+                             * third component keeps the record's sign convention) and the camera time */
+                            const float *t = det->tel_xyzr + 4*ph.tel;
+                            double c[3] = { t[0], t[1], t[2] }, res[6];
+                            if (orc_last_mile(det, Ip, ua, c, res) == 1) {
+                                ph.pix = 0;
+                                lc[ORC_CNT_CAM_HIT]++;
+                                ph.x = res[0]; ph.y = res[1];
+                                ph.ux = res[2]; ph.uy = res[3]; ph.uz = -res[4];
+                                ph.t += res[5] / ORC_C_M_PER_NS;
+                            }
                         }
                         if (det->cam_enabled) {
                             ph.pix = orc_camera_pixel(det, ua);

@@ -59,7 +59,10 @@ class Detector(C.Structure):
                 ("n_tel", C.c_int32), ("cam_enabled", C.c_int32), ("tel_xyzr", C.POINTER(C.c_float)),
                 ("cam_az_deg", C.c_double), ("cam_el_deg", C.c_double), ("cam_pix_deg", C.c_double),
                 ("cam_rows", C.c_int32), ("cam_cols", C.c_int32), ("n_tbins", C.c_int32), ("pad", C.c_int32),
-                ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_double)]
+                ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_double),
+                ("opt_enabled", C.c_int32), ("pad3", C.c_int32),
+                ("opt_az_deg", C.c_double), ("opt_el_deg", C.c_double),
+                ("opt_focal_m", C.c_double), ("opt_mirror_radius_m", C.c_double), ("opt_camera_radius_m", C.c_double)]
 
 
 class Params(C.Structure):
@@ -114,6 +117,8 @@ def lib():
             L.orc_cherenkov_yield_dispersive.argtypes = [C.c_double] * 8
             L.orc_dispersion_factor.restype = C.c_double
             L.orc_dispersion_factor.argtypes = [C.c_double] * 3
+            L.orc_last_mile.restype = C.c_int
+            L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 4
             L.orc_efficiency.restype = C.c_double
             L.orc_efficiency.argtypes = [C.POINTER(Params), C.c_double]
             L.orc_straight_line.restype = C.c_double
@@ -175,6 +180,11 @@ def detector_struct(det: dict, keep: _Keep) -> Detector:
     s.cam_az_deg, s.cam_el_deg, s.cam_pix_deg = (float(np.float32(det[k])) for k in ("cam_az_deg", "cam_el_deg", "cam_pix_deg"))
     s.cam_rows, s.cam_cols, s.n_tbins = int(det["cam_rows"]), int(det["cam_cols"]), int(det["n_tbins"])
     s.t_ref_ns, s.t_bin_ns = float(det["t_ref_ns"]), float(np.float32(det["t_bin_ns"]))
+    s.opt_enabled = int(bool(det.get("opt_enabled", False)))
+    s.opt_az_deg, s.opt_el_deg = float(np.float32(det.get("opt_az_deg", 0.0))), float(np.float32(det.get("opt_el_deg", 90.0)))
+    s.opt_focal_m = float(np.float32(det.get("opt_focal_m", 1.0)))
+    s.opt_mirror_radius_m = float(np.float32(det.get("opt_mirror_radius_m", 0.0)))
+    s.opt_camera_radius_m = float(np.float32(det.get("opt_camera_radius_m", 0.0)))
     return s
 
 

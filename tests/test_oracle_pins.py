@@ -649,3 +649,117 @@ def test_detector_efficiency_folding():
     ph = rs["photons"]
     landed = ph[ph["status"] == O.ST_LANDED]
     assert len(landed) > 1000 and landed["lambda_nm"].min() >= 449.9
+
+
+# ---------------------------------------------------------------------------------- last mile (R15, row f3)
+def _optics_det(az=30.0, el=70.0, f=17.0, rm=8.5, rc=0.735):
+    det = dict(W.make_config(4, n_segments=1)["detector"])
+    det.update(opt_enabled=True, opt_az_deg=az, opt_el_deg=el, opt_focal_m=f, opt_mirror_radius_m=rm, opt_camera_radius_m=rc)
+    return det
+
+
+def _last_mile(ds, I, u, c):
+    arr = lambda v: (C.c_double * len(v))(*[float(x) for x in v])
+    res = (C.c_double * 6)()
+    rc = O.lib().orc_last_mile(C.byref(ds), arr(I), arr(u), arr(c), res)
+    return rc, np.array(res[:])
+
+
+def test_last_mile_parabolic_mirror_and_camera():
+    """Thesis sec. 6.4, the MAGIC-like telescope it shows (17 m parabola, f = 17 m, camera
+    1.47 m): rays parallel to the axis focus to the camera centre with the constant path length of the
+    focus-directrix property; the camera shadows (R_c/R_m)^2 of the aperture; the ray through the vertex
+    is shadowed exactly while f tan(delta) <= R_c; |u'| = 1; and an independent numerical intersection (root bracketing on the
+    surface function, normal from its gradient) gives the same camera point for skew rays."""
+    from scipy import optimize
+    keep = O._Keep()
+    az, el, f, rm, rc = 30.0, 70.0, 17.0, 8.5, 0.735
+    ds = O.detector_struct(_optics_det(az, el, f, rm, rc), keep)
+    a, e = np.radians(az), np.radians(el)
+    w = np.array([np.cos(e) * np.cos(a), np.cos(e) * np.sin(a), np.sin(e)])
+    er = np.array([-np.sin(a), np.cos(a), 0.0])
+    eu = np.cross(w, er)
+    c = np.array([120.0, -40.0, 9.0])
+    V = c - 0.5 * f * w
+    rng = np.random.default_rng(5)
+    n_hit = n_shadow = 0
+    for _ in range(4000):
+        rho, ph = rm * np.sqrt(rng.uniform()), rng.uniform(0, 2 * np.pi)
+        x, y = rho * np.cos(ph), rho * np.sin(ph)
+        z_start = 30.0
+        I = V + x * er + y * eu + z_start * w
+        code, res = _last_mile(ds, I, -w, c)
+        if rho <= rc:
+            assert code == -1
+            n_shadow += 1
+        else:
+            assert code == 1 and np.hypot(res[0], res[1]) < 1e-9
+            assert abs(res[5] - (z_start + f)) < 1e-9                    # focus-directrix: constant path
+            assert abs(np.linalg.norm(res[2:5]) - 1.0) < 1e-12
+            n_hit += 1
+    assert abs(n_shadow / 4000.0 - (rc / rm) ** 2) < 5 * math.sqrt((rc / rm) ** 2 / 4000.0)
+    # outside the aperture / wrong way
+    assert _last_mile(ds, V + (rm + 0.01) * er + 30.0 * w, -w, c)[0] == 0
+    assert _last_mile(ds, V + 3.0 * er + 30.0 * w, w, c)[0] == 0
+    # the ray through the vertex, tilted by delta, crosses the camera plane at f tan(delta) on its way in and
+    # would image at the mirrored point: shadowed while that is inside the camera, a miss beyond it
+    for delta in (0.002, 0.01, 0.03, 0.05, 0.08):
+        d = np.sin(delta) * er - np.cos(delta) * w
+        code, res = _last_mile(ds, V - 40.0 * d, d, c)
+        assert code == (-1 if f * np.tan(delta) <= rc else 0)
+    # skew rays against an independent numerical construction
+    checked = 0
+    for _ in range(300):
+        tilt, pa = rng.uniform(0, 0.03), rng.uniform(0, 2 * np.pi)
+        d = np.sin(tilt) * (np.cos(pa) * er + np.sin(pa) * eu) - np.cos(tilt) * w
+        rho, ph = rm * np.sqrt(rng.uniform()), rng.uniform(0, 2 * np.pi)
+        I = V + rho * np.cos(ph) * er + rho * np.sin(ph) * eu + 25.0 * w
+        code, res = _last_mile(ds, I, d, c)
+        loc = lambda s: np.array([(I + s * d - V) @ er, (I + s * d - V) @ eu, (I + s * d - V) @ w])
+        g = lambda s: loc(s)[2] - (loc(s)[0] ** 2 + loc(s)[1] ** 2) / (4 * f)
+        s_hit = optimize.brentq(g, 0.0, 60.0, xtol=1e-13)
+        p = loc(s_hit)
+        cam_cross = loc((f - (I - V) @ w) / (d @ w))
+        if np.hypot(cam_cross[0], cam_cross[1]) <= rc:
+            assert code == -1
+            continue
+        if np.hypot(p[0], p[1]) > rm:
+            assert code == 0
+            continue
+        grad = np.array([-p[0] / (2 * f), -p[1] / (2 * f), 1.0])
+        nrm = grad / np.linalg.norm(grad)
+        dl = np.array([d @ er, d @ eu, d @ w])
+        r = dl - 2 * (dl @ nrm) * nrm
+        s2 = (f - p[2]) / r[2]
+        xc, yc = p[0] + s2 * r[0], p[1] + s2 * r[1]
+        if np.hypot(xc, yc) <= rc:
+            assert code == 1 and abs(res[0] - xc) < 1e-9 and abs(res[1] - yc) < 1e-9 and abs(res[5] - (s_hit + s2)) < 1e-9
+            checked += 1
+        else:
+            assert code == 0
+    assert checked > 50
+
+
+def test_last_mile_in_the_run():
+    """With optics on, camera hits are a subset of the sphere hits, the rest of the run is unchanged, and
+    the recorded camera points lie inside the camera disc; arrival at the camera is later than at the
+    bounding sphere's entry by at most the sphere diameter plus the focal length."""
+    cfg = W.make_config(4, n_segments=400)
+    tel = cfg["detector"]["tel_xyzr"].copy()
+    tel[:, 3] = 12.0                                                      # sphere holds mirror and camera
+    cfg["detector"]["tel_xyzr"] = tel
+    base = O.run(cfg, record=True)
+    cfg["detector"].update(opt_enabled=True, opt_az_deg=0.0, opt_el_deg=70.0, opt_focal_m=17.0,
+                           opt_mirror_radius_m=8.5, opt_camera_radius_m=0.735)
+    opt = O.run(cfg, record=True)
+    for k in ("emitted", "landed", "in_grid", "tel_hit"):
+        assert opt["counters"][k] == base["counters"][k]
+    assert 0 < opt["counters"]["cam_hit"] < opt["counters"]["tel_hit"]
+    ph = opt["photons"]
+    cam = ph[ph["pix"] == 0]
+    assert len(cam) == opt["counters"]["cam_hit"] and np.all(cam["tel"] >= 0)
+    assert np.all(np.hypot(cam["x"], cam["y"]) <= 0.735 + 1e-12)
+    b = base["photons"]
+    kb = {(int(s), int(j)): t for s, j, t in zip(b["seg"], b["j"], b["t"])}
+    dt = np.array([t - kb[(int(s), int(j))] for s, j, t in zip(cam["seg"], cam["j"], cam["t"])])
+    assert np.all(np.abs(dt) < (24.0 + 17.0 + 20.0) / 0.299792458)
