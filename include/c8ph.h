@@ -97,6 +97,16 @@ typedef struct {
     int32_t cam_rows, cam_cols, n_tbins;
     double t_ref_ns;                 /* photon times are reported relative to t_ref               */
     float t_bin_ns;
+    /* Last-mile optics inside the bounding spheres (thesis sec. 6.4): every telescope is a
+     * parabolic first-surface mirror (focal length f, aperture radius R_m, vertex at centre - (f/2) w)
+     * with a camera disc (radius R_c, at centre + (f/2) w) that also shadows the mirror; w = pointing
+     * direction (azimuth from +x towards +y, elevation above the horizon).  With WRITE_TEL only camera
+     * hits are written: record.x,y = camera-plane coordinates [m] along (right, up) =
+     * ((-sin az, cos az, 0), w x right), record.ux,uy = reflected direction along (right, up) (the ray
+     * travels towards +w), t = arrival at the camera; counters[CAM_HIT] counts them.  The spheres must
+     * contain mirror and camera.  Excludes cam_enabled and WRITE_ALL.                               */
+    int32_t opt_enabled;
+    float opt_az_deg, opt_el_deg, opt_focal_m, opt_mirror_radius_m, opt_camera_radius_m;
 } c8ph_detector;
 /* Copies the telescope list and builds the two uniform-grid accelerators on the host (per cell: the
  * candidate telescopes sorted by a lower-bound key, the smallest key, an accept bound); synchronous.

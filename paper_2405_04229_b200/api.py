@@ -62,7 +62,9 @@ class Detector(C.Structure):
                 ("n_tel", C.c_int32), ("tel_xyzr", _fp), ("cam_enabled", C.c_int32),
                 ("cam_axis_az_deg", C.c_float), ("cam_axis_el_deg", C.c_float), ("cam_pix_deg", C.c_float),
                 ("cam_rows", C.c_int32), ("cam_cols", C.c_int32), ("n_tbins", C.c_int32),
-                ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_float)]
+                ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_float),
+                ("opt_enabled", C.c_int32), ("opt_az_deg", C.c_float), ("opt_el_deg", C.c_float),
+                ("opt_focal_m", C.c_float), ("opt_mirror_radius_m", C.c_float), ("opt_camera_radius_m", C.c_float)]
 
 
 class Params(C.Structure):
@@ -216,6 +218,10 @@ class Context:
         d.cam_pix_deg = float(det["cam_pix_deg"])
         d.cam_rows, d.cam_cols, d.n_tbins = int(det["cam_rows"]), int(det["cam_cols"]), int(det["n_tbins"])
         d.t_ref_ns, d.t_bin_ns = float(det["t_ref_ns"]), float(det["t_bin_ns"])
+        d.opt_enabled = int(bool(det.get("opt_enabled", False)))
+        d.opt_az_deg, d.opt_el_deg = float(det.get("opt_az_deg", 0.0)), float(det.get("opt_el_deg", 90.0))
+        d.opt_focal_m = float(det.get("opt_focal_m", 1.0))
+        d.opt_mirror_radius_m, d.opt_camera_radius_m = float(det.get("opt_mirror_radius_m", 0.0)), float(det.get("opt_camera_radius_m", 0.0))
         self._check(self.lib.c8ph_set_detector(self._h, C.byref(d)))
         self._det = dict(det)
         self._n_tel = tel.shape[0]

@@ -67,6 +67,9 @@ struct DevDet {
     float cam_pitch, cam_inv_pitch;       // [rad]
     double t_ref;
     float t_bin, inv_t_bin;
+    int opt_enabled;                      // last-mile optics inside the bounding spheres
+    float opt_w[3], opt_r[3], opt_u[3];   // telescope frame: pointing axis, right, up
+    float opt_f, opt_rm2, opt_rc2;        // focal length, mirror radius^2, camera radius^2
 };
 
 struct DevRun {

@@ -415,6 +415,14 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
     if (d->n_tel < 0 || d->n_tel >= (int)C8PH_TEL_NONE || (d->n_tel > 0 && !d->tel_xyzr)) return fail(ctx, C8PH_E_ARG, "set_detector: telescopes");
     if (d->cam_enabled && (d->n_tel < 1 || d->cam_rows < 1 || d->cam_cols < 1 || d->n_tbins < 1 || !(d->cam_pix_deg > 0.f) || !(d->t_bin_ns > 0.f)))
         return fail(ctx, C8PH_E_ARG, "set_detector: camera needs a telescope, rows, cols, time bins");
+    if (d->opt_enabled) {
+        if (d->cam_enabled || d->n_tel < 1 || !(d->opt_focal_m > 0.f) || !(d->opt_mirror_radius_m > 0.f) || !(d->opt_camera_radius_m > 0.f))
+            return fail(ctx, C8PH_E_ARG, "set_detector: optics need telescopes, focal length, mirror and camera radius; not with cam_enabled");
+        const double f = d->opt_focal_m, rm = d->opt_mirror_radius_m, rc = d->opt_camera_radius_m;
+        const double need = std::max(std::sqrt(0.25 * f * f + rc * rc), std::sqrt(std::pow(0.5 * f - rm * rm / (4.0 * f), 2) + rm * rm));
+        for (int k = 0; k < d->n_tel; ++k)
+            if (d->tel_xyzr[4 * k + 3] < need) return fail(ctx, C8PH_E_ARG, "set_detector: a bounding sphere does not contain the mirror and the camera");
+    }
     CU(cudaSetDevice(ctx->device));
     DevDet o{};
     o.hist_nx = d->hist_nx; o.hist_ny = d->hist_ny;
@@ -444,6 +452,17 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
         for (int k = 0; k < 3; ++k) { o.cam_w[k] = (float)w[k]; o.cam_r[k] = (float)r[k]; o.cam_u[k] = (float)u[k]; }
         o.cam_pitch = (float)(d->cam_pix_deg * d2r);
         o.cam_inv_pitch = d->cam_pix_deg > 0.f ? (float)(1.0 / (d->cam_pix_deg * d2r)) : 0.f;
+    }
+    o.opt_enabled = d->opt_enabled ? 1 : 0;
+    {
+        const double d2r = 3.14159265358979323846 / 180.0;
+        const double az = d->opt_az_deg * d2r, el = d->opt_el_deg * d2r;
+        const double w[3] = {std::cos(el) * std::cos(az), std::cos(el) * std::sin(az), std::sin(el)};
+        const double r[3] = {-std::sin(az), std::cos(az), 0.0};
+        const double u[3] = {w[1] * r[2] - w[2] * r[1], w[2] * r[0] - w[0] * r[2], w[0] * r[1] - w[1] * r[0]};
+        for (int k = 0; k < 3; ++k) { o.opt_w[k] = (float)w[k]; o.opt_r[k] = (float)r[k]; o.opt_u[k] = (float)u[k]; }
+        o.opt_f = d->opt_focal_m; o.opt_rm2 = d->opt_mirror_radius_m * d->opt_mirror_radius_m;
+        o.opt_rc2 = d->opt_camera_radius_m * d->opt_camera_radius_m;
     }
     o.t_ref = d->t_ref_ns; o.t_bin = d->t_bin_ns; o.inv_t_bin = d->t_bin_ns > 0.f ? 1.0f / d->t_bin_ns : 0.f;
     dfree(ctx->d_tel);
@@ -485,6 +504,8 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     if (p->trace == C8PH_TRACE_NUMERIC && p->emit == C8PH_EMIT_FLUORESCENCE) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence + numeric tracing");
     if (p->emit == C8PH_EMIT_CHERENKOV && !(p->lambda_min_nm > 0.f && p->lambda_max_nm > p->lambda_min_nm))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: wavelength band");
+    if (ctx->det.opt_enabled && p->write == C8PH_WRITE_ALL)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: WRITE_ALL is not defined with last-mile optics (records are camera hits)");
     if (!(p->disp_b_nm2 >= 0.f) || (p->disp_b_nm2 > 0.f && !(p->disp_lambda0_nm > 0.f)))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: dispersion needs disp_b_nm2 >= 0 and disp_lambda0_nm > 0");
     if (p->n_eff < 0 || (p->n_eff > 0 && (!p->eff || p->trans == C8PH_TRANS_OFF || (p->n_eff > 1 && !(p->eff_dlambda_nm > 0.f)))))

@@ -475,6 +475,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_aer = SPEC ? false : atm.aer_L > 0.f;
     const bool f_disp = SPEC ? false : run.disp_b != 0.f;
     const bool f_eff = SPEC ? false : run.n_eff > 0;
+    const bool f_opt = SPEC ? false : det.opt_enabled != 0;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -492,6 +493,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         const uint32_t jslot = __float_as_uint(q3.w);
         int tel = -1;
         float uax = ux, uay = uy, uaz = uz, t_arr = 0.f;
+        float rx_out = xg, ry_out = yg;                       // record position (ground plane, or camera plane with optics)
+        bool opt_hit = false;
         const SegSlot *sl = g_slot + (jslot & 31u);
         const SegHot *sh = &sl->h;
         const SegCold *sc = &sl->c;
@@ -534,6 +537,57 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             if (tel >= 0) {
                 pkC += 0x10000u;
                 if (f_telc) atomicAdd(run.out.tel_counts + tel, wgt);
+                if (f_opt) {
+                    // last mile (thesis sec. 6.4): camera shadow, parabolic mirror z = rho^2/(4f) about the
+                    // pointing axis (vertex at centre - (f/2) w), reflection, camera disc at z = f
+                    const float4 tc = __ldg(det.tel + tel);
+                    const float f = det.opt_f, hf = 0.5f * f;
+                    const float px = xg - (tc.x - hf * det.opt_w[0]), py = yg - (tc.y - hf * det.opt_w[1]), pz = -(tc.z - hf * det.opt_w[2]);
+                    const float a0 = px * det.opt_r[0] + py * det.opt_r[1] + pz * det.opt_r[2];
+                    const float b0 = px * det.opt_u[0] + py * det.opt_u[1] + pz * det.opt_u[2];
+                    const float z0 = px * det.opt_w[0] + py * det.opt_w[1] + pz * det.opt_w[2];
+                    const float dr = uax * det.opt_r[0] + uay * det.opt_r[1] + uaz * det.opt_r[2];
+                    const float du = uax * det.opt_u[0] + uay * det.opt_u[1] + uaz * det.opt_u[2];
+                    const float dw = uax * det.opt_w[0] + uay * det.opt_w[1] + uaz * det.opt_w[2];
+                    if (dw < 0.f) {
+                        const float sc0 = (f - z0) * rcp_fast(dw);
+                        const float xs = fmaf(sc0, dr, a0), ys = fmaf(sc0, du, b0);
+                        if (xs * xs + ys * ys > det.opt_rc2) {                       // not shadowed by the camera
+                            const float A = dr * dr + du * du, B = 2.f * (a0 * dr + b0 * du) - 4.f * f * dw;
+                            const float C = a0 * a0 + b0 * b0 - 4.f * f * z0;
+                            float sh = 0.f;
+                            bool ok = true;
+                            if (A < 1e-12f) sh = -C * rcp_fast(B);
+                            else {
+                                const float disc = B * B - 4.f * A * C;
+                                ok = disc >= 0.f;
+                                const float sq = sqrt_fast(fmaxf(disc, 0.f));
+                                const float qq = -0.5f * (B + (B >= 0.f ? sq : -sq));
+                                const float s1 = qq * rcp_fast(A), s2 = qq != 0.f ? C * rcp_fast(qq) : s1;
+                                sh = fmaxf(s1, s2);                                  // the ray leaves the bowl at the larger root
+                            }
+                            const float x = fmaf(sh, dr, a0), y = fmaf(sh, du, b0), z = fmaf(sh, dw, z0);
+                            if (ok && x * x + y * y <= det.opt_rm2) {
+                                const float i2f = 0.5f * rcp_fast(f);
+                                float nx = -x * i2f, ny = -y * i2f;
+                                const float inn = rsqrt_fast(nx * nx + ny * ny + 1.f);
+                                nx *= inn; ny *= inn;
+                                const float dn = dr * nx + du * ny + dw * inn;
+                                const float r0 = fmaf(-2.f * dn, nx, dr), r1 = fmaf(-2.f * dn, ny, du), r2 = fmaf(-2.f * dn, inn, dw);
+                                if (r2 > 0.f) {
+                                    const float s2c = (f - z) * rcp_fast(r2);
+                                    const float xc = fmaf(s2c, r0, x), yc = fmaf(s2c, r1, y);
+                                    if (xc * xc + yc * yc <= det.opt_rc2) {
+                                        opt_hit = true;
+                                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                                        rx_out = xc; ry_out = yc; uax = r0; uay = r1;
+                                        t_arr = fmaf(sh + s2c, kInvC, t_arr);
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
                 if (f_cam) {
                     const int pix = camera_pixel(det, uax, uay, uaz);
                     const float tb = floorf(t_arr * det.inv_t_bin);
@@ -546,7 +600,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         }
         // a16: survivors are ranked by warp ballot and stored straight from registers: one cursor
         // atomic per call, consecutive 32 B records
-        const bool write = act && (f_write == C8PH_WRITE_ALL || (f_write == C8PH_WRITE_TEL && tel >= 0));
+        const bool write = act && (f_write == C8PH_WRITE_ALL || (f_write == C8PH_WRITE_TEL && (f_opt ? opt_hit : tel >= 0)));
         if (f_photons) {
             const unsigned wm = __ballot_sync(FULL, write);
             if (wm) {
@@ -557,7 +611,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const long long idx = (long long)base + __popc(wm & ((1u << lane) - 1u));
                     if (idx < run.out.photon_capacity) {
                         uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + idx);
-                        dst[0] = make_uint4(__float_as_uint(xg), __float_as_uint(yg), __float_as_uint(uax), __float_as_uint(uay));
+                        dst[0] = make_uint4(__float_as_uint(rx_out), __float_as_uint(ry_out), __float_as_uint(uax), __float_as_uint(uay));
                         dst[1] = make_uint4(__float_as_uint(t_arr), __float_as_uint(rcp_fast(lam_inv)), sc->local,
                                             ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE));
                         if (run.out.photon_weight) run.out.photon_weight[idx] = wgt;
@@ -1187,7 +1241,7 @@ static bool array_production_setting(const KArgs &a)
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0;
+           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled;
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)

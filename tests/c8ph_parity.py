@@ -70,6 +70,8 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
     oph = ora["photons"]
     if par["write"] == "all":
         want = oph[oph["status"] == O.ST_LANDED]
+    elif par["write"] == "tel" and det.get("opt_enabled"):
+        want = oph[(oph["status"] == O.ST_LANDED) & (oph["tel"] >= 0) & (oph["pix"] >= 0)]   # camera hits (R15)
     elif par["write"] == "tel":
         want = oph[(oph["status"] == O.ST_LANDED) & (oph["tel"] >= 0)]
     else:
@@ -117,7 +119,7 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
         w = gpu["photon_weight"][gi][ia][near]
         assert np.allclose(w, o["weight"], rtol=2e-5, atol=0), "photon weight"
     # per-photon bin agreement recomputed from the device positions (hist grid only)
-    if det["hist_nx"] > 0 and not det["cam_enabled"] and len(g):
+    if det["hist_nx"] > 0 and not det["cam_enabled"] and not det.get("opt_enabled") and len(g):
         bx = np.floor((g["x"].astype(np.float64) - det["hist_x0"]) / det["hist_cell"])
         by = np.floor((g["y"].astype(np.float64) - det["hist_y0"]) / det["hist_cell"])
         inside = (bx >= 0) & (bx < det["hist_nx"]) & (by >= 0) & (by < det["hist_ny"])

@@ -453,3 +453,28 @@ def test_detector_efficiency_folding():
     with pytest.raises(api.C8phError) as e:
         api.run_config(cfg)
     assert e.value.code == api.E_ARG
+
+
+def test_last_mile_optics():
+    """Row f3 (thesis sec. 6.4): parabolic mirror + shadowing camera inside the bounding spheres, fused
+    after the sphere test so that only camera hits are written.  The MAGIC-like telescope of the thesis
+    (17 m parabola, f = 17 m, 1.47 m camera) on cfg4's lattice and on cfg2's inclined shower with the
+    telescopes pointed at the shower; records are camera-plane points, compared photon by photon."""
+    for k, n, az, el in ((4, 4000, 0.0, 70.0), (2, 40000, 30.0, 30.0)):
+        cfg = W.make_config(k, n_segments=n)
+        tel = cfg["detector"]["tel_xyzr"].copy()
+        tel[:, 3] = 12.0
+        cfg["detector"]["tel_xyzr"] = tel
+        base = api.run_config(cfg)
+        cfg["detector"].update(opt_enabled=True, opt_az_deg=az, opt_el_deg=el, opt_focal_m=17.0,
+                               opt_mirror_radius_m=8.5, opt_camera_radius_m=0.735)
+        ora, gpu, rep = _both(cfg)
+        c = gpu["counters"]
+        assert c["tel_hit"] == base["counters"]["tel_hit"] and 50 < c["cam_hit"] == c["written"] < c["tel_hit"]
+        ph = gpu["photons"]
+        assert np.all(np.hypot(ph["x"], ph["y"]) <= 0.735 * (1 + 1e-5))
+        assert rep["max_dpos_m"] < 2e-3                                    # camera-plane agreement: mm
+    cfg["detector"]["tel_xyzr"][:, 3] = 6.0                                # sphere too small for the optics
+    with pytest.raises(api.C8phError) as e:
+        api.setup_context(cfg)
+    assert e.value.code == api.E_ARG
