@@ -117,6 +117,9 @@ def lib():
             L.orc_cherenkov_yield_dispersive.argtypes = [C.c_double] * 8
             L.orc_dispersion_factor.restype = C.c_double
             L.orc_dispersion_factor.argtypes = [C.c_double] * 3
+            L.orc_substep_track.restype = C.c_int32
+            L.orc_substep_track.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)] + [C.c_double] * 5 + \
+                                           [C.POINTER(C.c_double), C.c_double, C.c_int32, C.POINTER(C.c_float)]
             L.orc_last_mile.restype = C.c_int
             L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 4
             L.orc_efficiency.restype = C.c_double
@@ -382,3 +385,29 @@ def run(cfg: dict, record: bool = True, table_data: np.ndarray | None = None, th
         raise RuntimeError(f"orc_run failed: {rc}")
     return dict(hist=hist[:n_hist], tel_counts=tel[:det.n_tel], n_bunch=n_bunch, total_bunches=int(total),
                 counters={k: int(v) for k, v in zip(COUNTER_NAMES, cnt)}, photons=photons)
+
+
+def substep_tracks(tracks: dict, B, tol_m: float, max_sub: int = 4096) -> dict:
+    """R16: cut helical tracks (dict of float32 arrays x,y,z,dx,dy,dz,len,beta,t0,charge,p_GeV) into chords.
+    Returns dict(segments={x..charge,edep}, offsets=int64[n+1])."""
+    L = lib()
+    n = len(tracks["x"])
+    Bd = (C.c_double * 3)(*[float(np.float32(b)) for b in B])
+    counts = np.zeros(n, dtype=np.int64)
+    arr = lambda v: (C.c_double * 3)(*[float(x) for x in v])
+    args = []
+    for i in range(n):
+        a = (arr([tracks[k][i] for k in ("x", "y", "z")]), arr([tracks[k][i] for k in ("dx", "dy", "dz")]),
+             float(tracks["len"][i]), float(tracks["beta"][i]), float(tracks["t0"][i]), float(tracks["charge"][i]),
+             float(tracks["p_GeV"][i]))
+        args.append(a)
+        counts[i] = L.orc_substep_track(a[0], a[1], a[2], a[3], a[4], a[5], a[6], Bd, float(np.float32(tol_m)), int(max_sub), None)
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    out = np.zeros((int(offsets[-1]), 10), dtype=np.float32)
+    for i, a in enumerate(args):
+        L.orc_substep_track(a[0], a[1], a[2], a[3], a[4], a[5], a[6], Bd, float(np.float32(tol_m)), int(max_sub),
+                            out[offsets[i]:].ctypes.data_as(C.POINTER(C.c_float)))
+    names = ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge")
+    seg = {k: np.ascontiguousarray(out[:, j]) for j, k in enumerate(names)}
+    seg["edep"] = np.zeros(len(out), dtype=np.float32)
+    return dict(segments=seg, offsets=offsets)

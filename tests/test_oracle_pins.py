@@ -763,3 +763,72 @@ def test_last_mile_in_the_run():
     kb = {(int(s), int(j)): t for s, j, t in zip(b["seg"], b["j"], b["t"])}
     dt = np.array([t - kb[(int(s), int(j))] for s, j, t in zip(cam["seg"], cam["j"], cam["t"])])
     assert np.all(np.abs(dt) < (24.0 + 17.0 + 20.0) / 0.299792458)
+
+
+# ---------------------------------------------------------------------------------- sub-stepping (R16, row f2)
+def test_substepping_follows_the_lorentz_helix():
+    """Thesis sec. 4.2.1: chords of the magnetic path.  The chord end points agree with an
+    independent RK4 integration of dP/ds = kappa P x B/|B|; every chord's sagitta is <= tol (and the
+    piece count is the smallest that achieves it); chord lengths and clocks add up; no field or a stiff
+    particle returns the track unchanged; opposite charges bend to opposite sides."""
+    rng = np.random.default_rng(11)
+    n = 40
+    v = rng.normal(size=(n, 3)); v[:, 2] = -np.abs(v[:, 2]) - 0.5
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    trk = dict(x=rng.uniform(-100, 100, n), y=rng.uniform(-100, 100, n), z=rng.uniform(3e3, 2e4, n),
+               dx=v[:, 0], dy=v[:, 1], dz=v[:, 2], len=rng.uniform(20, 300, n), beta=np.full(n, 0.9999),
+               t0=rng.uniform(0, 1e4, n), charge=rng.choice([-1.0, 1.0], n), p_GeV=10 ** rng.uniform(-2, 0.5, n))
+    trk = {k: np.asarray(a, dtype=np.float32) for k, a in trk.items()}
+    B, tol = (2.0e-5, -0.5e-5, -4.3e-5), 0.01
+    res = O.substep_tracks(trk, B, tol)
+    seg, off = res["segments"], res["offsets"]
+    assert off[-1] > 2 * n and np.all(np.diff(off) >= 1)
+    Bv = np.array([float(np.float32(b)) for b in B]); bh = Bv / np.linalg.norm(Bv)
+    for i in range(n):
+        A = np.array([trk["x"][i], trk["y"][i], trk["z"][i]], dtype=np.float64)
+        P = np.array([trk["dx"][i], trk["dy"][i], trk["dz"][i]], dtype=np.float64); P /= np.linalg.norm(P)
+        L, q, p = float(trk["len"][i]), float(trk["charge"][i]), float(trk["p_GeV"][i])
+        kappa = 0.299792458 * q * np.linalg.norm(Bv) / p
+        m = off[i + 1] - off[i]
+        # independent RK4 on (X, P)
+        steps = 400 * m
+        h = L / steps
+        X, Pv = A.copy(), P.copy()
+        f = lambda Pq: kappa * np.cross(Pq, bh)
+        ends = [X.copy()]; mids = []
+        for s in range(steps):
+            k1 = f(Pv); k2 = f(Pv + 0.5 * h * k1); k3 = f(Pv + 0.5 * h * k2); k4 = f(Pv + h * k3)
+            X = X + h * (Pv + (h / 6.0) * (k1 + k2 + k3))
+            Pv = Pv + (h / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
+            if (s + 1) % 400 == 0: ends.append(X.copy())
+            if (s + 1) % 400 == 200: mids.append(X.copy())
+        ends = np.array(ends)
+        got0 = np.stack([seg[k][off[i]:off[i + 1]] for k in ("x", "y", "z")], axis=1).astype(np.float64)
+        d = np.stack([seg[k][off[i]:off[i + 1]] for k in ("dx", "dy", "dz")], axis=1).astype(np.float64)
+        ln = seg["len"][off[i]:off[i + 1]].astype(np.float64)
+        got1 = got0 + d * ln[:, None]
+        scale = 4e-7 * np.abs(A).max() + 1e-4                                # fp32 storage of km coordinates
+        assert np.abs(got0 - ends[:-1]).max() < scale and np.abs(got1 - ends[1:]).max() < scale + 1e-5 * L
+        sag = np.linalg.norm(0.5 * (ends[:-1] + ends[1:]) - np.array(mids), axis=1)
+        assert sag.max() <= tol * 1.001 + 1e-9
+        if m > 1:                                                            # one piece fewer would exceed tol
+            curv = abs(kappa) * np.linalg.norm(P - (P @ bh) * bh)
+            assert (L / (m - 1)) ** 2 * curv / 8.0 > tol * 0.999
+        assert ln.sum() <= L * (1 + 1e-6) and ln.sum() > L * (1 - 1e-3)
+        t_want = trk["t0"][i] + (L * np.arange(m) / m) / (float(trk["beta"][i]) * 0.299792458)
+        assert np.allclose(seg["t0"][off[i]:off[i + 1]], t_want, rtol=2e-7, atol=1e-3)
+        assert np.all(seg["charge"][off[i]:off[i + 1]] == q) and np.all(seg["beta"][off[i]:off[i + 1]] == trk["beta"][i])
+    same = O.substep_tracks(trk, (0.0, 0.0, 0.0), tol)
+    assert same["offsets"][-1] == n
+    for k in ("x", "y", "z", "len", "t0"):
+        assert np.allclose(same["segments"][k], trk[k], rtol=1e-6, atol=1e-6)
+    stiff = dict(trk, p_GeV=np.full(n, 1e6, np.float32))
+    assert O.substep_tracks(stiff, B, tol)["offsets"][-1] == n
+    flip = dict(trk, charge=-trk["charge"])
+    r2 = O.substep_tracks(flip, B, tol)
+    assert np.array_equal(r2["offsets"], off)
+    e0 = np.stack([seg[k] for k in ("x", "y", "z")], 1).astype(np.float64)
+    e1 = np.stack([r2["segments"][k] for k in ("x", "y", "z")], 1).astype(np.float64)
+    first = off[:-1]
+    inner = np.setdiff1d(np.arange(off[-1]), first)
+    assert np.abs(e0[first] - e1[first]).max() < 1e-3 and np.abs(e0[inner] - e1[inner]).max() > 1e-2
