@@ -202,6 +202,28 @@ int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, 
                              int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
                              const c8ph_outputs *host_out);
 
+/* ---- sub-stepping: the step before the hot path (thesis sec. 4.2.1) -------------------
+ * Long particle steps are cut into linear pieces that follow the magnetically deflected path
+ * f_mag:[0,1]->R^3 to the telescopes' resolution.  Uniform field B [T]: the path is
+ * the Lorentz helix with kappa = 0.299792458 q B / p [1/m]; a track of arc length `len` becomes
+ * n = ceil(len / sqrt(8 tol / curvature)) chords (sagitta of each <= tol_m), n <= max_sub.
+ * Two calls, both asynchronous on `stream`, no allocation:
+ *   c8ph_substep_plan  writes offsets[0..n_tracks] (exclusive prefix sum of the piece counts); the
+ *                      caller reads offsets[n_tracks] to size the segment arrays;
+ *   c8ph_substep_fill  writes the pieces of track i to segments[offsets[i] .. offsets[i+1]).
+ * tracks: the c8ph_segments SoA (x,y,z = start, dx,dy,dz = initial direction, len = arc length,
+ * beta, t0, charge; edep ignored) plus p_GeV (momentum [GeV/c]); all DEVICE pointers.
+ * out: DEVICE SoA of capacity >= offsets[n_tracks] per array (edep, if given, is zeroed).        */
+int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
+                      const float B_tesla[3], float tol_m, int32_t max_sub, int64_t *offsets, void *stream);
+typedef struct {                            /* like c8ph_segments, but written */
+    uint32_t size;
+    float *x, *y, *z, *dx, *dy, *dz, *len, *beta, *t0, *charge, *edep;
+} c8ph_segments_out;
+int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
+                      const float B_tesla[3], float tol_m, int32_t max_sub, const int64_t *offsets,
+                      const c8ph_segments_out *out, void *stream);
+
 /* Device time of the last c8ph_emit_propagate kernel of this context in ms (CUDA events on the
  * launch stream; synchronises on the end event).  Returns < 0 if nothing was launched.          */
 float c8ph_last_kernel_ms(c8ph_ctx *ctx);

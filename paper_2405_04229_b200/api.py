@@ -32,7 +32,7 @@ N_COUNTERS = len(COUNTER_NAMES)
 EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8ph_init_atmosphere",
            "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
            "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
-           "c8ph_counter_name")
+           "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill")
 
 PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
                          ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
@@ -82,6 +82,11 @@ class Segments(C.Structure):
                                           ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
 
 
+class SegmentsOut(C.Structure):
+    _fields_ = [("size", C.c_uint32)] + [(k, C.c_void_p) for k in
+                                          ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
+
+
 class Outputs(C.Structure):
     _fields_ = [("size", C.c_uint32), ("hist", C.c_void_p), ("tel_counts", C.c_void_p), ("photons", C.c_void_p),
                 ("photon_weight", C.c_void_p), ("photon_capacity", C.c_int64), ("counters", C.c_void_p)]
@@ -117,6 +122,10 @@ def load_library():
         L.c8ph_last_kernel_ms.restype = C.c_float
         L.c8ph_launch_count.argtypes = [C.c_void_p]
         L.c8ph_launch_count.restype = C.c_int64
+        L.c8ph_substep_plan.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(C.c_float),
+                                        C.c_float, C.c_int32, C.c_void_p, C.c_void_p]
+        L.c8ph_substep_fill.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(C.c_float),
+                                        C.c_float, C.c_int32, C.c_void_p, C.POINTER(SegmentsOut), C.c_void_p]
         L.c8ph_counter_name.argtypes = [C.c_int]
         L.c8ph_counter_name.restype = C.c_char_p
         _lib = L
@@ -334,6 +343,33 @@ class Context:
                     photons=np.zeros(int(photon_capacity), dtype=PHOTON_DTYPE),
                     photon_weight=np.zeros(int(photon_capacity), dtype=np.float32) if want_weight else None,
                     counters_raw=np.zeros(N_COUNTERS, dtype=np.uint64))
+
+    # ---- sub-stepping (the step before the hot path) ---------------------------------------------
+    def substep_tracks(self, trk_dev: dict, n_tracks: int, B_tesla, tol_m: float, max_sub: int = 4096, stream=None):
+        """trk_dev: dict of torch CUDA float32 tensors x,y,z,dx,dy,dz,len,beta,t0,charge,p_GeV.
+        Returns (segments dict of torch CUDA tensors incl. edep = 0, offsets int64[n+1] CUDA tensor).
+        c8ph_substep_plan -> read offsets[n] (one 8-byte D2H) -> allocate -> c8ph_substep_fill."""
+        import torch
+        dev = trk_dev["x"].device
+        t = Segments()
+        t.size = C.sizeof(Segments)
+        for k in SEG_FIELDS:
+            v = trk_dev.get(k)
+            setattr(t, k, _dev_ptr(v, "float32", n_tracks) if (v is not None and k != "edep") else None)
+        p = _dev_ptr(trk_dev["p_GeV"], "float32", n_tracks)
+        Bv = (C.c_float * 3)(*[float(b) for b in B_tesla])
+        offsets = torch.zeros(n_tracks + 1, dtype=torch.int64, device=dev)
+        self._check(self.lib.c8ph_substep_plan(self._h, C.byref(t), p, int(n_tracks), Bv, float(tol_m), int(max_sub),
+                                               offsets.data_ptr(), _stream_ptr(stream)))
+        total = int(offsets[-1].item())
+        seg = {k: torch.empty(max(total, 1), dtype=torch.float32, device=dev) for k in SEG_FIELDS}
+        o = SegmentsOut()
+        o.size = C.sizeof(SegmentsOut)
+        for k in SEG_FIELDS:
+            setattr(o, k, seg[k].data_ptr())
+        self._check(self.lib.c8ph_substep_fill(self._h, C.byref(t), p, int(n_tracks), Bv, float(tol_m), int(max_sub),
+                                               offsets.data_ptr(), C.byref(o), _stream_ptr(stream)))
+        return {k: v[:total] for k, v in seg.items()}, offsets
 
     def last_kernel_ms(self) -> float:
         return float(self.lib.c8ph_last_kernel_ms(self._h))

@@ -132,11 +132,25 @@ struct TableBuildArgs {
     float4 *hot;                    // [n_h][n_zen]
 };
 
+struct SubstepArgs {
+    c8ph_segments trk;              // DEVICE
+    const float *p_GeV;
+    long long n;
+    double B[3], Bn;                // field [T] and its norm
+    double tol;
+    int max_sub;
+    long long *offsets;             // [n+1]
+    c8ph_segments_out out;          // DEVICE (fill only)
+};
+
 // kernels / launchers (c8ph_kernels.cu)
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st);
 cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st);
 size_t emit_smem_bytes(const KArgs &a);
 size_t segment_slot_bytes(int n_sm);
+cudaError_t launch_substep_plan(const SubstepArgs &a, long long *block_sums, cudaStream_t st);
+cudaError_t launch_substep_fill(const SubstepArgs &a, cudaStream_t st);
+size_t substep_scratch_elems(long long n);
 void segment_slot_pointers(void *base, int n_sm, DevRun &run);
 
 }  // namespace c8ph

@@ -12,6 +12,7 @@
 
 using namespace c8ph;
 
+static const size_t kSubstepBlockSums = 1u << 17;   // scan scratch: up to 2^27 tracks per sub-stepping call
 static const int kMaxChunks = 16;           // host path: pipeline depth (chunks of segments per call)
 
 struct c8ph_ctx {
@@ -41,6 +42,7 @@ struct c8ph_ctx {
     // run scratch
     unsigned long long *d_cursor = nullptr;
     void *d_slots = nullptr;           // prepared-segment slots of the resident warps
+    long long *d_bsums = nullptr;      // sub-stepping: block totals of the piece-count scan
     float *d_lines = nullptr;          // [2][max_lines]
     int lines_cap = 0;
     float *d_eff = nullptr;            // detector efficiency table
@@ -101,6 +103,7 @@ extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
         (e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_slots, segment_slot_bytes(ctx->n_sm))) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_bsums, kSubstepBlockSums * sizeof(long long))) != cudaSuccess ||
         (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess) {
         g_create_err = std::string("c8ph_create: ") + cudaGetErrorString(e);
         delete ctx;
@@ -120,6 +123,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     dfree(ctx->d_g_kacc);
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
+    dfree(ctx->d_bsums);
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
     if (ctx->st_h2d) {
         cudaStreamDestroy(ctx->st_h2d); cudaStreamDestroy(ctx->st_run); cudaStreamDestroy(ctx->st_d2h);
@@ -741,6 +745,59 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
     CU(cudaStreamSynchronize(s_run));
     CU(cudaStreamSynchronize(s_out));
     if (ho->counters) memcpy(ho->counters, cnt, C8PH_N_COUNTERS * sizeof(uint64_t));
+    return C8PH_OK;
+}
+
+// ------------------------------------------------------------------------------------ sub-stepping
+static int substep_args(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3], float tol,
+                        int32_t max_sub, SubstepArgs &a)
+{
+    if (!t || t->size != sizeof(c8ph_segments) || !B) return fail(ctx, C8PH_E_ARG, "substep: NULL struct or size mismatch");
+    if (n < 0 || substep_scratch_elems(n) > kSubstepBlockSums) return fail(ctx, C8PH_E_ARG, "substep: n_tracks out of range (<= 2^27 per call)");
+    if (n > 0 && (!t->x || !t->y || !t->z || !t->dx || !t->dy || !t->dz || !t->len || !t->beta || !t->t0 || !t->charge || !p_GeV))
+        return fail(ctx, C8PH_E_ARG, "substep: NULL track array");
+    if (!(tol > 0.f) || max_sub < 1) return fail(ctx, C8PH_E_ARG, "substep: tol_m > 0 and max_sub >= 1 required");
+    a.trk = *t; a.p_GeV = p_GeV; a.n = n;
+    for (int k = 0; k < 3; ++k) a.B[k] = B[k];
+    a.Bn = std::sqrt(a.B[0] * a.B[0] + a.B[1] * a.B[1] + a.B[2] * a.B[2]);
+    a.tol = tol; a.max_sub = max_sub;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3],
+                                 float tol, int32_t max_sub, int64_t *offsets, void *stream)
+{
+    if (!ctx) return C8PH_E_ARG;
+    SubstepArgs a{};
+    int rc = substep_args(ctx, t, p_GeV, n, B, tol, max_sub, a);
+    if (rc) return rc;
+    if (!offsets) return fail(ctx, C8PH_E_ARG, "substep_plan: offsets is NULL");
+    CU(cudaSetDevice(ctx->device));
+    a.offsets = reinterpret_cast<long long *>(offsets);
+    if (n == 0) { CU(cudaMemsetAsync(offsets, 0, sizeof(int64_t), (cudaStream_t)stream)); return C8PH_OK; }
+    cudaError_t e = launch_substep_plan(a, ctx->d_bsums, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "substep_plan launch");
+    ctx->launches += 3;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3],
+                                 float tol, int32_t max_sub, const int64_t *offsets, const c8ph_segments_out *out, void *stream)
+{
+    if (!ctx) return C8PH_E_ARG;
+    SubstepArgs a{};
+    int rc = substep_args(ctx, t, p_GeV, n, B, tol, max_sub, a);
+    if (rc) return rc;
+    if (!offsets || !out || out->size != sizeof(c8ph_segments_out) || !out->x || !out->y || !out->z || !out->dx || !out->dy ||
+        !out->dz || !out->len || !out->beta || !out->t0 || !out->charge)
+        return fail(ctx, C8PH_E_ARG, "substep_fill: NULL offsets / output array or size mismatch");
+    if (n == 0) return C8PH_OK;
+    CU(cudaSetDevice(ctx->device));
+    a.offsets = const_cast<long long *>(reinterpret_cast<const long long *>(offsets));
+    a.out = *out;
+    cudaError_t e = launch_substep_fill(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "substep_fill launch");
+    ctx->launches++;
     return C8PH_OK;
 }
 
