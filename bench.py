@@ -204,6 +204,55 @@ def run_reference(args):
     return 0
 
 
+def _apply_variant(cfg: dict, variant: str) -> None:
+    """Optional features (R13-R15) on top of a BASELINE config."""
+    if variant == "dispersion":
+        cfg["params"].update(disp_b_nm2=5700.0, disp_lambda0_nm=400.0)
+    elif variant == "efficiency":
+        lam = np.arange(200.0, 801.0, 10.0)
+        cfg["params"].update(eff=(0.85 * np.exp(-0.5 * ((lam - 420.0) / 90.0) ** 2)).astype(np.float32),
+                             eff_lambda0_nm=200.0, eff_dlambda_nm=10.0)
+    elif variant == "optics":
+        tel = cfg["detector"]["tel_xyzr"].copy()
+        tel[:, 3] = 12.0
+        cfg["detector"]["tel_xyzr"] = tel
+        cfg["detector"].update(opt_enabled=True, opt_az_deg=0.0, opt_el_deg=70.0, opt_focal_m=17.0,
+                               opt_mirror_radius_m=8.5, opt_camera_radius_m=0.735)
+
+
+def run_substep(args):
+    """Throughput of the sub-stepping entry points (row f2) on synthetic tracks: cfg4's segment recipe
+    with track lengths 5-400 m and momenta 10 MeV - 10 GeV in a 45 uT field, 1 cm sagitta."""
+    import torch
+    from paper_2405_04229_b200 import api, build, workloads as W
+    build.build()
+    n = args.substep
+    cfg = W.make_config(4, n_segments=n)
+    rng = np.random.default_rng(7)
+    trk = {kk: v for kk, v in cfg["segments"].items() if kk != "edep"}
+    trk["len"] = rng.uniform(5.0, 400.0, n).astype(np.float32)
+    trk["p_GeV"] = (10 ** rng.uniform(-2.0, 1.0, n)).astype(np.float32)
+    ctx = api.setup_context(W.make_config(0, n_segments=1))
+    dev = {kk: torch.from_numpy(v).cuda() for kk, v in trk.items()}
+    B, tol = (2.0e-5, -0.5e-5, -4.3e-5), 0.01
+    ms = []
+    for i in range(args.warmup + args.steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        seg, off = ctx.substep_tracks(dev, n, B, tol)
+        e1.record()
+        torch.cuda.synchronize()
+        if i >= args.warmup:
+            ms.append(e0.elapsed_time(e1))
+    pieces = int(off[-1].item())
+    t = float(np.median(ms)) * 1e-3
+    print(json.dumps({"metric": "sub-stepped tracks/sec", "value": n / t, "unit": "tracks/s", "pieces_per_s": pieces / t,
+                      "tracks": n, "pieces": pieces, "ms": 1e3 * t, "steps": args.steps, "warmup": args.warmup,
+                      "note": "plan (3 kernels) + 8-byte D2H of the total + allocation + fill (1 kernel), CUDA events",
+                      "alg_bytes": 44 * n + 8 * (n + 1) + 40 * pieces, "gpu_launches": 4 * args.steps}), flush=True)
+    return 0
+
+
 # ------------------------------------------------------------------------------------------ GPU arm
 def run_ours(args):
     import torch
@@ -223,6 +272,7 @@ def run_ours(args):
     k = args.config
     n = W.FULL_SEGMENTS[k] if args.segments is None else args.segments
     cfg = W.make_config(k, n_segments=n)
+    _apply_variant(cfg, args.variant)
     seg_id_base = rank * n                               # weak scaling: disjoint segment ids per rank
     ctx = api.setup_context(cfg, device=local)
     par, seed = cfg["params"], cfg["seed"]
@@ -341,7 +391,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": _workload_name(k, n), "segments_per_gpu": n, "photons_per_step_per_gpu": photons_rank,
+            "config": {"workload": _workload_name(k, n) + ("" if args.variant == "base" else f" + {args.variant}"), "segments_per_gpu": n, "photons_per_step_per_gpu": photons_rank,
                        "landed": cnt["landed"], "in_grid": cnt["in_grid"], "tel_hit": cnt["tel_hit"], "written": cnt["written"],
                        "l2": "inputs (400 MB of segments, 4.8 GB photon list) larger than L2; outputs re-zeroed each step",
                        "parallelism": f"segments sharded, {world} independent id ranges" if world > 1 else "1 GPU"},
@@ -366,7 +416,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", choices=("base", "dispersion", "efficiency", "optics"), default="base",
+                    help="optional features of SURVEY 8(f) switched on (generic kernel variant); the headline is 'base'")
+    ap.add_argument("--substep", type=int, default=0, help="time c8ph_substep_plan + c8ph_substep_fill on this many tracks and exit")
     args = ap.parse_args()
+    if args.substep:
+        return run_substep(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
