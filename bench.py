@@ -259,11 +259,19 @@ def run_ours(args):
     rank, world, local = _dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    # one rank per GPU; C8PH_BENCH_BACKEND=gloo lets the N>1 plumbing be exercised on a box with fewer GPUs
+    # than ranks (ranks then share devices; a plumbing check, not a measurement)
+    backend = os.environ.get("C8PH_BENCH_BACKEND", "nccl")
+    local = local % torch.cuda.device_count()
+    red_dev = f"cuda:{local}" if backend == "nccl" else "cpu"
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        else:
+            dist.init_process_group(backend)
     from paper_2405_04229_b200 import api, build, shard, workloads as W
     if rank == 0:
         build.build()
@@ -319,9 +327,9 @@ def run_ours(args):
         dist.barrier()
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     kern_ms = [e[1].elapsed_time(e[2]) for e in ev]
-    total_ms = shard.max_over_ranks(total_ms, f"cuda:{local}")
+    total_ms = shard.max_over_ranks(total_ms, red_dev)
     photons_rank = cnt["emitted"] * w
-    photons_job = shard.sum_over_ranks(photons_rank, f"cuda:{local}")
+    photons_job = shard.sum_over_ranks(photons_rank, red_dev)
     value = photons_job * args.steps / (total_ms * 1e-3)
 
     # ---- roofline of the one kernel of the step (ALU issue bound)
@@ -373,7 +381,7 @@ def run_ours(args):
             res = ctx.emit_propagate_host(pin, n, seg_id_base, par, seed, out=hout)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        dt = shard.max_over_ranks(dt, f"cuda:{local}")
+        dt = shard.max_over_ranks(dt, red_dev)
         h2d = sum(int(v.numel()) * 4 for v in pin.values())
         d2h = 4 * (ctx.n_hist() + ctx._n_tel) + 8 * api.N_COUNTERS + 32 * res["counters"]["written"]
         assert res["counters"]["emitted"] == cnt["emitted"] and res["counters"]["overflow"] == 0
@@ -393,7 +401,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": _workload_name(k, n) + ("" if args.variant == "base" else f" + {args.variant}"), "segments_per_gpu": n, "photons_per_step_per_gpu": photons_rank,
                        "landed": cnt["landed"], "in_grid": cnt["in_grid"], "tel_hit": cnt["tel_hit"], "written": cnt["written"],
-                       "l2": "inputs (400 MB of segments, 4.8 GB photon list) larger than L2; outputs re-zeroed each step",
+                       "l2": f"inputs ({40 * n / 1e6:.0f} MB of segments) and photon list ({32 * cnt['written'] / 1e9:.2f} GB) vs 126 MB L2; outputs re-zeroed each step",
                        "parallelism": f"segments sharded, {world} independent id ranges" if world > 1 else "1 GPU"},
             "clocks": clocks, "clock_rejected": bool(bad),
             "e2e": e2e, "gpu_launches": args.steps * 1, "roofline": roofline, "cpu_baseline": base,
