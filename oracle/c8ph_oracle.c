@@ -36,6 +36,8 @@
  *                       with the smallest piece count, lengths / clocks, zero-field and stiff limits.
  *   orc_last_mile (R15) focus and constant path of axis-parallel rays, camera shadow fraction,
  *                       vertex-ray shadow rule, independent numerical intersection of skew rays.
+ *   tabulated extinction (R17) table filled from the Rayleigh law reproduces orc_transmission (nodes,
+ *                       slant scaling, whole runs), tau linear in the table.
  *   efficiency (R14)    lookup values, eps = 1 identity, constant eps scaling, step curve.
  *   dispersion (R13)    b -> 0 limit, closed form of the yield integral incl. threshold
  *                       inside the band, u.P = 1/(beta n(lambda)), KS test of the spectrum.
@@ -60,6 +62,11 @@ typedef struct {
     double earth_radius, h_obs;
     double rayleigh_X, rayleigh_lambda;            /* X_R [g/cm^2] at lambda_R [nm]; 0 = off */
     double aer_L, aer_H, aer_lambda, aer_angstrom; /* aer_L = 0 => no aerosol */
+    /* tabulated extinction (reading R17): vertical optical depth from the observation level up to the
+     * nodes of the height grid, per wavelength node; replaces the Rayleigh / aerosol laws when given */
+    int32_t n_ext_lambda, pad4;
+    double ext_lambda0, ext_dlambda;
+    const float *ext_tau_v;                        /* [n_ext_lambda][n_nodes] or NULL */
 } orc_atmosphere;
 
 typedef struct {
@@ -456,6 +463,34 @@ double orc_transmission(const orc_atmosphere *atm, double x_slant, double tau_ae
     }
     if (atm->aer_L > 0.0) tau += tau_aer * pow(atm->aer_lambda / lambda_nm, atm->aer_angstrom);
     return exp(-tau);
+}
+
+/* Tabulated atmospheric extinction (transmission curves per wavelength and emission height
+ * "with vertical flight direction", Fig. 4.7a, generated with MODTRAN).  Reading R17: the user gives the
+ * vertical optical depth tau_v(lambda_i, h_k) between the observation level and the height nodes of
+ * Listing 4.1's grid on a uniform wavelength grid; bilinear in (lambda, h), both clamped; a slanted,
+ * refracted path scales it with the air-mass factor X_slant / (X_v(h_obs) - X_v(h_e)). */
+double orc_ext_tau_vertical(const orc_atmosphere *atm, double lambda_nm, double h)
+{
+    if (atm->n_ext_lambda <= 0 || !atm->ext_tau_v) return 0.0;
+    double g = atm->n_ext_lambda > 1 ? (lambda_nm - atm->ext_lambda0) / atm->ext_dlambda : 0.0;
+    if (g < 0.0) g = 0.0;
+    if (g > (double)(atm->n_ext_lambda - 1)) g = (double)(atm->n_ext_lambda - 1);
+    int il = (int)floor(g);
+    if (il > atm->n_ext_lambda - 2) il = atm->n_ext_lambda - 2;
+    if (il < 0) il = 0;
+    double gl = g - il;
+    int il1 = il + 1 < atm->n_ext_lambda ? il + 1 : il;
+    double lo = table_lerp(atm->ext_tau_v + (size_t)il * atm->n_nodes, atm->n_nodes, atm->h0, atm->dh, h);
+    double hi = table_lerp(atm->ext_tau_v + (size_t)il1 * atm->n_nodes, atm->n_nodes, atm->h0, atm->dh, h);
+    return (1.0 - gl) * lo + gl * hi;
+}
+
+double orc_transmission_tabulated(const orc_atmosphere *atm, double x_slant, double h_e, double lambda_nm)
+{
+    double dxv = orc_overburden(atm, atm->h_obs) - orc_overburden(atm, h_e);
+    if (!(dxv > 0.0)) return 1.0;
+    return exp(-orc_ext_tau_vertical(atm, lambda_nm, h_e) * (x_slant / dxv));
 }
 
 /* detector efficiency eps(lambda) ("reduce the number of photons by one to two orders of
@@ -875,7 +910,9 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 }
                 /* O11 transmission */
                 if (par->trans != ORC_TRANS_OFF) {
-                    ph.T = orc_transmission(atm, x_slant, tau_aer, ph.lambda_nm) * orc_efficiency(par, ph.lambda_nm);
+                    ph.T = (atm->n_ext_lambda > 0 ? orc_transmission_tabulated(atm, x_slant, h_e, ph.lambda_nm)
+                                                  : orc_transmission(atm, x_slant, tau_aer, ph.lambda_nm))
+                           * orc_efficiency(par, ph.lambda_nm);
                     if (par->trans == ORC_TRANS_ROULETTE) {
                         if (!(u4[3] < ph.T)) { ph.status = ORC_ST_ROULETTE; lc[ORC_CNT_ROULETTE]++; goto store; }
                     } else ph.weight = par->bunch_weight * ph.T;

@@ -40,7 +40,9 @@ class Atmosphere(C.Structure):
                 ("earth_radius", C.c_double), ("h_obs", C.c_double),
                 ("rayleigh_X", C.c_double), ("rayleigh_lambda", C.c_double),
                 ("aer_L", C.c_double), ("aer_H", C.c_double), ("aer_lambda", C.c_double),
-                ("aer_angstrom", C.c_double)]
+                ("aer_angstrom", C.c_double),
+                ("n_ext_lambda", C.c_int32), ("pad4", C.c_int32), ("ext_lambda0", C.c_double), ("ext_dlambda", C.c_double),
+                ("ext_tau_v", C.POINTER(C.c_float))]
 
 
 class Table(C.Structure):
@@ -122,6 +124,10 @@ def lib():
                                            [C.POINTER(C.c_double), C.c_double, C.c_int32, C.POINTER(C.c_float)]
             L.orc_last_mile.restype = C.c_int
             L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 4
+            L.orc_ext_tau_vertical.restype = C.c_double
+            L.orc_ext_tau_vertical.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double]
+            L.orc_transmission_tabulated.restype = C.c_double
+            L.orc_transmission_tabulated.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double, C.c_double]
             L.orc_efficiency.restype = C.c_double
             L.orc_efficiency.argtypes = [C.POINTER(Params), C.c_double]
             L.orc_straight_line.restype = C.c_double
@@ -169,6 +175,11 @@ def atmosphere_struct(atm: dict, keep: _Keep) -> Atmosphere:
     s.earth_radius, s.h_obs = float(atm["earth_radius"]), float(atm["h_obs"])
     for k in ("rayleigh_X", "rayleigh_lambda", "aer_L", "aer_H", "aer_lambda", "aer_angstrom"):
         setattr(s, k, float(np.float32(atm[k])))
+    ext = atm.get("ext_tau_v")
+    s.n_ext_lambda = 0 if ext is None else int(np.asarray(ext).shape[0])
+    s.ext_tau_v = keep.f32(np.asarray(ext).reshape(-1)) if s.n_ext_lambda else None
+    s.ext_lambda0 = float(np.float32(atm.get("ext_lambda0_nm", 0.0)))
+    s.ext_dlambda = float(np.float32(atm.get("ext_dlambda_nm", 1.0)))
     return s
 
 

@@ -832,3 +832,46 @@ def test_substepping_follows_the_lorentz_helix():
     first = off[:-1]
     inner = np.setdiff1d(np.arange(off[-1]), first)
     assert np.abs(e0[first] - e1[first]).max() < 1e-3 and np.abs(e0[inner] - e1[inner]).max() > 1e-2
+
+
+# ---------------------------------------------------------------------------------- tabulated extinction (R17, row f4)
+def _rayleigh_ext_table(atm, lam):
+    """tau_v(lambda, h) of the Rayleigh law of R11 on the atmosphere's height grid (vertical, obs level -> h)."""
+    xv = atm["overburden"].astype(np.float64)
+    h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
+    xg = np.interp(atm["h_obs"], h, xv)
+    return ((400.0 / lam[:, None]) ** 4 * np.maximum(xg - xv[None, :], 0.0) / 2970.0).astype(np.float32)
+
+
+def test_tabulated_extinction_reproduces_the_rayleigh_law():
+    """A tau_v(lambda, h) table filled from the analytic Rayleigh law must reproduce R11's transmission:
+    node values exactly, between wavelength nodes to the interpolation error of lambda^-4 on a 2 nm grid;
+    the slant scaling by the air-mass factor X_slant / (X_v(h_obs) - X_v(h_e)) is exact for it; whole runs
+    agree photon by photon (same roulette decisions up to ~1e-4 of the photons); tau scales linearly."""
+    cfg = W.make_config(2, n_segments=3000)
+    atm = cfg["atmosphere"]
+    lam = np.arange(240.0, 711.0, 2.0)
+    tab = copy.deepcopy(cfg)
+    tab["atmosphere"].update(ext_tau_v=_rayleigh_ext_table(atm, lam), ext_lambda0_nm=240.0, ext_dlambda_nm=2.0)
+    keep = O._Keep()
+    a_tab, a_ana = O.atmosphere_struct(tab["atmosphere"], keep), O.atmosphere_struct(atm, keep)
+    L = O.lib()
+    for lam_q, h in ((300.0, 8000.0), (452.0, 12340.0), (601.0, 30.0), (333.3, 5555.5)):
+        xs = 1.7 * (L.orc_overburden(C.byref(a_ana), 0.0) - L.orc_overburden(C.byref(a_ana), h))   # some slant path
+        t_tab = L.orc_transmission_tabulated(C.byref(a_tab), xs, h, lam_q)
+        t_ana = L.orc_transmission(C.byref(a_ana), xs, 0.0, lam_q)
+        tol = 2e-6 if lam_q % 2 == 0 else 3e-4                           # on / between wavelength nodes
+        assert abs(t_tab - t_ana) < tol * max(1.0, -math.log(t_ana)), (lam_q, h, t_tab, t_ana)
+    assert L.orc_transmission_tabulated(C.byref(a_tab), 10.0, 0.0, 400.0) == 1.0   # emission at the observation level
+    r_ana, r_tab = O.run(cfg, record=True), O.run(tab, record=True)
+    assert r_ana["counters"]["emitted"] == r_tab["counters"]["emitted"]
+    flips = int((r_ana["photons"]["status"] != r_tab["photons"]["status"]).sum())
+    assert flips <= 3e-4 * r_ana["counters"]["emitted"] + 3
+    same = r_ana["photons"]["status"] == r_tab["photons"]["status"]
+    assert np.abs(r_ana["photons"]["T"][same] - r_tab["photons"]["T"][same]).max() < 3e-4
+    dbl = copy.deepcopy(tab)
+    dbl["atmosphere"]["ext_tau_v"] = 2.0 * tab["atmosphere"]["ext_tau_v"]
+    r_dbl = O.run(dbl, record=True)
+    m = (r_tab["photons"]["T"] > 0) & (r_tab["photons"]["status"] >= O.ST_ROULETTE - 4) & (r_tab["photons"]["T"] < 1)
+    both = m & (r_dbl["photons"]["T"] > 0) & (r_dbl["photons"]["T"] < 1)
+    assert both.sum() > 1000 and np.allclose(r_dbl["photons"]["T"][both], r_tab["photons"]["T"][both] ** 2, rtol=1e-9)
