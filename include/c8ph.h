@@ -65,6 +65,14 @@ typedef struct {
     float earth_radius_m, h_obs_m;   /* R and the altitude of the observation level                */
     float rayleigh_X_gcm2, rayleigh_lambda_nm; /* tau_R = X_slant (lambda_R/lambda)^4 / X_R; X_R = 0: off */
     float aer_L_m, aer_H_m, aer_lambda_nm, aer_angstrom; /* aerosol: alpha = exp(-h/H)/L (lambda_a/lambda)^a; L = 0: off */
+    /* Tabulated extinction (thesis P:772-796, Fig. 4.7a: MODTRAN-type curves per wavelength and height for
+     * vertical flight): vertical optical depth between the observation level and node k of the height grid
+     * for wavelength node i on the uniform grid ext_lambda0_nm + i ext_dlambda_nm; bilinear, clamped; a
+     * slanted path scales it with X_slant / (X_v(h_obs) - X_v(h_e)) (needs overburden_gcm2).  When given
+     * (n_ext_lambda > 0) it replaces the Rayleigh / aerosol laws above.                                   */
+    int32_t n_ext_lambda;
+    float ext_lambda0_nm, ext_dlambda_nm;
+    const float *ext_tau_v;          /* HOST [n_ext_lambda][n_nodes]; copied                      */
 } c8ph_atmosphere_desc;
 /* Copies the tables to the device (synchronous).  Invalidates a previously built trace table. */
 int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *desc);

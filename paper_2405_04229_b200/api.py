@@ -48,7 +48,8 @@ class AtmosphereDesc(C.Structure):
                 ("earth_radius_m", C.c_float), ("h_obs_m", C.c_float),
                 ("rayleigh_X_gcm2", C.c_float), ("rayleigh_lambda_nm", C.c_float),
                 ("aer_L_m", C.c_float), ("aer_H_m", C.c_float), ("aer_lambda_nm", C.c_float),
-                ("aer_angstrom", C.c_float)]
+                ("aer_angstrom", C.c_float),
+                ("n_ext_lambda", C.c_int32), ("ext_lambda0_nm", C.c_float), ("ext_dlambda_nm", C.c_float), ("ext_tau_v", _fp)]
 
 
 class TableDesc(C.Structure):
@@ -187,6 +188,12 @@ class Context:
         d.rayleigh_X_gcm2, d.rayleigh_lambda_nm = float(atm["rayleigh_X"]), float(atm["rayleigh_lambda"])
         d.aer_L_m, d.aer_H_m = float(atm["aer_L"]), float(atm["aer_H"])
         d.aer_lambda_nm, d.aer_angstrom = float(atm["aer_lambda"]), float(atm["aer_angstrom"])
+        ext = atm.get("ext_tau_v")
+        if ext is not None:
+            ext = _f32(np.asarray(ext))
+            d.n_ext_lambda = ext.shape[0]
+            d.ext_tau_v = ext.ctypes.data_as(_fp)
+            d.ext_lambda0_nm, d.ext_dlambda_nm = float(atm["ext_lambda0_nm"]), float(atm["ext_dlambda_nm"])
         self._check(self.lib.c8ph_init_atmosphere(self._h, C.byref(d)))
 
     @staticmethod

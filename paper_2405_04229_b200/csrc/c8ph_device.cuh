@@ -23,6 +23,10 @@ struct DevAtm {
     float ray_inv_X;        // 1 / X_R, 0 = Rayleigh off
     float ray_lambda;       // lambda_R [nm]
     float aer_L, aer_H, aer_lambda, aer_angstrom;
+    int n_ext;              // tabulated extinction: wavelength nodes (0: off)
+    float ext_l0, ext_inv_dl;
+    const float *ext;       // DEVICE [n_ext][n_nodes] vertical optical depth obs level -> node
+    float xv_g;             // X_v at the observation level
 };
 
 struct DevTable {

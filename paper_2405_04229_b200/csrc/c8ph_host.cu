@@ -24,7 +24,7 @@ struct c8ph_ctx {
     DevAtm atm{};
     bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
     double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
-    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr;
+    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr;
     // table
     bool have_table = false;
     DevTable tab{};
@@ -117,7 +117,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
 {
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
-    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_g_kacc);
@@ -193,6 +193,19 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
     a.ray_lambda = d->rayleigh_lambda_nm;
     a.aer_L = d->aer_L_m; a.aer_H = d->aer_H_m; a.aer_lambda = d->aer_lambda_nm; a.aer_angstrom = d->aer_angstrom;
     if (a.aer_L > 0.f && !(a.aer_H > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: aerosol scale height");
+    a.xv_g = (float)lerp_table(xv, h0, dh, d->h_obs_m);
+    a.n_ext = 0; a.ext = nullptr; a.ext_l0 = 0.f; a.ext_inv_dl = 0.f;
+    dfree(ctx->d_ext);
+    if (d->n_ext_lambda > 0) {
+        if (d->model == C8PH_ATM_HOMOGENEOUS || !d->ext_tau_v || !d->overburden_gcm2 || (d->n_ext_lambda > 1 && !(d->ext_dlambda_nm > 0.f)) || d->n_ext_lambda > 4096)
+            return fail(ctx, C8PH_E_ARG, "init_atmosphere: extinction table needs a height grid, overburden, ext_tau_v and ext_dlambda_nm > 0");
+        const size_t ne = (size_t)d->n_ext_lambda * n;
+        for (size_t k = 0; k < ne; ++k) if (!(d->ext_tau_v[k] >= 0.f) || !std::isfinite(d->ext_tau_v[k])) return fail(ctx, C8PH_E_ARG, "init_atmosphere: extinction table entry < 0 or not finite");
+        CU(cudaMalloc(&ctx->d_ext, ne * sizeof(float)));
+        CU(cudaMemcpy(ctx->d_ext, d->ext_tau_v, ne * sizeof(float), cudaMemcpyHostToDevice));
+        a.n_ext = d->n_ext_lambda; a.ext = ctx->d_ext; a.ext_l0 = d->ext_lambda0_nm;
+        a.ext_inv_dl = d->n_ext_lambda > 1 ? 1.0f / d->ext_dlambda_nm : 0.f;
+    }
     ctx->have_atm = true;
     ctx->have_table = false;
     return C8PH_OK;

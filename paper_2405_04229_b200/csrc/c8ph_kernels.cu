@@ -476,6 +476,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_disp = SPEC ? false : run.disp_b != 0.f;
     const bool f_eff = SPEC ? false : run.n_eff > 0;
     const bool f_opt = SPEC ? false : det.opt_enabled != 0;
+    const bool f_ext = SPEC ? false : atm.n_ext > 0;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -999,12 +1000,28 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (f_trans != C8PH_TRANS_OFF) {
                         // a12: transmission, Rayleigh ~ lambda^-4 scaled by slant depth (+ aerosol)
                         float tau = 0.f;
+                        if (f_ext) {
+                            // tabulated extinction (Fig. 4.7a): vertical optical depth tau_v(lambda, h_e),
+                            // bilinear, times the air-mass factor X_slant / (X_v(h_obs) - X_v(h_e)); in units of ln 2
+                            const float fh = fminf(fmaxf((h_e - atm.h0) * atm.inv_dh, 0.f), atm.f_max);
+                            const int kh = min((int)fh, atm.n_nodes - 2);
+                            const float wh = fh - (float)kh;
+                            const float gl = fminf(fmaxf((rcp_fast(lam_inv) - atm.ext_l0) * atm.ext_inv_dl, 0.f), (float)(atm.n_ext - 1));
+                            const int kl = min((int)gl, max(atm.n_ext - 2, 0));
+                            const float wl = gl - (float)kl;
+                            const float *r0 = atm.ext + (size_t)kl * atm.n_nodes + kh;
+                            const float *r1 = atm.ext + (size_t)min(kl + 1, atm.n_ext - 1) * atm.n_nodes + kh;
+                            const float t0 = fmaf(wh, __ldg(r0 + 1) - __ldg(r0), __ldg(r0)), t1 = fmaf(wh, __ldg(r1 + 1) - __ldg(r1), __ldg(r1));
+                            const float xe = fmaf(wh, __ldg(atm.xv + kh + 1) - __ldg(atm.xv + kh), __ldg(atm.xv + kh));
+                            const float dxv = atm.xv_g - xe;
+                            tau = dxv > 0.f ? 1.4426950408889634f * fmaf(wl, t1 - t0, t0) * Xs * rcp_fast(dxv) : 0.f;
+                        } else
                         if (f_ray) {
                             float qq = hc.ray_lambda * lam_inv;
                             qq *= qq; qq *= qq;
                             tau = Xs * qq * hc.ray_k;                        // optical depth in units of ln 2
                         }
-                        if (f_aer) tau = fmaf(1.4426950408889634f * ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
+                        if (f_aer && !f_ext) tau = fmaf(1.4426950408889634f * ta, __powf(atm.aer_lambda * lam_inv, atm.aer_angstrom), tau);
                         float T = exp2_fast(-tau);
                         if (f_eff) {
                             // detector efficiency eps(lambda): linear on a uniform grid, ends held
@@ -1239,7 +1256,7 @@ static bool array_production_setting(const KArgs &a)
     const DevRun &r = a.run;
     const DevDet &d = a.det;
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
-           a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
+           a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && a.atm.n_ext == 0 && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
            r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled;
 }

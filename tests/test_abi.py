@@ -44,7 +44,7 @@ def test_version_and_counter_names(lib):
 def test_struct_layouts_match_the_header(tmp_path):
     """sizeof/offsetof from a C compile of the header against the ctypes mirrors."""
     fields = {
-        "c8ph_atmosphere_desc": (api.AtmosphereDesc, ["size", "refractivity", "earth_radius_m", "aer_angstrom"]),
+        "c8ph_atmosphere_desc": (api.AtmosphereDesc, ["size", "refractivity", "earth_radius_m", "aer_angstrom", "n_ext_lambda", "ext_tau_v"]),
         "c8ph_table_desc": (api.TableDesc, ["size", "h_max_m", "substeps"]),
         "c8ph_detector": (api.Detector, ["size", "tel_xyzr", "cam_enabled", "t_ref_ns", "t_bin_ns", "opt_enabled", "opt_camera_radius_m"]),
         "c8ph_params": (api.Params, ["size", "write", "bunch_weight", "n_lines", "line_cdf", "disp_lambda0_nm", "n_eff", "eff"]),

@@ -520,3 +520,30 @@ def test_substepping_matches_the_oracle_and_feeds_the_hot_path():
         parity.compare(sub, ora, gpu)
     else:                                                                 # last-bit differences in the pieces: totals only
         assert abs(gpu["counters"]["emitted"] - ora["counters"]["emitted"]) <= 1e-3 * ora["counters"]["emitted"]
+
+
+def test_tabulated_extinction():
+    """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
+    scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an
+    aerosol-like layer on a 10 nm grid), roulette (cfg2, cfg4) and weight mode (cfg1)."""
+    lam = np.arange(240.0, 711.0, 10.0)
+    for k, n in ((2, 20000), (4, 2500), (1, 600)):
+        cfg = W.make_config(k, n_segments=n)
+        atm = cfg["atmosphere"]
+        xv = atm["overburden"].astype(np.float64)
+        h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
+        xg = np.interp(atm["h_obs"], h, xv)
+        ray = (400.0 / lam[:, None]) ** 4 * np.maximum(xg - xv[None, :], 0.0) / 2970.0
+        aer = (350.0 / lam[:, None]) * (1200.0 / 15000.0) * np.maximum(np.exp(-atm["h_obs"] / 1200.0) - np.exp(-h[None, :] / 1200.0), 0.0)
+        atm.update(ext_tau_v=(ray + aer).astype(np.float32), ext_lambda0_nm=240.0, ext_dlambda_nm=10.0)
+        ora, gpu, rep = _both(cfg)
+        off = api.run_config(W.make_config(k, n_segments=n))
+        if k == 1:
+            assert gpu["hist"].sum() < off["hist"].sum()
+        else:
+            assert gpu["counters"]["roulette"] > off["counters"]["roulette"]        # the aerosol layer removes more
+    cfg = W.make_config(0, n_segments=10)                                           # homogeneous model: refused
+    cfg["atmosphere"].update(ext_tau_v=np.zeros((2, cfg["atmosphere"]["n_nodes"]), np.float32), ext_lambda0_nm=300.0, ext_dlambda_nm=300.0)
+    with pytest.raises(api.C8phError) as e:
+        api.setup_context(cfg)
+    assert e.value.code == api.E_ARG
