@@ -92,3 +92,14 @@ def test_product_does_not_import_the_oracle():
                 assert "import oracle" not in txt and "from oracle" not in txt and "c8ph_oracle" not in txt, f
     otxt = open(os.path.join(ROOT, "oracle", "c8ph_oracle.c")).read()
     assert "#include \"" not in otxt                       # the oracle includes no project header
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    """No silent fallback: without libc8ph.so the binding raises and names the build step."""
+    monkeypatch.setattr(api, "_lib", None)
+    monkeypatch.setattr(api, "LIB_PATH", str(tmp_path / "libc8ph.so"))
+    with pytest.raises(RuntimeError) as e:
+        api.load_library()
+    assert "no CPU fallback" in str(e.value) and "build" in str(e.value)
+    with pytest.raises(RuntimeError):
+        api.Context(0)
