@@ -323,7 +323,7 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     }
     const double ext = std::max(x1 - x0, y1 - y0);
     // cell size: about one telescope radius, but no more than ~4e6 list entries and 1536^2 cells
-    double cs = mode == 0 ? rz_min : r_max;
+    double cs = mode == 0 ? 0.5 * rz_min : r_max;       // hit grid: half a radius (fewer false candidates; measured)
     {
         double area = 0.0;
         for (int k = 0; k < n; ++k) area += 3.14159265358979 * reach(k) * reach(k);
