@@ -34,6 +34,8 @@
  *                       pixel-centre round trip.
  *   orc_substep_track (R16) chord end points vs an independent RK4 Lorentz integration, sagitta <= tol
  *                       with the smallest piece count, lengths / clocks, zero-field and stiff limits.
+ *   orc_substep_track_ms (R18) Highland width values, Var(theta), Var(y), Cov(y, theta) of one piece,
+ *                       accumulation over pieces, zero-density identity with R16, id-keyed draws.
  *   orc_last_mile (R15) focus and constant path of axis-parallel rays, camera shadow fraction,
  *                       vertex-ray shadow rule, independent numerical intersection of skew rays.
  *   tabulated extinction (R17) table filled from the Rayleigh law reproduces orc_transmission (nodes,
@@ -1060,6 +1062,102 @@ int32_t orc_substep_track(const double A[3], const double Pin[3], double L, doub
             o[6] = (float)len; o[7] = (float)beta; o[8] = (float)(t0 + s0 / (beta * ORC_C_M_PER_NS)); o[9] = (float)charge;
         }
         for (int k = 0; k < 3; ++k) Xp[k] = Xn[k];
+    }
+    return n;
+}
+
+/* ------------------------------------------------------------------ multiple-scattering sub-steps (R18)
+ * Thesis P:738-746: "instead of calculating the multiple scattering path deviation to the next
+ * interaction in a single step, several substeps could be sampled according to the required precision
+ * and stored ... the first approach is used ... due to the additional displacement included, which
+ * emulates a random walk between each substep"; the angular law comes from an approximation "which
+ * employs the initial energy and the particles traversed grammage", Highland or Moliere.  The thesis
+ * calls PROPOSAL for it; reading: Highland's width in the PDG (Lynch-Dahl) form
+ *   theta0 = 13.6 MeV / (beta c p) |z| sqrt(t) (1 + 0.038 ln(t z^2 / beta^2)),  t = x / X0,
+ * per sub-step of arc length ds and grammage x = rho(h_mid) ds, and per transverse plane the correlated
+ * Gaussian pair  theta = z2 theta0,  y = (z1/sqrt(12) + z2/2) ds theta0  (z1, z2 ~ N(0,1), Box-Muller on
+ * the uniforms of Philox counter (piece, track id, stream 16)).  The magnetic step of R16 is applied
+ * first (exact rotation about B), then the offset and the deflection. */
+double orc_highland_theta0(double beta, double p_GeV, double charge, double t)
+{
+    if (!(t > 0.0) || !(p_GeV > 0.0)) return 0.0;
+    double corr = 1.0 + 0.038 * log(t * charge * charge / (beta * beta));
+    if (corr < 0.0) corr = 0.0;
+    return 0.0136 / (beta * p_GeV) * fabs(charge) * sqrt(t) * corr;
+}
+
+/* density [g/cm^2 per m] of the cell of the overburden table that holds height h (X_v is linear per cell) */
+static double cell_density(const orc_atmosphere *atm, double h)
+{
+    if (!atm->overburden || atm->model == 0) return 0.0;
+    double f = (h - atm->h0) / atm->dh;
+    if (f < 0.0) f = 0.0;
+    if (f > (double)(atm->n_nodes - 1)) f = (double)(atm->n_nodes - 1);
+    int k = (int)floor(f);
+    if (k > atm->n_nodes - 2) k = atm->n_nodes - 2;
+    return ((double)atm->overburden[k] - (double)atm->overburden[k + 1]) / atm->dh;
+}
+
+int32_t orc_substep_track_ms(const orc_atmosphere *atm, const double A[3], const double Pin[3], double L, double beta,
+                             double t0, double charge, double p_GeV, const double B[3], double tol_m,
+                             double ms_max_step_m, double ms_X0, uint64_t seed, uint64_t track_id,
+                             int32_t max_sub, float *seg_out)
+{
+    int32_t n = orc_substep_track(A, Pin, L, beta, t0, charge, p_GeV, B, tol_m, max_sub, NULL);
+    if (ms_max_step_m > 0.0 && L > 0.0) {
+        double nn = ceil(L / ms_max_step_m);
+        int32_t n2 = nn > (double)max_sub ? max_sub : (int32_t)nn;
+        if (n2 > n) n = n2;
+    }
+    if (!seg_out) return n;
+    double P[3] = { Pin[0], Pin[1], Pin[2] }, X[3] = { A[0], A[1], A[2] };
+    norm3(P);
+    double Bn = sqrt(B[0]*B[0] + B[1]*B[1] + B[2]*B[2]);
+    double kappa = (Bn > 0.0 && p_GeV > 0.0) ? 0.299792458 * charge * Bn / p_GeV : 0.0;
+    double bh[3] = { 0, 0, 1 };
+    if (Bn > 0.0) { bh[0] = B[0]/Bn; bh[1] = B[1]/Bn; bh[2] = B[2]/Bn; }
+    const double ds = L / (double)n;
+    for (int i = 0; i < n; ++i) {
+        /* magnetic step: P' = P_par + cos(k ds) P_perp + sin(k ds) (P_perp x b), displacement = its integral */
+        double ppar = P[0]*bh[0] + P[1]*bh[1] + P[2]*bh[2];
+        double Pp[3] = { P[0] - ppar*bh[0], P[1] - ppar*bh[1], P[2] - ppar*bh[2] };
+        double Pc[3] = { Pp[1]*bh[2] - Pp[2]*bh[1], Pp[2]*bh[0] - Pp[0]*bh[2], Pp[0]*bh[1] - Pp[1]*bh[0] };
+        double dX[3], Pn[3];
+        double sn = sin(kappa * ds), cs = cos(kappa * ds);
+        for (int k = 0; k < 3; ++k) {
+            if (kappa != 0.0) {
+                dX[k] = ppar * bh[k] * ds + (sn * Pp[k] + (1.0 - cs) * Pc[k]) / kappa;
+                Pn[k] = ppar * bh[k] + cs * Pp[k] + sn * Pc[k];
+            } else { dX[k] = P[k] * ds; Pn[k] = P[k]; }
+        }
+        /* multiple scattering of the piece */
+        double mid[3] = { X[0] + 0.5*dX[0], X[1] + 0.5*dX[1], X[2] + 0.5*dX[2] };
+        double rho = cell_density(atm, orc_height(atm, mid));
+        double th0 = orc_highland_theta0(beta, p_GeV, charge, rho * ds / ms_X0);
+        double u[4];
+        orc_draw(seed, track_id, (uint32_t)i, 16u, u);
+        double r1 = sqrt(-2.0 * log(u[0])), r2 = sqrt(-2.0 * log(u[2]));
+        double z1 = r1 * cos(2.0 * ORC_PI * u[1]), z2 = r1 * sin(2.0 * ORC_PI * u[1]);
+        double z3 = r2 * cos(2.0 * ORC_PI * u[3]), z4 = r2 * sin(2.0 * ORC_PI * u[3]);
+        double ea[3] = { Pn[1], -Pn[0], 0.0 };                        /* P' x z */
+        double na = sqrt(ea[0]*ea[0] + ea[1]*ea[1]);
+        if (na < 1e-12) { ea[0] = 1.0; ea[1] = 0.0; na = 1.0; }
+        ea[0] /= na; ea[1] /= na;
+        double eb[3] = { Pn[1]*ea[2] - Pn[2]*ea[1], Pn[2]*ea[0] - Pn[0]*ea[2], Pn[0]*ea[1] - Pn[1]*ea[0] };
+        double ya = (z1 / sqrt(12.0) + 0.5 * z2) * ds * th0, yb = (z3 / sqrt(12.0) + 0.5 * z4) * ds * th0;
+        double Xe[3], Pe[3];
+        for (int k = 0; k < 3; ++k) {
+            Xe[k] = X[k] + dX[k] + ya * ea[k] + yb * eb[k];
+            Pe[k] = Pn[k] + z2 * th0 * ea[k] + z4 * th0 * eb[k];
+        }
+        norm3(Pe);
+        double d[3] = { Xe[0]-X[0], Xe[1]-X[1], Xe[2]-X[2] };
+        double len = sqrt(d[0]*d[0] + d[1]*d[1] + d[2]*d[2]);
+        float *o = seg_out + 10 * (size_t)i;
+        o[0] = (float)X[0]; o[1] = (float)X[1]; o[2] = (float)X[2];
+        o[3] = (float)(d[0]/len); o[4] = (float)(d[1]/len); o[5] = (float)(d[2]/len);
+        o[6] = (float)len; o[7] = (float)beta; o[8] = (float)(t0 + (double)i * ds / (beta * ORC_C_M_PER_NS)); o[9] = (float)charge;
+        for (int k = 0; k < 3; ++k) { X[k] = Xe[k]; P[k] = Pe[k]; }
     }
     return n;
 }

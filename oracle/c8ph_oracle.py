@@ -122,6 +122,12 @@ def lib():
             L.orc_substep_track.restype = C.c_int32
             L.orc_substep_track.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)] + [C.c_double] * 5 + \
                                            [C.POINTER(C.c_double), C.c_double, C.c_int32, C.POINTER(C.c_float)]
+            L.orc_highland_theta0.restype = C.c_double
+            L.orc_highland_theta0.argtypes = [C.c_double] * 4
+            L.orc_substep_track_ms.restype = C.c_int32
+            L.orc_substep_track_ms.argtypes = [C.POINTER(Atmosphere), C.POINTER(C.c_double), C.POINTER(C.c_double)] + [C.c_double] * 5 + \
+                                              [C.POINTER(C.c_double), C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64,
+                                               C.c_int32, C.POINTER(C.c_float)]
             L.orc_last_mile.restype = C.c_int
             L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 4
             L.orc_ext_tau_vertical.restype = C.c_double
@@ -418,6 +424,38 @@ def substep_tracks(tracks: dict, B, tol_m: float, max_sub: int = 4096) -> dict:
     for i, a in enumerate(args):
         L.orc_substep_track(a[0], a[1], a[2], a[3], a[4], a[5], a[6], Bd, float(np.float32(tol_m)), int(max_sub),
                             out[offsets[i]:].ctypes.data_as(C.POINTER(C.c_float)))
+    names = ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge")
+    seg = {k: np.ascontiguousarray(out[:, j]) for j, k in enumerate(names)}
+    seg["edep"] = np.zeros(len(out), dtype=np.float32)
+    return dict(segments=seg, offsets=offsets)
+
+
+def substep_tracks_ms(atm: dict, tracks: dict, B, tol_m: float, ms_max_step_m: float, ms_X0: float = 36.62,
+                      seed: int = 1, track_id_base: int = 0, max_sub: int = 4096) -> dict:
+    """R18: R16's magnetic pieces plus Highland multiple scattering per piece (sequential random walk)."""
+    L = lib()
+    keep = _Keep()
+    a_s = atmosphere_struct(atm, keep)
+    n = len(tracks["x"])
+    Bd = (C.c_double * 3)(*[float(np.float32(b)) for b in B])
+    arr = lambda v: (C.c_double * 3)(*[float(x) for x in v])
+    counts = np.zeros(n, dtype=np.int64)
+    calls = []
+    for i in range(n):
+        a = (arr([tracks[k][i] for k in ("x", "y", "z")]), arr([tracks[k][i] for k in ("dx", "dy", "dz")]),
+             float(tracks["len"][i]), float(tracks["beta"][i]), float(tracks["t0"][i]), float(tracks["charge"][i]),
+             float(tracks["p_GeV"][i]))
+        calls.append(a)
+        counts[i] = L.orc_substep_track_ms(C.byref(a_s), a[0], a[1], a[2], a[3], a[4], a[5], a[6], Bd, float(np.float32(tol_m)),
+                                           float(np.float32(ms_max_step_m)), float(np.float32(ms_X0)), C.c_uint64(seed),
+                                           C.c_uint64(track_id_base + i), int(max_sub), None)
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    out = np.zeros((int(offsets[-1]), 10), dtype=np.float32)
+    for i, a in enumerate(calls):
+        L.orc_substep_track_ms(C.byref(a_s), a[0], a[1], a[2], a[3], a[4], a[5], a[6], Bd, float(np.float32(tol_m)),
+                               float(np.float32(ms_max_step_m)), float(np.float32(ms_X0)), C.c_uint64(seed),
+                               C.c_uint64(track_id_base + i), int(max_sub),
+                               out[offsets[i]:].ctypes.data_as(C.POINTER(C.c_float)))
     names = ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge")
     seg = {k: np.ascontiguousarray(out[:, j]) for j, k in enumerate(names)}
     seg["edep"] = np.zeros(len(out), dtype=np.float32)

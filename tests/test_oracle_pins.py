@@ -875,3 +875,63 @@ def test_tabulated_extinction_reproduces_the_rayleigh_law():
     m = (r_tab["photons"]["T"] > 0) & (r_tab["photons"]["status"] >= O.ST_ROULETTE - 4) & (r_tab["photons"]["T"] < 1)
     both = m & (r_dbl["photons"]["T"] > 0) & (r_dbl["photons"]["T"] < 1)
     assert both.sum() > 1000 and np.allclose(r_dbl["photons"]["T"][both], r_tab["photons"]["T"][both] ** 2, rtol=1e-9)
+
+
+# ---------------------------------------------------------------------------------- multiple scattering (R18, row f2)
+def test_multiple_scattering_substeps():
+    """Highland / PDG width, and the correlated (offset, angle) pair per plane: for one piece in a
+    constant-density slab and no field, Var(theta_plane) = theta0^2, Var(y_plane) = ds^2 theta0^2 / 3,
+    corr(y, theta) = sqrt(3)/2; after n pieces the angular variance adds up; zero density or a stiff
+    particle reproduce R16's pieces; the draw depends on (seed, track id, piece) only."""
+    L = O.lib()
+    assert abs(L.orc_highland_theta0(1.0, 1.0, 1.0, 0.1) - 0.0136 * math.sqrt(0.1) * (1 + 0.038 * math.log(0.1))) < 1e-15
+    assert abs(L.orc_highland_theta0(0.5, 2.0, 2.0, 0.01) - 0.0136 / (0.5 * 2.0) * 2.0 * 0.1 * (1 + 0.038 * math.log(0.01 * 4 / 0.25))) < 1e-15
+    assert L.orc_highland_theta0(1.0, 1.0, 1.0, 0.0) == 0.0
+    atm = W.make_atmosphere("planar_exp")
+    n_nodes = atm["n_nodes"]
+    rho = 0.1                                                             # g/cm^2 per m, constant
+    atm["overburden"] = (rho * atm["dh"] * (n_nodes - 1 - np.arange(n_nodes))).astype(np.float32)
+    n = 20000
+    trk = dict(x=np.zeros(n), y=np.zeros(n), z=np.full(n, 20000.0), dx=np.zeros(n), dy=np.zeros(n), dz=-np.ones(n),
+               len=np.full(n, 50.0), beta=np.ones(n), t0=np.zeros(n), charge=-np.ones(n), p_GeV=np.full(n, 0.05))
+    trk = {k: np.asarray(v, np.float32) for k, v in trk.items()}
+    one = O.substep_tracks_ms(atm, trk, (0, 0, 0), 0.01, 50.0, 36.62)
+    assert one["offsets"][-1] == n
+    th0 = L.orc_highland_theta0(1.0, float(np.float32(0.05)), -1.0, rho * 50.0 / float(np.float32(36.62)))
+    s = one["segments"]
+    # chord of a single piece: end point = start + (0,0,-ds) + (ya, yb, 0) -> transverse direction components = y/len
+    yx, yy = s["dx"].astype(np.float64) * s["len"], s["dy"].astype(np.float64) * s["len"]
+    for y in (yx, yy):
+        assert abs(y.var() / (50.0 ** 2 * th0 ** 2 / 3.0) - 1.0) < 5 * math.sqrt(2.0 / n)
+        assert abs(y.mean()) < 5 * 50.0 * th0 / math.sqrt(3.0 * n)
+    # several pieces: direction of the last chord carries the accumulated deflection
+    m = 8
+    many = O.substep_tracks_ms(atm, trk, (0, 0, 0), 0.01, 50.0 / m, 36.62)
+    assert many["offsets"][-1] == n * m
+    th0m = L.orc_highland_theta0(1.0, float(np.float32(0.05)), -1.0, rho * (50.0 / m) / float(np.float32(36.62)))
+    sm = many["segments"]
+    last = np.arange(n) * m + (m - 1)
+    # last chord direction = accumulated angle of m-1 pieces + own offset/len: Var = (m-1) th0m^2 + th0m^2/3
+    want = (m - 1 + 1.0 / 3.0) * th0m ** 2
+    assert abs(sm["dx"][last].astype(np.float64).var() / want - 1.0) < 6 * math.sqrt(2.0 / n)
+    # continuity of the walk: piece 1 starts where piece 0 ended
+    a1 = sm["dx"][np.arange(n) * m].astype(np.float64) * sm["len"][np.arange(n) * m]   # y of piece 0
+    x0 = sm["x"][np.arange(n) * m + 1].astype(np.float64)                 # start of piece 1 = y of piece 0 (x started at 0)
+    assert np.allclose(a1, x0, atol=2e-4)
+    # the (offset, angle) pair of one piece is correlated: Cov(y_0, theta_0) = ds theta0^2 / 2, i.e. corr = sqrt(3)/2;
+    # chord 1's direction = theta_0 + (independent offset of piece 1)/ds
+    dir1 = sm["dx"][np.arange(n) * m + 1].astype(np.float64)
+    cov = np.mean((a1 - a1.mean()) * (dir1 - dir1.mean()))
+    assert abs(cov / ((50.0 / m) * th0m ** 2 / 2.0) - 1.0) < 0.06
+    # zero density: identical to the magnetic pieces
+    vac = dict(atm, overburden=np.zeros(n_nodes, np.float32))
+    B = (2.0e-5, -0.5e-5, -4.3e-5)
+    sub = {k: v[:200] for k, v in trk.items()}
+    r16 = O.substep_tracks(sub, B, 0.01)
+    r18 = O.substep_tracks_ms(vac, sub, B, 0.01, 0.0, 36.62)
+    assert np.array_equal(r16["offsets"], r18["offsets"])
+    for k in ("x", "y", "z", "dx", "dy", "dz", "len", "t0"):
+        assert np.allclose(r16["segments"][k], r18["segments"][k], rtol=2e-6, atol=2e-3), k
+    # draws depend on (seed, track id, piece): shifting the id base shifts the result
+    a = O.substep_tracks_ms(atm, {k: v[5:9] for k, v in trk.items()}, (0, 0, 0), 0.01, 50.0, 36.62, track_id_base=5)
+    assert np.array_equal(a["segments"]["dx"], one["segments"]["dx"][5:9])
