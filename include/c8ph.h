@@ -211,10 +211,15 @@ int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, 
                              const c8ph_outputs *host_out);
 
 /* ---- sub-stepping: the step before the hot path (thesis sec. 4.2.1) -------------------
- * Long particle steps are cut into linear pieces that follow the magnetically deflected path
- * f_mag:[0,1]->R^3 to the telescopes' resolution.  Uniform field B [T]: the path is
+ * Long particle steps are cut into linear pieces that follow the physical path to the telescopes'
+ * resolution.  Magnetic deflection: uniform field B [T], the path f_mag:[0,1]->R^3 is
  * the Lorentz helix with kappa = 0.299792458 q B / p [1/m]; a track of arc length `len` becomes
- * n = ceil(len / sqrt(8 tol / curvature)) chords (sagitta of each <= tol_m), n <= max_sub.
+ * n = ceil(len / sqrt(8 tol / curvature)) pieces (sagitta of each chord <= tol_m).  Multiple
+ * scattering (optional): n >= ceil(len / ms_max_step_m); every piece gets Highland's
+ * width theta0 = 13.6 MeV/(beta c p) |z| sqrt(t)(1 + 0.038 ln(t z^2/beta^2)), t = rho(h) ds / X0, and
+ * per transverse plane the correlated Gaussian offset / deflection pair, drawn from Philox
+ * (seed; piece index, track_id_base + i, stream 16): a random walk from piece to piece.  Needs the
+ * atmosphere (overburden table) of the context for the density.  n <= max_sub.
  * Two calls, both asynchronous on `stream`, no allocation:
  *   c8ph_substep_plan  writes offsets[0..n_tracks] (exclusive prefix sum of the piece counts); the
  *                      caller reads offsets[n_tracks] to size the segment arrays;
@@ -222,14 +227,24 @@ int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, 
  * tracks: the c8ph_segments SoA (x,y,z = start, dx,dy,dz = initial direction, len = arc length,
  * beta, t0, charge; edep ignored) plus p_GeV (momentum [GeV/c]); all DEVICE pointers.
  * out: DEVICE SoA of capacity >= offsets[n_tracks] per array (edep, if given, is zeroed).        */
+typedef struct {
+    uint32_t size;
+    float B_tesla[3];
+    float tol_m;                            /* sagitta bound of the magnetic chords (> 0)          */
+    int32_t max_sub;                        /* pieces per track <= max_sub (>= 1)                  */
+    int32_t ms_enabled;                     /* multiple-scattering sub-steps                       */
+    float ms_max_step_m, ms_X0_gcm2;        /* piece length bound; radiation length (air: 36.62)   */
+    uint64_t seed;
+    int64_t track_id_base;
+} c8ph_substep_desc;
 int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
-                      const float B_tesla[3], float tol_m, int32_t max_sub, int64_t *offsets, void *stream);
+                      const c8ph_substep_desc *desc, int64_t *offsets, void *stream);
 typedef struct {                            /* like c8ph_segments, but written */
     uint32_t size;
     float *x, *y, *z, *dx, *dy, *dz, *len, *beta, *t0, *charge, *edep;
 } c8ph_segments_out;
 int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
-                      const float B_tesla[3], float tol_m, int32_t max_sub, const int64_t *offsets,
+                      const c8ph_substep_desc *desc, const int64_t *offsets,
                       const c8ph_segments_out *out, void *stream);
 
 /* Device time of the last c8ph_emit_propagate kernel of this context in ms (CUDA events on the

@@ -88,6 +88,12 @@ class SegmentsOut(C.Structure):
                                           ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
 
 
+class SubstepDesc(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("B_tesla", C.c_float * 3), ("tol_m", C.c_float), ("max_sub", C.c_int32),
+                ("ms_enabled", C.c_int32), ("ms_max_step_m", C.c_float), ("ms_X0_gcm2", C.c_float),
+                ("seed", C.c_uint64), ("track_id_base", C.c_int64)]
+
+
 class Outputs(C.Structure):
     _fields_ = [("size", C.c_uint32), ("hist", C.c_void_p), ("tel_counts", C.c_void_p), ("photons", C.c_void_p),
                 ("photon_weight", C.c_void_p), ("photon_capacity", C.c_int64), ("counters", C.c_void_p)]
@@ -123,10 +129,10 @@ def load_library():
         L.c8ph_last_kernel_ms.restype = C.c_float
         L.c8ph_launch_count.argtypes = [C.c_void_p]
         L.c8ph_launch_count.restype = C.c_int64
-        L.c8ph_substep_plan.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(C.c_float),
-                                        C.c_float, C.c_int32, C.c_void_p, C.c_void_p]
-        L.c8ph_substep_fill.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(C.c_float),
-                                        C.c_float, C.c_int32, C.c_void_p, C.POINTER(SegmentsOut), C.c_void_p]
+        L.c8ph_substep_plan.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(SubstepDesc),
+                                        C.c_void_p, C.c_void_p]
+        L.c8ph_substep_fill.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(SubstepDesc),
+                                        C.c_void_p, C.POINTER(SegmentsOut), C.c_void_p]
         L.c8ph_counter_name.argtypes = [C.c_int]
         L.c8ph_counter_name.restype = C.c_char_p
         _lib = L
@@ -352,9 +358,11 @@ class Context:
                     counters_raw=np.zeros(N_COUNTERS, dtype=np.uint64))
 
     # ---- sub-stepping (the step before the hot path) ---------------------------------------------
-    def substep_tracks(self, trk_dev: dict, n_tracks: int, B_tesla, tol_m: float, max_sub: int = 4096, stream=None):
+    def substep_tracks(self, trk_dev: dict, n_tracks: int, B_tesla, tol_m: float, max_sub: int = 4096, stream=None,
+                       ms_max_step_m=None, ms_X0_gcm2: float = 36.62, seed: int = 1, track_id_base: int = 0):
         """trk_dev: dict of torch CUDA float32 tensors x,y,z,dx,dy,dz,len,beta,t0,charge,p_GeV.
         Returns (segments dict of torch CUDA tensors incl. edep = 0, offsets int64[n+1] CUDA tensor).
+        ms_max_step_m is not None: multiple-scattering pieces (0 = no cap on the piece length).
         c8ph_substep_plan -> read offsets[n] (one 8-byte D2H) -> allocate -> c8ph_substep_fill."""
         import torch
         dev = trk_dev["x"].device
@@ -364,9 +372,15 @@ class Context:
             v = trk_dev.get(k)
             setattr(t, k, _dev_ptr(v, "float32", n_tracks) if (v is not None and k != "edep") else None)
         p = _dev_ptr(trk_dev["p_GeV"], "float32", n_tracks)
-        Bv = (C.c_float * 3)(*[float(b) for b in B_tesla])
+        d = SubstepDesc()
+        d.size = C.sizeof(SubstepDesc)
+        d.B_tesla = (C.c_float * 3)(*[float(b) for b in B_tesla])
+        d.tol_m, d.max_sub = float(tol_m), int(max_sub)
+        d.ms_enabled = 0 if ms_max_step_m is None else 1
+        d.ms_max_step_m = 0.0 if ms_max_step_m is None else float(ms_max_step_m)
+        d.ms_X0_gcm2, d.seed, d.track_id_base = float(ms_X0_gcm2), int(seed), int(track_id_base)
         offsets = torch.zeros(n_tracks + 1, dtype=torch.int64, device=dev)
-        self._check(self.lib.c8ph_substep_plan(self._h, C.byref(t), p, int(n_tracks), Bv, float(tol_m), int(max_sub),
+        self._check(self.lib.c8ph_substep_plan(self._h, C.byref(t), p, int(n_tracks), C.byref(d),
                                                offsets.data_ptr(), _stream_ptr(stream)))
         total = int(offsets[-1].item())
         seg = {k: torch.empty(max(total, 1), dtype=torch.float32, device=dev) for k in SEG_FIELDS}
@@ -374,7 +388,7 @@ class Context:
         o.size = C.sizeof(SegmentsOut)
         for k in SEG_FIELDS:
             setattr(o, k, seg[k].data_ptr())
-        self._check(self.lib.c8ph_substep_fill(self._h, C.byref(t), p, int(n_tracks), Bv, float(tol_m), int(max_sub),
+        self._check(self.lib.c8ph_substep_fill(self._h, C.byref(t), p, int(n_tracks), C.byref(d),
                                                offsets.data_ptr(), C.byref(o), _stream_ptr(stream)))
         return {k: v[:total] for k, v in seg.items()}, offsets
 

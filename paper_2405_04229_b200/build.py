@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libc8ph.so")
 SOURCES = ("c8ph_host.cu", "c8ph_kernels.cu", "c8ph_substep.cu")
-HEADERS = ("c8ph_device.cuh", os.path.join("..", "..", "include", "c8ph.h"))
+HEADERS = ("c8ph_device.cuh", "c8ph_philox.cuh", os.path.join("..", "..", "include", "c8ph.h"))
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -145,6 +145,11 @@ struct SubstepArgs {
     int max_sub;
     long long *offsets;             // [n+1]
     c8ph_segments_out out;          // DEVICE (fill only)
+    int ms_enabled;                 // multiple-scattering sub-steps (R18)
+    double ms_max_step, ms_X0;
+    uint2 key[10];                  // Philox round keys
+    long long id_base;
+    DevAtm atm;                     // density from the overburden table
 };
 
 // kernels / launchers (c8ph_kernels.cu)
@@ -153,7 +158,7 @@ cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st);
 size_t emit_smem_bytes(const KArgs &a);
 size_t segment_slot_bytes(int n_sm);
 cudaError_t launch_substep_plan(const SubstepArgs &a, long long *block_sums, cudaStream_t st);
-cudaError_t launch_substep_fill(const SubstepArgs &a, cudaStream_t st);
+cudaError_t launch_substep_fill(const SubstepArgs &a, int n_sm, cudaStream_t st);
 size_t substep_scratch_elems(long long n);
 void segment_slot_pointers(void *base, int n_sm, DevRun &run);
 

@@ -762,27 +762,38 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
 }
 
 // ------------------------------------------------------------------------------------ sub-stepping
-static int substep_args(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3], float tol,
-                        int32_t max_sub, SubstepArgs &a)
+static int substep_args(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const c8ph_substep_desc *d,
+                        SubstepArgs &a)
 {
-    if (!t || t->size != sizeof(c8ph_segments) || !B) return fail(ctx, C8PH_E_ARG, "substep: NULL struct or size mismatch");
+    if (!t || t->size != sizeof(c8ph_segments) || !d || d->size != sizeof(c8ph_substep_desc))
+        return fail(ctx, C8PH_E_ARG, "substep: NULL struct or size mismatch");
     if (n < 0 || substep_scratch_elems(n) > kSubstepBlockSums) return fail(ctx, C8PH_E_ARG, "substep: n_tracks out of range (<= 2^27 per call)");
     if (n > 0 && (!t->x || !t->y || !t->z || !t->dx || !t->dy || !t->dz || !t->len || !t->beta || !t->t0 || !t->charge || !p_GeV))
         return fail(ctx, C8PH_E_ARG, "substep: NULL track array");
-    if (!(tol > 0.f) || max_sub < 1) return fail(ctx, C8PH_E_ARG, "substep: tol_m > 0 and max_sub >= 1 required");
+    if (!(d->tol_m > 0.f) || d->max_sub < 1) return fail(ctx, C8PH_E_ARG, "substep: tol_m > 0 and max_sub >= 1 required");
+    if (d->ms_enabled) {
+        if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "substep: multiple scattering needs the atmosphere (overburden) of the context");
+        if (!(d->ms_X0_gcm2 > 0.f) || !(d->ms_max_step_m >= 0.f) || d->track_id_base < 0)
+            return fail(ctx, C8PH_E_ARG, "substep: ms_X0_gcm2 > 0, ms_max_step_m >= 0 and track_id_base >= 0 required");
+    }
     a.trk = *t; a.p_GeV = p_GeV; a.n = n;
-    for (int k = 0; k < 3; ++k) a.B[k] = B[k];
+    for (int k = 0; k < 3; ++k) a.B[k] = d->B_tesla[k];
     a.Bn = std::sqrt(a.B[0] * a.B[0] + a.B[1] * a.B[1] + a.B[2] * a.B[2]);
-    a.tol = tol; a.max_sub = max_sub;
+    a.tol = d->tol_m; a.max_sub = d->max_sub;
+    a.ms_enabled = d->ms_enabled ? 1 : 0; a.ms_max_step = d->ms_max_step_m; a.ms_X0 = d->ms_X0_gcm2;
+    a.id_base = d->track_id_base;
+    for (int k = 0; k < 10; ++k)
+        a.key[k] = make_uint2((uint32_t)d->seed + (uint32_t)k * 0x9E3779B9u, (uint32_t)(d->seed >> 32) + (uint32_t)k * 0xBB67AE85u);
+    if (ctx->have_atm) a.atm = ctx->atm;
     return C8PH_OK;
 }
 
-extern "C" int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3],
-                                 float tol, int32_t max_sub, int64_t *offsets, void *stream)
+extern "C" int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n,
+                                 const c8ph_substep_desc *d, int64_t *offsets, void *stream)
 {
     if (!ctx) return C8PH_E_ARG;
     SubstepArgs a{};
-    int rc = substep_args(ctx, t, p_GeV, n, B, tol, max_sub, a);
+    int rc = substep_args(ctx, t, p_GeV, n, d, a);
     if (rc) return rc;
     if (!offsets) return fail(ctx, C8PH_E_ARG, "substep_plan: offsets is NULL");
     CU(cudaSetDevice(ctx->device));
@@ -794,12 +805,12 @@ extern "C" int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *t, const fl
     return C8PH_OK;
 }
 
-extern "C" int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n, const float B[3],
-                                 float tol, int32_t max_sub, const int64_t *offsets, const c8ph_segments_out *out, void *stream)
+extern "C" int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_GeV, int64_t n,
+                                 const c8ph_substep_desc *d, const int64_t *offsets, const c8ph_segments_out *out, void *stream)
 {
     if (!ctx) return C8PH_E_ARG;
     SubstepArgs a{};
-    int rc = substep_args(ctx, t, p_GeV, n, B, tol, max_sub, a);
+    int rc = substep_args(ctx, t, p_GeV, n, d, a);
     if (rc) return rc;
     if (!offsets || !out || out->size != sizeof(c8ph_segments_out) || !out->x || !out->y || !out->z || !out->dx || !out->dy ||
         !out->dz || !out->len || !out->beta || !out->t0 || !out->charge)
@@ -808,7 +819,7 @@ extern "C" int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *t, const fl
     CU(cudaSetDevice(ctx->device));
     a.offsets = const_cast<long long *>(reinterpret_cast<const long long *>(offsets));
     a.out = *out;
-    cudaError_t e = launch_substep_fill(a, (cudaStream_t)stream);
+    cudaError_t e = launch_substep_fill(a, ctx->n_sm, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "substep_fill launch");
     ctx->launches++;
     return C8PH_OK;

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 #include "c8ph_device.cuh"
+#include "c8ph_philox.cuh"
 
 namespace c8ph {
 
@@ -44,12 +45,20 @@ __device__ __forceinline__ Helix helix_of(const SubstepArgs &a, long long i)
     return h;
 }
 
-// number of chords: sagitta L_piece^2 curvature / 8 <= tol
-__device__ __forceinline__ int pieces_of(const Helix &h, double tol, int max_sub)
+// number of pieces: sagitta L_piece^2 curvature / 8 <= tol, and (multiple scattering) L_piece <= ms_max_step
+__device__ __forceinline__ int pieces_of(const Helix &h, const SubstepArgs &a)
 {
-    if (!(h.curv > 0.0) || !(h.L > 0.0)) return 1;
-    const double nn = ceil(h.L / sqrt(8.0 * tol / h.curv));
-    return nn < 1.0 ? 1 : (nn > (double)max_sub ? max_sub : (int)nn);
+    int n = 1;
+    if (h.curv > 0.0 && h.L > 0.0) {
+        const double nn = ceil(h.L / sqrt(8.0 * a.tol / h.curv));
+        n = nn < 1.0 ? 1 : (nn > (double)a.max_sub ? a.max_sub : (int)nn);
+    }
+    if (a.ms_enabled && a.ms_max_step > 0.0 && h.L > 0.0) {
+        const double nn = ceil(h.L / a.ms_max_step);
+        const int n2 = nn > (double)a.max_sub ? a.max_sub : (int)nn;
+        if (n2 > n) n = n2;
+    }
+    return n;
 }
 
 __device__ __forceinline__ void point_on(const Helix &h, double s, double X[3])
@@ -68,7 +77,7 @@ __global__ void __launch_bounds__(kScanThreads) k_substep_count(const __grid_con
     __shared__ long long s_warp[32];
     const long long i = (long long)blockIdx.x * kScanThreads + threadIdx.x;
     long long v = 0;
-    if (i < a.n) v = pieces_of(helix_of(a, i), a.tol, a.max_sub);
+    if (i < a.n) v = pieces_of(helix_of(a, i), a);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int d = 1; d < 32; d <<= 1) {
         const long long t = __shfl_up_sync(0xFFFFFFFFu, v, d);
@@ -162,6 +171,85 @@ __global__ void __launch_bounds__(256) k_substep_fill(const __grid_constant__ Su
     }
 }
 
+// fill with multiple scattering (R18): the pieces of a track are a random walk, so one thread walks one
+// track: exact magnetic rotation of the piece, then Highland's correlated offset / deflection per plane
+__global__ void __launch_bounds__(128) k_substep_fill_ms(const __grid_constant__ SubstepArgs a)
+{
+    const DevAtm &atm = a.atm;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
+        const Helix h = helix_of(a, i);
+        const long long g0 = a.offsets[i];
+        const int n = (int)(a.offsets[i + 1] - g0);
+        const double ds = h.L / (double)n;
+        const double p = a.p_GeV[i];
+        const unsigned long long tid = (unsigned long long)(a.id_base + i);
+        double X[3] = {h.A[0], h.A[1], h.A[2]};
+        double P[3];
+        for (int k = 0; k < 3; ++k) P[k] = h.ppar * h.bh[k] + h.pperp * h.e1[k];
+        double sn, cs;
+        sincos(h.kappa * ds, &sn, &cs);
+        for (int j = 0; j < n; ++j) {
+            const double ppar = P[0] * h.bh[0] + P[1] * h.bh[1] + P[2] * h.bh[2];
+            const double Pp[3] = {P[0] - ppar * h.bh[0], P[1] - ppar * h.bh[1], P[2] - ppar * h.bh[2]};
+            const double Pc[3] = {Pp[1] * h.bh[2] - Pp[2] * h.bh[1], Pp[2] * h.bh[0] - Pp[0] * h.bh[2], Pp[0] * h.bh[1] - Pp[1] * h.bh[0]};
+            double dX[3], Pn[3];
+            for (int k = 0; k < 3; ++k) {
+                if (h.kappa != 0.0) {
+                    dX[k] = ppar * h.bh[k] * ds + (sn * Pp[k] + (1.0 - cs) * Pc[k]) / h.kappa;
+                    Pn[k] = ppar * h.bh[k] + cs * Pp[k] + sn * Pc[k];
+                } else { dX[k] = P[k] * ds; Pn[k] = P[k]; }
+            }
+            // density of the overburden-table cell at the piece's mid height
+            const double mx = X[0] + 0.5 * dX[0], my = X[1] + 0.5 * dX[1], mz = X[2] + 0.5 * dX[2];
+            double hm = atm.h_obs + mz;
+            if (atm.model == C8PH_ATM_SPHERICAL) hm = sqrt(mx * mx + my * my + (mz + atm.Rg) * (mz + atm.Rg)) - atm.R;
+            double rho = 0.0;
+            if (atm.model != C8PH_ATM_HOMOGENEOUS) {
+                double f = (hm - (double)atm.h0) / (double)atm.dh;
+                f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
+                const int k = min((int)f, atm.n_nodes - 2);
+                rho = ((double)__ldg(atm.xv + k) - (double)__ldg(atm.xv + k + 1)) / (double)atm.dh;
+            }
+            double th0 = 0.0;
+            const double t = rho * ds / a.ms_X0;
+            if (t > 0.0 && p > 0.0) {
+                const double corr = fmax(1.0 + 0.038 * log(t * h.charge * h.charge / (h.beta * h.beta)), 0.0);
+                th0 = 0.0136 / (h.beta * p) * fabs(h.charge) * sqrt(t) * corr;
+            }
+            const uint4 r = philox4x32_10((uint32_t)j, (uint32_t)tid, (uint32_t)(tid >> 32), 16u, a.key);
+            auto u01d = [](uint32_t v) { return ((double)(v >> 9) + 0.5) * (1.0 / 8388608.0); };
+            const double r1 = sqrt(-2.0 * log(u01d(r.x))), r2 = sqrt(-2.0 * log(u01d(r.z)));
+            double s1, c1, s2, c2;
+            sincos(2.0 * 3.14159265358979323846 * u01d(r.y), &s1, &c1);
+            sincos(2.0 * 3.14159265358979323846 * u01d(r.w), &s2, &c2);
+            const double z1 = r1 * c1, z2 = r1 * s1, z3 = r2 * c2, z4 = r2 * s2;
+            double ea[3] = {Pn[1], -Pn[0], 0.0};
+            double na = sqrt(ea[0] * ea[0] + ea[1] * ea[1]);
+            if (na < 1e-12) { ea[0] = 1.0; ea[1] = 0.0; na = 1.0; }
+            ea[0] /= na; ea[1] /= na;
+            const double eb[3] = {Pn[1] * ea[2] - Pn[2] * ea[1], Pn[2] * ea[0] - Pn[0] * ea[2], Pn[0] * ea[1] - Pn[1] * ea[0]};
+            const double ya = (z1 / sqrt(12.0) + 0.5 * z2) * ds * th0, yb = (z3 / sqrt(12.0) + 0.5 * z4) * ds * th0;
+            double Xe[3], Pe[3];
+            for (int k = 0; k < 3; ++k) {
+                Xe[k] = X[k] + dX[k] + ya * ea[k] + yb * eb[k];
+                Pe[k] = Pn[k] + z2 * th0 * ea[k] + z4 * th0 * eb[k];
+            }
+            const double pn = 1.0 / sqrt(Pe[0] * Pe[0] + Pe[1] * Pe[1] + Pe[2] * Pe[2]);
+            const double d[3] = {Xe[0] - X[0], Xe[1] - X[1], Xe[2] - X[2]};
+            const double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            const long long g = g0 + j;
+            a.out.x[g] = (float)X[0]; a.out.y[g] = (float)X[1]; a.out.z[g] = (float)X[2];
+            a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            a.out.len[g] = (float)len;
+            a.out.beta[g] = (float)h.beta;
+            a.out.t0[g] = (float)(h.t0 + (double)j * ds / (h.beta * 0.299792458));
+            a.out.charge[g] = (float)h.charge;
+            if (a.out.edep) a.out.edep[g] = 0.f;
+            for (int k = 0; k < 3; ++k) { X[k] = Xe[k]; P[k] = Pe[k] * pn; }
+        }
+    }
+}
+
 }  // namespace
 
 size_t substep_scratch_elems(long long n) { return (size_t)((n + kScanThreads - 1) / kScanThreads); }
@@ -175,9 +263,10 @@ cudaError_t launch_substep_plan(const SubstepArgs &a, long long *block_sums, cud
     return cudaGetLastError();
 }
 
-cudaError_t launch_substep_fill(const SubstepArgs &a, cudaStream_t st)
+cudaError_t launch_substep_fill(const SubstepArgs &a, int n_sm, cudaStream_t st)
 {
-    k_substep_fill<<<148 * 8, 256, 0, st>>>(a);
+    if (a.ms_enabled) k_substep_fill_ms<<<n_sm * 8, 128, 0, st>>>(a);
+    else k_substep_fill<<<n_sm * 8, 256, 0, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -522,6 +522,48 @@ def test_substepping_matches_the_oracle_and_feeds_the_hot_path():
         assert abs(gpu["counters"]["emitted"] - ora["counters"]["emitted"]) <= 1e-3 * ora["counters"]["emitted"]
 
 
+def test_multiple_scattering_substeps_match_the_oracle():
+    """Row f2 with multiple scattering (R18): one thread walks one track (magnetic rotation, Highland
+    offset and deflection per piece, normals from Philox counter (piece, track id, 16)).  Piece counts
+    bit-exact; both sides walk in fp64, so the random walk agrees to rounding: positions to fp32 storage +
+    1e-4 m, directions 1e-6, lengths 1e-5 relative; ids offset by track_id_base; E_STATE without an atmosphere."""
+    rng = np.random.default_rng(22)
+    n = 3000
+    cfg = W.make_config(4, n_segments=n)
+    trk = {k: v.copy() for k, v in cfg["segments"].items() if k != "edep"}
+    trk["len"] = rng.uniform(5.0, 400.0, n).astype(np.float32)
+    trk["p_GeV"] = (10 ** rng.uniform(-2.0, 1.0, n)).astype(np.float32)
+    B, tol, step, seed, base = (2.0e-5, -0.5e-5, -4.3e-5), 0.01, 25.0, 77, 1 << 33
+    want = O.substep_tracks_ms(cfg["atmosphere"], trk, B, tol, step, seed=seed, track_id_base=base)
+    ctx = api.setup_context(cfg)
+    dev = {k: torch.from_numpy(v).cuda() for k, v in trk.items()}
+    seg, off = ctx.substep_tracks(dev, n, B, tol, ms_max_step_m=step, seed=seed, track_id_base=base)
+    assert np.array_equal(off.cpu().numpy(), want["offsets"]) and want["offsets"][-1] > 5 * n
+    got = {k: v.cpu().numpy() for k, v in seg.items()}
+    ws = want["segments"]
+    for k in ("x", "y", "z"):
+        assert np.abs(got[k].astype(np.float64) - ws[k]).max() <= 2 * np.spacing(np.float32(np.abs(ws[k]).max())) + 1e-4
+    for k in ("dx", "dy", "dz"):
+        assert np.abs(got[k] - ws[k]).max() < 1e-6
+    assert np.allclose(got["len"], ws["len"], rtol=1e-5, atol=0) and np.allclose(got["t0"], ws["t0"], rtol=0, atol=5e-3)
+    assert np.array_equal(got["beta"], ws["beta"]) and np.array_equal(got["charge"], ws["charge"]) and not got["edep"].any()
+    # the walk really scatters: the pieces differ from the helix chords of the same count by far more than rounding
+    seg_h, off_h = ctx.substep_tracks(dev, n, B, tol)
+    assert int(off[-1]) > int(off_h[-1])
+    low = trk["p_GeV"] < 0.05
+    first, last = want["offsets"][:-1][low], want["offsets"][1:][low] - 1
+    bend = np.abs(got["dx"][last] - got["dx"][first]) + np.abs(got["dy"][last] - got["dy"][first])
+    assert np.median(bend) > 1e-3
+    # another id base draws other normals
+    seg2, _ = ctx.substep_tracks(dev, n, B, tol, ms_max_step_m=step, seed=seed, track_id_base=0)
+    assert np.abs(seg2["x"].cpu().numpy() - got["x"]).max() > 1e-3
+    # no atmosphere in the context: refused
+    bare = api.Context()
+    with pytest.raises(api.C8phError) as e:
+        bare.substep_tracks(dev, n, B, tol, ms_max_step_m=step)
+    assert e.value.code == api.E_STATE
+
+
 def test_tabulated_extinction():
     """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
     scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an
