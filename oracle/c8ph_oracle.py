@@ -76,7 +76,7 @@ class Params(C.Structure):
                 ("n_lines", C.c_int32), ("pad", C.c_int32),
                 ("line_nm", C.POINTER(C.c_float)), ("line_cdf", C.POINTER(C.c_float)),
                 ("disp_b_nm2", C.c_double), ("disp_lambda0_nm", C.c_double),
-                ("n_eff", C.c_int32), ("pad2", C.c_int32),
+                ("n_eff", C.c_int32), ("flat_plane", C.c_int32),
                 ("eff_lambda0_nm", C.c_double), ("eff_dlambda_nm", C.c_double), ("eff", C.POINTER(C.c_float))]
 
 
@@ -222,6 +222,7 @@ def params_struct(par: dict, keep: _Keep) -> Params:
     s.disp_lambda0_nm = float(np.float32(par.get("disp_lambda0_nm", 400.0)))
     eff = par.get("eff")
     s.n_eff = 0 if eff is None else len(eff)
+    s.flat_plane = int(bool(par.get("flat_plane", False)))
     s.eff = keep.f32(eff) if s.n_eff else None
     s.eff_lambda0_nm = float(np.float32(par.get("eff_lambda0_nm", 0.0)))
     s.eff_dlambda_nm = float(np.float32(par.get("eff_dlambda_nm", 1.0)))
