@@ -150,6 +150,15 @@ typedef struct {
     int32_t n_eff;
     float eff_lambda0_nm, eff_dlambda_nm;
     const float *eff;                       /* HOST [n_eff]; copied at every call                  */
+    /* Flat observation plane in the spherical model (thesis Fig. 4.10: the correction tables are
+     * "relative to a flat observation plane"; R19).  The (height, zenith) table describes the ray
+     * where it meets the observation SPHERE; 0: its displacement is applied at the straight-line point of
+     * the plane z = 0 (the sag of the sphere under the plane is ignored: < 1 mm within 5 km of the
+     * origin, centimetres beyond 15 km); 1: line on to the sphere, arc along the flight direction, back
+     * along the arrival direction to z = 0 (0.1 mm / 1 ps against a 3-D ray integration out to 25 km).
+     * Photons whose straight line misses the sphere count as C8PH_CNT_TABLE_RANGE.  Ignored for the
+     * planar / homogeneous models and the straight trace.                                          */
+    int32_t flat_plane;
 } c8ph_params;
 
 /* ---- segments, outputs ------------------------------------------------------------------------- */

@@ -75,7 +75,8 @@ class Params(C.Structure):
                 ("lv1_margin_rad", C.c_float), ("lv2_margin_m", C.c_float),
                 ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float), ("n_lines", C.c_int32),
                 ("line_nm", _fp), ("line_cdf", _fp), ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float),
-                ("n_eff", C.c_int32), ("eff_lambda0_nm", C.c_float), ("eff_dlambda_nm", C.c_float), ("eff", _fp)]
+                ("n_eff", C.c_int32), ("eff_lambda0_nm", C.c_float), ("eff_dlambda_nm", C.c_float), ("eff", _fp),
+                ("flat_plane", C.c_int32)]
 
 
 class Segments(C.Structure):
@@ -275,6 +276,7 @@ class Context:
         if ef is not None:
             p.eff = ef.ctypes.data_as(_fp)
         p.eff_lambda0_nm, p.eff_dlambda_nm = float(par.get("eff_lambda0_nm", 0.0)), float(par.get("eff_dlambda_nm", 1.0))
+        p.flat_plane = int(bool(par.get("flat_plane", False)))
         return p, (ln, lc, ef)
 
     # ---- the hot call, DEVICE buffers ------------------------------------------------------------

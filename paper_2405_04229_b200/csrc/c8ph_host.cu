@@ -571,6 +571,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         if (p->trace == C8PH_TRACE_STRAIGHT) r.hit_infl = 1.0f + 1e-5f;
     }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
+    r.flat_plane = (p->flat_plane && ctx->atm.model == C8PH_ATM_SPHERICAL && p->trace != C8PH_TRACE_STRAIGHT) ? 1 : 0;
     r.n_eff = p->n_eff; r.eff = nullptr;
     r.eff_l0 = p->eff_lambda0_nm; r.eff_inv_dl = p->n_eff > 1 ? 1.0f / p->eff_dlambda_nm : 0.f;
     if (p->n_eff > 0) {

@@ -462,12 +462,35 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_eff = SPEC ? false : run.n_eff > 0;
     const bool f_opt = SPEC ? false : det.opt_enabled != 0;
     const bool f_ext = SPEC ? false : atm.n_ext > 0;
+    const bool f_flat = (SPEC || !SPH || TRACE == C8PH_TRACE_STRAIGHT) ? false : run.flat_plane != 0;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
     const bool f_telc = SPEC ? true : run.out.tel_counts != nullptr;
     const float inv_ng = 1.0f / (1.0f + atm.eta_g);
     int q_head = 0;                                           // ring position of the oldest queue entry
+
+    // arrival direction: u turned in the ray plane (u, local vertical) by the angle that follows from the
+    // Snell / Bouguer invariant (R9), small-angle form
+    auto arrival_dir = [&](const SegCold *sc, float ux, float uy, float uz, float cz, float eta_e, float h_e, float dd,
+                           float &uax, float &uay, float &uaz) {
+        uax = ux; uay = uy; uaz = uz;
+        const float sinz = sqrt_fast(fmaxf(1.f - cz * cz, 0.f));
+        if (TRACE != C8PH_TRACE_STRAIGHT && sinz >= 1e-6f) {
+            const float eps = (eta_e - atm.eta_g) * inv_ng;
+            const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * run.inv_Rg : 1.f;
+            const float al = sinz * scale;
+            const float cyy = sqrt_fast(fmaxf(1.f - al * al, 0.f));
+            const float at = al * (1.f + eps);
+            const float cxx = sqrt_fast(fmaxf(1.f - at * at, 0.f));
+            float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * rcp_fast(cyy + cxx));
+            if (SPH) dl -= dd * run.inv_Rg;
+            const float k2 = dl * rcp_fast(sinz), k1 = fmaf(k2, cz, fmaf(-0.5f * dl, dl, 1.f));
+            uax = fmaf(k1, ux, k2 * sc->rx);
+            uay = fmaf(k1, uy, k2 * sc->ry);
+            uaz = fmaf(k1, uz, k2 * sc->rz);
+        }
+    };
 
     // ---- a13/a14/a16 for photons that may hit a telescope or are written anyway: arrival direction
     // (rotation in the ray plane by the Snell / Bouguer invariant), exact sphere search, counters,
@@ -498,21 +521,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 const float D = -fmaf(s, sh->Pz, sh->Az) * rcp_fast(uz);
                 t_arr = sc->Tg + fmaf(fmaf(s, sh->inv_beta, D), kInvC, dt);
             }
-            const float sinz = sqrt_fast(fmaxf(1.f - cz * cz, 0.f));
-            if (TRACE != C8PH_TRACE_STRAIGHT && sinz >= 1e-6f) {
-                const float eps = (eta_e - atm.eta_g) * inv_ng;
-                const float scale = SPH ? 1.f + (h_e - (float)atm.h_obs) * run.inv_Rg : 1.f;
-                const float al = sinz * scale;
-                const float cyy = sqrt_fast(fmaxf(1.f - al * al, 0.f));
-                const float at = al * (1.f + eps);
-                const float cxx = sqrt_fast(fmaxf(1.f - at * at, 0.f));
-                float dl = al * (eps * cyy + al * al * eps * (2.f + eps) * rcp_fast(cyy + cxx));
-                if (SPH) dl -= dd * run.inv_Rg;
-                const float k2 = dl * rcp_fast(sinz), k1 = fmaf(k2, cz, fmaf(-0.5f * dl, dl, 1.f));
-                uax = fmaf(k1, ux, k2 * sc->rx);
-                uay = fmaf(k1, uy, k2 * sc->ry);
-                uaz = fmaf(k1, uz, k2 * sc->rz);
-            }
+            arrival_dir(sc, ux, uy, uz, cz, eta_e, h_e, dd, uax, uay, uaz);
             if (f_tel && cell != -1) {
                 // the pre-test threshold must cover the rotated direction; if it does not (never in
                 // air), search all telescopes
@@ -1023,7 +1032,33 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float hn2 = ux * ux + uy * uy;
                     const float ih = hn2 >= 1e-18f ? rsqrt_fast(hn2) : 0.f;            // vertical photon: no correction
                     const float ehx = ux * ih, ehy = uy * ih;
-                    const float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);         // offset from the anchor
+                    float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);               // offset from the anchor
+                    if (f_flat) {
+                        // R19, flat observation plane (thesis Fig. 4.10): dd, dt and the rotation hold where
+                        // the ray meets the observation sphere; the plane z = 0 lies h_I above it at the line point.
+                        // Line on to the sphere (s1), arc dd along the flight direction on the sphere, back along
+                        // the arrival direction to z = 0; all in cancellation-free perturbation form about I.
+                        const float Rg = (float)atm.Rg;
+                        const float rho2 = fmaf(xl, xl, yl * yl);
+                        const float hI = rho2 * rcp_fast(Rg + sqrt_fast(fmaf(Rg, Rg, rho2)));
+                        const float m = hI * fmaf(2.f, Rg, hI);                         // |I - C|^2 - Rg^2
+                        const float uw = fmaf(ux, xl, fmaf(uy, yl, uz * Rg));           // u . (I - C)
+                        const float disc = fmaf(uw, uw, -m);
+                        if (!(disc > 0.f) || !(uw < 0.f)) { pkB += 1u; break; }         // the line misses the sphere
+                        const float s1 = m * rcp_fast(sqrt_fast(disc) - uw);
+                        const float rwx = fmaf(s1, ux, xl) * run.inv_Rg, rwy = fmaf(s1, uy, yl) * run.inv_Rg;
+                        const float rwz = fmaf(s1 * uz, run.inv_Rg, 1.f);               // unit radial at the sphere point
+                        const float cw = fmaf(ux, rwx, fmaf(uy, rwy, uz * rwz));
+                        const float st2 = fmaf(-cw, cw, 1.f);
+                        const float ie = st2 >= 1e-18f ? rsqrt_fast(st2) : 0.f;
+                        const float etx = fmaf(-cw, rwx, ux) * ie, ety = fmaf(-cw, rwy, uy) * ie, etz = fmaf(-cw, rwz, uz) * ie;
+                        float uax, uay, uaz;
+                        arrival_dir(sc, ux, uy, uz, cz, eta_e, h_e, dd, uax, uay, uaz);
+                        const float sb = fmaf(dd, etz, s1 * uz) * rcp_fast(uaz);
+                        cx = ox + fmaf(dd, etx, fmaf(s1, ux, -sb * uax));
+                        cy = oy + fmaf(dd, ety, fmaf(s1, uy, -sb * uay));
+                        dt = fmaf(fmaf(-(1.f + atm.eta_g), sb, s1), kInvC, dt);
+                    }
                     const float xg = sg.Gx + cx, yg = sg.Gy + cy;
                     // a14 pre-test: the photon can hit a sphere of its grid cell only if the cell's
                     // smallest key <= 1/|u_z| (inflated for the refraction rotation of the direction); the
@@ -1243,7 +1278,7 @@ static bool array_production_setting(const KArgs &a)
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && a.atm.n_ext == 0 && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled;
+           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled && !r.flat_plane;
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)

@@ -564,6 +564,54 @@ def test_multiple_scattering_substeps_match_the_oracle():
     assert e.value.code == api.E_STATE
 
 
+def _off_centre(k, n, shift_m, zen_deg=None, **par):
+    """cfg k with segments, ground grid and telescopes moved rigidly by shift_m along x: the array sits that far
+    from the point where the plane z = 0 touches the observation sphere.  zen_deg: the segments become inclined
+    tracks of that zenith angle (random azimuth) whose axes pass within ~60 m of the array centre."""
+    cfg = W.make_config(k, n_segments=n)
+    s = cfg["segments"]
+    if zen_deg is not None:
+        rng = np.random.default_rng(5)
+        az, th = rng.uniform(0, 2 * np.pi, n), np.radians(zen_deg)
+        s["dx"] = (np.sin(th) * np.cos(az)).astype(np.float32)
+        s["dy"] = (np.sin(th) * np.sin(az)).astype(np.float32)
+        s["dz"] = np.full(n, -np.cos(th), np.float32)
+        s["x"] = (-s["z"] * np.tan(th) * np.cos(az) + rng.normal(0, 60, n)).astype(np.float32)
+        s["y"] = (-s["z"] * np.tan(th) * np.sin(az) + rng.normal(0, 60, n)).astype(np.float32)
+    s["x"] = (s["x"] + np.float32(shift_m)).astype(np.float32)
+    cfg["detector"]["hist_x0"] = cfg["detector"]["hist_x0"] + shift_m
+    tel = cfg["detector"]["tel_xyzr"].copy()
+    tel[:, 0] += np.float32(shift_m)
+    cfg["detector"]["tel_xyzr"] = tel
+    cfg["params"].update(par)
+    return cfg
+
+
+def test_flat_observation_plane_far_from_the_origin():
+    """Row f1 (thesis Fig. 4.10; R19): the detector plane z = 0 against the observation sphere of
+    the (height, zenith) table.  cfg4's array 18 km from the origin (sag 25 m): device against oracle photon by
+    photon with the flat-plane step on - cfg4's own near-vertical tracks, tracks inclined by 60 and 70 degrees
+    (where the step moves photons by up to 8 and 37 cm and the clock by up to 0.2 and 1.2 ns: more than the
+    tolerances); at the origin the step changes nothing.  (The per-photon layered sum is planar only.)"""
+    shift = 18000.0
+    for zen, n, d_med, d_max, t_med in ((None, 2500, 5e-4, 2e-3, 0.02), (60.0, 1500, 0.01, 0.07, 0.015), (70.0, 1500, 0.03, 0.3, 0.04)):
+        cfg = _off_centre(4, n, shift, zen, flat_plane=True)
+        ora, gpu, rep = _both(cfg)
+        assert gpu["counters"]["tel_hit"] > 1e4 and gpu["counters"]["in_grid"] > 1e5
+        assert rep["max_dpos_m"] < 0.02 and rep["max_dt_ns"] < 0.05
+        off = O.run(_off_centre(4, n, shift, zen, flat_plane=False))
+        a, b = ora["photons"], off["photons"]
+        both = (a["status"] == O.ST_LANDED) & (b["status"] == O.ST_LANDED)
+        d = np.hypot(a["x"][both] - b["x"][both], a["y"][both] - b["y"][both])
+        assert both.sum() > 1e5 and np.median(d) > d_med and d.max() > d_max
+        assert np.median(np.abs(a["t"][both] - b["t"][both])) > t_med
+    # at the origin the step is below the tolerances: same histogram with and without it
+    near_on = api.run_config(_off_centre(4, 1500, 0.0, flat_plane=True))
+    near_off = api.run_config(_off_centre(4, 1500, 0.0, flat_plane=False))
+    moved = 0.5 * np.abs(near_on["hist"].astype(np.float64) - near_off["hist"]).sum()
+    assert near_on["counters"]["landed"] == near_off["counters"]["landed"] and moved <= 1e-4 * near_on["counters"]["emitted"]
+
+
 def test_tabulated_extinction():
     """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
     scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an
