@@ -40,16 +40,20 @@ struct DevTable {
 
 // Uniform grid over the telescope array.  Every cell lists the telescopes that a point of the cell
 // can reach, SORTED by a lower-bound key, together with the smallest key of the cell, so that the
-// common "nothing near" case exits after one 4-byte load and a search stops at the first key
-// above the photon's threshold.
+// common "nothing near" case exits after one load (hit grid: one byte per cell, the key quantised
+// downwards, so that the cells under a shower stay in L1) and a search stops at the first key above
+// the photon's threshold.
 //   hit grid: key = dist(cell rectangle, centre_xy) / (r + |z|);  a photon with direction u at a
 //             point of the cell can hit the sphere only if key <= 1/|u_z|
 //   LV2 grid: key = dist(cell rectangle, centre_xy) [m];  the point can be within r/|u_z| + margin
 //             of the centre only if key <= r_max/|u_z| + margin
+constexpr float kHitKeyScale = 64.f;    // quantisation of the hit grid's per-cell smallest key (one byte per cell)
+
 struct DevGrid {
     float x0, y0, inv_cs;
     int nx, ny;
     const float *kmin;              // DEVICE [nx*ny]   smallest key of the cell (+inf: empty)
+    const uint8_t *kq;              // hit grid only, DEVICE [nx*ny]: floor(kmin * kHitKeyScale), 254 at most; 255: empty
     const float2 *kacc;             // LV2 grid only, DEVICE [nx*ny]: (kmin, acc) with acc = min_k(max dist(cell, centre_k) - r_k):
                                     // every point of the cell is within r_k/|u_z| + margin of a centre if acc <= margin
     const int *start;               // DEVICE [nx*ny+1] CSR offsets into items
@@ -114,11 +118,11 @@ struct alignas(16) HotConst {
     float eta_h0, eta_inv_dh, eta_fmax; int eta_kmax;   // n(h) lookup: origin, 1/dh, n_nodes-1, n_nodes-2
     const float *eta; float il1, dil;                   // n(h) nodes; 1/lambda_min, 1/lambda_min - 1/lambda_max
     float box_x0, box_x1, box_y0, box_y1;               // LV2 keep-box
-    float lv2_margin, r_max, grid_min_cos, hit_infl;
+    float lv2_margin, r_max, grid_min_cos, hit_infl_q;  // hit_infl_q = DevRun::hit_infl * kHitKeyScale
     float ray_lambda, ray_k, w, pad0;                   // ray_k = log2(e) / X_R
     float hit_x0, hit_y0, hit_inv_cs; int hit_nx;       // hit grid
     int hit_ny; float hist_inv_cell; int hist_nx, hist_ny;
-    const float *hit_kmin; float *hist;
+    const uint8_t *hit_kq; float *hist;
 };
 
 struct KArgs {

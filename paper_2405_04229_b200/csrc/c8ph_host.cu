@@ -38,6 +38,7 @@ struct c8ph_ctx {
     int *d_g_start[2] = {nullptr, nullptr};
     float2 *d_g_items[2] = {nullptr, nullptr};
     float *d_g_kmin[2] = {nullptr, nullptr};
+    uint8_t *d_g_kq = nullptr;
     float2 *d_g_kacc = nullptr;
     // run scratch
     unsigned long long *d_cursor = nullptr;
@@ -120,6 +121,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
+    dfree(ctx->d_g_kq);
     dfree(ctx->d_g_kacc);
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
@@ -390,6 +392,18 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     g.x0 = (float)x0; g.y0 = (float)y0; g.inv_cs = (float)(1.0 / cs); g.nx = nx; g.ny = ny;
     g.kmin = ctx->d_g_kmin[which]; g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
     g.kacc = nullptr;
+    g.kq = nullptr;
+    if (mode == 0) {
+        // hit pre-test: the smallest key of a cell in 1/64 steps, rounded down (conservative: a false candidate is
+        // rejected by the exact search), one byte per cell so that the cells under the shower stay in L1
+        std::vector<uint8_t> kq(ncell);
+        for (size_t i = 0; i < ncell; ++i)
+            kq[i] = std::isinf(kmin[i]) ? 255 : (uint8_t)std::min(254.0, std::floor((double)kmin[i] * kHitKeyScale));
+        dfree(ctx->d_g_kq);
+        CU(cudaMalloc(&ctx->d_g_kq, ncell));
+        CU(cudaMemcpy(ctx->d_g_kq, kq.data(), ncell, cudaMemcpyHostToDevice));
+        g.kq = ctx->d_g_kq;
+    }
     if (mode == 1) {
         std::vector<float2> ka(ncell);
         for (size_t i = 0; i < ncell; ++i) ka[i] = make_float2(kmin[i], acc[i]);
@@ -615,11 +629,11 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         h.eta_h0 = a.atm.h0; h.eta_inv_dh = a.atm.inv_dh; h.eta_fmax = a.atm.f_max; h.eta_kmax = a.atm.n_nodes - 2;
         h.eta = a.atm.eta; h.il1 = r.il1; h.dil = r.il1 - r.il2;
         h.box_x0 = r.box_x0; h.box_x1 = r.box_x1; h.box_y0 = r.box_y0; h.box_y1 = r.box_y1;
-        h.lv2_margin = r.lv2_margin; h.r_max = a.det.r_max; h.grid_min_cos = a.det.grid_min_cos; h.hit_infl = r.hit_infl;
+        h.lv2_margin = r.lv2_margin; h.r_max = a.det.r_max; h.grid_min_cos = a.det.grid_min_cos; h.hit_infl_q = r.hit_infl * kHitKeyScale;
         h.ray_lambda = a.atm.ray_lambda; h.ray_k = (float)(1.4426950408889634 * (double)a.atm.ray_inv_X); h.w = r.w; h.pad0 = 0.f;
         h.hit_x0 = a.det.hit.x0; h.hit_y0 = a.det.hit.y0; h.hit_inv_cs = a.det.hit.inv_cs; h.hit_nx = a.det.hit.nx;
         h.hit_ny = a.det.hit.ny; h.hist_inv_cell = a.det.hist_inv_cell; h.hist_nx = a.det.hist_nx; h.hist_ny = a.det.hist_ny;
-        h.hit_kmin = a.det.hit.kmin; h.hist = r.out.hist;
+        h.hit_kq = a.det.hit.kq; h.hist = r.out.hist;
     }
     if (emit_smem_bytes(a) > 200 * 1024) return fail(ctx, C8PH_E_ARG, "emit_propagate: atmosphere table too large for shared memory");
     return C8PH_OK;

@@ -1064,14 +1064,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // smallest key <= 1/|u_z| (inflated for the refraction rotation of the direction); the
                     // load is issued before the binning arithmetic so its latency overlaps
                     int cell = -1;
-                    float kmin = CUDART_INF_F;
+                    float kmin = 255.f;                               // quantised smallest key of the cell (255: empty)
                     if (f_tel) {
                         const bool brute = f_hit_brute || !f_grid || -uz < hc.grid_min_cos;
                         if (f_grid) {
                             const int gx = __float2int_rd((xg - hc.hit_x0) * hc.hit_inv_cs), gy = __float2int_rd((yg - hc.hit_y0) * hc.hit_inv_cs);
                             cell = ((unsigned)gx < (unsigned)hc.hit_nx && (unsigned)gy < (unsigned)hc.hit_ny) ? gy * hc.hit_nx + gx : -1;
-                            kmin = __ldg(hc.hit_kmin + max(cell, 0));       // cell -1 (outside): never a candidate
-                            if (cell < 0) kmin = CUDART_INF_F;
+                            kmin = (float)__ldg(hc.hit_kq + max(cell, 0));  // cell -1 (outside): never a candidate
+                            if (cell < 0) kmin = 255.f;
                         }
                         if (brute) cell = -2;
                     }
@@ -1085,7 +1085,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             if (has_hist) atomicAdd(hc.hist + (iy * hc.hist_nx + ix), wgt);
                         }
                     }
-                    const bool cand = cell < -1 || kmin <= -inv_uz * hc.hit_infl;
+                    const bool cand = cell < -1 || (kmin <= -inv_uz * hc.hit_infl_q && kmin < 255.f);
                     if (!cand) {
                         if (f_write != C8PH_WRITE_ALL) break;
                         cell = -1;
