@@ -206,8 +206,19 @@ def run_reference(args):
 
 
 def _apply_variant(cfg: dict, variant: str) -> None:
-    """Optional features (R13-R15) on top of a BASELINE config."""
-    if variant == "dispersion":
+    """Optional features (R13-R15, R17, R19) on top of a BASELINE config."""
+    if variant == "flat":
+        cfg["params"].update(flat_plane=True)
+    elif variant == "extinction":
+        # a tau_v(lambda, h) table filled from the Rayleigh law of the config on a 10 nm grid
+        atm = cfg["atmosphere"]
+        lam = np.arange(240.0, 711.0, 10.0)
+        xv = atm["overburden"].astype(np.float64)
+        h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
+        xg = np.interp(atm["h_obs"], h, xv)
+        tau = np.outer((atm["rayleigh_lambda"] / lam) ** 4 / atm["rayleigh_X"], np.maximum(xg - xv, 0.0))
+        atm.update(ext_lambda0_nm=float(lam[0]), ext_dlambda_nm=10.0, ext_tau_v=tau.astype(np.float32))
+    elif variant == "dispersion":
         cfg["params"].update(disp_b_nm2=5700.0, disp_lambda0_nm=400.0)
     elif variant == "efficiency":
         lam = np.arange(200.0, 801.0, 10.0)
@@ -233,14 +244,14 @@ def run_substep(args):
     trk = {kk: v for kk, v in cfg["segments"].items() if kk != "edep"}
     trk["len"] = rng.uniform(5.0, 400.0, n).astype(np.float32)
     trk["p_GeV"] = (10 ** rng.uniform(-2.0, 1.0, n)).astype(np.float32)
-    ctx = api.setup_context(W.make_config(0, n_segments=1))
+    ctx = api.setup_context(W.make_config(4 if args.substep_ms is not None else 0, n_segments=1))
     dev = {kk: torch.from_numpy(v).cuda() for kk, v in trk.items()}
     B, tol = (2.0e-5, -0.5e-5, -4.3e-5), 0.01
     ms = []
     for i in range(args.warmup + args.steps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        seg, off = ctx.substep_tracks(dev, n, B, tol)
+        seg, off = ctx.substep_tracks(dev, n, B, tol, ms_max_step_m=args.substep_ms)
         e1.record()
         torch.cuda.synchronize()
         if i >= args.warmup:
@@ -248,7 +259,7 @@ def run_substep(args):
     pieces = int(off[-1].item())
     t = float(np.median(ms)) * 1e-3
     print(json.dumps({"metric": "sub-stepped tracks/sec", "value": n / t, "unit": "tracks/s", "pieces_per_s": pieces / t,
-                      "tracks": n, "pieces": pieces, "ms": 1e3 * t, "steps": args.steps, "warmup": args.warmup,
+                      "tracks": n, "pieces": pieces, "multiple_scattering_step_m": args.substep_ms, "ms": 1e3 * t, "steps": args.steps, "warmup": args.warmup,
                       "note": "plan (3 kernels) + 8-byte D2H of the total + allocation + fill (1 kernel), CUDA events",
                       "alg_bytes": 44 * n + 8 * (n + 1) + 40 * pieces, "gpu_launches": 4 * args.steps}), flush=True)
     return 0
@@ -425,10 +436,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--variant", choices=("base", "dispersion", "efficiency", "optics"), default="base",
+    ap.add_argument("--variant", choices=("base", "generic", "flat", "extinction", "dispersion", "efficiency", "optics"), default="base",
                     help="optional features of SURVEY 8(f) switched on (generic kernel variant); the headline is 'base'")
     ap.add_argument("--substep", type=int, default=0, help="time c8ph_substep_plan + c8ph_substep_fill on this many tracks and exit")
+    ap.add_argument("--substep-ms", type=float, default=None, metavar="STEP_M",
+                    help="with --substep: multiple-scattering pieces of at most STEP_M metres (DESIGN.md R18)")
     args = ap.parse_args()
+    if args.variant == "generic":                                     # same switches as 'base' through the generic kernel variant
+        os.environ["C8PH_FORCE_GENERIC"] = "1"
     if args.substep:
         return run_substep(args)
     if args.impl == "reference":

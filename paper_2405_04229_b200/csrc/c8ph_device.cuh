@@ -97,6 +97,7 @@ struct DevRun {
     float disp_b, disp_c0;          // dispersion D(k) = disp_c0 + disp_b k^2, k = 1/lambda [1/nm]; disp_b = 0: off
     double disp_k0sq;               // 1/lambda0^2
     double il1_d, il2_d;            // 1/lambda_min, 1/lambda_max in fp64 (dispersive yield integral)
+    int force_generic;              // validation / timing: use the generic kernel variant even for the production setting
     int flat_plane;                 // spherical model: exact step from the observation sphere to the plane z = 0 (R19)
     int n_eff;                      // detector efficiency table (0: off)
     float eff_l0, eff_inv_dl;       // grid origin [nm], 1 / spacing

@@ -23,6 +23,7 @@ struct c8ph_ctx {
     bool have_atm = false;
     DevAtm atm{};
     bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
+    bool force_generic = false;        // C8PH_FORCE_GENERIC=1: never pick the production-setting kernel variant
     double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
     float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr;
     // table
@@ -100,6 +101,7 @@ extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
     if (!ctx) return fail(nullptr, C8PH_E_NOMEM, "c8ph_create: out of host memory");
     ctx->device = cuda_device;
     { const char *e = getenv("C8PH_FORCE_BRUTE"); ctx->force_brute = e && e[0] == '1'; }
+    { const char *e = getenv("C8PH_FORCE_GENERIC"); ctx->force_generic = e && e[0] == '1'; }
     if ((e = cudaSetDevice(cuda_device)) != cudaSuccess ||
         (e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
@@ -585,6 +587,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         if (p->trace == C8PH_TRACE_STRAIGHT) r.hit_infl = 1.0f + 1e-5f;
     }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
+    r.force_generic = ctx->force_generic ? 1 : 0;
     r.flat_plane = (p->flat_plane && ctx->atm.model == C8PH_ATM_SPHERICAL && p->trace != C8PH_TRACE_STRAIGHT) ? 1 : 0;
     r.n_eff = p->n_eff; r.eff = nullptr;
     r.eff_l0 = p->eff_lambda0_nm; r.eff_inv_dl = p->n_eff > 1 ? 1.0f / p->eff_dlambda_nm : 0.f;

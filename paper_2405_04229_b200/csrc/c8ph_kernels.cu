@@ -1278,7 +1278,7 @@ static bool array_production_setting(const KArgs &a)
     return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && a.atm.n_ext == 0 && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled && !r.flat_plane;
+           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled && !r.flat_plane && !r.force_generic;
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
