@@ -385,9 +385,11 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2,
        WC_CAM, WC_WRITTEN, WC_OVERFLOW, WC_N };
 
 // ================================================================================================
-// SPEC = 1 fixes the run-time switches to the array-detector production setting (LV2 on, Rayleigh
-// roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present):
-// the host picks it when the call matches (launch_emit_propagate); SPEC = 0 reads the switches.
+// SPEC != 0 fixes the run-time switches to the array-detector production setting (LV2 on, Rayleigh
+// roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present) and
+// compiles in the optional features whose bits are set; the host picks the variant when the call
+// matches one that is instantiated (launch_emit_propagate).  SPEC = 0 reads every switch at run time.
+constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32;
 template <int EMIT, int TRACE, bool SPH, int SPEC>
 __global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 2 : kMinBlocks)
 k_emit_propagate(const __grid_constant__ KArgs a)
@@ -458,11 +460,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const int f_trans = SPEC ? (int)C8PH_TRANS_ROULETTE : run.trans;
     const bool f_ray = SPEC ? true : atm.ray_inv_X > 0.f;
     const bool f_aer = SPEC ? false : atm.aer_L > 0.f;
-    const bool f_disp = SPEC ? false : run.disp_b != 0.f;
-    const bool f_eff = SPEC ? false : run.n_eff > 0;
-    const bool f_opt = SPEC ? false : det.opt_enabled != 0;
-    const bool f_ext = SPEC ? false : atm.n_ext > 0;
-    const bool f_flat = (SPEC || !SPH || TRACE == C8PH_TRACE_STRAIGHT) ? false : run.flat_plane != 0;
+    const bool f_disp = SPEC ? (SPEC & kSpecDisp) != 0 : run.disp_b != 0.f;
+    const bool f_eff = SPEC ? (SPEC & kSpecEff) != 0 : run.n_eff > 0;
+    const bool f_opt = SPEC ? (SPEC & kSpecOpt) != 0 : det.opt_enabled != 0;
+    const bool f_ext = SPEC ? (SPEC & kSpecExt) != 0 : atm.n_ext > 0;
+    const bool f_flat = (!SPH || TRACE == C8PH_TRACE_STRAIGHT) ? false : (SPEC ? (SPEC & kSpecFlat) != 0 : run.flat_plane != 0);
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -1270,24 +1272,45 @@ size_t emit_smem_bytes(const KArgs &a)
     return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
 }
 
-// true iff the call matches the switches k_emit_propagate<.., SPEC = 1> is compiled for
-static bool array_production_setting(const KArgs &a)
+// SPEC mask of the call: 0 unless it matches the switches the SPEC != 0 variants are compiled for,
+// else kSpecBase | the optional features that are on
+static int array_production_setting(const KArgs &a)
 {
     const DevRun &r = a.run;
     const DevDet &d = a.det;
-    return r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
-           a.atm.ray_inv_X > 0.f && !(a.atm.aer_L > 0.f) && a.atm.n_ext == 0 && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
+    const bool base = r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
+           (a.atm.ray_inv_X > 0.f || a.atm.n_ext > 0) && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
-           r.out.tel_counts != nullptr && r.disp_b == 0.f && r.n_eff == 0 && !d.opt_enabled && !r.flat_plane && !r.force_generic;
+           r.out.tel_counts != nullptr && !r.force_generic;
+    if (!base) return 0;
+    return kSpecBase | (r.flat_plane ? kSpecFlat : 0) | (a.atm.n_ext > 0 ? kSpecExt : 0) | (r.disp_b != 0.f ? kSpecDisp : 0) |
+           (r.n_eff > 0 ? kSpecEff : 0) | (d.opt_enabled ? kSpecOpt : 0);
 }
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 {
     const size_t smem = emit_smem_bytes(a);
     const bool sph = a.atm.model == C8PH_ATM_SPHERICAL;
-    if (array_production_setting(a))
-        return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, 1>(a, n_sm, smem, st)
-                   : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, 1>(a, n_sm, smem, st);
+    const int spec = array_production_setting(a);
+    if (spec == kSpecBase)
+        return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase>(a, n_sm, smem, st)
+                   : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, kSpecBase>(a, n_sm, smem, st);
+    // production setting + optional features (spherical model): the combinations that are compiled
+#define C8_SPEC(M) \
+    if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, smem, st);
+    C8_SPEC(kSpecFlat)
+    C8_SPEC(kSpecExt)
+    C8_SPEC(kSpecDisp)
+    C8_SPEC(kSpecEff)
+    C8_SPEC(kSpecOpt)
+    C8_SPEC(kSpecEff | kSpecOpt)
+    C8_SPEC(kSpecExt | kSpecEff)
+    C8_SPEC(kSpecExt | kSpecEff | kSpecOpt)
+    C8_SPEC(kSpecDisp | kSpecEff | kSpecOpt)
+    C8_SPEC(kSpecDisp | kSpecExt | kSpecEff | kSpecOpt)
+    C8_SPEC(kSpecFlat | kSpecExt | kSpecEff | kSpecOpt)
+    C8_SPEC(kSpecFlat | kSpecDisp | kSpecExt | kSpecEff | kSpecOpt)
+#undef C8_SPEC
 #define C8_CASE(E, T)                                                             \
     if (a.run.emit == E && a.run.trace == T)                                      \
         return sph ? launch_one<E, T, true, 0>(a, n_sm, smem, st) : launch_one<E, T, false, 0>(a, n_sm, smem, st);
