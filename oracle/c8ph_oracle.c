@@ -904,15 +904,19 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 }
                 if (par->trace != ORC_TRACE_STRAIGHT) {
                     /* arrival direction from the Snell / Bouguer invariant: the direction
-                     * turns in the ray plane by delta = theta_arr - psi_true - theta_z  (R9) */
+                     * turns in the ray plane by delta = theta_arr - psi_true - theta_z  (R9).  The ray is the
+                     * one the n(h) table defines (dd, dt come from it), so the invariant takes the table's
+                     * index at both ends, also when the cone angle is dispersive (R13: the table is valid at
+                     * lambda0 and refraction is not dispersive) */
+                    const double n_ray = 1.0 + eta_e;
                     if (atm->model == 2) {
                         double re = atm->earth_radius + h_e;
                         double a_line = re * sin_zen / Rg;
-                        double a_true = n_e * re * sin_zen / (n_ground * Rg);
+                        double a_true = n_ray * re * sin_zen / (n_ground * Rg);
                         double psi_line = asin(a_line) - acos(cos_zen);
                         delta = asin(a_true) - (psi_line + dd / Rg) - acos(cos_zen);
                     } else {
-                        delta = asin(n_e * sin_zen / n_ground) - acos(cos_zen);
+                        delta = asin(n_ray * sin_zen / n_ground) - acos(cos_zen);
                     }
                 }
                 /* O11 transmission */

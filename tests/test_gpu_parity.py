@@ -612,6 +612,53 @@ def test_flat_observation_plane_far_from_the_origin():
     assert near_on["counters"]["landed"] == near_off["counters"]["landed"] and moved <= 1e-4 * near_on["counters"]["emitted"]
 
 
+def test_compiled_feature_variants_and_the_generic_kernel_agree(monkeypatch):
+    """The "production setting + optional features" calls run kernel variants with the features compiled in (SPEC bit
+    mask); C8PH_FORCE_GENERIC=1 sends the same call through the generic variant that reads every switch at run time.
+    Both against the oracle photon by photon, for the plain production setting, one feature (efficiency), and all five
+    together (flat plane, tabulated extinction, dispersion, efficiency, optics), and the dispersive, flat-plane case with
+    the array 18 km off centre on tracks inclined by 60 degrees (arrival directions to 1e-5 rad).  (The optics stay at
+    the origin: the ray's position on the mirror is formed from fp32 ground coordinates, R15.)"""
+    lam = np.arange(200.0, 801.0, 10.0)
+    eff = dict(eff=(0.85 * np.exp(-0.5 * ((lam - 420.0) / 90.0) ** 2)).astype(np.float32), eff_lambda0_nm=200.0, eff_dlambda_nm=10.0)
+
+    def all_five():
+        cfg = _off_centre(4, 2500, 0.0, None, flat_plane=True, disp_b_nm2=5700.0, disp_lambda0_nm=400.0, **eff)
+        atm = cfg["atmosphere"]
+        xv = atm["overburden"].astype(np.float64)
+        h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
+        lam_e = np.arange(240.0, 711.0, 10.0)
+        tau = (400.0 / lam_e[:, None]) ** 4 * np.maximum(np.interp(atm["h_obs"], h, xv) - xv[None, :], 0.0) / 2970.0
+        atm.update(ext_tau_v=tau.astype(np.float32), ext_lambda0_nm=240.0, ext_dlambda_nm=10.0)
+        cfg["detector"]["tel_xyzr"][:, 3] = 12.0
+        cfg["detector"].update(opt_enabled=True, opt_az_deg=0.0, opt_el_deg=70.0, opt_focal_m=17.0,
+                               opt_mirror_radius_m=8.5, opt_camera_radius_m=0.735)
+        return cfg
+
+    def inclined():
+        return _off_centre(4, 1500, 18000.0, 60.0, flat_plane=True, disp_b_nm2=5700.0, disp_lambda0_nm=400.0)
+
+    def one():
+        cfg = W.make_config(4, n_segments=2500)
+        cfg["params"].update(eff)
+        return cfg
+
+    for make in (lambda: W.make_config(4, n_segments=2500), one, all_five, inclined):
+        cfg = make()
+        ora = O.run(cfg)
+        res = {}
+        for mode in ("compiled", "generic"):
+            monkeypatch.setenv("C8PH_FORCE_GENERIC", "1" if mode == "generic" else "0")
+            ctx = api.setup_context(cfg)                               # the switch is read at c8ph_create
+            res[mode] = api.run_config(cfg, ctx=ctx, photon_capacity=1 << 22)
+            ctx.close()
+            parity.compare(cfg, ora, res[mode])
+        a, b = res["compiled"]["counters"], res["generic"]["counters"]
+        assert a["emitted"] > 1e5 and all(abs(a[k] - b[k]) <= 3 for k in a), (a, b)
+        if make is all_five:
+            assert a["cam_hit"] > 50
+
+
 def test_tabulated_extinction():
     """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
     scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an

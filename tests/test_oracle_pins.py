@@ -973,11 +973,11 @@ def _brute_force_ray_3d(atm, A, U, ds=2.0):
     return out[:, :2], u, out[:, 6] / C_LIGHT
 
 
-def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10):
+def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10, **par):
     """One 1 mm segment (emission point known to 1 mm) at horizontal distance d from the origin; the
     landed photons of the whole oracle run against the 3-D integration of the same rays."""
     cfg = W.make_config(4, n_segments=1)
-    cfg["params"].update(trace=trace, trans="weight", lv1=False, lv2=False, write="all", bunch_weight=2e-5, flat_plane=flat)
+    cfg["params"].update(trace=trace, trans="weight", lv1=False, lv2=False, write="all", bunch_weight=2e-5, flat_plane=flat, **par)
     cfg["detector"]["tel_xyzr"] = np.zeros((0, 4), np.float32)
     if trace != "table":
         cfg["table"] = None
@@ -1017,6 +1017,10 @@ def test_whole_photons_against_3d_ray_integration_flat_plane():
     # the table path takes the same step (bilinear error of the 512 x 256 table on top: < 1 cm, 0.01 ns)
     dpos, dt, ddir, shift, rho = _photons_vs_3d(8.0, 170.0, 60.0, 12000.0, True, "table")
     assert rho > 12000 and dpos < 1e-2 and dt < 1e-2 and ddir < 5e-6
+    # a dispersive cone angle (R13) does not change the ray: the n(h) table (valid at lambda0) refracts, so the
+    # arrival direction still follows the 3-D integration in that medium
+    dpos, dt, ddir, shift, rho = _photons_vs_3d(2.0, 200.0, 60.0, 12000.0, True, "numeric", disp_b_nm2=5700.0, disp_lambda0_nm=400.0)
+    assert dpos < 5e-4 and dt < 1e-3 and ddir < 5e-6
     # without the flat-plane step the same photons are off by centimetres at 19 km from the origin
     dpos, dt, ddir, shift, rho = _photons_vs_3d(2.0, 200.0, 60.0, 12000.0, False, "numeric")
     assert rho > 18000 and 0.05 < dpos < 0.15 and 0.1 < dt < 0.4
