@@ -50,14 +50,14 @@ I_ALG = {
     "landed": 50.0,       # a15 + a14 pre-test: corrected position, telescope-grid cell + smallest key, bin index
     "in_grid": 6.0,       # a15: bin address + RED.ADD.F32
     "tel_hit": 193.0,     # a13/a14/a16: queue push 27 + finish 166 (time, arrival direction, sphere search, record);
-                          # the current finish() has 203 instructions (finer hit grid): the smaller audited count is kept
+                          # the current finish() has 183 instructions (finer hit grid): the smaller audited count is kept
 }
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_emit_propagate launch on the N=1 workload, from the
-# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.836 GB + 5.989 GB).  Reported as
+# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.581 GB + 5.003 GB).  Reported as
 # `roofline.traffic` only when the run is that workload (cfg4, 1e7 segments); otherwise null.
-NCU_TRAFFIC_BYTES_CFG4 = 0.836459008e9 + 5.989187e9
+NCU_TRAFFIC_BYTES_CFG4 = 0.580875008e9 + 5.002906e9
 
 
 def _stage_population(cnt: dict) -> dict:

@@ -608,10 +608,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const long long idx = (long long)base + __popc(wm & ((1u << lane) - 1u));
                     if (idx < run.out.photon_capacity) {
                         uint4 *dst = reinterpret_cast<uint4 *>(run.out.photons + idx);
-                        dst[0] = make_uint4(__float_as_uint(rx_out), __float_as_uint(ry_out), __float_as_uint(uax), __float_as_uint(uay));
-                        dst[1] = make_uint4(__float_as_uint(t_arr), __float_as_uint(rcp_fast(lam_inv)), sc->local,
-                                            ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE));
-                        if (run.out.photon_weight) run.out.photon_weight[idx] = wgt;
+                        // records are written once and never read here: streaming stores (evict first)
+                        __stcs(dst, make_uint4(__float_as_uint(rx_out), __float_as_uint(ry_out), __float_as_uint(uax), __float_as_uint(uay)));
+                        __stcs(dst + 1, make_uint4(__float_as_uint(t_arr), __float_as_uint(rcp_fast(lam_inv)), sc->local,
+                                                   ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE)));
+                        if (run.out.photon_weight) __stcs(run.out.photon_weight + idx, wgt);
                     } else {
                         atomicAdd(&s_cnt[warp][WC_OVERFLOW], 1ull);
                     }
@@ -652,9 +653,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             if (lane < run.segs_per_grab && i < run.n_seg) {
                 SegHot me;
                 SegCold mc;
-                const double Ax = run.seg.x[i], Ay = run.seg.y[i], Az = run.seg.z[i];
-                double Px = run.seg.dx[i], Py = run.seg.dy[i], Pz = run.seg.dz[i];
-                const double L = run.seg.len[i], beta = run.seg.beta[i], t0 = run.seg.t0[i];
+                // inputs are read once: streaming loads, so that they do not push the tables out of L2
+                const double Ax = __ldcs(run.seg.x + i), Ay = __ldcs(run.seg.y + i), Az = __ldcs(run.seg.z + i);
+                double Px = __ldcs(run.seg.dx + i), Py = __ldcs(run.seg.dy + i), Pz = __ldcs(run.seg.dz + i);
+                const double L = __ldcs(run.seg.len + i), beta = __ldcs(run.seg.beta + i), t0 = __ldcs(run.seg.t0 + i);
                 const double pn = 1.0 / sqrt(Px * Px + Py * Py + Pz * Pz);
                 Px *= pn; Py *= pn; Pz *= pn;
                 const unsigned long long gid = (unsigned long long)(run.seg_id_base + i);
@@ -682,7 +684,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // Frank-Tamm, Eq. 2.2-2.4, n at the segment mid height
                     const double eta_mid = eta_lookup_d(atm, h_mid);
                     double n_mid = 1.0 + eta_mid;
-                    const double zq = run.seg.charge[i];
+                    const double zq = __ldcs(run.seg.charge + i);
                     mc.eta_mid = (float)eta_mid;                      // eta at the mid height (dispersive sampling)
                     if (run.disp_b != 0.f) {
                         // dispersion: yield integral over the band with the threshold;
