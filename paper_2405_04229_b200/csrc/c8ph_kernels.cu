@@ -114,7 +114,7 @@ struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
     float fbx, fby;                                   // fractional grid coordinate of the anchor
     int ibx, iby;                                     // integer grid coordinate of the anchor
     float rx, ry, rz;                                 // local vertical at A
-    float Ax, Ay;                                     // start point (non-anchor form)
+    float Ax, Ay;                                     // start point (non-anchor form); anchor form: G - (float)G
     float aimx, aimy, aimz, omc;                      // fluorescence: aim point, 1 - cos(psi)
     float Tg;                                         // anchor clock - t_ref  (or t0 - t_ref)
     uint32_t local;                                   // segment index within the call
@@ -498,17 +498,21 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // (rotation in the ray plane by the Snell / Bouguer invariant), exact sphere search, counters,
     // ballot-compacted record store.  Called warp-converged; `act` marks the lanes that carry a photon.
     auto finish = [&](bool act, float4 q0, float4 q1, float4 q2, float4 q3) {
-        const float xg = q0.x, yg = q0.y, ux = q0.z, uy = q0.w, uz = q1.x, s = q1.y, qw = q1.z, dt = q1.w;
+        const float ux = q0.z, uy = q0.w, uz = q1.x, s = q1.y, qw = q1.z, dt = q1.w;
         const float lam_inv = q2.x, wgt = q2.y, eta_e = q2.z, h_e = q2.w, dd = q3.x, cz = q3.y;
         int cell = __float_as_int(q3.z);
         const uint32_t jslot = __float_as_uint(q3.w);
         int tel = -1;
         float uax = ux, uay = uy, uaz = uz, t_arr = 0.f;
-        float rx_out = xg, ry_out = yg;                       // record position (ground plane, or camera plane with optics)
+        float rx_out = 0.f, ry_out = 0.f;                     // record position (ground plane, or camera plane with optics)
         bool opt_hit = false;
         const SegSlot *sl = g_slot + (jslot & 31u);
         const SegHot *sh = &sl->h;
         const SegCold *sc = &sl->c;
+        // with optics the entry carries the offset from the segment anchor, so that the ray's position on the
+        // mirror does not go through an fp32 ground coordinate (0.24 mm at 3 km is 1.4e-5 rad after the mirror)
+        const float xg = (f_opt && act) ? sh->Gx + q0.x : q0.x, yg = (f_opt && act) ? sh->Gy + q0.y : q0.y;
+        rx_out = xg; ry_out = yg;
         if (act) {
             // a13: arrival time relative to t_ref
             if (sh->anchor) {
@@ -539,7 +543,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // pointing axis (vertex at centre - (f/2) w), reflection, camera disc at z = f
                     const float4 tc = __ldg(det.tel + tel);
                     const float f = det.opt_f, hf = 0.5f * f;
-                    const float px = xg - (tc.x - hf * det.opt_w[0]), py = yg - (tc.y - hf * det.opt_w[1]), pz = -(tc.z - hf * det.opt_w[2]);
+                    const float lox = sh->anchor ? sc->Ax : 0.f, loy = sh->anchor ? sc->Ay : 0.f;
+                    const float px = (sh->Gx - tc.x) + (q0.x + lox) + hf * det.opt_w[0];
+                    const float py = (sh->Gy - tc.y) + (q0.y + loy) + hf * det.opt_w[1], pz = -(tc.z - hf * det.opt_w[2]);
                     const float a0 = px * det.opt_r[0] + py * det.opt_r[1] + pz * det.opt_r[2];
                     const float b0 = px * det.opt_u[0] + py * det.opt_u[1] + pz * det.opt_u[2];
                     const float z0 = px * det.opt_w[0] + py * det.opt_w[1] + pz * det.opt_w[2];
@@ -783,6 +789,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         const double azp = Az / Pz;
                         const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
                         me.Gx = (float)Gx; me.Gy = (float)Gy; me.AzP = (float)azp;
+                        // anchor form: Ax, Ay are free and carry what fp32 loses of the anchor (last-mile optics)
+                        mc.Ax = (float)(Gx - (double)me.Gx); mc.Ay = (float)(Gy - (double)me.Gy);
                         mc.Tg = (float)(t0 - azp / kC - det.t_ref);
                         if (has_grid_geom) {
                             const double bx = (Gx - (double)det.hist_x0) / (double)det.hist_cell;
@@ -1103,7 +1111,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])), "r"(__popc(am)) : "memory");
                     qb = __shfl_sync(am, qb, leader);
                     float4 *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
-                    e[0] = make_float4(xg, yg, ux, uy);
+                    e[0] = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
                     e[1] = make_float4(uz, s, q * wz, dt);
                     e[2] = make_float4(lam_inv, wgt, eta_e, h_e);
                     e[3] = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));

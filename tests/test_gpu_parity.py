@@ -616,14 +616,14 @@ def test_compiled_feature_variants_and_the_generic_kernel_agree(monkeypatch):
     """The "production setting + optional features" calls run kernel variants with the features compiled in (SPEC bit
     mask); C8PH_FORCE_GENERIC=1 sends the same call through the generic variant that reads every switch at run time.
     Both against the oracle photon by photon, for the plain production setting, one feature (efficiency), and all five
-    together (flat plane, tabulated extinction, dispersion, efficiency, optics), and the dispersive, flat-plane case with
-    the array 18 km off centre on tracks inclined by 60 degrees (arrival directions to 1e-5 rad).  (The optics stay at
-    the origin: the ray's position on the mirror is formed from fp32 ground coordinates, R15.)"""
+    together (flat plane, tabulated extinction, dispersion, efficiency, optics) with the array 18 km off centre (the
+    reflected directions keep 1e-5 rad there because the mirror coordinates are formed relative to the segment
+    anchor, not from fp32 ground coordinates), and the dispersive, flat-plane case on tracks inclined by 60 degrees."""
     lam = np.arange(200.0, 801.0, 10.0)
     eff = dict(eff=(0.85 * np.exp(-0.5 * ((lam - 420.0) / 90.0) ** 2)).astype(np.float32), eff_lambda0_nm=200.0, eff_dlambda_nm=10.0)
 
     def all_five():
-        cfg = _off_centre(4, 2500, 0.0, None, flat_plane=True, disp_b_nm2=5700.0, disp_lambda0_nm=400.0, **eff)
+        cfg = _off_centre(4, 2500, 18000.0, None, flat_plane=True, disp_b_nm2=5700.0, disp_lambda0_nm=400.0, **eff)
         atm = cfg["atmosphere"]
         xv = atm["overburden"].astype(np.float64)
         h = atm["h0"] + atm["dh"] * np.arange(atm["n_nodes"])
