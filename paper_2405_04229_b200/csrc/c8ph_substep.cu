@@ -1,6 +1,6 @@
 // c8ph_substep.cu — sub-stepping of particle tracks along the magnetically deflected path
 // (thesis sec. 4.2.1): the step before the hot path.  Three small kernels plan the pieces
-// (count per track + exclusive prefix sum), one fills them (one thread per piece).  fp64: the pieces
+// (count per track + exclusive prefix sum), one fills them (a warp expands 32 tracks cooperatively).  fp64: the pieces
 // must reproduce km-scale positions to well below the 15 cm resolution the thesis quotes.
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -143,31 +143,52 @@ __global__ void __launch_bounds__(kScanThreads) k_substep_add_blocks(const __gri
     if (i == 0) a.offsets[0] = 0;
 }
 
-// fill: one thread per piece (grid-stride over offsets[n] pieces), owner track by binary search
+// fill: a warp takes 32 consecutive tracks and expands them cooperatively - lane l writes the pieces
+// base + l, base + l + 32, ... of the group (coalesced), the owner track of a piece by a five-step
+// search over the group's 32 start offsets held one per lane (shuffles, no global binary search)
 __global__ void __launch_bounds__(256) k_substep_fill(const __grid_constant__ SubstepArgs a)
 {
-    const long long total = a.offsets[a.n];
-    for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long long)gridDim.x * blockDim.x) {
-        long long lo = 0, hi = a.n;                                    // largest i with offsets[i] <= g
-        while (hi - lo > 1) {
-            const long long mid = (lo + hi) >> 1;
-            if (a.offsets[mid] <= g) lo = mid; else hi = mid;
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31;
+    const long long n_groups = (a.n + 31) >> 5;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long grp = warp0; grp < n_groups; grp += n_warps) {
+        const long long i0 = grp << 5;
+        const long long base = a.offsets[i0];
+        const long long i_me = i0 + lane < a.n ? i0 + lane : a.n;
+        const long long i_end = i0 + 32 < a.n ? i0 + 32 : a.n;
+        const int rel = (int)(a.offsets[i_me] - base);                 // start of my track within the group (<= 32 * max_sub)
+        const int total = (int)(a.offsets[i_end] - base);              // lanes beyond the last track hold `total`
+        for (int p0 = 0; p0 < total; p0 += 32) {
+            __syncwarp();                                              // lanes that skipped the tail of the last pass rejoin
+            const int p = p0 + lane;
+            int lo = 0;                                                // largest t with rel[t] <= p
+#pragma unroll
+            for (int step = 16; step >= 1; step >>= 1) {
+                const int v = __shfl_sync(FULL, rel, (lo + step) & 31);
+                if (v <= p) lo += step;
+            }
+            const int r0 = __shfl_sync(FULL, rel, lo);
+            int r1 = __shfl_sync(FULL, rel, (lo + 1) & 31);
+            if (lo == 31) r1 = total;
+            if (p >= total) continue;
+            const Helix h = helix_of(a, i0 + lo);
+            const int m = r1 - r0, j = p - r0;
+            const double s0 = h.L * (double)j / (double)m, s1 = h.L * (double)(j + 1) / (double)m;
+            double X0[3], X1[3];
+            point_on(h, s0, X0);
+            point_on(h, s1, X1);
+            const double d[3] = {X1[0] - X0[0], X1[1] - X0[1], X1[2] - X0[2]};
+            const double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            const long long g = base + p;
+            a.out.x[g] = (float)X0[0]; a.out.y[g] = (float)X0[1]; a.out.z[g] = (float)X0[2];
+            a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            a.out.len[g] = (float)len;
+            a.out.beta[g] = (float)h.beta;
+            a.out.t0[g] = (float)(h.t0 + s0 / (h.beta * 0.299792458));
+            a.out.charge[g] = (float)h.charge;
+            if (a.out.edep) a.out.edep[g] = 0.f;
         }
-        const Helix h = helix_of(a, lo);
-        const long long m = a.offsets[lo + 1] - a.offsets[lo], j = g - a.offsets[lo];
-        const double s0 = h.L * (double)j / (double)m, s1 = h.L * (double)(j + 1) / (double)m;
-        double X0[3], X1[3];
-        point_on(h, s0, X0);
-        point_on(h, s1, X1);
-        const double d[3] = {X1[0] - X0[0], X1[1] - X0[1], X1[2] - X0[2]};
-        const double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-        a.out.x[g] = (float)X0[0]; a.out.y[g] = (float)X0[1]; a.out.z[g] = (float)X0[2];
-        a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
-        a.out.len[g] = (float)len;
-        a.out.beta[g] = (float)h.beta;
-        a.out.t0[g] = (float)(h.t0 + s0 / (h.beta * 0.299792458));
-        a.out.charge[g] = (float)h.charge;
-        if (a.out.edep) a.out.edep[g] = 0.f;
     }
 }
 

@@ -482,7 +482,7 @@ def test_last_mile_optics():
 
 def test_substepping_matches_the_oracle_and_feeds_the_hot_path():
     """Row f2 (thesis sec. 4.2.1): tracks cut into chords of the Lorentz helix on the device (plan =
-    count + prefix sum, fill = one thread per piece) against the oracle: piece counts bit-exact,
+    count + prefix sum, fill = a warp per 32 tracks) against the oracle: piece counts bit-exact,
     positions to fp32 storage, directions 1e-6, lengths 1e-5 relative, clocks 1e-3 ns; the segments then
     run through c8ph_emit_propagate and agree with the oracle run on the oracle's segments."""
     rng = np.random.default_rng(21)
