@@ -226,6 +226,31 @@ def test_photon_buffer_overflow_is_counted_not_silent():
     assert np.array_equal(small["hist"], ref["hist"])                 # overflowing photons are still binned
 
 
+def test_bunch_count_cap_per_segment_is_counted_not_silent():
+    """Maximum size of one segment (R1): the record key holds 18 bits of photon index, so a segment emits at
+    most C8PH_MAX_BUNCHES_PER_SEGMENT - 1 = 262143 bunches; a segment asking for more (charge 30: 293365) is clipped,
+    counted in `clipped`, and the photons it does emit are the oracle's photons of the same indices."""
+    cfg = W.make_config(0, n_segments=3)
+    cfg["segments"]["charge"][1] = 30.0
+    ora = O.run(cfg)
+    assert ora["n_bunch"][1] > 262143 > ora["n_bunch"][0]
+    gpu = api.run_config(cfg, photon_capacity=1 << 19)
+    c = gpu["counters"]
+    cap = 262143
+    assert c["clipped"] == 1 and c["overflow"] == 0
+    assert c["emitted"] == ora["n_bunch"][0] + cap + ora["n_bunch"][2] == c["written"]
+    g = gpu["photons"]
+    j = (g["j_tel"] >> 14).astype(np.int64)
+    mid = g["seg"] == 1
+    assert mid.sum() == cap and np.array_equal(np.sort(j[mid]), np.arange(cap))
+    o = ora["photons"]
+    o = o[(o["seg"] == 1) & (o["j"] < cap)]
+    o = o[np.argsort(o["j"])]
+    gm = g[mid][np.argsort(j[mid])]
+    assert np.abs(gm["x"] - o["x"]).max() < 0.05 and np.abs(gm["y"] - o["y"]).max() < 0.05
+    assert np.allclose(gm["lambda_nm"], o["lambda_nm"], rtol=2e-6)
+
+
 def test_host_buffer_entry_point_matches_device_path():
     cfg = W.make_config(4, n_segments=1500)
     ctx = api.setup_context(cfg)
