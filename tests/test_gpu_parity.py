@@ -330,6 +330,40 @@ def test_cfg4_full_size_sampled_windows_and_invariants():
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
 
 
+def test_cfg1_full_size_sampled_windows_and_invariants():
+    """BASELINE configs[1] at its full 1e5 segments (planar atmosphere, per-photon layered sum, weight mode,
+    every photon written: 8.1e6 records): whole-run identities plus photon-by-photon comparison with the
+    oracle on sampled segment windows."""
+    n = W.FULL_SEGMENTS[1]
+    cfg = W.make_config(1)
+    ctx = api.setup_context(cfg)
+    seg = api.segments_to_device(cfg["segments"])
+    out = api.alloc_device_outputs(ctx, 12_000_000, True)
+    ctx.emit_propagate(seg, n, 0, cfg["params"], cfg["seed"], out)
+    torch.cuda.synchronize()
+    cnt = {k: int(v) for k, v in zip(api.COUNTER_NAMES, out["counters"].cpu().numpy())}
+    assert cnt["segments"] == n and cnt["overflow"] == 0 and cnt["clipped"] == 0
+    assert cnt["emitted"] == cnt["upgoing"] + cnt["lv2"] + cnt["table_range"] + cnt["roulette"] + cnt["landed"]
+    assert cnt["emitted"] > 5e6 and cnt["written"] == cnt["landed"] and cnt["roulette"] == 0
+    wsum = out["photon_weight"][:cnt["written"]].double().sum().item()
+    assert 0.0 < out["hist"].double().sum().item() <= wsum * (1 + 1e-6)       # the grid holds part of the landed weight
+    rec_all = out["photons"][:cnt["written"]]
+    ph_seg = rec_all.view(torch.int32)[:, 6]
+    for lo, hi in ((0, 600), (50_017, 50_640), (n - 500, n)):
+        m = (ph_seg >= lo) & (ph_seg < hi)
+        rec = rec_all[m].cpu().numpy().view(api.PHOTON_DTYPE).reshape(-1).copy()
+        rec["seg"] -= lo
+        sub = copy.deepcopy(cfg)
+        sub["segments"] = W.slice_segments(cfg["segments"], lo, hi)
+        sub["seg_id_base"] = lo
+        ora = O.run(sub)
+        win = api.run_config(sub, ctx=ctx)
+        parity.compare(sub, ora, win)
+        k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
+        k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
+        assert len(rec) > 2e4 and np.array_equal(rec[k1], win["photons"][k2])   # full-size run == window run, bit for bit
+
+
 def test_cfg3_full_size_against_the_whole_oracle():
     """BASELINE configs[3] at its full 1e6 segments (forced-cone fluorescence: ~1.7e5 photons, which
     the oracle runs completely): counters, camera histogram and every photon record."""
