@@ -23,6 +23,8 @@ struct DevAtm {
     float ray_inv_X;        // 1 / X_R, 0 = Rayleigh off
     float ray_lambda;       // lambda_R [nm]
     float aer_L, aer_H, aer_lambda, aer_angstrom;
+    const float *aexp;      // DEVICE [n_pad] aerosol column A(h_k) = (H/L) exp(-h_k/H) at the nodes (zeros without aerosol)
+    float aer_HL, aer_invH, aer_Ag;   // H/L, 1/H, A(h_obs)
     int n_ext;              // tabulated extinction: wavelength nodes (0: off)
     float ext_l0, ext_inv_dl;
     const float *ext;       // DEVICE [n_ext][n_nodes] vertical optical depth obs level -> node

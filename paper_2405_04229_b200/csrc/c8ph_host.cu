@@ -25,7 +25,7 @@ struct c8ph_ctx {
     bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
     bool force_generic = false;        // C8PH_FORCE_GENERIC=1: never pick the production-setting kernel variant
     double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
-    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr;
+    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr, *d_aexp = nullptr;
     // table
     bool have_table = false;
     DevTable tab{};
@@ -120,7 +120,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
 {
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
-    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_g_kq);
@@ -197,6 +197,20 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
     a.ray_lambda = d->rayleigh_lambda_nm;
     a.aer_L = d->aer_L_m; a.aer_H = d->aer_H_m; a.aer_lambda = d->aer_lambda_nm; a.aer_angstrom = d->aer_angstrom;
     if (a.aer_L > 0.f && !(a.aer_H > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: aerosol scale height");
+    {
+        // aerosol column at the nodes for the per-photon layered sum: A(h) = (H/L) exp(-h/H)
+        std::vector<float> aexp(n_pad, 0.f);
+        a.aer_HL = a.aer_invH = a.aer_Ag = 0.f;
+        if (a.aer_L > 0.f) {
+            const double H = a.aer_H, HL = (double)a.aer_H / (double)a.aer_L;
+            for (int k = 0; k < n; ++k) aexp[k] = (float)(HL * std::exp(-(h0 + dh * k) / H));
+            a.aer_HL = (float)HL; a.aer_invH = (float)(1.0 / H); a.aer_Ag = (float)(HL * std::exp(-(double)d->h_obs_m / H));
+        }
+        dfree(ctx->d_aexp);
+        CU(cudaMalloc(&ctx->d_aexp, bytes));
+        CU(cudaMemcpy(ctx->d_aexp, aexp.data(), bytes, cudaMemcpyHostToDevice));
+        a.aexp = ctx->d_aexp;
+    }
     a.xv_g = (float)lerp_table(xv, h0, dh, d->h_obs_m);
     a.n_ext = 0; a.ext = nullptr; a.ext_l0 = 0.f; a.ext_inv_dl = 0.f;
     dfree(ctx->d_ext);

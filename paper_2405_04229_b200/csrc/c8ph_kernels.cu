@@ -29,6 +29,7 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <cstdint>
+#include <type_traits>
 #include "c8ph_device.cuh"
 #include "c8ph_philox.cuh"
 
@@ -410,7 +411,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // ---- shared memory carve-up: [n(h) tables] | per-warp candidate queue (SoA, kQueue entries)
     float *s_eta = reinterpret_cast<float *>(smem_raw);
     float *s_dxv = s_eta + (STAGED ? atm.n_pad : 0);
-    float *s_end = s_dxv + (STAGED ? atm.n_pad : 0);
+    float *s_aexp = s_dxv + (STAGED ? atm.n_pad : 0);       // aerosol column A(h_k) = (H/L) exp(-h_k/H), staged only with aerosol
+    const bool aer_staged = STAGED && atm.aer_L > 0.f;
+    float *s_end = s_aexp + (aer_staged ? atm.n_pad : 0);
     float4 *s_q = reinterpret_cast<float4 *>(s_end) + warp * (kQueue * 4);   // s_q[slot * 4 + part]
     __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
@@ -423,9 +426,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         if (threadIdx.x == 0) {
             mbar_init(&s_bar, 1);
             const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
-            mbar_expect_tx(&s_bar, bytes * 2u);
+            mbar_expect_tx(&s_bar, bytes * (aer_staged ? 3u : 2u));
             bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
             bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
+            if (aer_staged) bulk_g2s(s_aexp, atm.aexp, bytes, &s_bar);
         }
         __syncthreads();
         mbar_wait(&s_bar, 0);
@@ -977,9 +981,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         const float fg = fminf(fmaxf(((float)atm.h_obs - atm.h0) * atm.inv_dh, 0.f), (float)(atm.n_nodes - 1));
                         const int ke = min((int)fe, atm.n_nodes - 2), kg = min((int)fg, atm.n_nodes - 2);
                         const float fre = fe - (float)ke, frg = fg - (float)kg;
-                        float aX = 0.f, aT = 0.f, aS = 0.f;
+                        float aX = 0.f, aT = 0.f, aS = 0.f, aA = 0.f;
                         bool ok = cz > 0.f;
-                        auto layer = [&](float eta_l, float thick, float dxv_l) {
+                        // da = A(layer bottom) - A(layer top), A(h) = (H/L) exp(-h/H): the layer's vertical aerosol depth
+                        auto layer = [&](auto aer, float eta_l, float thick, float dxv_l, float da) {
                             const float n_l = 1.f + eta_l;
                             const float ql = fmaf(n_l, n_l, -K * K);
                             ok = ok && (ql > 0.f);
@@ -989,18 +994,29 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             aX = fmaf(thick * K, dr, aX);
                             aT = fmaf(thick, fmaf(n_l * n_l, dr, r_e * (fmaf(eta_l, eta_l, 2.f * eta_l) - eta_e)), aT);
                             aS = fmaf(dxv_l * n_l, r_l, aS);
+                            if (decltype(aer)::value) aA = fmaf(da * n_l, r_l, aA);
                         };
-                        if (ke == kg) {
-                            const float fm = 0.5f * (fre + frg);
-                            layer(fmaf(fm, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), (fre - frg) * atm.dh, (fre - frg) * s_dxv[ke]);
-                        } else {
-                            if (fre > 0.f)
-                                layer(fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke]);
-                            for (int k = ke - 1; k > kg; --k) layer(0.5f * (s_eta[k] + s_eta[k + 1]), atm.dh, s_dxv[k]);   // n at the layer mid height
-                            layer(fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg]);
-                        }
+                        auto walk = [&](auto aer) {
+                            float Ae = 0.f, Ag = 0.f;                   // A at the emission height and at the observation level
+                            if (decltype(aer)::value) {
+                                Ae = atm.aer_HL * exp2_fast(-1.4426950408889634f * h_e * atm.aer_invH);
+                                Ag = atm.aer_Ag;
+                            }
+                            auto A = [&](int k) { return decltype(aer)::value ? s_aexp[k] : 0.f; };
+                            if (ke == kg) {
+                                const float fm = 0.5f * (fre + frg);
+                                layer(aer, fmaf(fm, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), (fre - frg) * atm.dh, (fre - frg) * s_dxv[ke], Ag - Ae);
+                            } else {
+                                if (fre > 0.f)
+                                    layer(aer, fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]), fre * atm.dh, fre * s_dxv[ke], A(ke) - Ae);
+                                for (int k = ke - 1; k > kg; --k)             // n at the layer mid height
+                                    layer(aer, 0.5f * (s_eta[k] + s_eta[k + 1]), atm.dh, s_dxv[k], A(k) - A(k + 1));
+                                layer(aer, fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg], Ag - A(kg + 1));
+                            }
+                        };
+                        if (aer_staged) walk(std::true_type{}); else walk(std::false_type{});
                         if (!ok) { pkB += 1u; break; }
-                        dd = aX; dt = aT * kInvC; Xs = aS;
+                        dd = aX; dt = aT * kInvC; Xs = aS; ta = aA;
                     }
                     float wgt = hc.w;
                     if (f_trans != C8PH_TRANS_OFF) {
@@ -1278,7 +1294,7 @@ void segment_slot_pointers(void *base, int n_sm, DevRun &run)
 
 size_t emit_smem_bytes(const KArgs &a)
 {
-    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * 2u : 0u;
+    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
     return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
 }
 

@@ -718,6 +718,37 @@ def test_compiled_feature_variants_and_the_generic_kernel_agree(monkeypatch):
             assert a["cam_hit"] > 50
 
 
+@pytest.mark.parametrize("trial", range(16))
+def test_random_switch_combinations(trial):
+    """The generic kernel variants under seeded random combinations of the run-time switches (filters, transmission
+    mode, write mode, bunch weight, margins, aerosol, trace method, detectors present or not), device against
+    oracle photon by photon: combinations that none of the BASELINE configs uses."""
+    rng = np.random.default_rng(4200 + trial)
+    k = int(rng.choice([0, 1, 2, 4]))
+    cfg = W.make_config(k, n_segments={0: 400, 1: 250, 2: 8000, 4: 1500}[k])
+    par, det, atm = cfg["params"], cfg["detector"], cfg["atmosphere"]
+    par["lv1"], par["lv2"] = bool(rng.integers(2)), bool(rng.integers(2))
+    par["trans"] = str(rng.choice(["off", "weight", "roulette"]))
+    par["write"] = str(rng.choice(["all", "tel", "none"]))
+    par["bunch_weight"] = float(rng.choice([0.5, 1.0, 2.5]))
+    par["lv2_margin_m"] = float(rng.uniform(0.0, 40.0))
+    par["lv1_margin_rad"] = float(rng.uniform(0.0, 0.03))
+    if k != 0 and rng.integers(2):
+        atm["aer_L"] = 15000.0                                          # aerosol extinction on
+    if k in (2, 4) and rng.integers(3) == 0:
+        par["trace"], cfg["table"] = "straight", None
+    if k == 1 and rng.integers(3) == 0:
+        par["trace"] = "straight"
+    if len(det["tel_xyzr"]) and rng.integers(4) == 0:
+        det["tel_xyzr"] = np.zeros((0, 4), np.float32)                  # no telescopes
+    elif det["hist_nx"] > 0 and rng.integers(4) == 0:
+        det["hist_nx"] = det["hist_ny"] = 0                             # no ground grid
+    if k == 4 and rng.integers(3) == 0:
+        par["flat_plane"] = True
+    ora, gpu, rep = _both(cfg)
+    assert gpu["counters"]["emitted"] > 2000
+
+
 def test_tabulated_extinction():
     """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
     scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an
