@@ -284,7 +284,10 @@ __device__ __forceinline__ void sphere_test(const DevDet &det, int k, float x, f
     const float4 t = __ldg(det.tel + k);
     const float dx = t.x - x, dy = t.y - y, dz = t.z;
     const float du = dx * ux + dy * uy + dz * uz;
-    const float m2 = dx * dx + dy * dy + dz * dz - du * du;
+    // squared miss distance from the perpendicular part of (centre - point): |d|^2 - du^2 cancels when a grazing ray
+    // meets the plane kilometres from the telescope (10 cm at 2 km in fp32)
+    const float qx = fmaf(-du, ux, dx), qy = fmaf(-du, uy, dy), qz = fmaf(-du, uz, dz);
+    const float m2 = qx * qx + qy * qy + qz * qz;
     const float r2 = t.w * t.w;
     if (m2 <= r2) {
         const float s_in = du - sqrtf(r2 - m2);
