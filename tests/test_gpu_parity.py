@@ -760,6 +760,48 @@ def test_random_switch_combinations(trial):
     assert gpu["counters"]["emitted"] > 2000
 
 
+@pytest.mark.parametrize("trial", range(10))
+def test_random_geometry_tables_ids_and_entry_points(trial):
+    """Seeded random variations of what the BASELINE configs keep fixed: seed and 40-bit segment id base, observation
+    level, correction-table dimensions and limits, histogram geometry, irregular telescope arrays with radii and
+    altitudes, margins, weights - through the device and the host entry point, against the oracle photon by photon."""
+    rng = np.random.default_rng(777000 + trial)
+    k = int(rng.choice([0, 1, 2, 4, 4]))
+    cfg = W.make_config(k, n_segments={0: 400, 1: 250, 2: 8000, 4: 1500}[k])
+    par, det, atm = cfg["params"], cfg["detector"], cfg["atmosphere"]
+    cfg["seed"], cfg["seg_id_base"] = int(rng.integers(1, 2 ** 62)), int(rng.integers(0, 2 ** 40))
+    if k in (1, 2, 4) and rng.integers(2):
+        atm["h_obs"] = float(rng.choice([0.0, 800.0, 1800.0, 2200.0]))
+    if cfg.get("table") is not None and rng.integers(2):
+        cfg["table"] = dict(n_h=int(rng.choice([128, 300, 512])), n_zen=int(rng.choice([64, 200, 256])),
+                            h_max=float(rng.choice([60000.0, 100000.0])), zen_max_deg=float(rng.choice([80.0, 89.0])))
+    if det["hist_nx"] > 0 and rng.integers(2):
+        cell, nx, ny = float(rng.choice([0.5, 1.0, 2.5, 7.0])), int(rng.integers(50, 700)), int(rng.integers(50, 700))
+        det.update(hist_cell=cell, hist_nx=nx, hist_ny=ny, hist_x0=float(-0.5 * nx * cell + rng.uniform(-100, 100)),
+                   hist_y0=float(-0.5 * ny * cell + rng.uniform(-100, 100)))
+    if len(det["tel_xyzr"]) and rng.integers(2):
+        t = det["tel_xyzr"].copy()
+        t[:, 3] = rng.uniform(2.0, 9.0, len(t)).astype(np.float32)
+        t[:, 2] = rng.uniform(-3.0, 3.0, len(t)).astype(np.float32)
+        t[:, 0] += rng.uniform(-8, 8, len(t)).astype(np.float32)
+        t[:, 1] += rng.uniform(-8, 8, len(t)).astype(np.float32)
+        det["tel_xyzr"] = t
+    par["lv1"], par["lv2"] = bool(rng.integers(2)), True
+    par["trans"] = str(rng.choice(["off", "weight", "roulette"]))
+    par["write"] = str(rng.choice(["tel", "none", "tel"]))
+    par["bunch_weight"] = float(rng.choice([0.5, 1.0, 2.5]))
+    par["lv2_margin_m"] = float(rng.uniform(0.0, 60.0))
+    ora = O.run(cfg)
+    if rng.integers(2):
+        ctx = api.setup_context(cfg)
+        gpu = ctx.emit_propagate_host(cfg["segments"], len(cfg["segments"]["x"]), cfg["seg_id_base"], par, cfg["seed"],
+                                      photon_capacity=1 << 22, want_weight=True)
+    else:
+        gpu = api.run_config(cfg, photon_capacity=1 << 22)
+    parity.compare(cfg, ora, gpu)
+    assert gpu["counters"]["emitted"] > 2000
+
+
 def test_tabulated_extinction():
     """Row f4: transmission from a tau_v(lambda, h) table (MODTRAN-type, thesis Fig. 4.7a) with air-mass
     scaling instead of the analytic laws: device against oracle on the same table (Rayleigh + an
