@@ -623,6 +623,38 @@ def test_multiple_scattering_substeps_match_the_oracle():
     assert e.value.code == api.E_STATE
 
 
+@pytest.mark.parametrize("trial", range(8))
+def test_random_substepping_inputs(trial):
+    """Sub-stepping under seeded random inputs: track counts around the warp / scan-block sizes (1, 31, 33, 700, 2049),
+    neutral and doubly charged particles, zero and random fields, tolerances, piece caps, with and without multiple
+    scattering (steps 0 = no cap, 10, 50 m), 40-bit id bases - piece counts bit-exact, pieces to fp32 storage."""
+    rng = np.random.default_rng(31000 + trial)
+    n, k = int(rng.choice([1, 31, 33, 700, 2049])), int(rng.choice([1, 4]))
+    cfg = W.make_config(k, n_segments=n)
+    trk = {kk: v.copy() for kk, v in cfg["segments"].items() if kk != "edep"}
+    trk["len"] = rng.uniform(0.5, 900.0, n).astype(np.float32)
+    trk["p_GeV"] = (10 ** rng.uniform(-2.3, 1.5, n)).astype(np.float32)
+    trk["charge"] = rng.choice([-1.0, 1.0, 2.0, 0.0], n).astype(np.float32)
+    B = tuple(float(x) for x in rng.normal(0, 3e-5, 3)) if rng.integers(4) else (0.0, 0.0, 0.0)
+    tol, max_sub = float(rng.choice([0.001, 0.01, 0.1])), int(rng.choice([8, 64, 4096]))
+    ms = None if rng.integers(2) else float(rng.choice([0.0, 10.0, 50.0]))
+    seed, base = int(rng.integers(1, 2 ** 60)), int(rng.integers(0, 2 ** 40))
+    if ms is None:
+        want = O.substep_tracks(trk, B, tol, max_sub)
+    else:
+        want = O.substep_tracks_ms(cfg["atmosphere"], trk, B, tol, ms, seed=seed, track_id_base=base, max_sub=max_sub)
+    ctx = api.setup_context(cfg)
+    dev = {kk: torch.from_numpy(v).cuda() for kk, v in trk.items()}
+    seg, off = ctx.substep_tracks(dev, n, B, tol, max_sub, ms_max_step_m=ms, seed=seed, track_id_base=base)
+    assert np.array_equal(off.cpu().numpy(), want["offsets"])
+    got, ws = {kk: v.cpu().numpy() for kk, v in seg.items()}, want["segments"]
+    for kk in ("x", "y", "z"):
+        assert np.abs(got[kk].astype(np.float64) - ws[kk]).max() <= 2 * np.spacing(np.float32(np.abs(ws[kk]).max())) + 2e-4
+    for kk in ("dx", "dy", "dz"):
+        assert np.abs(got[kk] - ws[kk]).max() < 2e-6
+    assert np.allclose(got["len"], ws["len"], rtol=2e-5, atol=1e-6) and np.allclose(got["t0"], ws["t0"], rtol=0, atol=6e-3)
+
+
 def _off_centre(k, n, shift_m, zen_deg=None, **par):
     """cfg k with segments, ground grid and telescopes moved rigidly by shift_m along x: the array sits that far
     from the point where the plane z = 0 touches the observation sphere.  zen_deg: the segments become inclined
