@@ -116,7 +116,7 @@ struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
     int ibx, iby;                                     // integer grid coordinate of the anchor
     float rx, ry, rz;                                 // local vertical at A
     float Ax, Ay;                                     // start point (non-anchor form); anchor form: G - (float)G
-    float aimx, aimy, aimz, omc;                      // fluorescence: aim point, 1 - cos(psi)
+    float aimx, aimy, aimz, omc;                      // fluorescence: aim point - A, 1 - cos(psi)
     float Tg;                                         // anchor clock - t_ref  (or t0 - t_ref)
     uint32_t local;                                   // segment index within the call
     float eta_mid;                                    // refractivity at the segment mid height (dispersion)
@@ -759,7 +759,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             }
                         }
                     }
-                    mc.aimx = (float)aimx; mc.aimy = (float)aimy; mc.aimz = t0v.z;
+                    // relative to the start point, in fp64: the cone axis must not go through fp32 ground coordinates
+                    // (2 mm at 20 km is 2e-4 rad for an emission point 10 m from the telescope)
+                    mc.aimx = (float)(aimx - Ax); mc.aimy = (float)(aimy - Ay); mc.aimz = (float)((double)t0v.z - Az);
                     const double rho = run.aim_factor * (double)t0v.w;
                     const double sp = fmin(1.0, rho / dist);
                     const double cps = sqrt(1.0 - sp * sp);
@@ -901,8 +903,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         while (li < run.n_lines - 1 && u2 >= __ldg(run.line_cdf + li)) ++li;
                         lam_inv = 1.0f / __ldg(run.line_nm + li);
                         const uint4 rb = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 1u, hc.key);
-                        const float xe = fmaf(s, sg.Px, sc->Ax), ye = fmaf(s, sg.Py, sc->Ay), ze = fmaf(s, sg.Pz, sg.Az);
-                        float ax = sc->aimx - xe, ay = sc->aimy - ye, az = sc->aimz - ze;
+                        float ax = fmaf(-s, sg.Px, sc->aimx), ay = fmaf(-s, sg.Py, sc->aimy), az = fmaf(-s, sg.Pz, sc->aimz);
                         const float an = rsqrtf(ax * ax + ay * ay + az * az);
                         ax *= an; ay *= an; az *= an;
                         const float tt = u01(rb.x) * sc->omc;            // 1 - cos(polar)

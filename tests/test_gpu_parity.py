@@ -756,7 +756,8 @@ def test_random_switch_combinations(trial):
     mode, write mode, bunch weight, margins, aerosol, trace method, detectors present or not), device against
     oracle photon by photon: combinations that none of the BASELINE configs uses.  (Not in the matrix, by
     conditioning rather than by method: WRITE_ALL without LV2 on cfg2's 60 degree shower and fluorescence with the
-    straight trace keep photons with |u_z| ~ 1e-3 whose plane point lies kilometres away.)"""
+    straight trace keep photons with |u_z| ~ 1e-3 whose plane point lies kilometres away and whose (u_x, u_y)
+    record cannot resolve u_z.)"""
     rng = np.random.default_rng(4200 + trial)
     k = int(rng.choice([0, 1, 2, 4])) if trial < 16 else 3
     cfg = W.make_config(k, n_segments={0: 400, 1: 250, 2: 8000, 3: 20000, 4: 1500}[k])
