@@ -623,6 +623,33 @@ def test_multiple_scattering_substeps_match_the_oracle():
     assert e.value.code == api.E_STATE
 
 
+@pytest.mark.parametrize("trial", range(6))
+def test_random_telescope_arrays(trial, monkeypatch):
+    """Seeded random telescope arrays: 1 to 16382 spheres (the record's 14-bit index allows 16382), radii 0.5-15 m at
+    altitudes +-5 m, packed into 60 m (heavily overlapping) up to 5 km squares, with a nested pair and an exact
+    duplicate (earliest entry, then lowest index): device against oracle, and grid search against search-all."""
+    rng = np.random.default_rng(55000 + trial)
+    k = int(rng.choice([2, 4]))
+    cfg = W.make_config(k, n_segments={2: 6000, 4: 1200}[k])
+    n_tel = (16382, 1, 150, 3000, 9, 2)[trial]
+    ext = float(rng.choice([30.0, 300.0, 2500.0]))
+    t = np.zeros((n_tel, 4), np.float32)
+    t[:, 0], t[:, 1] = rng.uniform(-ext, ext, n_tel), rng.uniform(-ext, ext, n_tel)
+    t[:, 2], t[:, 3] = rng.uniform(-5, 5, n_tel), rng.uniform(0.5, 15.0, n_tel)
+    if n_tel > 3:
+        t[1, :3] = t[0, :3] + np.float32([0.3, -0.2, 0.1])
+    if n_tel > 5:
+        t[4] = t[3]
+    cfg["detector"]["tel_xyzr"] = t
+    cfg["params"]["lv2_margin_m"] = float(rng.uniform(0, 50))
+    ora, gpu, rep = _both(cfg, capacity=1 << 23)
+    monkeypatch.setenv("C8PH_FORCE_BRUTE", "1")
+    ctx = api.setup_context(cfg)
+    br = api.run_config(cfg, ctx=ctx, photon_capacity=1 << 23)
+    ctx.close()
+    assert br["counters"] == gpu["counters"] and np.array_equal(br["tel_counts"], gpu["tel_counts"])
+
+
 @pytest.mark.parametrize("trial", range(8))
 def test_random_substepping_inputs(trial):
     """Sub-stepping under seeded random inputs: track counts around the warp / scan-block sizes (1, 31, 33, 700, 2049),
