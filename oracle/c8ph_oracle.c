@@ -839,7 +839,9 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                     for (int k = 0; k < 3; ++k) u[k] = cp*ax[k] + spn*(cos(phi)*e1[k] + sin(phi)*e2[k]);
                 }
                 /* O6: discard up-going / horizontal photons */
-                if (u[2] >= -1e-6) { ph.status = ORC_ST_UPGOING; lc[ORC_CNT_UPGOING]++; goto store; }
+                /* reading R7: Eq. 3.3 needs t* = -A_z/u_z > 0; a photon emitted at or below the observation
+                 * level cannot reach it going down and is dropped with the up-going ones */
+                if (u[2] >= -1e-6 || !(Ae[2] > 0.0)) { ph.status = ORC_ST_UPGOING; lc[ORC_CNT_UPGOING]++; goto store; }
                 /* O7 straight line to the observation level */
                 double I[3];
                 double D = orc_straight_line(Ae, u, I);

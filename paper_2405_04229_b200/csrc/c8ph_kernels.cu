@@ -790,7 +790,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     me.a1 = e1x * mc.rx + e1y * mc.ry + e1z * mc.rz;
                     me.a2 = e2x * mc.rx + e2y * mc.ry + e2z * mc.rz;
                     // axis landing anchor (fp64): G = A - A_z P / P_z, its clock, its grid coordinate
-                    me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05) ? 1 : 0;
+                    // (a segment that reaches z <= 0 takes the general form, which checks every emission point)
+                    me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05 && Az > 0.0 && Az + L * Pz > 0.0) ? 1 : 0;
                     me.Gx = me.Gy = me.AzP = 0.f;
                     mc.fbx = mc.fby = 0.f; mc.ibx = mc.iby = 0;
                     me.dob = (float)((double)me.delta / beta); me.inv_beta = (float)(1.0 / beta);
@@ -931,6 +932,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         ox = zq * (wx * sg.Pz - sg.Px * wz);
                         oy = zq * (wy * sg.Pz - sg.Py * wz);
                     } else {
+                        if (!(Z > 0.f)) { pkA += 1u; break; }           // emitted at or below the observation level (R7: t* > 0)
                         line_general(sc, s, D, sg.Px, sg.Py, ux, uy, ox, oy);
                     }
                     const float xl = sg.Gx + ox, yl = sg.Gy + oy;

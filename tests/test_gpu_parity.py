@@ -173,6 +173,21 @@ def test_random_directions_upgoing_and_subthreshold():
         assert rep["beyond_range"] < 0.5 * gpu["counters"]["written"]
 
 
+def test_emission_at_or_below_the_observation_level_is_dropped():
+    """Reading R7 (t* = -A_z/u_z > 0): segments that start or end at or below the observation level - their photons
+    from z <= 0 are dropped and counted with the up-going ones, the rest is propagated as usual; per-photon layered
+    sum (cfg1), table (cfg4) and straight line (cfg0) against the oracle."""
+    for k, n in ((1, 200), (4, 1200), (0, 600)):
+        cfg = W.make_config(k, n_segments=n)
+        rng = np.random.default_rng(5)
+        s = cfg["segments"]
+        s["z"][::5] = rng.uniform(-100.0, 5.0, len(s["z"][::5])).astype(np.float32)
+        cfg["params"]["lv1"] = False
+        ref = api.run_config(W.make_config(k, n_segments=n))
+        ora, gpu, rep = _both(cfg)
+        assert gpu["counters"]["upgoing"] > ref["counters"]["upgoing"] + 100
+
+
 def test_filters_lossless_on_device():
     cfg = W.make_config(2, n_segments=20000)
     on = api.run_config(cfg)
