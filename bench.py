@@ -55,9 +55,9 @@ I_ALG = {
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_emit_propagate launch on the N=1 workload, from the
-# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.581 GB + 5.003 GB).  Reported as
+# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.580 GB + 5.000 GB).  Reported as
 # `roofline.traffic` only when the run is that workload (cfg4, 1e7 segments); otherwise null.
-NCU_TRAFFIC_BYTES_CFG4 = 0.580875008e9 + 5.002906e9
+NCU_TRAFFIC_BYTES_CFG4 = 0.580233984e9 + 5.000415e9
 
 
 def _stage_population(cnt: dict) -> dict:
