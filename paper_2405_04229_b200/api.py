@@ -14,7 +14,8 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libc8ph.so")
+# C8PH_LIB selects another build of the same library (an A/B build made with `build.py --define ... --out ...`)
+LIB_PATH = os.environ.get("C8PH_LIB") or os.path.join(_HERE, "libc8ph.so")
 
 OK, E_ARG, E_STATE, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4
 ATM = {"homogeneous": 0, "planar": 1, "spherical": 2}

@@ -7,7 +7,6 @@
 
 namespace c8ph {
 
-#define C8PH_MAX_BLOCKS_PER_SM 8
 
 struct DevAtm {
     int model;              // C8PH_ATM_*
@@ -38,6 +37,7 @@ struct DevTable {
     float f_max, g_max;             // (float)(n_h-1), (float)(n_zen-1)
     const float4 *hot;              // DEVICE [n_h][n_zen] = (dd, dt, X_slant, tau_aer)
     const float *full;              // DEVICE [n_h][n_zen][5]
+    cudaTextureObject_t tex;        // the hot texels as a 2-D float4 texture (x: zenith node, y: height node), linear filter
 };
 
 // Uniform grid over the telescope array.  Every cell lists the telescopes that a point of the cell
@@ -56,8 +56,12 @@ struct DevGrid {
     int nx, ny;
     const float *kmin;              // DEVICE [nx*ny]   smallest key of the cell (+inf: empty)
     const uint8_t *kq;              // hit grid only, DEVICE [nx*ny]: floor(kmin * kHitKeyScale), 254 at most; 255: empty
-    const float2 *kacc;             // LV2 grid only, DEVICE [nx*ny]: (kmin, acc) with acc = min_k(max dist(cell, centre_k) - r_k):
-                                    // every point of the cell is within r_k/|u_z| + margin of a centre if acc <= margin
+    const float4 *knear;            // LV2 grid only, DEVICE [nx*ny]: (kmin, x, y, r) = smallest key of the cell and the telescope
+                                    // nearest to the cell (least dist(cell centre, centre_k) - r_k), tested in line before any list
+                                    // walk; empty cell: (+inf, far away, far away, 0)
+    const float4 *first;            // hit grid only, DEVICE [nx*ny]: (x, y, z, r) of the cell's first listed telescope (smallest key)
+    const int2 *first_kn;           // hit grid only, DEVICE [nx*ny]: (its index, number of telescopes listed for the cell); finish()
+                                    // issues both loads before its arithmetic, so the usual one-telescope cell costs one memory latency
     const int *start;               // DEVICE [nx*ny+1] CSR offsets into items
     const float2 *items;            // DEVICE (key, telescope index as int bits), ascending key per cell
 };
@@ -168,6 +172,5 @@ size_t segment_slot_bytes(int n_sm);
 cudaError_t launch_substep_plan(const SubstepArgs &a, long long *block_sums, cudaStream_t st);
 cudaError_t launch_substep_fill(const SubstepArgs &a, int n_sm, cudaStream_t st);
 size_t substep_scratch_elems(long long n);
-void segment_slot_pointers(void *base, int n_sm, DevRun &run);
 
 }  // namespace c8ph

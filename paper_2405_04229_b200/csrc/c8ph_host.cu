@@ -32,6 +32,8 @@ struct c8ph_ctx {
     c8ph_table_desc tab_desc{};
     float *d_full = nullptr;
     float4 *d_hot = nullptr;
+    cudaArray_t tab_arr = nullptr;     // the hot texels as a 2-D array behind a texture object (DevTable::tex)
+    cudaTextureObject_t tab_tex = 0;
     // detector
     bool have_det = false;
     DevDet det{};
@@ -40,7 +42,9 @@ struct c8ph_ctx {
     float2 *d_g_items[2] = {nullptr, nullptr};
     float *d_g_kmin[2] = {nullptr, nullptr};
     uint8_t *d_g_kq = nullptr;
-    float2 *d_g_kacc = nullptr;
+    float4 *d_g_first = nullptr;
+    int2 *d_g_first_kn = nullptr;
+    float4 *d_g_knear = nullptr;
     // run scratch
     unsigned long long *d_cursor = nullptr;
     void *d_slots = nullptr;           // prepared-segment slots of the resident warps
@@ -122,9 +126,11 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     cudaSetDevice(ctx->device);
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
+    if (ctx->tab_tex) cudaDestroyTextureObject(ctx->tab_tex);
+    if (ctx->tab_arr) cudaFreeArray(ctx->tab_arr);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
-    dfree(ctx->d_g_kq);
-    dfree(ctx->d_g_kacc);
+    dfree(ctx->d_g_kq); dfree(ctx->d_g_first); dfree(ctx->d_g_first_kn);
+    dfree(ctx->d_g_knear);
     dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     dfree(ctx->d_bsums);
@@ -251,6 +257,33 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
     d.inv_dz = (float)((t->n_zen - 1) / zmax);
     d.f_max = (float)(t->n_h - 1); d.g_max = (float)(t->n_zen - 1);
     d.hot = ctx->d_hot; d.full = ctx->d_full;
+    // texture view of the hot texels: x = zenith node, y = height node, unnormalised coordinates, clamped, bilinear
+    if (ctx->tab_tex) { cudaDestroyTextureObject(ctx->tab_tex); ctx->tab_tex = 0; }
+    if (ctx->tab_arr) { cudaFreeArray(ctx->tab_arr); ctx->tab_arr = nullptr; }
+    d.tex = 0;
+    if (t->n_zen <= 65536 && t->n_h <= 65536) {
+        const cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float4>();
+        CU(cudaMallocArray(&ctx->tab_arr, &fmt, (size_t)t->n_zen, (size_t)t->n_h));
+        cudaResourceDesc res{};
+        res.resType = cudaResourceTypeArray;
+        res.res.array.array = ctx->tab_arr;
+        cudaTextureDesc td{};
+        td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
+        td.filterMode = cudaFilterModeLinear;
+        td.readMode = cudaReadModeElementType;
+        td.normalizedCoords = 0;
+        CU(cudaCreateTextureObject(&ctx->tab_tex, &res, &td, nullptr));
+        d.tex = ctx->tab_tex;
+    }
+    return C8PH_OK;
+}
+
+// copy the hot texels into the texture's array (device to device, on `st`)
+static int fill_table_texture(c8ph_ctx *ctx, cudaStream_t st)
+{
+    if (!ctx->tab_arr) return C8PH_OK;
+    const size_t row = (size_t)ctx->tab.n_zen * sizeof(float4);
+    CU(cudaMemcpy2DToArrayAsync(ctx->tab_arr, 0, 0, ctx->d_hot, row, row, (size_t)ctx->tab.n_h, cudaMemcpyDeviceToDevice, st));
     return C8PH_OK;
 }
 
@@ -267,6 +300,8 @@ extern "C" int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, v
     a.full = ctx->d_full; a.hot = ctx->d_hot;
     cudaError_t e = launch_build_table(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "build_trace_table launch");
+    rc = fill_table_texture(ctx, (cudaStream_t)stream);
+    if (rc) return rc;
     ctx->launches++;
     ctx->have_table = true;
     return C8PH_OK;
@@ -298,6 +333,9 @@ extern "C" int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, con
     }
     CU(cudaMemcpy(ctx->d_full, host_in, n * C8PH_TABLE_CHANNELS * sizeof(float), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_hot, hot.data(), n * sizeof(float4), cudaMemcpyHostToDevice));
+    rc = fill_table_texture(ctx, nullptr);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(nullptr));
     ctx->have_table = true;
     return C8PH_OK;
 }
@@ -355,7 +393,8 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     const double pad = 1e-3 * cs + 8.0 * (coord_max + ext) * 1.2e-7 + 1e-4;
     struct Entry { uint32_t cell; float key; int k; };
     std::vector<Entry> ent;
-    std::vector<float> acc(mode == 1 ? ncell : 0, INFINITY);
+    std::vector<float> near_d(mode == 1 ? ncell : 0, INFINITY);      // LV2: least dist(cell centre, centre_k) - r_k so far
+    std::vector<int> near_k(mode == 1 ? ncell : 0, -1);
     ent.reserve((size_t)n * 64);
     for (int k = 0; k < n; ++k) {
         const double cx_ = tel[4 * k], cy_ = tel[4 * k + 1], rc = reach(k);
@@ -370,13 +409,11 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
                 const double dist = std::sqrt((px - cx_) * (px - cx_) + (py - cy_) * (py - cy_));
                 if (dist > rc) continue;
                 if (mode == 1) {
-                    // farthest point of the padded cell from the centre, minus the radius, rounded up
-                    const double fx = std::max(std::fabs(bx0 - cx_), std::fabs(bx1 - cx_)), fy = std::max(std::fabs(by0 - cy_), std::fabs(by1 - cy_));
-                    const double av = (std::sqrt(fx * fx + fy * fy) - (double)tel[4 * k + 3]) * (1.0 + 1e-6) + 1e-4;
-                    float af = (float)av;
-                    if ((double)af < av) af = std::nextafterf(af, INFINITY);
-                    float &slot = acc[(size_t)iy * nx + ix];
-                    if (af < slot) slot = af;
+                    // the telescope nearest to the cell: the device tests it in line before walking the list
+                    const double mx_ = x0 + (ix + 0.5) * cs - cx_, my_ = y0 + (iy + 0.5) * cs - cy_;
+                    const float dn = (float)(std::sqrt(mx_ * mx_ + my_ * my_) - (double)tel[4 * k + 3]);
+                    const size_t ci = (size_t)iy * nx + ix;
+                    if (dn < near_d[ci]) { near_d[ci] = dn; near_k[ci] = k; }
                 }
                 const double key = mode == 0 ? dist / rz : dist;
                 ent.push_back({(uint32_t)((size_t)iy * nx + ix), f32_down(key * (1.0 - 1e-6)), k});
@@ -407,8 +444,9 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     CU(cudaMemcpy(ctx->d_g_kmin[which], kmin.data(), kmin.size() * sizeof(float), cudaMemcpyHostToDevice));
     g.x0 = (float)x0; g.y0 = (float)y0; g.inv_cs = (float)(1.0 / cs); g.nx = nx; g.ny = ny;
     g.kmin = ctx->d_g_kmin[which]; g.start = ctx->d_g_start[which]; g.items = ctx->d_g_items[which];
-    g.kacc = nullptr;
+    g.knear = nullptr;
     g.kq = nullptr;
+    g.first = nullptr; g.first_kn = nullptr;
     if (mode == 0) {
         // hit pre-test: the smallest key of a cell in 1/64 steps, rounded down (conservative: a false candidate is
         // rejected by the exact search), one byte per cell so that the cells under the shower stay in L1
@@ -419,14 +457,32 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
         CU(cudaMalloc(&ctx->d_g_kq, ncell));
         CU(cudaMemcpy(ctx->d_g_kq, kq.data(), ncell, cudaMemcpyHostToDevice));
         g.kq = ctx->d_g_kq;
+        // the first listed telescope of every cell, in line (finish() tests it without walking the list)
+        std::vector<float4> first(ncell, make_float4(0.f, 0.f, 0.f, 0.f));
+        std::vector<int2> first_kn(ncell, make_int2(-1, 0));
+        for (size_t i = 0; i < ncell; ++i)
+            if (start[i + 1] > start[i]) {
+                const int k = ent[start[i]].k;
+                first[i] = make_float4(tel[4 * k], tel[4 * k + 1], tel[4 * k + 2], tel[4 * k + 3]);
+                first_kn[i] = make_int2(k, start[i + 1] - start[i]);
+            }
+        dfree(ctx->d_g_first); dfree(ctx->d_g_first_kn);
+        CU(cudaMalloc(&ctx->d_g_first, ncell * sizeof(float4)));
+        CU(cudaMalloc(&ctx->d_g_first_kn, ncell * sizeof(int2)));
+        CU(cudaMemcpy(ctx->d_g_first, first.data(), ncell * sizeof(float4), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->d_g_first_kn, first_kn.data(), ncell * sizeof(int2), cudaMemcpyHostToDevice));
+        g.first = ctx->d_g_first; g.first_kn = ctx->d_g_first_kn;
     }
     if (mode == 1) {
-        std::vector<float2> ka(ncell);
-        for (size_t i = 0; i < ncell; ++i) ka[i] = make_float2(kmin[i], acc[i]);
-        dfree(ctx->d_g_kacc);
-        CU(cudaMalloc(&ctx->d_g_kacc, ncell * sizeof(float2)));
-        CU(cudaMemcpy(ctx->d_g_kacc, ka.data(), ncell * sizeof(float2), cudaMemcpyHostToDevice));
-        g.kacc = ctx->d_g_kacc;
+        std::vector<float4> kn(ncell);
+        for (size_t i = 0; i < ncell; ++i) {
+            const int k = near_k[i];
+            kn[i] = k >= 0 ? make_float4(kmin[i], tel[4 * k], tel[4 * k + 1], tel[4 * k + 3]) : make_float4(INFINITY, 3.0e18f, 3.0e18f, 0.f);
+        }
+        dfree(ctx->d_g_knear);
+        CU(cudaMalloc(&ctx->d_g_knear, ncell * sizeof(float4)));
+        CU(cudaMemcpy(ctx->d_g_knear, kn.data(), ncell * sizeof(float4), cudaMemcpyHostToDevice));
+        g.knear = ctx->d_g_knear;
     }
     return C8PH_OK;
 }
@@ -636,7 +692,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     r.n_seg = n_seg; r.seg_id_base = base; r.local_base = 0;
     r.seg = *s; r.out = *o;
     r.cursor = ctx->d_cursor;
-    segment_slot_pointers(ctx->d_slots, ctx->n_sm, r);
+    r.slots = ctx->d_slots;
     const long long warps = (long long)ctx->n_sm * 2 * 8;
     long long g = n_seg / (warps * 4);
     r.segs_per_grab = (int)std::min<long long>(32, std::max<long long>(1, g));

@@ -29,24 +29,55 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <cstdint>
+#include <cstdlib>
 #include <type_traits>
 #include "c8ph_device.cuh"
 #include "c8ph_philox.cuh"
+
+// ---- compile-time A/B knobs (`python -m paper_2405_04229_b200.build --define NAME=VALUE --out lib.so`, then
+// C8PH_LIB=lib.so).  The defaults are what the measurements on cfg4 chose; profiles/r2_ab.md has one row per knob.
+#ifndef C8PH_SINCOS_MUFU
+#define C8PH_SINCOS_MUFU 1      // 1: azimuth sin / cos by MUFU.SIN / MUFU.COS (sin.approx), 0: polynomial from the uniform's bits
+#endif
+#ifndef C8PH_TABLE_TEX
+#define C8PH_TABLE_TEX 0        // 1: correction table through a 2-D float4 texture object with hardware bilinear filtering
+#endif
+#ifndef C8PH_HIST_MATCH
+#define C8PH_HIST_MATCH 0       // 1: lanes of a warp that hit the same ground bin are aggregated (match.any) into one RED
+#endif
+#ifndef C8PH_ETA_STAGED
+#define C8PH_ETA_STAGED 0       // 1: n(h) staged in shared memory by a TMA bulk copy also for the table-tracing variants
+#endif
+#ifndef C8PH_ETA_SEGFIT
+#define C8PH_ETA_SEGFIT 0       // 1: n(h_e) along a segment from a per-segment quadratic in s, fitted in fp64 and checked against the
+#endif                          //    piecewise-linear table (Listing 4.1) to 4e-7 relative; segments that fail it read the table per photon
+#ifndef C8PH_QUEUE_CONVERGED
+#define C8PH_QUEUE_CONVERGED 0  // 1: candidates are queued after the photon body's reconvergence point (one ballot, fill count in a
+#endif                          //    register); 0: inside the body, where the few candidate lanes are
+#ifndef C8PH_QUEUE_LANE_ATOMS
+#define C8PH_QUEUE_LANE_ATOMS 1 // (inside the body) 1: every candidate lane takes its slot with its own ATOMS; 0: one ATOMS per group of
+#endif                          //    lanes that arrive together, slot = base + rank (activemask, leader, shuffle)
+#ifndef C8PH_PROD_ONLY
+#define C8PH_PROD_ONLY 0        // 1: instantiate only the generic variants and SPEC = base (fast A/B builds)
+#endif
 
 namespace c8ph {
 
 namespace {
 
+// Launch shape.  Table / straight tracing: ONE CTA of 768 threads per SM (24 warps at 80 registers): the per-warp candidate
+// queues (4 KB each) plus one CTA's static and reserved shared memory then fit the 100 KB carve-out, which leaves
+// 156 KB of L1 instead of 124 KB with three CTAs of 256 threads (measured: profiles/r2_ab.md).  The layered-sum variant
+// stages 80-120 KB of tables per CTA and runs two CTAs of 256 threads.
 #ifndef C8PH_THREADS
-#define C8PH_THREADS 256
+#define C8PH_THREADS 768
 #endif
 #ifndef C8PH_MIN_BLOCKS
-#define C8PH_MIN_BLOCKS 3
+#define C8PH_MIN_BLOCKS 1
 #endif
-constexpr int kThreads = C8PH_THREADS;
-constexpr int kWarps = kThreads / 32;
-constexpr int kMaxBlocksPerSM = C8PH_MAX_BLOCKS_PER_SM;
-constexpr int kMinBlocks = C8PH_MIN_BLOCKS;                    // resident CTAs per SM the register budget is set for
+constexpr int kMaxWarpsPerSM = 64;                             // hardware limit; the segment-slot scratch is sized for it
+__host__ __device__ constexpr int kernel_threads(int trace) { return trace == C8PH_TRACE_NUMERIC ? 256 : C8PH_THREADS; }
+__host__ __device__ constexpr int kernel_min_blocks(int trace) { return trace == C8PH_TRACE_NUMERIC ? 2 : C8PH_MIN_BLOCKS; }
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
 constexpr double kAlphaFS = 1.0 / 137.035999;    // fine-structure constant (Eq. 2.3)
@@ -101,14 +132,16 @@ __device__ __forceinline__ double u01d(uint32_t r)
 // photon, kept in registers while the warp walks the segment; COLD = used by landed photons /
 // rare branches, re-read through L1 where it is needed (keeps the register count down).
 struct alignas(16) SegHot {                       // 28 words = 7 x 16 B
-    float Px, Py, Pz, e1x, e1y, e1z, e2x, e2y, e2z;   // direction and the two Rodrigues columns
+    float Px, Py, Pz, e1x, e1y, e2y;                  // direction and the Rodrigues columns (M symmetric, third column -P:
+                                                      // e2x = e1y, e1z = -P_x, e2z = -P_y)
+    float q0, q1, q2;                                 // n(h_e) - 1 = q0 + s (q1 + s q2) along the segment (anchor bit 1 set)
     float L, beta, delta;                             // length, beta, 1 - beta
     float hA, cA, k2;                                 // height of A, dh/ds, second-order term
     float Az, AzP;                                    // A_z, A_z / P_z (anchor form)
     float Gx, Gy;                                     // axis landing point (anchor) or unused
     float a1, a2, inv_rA;                             // e1.r, e2.r, 1/|A - C|
     uint32_t id_lo, id_hi;                            // global segment id (Philox counter words)
-    int N, anchor;                                    // bunches to emit; 1: anchor form valid
+    int N, anchor;                                    // bunches to emit; bit 0: anchor form valid, bit 1: q0..q2 valid
     float dob, inv_beta;                              // (1 - beta)/beta, 1/beta (read from the slot, not kept in registers)
 };
 struct alignas(16) SegCold {                      // 16 words = 4 x 16 B
@@ -197,6 +230,16 @@ __device__ __forceinline__ float acos01(float x)
 // 7e-8), then swap / sign by octant.
 __device__ __forceinline__ void sincos_2pi_u(uint32_t r, float &sphi, float &cphi)
 {
+#if C8PH_SINCOS_MUFU
+    // u - 1/2 = (v - 1.5) + 2^-24 with v = 1.m in [1, 2): exact in fp32; sin(2 pi u) = -sin(2 pi (u - 1/2)), same for cos.
+    // sin.approx = FMUL.RZ by 1/(2 pi) + MUFU.SIN on [-pi, pi] (PTX ISA: max absolute error 2^-20.9)
+    const float a = __uint_as_float(0x3F800000u | (r >> 9)) - 1.5f;
+    const float ph = fmaf(a, 6.2831853071795865f, 3.7450702829e-07f);       // 2 pi (u - 1/2)
+    float sv, cv;
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sv) : "f"(ph));
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cv) : "f"(ph));
+    sphi = -sv; cphi = -cv;
+#else
     const uint32_t m = r >> 9, o = m >> 20;
     uint32_t ml = m & 0xFFFFFu;
     if (o & 1u) ml ^= 0xFFFFFu;
@@ -215,6 +258,7 @@ __device__ __forceinline__ void sincos_2pi_u(uint32_t r, float &sphi, float &cph
     const float s0 = swap ? cv : sv, c0 = swap ? sv : cv;
     sphi = __uint_as_float(__float_as_uint(s0) ^ ((o & 4u) << 29));
     cphi = __uint_as_float(__float_as_uint(c0) ^ (((o + 2u) & 4u) << 29));
+#endif
 }
 
 // Dispersive Cherenkov yield integral (thesis P:318, unnumbered equation before Eq. 2.5):
@@ -252,6 +296,15 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
 {
     TabVal o;
     o.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f);
+#if C8PH_TABLE_TEX
+    {
+        // texel (b, a) = node (height a, zenith b); unnormalised coordinates, clamped addressing, linear filter
+        const float4 v = tex2D<float4>(t.tex, fmaf(thz, t.inv_dz, 0.5f), fmaf(h, t.inv_dh, 0.5f));
+        o.dd = v.x; o.dt = v.y; o.X = v.z; o.ta = v.w;
+        o.bad = o.bad || (o.dd != o.dd);
+        return o;
+    }
+#endif
     const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
     const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
     const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
@@ -278,27 +331,36 @@ __device__ __forceinline__ int grid_cell(const DevGrid &g, float x, float y)
 }
 
 // exact ray / bounding-sphere test of one telescope; updates the nearest entry
+__device__ __forceinline__ void sphere_test_rec(const float4 t, int k, float x, float y, float ux, float uy, float uz,
+                                                float &best_s, int &best_k);
 __device__ __forceinline__ void sphere_test(const DevDet &det, int k, float x, float y, float ux, float uy, float uz,
                                             float &best_s, int &best_k)
 {
-    const float4 t = __ldg(det.tel + k);
+    sphere_test_rec(__ldg(det.tel + k), k, x, y, ux, uy, uz, best_s, best_k);
+}
+__device__ __forceinline__ void sphere_test_rec(const float4 t, int k, float x, float y, float ux, float uy, float uz,
+                                                float &best_s, int &best_k)
+{
+    // every product is written as an explicit fma / rounded multiply: the function is inlined at several places and the
+    // tie-break between duplicate spheres (lowest index) needs the same bits from each of them
     const float dx = t.x - x, dy = t.y - y, dz = t.z;
-    const float du = dx * ux + dy * uy + dz * uz;
+    const float du = fmaf(dx, ux, fmaf(dy, uy, __fmul_rn(dz, uz)));
     // squared miss distance from the perpendicular part of (centre - point): |d|^2 - du^2 cancels when a grazing ray
     // meets the plane kilometres from the telescope (10 cm at 2 km in fp32)
     const float qx = fmaf(-du, ux, dx), qy = fmaf(-du, uy, dy), qz = fmaf(-du, uz, dz);
-    const float m2 = qx * qx + qy * qy + qz * qz;
-    const float r2 = t.w * t.w;
+    const float m2 = fmaf(qx, qx, fmaf(qy, qy, __fmul_rn(qz, qz)));
+    const float r2 = __fmul_rn(t.w, t.w);
     if (m2 <= r2) {
-        const float s_in = du - sqrtf(r2 - m2);
+        const float s_in = __fsub_rn(du, sqrtf(__fsub_rn(r2, m2)));
         if (s_in < best_s || (s_in == best_s && k < best_k)) { best_s = s_in; best_k = k; }
     }
 }
 
 // nearest entry along the arrival ray, lowest index on ties.  `cell` < -1: brute force over all
 // telescopes; otherwise the sorted candidates of the cell while key <= thr (thr >= 1/|u_z|).
+// (t0, kn0) = the cell's first listed telescope and (its index, list length), loaded by the caller ahead of time.
 __device__ __forceinline__ int tel_hit_search(const DevDet &det, int cell, float thr, float x, float y,
-                                           float ux, float uy, float uz)
+                                           float ux, float uy, float uz, const float4 t0, const int2 kn0)
 {
     int best_k = -1;
     float best_s = CUDART_INF_F;
@@ -306,9 +368,12 @@ __device__ __forceinline__ int tel_hit_search(const DevDet &det, int cell, float
         for (int k = 0; k < det.n_tel; ++k) sphere_test(det, k, x, y, ux, uy, uz, best_s, best_k);
         return best_k;
     }
-    if (cell < 0) return -1;
+    if (cell < 0 || kn0.y <= 0) return -1;
+    // the first entry has the smallest key; the pre-test already compared it (rounded down) with the threshold
+    sphere_test_rec(t0, kn0.x, x, y, ux, uy, uz, best_s, best_k);
+    if (kn0.y == 1) return best_k;
     const int hi = __ldg(det.hit.start + cell + 1);
-    for (int i = __ldg(det.hit.start + cell); i < hi; ++i) {
+    for (int i = __ldg(det.hit.start + cell) + 1; i < hi; ++i) {
         const float2 e = __ldg(det.hit.items + i);
         if (e.x > thr) break;
         sphere_test(det, __float_as_int(e.y), x, y, ux, uy, uz, best_s, best_k);
@@ -395,9 +460,10 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2,
 // matches one that is instantiated (launch_emit_propagate).  SPEC = 0 reads every switch at run time.
 constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32;
 template <int EMIT, int TRACE, bool SPH, int SPEC>
-__global__ void __launch_bounds__(kThreads, TRACE == C8PH_TRACE_NUMERIC ? 2 : kMinBlocks)
+__global__ void __launch_bounds__(kernel_threads(TRACE), kernel_min_blocks(TRACE))
 k_emit_propagate(const __grid_constant__ KArgs a)
 {
+    constexpr int kWarps = kernel_threads(TRACE) / 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
     __shared__ unsigned long long s_cnt[kWarps][WC_N];
@@ -409,29 +475,34 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned FULL = 0xFFFFFFFFu;
     unsigned long long *cntp = reinterpret_cast<unsigned long long *>(run.out.counters);
-    constexpr bool STAGED = TRACE == C8PH_TRACE_NUMERIC;     // n(h) tables in shared memory
+    constexpr bool STAGED = TRACE == C8PH_TRACE_NUMERIC;     // n(h), overburden steps (and aerosol column) in shared memory
+    constexpr bool STAGE_ETA = STAGED || (C8PH_ETA_STAGED && TRACE == C8PH_TRACE_TABLE);   // n(h) in shared memory
 
     // ---- shared memory carve-up: [n(h) tables] | per-warp candidate queue (SoA, kQueue entries)
     float *s_eta = reinterpret_cast<float *>(smem_raw);
-    float *s_dxv = s_eta + (STAGED ? atm.n_pad : 0);
+    float *s_dxv = s_eta + (STAGE_ETA ? atm.n_pad : 0);
     float *s_aexp = s_dxv + (STAGED ? atm.n_pad : 0);       // aerosol column A(h_k) = (H/L) exp(-h_k/H), staged only with aerosol
     const bool aer_staged = STAGED && atm.aer_L > 0.f;
     float *s_end = s_aexp + (aer_staged ? atm.n_pad : 0);
     float4 *s_q = reinterpret_cast<float4 *>(s_end) + warp * (kQueue * 4);   // s_q[slot * 4 + part]
+#if !C8PH_QUEUE_CONVERGED
     __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
+#endif
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
     SegSlot *g_slot = static_cast<SegSlot *>(run.slots) + ((size_t)blockIdx.x * kWarps + warp) * 32;
 
     if (lane < WC_N) s_cnt[warp][lane] = 0ull;
+#if !C8PH_QUEUE_CONVERGED
     if (lane == 0) s_qn[warp] = 0;
+#endif
     // ---- layered-sum variant: stage the atmosphere tables with one TMA bulk copy per array
-    if (STAGED) {
+    if (STAGE_ETA) {
         if (threadIdx.x == 0) {
             mbar_init(&s_bar, 1);
             const uint32_t bytes = (uint32_t)atm.n_pad * 4u;
-            mbar_expect_tx(&s_bar, bytes * (aer_staged ? 3u : 2u));
+            mbar_expect_tx(&s_bar, bytes * (STAGED ? (aer_staged ? 3u : 2u) : 1u));
             bulk_g2s(s_eta, atm.eta, bytes, &s_bar);
-            bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
+            if (STAGED) bulk_g2s(s_dxv, atm.dxv, bytes, &s_bar);
             if (aer_staged) bulk_g2s(s_aexp, atm.aexp, bytes, &s_bar);
         }
         __syncthreads();
@@ -440,7 +511,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     __syncwarp();
     // n(h) node: shared memory when staged, otherwise through L1 (the lanes of a warp emit from one
     // short segment: 1-3 adjacent words, one cache line)
-    auto eta_node = [&](int k) -> float { return STAGED ? s_eta[k] : __ldg(hc.eta + k); };
+    auto eta_node = [&](int k) -> float { return STAGE_ETA ? s_eta[k] : __ldg(hc.eta + k); };
 
     // per-lane event counters of the photon loop, two 16-bit fields per register, flushed to
     // s_cnt before a field can overflow
@@ -478,6 +549,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_telc = SPEC ? true : run.out.tel_counts != nullptr;
     const float inv_ng = 1.0f / (1.0f + atm.eta_g);
     int q_head = 0;                                           // ring position of the oldest queue entry
+#if C8PH_QUEUE_CONVERGED
+    int q_n = 0;                                              // entries waiting in the warp's queue (warp-uniform register)
+#endif
 
     // arrival direction: u turned in the ray plane (u, local vertical) by the angle that follows from the
     // Snell / Bouguer invariant (R9), small-angle form
@@ -512,6 +586,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         int tel = -1;
         float uax = ux, uay = uy, uaz = uz, t_arr = 0.f;
         float rx_out = 0.f, ry_out = 0.f;                     // record position (ground plane, or camera plane with optics)
+        // a14: the first listed telescope of the photon's hit cell; loaded first so that the latency overlaps a13
+        float4 t0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        int2 kn0 = make_int2(-1, 0);
+        if (act && f_tel && cell >= 0) { t0 = __ldg(det.hit.first + cell); kn0 = __ldg(det.hit.first_kn + cell); }
         bool opt_hit = false;
         const SegSlot *sl = g_slot + (jslot & 31u);
         const SegHot *sh = &sl->h;
@@ -522,7 +600,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         rx_out = xg; ry_out = yg;
         if (act) {
             // a13: arrival time relative to t_ref
-            if (sh->anchor) {
+            if (sh->anchor & 1) {
                 // (t - T_G) c = s delta/beta + (s + A_z/P_z)(q w_z - bn1 P_z)/(P_z + q w_z) + c dt
                 const float Pz = sh->Pz;
                 const float eta_c = f_disp ? eta_e * fmaf(run.disp_b, lam_inv * lam_inv, run.disp_c0) : eta_e;
@@ -540,7 +618,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 // air), search all telescopes
                 const float thr = -rcp_fast(uz) * run.hit_infl;
                 if (cell >= 0 && !(-uaz * thr >= 1.f)) cell = -2;
-                tel = tel_hit_search(det, cell, thr, xg, yg, uax, uay, uaz);
+                tel = tel_hit_search(det, cell, thr, xg, yg, uax, uay, uaz, t0, kn0);
             }
             if (tel >= 0) {
                 pkC += 0x10000u;
@@ -550,7 +628,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // pointing axis (vertex at centre - (f/2) w), reflection, camera disc at z = f
                     const float4 tc = __ldg(det.tel + tel);
                     const float f = det.opt_f, hf = 0.5f * f;
-                    const float lox = sh->anchor ? sc->Ax : 0.f, loy = sh->anchor ? sc->Ay : 0.f;
+                    const float lox = (sh->anchor & 1) ? sc->Ax : 0.f, loy = (sh->anchor & 1) ? sc->Ay : 0.f;
                     const float px = (sh->Gx - tc.x) + (q0.x + lox) + hf * det.opt_w[0];
                     const float py = (sh->Gy - tc.y) + (q0.y + loy) + hf * det.opt_w[1], pz = -(tc.z - hf * det.opt_w[2]);
                     const float a0 = px * det.opt_r[0] + py * det.opt_r[1] + pz * det.opt_r[2];
@@ -637,7 +715,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // take up to 32 queued candidates (all of them if `all`) through finish()
     auto drain = [&](bool all) {
         __syncwarp();
+#if C8PH_QUEUE_CONVERGED
+        int n = q_n;
+#else
         int n = s_qn[warp];
+#endif
         while (n >= 32 || (all && n > 0)) {
             const int take = n < 32 ? n : 32;
             const float4 *e = s_q + ((q_head + lane) & (kQueue - 1)) * 4;
@@ -646,8 +728,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             q_head = (q_head + take) & (kQueue - 1);
             n -= take;
             __syncwarp();
+#if C8PH_QUEUE_CONVERGED
+            q_n = n;
+#else
             if (lane == 0) s_qn[warp] = n;
             __syncwarp();
+#endif
         }
     };
 
@@ -782,7 +868,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 if (myN > 0) {
                     me.N = myN;
                     me.Px = (float)Px; me.Py = (float)Py; me.Pz = (float)Pz;
-                    me.e1x = e1x; me.e1y = e1y; me.e1z = e1z; me.e2x = e2x; me.e2y = e2y; me.e2z = e2z;
+                    me.e1x = e1x; me.e1y = e1y; me.e2y = e2y;
+                    me.q0 = me.q1 = me.q2 = 0.f;
                     mc.Ax = (float)Ax; mc.Ay = (float)Ay; me.Az = (float)Az;
                     me.L = (float)L; me.beta = (float)beta; me.delta = 1.0f - (float)beta;
                     me.hA = (float)hA; me.cA = (float)cA; me.k2 = SPH ? (float)((1.0 - cA * cA) / (2.0 * rA)) : 0.f;
@@ -792,10 +879,45 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     // axis landing anchor (fp64): G = A - A_z P / P_z, its clock, its grid coordinate
                     // (a segment that reaches z <= 0 takes the general form, which checks every emission point)
                     me.anchor = (EMIT == C8PH_EMIT_CHERENKOV && Pz < -0.05 && Az > 0.0 && Az + L * Pz > 0.0) ? 1 : 0;
+#if C8PH_ETA_SEGFIT
+                    if (EMIT == C8PH_EMIT_CHERENKOV && TRACE != C8PH_TRACE_NUMERIC) {
+                        // Listing 4.1 along the segment: eta(h(s)) is piecewise quadratic in s (linear in h between nodes,
+                        // h quadratic in s).  One quadratic through s = 0, L/2, L replaces the per-photon lookup if it
+                        // reproduces the table at every node the segment crosses and half-way between them.
+                        const double hA32 = (double)me.hA, cA32 = (double)me.cA, k232 = (double)me.k2;   // what the photon uses
+                        auto h_of = [&](double sv) { return hA32 + sv * (cA32 + sv * k232); };
+                        const double f0 = eta_lookup_d(atm, h_of(0.0)), fm = eta_lookup_d(atm, h_of(0.5 * L)), f1 = eta_lookup_d(atm, h_of(L));
+                        const double c2 = L > 0.0 ? 2.0 * (f1 - 2.0 * fm + f0) / (L * L) : 0.0;
+                        const double c1 = L > 0.0 ? (-3.0 * f0 + 4.0 * fm - f1) / L : 0.0;
+                        const float q0f = (float)f0, q1f = (float)c1, q2f = (float)c2;
+                        auto fit = [&](double sv) { return (double)q0f + sv * ((double)q1f + sv * (double)q2f); };
+                        const double ha = h_of(0.0), hb = h_of(L), dhn = (double)atm.dh;
+                        const double ka = (fmin(ha, hb) - (double)atm.h0) / dhn, kb = (fmax(ha, hb) - (double)atm.h0) / dhn;
+                        bool ok = fabs(cA32) > 1e-3 && kb - ka < 8.0;                 // monotonic height, a few nodes at most
+                        if (ok) {
+                            const double tol = 4e-7 * fmax(fabs(fm), 1e-12);
+                            double s_prev = 0.0, err = fmax(fabs(fit(0.5 * L) - fm), fabs(fit(L) - f1));
+                            const int k_lo = (int)ceil(ka), k_hi = (int)floor(kb);
+                            // nodes in the order the particle meets them
+                            for (int t = 0; t <= k_hi - k_lo + 1; ++t) {
+                                double s_k = L;
+                                if (t <= k_hi - k_lo) {
+                                    const int kn = cA32 < 0.0 ? k_hi - t : k_lo + t;
+                                    s_k = fmin(fmax((((double)atm.h0 + kn * dhn) - hA32) / cA32, 0.0), L);
+                                }
+                                const double sm = 0.5 * (s_prev + s_k);
+                                err = fmax(err, fmax(fabs(fit(sm) - eta_lookup_d(atm, h_of(sm))), fabs(fit(s_k) - eta_lookup_d(atm, h_of(s_k)))));
+                                s_prev = s_k;
+                            }
+                            ok = err <= tol;
+                        }
+                        if (ok) { me.q0 = q0f; me.q1 = q1f; me.q2 = q2f; me.anchor |= 2; }
+                    }
+#endif
                     me.Gx = me.Gy = me.AzP = 0.f;
                     mc.fbx = mc.fby = 0.f; mc.ibx = mc.iby = 0;
                     me.dob = (float)((double)me.delta / beta); me.inv_beta = (float)(1.0 / beta);
-                    if (me.anchor) {
+                    if (me.anchor & 1) {
                         const double azp = Az / Pz;
                         const double Gx = Ax - azp * Px, Gy = Ay - azp * Py;
                         me.Gx = (float)Gx; me.Gy = (float)Gy; me.AzP = (float)azp;
@@ -847,6 +969,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             iters_pending += n_iter;
             for (int it = 0; it < n_iter; ++it) {
                 const int j = it * 32 + lane;
+#if C8PH_QUEUE_CONVERGED
+                bool qpush = false;
+                float4 qe0, qe1, qe2, qe3;                            // defined where qpush is set
+#endif
                 // one photon per lane; every cut leaves through the same exit (one reconvergence point)
                 if (j < sg.N) do {
                     const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, hc.key);
@@ -855,6 +981,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float s = u1 * sg.L;
                     const float h_e = fmaf(s, fmaf(s, sg.k2, sg.cA), sg.hA);
                     float eta_e;
+#if C8PH_ETA_SEGFIT
+                    if (sg.anchor & 2) eta_e = fmaf(s, fmaf(s, sg.q2, sg.q1), sg.q0);     // warp-uniform branch
+                    else
+#endif
                     {
                         float f = (h_e - hc.eta_h0) * hc.eta_inv_dh;
                         f = fminf(fmaxf(f, 0.f), hc.eta_fmax);
@@ -927,7 +1057,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float inv_uz = rcp_fast(uz);
                     const float Z = fmaf(s, sg.Pz, sg.Az);
                     const float D = -Z * inv_uz;
-                    if (sg.anchor) {
+                    if (sg.anchor & 1) {
                         const float zq = -Z * q * rcp_fast(sg.Pz * pqz);
                         ox = zq * (wx * sg.Pz - sg.Px * wz);
                         oy = zq * (wy * sg.Pz - sg.Py * wz);
@@ -945,11 +1075,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                             const bool brute = !f_grid || -uz < hc.grid_min_cos;
                             const float thr = fmaf(hc.r_max, -inv_uz, hc.lv2_margin);
                             const int cell = brute ? -2 : grid_cell(det.lv2, xl, yl);
-                            // per cell: (smallest key, acc); acc <= margin: every point of the cell is near
-                            // a telescope; smallest key > thr: none is; otherwise walk the sorted list
-                            float2 ka = make_float2(CUDART_INF_F, CUDART_INF_F);
-                            if (cell >= 0) ka = __ldg(det.lv2.kacc + cell);
-                            keep = ka.y <= hc.lv2_margin;
+                            // per cell: (smallest key, x, y, r of the telescope nearest to the cell): that one is tested
+                            // in line; if it is out of reach and the smallest key <= thr the sorted list is walked
+                            float4 ka = make_float4(CUDART_INF_F, 3.0e18f, 3.0e18f, 0.f);
+                            if (cell >= 0) ka = __ldg(det.lv2.knear + cell);
+                            {
+                                const float dx = xl - ka.y, dy = yl - ka.z, reach = fmaf(ka.w, -inv_uz, hc.lv2_margin);
+                                keep = dx * dx + dy * dy <= reach * reach;
+                            }
                             if (!keep && (cell < -1 || ka.x <= thr))
                                 keep = tel_near_search(det, cell, thr, xl, yl, -inv_uz, hc.lv2_margin);
                         }
@@ -1116,6 +1249,13 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         const int iy = __float_as_int(fb.w) + __float2int_rd(fmaf(cy, hc.hist_inv_cell, fb.y));
                         if ((unsigned)ix < (unsigned)hc.hist_nx && (unsigned)iy < (unsigned)hc.hist_ny) {
                             pkC += 1u;
+#if C8PH_HIST_MATCH
+                            if (SPEC) {                                  // roulette mode: every bunch has weight w
+                                const int bin = iy * hc.hist_nx + ix;
+                                const unsigned peers = __match_any_sync(__activemask(), bin);
+                                if (lane == __ffs(peers) - 1) atomicAdd(hc.hist + bin, wgt * (float)__popc(peers));
+                            } else
+#endif
                             if (has_hist) atomicAdd(hc.hist + (iy * hc.hist_nx + ix), wgt);
                         }
                     }
@@ -1124,8 +1264,22 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         if (f_write != C8PH_WRITE_ALL) break;
                         cell = -1;
                     }
-                    // queue the photon for finish() (a13/a14/a16): slots are handed out per group of lanes
+                    // queue the photon for finish() (a13/a14/a16)
+#if C8PH_QUEUE_CONVERGED
+                    // the entry leaves the body in registers and is stored after the reconvergence point
+                    qe0 = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
+                    qe1 = make_float4(uz, s, q * wz, dt);
+                    qe2 = make_float4(lam_inv, wgt, eta_e, h_e);
+                    qe3 = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+                    qpush = true;
+#else
+                    // slots are handed out per group of lanes
                     // that arrive here together (one shared-memory atomic per group), four 16 B stores
+#if C8PH_QUEUE_LANE_ATOMS
+                    int qb;                                              // inline asm: no compiler-generated warp aggregation
+                    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])) : "memory");
+                    float4 *e = s_q + ((q_head + qb) & (kQueue - 1)) * 4;
+#else
                     const unsigned am = __activemask();
                     const int leader = __ffs(am) - 1;
                     int qb = 0;
@@ -1133,13 +1287,32 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])), "r"(__popc(am)) : "memory");
                     qb = __shfl_sync(am, qb, leader);
                     float4 *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
+#endif
                     e[0] = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
                     e[1] = make_float4(uz, s, q * wz, dt);
                     e[2] = make_float4(lam_inv, wgt, eta_e, h_e);
                     e[3] = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+#endif
                 } while (false);
+#if C8PH_QUEUE_CONVERGED
+                // all lanes are back together: one ballot ranks the candidates, four 16 B stores each, the fill count
+                // stays in a (warp-uniform) register
+                {
+                    const unsigned pm = __ballot_sync(FULL, qpush);
+                    if (pm) {
+                        if (qpush) {
+                            float4 *e = s_q + ((q_head + q_n + __popc(pm & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
+                            e[0] = qe0; e[1] = qe1; e[2] = qe2; e[3] = qe3;
+                        }
+                        q_n += __popc(pm);
+                        // a14/a16: once 32 candidates wait, a full warp takes them through finish()
+                        if (q_n >= 32) drain(false);
+                    }
+                }
+#else
                 // a14/a16: once 32 candidates wait, a full warp takes them through finish()
                 drain(false);
+#endif
             }
         }
         drain(true);                                                  // slots are rewritten by the next group
@@ -1271,11 +1444,16 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
     auto kern = k_emit_propagate<EMIT, TRACE, SPH, SPEC>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    {
+        static const char *cv = getenv("C8PH_CARVEOUT");               // experiment: shared-memory carve-out in percent
+        if (cv) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv));
+    }
     int per_sm = 0;
+    constexpr int kThreads = kernel_threads(TRACE), kWarps = kThreads / 32;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    if (per_sm > kMaxBlocksPerSM) per_sm = kMaxBlocksPerSM;         // the segment-slot scratch is sized for this
+    if (per_sm * kWarps > kMaxWarpsPerSM) per_sm = kMaxWarpsPerSM / kWarps;   // the segment-slot scratch is sized for this
     long long warps_needed = (a.run.n_seg + a.run.segs_per_grab - 1) / a.run.segs_per_grab;
     long long blocks = (warps_needed + kWarps - 1) / kWarps;
     const long long max_blocks = (long long)n_sm * per_sm;          // persistent: one resident wave
@@ -1289,19 +1467,14 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
 
 size_t segment_slot_bytes(int n_sm)
 {
-    return (size_t)n_sm * kMaxBlocksPerSM * kWarps * 32 * sizeof(SegSlot);
-}
-
-void segment_slot_pointers(void *base, int n_sm, DevRun &run)
-{
-    (void)n_sm;
-    run.slots = base;
+    return (size_t)n_sm * kMaxWarpsPerSM * 32 * sizeof(SegSlot);
 }
 
 size_t emit_smem_bytes(const KArgs &a)
 {
-    const size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
-    return tables + (size_t)kWarps * kQueue * Q_WORDS * sizeof(float);
+    size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
+    if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
+    return tables + (size_t)(kernel_threads(a.run.trace) / 32) * kQueue * Q_WORDS * sizeof(float);
 }
 
 // SPEC mask of the call: 0 unless it matches the switches the SPEC != 0 variants are compiled for,
@@ -1328,8 +1501,12 @@ cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
         return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase>(a, n_sm, smem, st)
                    : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, kSpecBase>(a, n_sm, smem, st);
     // production setting + optional features (spherical model): the combinations that are compiled
+#if C8PH_PROD_ONLY
+#define C8_SPEC(M)
+#else
 #define C8_SPEC(M) \
     if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, smem, st);
+#endif
     C8_SPEC(kSpecFlat)
     C8_SPEC(kSpecExt)
     C8_SPEC(kSpecDisp)

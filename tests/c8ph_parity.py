@@ -16,6 +16,11 @@ TOL_T_NS = 0.1
 TOL_DIR_RAD = 1e-5
 TOL_FLIP_FRAC = 1e-4
 TOL_TOTAL_REL = 1e-5
+# A total of fewer than 3e5 photon weights cannot be held to 1e-5 by any implementation whose survival decisions are
+# taken in another floating-point precision (one roulette or edge flip is 1/total): below that size the total may
+# differ by this many photon weights ("tolerances"); every BASELINE config at full size except
+# cfg3 (9.5e3 camera photons) is above it, so there the 1e-5 arm binds.
+TOL_TOTAL_MIN_PHOTONS = 3
 
 
 def _key(seg, j):
@@ -53,12 +58,14 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
         wmean = tot / max(1, (oc["cam_hit"] if det["cam_enabled"] else oc["in_grid"]))
         moved = 0.5 * np.abs(ho - hg).sum() / max(wmean, 1e-300)
         rep["hist_moved_photons"] = moved
+        rep["hist_moved_frac"] = moved / n_emit                       # north_star: <= 1e-4 of photons changing bin
         rep["hist_total"] = (tot, hg.sum())
+        rep["hist_total_rel"] = abs(hg.sum() - tot) / tot if tot > 0 else 0.0
         assert moved <= budget, (moved, budget)
         if tot > 0:
-            # order-dependent fp32 accumulation is exact for integral weights; weight mode adds
-            # fp32 rounding of ~1e-7 per add, well inside the budget
-            assert abs(hg.sum() - tot) / tot <= max(TOL_TOTAL_REL, 1.5 * budget * wmean / tot), rep["hist_total"]
+            # north_star: total weighted hit count within 1e-5 relative (order-dependent fp32 accumulation is
+            # exact for integral weights; weight mode adds fp32 rounding of ~1e-7 per add)
+            assert abs(hg.sum() - tot) <= max(TOL_TOTAL_REL * tot, TOL_TOTAL_MIN_PHOTONS * wmean), rep["hist_total"]
     if len(ora["tel_counts"]):
         to, tg = ora["tel_counts"], gpu["tel_counts"].astype(np.float64)
         assert 0.5 * np.abs(to - tg).sum() / float(par["bunch_weight"]) <= budget + 1e-6 * to.sum()
@@ -88,6 +95,7 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
     unmatched = (len(gk) - len(common)) + (len(ok) - len(common))
     rep["written"] = (len(ok), len(gk))
     rep["unmatched_keys"] = unmatched
+    rep["unmatched_frac"] = unmatched / n_emit
     assert unmatched <= budget, (unmatched, budget)
     g = gph[gi][ia]
     o = want[oi][ib]
@@ -125,4 +133,14 @@ def compare(cfg: dict, ora: dict, gpu: dict, check_photons: bool = True, max_ran
         inside = (bx >= 0) & (bx < det["hist_nx"]) & (by >= 0) & (by < det["hist_ny"])
         gbin = np.where(inside, by * det["hist_nx"] + bx, -1).astype(np.int64)
         rep["bin_flips_from_xy"] = int((gbin != o["bin"]).sum())
+        rep["bin_flip_frac"] = rep["bin_flips_from_xy"] / max(len(g), 1)
     return rep
+
+
+def summary(rep: dict) -> str:
+    """One line with the measured values behind every north_star tolerance (printed by smoke() and the full-size tests)."""
+    f = lambda k, fmt="%.2e": (fmt % rep[k]) if rep.get(k) is not None else "n/a"
+    return (f"hist_total_rel={f('hist_total_rel')} (tol {TOL_TOTAL_REL:g}) hist_moved_frac={f('hist_moved_frac')} "
+            f"bin_flip_frac={f('bin_flip_frac')} unmatched_frac={f('unmatched_frac')} (tol {TOL_FLIP_FRAC:g}) "
+            f"max_dpos_m={f('max_dpos_m')} (tol {TOL_POS_M:g}) max_dt_ns={f('max_dt_ns')} (tol {TOL_T_NS:g}) "
+            f"max_ddir_rad={f('max_ddir_rad')} (tol {TOL_DIR_RAD:g})")

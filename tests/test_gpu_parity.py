@@ -30,6 +30,7 @@ def _both(cfg, capacity=1 << 22, check_photons=True, ctx=None, max_range_m=None)
     ora = O.run(cfg, record=check_photons)
     gpu = api.run_config(cfg, ctx=ctx, photon_capacity=capacity)
     rep = parity.compare(cfg, ora, gpu, check_photons=check_photons, max_range_m=max_range_m)
+    print("parity:", parity.summary(rep))
     return ora, gpu, rep
 
 
@@ -339,7 +340,7 @@ def test_cfg4_full_size_sampled_windows_and_invariants():
         assert len(gk) + len(ok) - 2 * len(common) <= budget
         # element-by-element on the window via the standard comparison of a window-only device run
         win = api.run_config(sub, ctx=ctx)
-        parity.compare(sub, ora, win)
+        print(f"window [{lo}, {hi}):", parity.summary(parity.compare(sub, ora, win)))
         k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
         k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
@@ -373,7 +374,7 @@ def test_cfg1_full_size_sampled_windows_and_invariants():
         sub["seg_id_base"] = lo
         ora = O.run(sub)
         win = api.run_config(sub, ctx=ctx)
-        parity.compare(sub, ora, win)
+        print(f"window [{lo}, {hi}):", parity.summary(parity.compare(sub, ora, win)))
         k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
         k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
         assert len(rec) > 2e4 and np.array_equal(rec[k1], win["photons"][k2])   # full-size run == window run, bit for bit
@@ -417,7 +418,7 @@ def test_cfg2_full_size_sampled_windows_and_invariants():
         sub["seg_id_base"] = lo
         ora = O.run(sub)
         win = api.run_config(sub, ctx=ctx)
-        parity.compare(sub, ora, win)
+        print(f"window [{lo}, {hi}):", parity.summary(parity.compare(sub, ora, win)))
         k2 = np.argsort(win["photons"]["seg"].astype(np.int64) << 32 | win["photons"]["j_tel"])
         k1 = np.argsort(rec["seg"].astype(np.int64) << 32 | rec["j_tel"])
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit

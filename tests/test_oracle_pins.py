@@ -155,6 +155,63 @@ def test_constant_n_ring_and_arrival_time():
     assert abs(np.mean(s) - 5.0) < 5 * 10 / math.sqrt(12 * len(s))           # O2: uniform on the track
 
 
+def test_emission_at_or_below_the_observation_level_is_dropped():
+    """Reading R7 (Eq. 3.3 P:495 needs t* = -A_z/u_z > 0): a vertical track that straddles z = 0 lands the
+    photons emitted above the plane on the analytic ring r = z_e tan(theta_c) and drops the others as up-going.  The
+    emission point of every photon is re-derived here from the (known-answer pinned) Philox words, not from the run."""
+    cfg = _one_segment_cfg(z=5.0, L=10.0)
+    cfg["segments"]["charge"][:] = 3.0                                # 9x the photons
+    res = O.run(cfg)
+    ph = res["photons"]
+    assert len(ph) > 3000
+    n = float(np.float32(0.000293)) + 1.0
+    tan_c = math.sqrt(n * n - 1.0)
+    seed = cfg["seed"]
+    s = np.array([O.uniform(O.philox4x32_10([int(j), 0, 0, 0], [seed & 0xFFFFFFFF, seed >> 32])[1]) * 10.0 for j in ph["j"]])
+    z_e = 5.0 - s
+    above = z_e > 0.0
+    assert 0.4 < above.mean() < 0.6
+    assert np.all(ph["status"][above] == O.ST_LANDED) and np.all(ph["status"][~above] == O.ST_UPGOING)
+    assert np.allclose(np.hypot(ph["x"], ph["y"])[above], z_e[above] * tan_c, atol=1e-9, rtol=0)
+    c = res["counters"]
+    assert c["upgoing"] == int((~above).sum()) and c["landed"] == int(above.sum())
+    # a track that ends exactly on the plane keeps every photon (z_e > 0 for s < L), one that starts on it keeps none
+    assert np.all(O.run(_one_segment_cfg(z=10.0, L=10.0))["photons"]["status"] == O.ST_LANDED)
+    assert np.all(O.run(_one_segment_cfg(z=0.0, L=10.0))["photons"]["status"] == O.ST_UPGOING)
+
+
+def test_telescope_tie_break_earliest_entry_then_lowest_index():
+    """O12 / R12: among several bounding spheres the ray enters, the earliest entry wins, then the lowest index.
+    Two overlapping spheres (the second one raised, so that it is entered earlier by part of the rays) and an exact
+    duplicate of each; entry parameters recomputed here in closed form from the photon records."""
+    cfg = _one_segment_cfg(z=1000.0, L=200.0)
+    cfg["segments"]["charge"][:] = 2.0
+    tel = np.array([[20.0, 0.0, 0.0, 10.0], [25.0, 0.0, 5.0, 10.0], [25.0, 0.0, 5.0, 10.0], [20.0, 0.0, 0.0, 10.0]], dtype=np.float32)
+    cfg["detector"]["tel_xyzr"] = tel
+    ph = O.run(cfg)["photons"]
+    ph = ph[ph["status"] == O.ST_LANDED]
+    I = np.stack([ph["x"], ph["y"], np.zeros(len(ph))], axis=1)
+    u = np.stack([ph["ux"], ph["uy"], ph["uz"]], axis=1)
+    s_in = np.full((len(ph), 4), np.inf)
+    for k in range(4):
+        d = tel[k, :3].astype(np.float64) - I
+        du = (d * u).sum(axis=1)
+        m2 = (d * d).sum(axis=1) - du * du
+        hit = m2 <= float(tel[k, 3]) ** 2
+        s_in[hit, k] = du[hit] - np.sqrt(float(tel[k, 3]) ** 2 - m2[hit])
+    want = np.where(np.isfinite(s_in.min(axis=1)), s_in.argmin(axis=1), -1)   # argmin returns the lowest index on ties
+    both = np.isfinite(s_in[:, 0]) & np.isfinite(s_in[:, 1])
+    gap = np.ones(len(ph))
+    gap[both] = np.abs(s_in[both, 0] - s_in[both, 1])
+    clear = gap > 1e-6                                                # not within rounding of an exact tie of k0 and k1
+    assert np.array_equal(ph["tel"][clear], want[clear])
+    assert not np.any(np.isin(ph["tel"], (2, 3)))                     # a duplicate never wins against its lower index
+    print("both & k0 / both & k1 / k0 only / k1 only / none:", (both & (want == 0)).sum(), (both & (want == 1)).sum(),
+          (~both & (want == 0)).sum(), (~both & (want == 1)).sum(), (want == -1).sum())
+    assert (both & (want == 0)).sum() > 20 and (both & (want == 1)).sum() > 20 and (want == -1).sum() > 100
+    assert (~both & (want >= 0)).sum() > 5                             # rays that enter one sphere only
+
+
 def test_wavelength_law():
     cfg = _one_segment_cfg(L=200.0)
     ph = O.run(cfg)["photons"]
