@@ -51,6 +51,18 @@
 #ifndef C8PH_ETA_SEGFIT
 #define C8PH_ETA_SEGFIT 0       // 1: n(h_e) along a segment from a per-segment quadratic in s, fitted in fp64 and checked against the
 #endif                          //    piecewise-linear table (Listing 4.1) to 4e-7 relative; segments that fail it read the table per photon
+#ifndef C8PH_SLOT_PREFETCH
+#define C8PH_SLOT_PREFETCH 1    // 1: the next emitting segment's slot (two 128 B lines) is prefetched into L1 while the current one runs
+#endif
+#ifndef C8PH_HIT_PREFETCH
+#define C8PH_HIT_PREFETCH 0     // 1: a lane that queues a telescope candidate prefetches the hit cell's first-telescope record (finish() reads it)
+#endif
+#ifndef C8PH_QUEUE_VOTE
+#define C8PH_QUEUE_VOTE 1       // 1: "32 candidates wait" is decided by a vote of the lanes that pushed; 0: by reading the fill count
+#endif
+#ifndef C8PH_TABLE_EARLY
+#define C8PH_TABLE_EARLY 0      // 1 (production variants): the four texel loads of the correction table are issued before the straight
+#endif                          //    line and the LV2 test and combined after them, so that their latency overlaps that arithmetic
 #ifndef C8PH_QUEUE_CONVERGED
 #define C8PH_QUEUE_CONVERGED 0  // 1: candidates are queued after the photon body's reconvergence point (one ballot, fill count in a
 #endif                          //    register); 0: inside the body, where the few candidate lanes are
@@ -289,6 +301,33 @@ __device__ __forceinline__ double disp_yield_integral(double beta, double eta, d
 }
 
 struct TabVal { float dd, dt, X, ta; bool bad; };
+struct TabRaw { float4 v00, v01, v10, v11; float ff, gg; bool bad; };
+
+// the two halves of table_lookup below: issue the four texel loads / combine them
+__device__ __forceinline__ TabRaw table_issue(const DevTable &t, float h, float thz)
+{
+    TabRaw r;
+    r.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f);
+    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
+    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
+    const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
+    r.ff = f - (float)ia; r.gg = g - (float)ib;
+    const float4 *p = t.hot + (unsigned)(ia * t.n_zen + ib);
+    const float4 *p1 = p + (unsigned)t.n_zen;
+    r.v00 = __ldg(p); r.v01 = __ldg(p + 1); r.v10 = __ldg(p1); r.v11 = __ldg(p1 + 1);
+    return r;
+}
+__device__ __forceinline__ TabVal table_combine(const TabRaw &r)
+{
+    TabVal o;
+    const float w11 = r.ff * r.gg, w10 = r.ff - w11, w01 = r.gg - w11, w00 = (1.f - r.ff) - w01;
+    o.dd = fmaf(w11, r.v11.x, fmaf(w10, r.v10.x, fmaf(w01, r.v01.x, w00 * r.v00.x)));
+    o.dt = fmaf(w11, r.v11.y, fmaf(w10, r.v10.y, fmaf(w01, r.v01.y, w00 * r.v00.y)));
+    o.X = fmaf(w11, r.v11.z, fmaf(w10, r.v10.z, fmaf(w01, r.v01.z, w00 * r.v00.z)));
+    o.ta = fmaf(w11, r.v11.w, fmaf(w10, r.v10.w, fmaf(w01, r.v01.w, w00 * r.v00.w)));
+    o.bad = r.bad || (o.dd != o.dd);
+    return o;
+}
 
 // bilinear lookup in the correction table (linear interpolation between support points):
 // four LDG.128 texels (dd, dt, X_slant, tau_aer); indices clamped; out of range / no-ground -> bad
@@ -964,11 +1003,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             SegHot sg;
             copy16(&sg, &sl->h);                                      // uniform address: one sector per LDG.128
             const SegCold *sc = &sl->c;                               // cold fields are re-read (L1) where used
+#if C8PH_SLOT_PREFETCH
+            if (emask && lane < 3)                                    // next emitting segment of the group: 176 B from L2 into L1
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(g_slot + (__ffs(emask) - 1)) + lane * 88 - (lane >> 1)));
+#endif
             const int n_iter = (sg.N + 31) >> 5;
             if (iters_pending + n_iter > 60000) flush_counts();
             iters_pending += n_iter;
             for (int it = 0; it < n_iter; ++it) {
                 const int j = it * 32 + lane;
+#if C8PH_QUEUE_VOTE && C8PH_QUEUE_LANE_ATOMS && !C8PH_QUEUE_CONVERGED
+                bool qfull = false;
+#endif
 #if C8PH_QUEUE_CONVERGED
                 bool qpush = false;
                 float4 qe0, qe1, qe2, qe3;                            // defined where qpush is set
@@ -1049,6 +1095,19 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         uy = cp * ay + sp2 * (cphi * e1y + sphi * e2y);
                         uz = cp * az + sp2 * (sphi * e2z);
                     }
+                    // (production variants) zenith angle and the table's texel loads ahead of a8-a10
+                    constexpr bool EARLY_TAB = C8PH_TABLE_EARLY && SPEC != 0 && EMIT == C8PH_EMIT_CHERENKOV && TRACE == C8PH_TRACE_TABLE;
+                    TabRaw traw;
+                    float cz_e = 0.f;
+                    if (EARLY_TAB) {
+                        if (SPH) {
+                            const float ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
+                            const float sr = s * sg.inv_rA;
+                            cz_e = -(fmaf(-sr * sg.cA, ur, ur) + sr * cth);
+                        } else cz_e = -uz;
+                        cz_e = fminf(cz_e, 1.f);
+                        traw = table_issue(a.tab, h_e, acos01(fmaxf(cz_e, 0.f)));
+                    }
                     // a8: up-going / horizontal photons are discarded
                     if (uz >= kUpCut) { pkA += 1u; break; }
                     // a9: straight line to z = 0 (Eq. 3.3), anchor + offset form
@@ -1091,7 +1150,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     }
                     // local zenith angle of the photon at the emission point
                     float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz;
-                    if (SPH) {
+                    if (EARLY_TAB) cz = cz_e;
+                    else if (SPH) {
                         float ur;
                         if (EMIT == C8PH_EMIT_CHERENKOV) ur = cth * fmaf(q, fmaf(cphi, sg.a1, sphi * sg.a2), sg.cA);
                         else ur = ux * sc->rx + uy * sc->ry + uz * sc->rz;
@@ -1106,7 +1166,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (TRACE == C8PH_TRACE_STRAIGHT) {
                         dt = eta_e * D * kInvC;                          // homogeneous: t = t_e + n D / c
                     } else if (TRACE == C8PH_TRACE_TABLE) {
-                        const TabVal v = table_lookup(a.tab, h_e, acos01(fmaxf(cz, 0.f)));
+                        const TabVal v = EARLY_TAB ? table_combine(traw) : table_lookup(a.tab, h_e, acos01(fmaxf(cz, 0.f)));
                         if (v.bad || !(cz > 0.f)) { pkB += 1u; break; }
                         dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
                     } else {
@@ -1275,9 +1335,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #else
                     // slots are handed out per group of lanes
                     // that arrive here together (one shared-memory atomic per group), four 16 B stores
+#if C8PH_HIT_PREFETCH
+                    if (f_tel && cell >= 0) {
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(det.hit.first + cell));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(det.hit.first_kn + cell));
+                    }
+#endif
 #if C8PH_QUEUE_LANE_ATOMS
                     int qb;                                              // inline asm: no compiler-generated warp aggregation
                     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])) : "memory");
+#if C8PH_QUEUE_VOTE
+                    qfull = qb >= 31;
+#endif
                     float4 *e = s_q + ((q_head + qb) & (kQueue - 1)) * 4;
 #else
                     const unsigned am = __activemask();
@@ -1311,7 +1380,11 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 }
 #else
                 // a14/a16: once 32 candidates wait, a full warp takes them through finish()
+#if C8PH_QUEUE_VOTE && C8PH_QUEUE_LANE_ATOMS
+                if (__any_sync(FULL, qfull)) drain(false);
+#else
                 drain(false);
+#endif
 #endif
             }
         }
