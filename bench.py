@@ -38,26 +38,32 @@ import numpy as np
 METRIC = "propagated photons/sec"
 UNIT = "photons/s"
 
-# Algorithmic thread-instructions per unit of each stage of the fused kernel, audited from the SASS
-# of k_emit_propagate<CHERENKOV,TABLE,SPH,SPEC=1> with ncu's per-instruction execution counts
-# (DESIGN.md section 5 "Roofline"; profiles/r1_cfg4_final.md): the instructions every unit of a
-# stage executes exactly once on its way through.  What is NOT counted: telescope candidates that turn
-# out to miss, LV2 list searches, queue drains of partly filled warps, idle lanes.
-I_ALG = {
-    "segment": 1000.0,    # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor, slot store (per segment)
-    "emitted": 249.0,     # a5-a12: loop slot 16 + Philox4x32-10, uniforms, emission point, n(h), cone, sincos,
-                          #         straight line, LV2 box, zenith, acos, bilinear float4 lookup, transmission, roulette: 233
-    "landed": 50.0,       # a15 + a14 pre-test: corrected position, telescope-grid cell + smallest key, bin index
+# Roofline numerator 1 (`roofline.frac`): SURVEY.md section 8(d) "Algorithmic work per photon", an estimate made from the
+# method's arithmetic BEFORE any kernel existed: Philox4x32-10 40, uniforms 8, wavelength 3, emission point / height 14,
+# n(h_e) 6, cone angle 8, sincos 4, direction 12, straight line 14, LV2 + lattice index 20, zenith + acos 18, bilinear
+# float4 lookup 25, apply + arrival angle + time 22, transmission + roulette 10, ray-sphere 14, bin + RED 8, compaction 6,
+# loop / predicates 15 = 250 thread-instructions per emitted photon (+- 40).  Independent of this implementation.
+I_ALG_SURVEY_PER_PHOTON = 250.0
+
+# Roofline numerator 2 (`roofline.frac_own_audit`): instructions one unit of each stage executes on its way through THIS
+# kernel, k_emit_propagate<CHERENKOV,TABLE,SPH,SPEC=1>, derived by tests/roofline_audit.py from the committed ncu source
+# page profiles/r2_cfg4_source.csv.gz (tests/test_roofline_audit.py checks these numbers against it).  Not counted: the
+# loop slot, the queue push, LV2 list walks, candidates that miss, partly filled drains, idle lanes.
+I_ALG_OWN = {
+    "segment": 1081.2,    # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor, slot store (per segment)
+    "emitted": 212.0,     # a5-a12: Philox4x32-10, uniforms, emission point, n(h), cone, sincos, straight line, LV2 box, zenith,
+                          #         acos, bilinear float4 lookup, transmission, roulette
+    "landed": 54.0,       # a15 + a14 pre-test: corrected position, telescope-grid cell + smallest key, bin index
     "in_grid": 6.0,       # a15: bin address + RED.ADD.F32
-    "tel_hit": 193.0,     # a13/a14/a16: queue push 27 + finish 166 (time, arrival direction, sphere search, record);
-                          # the current finish() has 183 instructions (finer hit grid): the smaller audited count is kept
+    "tel_hit": 155.0,     # a13/a14/a16: finish() (time, arrival direction, sphere search, record), once per hit
 }
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_emit_propagate launch on the N=1 workload, from the
-# ncu --set full capture summarised in profiles/r1_cfg4_final.md (0.580 GB + 5.000 GB).  Reported as
-# `roofline.traffic` only when the run is that workload (cfg4, 1e7 segments); otherwise null.
-NCU_TRAFFIC_BYTES_CFG4 = 0.580233984e9 + 5.000415e9
+# ncu --set full capture summarised in profiles/r2_cfg4_final.md.  Reported as `roofline.traffic` only when the run is
+# that workload (cfg4, 1e7 segments); otherwise null.
+NCU_TRAFFIC_BYTES_CFG4 = 0.620197120e9 + 5.037879e9
+NCU_ISSUE_SLOTS_BUSY_CFG4 = 0.7119                 # smsp issue slots busy of the same capture
 
 
 def _stage_population(cnt: dict) -> dict:
@@ -67,7 +73,7 @@ def _stage_population(cnt: dict) -> dict:
 
 def algorithmic_instructions(cnt: dict) -> float:
     pop = _stage_population(cnt)
-    return float(sum(I_ALG[k] * pop[k] for k in I_ALG))
+    return float(sum(I_ALG_OWN[k] * pop[k] for k in I_ALG_OWN))
 
 
 def algorithmic_bytes(cnt: dict, n_hist: int, n_tel: int) -> float:
@@ -159,7 +165,20 @@ def _oracle_setup(cfg):
     return cores
 
 
-def cpu_baseline(cfg, target_s: float = 20.0) -> dict:
+def _cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_baseline(cfg, target_s: float = 12.0) -> dict:
+    """The oracle as it stands (unoptimised fp64 test oracle: e.g. brute force over all telescopes per landed photon)
+    on a prefix of the workload: all host cores (`value`) and one thread (`single_thread`).  A stated baseline, not a
+    tuned CPU implementation."""
     cores = _oracle_setup(cfg)
     n_total = len(cfg["segments"]["x"])
     n0 = min(n_total, 400)
@@ -168,8 +187,13 @@ def cpu_baseline(cfg, target_s: float = 20.0) -> dict:
     per_seg = ph0 / n0
     n1 = int(min(n_total, max(n0, target_s * rate0 / max(per_seg, 1e-9))))
     ph, dt = _oracle_rate(cfg, n1)
-    return {"value": ph / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {n1} segments of the workload ({int(ph)} photons, {dt:.1f} s, fp64, OpenMP over segments)"}
+    n2 = int(min(n_total, max(100, n1 // max(cores, 1) // 2)))          # ~ half that time on one thread
+    ph1, dt1 = _oracle_rate(cfg, n2, threads=1)
+    return {"value": ph / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": _cpu_model(),
+            "sample": f"first {n1} segments of the workload ({int(ph)} photons, {dt:.1f} s, fp64, OpenMP over segments)",
+            "single_thread": {"value": ph1 / dt1, "unit": UNIT, "cores": 1,
+                              "sample": f"first {n2} segments ({int(ph1)} photons, {dt1:.1f} s)"},
+            "note": "unoptimised fp64 test oracle; the ratio to it says nothing about kernel quality"}
 
 
 def run_reference(args):
@@ -293,7 +317,14 @@ def run_ours(args):
     n = W.FULL_SEGMENTS[k] if args.segments is None else args.segments
     cfg = W.make_config(k, n_segments=n)
     _apply_variant(cfg, args.variant)
-    seg_id_base = rank * n                               # weak scaling: disjoint segment ids per rank
+    n_total = n
+    if args.scaling == "strong" and world > 1:
+        # ONE shower sharded over the ranks by contiguous id range: total work fixed
+        lo, hi = shard.shard_of(n_total, rank, world)
+        cfg["segments"] = W.slice_segments(cfg["segments"], lo, hi)
+        n, seg_id_base = hi - lo, lo
+    else:
+        seg_id_base = rank * n                           # weak scaling: disjoint segment ids per rank
     ctx = api.setup_context(cfg, device=local)
     par, seed = cfg["params"], cfg["seed"]
     w = float(par["bunch_weight"])
@@ -307,6 +338,20 @@ def run_ours(args):
     def zero(o):
         o["hist"].zero_(); o["tel_counts"].zero_(); o["counters"].zero_()
 
+    def exchange(o):
+        """The one exchange step of the sharded path: SUM all-reduce of histogram, telescope
+        counters and event counters; NCCL on the launch stream (gloo: through host copies, plumbing check only)."""
+        if not dist:
+            return o
+        if backend == "nccl":
+            return shard.reduce_results(o)
+        host = {kk: o[kk].cpu() for kk in ("hist", "tel_counts", "counters")}
+        shard.reduce_results(host)
+        for kk, v in host.items():
+            if kk != "written_local" and hasattr(v, "shape"):
+                o[kk].copy_(v)
+        return o
+
     def step():
         zero(out)
         ctx.emit_propagate(seg_dev, n, seg_id_base, par, seed, out)
@@ -317,10 +362,13 @@ def run_ours(args):
     cnt = {kk: int(v) for kk, v in zip(api.COUNTER_NAMES, out["counters"].cpu().numpy())}
     if cnt["overflow"]:
         raise SystemExit(f"bench.py: photon list overflow ({cnt['overflow']}); raise --photon-capacity")
+    if dist:
+        exchange(out)                                    # warm-up of the collective (communicator set-up)
 
     # ---- timed region: K steps, device-resident inputs (400 MB of segments > 126 MB L2)
     sampler = ClockSampler(local)
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    launches0 = ctx.launch_count()
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
@@ -332,26 +380,38 @@ def run_ours(args):
         ev[s][1].record()
         ctx.emit_propagate(seg_dev, n, seg_id_base, par, seed, out)
         ev[s][2].record()
+        exchange(out)
+        ev[s][3].record()
     torch.cuda.synchronize()
     t_wall = time.perf_counter() - t_wall
     clocks = sampler.stop()
     if dist:
         dist.barrier()
-    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    # our kernels inside the timed region (the library's own count) + torch's three fill kernels per step
+    gpu_launches = int(ctx.launch_count() - launches0) + 3 * args.steps
+    total_ms = ev[0][0].elapsed_time(ev[-1][3])
     kern_ms = [e[1].elapsed_time(e[2]) for e in ev]
+    exch_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in ev])) if dist else 0.0
     total_ms = shard.max_over_ranks(total_ms, red_dev)
     photons_rank = cnt["emitted"] * w
     photons_job = shard.sum_over_ranks(photons_rank, red_dev)
     value = photons_job * args.steps / (total_ms * 1e-3)
+    # checksum of the (reduced) result: N = 1 and a strong-scaling run at any N give the same bits (integral weights)
+    import zlib
+    hist_host = out["hist"].cpu().numpy()
+    checksum = {"hist_sum": float(hist_host.astype(np.float64).sum()), "hist_crc32": int(zlib.crc32(hist_host.tobytes())),
+                "tel_sum": float(out["tel_counts"].double().sum().item())}
 
     # ---- roofline of the one kernel of the step (ALU issue bound)
     props = torch.cuda.get_device_properties(local)
     n_sm = props.multi_processor_count
     k_ms = float(np.mean(kern_ms))
-    i_alg = algorithmic_instructions(cnt)
+    i_own = algorithmic_instructions(cnt)
+    i_survey = I_ALG_SURVEY_PER_PHOTON * cnt["emitted"]
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak = n_sm * 128 * sm_max * 1e6 / 1e9                # G thread-inst/s at clocks.max.sm
-    achieved = i_alg / (k_ms * 1e-3) / 1e9
+    achieved = i_survey / (k_ms * 1e-3) / 1e9
+    achieved_own = i_own / (k_ms * 1e-3) / 1e9
     peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
     hbm_peak, peak_src = 6650.0, "fallback"
     if os.path.exists(peaks_file):
@@ -360,13 +420,18 @@ def run_ours(args):
         except Exception:
             pass
     alg_bytes = algorithmic_bytes(cnt, ctx.n_hist(), ctx._n_tel)
+    headline = (k == 4 and n == W.FULL_SEGMENTS[4] and args.variant == "base")
     roofline = {"bound": "alu", "kernel": "k_emit_propagate", "achieved": achieved, "peak": peak,
                 "unit": "Ginst/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES_CFG4 if (k == 4 and n == W.FULL_SEGMENTS[4]) else None,
+                "numerator": "SURVEY 8(d): 250 thread-instructions per emitted photon (implementation-independent estimate)",
+                "frac_own_audit": achieved_own / peak, "achieved_own_audit": achieved_own,
+                "own_audit_inst_per_photon": i_own / max(cnt["emitted"], 1),
+                "own_audit": "tests/roofline_audit.py on profiles/r2_cfg4_source.csv.gz (stage counts of this kernel's SASS)",
+                "issue_slots_busy_ncu": NCU_ISSUE_SLOTS_BUSY_CFG4 if headline else None,
+                "traffic": NCU_TRAFFIC_BYTES_CFG4 if headline else None,
                 "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic bytes = %.4g" % alg_bytes,
                 "peak_def": f"{n_sm} SMs x 4 schedulers x 32 lanes x clocks.max.sm {sm_max:.0f} MHz (issue slots)",
                 "frac_at_measured_clock": (achieved / (n_sm * 128 * clocks["sm_mhz"] * 1e-3)) if clocks.get("sm_mhz") else None,
-                "alg_inst_per_photon": i_alg / max(cnt["emitted"], 1),
                 "kernel_ms": k_ms,
                 "hbm": {"achieved": alg_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                         "frac": alg_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
@@ -410,13 +475,15 @@ def run_ours(args):
     bad = [r for r in clocks.get("reasons", []) if r in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown")]
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": _workload_name(k, n) + ("" if args.variant == "base" else f" + {args.variant}"), "segments_per_gpu": n, "photons_per_step_per_gpu": photons_rank,
+            "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": _workload_name(k, n_total) + ("" if args.variant == "base" else f" + {args.variant}"), "segments_per_gpu": n, "photons_per_step_per_gpu": photons_rank,
                        "landed": cnt["landed"], "in_grid": cnt["in_grid"], "tel_hit": cnt["tel_hit"], "written": cnt["written"],
                        "l2": f"inputs ({40 * n / 1e6:.0f} MB of segments) and photon list ({32 * cnt['written'] / 1e9:.2f} GB) vs 126 MB L2; outputs re-zeroed each step",
-                       "parallelism": f"segments sharded, {world} independent id ranges" if world > 1 else "1 GPU"},
-            "clocks": clocks, "clock_rejected": bool(bad),
-            "e2e": e2e, "gpu_launches": args.steps * 1, "roofline": roofline, "cpu_baseline": base,
+                       "parallelism": (f"segments sharded over {world} ranks by id range ({args.scaling}), results SUM all-reduced "
+                                       f"each step ({backend})") if world > 1 else "1 GPU"},
+            "counters": cnt, "clocks": clocks, "clock_rejected": bool(bad),
+            "e2e": e2e, "gpu_launches": gpu_launches, "roofline": roofline, "cpu_baseline": base,
+            "exchange_ms_per_step": exch_ms, "result_checksum": checksum,
             "wall_ms_per_step": 1e3 * t_wall / args.steps}
     print(json.dumps(line), flush=True)
     if dist:
@@ -431,6 +498,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--scaling", choices=("weak", "strong"), default="weak",
+                    help="N > 1: weak = every rank its own full batch (default, the driver's contract); strong = ONE batch sharded "
+                         "by contiguous segment-id range (SURVEY 8(e)); both end each step with the SUM all-reduce of the results")
     ap.add_argument("--segments", type=int, default=None, help="override the segment count (debugging only)")
     ap.add_argument("--photon-capacity", type=int, default=220_000_000)
     ap.add_argument("--e2e-steps", type=int, default=3)

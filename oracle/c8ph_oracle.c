@@ -1036,6 +1036,13 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
 }
 
 int orc_sizeof_photon(void) { return (int)sizeof(orc_photon); }
+/* harness only (no arithmetic): threads of the next orc_run; n <= 0 restores the OpenMP default; returns what is in force */
+#ifdef _OPENMP
+#include <omp.h>
+int orc_set_threads(int n) { omp_set_num_threads(n > 0 ? n : omp_get_num_procs()); return omp_get_max_threads(); }
+#else
+int orc_set_threads(int n) { (void)n; return 1; }
+#endif
 int orc_n_counters(void) { return ORC_N_COUNTERS; }
 
 /* ------------------------------------------------------------------ sub-stepping (row f2, reading R16)

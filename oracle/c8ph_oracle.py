@@ -365,8 +365,9 @@ def run(cfg: dict, record: bool = True, table_data: np.ndarray | None = None, th
     emitted photon with its status; only if record)).
     """
     L = lib()
-    if threads is not None:
-        os.environ["OMP_NUM_THREADS"] = str(threads)
+    L.orc_set_threads.argtypes = [C.c_int]
+    L.orc_set_threads.restype = C.c_int
+    L.orc_set_threads(int(threads) if threads is not None else 0)
     keep = _Keep()
     atm = atmosphere_struct(cfg["atmosphere"], keep)
     det = detector_struct(cfg["detector"], keep)
