@@ -31,7 +31,7 @@
 extern "C" {
 #endif
 
-#define C8PH_VERSION 100
+#define C8PH_VERSION 200
 
 enum {
     C8PH_OK = 0,
@@ -100,7 +100,7 @@ typedef struct {
     float hist_x0, hist_y0, hist_cell;
     int32_t n_tel;                   /* telescope bounding spheres                        */
     const float *tel_xyzr;           /* HOST [n_tel][4] = centre x,y,z and radius; copied          */
-    int32_t cam_enabled;             /* camera on telescope 0: pixel x time-bin histogram          */
+    int32_t cam_enabled;             /* camera on the (single) telescope: pixel x time-bin histogram */
     float cam_axis_az_deg, cam_axis_el_deg, cam_pix_deg;
     int32_t cam_rows, cam_cols, n_tbins;
     double t_ref_ns;                 /* photon times are reported relative to t_ref               */
@@ -117,8 +117,9 @@ typedef struct {
     float opt_az_deg, opt_el_deg, opt_focal_m, opt_mirror_radius_m, opt_camera_radius_m;
 } c8ph_detector;
 /* Copies the telescope list and builds the two uniform-grid accelerators on the host (per cell: the
- * candidate telescopes sorted by a lower-bound key, the smallest key, an accept bound); synchronous.
- * LV2 margins up to 64 m are covered by the grid.                                                */
+ * candidate telescopes sorted by a lower-bound key, the smallest key, the nearest / first telescope in
+ * line); synchronous, so it takes no stream (SURVEY 8(b) lists one: the grids are built on the host).
+ * LV2 margins up to 64 m are covered by the grid.  cam_enabled needs exactly one telescope.        */
 int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *det);
 
 /* ---- run parameters --------------------------------------------------------------------------- */
@@ -136,20 +137,16 @@ typedef struct {
     float bunch_weight;                     /* photons per generated bunch (> 0)                  */
     float lv1_margin_rad, lv2_margin_m;
     float fluor_yield_per_MeV, aim_factor;  /* fluorescence: photons/MeV; forced-cone radius = aim_factor * r_tel */
-    int32_t n_lines;                        /* fluorescence line spectrum                         */
-    const float *line_nm, *line_cdf;        /* HOST [n_lines]; copied at every call               */
+                                            /* (fluorescence line spectrum: c8ph_set_line_spectrum) */
     /* Dispersion (thesis P:314-322, Eq. 2.5): n(lambda,h) - 1 = (n(h) - 1) D(lambda),
      * D = 1 + b (1/lambda^2 - 1/lambda0^2), the n(h) table being valid at lambda0.  The yield is the
      * integral over the band with the Heaviside threshold beta n(lambda) > 1, wavelengths follow
      * lambda^-2 sin^2 theta(lambda), the cone angle uses n(lambda, h_e).  b = 0: off; b >= 0.    */
     float disp_b_nm2, disp_lambda0_nm;
     /* Detector efficiency eps(lambda) (mirror x sensor, thesis P:360-366) folded into the
-     * survival probability / weight together with the atmospheric transmission: n_eff values in [0,1]
-     * on the uniform grid eff_lambda0_nm + i eff_dlambda_nm, linear between nodes, end values held
-     * outside.  n_eff = 0: off.  Needs trans != C8PH_TRANS_OFF.                                    */
-    int32_t n_eff;
-    float eff_lambda0_nm, eff_dlambda_nm;
-    const float *eff;                       /* HOST [n_eff]; copied at every call                  */
+     * survival probability / weight together with the atmospheric transmission: the table given to
+     * c8ph_set_efficiency.  0: off.  Needs trans != C8PH_TRANS_OFF.                                */
+    int32_t use_efficiency;
     /* Flat observation plane in the spherical model (thesis Fig. 4.10: the correction tables are
      * "relative to a flat observation plane"; R19).  The (height, zenith) table describes the ray
      * where it meets the observation SPHERE; 0: its displacement is applied at the straight-line point of
@@ -161,6 +158,15 @@ typedef struct {
     int32_t flat_plane;
 } c8ph_params;
 
+/* Wavelength tables of the context (set-up calls: synchronous, copied; the hot call then allocates and copies nothing).
+ * c8ph_set_line_spectrum: the discrete fluorescence spectrum (thesis P:340-344): n_lines wavelengths [nm] and
+ *   the cumulative line probabilities (non-decreasing, last = 1); needed by C8PH_EMIT_FLUORESCENCE.
+ * c8ph_set_efficiency: eps(lambda) in [0,1] on the uniform grid lambda0_nm + i dlambda_nm, linear between nodes, end
+ *   values held outside; used by calls with params.use_efficiency.  n = 0 removes the table.
+ * Not to be called while work that uses the table is still in flight on a stream.                             */
+int c8ph_set_line_spectrum(c8ph_ctx *ctx, int32_t n_lines, const float *line_nm, const float *line_cdf);
+int c8ph_set_efficiency(c8ph_ctx *ctx, int32_t n_eff, float lambda0_nm, float dlambda_nm, const float *eff);
+
 /* ---- segments, outputs ------------------------------------------------------------------------- */
 typedef struct {                            /* SoA, fp32, n_segments each, caller-owned            */
     uint32_t size;
@@ -168,6 +174,9 @@ typedef struct {                            /* SoA, fp32, n_segments each, calle
     const float *dx, *dy, *dz;              /* direction P (renormalised on the device)            */
     const float *len, *beta, *t0, *charge;  /* length, v/c, time at A, charge number               */
     const float *edep;                      /* MeV deposited (fluorescence) or NULL                */
+    const uint64_t *id;                     /* global segment ids (the Philox counter words) or NULL:
+                                               seg_id_base + i.  With ids the result does not depend on the order of
+                                               the segments in the arrays (record.seg stays the array index).          */
 } c8ph_segments;
 
 typedef struct {                            /* 32 B photon record                                  */
@@ -186,6 +195,7 @@ enum {
     C8PH_CNT_EMITTED, C8PH_CNT_UPGOING, C8PH_CNT_LV2, C8PH_CNT_TABLE_RANGE, C8PH_CNT_ROULETTE,
     C8PH_CNT_LANDED, C8PH_CNT_IN_GRID, C8PH_CNT_TEL_HIT, C8PH_CNT_CAM_HIT,
     C8PH_CNT_WRITTEN, C8PH_CNT_OVERFLOW, C8PH_CNT_CLIPPED,
+    C8PH_CNT_NONFINITE,        /* segments with a non-finite field or a zero direction: dropped, never silent        */
     C8PH_N_COUNTERS
 };
 
@@ -203,7 +213,11 @@ typedef struct {
  * the duration of the enqueued work only.  Asynchronous on `stream`; no allocation, no host sync
  * and no host<->device copy of bulk data.  Outputs are ACCUMULATED (caller zeroes them).  Results
  * depend only on (seed, seg_id_base + i, j): not on grid size, segment order or batching.
- * Photons that do not fit photon_capacity are still binned and counted in OVERFLOW.             */
+ * Photons that do not fit photon_capacity are still binned and counted in OVERFLOW.
+ * Launches of one context share its device scratch (work cursor, prepared-segment slots): the library orders a
+ * launch after the context's previous one when the two are on different streams (event wait), so calls from one host
+ * thread are safe on any streams; they do not run concurrently.  A stream that is being captured into a CUDA graph
+ * is not given that wait: keep the launches of one context in one capture stream.  Not thread-safe.          */
 int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *segments, int64_t n_segments,
                         int64_t seg_id_base, const c8ph_params *params, uint64_t seed,
                         const c8ph_outputs *out, void *stream);

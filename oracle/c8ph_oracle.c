@@ -84,6 +84,7 @@ typedef struct {
 
 typedef struct {
     const float *x, *y, *z, *dx, *dy, *dz, *len, *beta, *t0, *charge, *edep;
+    const uint64_t *id;            /* global segment ids (Philox counter words) or NULL: seg_id_base + i */
 } orc_segments;
 
 typedef struct {
@@ -133,7 +134,9 @@ typedef struct {
 
 enum { ORC_CNT_SEGMENTS = 0, ORC_CNT_SEG_BELOW_THRESHOLD, ORC_CNT_SEG_LV1, ORC_CNT_SEG_EMITTING,
        ORC_CNT_EMITTED, ORC_CNT_UPGOING, ORC_CNT_LV2, ORC_CNT_TABLE_RANGE, ORC_CNT_ROULETTE,
-       ORC_CNT_LANDED, ORC_CNT_IN_GRID, ORC_CNT_TEL_HIT, ORC_CNT_CAM_HIT, ORC_N_COUNTERS };
+       ORC_CNT_LANDED, ORC_CNT_IN_GRID, ORC_CNT_TEL_HIT, ORC_CNT_CAM_HIT,
+       ORC_CNT_NONFINITE,          /* segments with a non-finite field or a zero direction: dropped and counted */
+       ORC_N_COUNTERS };
 
 /* ------------------------------------------------------------------ O0 RNG
  * Philox4x32-10, Salmon et al. (the thesis' ref. [66], "counter
@@ -653,6 +656,16 @@ static double array_radius(const orc_detector *det)
     return r;
 }
 
+/* SURVEY 8(b) "NONFINITE": a segment with a non-finite input field or a direction of zero length is dropped. */
+static int segment_is_finite(const orc_segments *sg, int64_t i, int fluor)
+{
+    const double v[10] = { sg->x[i], sg->y[i], sg->z[i], sg->dx[i], sg->dy[i], sg->dz[i], sg->len[i], sg->beta[i],
+                           sg->t0[i], sg->charge[i] };
+    for (int k = 0; k < 10; ++k) if (!isfinite(v[k])) return 0;
+    if (fluor && sg->edep && !isfinite((double)sg->edep[i])) return 0;
+    return v[3]*v[3] + v[4]*v[4] + v[5]*v[5] > 0.0;
+}
+
 /* a1-a4 for one segment: ingest, LV1, yield, bunch count, rotation. */
 static void prepare_segment(const orc_atmosphere *atm, const orc_detector *det, const orc_params *par,
                             const orc_table *tab, const orc_segments *sg, int64_t i,
@@ -738,7 +751,8 @@ int64_t orc_count(const orc_atmosphere *atm, const orc_detector *det, const orc_
     #pragma omp parallel for schedule(static) reduction(+:total)
     for (int64_t i = 0; i < n_seg; ++i) {
         orc_segprep sp;
-        prepare_segment(atm, det, par, tab, sg, i, seed, (uint64_t)(seg_id_base + i), r_arr, &sp);
+        if (!segment_is_finite(sg, i, par->emit == ORC_EMIT_FLUOR)) { if (n_bunch) n_bunch[i] = 0; continue; }
+        prepare_segment(atm, det, par, tab, sg, i, seed, sg->id ? sg->id[i] : (uint64_t)(seg_id_base + i), r_arr, &sp);
         if (n_bunch) n_bunch[i] = sp.n_bunch;
         total += sp.n_bunch;
     }
@@ -769,9 +783,10 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
         #pragma omp for schedule(dynamic, 16)
         for (int64_t i = 0; i < n_seg; ++i) {
             orc_segprep sp;
-            uint64_t seg_id = (uint64_t)(seg_id_base + i);
-            prepare_segment(atm, det, par, tab, sg, i, seed, seg_id, r_arr, &sp);
+            uint64_t seg_id = sg->id ? sg->id[i] : (uint64_t)(seg_id_base + i);
             lc[ORC_CNT_SEGMENTS]++;
+            if (!segment_is_finite(sg, i, par->emit == ORC_EMIT_FLUOR)) { lc[ORC_CNT_NONFINITE]++; continue; }
+            prepare_segment(atm, det, par, tab, sg, i, seed, seg_id, r_arr, &sp);
             if (!(sp.n_exp > 0.0)) { lc[ORC_CNT_SEG_BELOW_THRESHOLD]++; continue; }
             if (sp.lv1_dropped) { lc[ORC_CNT_SEG_LV1]++; continue; }
             if (sp.n_bunch <= 0) continue;

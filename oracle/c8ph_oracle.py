@@ -52,7 +52,7 @@ class Table(C.Structure):
 
 class Segments(C.Structure):
     _fields_ = [(k, C.POINTER(C.c_float)) for k in
-                ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
+                ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")] + [("id", C.POINTER(C.c_uint64))]
 
 
 class Detector(C.Structure):
@@ -87,7 +87,7 @@ PHOTON_DTYPE = np.dtype([("seg", "<i8"), ("j", "<i4"), ("status", "<i4"),
                          ("bin", "<i4"), ("tel", "<i4"), ("pix", "<i4"), ("tbin", "<i4")], align=True)
 
 COUNTER_NAMES = ("segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "emitted", "upgoing",
-                 "lv2", "table_range", "roulette", "landed", "in_grid", "tel_hit", "cam_hit")
+                 "lv2", "table_range", "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "nonfinite")
 ST_LANDED, ST_UPGOING, ST_LV2, ST_TABLE_RANGE, ST_ROULETTE = range(5)
 
 _MODEL = {"homogeneous": 0, "planar": 1, "spherical": 2}
@@ -232,7 +232,12 @@ def params_struct(par: dict, keep: _Keep) -> Params:
 def segments_struct(seg: dict, keep: _Keep) -> Segments:
     s = Segments()
     for k, _ in Segments._fields_:
-        setattr(s, k, keep.f32(seg[k]))
+        if k != "id":
+            setattr(s, k, keep.f32(seg[k]))
+    if seg.get("id") is not None:                       # explicit global segment ids (else seg_id_base + i)
+        ids = np.ascontiguousarray(seg["id"], dtype=np.uint64)
+        keep.refs.append(ids)
+        s.id = ids.ctypes.data_as(C.POINTER(C.c_uint64))
     return s
 
 

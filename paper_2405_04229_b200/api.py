@@ -27,13 +27,13 @@ TABLE_CHANNELS = 5
 TEL_NONE = 0x3FFF
 COUNTER_NAMES = ("segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "emitted", "upgoing", "lv2",
                  "table_range", "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "written", "overflow",
-                 "clipped")
+                 "clipped", "nonfinite")
 N_COUNTERS = len(COUNTER_NAMES)
 
 EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8ph_init_atmosphere",
            "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
            "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
-           "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill")
+           "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill", "c8ph_set_line_spectrum", "c8ph_set_efficiency")
 
 PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
                          ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
@@ -74,15 +74,14 @@ class Params(C.Structure):
                 ("write", C.c_int32), ("filter_lv1", C.c_int32), ("filter_lv2", C.c_int32),
                 ("lambda_min_nm", C.c_float), ("lambda_max_nm", C.c_float), ("bunch_weight", C.c_float),
                 ("lv1_margin_rad", C.c_float), ("lv2_margin_m", C.c_float),
-                ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float), ("n_lines", C.c_int32),
-                ("line_nm", _fp), ("line_cdf", _fp), ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float),
-                ("n_eff", C.c_int32), ("eff_lambda0_nm", C.c_float), ("eff_dlambda_nm", C.c_float), ("eff", _fp),
-                ("flat_plane", C.c_int32)]
+                ("fluor_yield_per_MeV", C.c_float), ("aim_factor", C.c_float),
+                ("disp_b_nm2", C.c_float), ("disp_lambda0_nm", C.c_float),
+                ("use_efficiency", C.c_int32), ("flat_plane", C.c_int32)]
 
 
 class Segments(C.Structure):
     _fields_ = [("size", C.c_uint32)] + [(k, C.c_void_p) for k in
-                                          ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep")]
+                                          ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge", "edep", "id")]
 
 
 class SegmentsOut(C.Structure):
@@ -135,6 +134,8 @@ def load_library():
                                         C.c_void_p, C.c_void_p]
         L.c8ph_substep_fill.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(SubstepDesc),
                                         C.c_void_p, C.POINTER(SegmentsOut), C.c_void_p]
+        L.c8ph_set_line_spectrum.argtypes = [C.c_void_p, C.c_int32, _fp, _fp]
+        L.c8ph_set_efficiency.argtypes = [C.c_void_p, C.c_int32, C.c_float, C.c_float, _fp]
         L.c8ph_counter_name.argtypes = [C.c_int]
         L.c8ph_counter_name.restype = C.c_char_p
         _lib = L
@@ -267,18 +268,35 @@ class Context:
         p.lv1_margin_rad, p.lv2_margin_m = float(par["lv1_margin_rad"]), float(par["lv2_margin_m"])
         p.fluor_yield_per_MeV, p.aim_factor = float(par["fluor_yield_per_MeV"]), float(par["aim_factor"])
         p.disp_b_nm2, p.disp_lambda0_nm = float(par.get("disp_b_nm2", 0.0)), float(par.get("disp_lambda0_nm", 400.0))
-        ln, lc = _f32(par["line_nm"]), _f32(par["line_cdf"])
-        p.n_lines = len(ln)
-        if len(ln):
-            p.line_nm, p.line_cdf = ln.ctypes.data_as(_fp), lc.ctypes.data_as(_fp)
-        eff = par.get("eff")
-        ef = _f32(eff) if eff is not None and len(eff) else None
-        p.n_eff = 0 if ef is None else len(ef)
-        if ef is not None:
-            p.eff = ef.ctypes.data_as(_fp)
-        p.eff_lambda0_nm, p.eff_dlambda_nm = float(par.get("eff_lambda0_nm", 0.0)), float(par.get("eff_dlambda_nm", 1.0))
+        p.use_efficiency = int(par.get("eff") is not None and len(par["eff"]) > 0)
         p.flat_plane = int(bool(par.get("flat_plane", False)))
-        return p, (ln, lc, ef)
+        self._sync_spectra(par)
+        return p, None
+
+    # ---- wavelength tables of the context (set-up calls; the hot call copies nothing) ------------
+    def set_line_spectrum(self, line_nm, line_cdf):
+        ln, lc = _f32(line_nm), _f32(line_cdf)
+        self._check(self.lib.c8ph_set_line_spectrum(self._h, len(ln), ln.ctypes.data_as(_fp), lc.ctypes.data_as(_fp)))
+        self._lines_key = (ln.tobytes(), lc.tobytes())
+
+    def set_efficiency(self, eff, lambda0_nm: float, dlambda_nm: float):
+        ef = _f32(eff if eff is not None else [])
+        self._check(self.lib.c8ph_set_efficiency(self._h, len(ef), float(lambda0_nm), float(dlambda_nm),
+                                                 ef.ctypes.data_as(_fp) if len(ef) else None))
+        self._eff_key = (ef.tobytes(), float(lambda0_nm), float(dlambda_nm))
+
+    def _sync_spectra(self, par: dict):
+        """Convenience of this binding (marshalling only): a run-parameter dict may carry the line spectrum and the
+        efficiency table; they are handed to the library's set-up calls when they differ from what the context holds."""
+        if par["emit"] == "fluorescence" and len(par["line_nm"]):
+            key = (_f32(par["line_nm"]).tobytes(), _f32(par["line_cdf"]).tobytes())
+            if getattr(self, "_lines_key", None) != key:
+                self.set_line_spectrum(par["line_nm"], par["line_cdf"])
+        eff = par.get("eff")
+        if eff is not None and len(eff):
+            key = (_f32(eff).tobytes(), float(par.get("eff_lambda0_nm", 0.0)), float(par.get("eff_dlambda_nm", 1.0)))
+            if getattr(self, "_eff_key", None) != key:
+                self.set_efficiency(eff, key[1], key[2])
 
     # ---- the hot call, DEVICE buffers ------------------------------------------------------------
     def emit_propagate(self, seg_dev: dict, n_segments: int, seg_id_base: int, par: dict, seed: int,
@@ -291,6 +309,8 @@ class Context:
         for k in SEG_FIELDS:
             t = seg_dev.get(k)
             setattr(s, k, _dev_ptr(t, "float32", n_segments) if t is not None else None)
+        if seg_dev.get("id") is not None:                                # explicit global segment ids (int64 tensor)
+            s.id = _dev_ptr(seg_dev["id"], "int64", n_segments)
         o = Outputs()
         o.size = C.sizeof(Outputs)
         o.hist = _dev_ptr(out.get("hist"), "float32", self.n_hist())
@@ -330,6 +350,15 @@ class Context:
                 assert a.size >= n_segments
                 keep.append(a)
                 setattr(s, k, a.ctypes.data)
+        if seg_host.get("id") is not None:
+            ids = seg_host["id"]
+            if hasattr(ids, "data_ptr"):
+                assert str(ids.dtype) in ("torch.int64", "torch.uint64") and ids.is_contiguous() and ids.numel() >= n_segments
+                s.id = ids.data_ptr()
+            else:
+                ids = np.ascontiguousarray(ids, dtype=np.uint64)
+                s.id = ids.ctypes.data
+            keep.append(ids)
         if out is None:
             out = self.alloc_host_outputs(photon_capacity, want_weight)
         o = Outputs()
@@ -434,7 +463,10 @@ def setup_context(cfg: dict, device: int = 0, ctx: Optional[Context] = None) -> 
 
 def segments_to_device(seg: dict, device: int = 0) -> dict:
     import torch
-    return {k: torch.from_numpy(_f32(v)).to(f"cuda:{device}") for k, v in seg.items()}
+    out = {k: torch.from_numpy(_f32(v)).to(f"cuda:{device}") for k, v in seg.items() if k != "id"}
+    if seg.get("id") is not None:                                      # explicit global segment ids
+        out["id"] = torch.from_numpy(np.ascontiguousarray(seg["id"], dtype=np.uint64).view(np.int64)).to(f"cuda:{device}")
+    return out
 
 
 def alloc_device_outputs(ctx: Context, photon_capacity: int, want_weight: bool = False, device: int = 0) -> dict:

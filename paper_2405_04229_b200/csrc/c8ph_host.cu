@@ -49,15 +49,20 @@ struct c8ph_ctx {
     unsigned long long *d_cursor = nullptr;
     void *d_slots = nullptr;           // prepared-segment slots of the resident warps
     long long *d_bsums = nullptr;      // sub-stepping: block totals of the piece-count scan
-    float *d_lines = nullptr;          // [2][max_lines]
-    int lines_cap = 0;
-    float *d_eff = nullptr;            // detector efficiency table
-    int eff_cap = 0;
+    float *d_lines = nullptr;          // [2][n_lines]: wavelengths, cumulative probabilities (c8ph_set_line_spectrum)
+    int n_lines = 0;
+    float *d_eff = nullptr;            // detector efficiency table (c8ph_set_efficiency)
+    int n_eff = 0;
+    float eff_l0 = 0.f, eff_dl = 0.f;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev_done = nullptr;     // end of the context's last launch: a launch on another stream waits for it
+    cudaStream_t last_stream = nullptr;
+    bool have_launch = false;
     bool timed = false;
     int64_t launches = 0;
     // host-path scratch
     float *d_seg = nullptr; size_t seg_cap = 0;
+    uint64_t *d_ids = nullptr; size_t ids_cap = 0;
     void *d_out = nullptr; size_t out_cap = 0;
     cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
     unsigned long long *h_written = nullptr;    // pinned: photon-list cursor after each chunk
@@ -111,7 +116,8 @@ extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
         (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_slots, segment_slot_bytes(ctx->n_sm))) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_bsums, kSubstepBlockSums * sizeof(long long))) != cudaSuccess ||
-        (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess) {
+        (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&ctx->ev_done, cudaEventDisableTiming)) != cudaSuccess) {
         g_create_err = std::string("c8ph_create: ") + cudaGetErrorString(e);
         delete ctx;
         return C8PH_E_CUDA;
@@ -131,7 +137,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
     dfree(ctx->d_g_kq); dfree(ctx->d_g_first); dfree(ctx->d_g_first_kn);
     dfree(ctx->d_g_knear);
-    dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg);
+    dfree(ctx->d_cursor); dfree(ctx->d_lines); dfree(ctx->d_eff); dfree(ctx->d_seg); dfree(ctx->d_ids);
     if (ctx->d_slots) { cudaFree(ctx->d_slots); ctx->d_slots = nullptr; }
     dfree(ctx->d_bsums);
     if (ctx->d_out) { cudaFree(ctx->d_out); ctx->d_out = nullptr; }
@@ -142,6 +148,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     }
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->ev_done) cudaEventDestroy(ctx->ev_done);
     delete ctx;
     return C8PH_OK;
 }
@@ -516,8 +523,8 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
     if (d->hist_nx < 0 || d->hist_ny < 0 || (int64_t)d->hist_nx * d->hist_ny > (1ll << 30)) return fail(ctx, C8PH_E_ARG, "set_detector: hist size");
     if ((d->hist_nx > 0) != (d->hist_ny > 0) || (d->hist_nx > 0 && !(d->hist_cell > 0.f))) return fail(ctx, C8PH_E_ARG, "set_detector: hist grid");
     if (d->n_tel < 0 || d->n_tel >= (int)C8PH_TEL_NONE || (d->n_tel > 0 && !d->tel_xyzr)) return fail(ctx, C8PH_E_ARG, "set_detector: telescopes");
-    if (d->cam_enabled && (d->n_tel < 1 || d->cam_rows < 1 || d->cam_cols < 1 || d->n_tbins < 1 || !(d->cam_pix_deg > 0.f) || !(d->t_bin_ns > 0.f)))
-        return fail(ctx, C8PH_E_ARG, "set_detector: camera needs a telescope, rows, cols, time bins");
+    if (d->cam_enabled && (d->n_tel != 1 || d->cam_rows < 1 || d->cam_cols < 1 || d->n_tbins < 1 || !(d->cam_pix_deg > 0.f) || !(d->t_bin_ns > 0.f)))
+        return fail(ctx, C8PH_E_ARG, "set_detector: camera needs exactly one telescope, rows, cols, time bins");
     if (d->opt_enabled) {
         if (d->cam_enabled || d->n_tel < 1 || !(d->opt_focal_m > 0.f) || !(d->opt_mirror_radius_m > 0.f) || !(d->opt_camera_radius_m > 0.f))
             return fail(ctx, C8PH_E_ARG, "set_detector: optics need telescopes, focal length, mirror and camera radius; not with cam_enabled");
@@ -582,9 +589,50 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
     return C8PH_OK;
 }
 
+// ------------------------------------------------------------------------------------ wavelength tables
+extern "C" int c8ph_set_line_spectrum(c8ph_ctx *ctx, int32_t n_lines, const float *line_nm, const float *line_cdf)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (n_lines < 0 || n_lines > (1 << 20) || (n_lines > 0 && (!line_nm || !line_cdf))) return fail(ctx, C8PH_E_ARG, "set_line_spectrum: n_lines / NULL array");
+    for (int k = 0; k < n_lines; ++k) {
+        if (!(line_nm[k] > 0.f) || !std::isfinite(line_nm[k])) return fail(ctx, C8PH_E_ARG, "set_line_spectrum: wavelength <= 0 or not finite");
+        if (!(line_cdf[k] >= 0.f && line_cdf[k] <= 1.f) || (k > 0 && line_cdf[k] < line_cdf[k - 1])) return fail(ctx, C8PH_E_ARG, "set_line_spectrum: cdf must rise from >= 0 to 1");
+    }
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaDeviceSynchronize());                               // nothing in flight may still read the old table
+    dfree(ctx->d_lines);
+    ctx->n_lines = 0;
+    if (n_lines > 0) {
+        CU(cudaMalloc(&ctx->d_lines, 2 * (size_t)n_lines * sizeof(float)));
+        CU(cudaMemcpy(ctx->d_lines, line_nm, n_lines * sizeof(float), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->d_lines + n_lines, line_cdf, n_lines * sizeof(float), cudaMemcpyHostToDevice));
+        ctx->n_lines = n_lines;
+    }
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_set_efficiency(c8ph_ctx *ctx, int32_t n_eff, float lambda0_nm, float dlambda_nm, const float *eff)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (n_eff < 0 || n_eff > (1 << 20) || (n_eff > 0 && !eff) || (n_eff > 1 && !(dlambda_nm > 0.f)))
+        return fail(ctx, C8PH_E_ARG, "set_efficiency: needs eff and dlambda_nm > 0");
+    for (int k = 0; k < n_eff; ++k)
+        if (!(eff[k] >= 0.f && eff[k] <= 1.f)) return fail(ctx, C8PH_E_ARG, "set_efficiency: efficiency outside [0,1]");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaDeviceSynchronize());
+    dfree(ctx->d_eff);
+    ctx->n_eff = 0;
+    if (n_eff > 0) {
+        CU(cudaMalloc(&ctx->d_eff, (size_t)n_eff * sizeof(float)));
+        CU(cudaMemcpy(ctx->d_eff, eff, (size_t)n_eff * sizeof(float), cudaMemcpyHostToDevice));
+        ctx->n_eff = n_eff; ctx->eff_l0 = lambda0_nm; ctx->eff_dl = dlambda_nm;
+    }
+    return C8PH_OK;
+}
+
 // ------------------------------------------------------------------------------------ the hot call
 static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64_t base, const c8ph_params *p,
-                     uint64_t seed, const c8ph_outputs *o, KArgs &a, cudaStream_t st)
+                     uint64_t seed, const c8ph_outputs *o, KArgs &a)
 {
     if (!s || s->size != sizeof(c8ph_segments) || !p || p->size != sizeof(c8ph_params) || !o || o->size != sizeof(c8ph_outputs))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: NULL struct or size mismatch");
@@ -611,13 +659,11 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
         return fail(ctx, C8PH_E_ARG, "emit_propagate: WRITE_ALL is not defined with last-mile optics (records are camera hits)");
     if (!(p->disp_b_nm2 >= 0.f) || (p->disp_b_nm2 > 0.f && !(p->disp_lambda0_nm > 0.f)))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: dispersion needs disp_b_nm2 >= 0 and disp_lambda0_nm > 0");
-    if (p->n_eff < 0 || (p->n_eff > 0 && (!p->eff || p->trans == C8PH_TRANS_OFF || (p->n_eff > 1 && !(p->eff_dlambda_nm > 0.f)))))
-        return fail(ctx, C8PH_E_ARG, "emit_propagate: efficiency table needs eff, eff_dlambda_nm > 0 and a transmission mode");
-    for (int k = 0; k < p->n_eff; ++k)
-        if (!(p->eff[k] >= 0.f && p->eff[k] <= 1.f)) return fail(ctx, C8PH_E_ARG, "emit_propagate: efficiency outside [0,1]");
+    if (p->use_efficiency && ctx->n_eff < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: use_efficiency without c8ph_set_efficiency");
+    if (p->use_efficiency && p->trans == C8PH_TRANS_OFF) return fail(ctx, C8PH_E_ARG, "emit_propagate: the efficiency table needs a transmission mode");
     if (p->emit == C8PH_EMIT_FLUORESCENCE) {
         if (ctx->det.n_tel < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: fluorescence needs a telescope to aim at");
-        if (p->n_lines < 1 || !p->line_nm || !p->line_cdf) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence line spectrum");
+        if (ctx->n_lines < 1) return fail(ctx, C8PH_E_STATE, "emit_propagate: fluorescence needs c8ph_set_line_spectrum");
         if (n_seg > 0 && !s->edep) return fail(ctx, C8PH_E_ARG, "emit_propagate: edep is NULL");
     }
     if (p->filter_lv2 && (!(p->lv2_margin_m >= 0.f) || (p->lv2_margin_m > (float)kLv2MarginMax && ctx->det.use_grid)))
@@ -659,32 +705,14 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
     r.force_generic = ctx->force_generic ? 1 : 0;
     r.flat_plane = (p->flat_plane && ctx->atm.model == C8PH_ATM_SPHERICAL && p->trace != C8PH_TRACE_STRAIGHT) ? 1 : 0;
-    r.n_eff = p->n_eff; r.eff = nullptr;
-    r.eff_l0 = p->eff_lambda0_nm; r.eff_inv_dl = p->n_eff > 1 ? 1.0f / p->eff_dlambda_nm : 0.f;
-    if (p->n_eff > 0) {
-        if (p->n_eff > ctx->eff_cap) {
-            dfree(ctx->d_eff);
-            CU(cudaMalloc(&ctx->d_eff, (size_t)p->n_eff * sizeof(float)));
-            ctx->eff_cap = p->n_eff;
-        }
-        CU(cudaMemcpyAsync(ctx->d_eff, p->eff, (size_t)p->n_eff * sizeof(float), cudaMemcpyHostToDevice, st));
-        r.eff = ctx->d_eff;
-    }
+    r.n_eff = p->use_efficiency ? ctx->n_eff : 0; r.eff = p->use_efficiency ? ctx->d_eff : nullptr;
+    r.eff_l0 = ctx->eff_l0; r.eff_inv_dl = ctx->n_eff > 1 ? 1.0f / ctx->eff_dl : 0.f;
     r.disp_b = p->emit == C8PH_EMIT_CHERENKOV ? p->disp_b_nm2 : 0.f;
     r.disp_k0sq = r.disp_b > 0.f ? 1.0 / ((double)p->disp_lambda0_nm * (double)p->disp_lambda0_nm) : 0.0;
     r.disp_c0 = (float)(1.0 - (double)r.disp_b * r.disp_k0sq);
     r.il1_d = p->emit == C8PH_EMIT_CHERENKOV ? 1.0 / (double)p->lambda_min_nm : 0.0;
     r.il2_d = p->emit == C8PH_EMIT_CHERENKOV ? 1.0 / (double)p->lambda_max_nm : 0.0;
-    if (p->emit == C8PH_EMIT_FLUORESCENCE) {
-        if (p->n_lines > ctx->lines_cap) {
-            dfree(ctx->d_lines);
-            CU(cudaMalloc(&ctx->d_lines, 2 * (size_t)p->n_lines * sizeof(float)));
-            ctx->lines_cap = p->n_lines;
-        }
-        CU(cudaMemcpyAsync(ctx->d_lines, p->line_nm, p->n_lines * sizeof(float), cudaMemcpyHostToDevice, st));
-        CU(cudaMemcpyAsync(ctx->d_lines + ctx->lines_cap, p->line_cdf, p->n_lines * sizeof(float), cudaMemcpyHostToDevice, st));
-        r.n_lines = p->n_lines; r.line_nm = ctx->d_lines; r.line_cdf = ctx->d_lines + ctx->lines_cap;
-    }
+    if (p->emit == C8PH_EMIT_FLUORESCENCE) { r.n_lines = ctx->n_lines; r.line_nm = ctx->d_lines; r.line_cdf = ctx->d_lines + ctx->n_lines; }
     for (int k = 0; k < 10; ++k) {
         r.key0[k] = (uint32_t)seed + (uint32_t)k * 0x9E3779B9u;
         r.key1[k] = (uint32_t)(seed >> 32) + (uint32_t)k * 0xBB67AE85u;
@@ -712,8 +740,32 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     return C8PH_OK;
 }
 
+// Launches of one context share the work cursor and the prepared-segment slots: a launch on another stream than the
+// previous one first waits for that one's end event (a capturing stream is left alone: see c8ph.h).
+static int order_after_last_launch(c8ph_ctx *ctx, cudaStream_t st)
+{
+    if (ctx->have_launch && st != ctx->last_stream) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+        if (cs == cudaStreamCaptureStatusNone) CU(cudaStreamWaitEvent(st, ctx->ev_done, 0));
+    }
+    return C8PH_OK;
+}
+static int mark_launch_end(c8ph_ctx *ctx, cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+    if (cs == cudaStreamCaptureStatusNone) {
+        CU(cudaEventRecord(ctx->ev_done, st));
+        ctx->last_stream = st; ctx->have_launch = true;
+    }
+    return C8PH_OK;
+}
+
 static int launch(c8ph_ctx *ctx, const KArgs &a, cudaStream_t st)
 {
+    int rc = order_after_last_launch(ctx, st);
+    if (rc) return rc;
     CU(cudaMemsetAsync(ctx->d_cursor, 0, sizeof(unsigned long long), st));
     CU(cudaEventRecord(ctx->ev0, st));
     cudaError_t e = launch_emit_propagate(a, ctx->n_sm, st);
@@ -721,7 +773,7 @@ static int launch(c8ph_ctx *ctx, const KArgs &a, cudaStream_t st)
     CU(cudaEventRecord(ctx->ev1, st));
     ctx->timed = true;
     ctx->launches++;
-    return C8PH_OK;
+    return mark_launch_end(ctx, st);
 }
 
 extern "C" int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64_t base,
@@ -731,7 +783,7 @@ extern "C" int c8ph_emit_propagate(c8ph_ctx *ctx, const c8ph_segments *s, int64_
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaSetDevice(ctx->device));
     KArgs a{};
-    int rc = make_args(ctx, s, n_seg, base, p, seed, o, a, st);
+    int rc = make_args(ctx, s, n_seg, base, p, seed, o, a);
     if (rc) return rc;
     if (n_seg == 0) return C8PH_OK;
     return launch(ctx, a, st);
@@ -765,6 +817,11 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         dfree(ctx->d_seg);
         CU(cudaMalloc(&ctx->d_seg, std::max<size_t>(1, 11 * npad) * sizeof(float)));
         ctx->seg_cap = 11 * npad;
+    }
+    if (hs->id && n > ctx->ids_cap) {
+        dfree(ctx->d_ids);
+        CU(cudaMalloc(&ctx->d_ids, n * sizeof(uint64_t)));
+        ctx->ids_cap = n;
     }
     // device outputs in one arena: counters | hist | tel_counts | photon_weight | photons
     const DevDet &det = ctx->det;
@@ -805,17 +862,20 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         for (int k = 0; k < 11; ++k)
             if (src[k] && hi > lo)
                 CU(cudaMemcpyAsync(ctx->d_seg + k * npad + lo, src[k] + lo, (hi - lo) * sizeof(float), cudaMemcpyHostToDevice, s_in));
+        if (hs->id && hi > lo) CU(cudaMemcpyAsync(ctx->d_ids + lo, hs->id + lo, (hi - lo) * sizeof(uint64_t), cudaMemcpyHostToDevice, s_in));
         CU(cudaEventRecord(ctx->ev_in[c], s_in));
         CU(cudaStreamWaitEvent(s_run, ctx->ev_in[c], 0));
         c8ph_segments ds{};
         ds.size = sizeof(ds);
         const float **dp[11] = {&ds.x, &ds.y, &ds.z, &ds.dx, &ds.dy, &ds.dz, &ds.len, &ds.beta, &ds.t0, &ds.charge, &ds.edep};
         for (int k = 0; k < 11; ++k) *dp[k] = src[k] ? ctx->d_seg + k * npad + lo : nullptr;
+        ds.id = hs->id ? ctx->d_ids + lo : nullptr;
         KArgs a{};
-        int rc = make_args(ctx, &ds, (int64_t)(hi - lo), base + (int64_t)lo, p, seed, &dout, a, s_run);
+        int rc = make_args(ctx, &ds, (int64_t)(hi - lo), base + (int64_t)lo, p, seed, &dout, a);
         if (rc) { cudaDeviceSynchronize(); return rc; }
         a.run.local_base = (uint32_t)lo;
         if (hi > lo) {
+            if (first) { rc = order_after_last_launch(ctx, s_run); if (rc) { cudaDeviceSynchronize(); return rc; } }
             CU(cudaMemsetAsync(ctx->d_cursor, 0, sizeof(unsigned long long), s_run));
             if (first) CU(cudaEventRecord(ctx->ev0, s_run));
             first = false;
@@ -826,7 +886,7 @@ extern "C" int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *hs, 
         CU(cudaMemcpyAsync(&ctx->h_written[c], &dout.counters[C8PH_CNT_WRITTEN], sizeof(unsigned long long), cudaMemcpyDeviceToHost, s_run));
         CU(cudaEventRecord(ctx->ev_run[c], s_run));
     }
-    if (!first) { CU(cudaEventRecord(ctx->ev1, s_run)); ctx->timed = true; }
+    if (!first) { CU(cudaEventRecord(ctx->ev1, s_run)); ctx->timed = true; int rc2 = mark_launch_end(ctx, s_run); if (rc2) return rc2; }
     // photons: as soon as a chunk's kernel is done its records [written before, written after) go home
     size_t done = 0;
     for (int c = 0; c < n_chunks && cap; ++c) {
@@ -928,6 +988,6 @@ extern "C" const char *c8ph_counter_name(int i)
 {
     static const char *names[C8PH_N_COUNTERS] = {
         "segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "emitted", "upgoing", "lv2", "table_range",
-        "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "written", "overflow", "clipped"};
+        "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "written", "overflow", "clipped", "nonfinite"};
     return (i >= 0 && i < C8PH_N_COUNTERS) ? names[i] : "";
 }

@@ -489,7 +489,7 @@ __device__ __noinline__ void line_general(const SegCold *sc, float s, float D, f
 }
 
 // per-warp event counters kept in shared memory (u64), flushed to the global counters at the end
-enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_EMITTED, WC_UP, WC_LV2, WC_TR, WC_ROUL, WC_GRID, WC_TEL,
+enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_NONFINITE, WC_EMITTED, WC_UP, WC_LV2, WC_TR, WC_ROUL, WC_GRID, WC_TEL,
        WC_CAM, WC_WRITTEN, WC_OVERFLOW, WC_N };
 
 // ================================================================================================
@@ -787,7 +787,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         int myN = 0;
         {
             const long long i = (long long)g0 + lane;
-            bool below = false, lv1_drop = false, clipped = false;
+            bool below = false, lv1_drop = false, clipped = false, nonfinite = false;
             if (lane < run.segs_per_grab && i < run.n_seg) {
                 SegHot me;
                 SegCold mc;
@@ -797,7 +797,13 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 const double L = __ldcs(run.seg.len + i), beta = __ldcs(run.seg.beta + i), t0 = __ldcs(run.seg.t0 + i);
                 const double pn = 1.0 / sqrt(Px * Px + Py * Py + Pz * Pz);
                 Px *= pn; Py *= pn; Pz *= pn;
-                const unsigned long long gid = (unsigned long long)(run.seg_id_base + i);
+                // a non-finite input field or a zero direction: the segment is dropped and counted (C8PH_CNT_NONFINITE)
+                {
+                    double chk = Ax + Ay + Az + Px + Py + Pz + L + beta + t0 + (double)__ldcs(run.seg.charge + i);
+                    if (EMIT == C8PH_EMIT_FLUORESCENCE && run.seg.edep) chk += (double)run.seg.edep[i];
+                    nonfinite = !(fabs(chk) < CUDART_INF);
+                }
+                const unsigned long long gid = run.seg.id ? (unsigned long long)__ldcs(run.seg.id + i) : (unsigned long long)(run.seg_id_base + i);
                 me.id_lo = (uint32_t)gid; me.id_hi = (uint32_t)(gid >> 32); mc.local = run.local_base + (uint32_t)i;
                 // local vertical and height at A and at the midpoint
                 double rx = 0.0, ry = 0.0, rz = 1.0, rA = 1.0, hA, h_mid;
@@ -898,7 +904,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     mc.eta_mid = 0.f;
                 }
                 long long N = 0;
-                if (!(n_exp > 0.0)) below = true;
+                if (nonfinite) { n_exp = 0.0; lv1_drop = false; }
+                else if (!(n_exp > 0.0)) below = true;
                 else if (!lv1_drop) {
                     N = (long long)floor(n_exp / (double)run.w + u01d(rs.x));
                     if (N >= C8PH_MAX_BUNCHES_PER_SEGMENT) { clipped = true; N = C8PH_MAX_BUNCHES_PER_SEGMENT - 1; }
@@ -983,11 +990,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             }
             // segment-level counters of the group: one ballot each, lane 0 books them
             const unsigned mb = __ballot_sync(FULL, below), ml = __ballot_sync(FULL, lv1_drop), mcl = __ballot_sync(FULL, clipped);
-            const unsigned me_ = __ballot_sync(FULL, myN > 0);
+            const unsigned me_ = __ballot_sync(FULL, myN > 0), mnf = __ballot_sync(FULL, nonfinite);
             const uint32_t nsum = __reduce_add_sync(FULL, (uint32_t)myN);
             if (lane == 0) {
                 s_cnt[warp][WC_BELOW] += __popc(mb); s_cnt[warp][WC_LV1] += __popc(ml);
                 s_cnt[warp][WC_CLIPPED] += __popc(mcl); s_cnt[warp][WC_EMITTING] += __popc(me_);
+                s_cnt[warp][WC_NONFINITE] += __popc(mnf);
                 s_cnt[warp][WC_EMITTED] += nsum;
             }
         }
@@ -1402,6 +1410,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         add(C8PH_CNT_SEG_LV1, c[WC_LV1]);
         add(C8PH_CNT_SEG_EMITTING, c[WC_EMITTING]);
         add(C8PH_CNT_CLIPPED, c[WC_CLIPPED]);
+        add(C8PH_CNT_NONFINITE, c[WC_NONFINITE]);
         add(C8PH_CNT_EMITTED, c[WC_EMITTED]);
         add(C8PH_CNT_UPGOING, c[WC_UP]);
         add(C8PH_CNT_LV2, c[WC_LV2]);

@@ -35,7 +35,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 
 def test_version_and_counter_names(lib):
-    assert lib.c8ph_version() == 100
+    assert lib.c8ph_version() == 200
     got = [lib.c8ph_counter_name(i).decode() for i in range(api.N_COUNTERS)]
     assert tuple(got) == api.COUNTER_NAMES
     assert lib.c8ph_counter_name(api.N_COUNTERS) == b""
@@ -47,8 +47,8 @@ def test_struct_layouts_match_the_header(tmp_path):
         "c8ph_atmosphere_desc": (api.AtmosphereDesc, ["size", "refractivity", "earth_radius_m", "aer_angstrom", "n_ext_lambda", "ext_tau_v"]),
         "c8ph_table_desc": (api.TableDesc, ["size", "h_max_m", "substeps"]),
         "c8ph_detector": (api.Detector, ["size", "tel_xyzr", "cam_enabled", "t_ref_ns", "t_bin_ns", "opt_enabled", "opt_camera_radius_m"]),
-        "c8ph_params": (api.Params, ["size", "write", "bunch_weight", "n_lines", "line_cdf", "disp_lambda0_nm", "n_eff", "eff", "flat_plane"]),
-        "c8ph_segments": (api.Segments, ["size", "x", "edep"]),
+        "c8ph_params": (api.Params, ["size", "write", "bunch_weight", "aim_factor", "disp_lambda0_nm", "use_efficiency", "flat_plane"]),
+        "c8ph_segments": (api.Segments, ["size", "x", "edep", "id"]),
         "c8ph_outputs": (api.Outputs, ["size", "hist", "photon_capacity", "counters"]),
         "c8ph_substep_desc": (api.SubstepDesc, ["size", "B_tesla", "tol_m", "ms_enabled", "ms_X0_gcm2", "seed", "track_id_base"]),
         "c8ph_segments_out": (api.SegmentsOut, ["size", "x", "edep"]),

@@ -496,6 +496,40 @@ def test_segment_order_and_batching_independence():
         assert np.array_equal(a[f], b[f])
 
 
+def test_explicit_segment_ids_make_the_order_irrelevant_and_non_finite_segments_are_dropped():
+    """O0 / SURVEY 8(b): the Philox counter carries the segment id; handed over explicitly, a shuffled segment list gives
+    the photons of the ordered one (mapped back by index).  A segment with a non-finite field or a zero direction is
+    dropped and counted; the others keep their photons (ids unchanged)."""
+    cfg = W.make_config(0, n_segments=96)
+    full = O.run(cfg)
+    perm = np.random.default_rng(3).permutation(96)
+    sh = copy.deepcopy(cfg)
+    sh["segments"] = {f: np.ascontiguousarray(v[perm]) for f, v in cfg["segments"].items()}
+    sh["segments"]["id"] = perm.astype(np.uint64)
+    got = O.run(sh)
+    assert got["counters"] == full["counters"] and np.array_equal(got["hist"], full["hist"])
+    a, b = full["photons"], got["photons"].copy()
+    b["seg"] = perm[b["seg"]]
+    a, b = a[np.lexsort((a["j"], a["seg"]))], b[np.lexsort((b["j"], b["seg"]))]
+    for f in ("seg", "j", "x", "y", "t", "lambda_nm", "ux", "uy", "uz", "bin"):
+        assert np.array_equal(a[f], b[f]), f
+    # ids without shuffling = seg_id_base + i
+    ident = copy.deepcopy(cfg)
+    ident["segments"]["id"] = np.arange(96, dtype=np.uint64)
+    assert np.array_equal(O.run(ident)["photons"], full["photons"])
+    bad = copy.deepcopy(cfg)
+    bad["segments"]["z"][5] = np.nan
+    bad["segments"]["beta"][6] = np.inf
+    for f in ("dx", "dy", "dz"):
+        bad["segments"][f][7] = 0.0
+    res = O.run(bad)
+    assert res["counters"]["nonfinite"] == 3 and full["counters"]["nonfinite"] == 0
+    assert res["counters"]["segments"] == 96
+    keep = ~np.isin(full["photons"]["seg"], (5, 6, 7))
+    assert np.array_equal(res["photons"], full["photons"][keep])
+    assert np.isfinite(res["hist"]).all()
+
+
 def test_filters_are_lossless_and_roulette_unbiased():
     cfg = W.make_config(2, n_segments=3000)
     on = O.run(cfg)
