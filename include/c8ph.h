@@ -242,7 +242,8 @@ int c8ph_emit_propagate_host(c8ph_ctx *ctx, const c8ph_segments *host_segments, 
  * width theta0 = 13.6 MeV/(beta c p) |z| sqrt(t)(1 + 0.038 ln(t z^2/beta^2)), t = rho(h) ds / X0, and
  * per transverse plane the correlated Gaussian offset / deflection pair, drawn from Philox
  * (seed; piece index, track_id_base + i, stream 16): a random walk from piece to piece.  Needs the
- * atmosphere (overburden table) of the context for the density.  n <= max_sub.
+ * atmosphere (overburden table) of the context for the density.  n <= max_sub <= 2^20 (tracks that would need
+ * more are counted in desc->clipped).  A track of length 0 gives one piece of length 0 along its direction.
  * Two calls, both asynchronous on `stream`, no allocation:
  *   c8ph_substep_plan  writes offsets[0..n_tracks] (exclusive prefix sum of the piece counts); the
  *                      caller reads offsets[n_tracks] to size the segment arrays;
@@ -259,6 +260,8 @@ typedef struct {
     float ms_max_step_m, ms_X0_gcm2;        /* piece length bound; radiation length (air: 36.62)   */
     uint64_t seed;
     int64_t track_id_base;
+    uint64_t *clipped;                      /* DEVICE counter or NULL; c8ph_substep_plan adds the number of tracks whose
+                                               bounds asked for more than max_sub pieces (they get max_sub): never silent */
 } c8ph_substep_desc;
 int c8ph_substep_plan(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
                       const c8ph_substep_desc *desc, int64_t *offsets, void *stream);

@@ -18,7 +18,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "c8ph_oracle.c")
-_LIB = os.path.join(_HERE, "libc8ph_oracle.so")
+# C8PH_ORACLE_SANITIZE=1 (set before the first call): the oracle is compiled with -fsanitize=address,undefined into its
+# own file and loaded from there (the process needs libasan preloaded); used once by tests/test_oracle_pins.py.
+_SAN = os.environ.get("C8PH_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "libc8ph_oracle_san.so" if _SAN else "libc8ph_oracle.so")
 _lock = threading.Lock()
 _lib = None
 
@@ -27,7 +30,8 @@ def build(force: bool = False) -> str:
     """Compile the oracle (plain C, -O2, no fast-math, OpenMP over segments)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+        san = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
+        subprocess.check_call(["gcc", *san, "-std=c11", "-fPIC", "-shared", "-fopenmp",
                                "-fno-fast-math", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB

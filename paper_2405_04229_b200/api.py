@@ -92,7 +92,7 @@ class SegmentsOut(C.Structure):
 class SubstepDesc(C.Structure):
     _fields_ = [("size", C.c_uint32), ("B_tesla", C.c_float * 3), ("tol_m", C.c_float), ("max_sub", C.c_int32),
                 ("ms_enabled", C.c_int32), ("ms_max_step_m", C.c_float), ("ms_X0_gcm2", C.c_float),
-                ("seed", C.c_uint64), ("track_id_base", C.c_int64)]
+                ("seed", C.c_uint64), ("track_id_base", C.c_int64), ("clipped", C.c_void_p)]
 
 
 class Outputs(C.Structure):
@@ -412,6 +412,9 @@ class Context:
         d.ms_max_step_m = 0.0 if ms_max_step_m is None else float(ms_max_step_m)
         d.ms_X0_gcm2, d.seed, d.track_id_base = float(ms_X0_gcm2), int(seed), int(track_id_base)
         offsets = torch.zeros(n_tracks + 1, dtype=torch.int64, device=dev)
+        clipped = torch.zeros(1, dtype=torch.int64, device=dev)          # tracks clipped to max_sub pieces (read via .clipped_tracks)
+        d.clipped = clipped.data_ptr()
+        self.clipped_tracks = clipped
         self._check(self.lib.c8ph_substep_plan(self._h, C.byref(t), p, int(n_tracks), C.byref(d),
                                                offsets.data_ptr(), _stream_ptr(stream)))
         total = int(offsets[-1].item())

@@ -156,6 +156,7 @@ struct SubstepArgs {
     double tol;
     int max_sub;
     long long *offsets;             // [n+1]
+    unsigned long long *clipped;    // DEVICE counter (plan only) or NULL: += tracks clipped to max_sub pieces
     c8ph_segments_out out;          // DEVICE (fill only)
     int ms_enabled;                 // multiple-scattering sub-steps (R18)
     double ms_max_step, ms_X0;

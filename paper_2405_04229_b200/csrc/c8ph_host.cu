@@ -918,7 +918,7 @@ static int substep_args(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_Ge
     if (n < 0 || substep_scratch_elems(n) > kSubstepBlockSums) return fail(ctx, C8PH_E_ARG, "substep: n_tracks out of range (<= 2^27 per call)");
     if (n > 0 && (!t->x || !t->y || !t->z || !t->dx || !t->dy || !t->dz || !t->len || !t->beta || !t->t0 || !t->charge || !p_GeV))
         return fail(ctx, C8PH_E_ARG, "substep: NULL track array");
-    if (!(d->tol_m > 0.f) || d->max_sub < 1) return fail(ctx, C8PH_E_ARG, "substep: tol_m > 0 and max_sub >= 1 required");
+    if (!(d->tol_m > 0.f) || d->max_sub < 1 || d->max_sub > (1 << 20)) return fail(ctx, C8PH_E_ARG, "substep: tol_m > 0 and 1 <= max_sub <= 2^20 required");
     if (d->ms_enabled) {
         if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "substep: multiple scattering needs the atmosphere (overburden) of the context");
         if (!(d->ms_X0_gcm2 > 0.f) || !(d->ms_max_step_m >= 0.f) || d->track_id_base < 0)
@@ -930,6 +930,7 @@ static int substep_args(c8ph_ctx *ctx, const c8ph_segments *t, const float *p_Ge
     a.tol = d->tol_m; a.max_sub = d->max_sub;
     a.ms_enabled = d->ms_enabled ? 1 : 0; a.ms_max_step = d->ms_max_step_m; a.ms_X0 = d->ms_X0_gcm2;
     a.id_base = d->track_id_base;
+    a.clipped = reinterpret_cast<unsigned long long *>(d->clipped);
     for (int k = 0; k < 10; ++k)
         a.key[k] = make_uint2((uint32_t)d->seed + (uint32_t)k * 0x9E3779B9u, (uint32_t)(d->seed >> 32) + (uint32_t)k * 0xBB67AE85u);
     if (ctx->have_atm) a.atm = ctx->atm;

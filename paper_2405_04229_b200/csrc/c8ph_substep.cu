@@ -46,18 +46,23 @@ __device__ __forceinline__ Helix helix_of(const SubstepArgs &a, long long i)
 }
 
 // number of pieces: sagitta L_piece^2 curvature / 8 <= tol, and (multiple scattering) L_piece <= ms_max_step
-__device__ __forceinline__ int pieces_of(const Helix &h, const SubstepArgs &a)
+// `clipped` is set when the bounds ask for more than max_sub pieces (the track then gets max_sub: counted, never silent)
+__device__ __forceinline__ int pieces_of(const Helix &h, const SubstepArgs &a, bool *clipped = nullptr)
 {
     int n = 1;
+    bool cl = false;
     if (h.curv > 0.0 && h.L > 0.0) {
         const double nn = ceil(h.L / sqrt(8.0 * a.tol / h.curv));
-        n = nn < 1.0 ? 1 : (nn > (double)a.max_sub ? a.max_sub : (int)nn);
+        cl = nn > (double)a.max_sub;
+        n = nn < 1.0 ? 1 : (cl ? a.max_sub : (int)nn);
     }
     if (a.ms_enabled && a.ms_max_step > 0.0 && h.L > 0.0) {
         const double nn = ceil(h.L / a.ms_max_step);
+        cl = cl || nn > (double)a.max_sub;
         const int n2 = nn > (double)a.max_sub ? a.max_sub : (int)nn;
         if (n2 > n) n = n2;
     }
+    if (clipped) *clipped = cl;
     return n;
 }
 
@@ -77,7 +82,12 @@ __global__ void __launch_bounds__(kScanThreads) k_substep_count(const __grid_con
     __shared__ long long s_warp[32];
     const long long i = (long long)blockIdx.x * kScanThreads + threadIdx.x;
     long long v = 0;
-    if (i < a.n) v = pieces_of(helix_of(a, i), a);
+    bool cl = false;
+    if (i < a.n) v = pieces_of(helix_of(a, i), a, &cl);
+    if (a.clipped) {                                              // tracks that needed more than max_sub pieces
+        const unsigned m = __ballot_sync(0xFFFFFFFFu, cl);
+        if (m && (threadIdx.x & 31) == 0) atomicAdd(a.clipped, (unsigned long long)__popc(m));
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int d = 1; d < 32; d <<= 1) {
         const long long t = __shfl_up_sync(0xFFFFFFFFu, v, d);
@@ -178,11 +188,16 @@ __global__ void __launch_bounds__(256) k_substep_fill(const __grid_constant__ Su
             double X0[3], X1[3];
             point_on(h, s0, X0);
             point_on(h, s1, X1);
-            const double d[3] = {X1[0] - X0[0], X1[1] - X0[1], X1[2] - X0[2]};
-            const double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double d[3] = {X1[0] - X0[0], X1[1] - X0[1], X1[2] - X0[2]};
+            double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
             const long long g = base + p;
             a.out.x[g] = (float)X0[0]; a.out.y[g] = (float)X0[1]; a.out.z[g] = (float)X0[2];
-            a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            if (!(len > 0.0)) {                                   // zero-length track: a piece of length 0 along the direction of flight
+                for (int k = 0; k < 3; ++k) d[k] = h.ppar * h.bh[k] + h.pperp * h.e1[k];
+                a.out.dx[g] = (float)d[0]; a.out.dy[g] = (float)d[1]; a.out.dz[g] = (float)d[2];
+            } else {
+                a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            }
             a.out.len[g] = (float)len;
             a.out.beta[g] = (float)h.beta;
             a.out.t0[g] = (float)(h.t0 + s0 / (h.beta * 0.299792458));
@@ -260,7 +275,11 @@ __global__ void __launch_bounds__(128) k_substep_fill_ms(const __grid_constant__
             const double len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
             const long long g = g0 + j;
             a.out.x[g] = (float)X[0]; a.out.y[g] = (float)X[1]; a.out.z[g] = (float)X[2];
-            a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            if (!(len > 0.0)) {                                   // zero-length track: keep the direction of flight
+                a.out.dx[g] = (float)P[0]; a.out.dy[g] = (float)P[1]; a.out.dz[g] = (float)P[2];
+            } else {
+                a.out.dx[g] = (float)(d[0] / len); a.out.dy[g] = (float)(d[1] / len); a.out.dz[g] = (float)(d[2] / len);
+            }
             a.out.len[g] = (float)len;
             a.out.beta[g] = (float)h.beta;
             a.out.t0[g] = (float)(h.t0 + (double)j * ds / (h.beta * 0.299792458));

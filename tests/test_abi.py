@@ -50,7 +50,7 @@ def test_struct_layouts_match_the_header(tmp_path):
         "c8ph_params": (api.Params, ["size", "write", "bunch_weight", "aim_factor", "disp_lambda0_nm", "use_efficiency", "flat_plane"]),
         "c8ph_segments": (api.Segments, ["size", "x", "edep", "id"]),
         "c8ph_outputs": (api.Outputs, ["size", "hist", "photon_capacity", "counters"]),
-        "c8ph_substep_desc": (api.SubstepDesc, ["size", "B_tesla", "tol_m", "ms_enabled", "ms_X0_gcm2", "seed", "track_id_base"]),
+        "c8ph_substep_desc": (api.SubstepDesc, ["size", "B_tesla", "tol_m", "ms_enabled", "ms_X0_gcm2", "seed", "track_id_base", "clipped"]),
         "c8ph_segments_out": (api.SegmentsOut, ["size", "x", "edep"]),
     }
     lines = ['#include <stdio.h>', '#include <stddef.h>', f'#include "{HEADER}"', "int main(void){"]

@@ -226,3 +226,34 @@ def test_two_library_shards_reduce_to_the_single_run(tmp_path):
     for i, name in enumerate(api.COUNTER_NAMES):
         assert int(red["cnt"][i]) == single["counters"][name], name
     assert 0 < int(red["written_local"]) < single["counters"]["written"]
+
+
+def test_substepping_counts_clipped_tracks_and_keeps_zero_length_tracks_finite():
+    """c8ph_substep_plan never clips silently: tracks whose sagitta / step bounds ask for more than max_sub pieces are
+    counted; a track of length 0 gives one finite piece of length 0 along its direction; max_sub is bounded."""
+    n = 64
+    cfg = W.make_config(4, n_segments=n)
+    trk = {f: v.copy() for f, v in cfg["segments"].items() if f != "edep"}
+    trk["len"][:] = 400.0
+    trk["len"][:4] = 0.0
+    trk["p_GeV"] = np.full(n, 0.01, np.float32)                       # 10 MeV/c in 45 uT: ~740 m radius
+    ctx = api.setup_context(cfg)
+    dev = {f: torch.from_numpy(v).cuda() for f, v in trk.items()}
+    B = (2.0e-5, -0.5e-5, -4.3e-5)
+    seg, off = ctx.substep_tracks(dev, n, B, 1e-4, max_sub=8)
+    counts = np.diff(off.cpu().numpy())
+    assert int(ctx.clipped_tracks.item()) == int((counts == 8).sum()) == n - 4
+    assert np.all(counts[:4] == 1)
+    for f in ("x", "y", "z", "dx", "dy", "dz", "len", "beta", "t0", "charge"):
+        assert torch.isfinite(seg[f]).all(), f
+    first = off[:4].cpu().numpy()
+    assert np.all(seg["len"].cpu().numpy()[first] == 0.0)
+    d = np.stack([seg[f].cpu().numpy()[first] for f in ("dx", "dy", "dz")], axis=1)
+    want = np.stack([trk[f][:4] for f in ("dx", "dy", "dz")], axis=1).astype(np.float64)
+    want /= np.linalg.norm(want, axis=1, keepdims=True)
+    assert np.allclose(d, want, atol=1e-6)
+    seg, off = ctx.substep_tracks(dev, n, B, 1e-4, max_sub=4096)
+    assert int(ctx.clipped_tracks.item()) == 0
+    with pytest.raises(api.C8phError) as e:
+        ctx.substep_tracks(dev, n, B, 1e-4, max_sub=(1 << 20) + 1)
+    assert e.value.code == api.E_ARG

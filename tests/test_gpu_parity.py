@@ -346,6 +346,25 @@ def test_cfg4_full_size_sampled_windows_and_invariants():
         assert np.array_equal(rec[k1], win["photons"][k2])            # full-size run == window run, bit for bit
 
 
+def test_cfg4_first_1e5_segments_whole_histogram_and_every_telescope_counter():
+    """SURVEY 8(d) / BASELINE.md section 3: the first 1e5 segment ids of configs[4] (3.4e7 photons, about a minute of
+    oracle time on the box's cores) compared as a whole: the 1000 x 1000 ground histogram bin by bin (the hot core
+    bins hold hundreds of photons), all 10 000 telescope counters and every event counter."""
+    n = 100_000
+    cfg = W.make_config(4, n_segments=n)
+    ora = O.run(cfg, record=False)
+    gpu = api.run_config(cfg, photon_capacity=1 << 22)
+    rep = parity.compare(cfg, ora, gpu, check_photons=False)
+    print("parity (1e5 segments):", parity.summary(rep), "counters (oracle, device):",
+          {k: rep[k] for k in ("emitted", "landed", "in_grid", "tel_hit", "roulette", "lv2")})
+    ho, hg = ora["hist"], gpu["hist"].astype(np.float64)
+    assert ho.max() > 300 and rep["hist_total_rel"] <= 1e-5
+    assert np.abs(ho - hg).max() <= 3                                 # no bin off by more than a few flips
+    to, tg = ora["tel_counts"], gpu["tel_counts"].astype(np.float64)
+    assert (to > 0).sum() > 2000 and np.abs(to - tg).max() <= 3
+    assert abs(tg.sum() - to.sum()) <= max(3, 1e-5 * to.sum())
+
+
 def test_cfg1_full_size_sampled_windows_and_invariants():
     """BASELINE configs[1] at its full 1e5 segments (planar atmosphere, per-photon layered sum, weight mode,
     every photon written: 8.1e6 records): whole-run identities plus photon-by-photon comparison with the

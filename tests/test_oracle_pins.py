@@ -1115,3 +1115,42 @@ def test_whole_photons_against_3d_ray_integration_flat_plane():
     # without the flat-plane step the same photons are off by centimetres at 19 km from the origin
     dpos, dt, ddir, shift, rho = _photons_vs_3d(2.0, 200.0, 60.0, 12000.0, False, "numeric")
     assert rho > 18000 and 0.05 < dpos < 0.15 and 0.1 < dt < 0.4
+
+
+# ------------------------------------------------------------------ sanitizers
+def test_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers():
+    """The oracle compiled with -fsanitize=address,undefined (-fno-sanitize-recover) runs small instances of all five
+    configs, the optional features, the table builder and the sub-stepping without a report."""
+    import subprocess
+    import sys
+    asan = subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("libasan not available")
+    code = r"""
+import copy, numpy as np
+from oracle import c8ph_oracle as O
+from paper_2405_04229_b200 import workloads as W
+O.build()
+tot = 0
+for k, n in ((0, 30), (1, 10), (2, 300), (3, 2000), (4, 40)):
+    cfg = W.make_config(k, n_segments=n)
+    if k == 3:
+        cfg["segments"]["edep"][:] *= 400.0
+    tot += O.run(cfg, threads=2)["counters"]["emitted"]
+cfg = W.make_config(4, n_segments=40)
+cfg["params"].update(disp_b_nm2=5700.0, disp_lambda0_nm=400.0, flat_plane=True,
+                     eff=np.linspace(0.2, 0.9, 31).astype(np.float32), eff_lambda0_nm=250.0, eff_dlambda_nm=15.0)
+cfg["segments"]["x"][3] = np.nan
+cfg["segments"]["id"] = np.arange(40, dtype=np.uint64)[::-1].copy()
+tot += O.run(cfg, threads=2)["counters"]["emitted"]
+trk = {f: v[:16].copy() for f, v in W.make_config(4, n_segments=16)["segments"].items() if f != "edep"}
+trk["len"][:] = 300.0
+trk["p_GeV"] = np.full(16, 0.05, np.float32)
+tot += len(O.substep_tracks(trk, (2e-5, -0.5e-5, -4.3e-5), 0.01)["segments"]["x"])
+print("sanitized oracle ok", tot)
+"""
+    env = dict(os.environ, C8PH_ORACLE_SANITIZE="1", LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:abort_on_error=0",
+               UBSAN_OPTIONS="print_stacktrace=1:halt_on_error=1", PYTHONPATH=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "sanitized oracle ok" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
+    assert "ERROR: AddressSanitizer" not in r.stderr and "runtime error:" not in r.stderr, r.stderr[-4000:]
