@@ -80,6 +80,11 @@ typedef struct {
     int32_t pad;
     double h_max, zen_max_rad;
     const float *data;             /* [n_h][n_zen][n_ch], fp32 as stored */
+    /* reading R21: the table "relative to a flat observation plane" (Fig. 4.10): third axis rho (polar radius of
+     * the straight-line point on the plane z = 0, uniform, n_rho >= 2), fourth axis cos(pointing angle) as even / odd part */
+    int32_t n_rho, pad3;
+    double rho_max;
+    const float *data3;            /* [2][n_rho][n_h][n_zen][n_ch] or NULL */
 } orc_table;
 
 typedef struct {
@@ -386,6 +391,197 @@ int orc_trace(const orc_atmosphere *atm, int spherical, double h_e, double sin_z
     out[0] = spherical ? atan2(px, py) : px;
     out[1] = S; out[2] = cT; out[3] = X; out[4] = tau;
     return 0;
+}
+
+/* R19 (Fig. 4.10: the correction is "relative to a flat observation plane"): dd, dt and the arrival
+ * direction ua describe the ray where it meets the observation SPHERE r = Rg; the detector plane z = 0 touches that
+ * sphere at the origin and lies above it elsewhere.  Line from the emission point Ae along u to the sphere, arc dd
+ * along the direction of flight on the sphere, then back along the arrival direction (straight, at the ground index)
+ * to z = 0.  Returns 1 if the straight line misses the sphere.  t_rel = arrival time - emission time [ns]. */
+static void norm3(double v[3]);
+static int flat_plane_step(const orc_atmosphere *atm, const double Ae[3], const double u[3], double h_e,
+                           double sin_zen, double cos_zen, double dd, double dt_ns, const double ua[3],
+                           double *x, double *y, double *t_rel, double *path)
+{
+    const double Rg = atm->earth_radius + atm->h_obs;
+    const double n_ground = 1.0 + orc_refractivity(atm, atm->h_obs);
+    double re = atm->earth_radius + h_e, pp = re * sin_zen;
+    if (!(pp < Rg)) return 1;
+    double S_line = re * cos_zen - sqrt(Rg*Rg - pp*pp);
+    double w[3] = { Ae[0] + S_line*u[0], Ae[1] + S_line*u[1], Ae[2] + S_line*u[2] + Rg };
+    norm3(w);
+    double cw = u[0]*w[0] + u[1]*w[1] + u[2]*w[2];
+    double et[3] = { u[0] - cw*w[0], u[1] - cw*w[1], u[2] - cw*w[2] };
+    double en = sqrt(et[0]*et[0] + et[1]*et[1] + et[2]*et[2]);
+    if (en < 1e-12) { et[0] = et[1] = et[2] = 0.0; } else { et[0] /= en; et[1] /= en; et[2] /= en; }
+    double ca = cos(dd / Rg), sa = sin(dd / Rg);
+    double Pr[3] = { Rg*(ca*w[0] + sa*et[0]), Rg*(ca*w[1] + sa*et[1]), Rg*(ca*w[2] + sa*et[2]) - Rg };
+    double s_back = Pr[2] / ua[2];
+    *x = Pr[0] - s_back * ua[0];
+    *y = Pr[1] - s_back * ua[1];
+    *t_rel = S_line / ORC_C_M_PER_NS + dt_ns - n_ground * s_back / ORC_C_M_PER_NS;
+    if (path) *path = S_line - s_back;
+    return 0;
+}
+
+/* arrival direction: u turned in the ray plane (u, local vertical rv at the emission point) by delta (R9) */
+static void rotate_in_ray_plane(const double u[3], const double rv[3], double sin_zen, double cos_zen, double delta, double ua[3])
+{
+    for (int k = 0; k < 3; ++k) ua[k] = u[k];
+    if (sin_zen > 1e-9 && delta != 0.0) {
+        double ep[3];
+        for (int k = 0; k < 3; ++k) ep[k] = (cos_zen*u[k] + rv[k]) / sin_zen;
+        for (int k = 0; k < 3; ++k) ua[k] = cos(delta)*u[k] + sin(delta)*ep[k];
+    }
+}
+
+/* rotation of the direction between emission and arrival from the Bouguer invariant (spherical model, R9) */
+static double bouguer_delta(const orc_atmosphere *atm, double h_e, double sin_zen, double cos_zen, double dd)
+{
+    const double Rg = atm->earth_radius + atm->h_obs;
+    const double n_ground = 1.0 + orc_refractivity(atm, atm->h_obs), n_ray = 1.0 + orc_refractivity(atm, h_e);
+    double re = atm->earth_radius + h_e;
+    double a_line = re * sin_zen / Rg;
+    double a_true = n_ray * re * sin_zen / (n_ground * Rg);
+    double psi_line = asin(a_line) - acos(cos_zen);
+    return asin(a_true) - (psi_line + dd / Rg) - acos(cos_zen);
+}
+
+/* R21, the thesis' table "relative to a flat observation plane" for the spherical model (Fig. 4.10: height, zenith
+ * angle, distance d = "the radius in the polar coordinate frame of reference", and "an additional pointing angle": four
+ * dimensions).  Axes here: emission height and local zenith (as the 2-D table), rho = polar radius of the straight-line
+ * point on the plane z = 0 (uniform), and cos(chi), chi = angle between the horizontal direction of flight and the
+ * outward radial direction at that point, with its two end nodes -1 / +1 stored as even and odd part:
+ *     value(rho, chi) = E(rho) + cos(chi) O(rho),  E = (T(+rho) + T(-rho))/2,  O = (T(+rho) - T(-rho))/2,
+ * T(x) = the photon of Fig. 4.10: emitted at height h_a in the vertical plane through the origin with local zenith
+ * theta_b, flying towards +x on the straight line that meets the plane at the signed coordinate x, traced exactly to
+ * the observation sphere (orc_trace) and taken on to the plane by R19's construction.  Two things distinguish the plane
+ * from the sphere at distance rho: it lies rho^2/2Rg higher (E, even in x) and it is tilted by rho/Rg against the
+ * sphere's tangent along the direction of flight (O, odd in x, proportional to cos(chi)); terms of second order in
+ * rho/Rg (1e-5 of the correction) are not represented.  Channels as in the 2-D table, relative to the straight line to
+ * the PLANE: ch0 displacement along the horizontal direction of flight, ch1 path, ch2 time [ns], ch3 X_slant, ch4 tau_aer.
+ * Layout [2][n_rho][n_h][n_zen][5] (E then O; ch3 of O holds the transverse displacement P, see flat_node_tangential).
+ * E(rho = 0) is the 2-D table.  Nodes without such a photon hold NaN. */
+static int flat_node(const orc_atmosphere *atm, double h, double th, double sz, double cz, const double r[6], double x_target, double T[5])
+{
+    const double rg = atm->earth_radius + atm->h_obs, re = atm->earth_radius + h;
+    const double p = re * sz;
+    const double S_line_sph = re * cz - sqrt(rg * rg - p * p);
+    const double dd = rg * r[0] - rg * (asin(p / rg) - th);
+    /* emission point E = (re sin(beta), 0, re cos(beta) - rg), direction (sin(th - beta), 0, -cos(th - beta)): its
+     * straight line meets z = 0 at x(beta) = E_x + E_z tan(th - beta); solve x(beta) = x_target by bisection */
+    double lo = -0.2, hi = 0.2, beta = 0.0;                   /* central angle of the emission point, +-1270 km */
+    for (int it = 0; it < 64; ++it) {
+        beta = 0.5 * (lo + hi);
+        double Ex = re * sin(beta), Ez = re * cos(beta) - rg;
+        if (Ex + Ez * tan(th - beta) < x_target) lo = beta; else hi = beta;
+    }
+    double Ae[3] = { re * sin(beta), 0.0, re * cos(beta) - rg };
+    if (!(Ae[2] > 0.0) || !(cos(th - beta) > 1e-3) || fabs(Ae[0] + Ae[2] * tan(th - beta) - x_target) > 1e-6 * (1.0 + fabs(x_target))) return 1;
+    double u[3] = { sin(th - beta), 0.0, -cos(th - beta) };
+    double rv[3] = { sin(beta), 0.0, cos(beta) };
+    double ua[3], x, y, t_rel, path;
+    rotate_in_ray_plane(u, rv, sz, cz, bouguer_delta(atm, h, sz, cz, dd), ua);
+    if (flat_plane_step(atm, Ae, u, h, sz, cz, dd, (r[2] - S_line_sph) / ORC_C_M_PER_NS, ua, &x, &y, &t_rel, &path)) return 1;
+    const double D = Ae[2] / cos(th - beta);                   /* straight line to the plane */
+    T[0] = x - x_target;
+    T[1] = path + (r[1] - S_line_sph) - D;
+    T[2] = t_rel - D / ORC_C_M_PER_NS;
+    T[3] = r[3];
+    T[4] = r[4];
+    return 0;
+}
+
+/* The tilt of the plane against the sphere also has a component across the direction of flight: on the sphere the
+ * refraction displacement dd runs along the geodesic, whose projection on the plane leans towards the radial direction
+ * by cot(zenith) rho/Rg.  P(rho) = displacement towards the outward radial direction r^ of a photon in tangential flight
+ * (chi = 90 deg: straight-line point (rho, 0, 0), flying along +y); for any chi the transverse part is
+ * P (r^ - cos(chi) e_h).  Emission point in closed form: cos^2(global zenith) = (re^2 cos^2(theta) + rho^2 + Rg^2 - re^2)/Rg^2. */
+static int flat_node_tangential(const orc_atmosphere *atm, double h, double th, double sz, double cz, const double r[6], double rho, double *P)
+{
+    const double rg = atm->earth_radius + atm->h_obs, re = atm->earth_radius + h;
+    const double p = re * sz;
+    const double S_line_sph = re * cz - sqrt(rg * rg - p * p);
+    const double dd = rg * r[0] - rg * (asin(p / rg) - th);
+    const double c2 = (re * re * cz * cz + rho * rho + rg * rg - re * re) / (rg * rg);
+    if (!(c2 > 1e-6 && c2 <= 1.0)) return 1;
+    const double cg = sqrt(c2), sg = sqrt(1.0 - c2);
+    const double sdist = -rg * cg + re * cz;                   /* distance from the emission point to the plane point */
+    if (!(sdist > 0.0)) return 1;
+    double Ae[3] = { rho, -sdist * sg, sdist * cg };
+    double u[3] = { 0.0, sg, -cg };
+    double rv[3] = { Ae[0] / re, Ae[1] / re, (Ae[2] + rg) / re };
+    double ua[3], x, y, t_rel;
+    rotate_in_ray_plane(u, rv, sz, cz, bouguer_delta(atm, h, sz, cz, dd), ua);
+    if (flat_plane_step(atm, Ae, u, h, sz, cz, dd, (r[2] - S_line_sph) / ORC_C_M_PER_NS, ua, &x, &y, &t_rel, NULL)) return 1;
+    *P = x - rho;
+    return 0;
+}
+
+void orc_build_table_flat(const orc_atmosphere *atm, int n_h, int n_zen, int n_rho, double h_max, double zen_max_rad,
+                          double rho_max, int sub, float *out /* [2][n_rho][n_h][n_zen][5] */)
+{
+    const size_t half = (size_t)n_rho * n_h * n_zen * 5;
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int a = 0; a < n_h; ++a) {
+        double h = a * h_max / (n_h - 1);
+        for (int b = 0; b < n_zen; ++b) {
+            double th = b * zen_max_rad / (n_zen - 1);
+            double r[6];
+            double sz = sin(th), cz = cos(th);
+            int zero = h <= atm->h_obs, bad = 0;
+            if (!zero) bad = orc_trace(atm, 1, h, sz, cz, atm->h_obs, sub, r);
+            for (int c = 0; c < n_rho; ++c) {
+                float *e = out + (((size_t)c * n_h + a) * n_zen + b) * 5, *o = e + half;
+                if (zero) { for (int k = 0; k < 5; ++k) e[k] = o[k] = 0.0f; continue; }
+                const double rho = rho_max * c / (n_rho - 1);
+                double Tp[5], Tm[5], P = 0.0;
+                if (bad || flat_node(atm, h, th, sz, cz, r, rho, Tp) || flat_node(atm, h, th, sz, cz, r, -rho, Tm) ||
+                    flat_node_tangential(atm, h, th, sz, cz, r, rho, &P)) {
+                    for (int k = 0; k < 5; ++k) e[k] = o[k] = NAN;
+                    continue;
+                }
+                for (int k = 0; k < 5; ++k) { e[k] = (float)(0.5 * (Tp[k] + Tm[k])); o[k] = (float)(0.5 * (Tp[k] - Tm[k])); }
+                o[3] = (float)P;                                /* odd part, ch3: transverse displacement (X_slant has no odd part) */
+                o[4] = 0.0f;
+            }
+        }
+    }
+}
+
+/* lookup in the flat-plane table: trilinear in (height, zenith, rho) on E and on O (indices clamped), then
+ * E + cos(chi) O; cos_chi = (horizontal direction of flight) . (outward radial direction at the straight-line point);
+ * *perp = P, the displacement along (r^ - cos(chi) e_h) */
+int orc_table_flat_lookup(const orc_table *t, double h, double zen, double rho, double cos_chi, double out[5], double *perp)
+{
+    if (!t->data3 || t->n_rho < 2) return 1;
+    if (!(h >= 0.0) || h > t->h_max || !(zen >= 0.0) || zen > t->zen_max_rad || !(rho >= 0.0) || rho > t->rho_max) return 1;
+    double f = h / (t->h_max / (t->n_h - 1)), g = zen / (t->zen_max_rad / (t->n_zen - 1));
+    double e = rho / (t->rho_max / (t->n_rho - 1));
+    int a = (int)floor(f), b = (int)floor(g), c = (int)floor(e);
+    if (a > t->n_h - 2) a = t->n_h - 2;
+    if (b > t->n_zen - 2) b = t->n_zen - 2;
+    if (c > t->n_rho - 2) c = t->n_rho - 2;
+    double ff = f - a, gg = g - b, ee = e - c;
+    int bad = 0;
+    const size_t s = (size_t)t->n_ch, plane = (size_t)t->n_h * t->n_zen * s, half = plane * t->n_rho;
+    for (int k = 0; k < 5; ++k) {
+        double part[2];
+        for (int eo = 0; eo < 2; ++eo) {
+            double v[2];
+            for (int q = 0; q < 2; ++q) {
+                const float *d = t->data3 + eo * half + (size_t)(c + q) * plane;
+                double v00 = d[((size_t)a * t->n_zen + b) * s + k], v01 = d[((size_t)a * t->n_zen + b + 1) * s + k];
+                double v10 = d[((size_t)(a + 1) * t->n_zen + b) * s + k], v11 = d[((size_t)(a + 1) * t->n_zen + b + 1) * s + k];
+                v[q] = (1 - ff) * ((1 - gg) * v00 + gg * v01) + ff * ((1 - gg) * v10 + gg * v11);
+            }
+            part[eo] = (1 - ee) * v[0] + ee * v[1];
+        }
+        if (k >= 3) { out[k] = part[0]; if (k == 3 && perp) *perp = part[1]; }   /* X_slant, tau_aer: even part only */
+        else out[k] = part[0] + cos_chi * part[1];
+        if (isnan(out[k]) || isnan(part[1])) bad = 1;
+    }
+    return bad;
 }
 
 /* ------------------------------------------------------------------ A15 interpolation tracing
@@ -889,6 +1085,7 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 sin_zen = sqrt(fmax(0.0, 1.0 - cos_zen*cos_zen));
                 sin_arr = sin_zen;
                 double delta = 0.0;                          /* rotation of the direction in the ray plane */
+                double perp_flat = 0.0, rho_I = 0.0, cos_chi = 0.0;   /* R21: transverse displacement of the flat-plane table */
                 if (par->trace == ORC_TRACE_STRAIGHT) {
                     dt_ns = eta_e * D / ORC_C_M_PER_NS;      /* homogeneous: t = t_e + n D / c */
                     if (atm->model != 0) {
@@ -914,7 +1111,14 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                     x_slant = r[3]; tau_aer = r[4];
                 } else {
                     double corr[5];
-                    if (cos_zen <= 0.0 || orc_table_lookup(tab, h_e, acos(cos_zen), corr)) {
+                    /* R21: with flat_plane = 2 the flat-plane table (polar radius of the straight-line point, pointing
+                     * angle of the horizontal direction of flight against the outward radial direction there) gives the
+                     * correction relative to the plane z = 0 directly */
+                    const int t3 = par->flat_plane == 2 && atm->model == 2;
+                    rho_I = sqrt(I[0]*I[0] + I[1]*I[1]);
+                    cos_chi = rho_I > 1e-9 ? (eh[0]*I[0] + eh[1]*I[1]) / rho_I : 0.0;
+                    if (cos_zen <= 0.0 || (t3 ? orc_table_flat_lookup(tab, h_e, acos(cos_zen), rho_I, cos_chi, corr, &perp_flat)
+                                              : orc_table_lookup(tab, h_e, acos(cos_zen), corr))) {
                         ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store;
                     }
                     dd = corr[0]; dt_ns = corr[2]; x_slant = corr[3]; tau_aer = corr[4];
@@ -948,6 +1152,10 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 /* landed: corrected position, time, direction */
                 ph.x = I[0] + dd * eh[0];
                 ph.y = I[1] + dd * eh[1];
+                if (perp_flat != 0.0 && rho_I > 1e-9) {          /* R21: across the direction of flight, towards r^ */
+                    ph.x += perp_flat * (I[0] / rho_I - cos_chi * eh[0]);
+                    ph.y += perp_flat * (I[1] / rho_I - cos_chi * eh[1]);
+                }
                 ph.t = t_e + D / ORC_C_M_PER_NS + dt_ns;
                 {
                     double ua[3] = { u[0], u[1], u[2] };
@@ -957,27 +1165,13 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                         for (int k = 0; k < 3; ++k) ua[k] = cos(delta)*u[k] + sin(delta)*ep[k];
                     }
                     ph.ux = ua[0]; ph.uy = ua[1]; ph.uz = ua[2];
-                    if (par->flat_plane && atm->model == 2 && par->trace != ORC_TRACE_STRAIGHT) {
-                        /* R19 (Fig. 4.10: the correction is "relative to a flat observation plane"): dd, dt
-                         * and delta describe the ray where it meets the observation SPHERE r = Rg; the detector
-                         * plane z = 0 touches that sphere at the origin and lies above it elsewhere.  Line to the
-                         * sphere, arc dd along the direction of flight on the sphere, then back along the arrival
-                         * direction (straight, at the ground index) to z = 0. */
-                        double re = atm->earth_radius + h_e, pp = re * sin_zen;
-                        if (!(pp < Rg)) { ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store; }
-                        double S_line = re * cos_zen - sqrt(Rg*Rg - pp*pp);
-                        double w[3] = { Ae[0] + S_line*u[0], Ae[1] + S_line*u[1], Ae[2] + S_line*u[2] + Rg };
-                        norm3(w);
-                        double cw = u[0]*w[0] + u[1]*w[1] + u[2]*w[2];
-                        double et[3] = { u[0] - cw*w[0], u[1] - cw*w[1], u[2] - cw*w[2] };
-                        double en = sqrt(et[0]*et[0] + et[1]*et[1] + et[2]*et[2]);
-                        if (en < 1e-12) { et[0] = et[1] = et[2] = 0.0; } else { et[0] /= en; et[1] /= en; et[2] /= en; }
-                        double ca = cos(dd / Rg), sa = sin(dd / Rg);
-                        double Pr[3] = { Rg*(ca*w[0] + sa*et[0]), Rg*(ca*w[1] + sa*et[1]), Rg*(ca*w[2] + sa*et[2]) - Rg };
-                        double s_back = Pr[2] / ua[2];
-                        ph.x = Pr[0] - s_back * ua[0];
-                        ph.y = Pr[1] - s_back * ua[1];
-                        ph.t = t_e + S_line / ORC_C_M_PER_NS + dt_ns - n_ground * s_back / ORC_C_M_PER_NS;
+                    if (par->flat_plane == 1 && atm->model == 2 && par->trace != ORC_TRACE_STRAIGHT) {
+                        /* R19: from the observation sphere to the plane z = 0 (flat_plane_step above) */
+                        double t_rel;
+                        if (flat_plane_step(atm, Ae, u, h_e, sin_zen, cos_zen, dd, dt_ns, ua, &ph.x, &ph.y, &t_rel, NULL)) {
+                            ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store;
+                        }
+                        ph.t = t_e + t_rel;
                     }
                 }
                 (void)sin_arr;

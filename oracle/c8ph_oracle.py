@@ -51,7 +51,8 @@ class Atmosphere(C.Structure):
 
 class Table(C.Structure):
     _fields_ = [("n_h", C.c_int32), ("n_zen", C.c_int32), ("n_ch", C.c_int32), ("pad", C.c_int32),
-                ("h_max", C.c_double), ("zen_max_rad", C.c_double), ("data", C.POINTER(C.c_float))]
+                ("h_max", C.c_double), ("zen_max_rad", C.c_double), ("data", C.POINTER(C.c_float)),
+                ("n_rho", C.c_int32), ("pad3", C.c_int32), ("rho_max", C.c_double), ("data3", C.POINTER(C.c_float))]
 
 
 class Segments(C.Structure):
@@ -147,6 +148,12 @@ def lib():
             L.orc_build_table.restype = None
             L.orc_build_table.argtypes = [C.POINTER(Atmosphere), C.c_int, C.c_int, C.c_double, C.c_double,
                                           C.c_int, C.POINTER(C.c_float)]
+            L.orc_build_table_flat.restype = None
+            L.orc_build_table_flat.argtypes = [C.POINTER(Atmosphere), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                               C.c_double, C.c_int, C.POINTER(C.c_float)]
+            L.orc_table_flat_lookup.restype = C.c_int
+            L.orc_table_flat_lookup.argtypes = [C.POINTER(Table), C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double),
+                                                C.POINTER(C.c_double)]
             L.orc_table_lookup.restype = C.c_int
             L.orc_table_lookup.argtypes = [C.POINTER(Table), C.c_double, C.c_double, C.POINTER(C.c_double)]
             L.orc_transmission.restype = C.c_double
@@ -226,7 +233,7 @@ def params_struct(par: dict, keep: _Keep) -> Params:
     s.disp_lambda0_nm = float(np.float32(par.get("disp_lambda0_nm", 400.0)))
     eff = par.get("eff")
     s.n_eff = 0 if eff is None else len(eff)
-    s.flat_plane = int(bool(par.get("flat_plane", False)))
+    s.flat_plane = int(par.get("flat_plane", 0))       # 0: off, 1 / True: analytic step (R19), 2: 3-D table (R21)
     s.eff = keep.f32(eff) if s.n_eff else None
     s.eff_lambda0_nm = float(np.float32(par.get("eff_lambda0_nm", 0.0)))
     s.eff_dlambda_nm = float(np.float32(par.get("eff_dlambda_nm", 1.0)))
@@ -319,13 +326,35 @@ def build_table(atm: dict, table: dict, sub: int = 1) -> np.ndarray:
     return out
 
 
-def table_struct(table: dict, data: np.ndarray, keep: _Keep) -> Table:
+def build_table_flat(atm: dict, table: dict, sub: int = 1) -> np.ndarray:
+    """R21: [2 (even, odd in the pointing angle)][n_rho][n_h][n_zen][5], the correction relative to the flat plane."""
+    keep = _Keep()
+    out = np.empty((2, table["n_rho"], table["n_h"], table["n_zen"], 5), dtype=np.float32)
+    lib().orc_build_table_flat(C.byref(atmosphere_struct(atm, keep)), table["n_h"], table["n_zen"], table["n_rho"],
+                           float(table["h_max"]), math.radians(float(np.float32(table["zen_max_deg"]))),
+                           float(np.float32(table["rho_max_m"])), int(sub), _fp(out))
+    return out
+
+
+def table_struct(table: dict, data: np.ndarray, keep: _Keep, data3: np.ndarray | None = None) -> Table:
     t = Table()
     t.n_h, t.n_zen, t.n_ch = int(table["n_h"]), int(table["n_zen"]), int(data.shape[-1])
     t.h_max = float(table["h_max"])
     t.zen_max_rad = math.radians(float(np.float32(table["zen_max_deg"])))
     t.data = keep.f32(data)
+    if data3 is not None:
+        t.n_rho, t.rho_max = int(table["n_rho"]), float(np.float32(table["rho_max_m"]))
+        t.data3 = keep.f32(data3)
     return t
+
+
+def table_flat_lookup(table: dict, data: np.ndarray, data3: np.ndarray, h: float, zen_rad: float, rho: float, cos_chi: float):
+    keep = _Keep()
+    t = table_struct(table, data, keep, data3)
+    out = (C.c_double * 5)()
+    perp = C.c_double(0.0)
+    bad = lib().orc_table_flat_lookup(C.byref(t), float(h), float(zen_rad), float(rho), float(cos_chi), out, C.byref(perp))
+    return bool(bad), list(out), perp.value
 
 
 def table_lookup(table: dict, data: np.ndarray, h: float, zen_rad: float):
@@ -356,14 +385,28 @@ def camera_pixel(det: dict, u_arr) -> int:
 _table_cache = {}
 
 
+def _table_key(cfg: dict, sub: int):
+    atm = cfg["atmosphere"]
+    return (atm["model"], atm["h_obs"], atm["refractivity"].tobytes()[:4096], atm["overburden"].tobytes()[:4096],
+            atm["aer_L"], atm["aer_H"], tuple(sorted(cfg["table"].items())), sub)
+
+
 def table_for(cfg: dict, sub: int = 1) -> np.ndarray | None:
     if cfg.get("table") is None:
         return None
-    atm = cfg["atmosphere"]
-    key = (atm["model"], atm["h_obs"], atm["refractivity"].tobytes()[:4096], atm["overburden"].tobytes()[:4096],
-           atm["aer_L"], atm["aer_H"], tuple(sorted(cfg["table"].items())), sub)
+    key = _table_key(cfg, sub)
     if key not in _table_cache:
-        _table_cache[key] = build_table(atm, cfg["table"], sub)
+        _table_cache[key] = build_table(cfg["atmosphere"], cfg["table"], sub)
+    return _table_cache[key]
+
+
+def table_flat_for(cfg: dict, sub: int = 1) -> np.ndarray | None:
+    """The flat-plane table of R21 if the config's table has the extra axes (n_rho, rho_max_m)."""
+    if cfg.get("table") is None or not cfg["table"].get("n_rho"):
+        return None
+    key = ("t3",) + _table_key(cfg, sub)
+    if key not in _table_cache:
+        _table_cache[key] = build_table_flat(cfg["atmosphere"], cfg["table"], sub)
     return _table_cache[key]
 
 
@@ -387,7 +430,8 @@ def run(cfg: dict, record: bool = True, table_data: np.ndarray | None = None, th
     if cfg.get("table") is not None and cfg["params"]["trace"] == "table":
         if table_data is None:
             table_data = table_for(cfg)
-        tab = table_struct(cfg["table"], table_data, keep)
+        data3 = table_flat_for(cfg) if int(cfg["params"].get("flat_plane", 0)) == 2 else None
+        tab = table_struct(cfg["table"], table_data, keep, data3)
         tab_ptr = C.byref(tab)
     dd = cfg["detector"]
     n_hist = dd["n_tbins"] * dd["cam_rows"] * dd["cam_cols"] if dd["cam_enabled"] else dd["hist_nx"] * dd["hist_ny"]

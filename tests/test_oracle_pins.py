@@ -1064,7 +1064,7 @@ def _brute_force_ray_3d(atm, A, U, ds=2.0):
     return out[:, :2], u, out[:, 6] / C_LIGHT
 
 
-def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10, **par):
+def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10, table=None, return_photons=False, **par):
     """One 1 mm segment (emission point known to 1 mm) at horizontal distance d from the origin; the
     landed photons of the whole oracle run against the 3-D integration of the same rays."""
     cfg = W.make_config(4, n_segments=1)
@@ -1072,6 +1072,8 @@ def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10, **par):
     cfg["detector"]["tel_xyzr"] = np.zeros((0, 4), np.float32)
     if trace != "table":
         cfg["table"] = None
+    elif table is not None:
+        cfg["table"] = dict(cfg["table"], **table)
     s = cfg["segments"]
     th, az = math.radians(zen_deg), math.radians(az_deg)
     for k, v in zip(("x", "y", "z", "dx", "dy", "dz"),
@@ -1082,6 +1084,8 @@ def _photons_vs_3d(d_km, az_deg, zen_deg, h, flat, trace, n_ph=10, **par):
     ph = O.run(cfg)["photons"]
     ph = ph[ph["status"] == O.ST_LANDED][:n_ph]
     assert len(ph) == n_ph
+    if return_photons:
+        return ph
     I = np.stack([ph["x_line"], ph["y_line"], np.zeros(len(ph))], 1)
     U = I - A
     U /= np.linalg.norm(U, axis=1)[:, None]
@@ -1115,6 +1119,56 @@ def test_whole_photons_against_3d_ray_integration_flat_plane():
     # without the flat-plane step the same photons are off by centimetres at 19 km from the origin
     dpos, dt, ddir, shift, rho = _photons_vs_3d(2.0, 200.0, 60.0, 12000.0, False, "numeric")
     assert rho > 18000 and 0.05 < dpos < 0.15 and 0.1 < dt < 0.4
+
+
+def test_flat_plane_table_of_the_thesis_four_axes():
+    """R21 (Fig. 4.10): the table "relative to a flat observation plane" over (height, zenith, polar radius of the
+    straight-line point, pointing angle as even / odd part).  Pins: E(rho = 0) is the 2-D table and O(0) = 0; the lookup is
+    exact on functions that are trilinear in (h, zenith, rho) and linear in cos(chi); whole photons of orc_run through the
+    table land where R19's exact sphere-to-plane step (itself pinned by the 3-D ray integration) puts them, for outward,
+    inward and tangential flight (0.3 mm out to 30 km from the origin; the transverse part alone is 6 mm there), and where
+    the 3-D integration puts them; the even part grows like rho^2 (sag) and the odd part like rho (tilt of the plane
+    against the sphere)."""
+    tab = dict(n_h=128, n_zen=128, h_max=20000.0, zen_max_deg=75.0, n_rho=17, rho_max_m=32000.0)
+    cfg = W.make_config(4, n_segments=1)
+    t = dict(cfg["table"], **tab)
+    d2 = O.build_table(cfg["atmosphere"], t)
+    d4 = O.build_table_flat(cfg["atmosphere"], t)
+    assert d4.shape == (2, 17, 128, 128, 5)
+    ok = np.isfinite(d2[..., 0]) & np.isfinite(d4[0, 0, ..., 0])
+    # (the refracted ray lands |dd| short of the origin, where the sphere is already dd^2 / 2 Rg below the plane: 5e-5 relative)
+    assert ok.mean() > 0.95 and np.allclose(d4[0, 0][ok], d2[ok], rtol=5e-5, atol=1e-5) and np.all(d4[1, 0][ok] == 0)
+    # scaling with rho at a node well inside (12 km, 50 deg): even ~ rho^2, odd ~ rho
+    a, b = 77, 85
+    E, Od = d4[0, :, a, b, 0].astype(np.float64) - d4[0, 0, a, b, 0], d4[1, :, a, b, 0].astype(np.float64)
+    assert E[16] / E[8] == pytest.approx(4.0, rel=0.05) and Od[16] / Od[8] == pytest.approx(2.0, rel=0.05)
+    assert 0.002 < abs(E[16]) < 0.2 and 0.002 < abs(Od[16]) < 0.2        # millimetres to centimetres at 32 km
+    # exactness of the lookup on a function linear in every axis
+    lin = np.zeros_like(d4)
+    hh, zz, rr = np.meshgrid(np.linspace(0, 20000, 128), np.linspace(0, math.radians(float(np.float32(75.0))), 128), np.linspace(0, 32000, 17), indexing="ij")
+    for k in range(5):
+        lin[0, ..., k] = np.transpose(1.0 + 2e-4 * hh - 3.0 * zz + 5e-5 * rr + 1e-8 * hh * rr * zz, (2, 0, 1)) * (k + 1)
+        lin[1, ..., k] = np.transpose(0.5 - 1e-5 * hh + 2e-5 * rr * zz, (2, 0, 1)) * (k + 1)
+    for h, z, r, c in ((1234.5, 0.3, 7777.0, 0.4), (19999.0, 1.2, 31999.0, -1.0), (0.0, 0.0, 0.0, 1.0)):
+        bad, v, perp = O.table_flat_lookup(t, d2, lin, h, z, r, c)
+        ev, od = (1.0 + 2e-4 * h - 3.0 * z + 5e-5 * r + 1e-8 * h * r * z), (0.5 - 1e-5 * h + 2e-5 * r * z)
+        assert not bad and np.allclose(v[:3], (ev + c * od) * np.arange(1, 4), rtol=2e-6)
+        assert np.allclose(v[3:], ev * np.arange(4, 6), rtol=2e-6) and perp == pytest.approx(4 * od, rel=2e-6)
+    assert O.table_flat_lookup(t, d2, d4, 5000.0, 0.5, 33000.0, 0.0)[0]      # outside the table: TABLE_RANGE
+    # whole photons: table (flat_plane = 2) against R19's analytic step (flat_plane = 1) on the same 2-D table, and against
+    # the 3-D integration; flight outward (az 0), inward (180), tangential (90), oblique
+    worst = 0.0
+    for d_km, az, zen in ((15.0, 0.0, 50.0), (25.0, 180.0, 40.0), (20.0, 90.0, 55.0), (12.0, 230.0, 60.0), (0.3, 40.0, 20.0)):
+        p1 = _photons_vs_3d(d_km, az, zen, 12000.0, 1, "table", table=tab, return_photons=True)
+        p2 = _photons_vs_3d(d_km, az, zen, 12000.0, 2, "table", table=tab, return_photons=True)
+        assert np.array_equal(p1["j"], p2["j"])
+        dpos = np.hypot(p1["x"] - p2["x"], p1["y"] - p2["y"]).max()
+        worst = max(worst, dpos)
+        assert dpos < 3e-4 and np.abs(p1["t"] - p2["t"]).max() < 1e-3, (d_km, az, zen, dpos)   # second order in rho/Rg remains
+        assert np.abs(p1["ux"] - p2["ux"]).max() < 1e-7 and np.abs(p1["uz"] - p2["uz"]).max() < 1e-7
+        dpos3, dt3, ddir3, shift, rho = _photons_vs_3d(d_km, az, zen, 12000.0, 2, "table", table=tab)
+        assert dpos3 < 2e-2 and dt3 < 2e-2 and ddir3 < 5e-6, (d_km, az, zen, dpos3, dt3)   # + bilinear error of this coarse table
+    print("flat-plane table vs analytic step, worst position difference [m]:", worst)
 
 
 # ------------------------------------------------------------------ sanitizers (SURVEY section 5)
