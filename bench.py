@@ -232,7 +232,10 @@ def run_reference(args):
 def _apply_variant(cfg: dict, variant: str) -> None:
     """Optional features (R13-R15, R17, R19) on top of a BASELINE config."""
     if variant == "flat":
-        cfg["params"].update(flat_plane=True)
+        cfg["params"].update(flat_plane=1)
+    elif variant == "flattab":
+        cfg["params"].update(flat_plane=2)
+        cfg["table"] = dict(cfg["table"], n_rho=16, rho_max_m=30000.0)
     elif variant == "extinction":
         # a tau_v(lambda, h) table filled from the Rayleigh law of the config on a 10 nm grid
         atm = cfg["atmosphere"]
@@ -506,7 +509,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--variant", choices=("base", "generic", "flat", "extinction", "dispersion", "efficiency", "optics"), default="base",
+    ap.add_argument("--variant", choices=("base", "generic", "flat", "flattab", "extinction", "dispersion", "efficiency", "optics"), default="base",
                     help="optional features of SURVEY 8(f) switched on (generic kernel variant); the headline is 'base'")
     ap.add_argument("--substep", type=int, default=0, help="time c8ph_substep_plan + c8ph_substep_fill on this many tracks and exit")
     ap.add_argument("--substep-ms", type=float, default=None, metavar="STEP_M",

@@ -84,6 +84,12 @@ typedef struct {
     int32_t n_h, n_zen;              /* nodes: h_a = a h_max/(n_h-1) a.s.l., theta_b = b zen_max/(n_zen-1) */
     float h_max_m, zen_max_deg;
     int32_t substeps;                /* sub-layers per n(h) table cell in the builder (>= 1)       */
+    /* Table "relative to a flat observation plane" (thesis P:861, Fig. 4.10; R21; spherical model only):
+     * two more axes, rho = polar radius of the straight-line point on the plane z = 0 (n_rho >= 2 uniform nodes up to
+     * rho_max_m) and the pointing angle of the direction of flight against the outward radial direction there (kept
+     * as even / odd / transverse parts).  n_rho = 0: not built.  Used by params.flat_plane = 2.                    */
+    int32_t n_rho;
+    float rho_max_m;
 } c8ph_table_desc;
 /* One kernel, one thread per node: the exact layered-Snell ray (fp64) from (h_a, theta_b) to the
  * observation sphere/plane minus the straight line (asynchronous on `stream`, a cudaStream_t).   */
@@ -92,6 +98,9 @@ int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *desc, void *str
  * set_ lets a caller inject a table computed elsewhere.  No-ground nodes hold NaN.              */
 int c8ph_get_trace_table(c8ph_ctx *ctx, float *host_out, int64_t n_floats);
 int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *desc, const float *host_in);
+/* The flat-plane table as stored: HOST [2][n_rho][n_h][n_zen][4]; part 0 (even) = dd [m], dt [ns], X_slant, tau_aer
+ * relative to the straight line to the PLANE; part 1 = odd dd, odd dt, transverse displacement P [m], 0.  Synchronous. */
+int c8ph_get_trace_table_flat(c8ph_ctx *ctx, float *host_out, int64_t n_floats);
 
 /* ---- detector (thesis sec. 6.2; camera: BASELINE cfg3) ---------------------------- */
 typedef struct {
@@ -153,8 +162,10 @@ typedef struct {
      * the plane z = 0 (the sag of the sphere under the plane is ignored: < 1 mm within 5 km of the
      * origin, centimetres beyond 15 km); 1: line on to the sphere, arc along the flight direction, back
      * along the arrival direction to z = 0 (0.1 mm / 1 ps against a 3-D ray integration out to 25 km).
-     * Photons whose straight line misses the sphere count as C8PH_CNT_TABLE_RANGE.  Ignored for the
-     * planar / homogeneous models and the straight trace.                                          */
+     * Photons whose straight line misses the sphere count as C8PH_CNT_TABLE_RANGE.  2: the same result from the
+     * thesis' own construction, the table over (height, zenith, rho, pointing angle) built with n_rho >= 2 (R21):
+     * one lookup of 16 texels instead of the analytic step; straight-line points beyond rho_max_m count as
+     * TABLE_RANGE.  Ignored for the planar / homogeneous models and the straight trace.              */
     int32_t flat_plane;
 } c8ph_params;
 

@@ -33,7 +33,8 @@ N_COUNTERS = len(COUNTER_NAMES)
 EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8ph_init_atmosphere",
            "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
            "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
-           "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill", "c8ph_set_line_spectrum", "c8ph_set_efficiency")
+           "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill", "c8ph_set_line_spectrum", "c8ph_set_efficiency",
+           "c8ph_get_trace_table_flat")
 
 PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
                          ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
@@ -55,7 +56,8 @@ class AtmosphereDesc(C.Structure):
 
 class TableDesc(C.Structure):
     _fields_ = [("size", C.c_uint32), ("n_h", C.c_int32), ("n_zen", C.c_int32),
-                ("h_max_m", C.c_float), ("zen_max_deg", C.c_float), ("substeps", C.c_int32)]
+                ("h_max_m", C.c_float), ("zen_max_deg", C.c_float), ("substeps", C.c_int32),
+                ("n_rho", C.c_int32), ("rho_max_m", C.c_float)]
 
 
 class Detector(C.Structure):
@@ -121,6 +123,7 @@ def load_library():
         L.c8ph_build_trace_table.argtypes = [C.c_void_p, C.POINTER(TableDesc), C.c_void_p]
         L.c8ph_get_trace_table.argtypes = [C.c_void_p, _fp, C.c_int64]
         L.c8ph_set_trace_table.argtypes = [C.c_void_p, C.POINTER(TableDesc), _fp]
+        L.c8ph_get_trace_table_flat.argtypes = [C.c_void_p, _fp, C.c_int64]
         L.c8ph_set_detector.argtypes = [C.c_void_p, C.POINTER(Detector)]
         L.c8ph_emit_propagate.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_int64, C.c_int64,
                                           C.POINTER(Params), C.c_uint64, C.POINTER(Outputs), C.c_void_p]
@@ -212,7 +215,15 @@ class Context:
         t.n_h, t.n_zen = int(table["n_h"]), int(table["n_zen"])
         t.h_max_m, t.zen_max_deg = float(table["h_max"]), float(table["zen_max_deg"])
         t.substeps = int(table.get("substeps", 1))
+        t.n_rho, t.rho_max_m = int(table.get("n_rho", 0) or 0), float(table.get("rho_max_m", 0.0) or 0.0)
         return t
+
+    def get_trace_table_flat(self) -> np.ndarray:
+        """[2 (even, odd)][n_rho][n_h][n_zen][4] texels of the flat-plane table (R21)."""
+        t = self._table
+        out = np.empty((2, t["n_rho"], t["n_h"], t["n_zen"], 4), dtype=np.float32)
+        self._check(self.lib.c8ph_get_trace_table_flat(self._h, out.ctypes.data_as(_fp), out.size))
+        return out
 
     def build_trace_table(self, table: dict, stream=None):
         self._table = dict(table)
@@ -228,7 +239,7 @@ class Context:
         self._table = dict(table)
         data = _f32(data)
         assert data.shape == (table["n_h"], table["n_zen"], TABLE_CHANNELS)
-        self._check(self.lib.c8ph_set_trace_table(self._h, C.byref(self._table_desc(table)), data.ctypes.data_as(_fp)))
+        self._check(self.lib.c8ph_set_trace_table(self._h, C.byref(self._table_desc(dict(table, n_rho=0))), data.ctypes.data_as(_fp)))
 
     def set_detector(self, det: dict):
         d = Detector()
@@ -269,7 +280,7 @@ class Context:
         p.fluor_yield_per_MeV, p.aim_factor = float(par["fluor_yield_per_MeV"]), float(par["aim_factor"])
         p.disp_b_nm2, p.disp_lambda0_nm = float(par.get("disp_b_nm2", 0.0)), float(par.get("disp_lambda0_nm", 400.0))
         p.use_efficiency = int(par.get("eff") is not None and len(par["eff"]) > 0)
-        p.flat_plane = int(bool(par.get("flat_plane", False)))
+        p.flat_plane = int(par.get("flat_plane", 0))                   # 0 off, 1 / True analytic step (R19), 2 table (R21)
         self._sync_spectra(par)
         return p, None
 

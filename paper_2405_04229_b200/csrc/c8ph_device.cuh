@@ -38,6 +38,11 @@ struct DevTable {
     const float4 *hot;              // DEVICE [n_h][n_zen] = (dd, dt, X_slant, tau_aer)
     const float *full;              // DEVICE [n_h][n_zen][5]
     cudaTextureObject_t tex;        // the hot texels as a 2-D float4 texture (x: zenith node, y: height node), linear filter
+    // flat-plane table (R21): [n_rho][n_h][n_zen] texels; E = (dd, dt, X_slant, tau_aer) even in the pointing angle,
+    // O = (dd odd, dt odd, transverse displacement P, 0)
+    int n_rho;
+    float rho_max, inv_drho, e_max;
+    const float4 *flatE, *flatO;
 };
 
 // Uniform grid over the telescope array.  Every cell lists the telescopes that a point of the cell
@@ -146,6 +151,9 @@ struct TableBuildArgs {
     double h_max, zen_max;
     float *full;                    // [n_h][n_zen][5]
     float4 *hot;                    // [n_h][n_zen]
+    int n_rho;                      // flat-plane table (R21): nodes in rho, 0: none
+    double rho_max;
+    float4 *flatE, *flatO;          // [n_rho][n_h][n_zen] each
 };
 
 struct SubstepArgs {

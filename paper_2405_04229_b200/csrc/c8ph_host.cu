@@ -32,6 +32,7 @@ struct c8ph_ctx {
     c8ph_table_desc tab_desc{};
     float *d_full = nullptr;
     float4 *d_hot = nullptr;
+    float4 *d_flat = nullptr;          // flat-plane table (R21): E texels then O texels
     cudaArray_t tab_arr = nullptr;     // the hot texels as a 2-D array behind a texture object (DevTable::tex)
     cudaTextureObject_t tab_tex = 0;
     // detector
@@ -131,7 +132,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp);
-    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel);
+    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel); dfree(ctx->d_flat);
     if (ctx->tab_tex) cudaDestroyTextureObject(ctx->tab_tex);
     if (ctx->tab_arr) cudaFreeArray(ctx->tab_arr);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
@@ -250,8 +251,10 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
         !(t->zen_max_deg > 0.f) || !(t->zen_max_deg < 90.f))
         return fail(ctx, C8PH_E_ARG, "trace_table: need n_h,n_zen >= 2, h_max > 0, 0 < zen_max < 90");
     if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "trace_table: atmosphere not initialised");
+    if (t->n_rho < 0 || t->n_rho == 1 || t->n_rho > 4096 || (t->n_rho >= 2 && (!(t->rho_max_m > 0.f) || ctx->atm.model != C8PH_ATM_SPHERICAL)))
+        return fail(ctx, C8PH_E_ARG, "trace_table: the flat-plane table needs n_rho >= 2, rho_max_m > 0 and the spherical model");
     CU(cudaSetDevice(ctx->device));
-    dfree(ctx->d_full); dfree(ctx->d_hot);
+    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_flat);
     const size_t n = (size_t)t->n_h * t->n_zen;
     CU(cudaMalloc(&ctx->d_full, n * C8PH_TABLE_CHANNELS * sizeof(float)));
     CU(cudaMalloc(&ctx->d_hot, n * sizeof(float4)));
@@ -264,6 +267,13 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
     d.inv_dz = (float)((t->n_zen - 1) / zmax);
     d.f_max = (float)(t->n_h - 1); d.g_max = (float)(t->n_zen - 1);
     d.hot = ctx->d_hot; d.full = ctx->d_full;
+    d.n_rho = 0; d.rho_max = 0.f; d.inv_drho = 0.f; d.e_max = 0.f; d.flatE = d.flatO = nullptr;
+    if (t->n_rho >= 2) {
+        CU(cudaMalloc(&ctx->d_flat, 2 * (size_t)t->n_rho * n * sizeof(float4)));
+        d.n_rho = t->n_rho; d.rho_max = t->rho_max_m; d.inv_drho = (float)((t->n_rho - 1) / (double)t->rho_max_m);
+        d.e_max = (float)(t->n_rho - 1);
+        d.flatE = ctx->d_flat; d.flatO = ctx->d_flat + (size_t)t->n_rho * n;
+    }
     // texture view of the hot texels: x = zenith node, y = height node, unnormalised coordinates, clamped, bilinear
     if (ctx->tab_tex) { cudaDestroyTextureObject(ctx->tab_tex); ctx->tab_tex = 0; }
     if (ctx->tab_arr) { cudaFreeArray(ctx->tab_arr); ctx->tab_arr = nullptr; }
@@ -305,12 +315,26 @@ extern "C" int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, v
     a.h_max = t->h_max_m;
     a.zen_max = (double)t->zen_max_deg * (3.14159265358979323846 / 180.0);
     a.full = ctx->d_full; a.hot = ctx->d_hot;
+    a.n_rho = ctx->tab.n_rho; a.rho_max = ctx->tab.rho_max;
+    a.flatE = const_cast<float4 *>(ctx->tab.flatE); a.flatO = const_cast<float4 *>(ctx->tab.flatO);
     cudaError_t e = launch_build_table(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "build_trace_table launch");
     rc = fill_table_texture(ctx, (cudaStream_t)stream);
     if (rc) return rc;
-    ctx->launches++;
+    ctx->launches += ctx->tab.n_rho >= 2 ? 2 : 1;
     ctx->have_table = true;
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_get_trace_table_flat(c8ph_ctx *ctx, float *host_out, int64_t n_floats)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!ctx->have_table || ctx->tab.n_rho < 2) return fail(ctx, C8PH_E_STATE, "get_trace_table_flat: no flat-plane table");
+    const int64_t need = 2ll * ctx->tab.n_rho * ctx->tab.n_h * ctx->tab.n_zen * 4;
+    if (!host_out || n_floats < need) return fail(ctx, C8PH_E_ARG, "get_trace_table_flat: buffer too small");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(host_out, ctx->d_flat, need * sizeof(float), cudaMemcpyDeviceToHost));
     return C8PH_OK;
 }
 
@@ -330,6 +354,7 @@ extern "C" int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, con
 {
     if (!ctx) return C8PH_E_ARG;
     if (!host_in) return fail(ctx, C8PH_E_ARG, "set_trace_table: host_in is NULL");
+    if (t && t->size == sizeof(c8ph_table_desc) && t->n_rho != 0) return fail(ctx, C8PH_E_ARG, "set_trace_table: n_rho must be 0 (the flat-plane table is built, not injected)");
     int rc = alloc_table(ctx, t);
     if (rc) return rc;
     const size_t n = (size_t)t->n_h * t->n_zen;
@@ -704,7 +729,10 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     }
     r.n_lines = 0; r.line_nm = nullptr; r.line_cdf = nullptr;
     r.force_generic = ctx->force_generic ? 1 : 0;
-    r.flat_plane = (p->flat_plane && ctx->atm.model == C8PH_ATM_SPHERICAL && p->trace != C8PH_TRACE_STRAIGHT) ? 1 : 0;
+    if (p->flat_plane < 0 || p->flat_plane > 2) return fail(ctx, C8PH_E_ARG, "emit_propagate: flat_plane must be 0, 1 or 2");
+    r.flat_plane = (p->flat_plane && ctx->atm.model == C8PH_ATM_SPHERICAL && p->trace != C8PH_TRACE_STRAIGHT) ? p->flat_plane : 0;
+    if (r.flat_plane == 2 && (p->trace != C8PH_TRACE_TABLE || ctx->tab.n_rho < 2))
+        return fail(ctx, C8PH_E_STATE, "emit_propagate: flat_plane = 2 needs table tracing and a trace table built with n_rho >= 2");
     r.n_eff = p->use_efficiency ? ctx->n_eff : 0; r.eff = p->use_efficiency ? ctx->d_eff : nullptr;
     r.eff_l0 = ctx->eff_l0; r.eff_inv_dl = ctx->n_eff > 1 ? 1.0f / ctx->eff_dl : 0.f;
     r.disp_b = p->emit == C8PH_EMIT_CHERENKOV ? p->disp_b_nm2 : 0.f;

@@ -360,6 +360,48 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
     return o;
 }
 
+// R21: lookup in the flat-plane table: trilinear in (height, zenith, rho) on the even and the odd texels (16 LDG.128),
+// value = E + cos(chi) O along the direction of flight; perp = P, the displacement along (r^ - cos(chi) e_h)
+__device__ __forceinline__ TabVal table_lookup_flat(const DevTable &t, float h, float thz, float rho, float cos_chi, float &perp)
+{
+    TabVal o;
+    o.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f) || !(rho <= t.rho_max);
+    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
+    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
+    const float e = fminf(fmaxf(rho * t.inv_drho, 0.f), t.e_max);
+    const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2), ic = min((int)e, t.n_rho - 2);
+    const float ff = f - (float)ia, gg = g - (float)ib, ee = e - (float)ic;
+    const unsigned plane = (unsigned)(t.n_h * t.n_zen);
+    const unsigned base = (unsigned)ic * plane + (unsigned)(ia * t.n_zen + ib);
+    const float w11 = ff * gg, w10 = ff - w11, w01 = gg - w11, w00 = (1.f - ff) - w01;
+    float4 acc[2];
+#pragma unroll
+    for (int part = 0; part < 2; ++part) {
+        const float4 *p = (part ? t.flatO : t.flatE) + base;
+        float4 lay[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const float4 *pq = p + (unsigned)q * plane;
+            const float4 v00 = __ldg(pq), v01 = __ldg(pq + 1), v10 = __ldg(pq + t.n_zen), v11 = __ldg(pq + t.n_zen + 1);
+            lay[q].x = fmaf(w11, v11.x, fmaf(w10, v10.x, fmaf(w01, v01.x, w00 * v00.x)));
+            lay[q].y = fmaf(w11, v11.y, fmaf(w10, v10.y, fmaf(w01, v01.y, w00 * v00.y)));
+            lay[q].z = fmaf(w11, v11.z, fmaf(w10, v10.z, fmaf(w01, v01.z, w00 * v00.z)));
+            lay[q].w = fmaf(w11, v11.w, fmaf(w10, v10.w, fmaf(w01, v01.w, w00 * v00.w)));
+        }
+        acc[part].x = fmaf(ee, lay[1].x - lay[0].x, lay[0].x);
+        acc[part].y = fmaf(ee, lay[1].y - lay[0].y, lay[0].y);
+        acc[part].z = fmaf(ee, lay[1].z - lay[0].z, lay[0].z);
+        acc[part].w = fmaf(ee, lay[1].w - lay[0].w, lay[0].w);
+    }
+    o.dd = fmaf(cos_chi, acc[1].x, acc[0].x);
+    o.dt = fmaf(cos_chi, acc[1].y, acc[0].y);
+    o.X = acc[0].z;
+    o.ta = acc[0].w;
+    perp = acc[1].z;
+    o.bad = o.bad || (o.dd != o.dd) || (perp != perp);
+    return o;
+}
+
 // ---- telescope search (DevGrid: sorted candidate lists with a per-cell smallest key) -----------
 // cell of (x,y), or -1 outside the grid (outside => no telescope within reach)
 __device__ __forceinline__ int grid_cell(const DevGrid &g, float x, float y)
@@ -497,7 +539,7 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_NONFINITE, WC_EMITTED, 
 // roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present) and
 // compiles in the optional features whose bits are set; the host picks the variant when the call
 // matches one that is instantiated (launch_emit_propagate).  SPEC = 0 reads every switch at run time.
-constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32;
+constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32, kSpecFlatTab = 64;
 template <int EMIT, int TRACE, bool SPH, int SPEC>
 __global__ void __launch_bounds__(kernel_threads(TRACE), kernel_min_blocks(TRACE))
 k_emit_propagate(const __grid_constant__ KArgs a)
@@ -581,7 +623,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     const bool f_eff = SPEC ? (SPEC & kSpecEff) != 0 : run.n_eff > 0;
     const bool f_opt = SPEC ? (SPEC & kSpecOpt) != 0 : det.opt_enabled != 0;
     const bool f_ext = SPEC ? (SPEC & kSpecExt) != 0 : atm.n_ext > 0;
-    const bool f_flat = (!SPH || TRACE == C8PH_TRACE_STRAIGHT) ? false : (SPEC ? (SPEC & kSpecFlat) != 0 : run.flat_plane != 0);
+    // flat observation plane: 1 = analytic step from the sphere (R19), 2 = the thesis' table with rho and pointing axes (R21)
+    const int f_flat_mode = (!SPH || TRACE == C8PH_TRACE_STRAIGHT) ? 0 : (SPEC ? ((SPEC & kSpecFlat) ? 1 : ((SPEC & kSpecFlatTab) ? 2 : 0)) : run.flat_plane);
+    const bool f_flat = f_flat_mode == 1;
+    const bool f_flat_tab = TRACE == C8PH_TRACE_TABLE && f_flat_mode == 2;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
     const bool f_photons = SPEC ? true : run.out.photons != nullptr;
@@ -1158,6 +1203,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     }
                     // local zenith angle of the photon at the emission point
                     float dd = 0.f, dt = 0.f, Xs = 0.f, ta = 0.f, cz;
+                    float flat_perp = 0.f, flat_px = 0.f, flat_py = 0.f;      // R21: transverse displacement and its direction
                     if (EARLY_TAB) cz = cz_e;
                     else if (SPH) {
                         float ur;
@@ -1174,7 +1220,17 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (TRACE == C8PH_TRACE_STRAIGHT) {
                         dt = eta_e * D * kInvC;                          // homogeneous: t = t_e + n D / c
                     } else if (TRACE == C8PH_TRACE_TABLE) {
-                        const TabVal v = EARLY_TAB ? table_combine(traw) : table_lookup(a.tab, h_e, acos01(fmaxf(cz, 0.f)));
+                        TabVal v;
+                        if (f_flat_tab) {
+                            // R21: polar radius of the straight-line point and pointing angle of the direction of flight
+                            const float hn2f = ux * ux + uy * uy, rho2 = fmaf(xl, xl, yl * yl);
+                            const float ihf = hn2f >= 1e-18f ? rsqrt_fast(hn2f) : 0.f, irho = rho2 >= 1e-18f ? rsqrt_fast(rho2) : 0.f;
+                            const float rx = xl * irho, ry = yl * irho;          // outward radial direction
+                            const float cchi = (ux * rx + uy * ry) * ihf;
+                            v = table_lookup_flat(a.tab, h_e, acos01(fmaxf(cz, 0.f)), rho2 * irho, cchi, flat_perp);
+                            flat_px = fmaf(-cchi * ihf, ux, rx); flat_py = fmaf(-cchi * ihf, uy, ry);
+                        } else
+                            v = EARLY_TAB ? table_combine(traw) : table_lookup(a.tab, h_e, acos01(fmaxf(cz, 0.f)));
                         if (v.bad || !(cz > 0.f)) { pkB += 1u; break; }
                         dd = v.dd; dt = v.dt; Xs = v.X; ta = v.ta;
                     } else {
@@ -1268,6 +1324,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float ih = hn2 >= 1e-18f ? rsqrt_fast(hn2) : 0.f;            // vertical photon: no correction
                     const float ehx = ux * ih, ehy = uy * ih;
                     float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);               // offset from the anchor
+                    if (f_flat_tab) { cx = fmaf(flat_perp, flat_px, cx); cy = fmaf(flat_perp, flat_py, cy); }
                     if (f_flat) {
                         // R19, flat observation plane (thesis Fig. 4.10): dd, dt and the rotation hold where
                         // the ray meets the observation sphere; the plane z = 0 lies h_I above it at the line point.
@@ -1428,6 +1485,72 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 // Correction table: one thread per node, exact layered ray in fp64 by the Snell (planar) or
 // Bouguer (spherical) invariant, layer by layer on the n(h) grid (layers = table cells split in
 // `substeps`, n at the layer mid height), minus the straight line to the same sphere / plane.
+struct NodeRay { bool ground; double psi, S, cT, X, tau; };
+
+// exact layered ray from (h_e, zenith th) down to the observation level: central angle (spherical) or horizontal
+// displacement (planar), geometric path, optical path, slant depth, aerosol optical depth
+__device__ NodeRay trace_node(const DevAtm &atm, double h_e, double th, int substeps)
+{
+    NodeRay o;
+    o.ground = true; o.psi = o.S = o.cT = o.X = o.tau = 0.0;
+    const bool sph = atm.model == C8PH_ATM_SPHERICAL;
+    const double h_g = atm.h_obs;
+    const double sz = sin(th);
+    const double n_e = 1.0 + eta_lookup_d(atm, h_e);
+    const double K = sph ? n_e * (atm.R + h_e) * sz : n_e * sz;     // Bouguer / Snell invariant
+    const double step = atm.model == C8PH_ATM_HOMOGENEOUS ? 1.0e30 : (double)atm.dh / substeps;
+    double h_cur = h_e;
+    auto xv_at = [&](double h) {
+        double f = (h - (double)atm.h0) / (double)atm.dh;
+        f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
+        const int k = min((int)f, atm.n_nodes - 2);
+        const double fr = f - k;
+        return (1.0 - fr) * (double)__ldg(atm.xv + k) + fr * (double)__ldg(atm.xv + k + 1);
+    };
+    double xv_cur = xv_at(h_cur);
+    double ea_cur = atm.aer_L > 0.f ? exp(-h_cur / (double)atm.aer_H) : 0.0;
+    while (h_cur > h_g) {
+        double h_next;
+        if (atm.model == C8PH_ATM_HOMOGENEOUS) h_next = h_g;
+        else {
+            const double g = floor((h_cur - (double)atm.h0) / step);
+            h_next = (double)atm.h0 + g * step;
+            if (!(h_next < h_cur - 1e-9 * step)) h_next = (double)atm.h0 + (g - 1.0) * step;
+            if (h_next < h_g) h_next = h_g;
+        }
+        const double n_l = 1.0 + eta_lookup_d(atm, 0.5 * (h_cur + h_next));
+        const double dhl = h_cur - h_next;
+        double s;
+        if (sph) {
+            const double p = K / n_l;                                // impact parameter of the chord
+            const double rt = atm.R + h_cur, rb = atm.R + h_next;
+            if (!(rb > p)) { o.ground = false; break; }
+            const double at = sqrt(rt * rt - p * p), ab = sqrt(rb * rb - p * p);
+            s = dhl * (rt + rb) / (at + ab);                         // at - ab, cancellation-free
+            const double x = p * s / (rt * rb);                      // sin of the central-angle step
+            o.psi += x * (1.0 + x * x * (1.0 / 6.0 + x * x * (3.0 / 40.0)));
+        } else {
+            const double q2 = n_l * n_l - K * K;
+            if (!(q2 > 0.0)) { o.ground = false; break; }
+            const double iq = 1.0 / sqrt(q2);
+            s = dhl * n_l * iq;
+            o.psi += dhl * K * iq;                                   // horizontal displacement
+        }
+        o.S += s;
+        o.cT += n_l * s;
+        const double xv_next = xv_at(h_next);
+        o.X += (xv_next - xv_cur) * (s / dhl);
+        xv_cur = xv_next;
+        if (atm.aer_L > 0.f) {
+            const double ea_next = exp(-h_next / (double)atm.aer_H);
+            o.tau += ((double)atm.aer_H / (double)atm.aer_L) * (ea_next - ea_cur) * (s / dhl);
+            ea_cur = ea_next;
+        }
+        h_cur = h_next;
+    }
+    return o;
+}
+
 __global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ TableBuildArgs a)
 {
     const int node = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1441,76 +1564,24 @@ __global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ Tab
     const double h_g = atm.h_obs;
     if (h_e > h_g) {
         const double sz = sin(th), cz = cos(th);
-        const double n_e = 1.0 + eta_lookup_d(atm, h_e);
-        const double K = sph ? n_e * (atm.R + h_e) * sz : n_e * sz;     // Bouguer / Snell invariant
-        const double step = atm.model == C8PH_ATM_HOMOGENEOUS ? 1.0e30 : (double)atm.dh / a.substeps;
-        double h_cur = h_e, psi = 0.0, S = 0.0, cT = 0.0, X = 0.0, tau = 0.0;
-        bool ground = true;
-        auto xv_at = [&](double h) {
-            double f = (h - (double)atm.h0) / (double)atm.dh;
-            f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
-            const int k = min((int)f, atm.n_nodes - 2);
-            const double fr = f - k;
-            return (1.0 - fr) * (double)__ldg(atm.xv + k) + fr * (double)__ldg(atm.xv + k + 1);
-        };
-        double xv_cur = xv_at(h_cur);
-        double ea_cur = atm.aer_L > 0.f ? exp(-h_cur / (double)atm.aer_H) : 0.0;
-        while (h_cur > h_g) {
-            double h_next;
-            if (atm.model == C8PH_ATM_HOMOGENEOUS) h_next = h_g;
-            else {
-                const double g = floor((h_cur - (double)atm.h0) / step);
-                h_next = (double)atm.h0 + g * step;
-                if (!(h_next < h_cur - 1e-9 * step)) h_next = (double)atm.h0 + (g - 1.0) * step;
-                if (h_next < h_g) h_next = h_g;
-            }
-            const double n_l = 1.0 + eta_lookup_d(atm, 0.5 * (h_cur + h_next));
-            const double dhl = h_cur - h_next;
-            double s;
-            if (sph) {
-                const double p = K / n_l;                                // impact parameter of the chord
-                const double rt = atm.R + h_cur, rb = atm.R + h_next;
-                if (!(rb > p)) { ground = false; break; }
-                const double at = sqrt(rt * rt - p * p), ab = sqrt(rb * rb - p * p);
-                s = dhl * (rt + rb) / (at + ab);                         // at - ab, cancellation-free
-                const double x = p * s / (rt * rb);                      // sin of the central-angle step
-                psi += x * (1.0 + x * x * (1.0 / 6.0 + x * x * (3.0 / 40.0)));
-            } else {
-                const double q2 = n_l * n_l - K * K;
-                if (!(q2 > 0.0)) { ground = false; break; }
-                const double iq = 1.0 / sqrt(q2);
-                s = dhl * n_l * iq;
-                psi += dhl * K * iq;                                     // horizontal displacement
-            }
-            S += s;
-            cT += n_l * s;
-            const double xv_next = xv_at(h_next);
-            X += (xv_next - xv_cur) * (s / dhl);
-            xv_cur = xv_next;
-            if (atm.aer_L > 0.f) {
-                const double ea_next = exp(-h_next / (double)atm.aer_H);
-                tau += ((double)atm.aer_H / (double)atm.aer_L) * (ea_next - ea_cur) * (s / dhl);
-                ea_cur = ea_next;
-            }
-            h_cur = h_next;
-        }
-        if (ground) {
+        const NodeRay r = trace_node(atm, h_e, th, a.substeps);
+        if (r.ground) {
             double S_line, d_line, d_true;
             if (sph) {
                 const double re = atm.R + h_e, rg = atm.Rg, p = re * sz;
                 S_line = re * cz - sqrt(rg * rg - p * p);
                 d_line = rg * (asin(p / rg) - th);
-                d_true = rg * psi;
+                d_true = rg * r.psi;
             } else {
                 S_line = (h_e - h_g) / cz;
                 d_line = (h_e - h_g) * sz / cz;
-                d_true = psi;
+                d_true = r.psi;
             }
             out[0] = (float)(d_true - d_line);
-            out[1] = (float)(S - S_line);
-            out[2] = (float)((cT - S_line) / kC);
-            out[3] = (float)X;
-            out[4] = (float)tau;
+            out[1] = (float)(r.S - S_line);
+            out[2] = (float)((r.cT - S_line) / kC);
+            out[3] = (float)r.X;
+            out[4] = (float)r.tau;
         } else {
             const float nanv = __int_as_float(0x7FC00000);
             for (int k = 0; k < 5; ++k) out[k] = nanv;
@@ -1518,6 +1589,134 @@ __global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ Tab
     }
     for (int k = 0; k < 5; ++k) a.full[(size_t)node * 5 + k] = out[k];
     a.hot[node] = make_float4(out[0], out[2], out[3], out[4]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// R21: the thesis' table "relative to a flat observation plane" (Fig. 4.10; spherical model): axes height,
+// local zenith, rho = polar radius of the straight-line point on the plane z = 0, and the pointing angle chi of the
+// horizontal direction of flight against the outward radial direction there, kept as even part E (texels as the 2-D
+// table: dd, dt, X_slant, tau_aer), odd part O (dd, dt) and transverse displacement P in one more texel (O.dd, O.dt, P, 0):
+// value = E + cos(chi) O along the direction of flight, P (r^ - cos(chi) e_h) across it.  One thread per (height,
+// zenith) node traces the ray once and takes it from the observation sphere on to the plane for every rho.
+struct Vec3d { double x, y, z; };
+__device__ __forceinline__ double dot3(const Vec3d &a, const Vec3d &b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+
+// from the sphere to the plane: line from A along u to the sphere r = Rg, arc dd along the direction of flight, back
+// along the arrival direction ua (straight, ground index) to z = 0.  Returns false if the line misses the sphere.
+__device__ bool sphere_to_plane(const DevAtm &atm, const Vec3d &A, const Vec3d &u, double h_e, double sz, double cz, double dd,
+                                double dt_ns, const Vec3d &ua, double &x, double &y, double &t_rel)
+{
+    const double Rg = atm.Rg, re = atm.R + h_e, pp = re * sz;
+    if (!(pp < Rg)) return false;
+    const double S_line = re * cz - sqrt(Rg * Rg - pp * pp);
+    Vec3d w = {A.x + S_line * u.x, A.y + S_line * u.y, A.z + S_line * u.z + Rg};
+    const double wn = 1.0 / sqrt(dot3(w, w));
+    w.x *= wn; w.y *= wn; w.z *= wn;
+    const double cw = dot3(u, w);
+    Vec3d et = {u.x - cw * w.x, u.y - cw * w.y, u.z - cw * w.z};
+    const double en = sqrt(dot3(et, et));
+    if (en < 1e-12) et.x = et.y = et.z = 0.0; else { et.x /= en; et.y /= en; et.z /= en; }
+    const double ca = cos(dd / Rg), sa = sin(dd / Rg);
+    const Vec3d Pr = {Rg * (ca * w.x + sa * et.x), Rg * (ca * w.y + sa * et.y), Rg * (ca * w.z + sa * et.z) - Rg};
+    const double s_back = Pr.z / ua.z;
+    x = Pr.x - s_back * ua.x;
+    y = Pr.y - s_back * ua.y;
+    t_rel = S_line / kC + dt_ns - (1.0 + (double)atm.eta_g) * s_back / kC;
+    return true;
+}
+
+// the photon of Fig. 4.10 with its arrival direction: emission point A, direction u, local vertical rv
+__device__ bool flat_photon(const DevAtm &atm, const Vec3d &A, const Vec3d &u, const Vec3d &rv, double h_e, double th, double dd,
+                            double dt_ns, double &x, double &y, double &t_rel)
+{
+    const double sz = sin(th), cz = cos(th);
+    // rotation of the direction in the ray plane from the Bouguer invariant (R9), n at the observation level = 1 + eta_g
+    const double re = atm.R + h_e, Rg = atm.Rg, n_ray = 1.0 + eta_lookup_d(atm, h_e), n_g = 1.0 + (double)atm.eta_g;
+    const double psi_line = asin(re * sz / Rg) - th;
+    const double delta = asin(n_ray * re * sz / (n_g * Rg)) - (psi_line + dd / Rg) - th;
+    Vec3d ua = u;
+    if (sz > 1e-9 && delta != 0.0) {
+        const double cd = cos(delta), sd = sin(delta);
+        ua.x = cd * u.x + sd * (cz * u.x + rv.x) / sz;
+        ua.y = cd * u.y + sd * (cz * u.y + rv.y) / sz;
+        ua.z = cd * u.z + sd * (cz * u.z + rv.z) / sz;
+    }
+    return sphere_to_plane(atm, A, u, h_e, sz, cz, dd, dt_ns, ua, x, y, t_rel);
+}
+
+__global__ void __launch_bounds__(128) k_build_table_flat(const __grid_constant__ TableBuildArgs a)
+{
+    const int node = blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= a.n_h * a.n_zen) return;
+    const int ia = node / a.n_zen, ib = node % a.n_zen;
+    const DevAtm &atm = a.atm;
+    const double h_e = ia * a.h_max / (a.n_h - 1);
+    const double th = ib * a.zen_max / (a.n_zen - 1);
+    const size_t plane = (size_t)a.n_h * a.n_zen;
+    const float nanv = __int_as_float(0x7FC00000);
+    const bool zero = !(h_e > atm.h_obs);
+    NodeRay r;
+    r.ground = false;
+    double dd = 0.0, dt_sph = 0.0, S_line_sph = 0.0;
+    const double sz = sin(th), cz = cos(th), Rg = atm.Rg, re = atm.R + h_e;
+    if (!zero) {
+        r = trace_node(atm, h_e, th, a.substeps);
+        if (r.ground) {
+            const double p = re * sz;
+            S_line_sph = re * cz - sqrt(Rg * Rg - p * p);
+            dd = Rg * r.psi - Rg * (asin(p / Rg) - th);
+            dt_sph = (r.cT - S_line_sph) / kC;
+        }
+    }
+    for (int c = 0; c < a.n_rho; ++c) {
+        float4 E = make_float4(0.f, 0.f, 0.f, 0.f), O = E;
+        if (!zero) {
+            bool ok = r.ground;
+            const double rho = a.rho_max * c / (a.n_rho - 1);
+            double T[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, P = 0.0;
+            for (int sgn = 0; sgn < 2 && ok; ++sgn) {
+                // radial flight: emission point (re sin(beta), 0, re cos(beta) - Rg), direction (sin(th - beta), 0, -cos(th - beta));
+                // its straight line meets z = 0 at x(beta) = E_x + E_z tan(th - beta) = +-rho (bisection)
+                const double xt = sgn ? -rho : rho;
+                double lo = -0.2, hi = 0.2, beta = 0.0;
+                for (int it = 0; it < 64; ++it) {
+                    beta = 0.5 * (lo + hi);
+                    if (re * sin(beta) + (re * cos(beta) - Rg) * tan(th - beta) < xt) lo = beta; else hi = beta;
+                }
+                const Vec3d A = {re * sin(beta), 0.0, re * cos(beta) - Rg};
+                ok = A.z > 0.0 && cos(th - beta) > 1e-3 && fabs(A.x + A.z * tan(th - beta) - xt) <= 1e-6 * (1.0 + fabs(xt));
+                if (!ok) break;
+                const Vec3d u = {sin(th - beta), 0.0, -cos(th - beta)}, rv = {sin(beta), 0.0, cos(beta)};
+                double x, y, t_rel;
+                ok = flat_photon(atm, A, u, rv, h_e, th, dd, dt_sph, x, y, t_rel);
+                const double D = A.z / cos(th - beta);
+                T[sgn][0] = x - xt;
+                T[sgn][1] = t_rel - D / kC;
+            }
+            if (ok) {
+                // tangential flight: straight-line point (rho, 0, 0), flying along +y; emission point in closed form
+                const double c2 = (re * re * cz * cz + rho * rho + Rg * Rg - re * re) / (Rg * Rg);
+                ok = c2 > 1e-6 && c2 <= 1.0;
+                if (ok) {
+                    const double cg = sqrt(c2), sg = sqrt(1.0 - c2), sd = -Rg * cg + re * cz;
+                    ok = sd > 0.0;
+                    const Vec3d A = {rho, -sd * sg, sd * cg}, u = {0.0, sg, -cg};
+                    const Vec3d rv = {A.x / re, A.y / re, (A.z + Rg) / re};
+                    double x, y, t_rel;
+                    ok = ok && flat_photon(atm, A, u, rv, h_e, th, dd, dt_sph, x, y, t_rel);
+                    P = x - rho;
+                }
+            }
+            if (ok) {
+                E = make_float4((float)(0.5 * (T[0][0] + T[1][0])), (float)(0.5 * (T[0][1] + T[1][1])), (float)r.X, (float)r.tau);
+                O = make_float4((float)(0.5 * (T[0][0] - T[1][0])), (float)(0.5 * (T[0][1] - T[1][1])), (float)P, 0.f);
+            } else {
+                E = O = make_float4(nanv, nanv, nanv, nanv);
+            }
+        }
+        a.flatE[(size_t)c * plane + node] = E;
+        a.flatO[(size_t)c * plane + node] = O;
+    }
 }
 
 template <int EMIT, int TRACE, bool SPH, int SPEC>
@@ -1570,7 +1769,7 @@ static int array_production_setting(const KArgs &a)
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
            r.out.tel_counts != nullptr && !r.force_generic;
     if (!base) return 0;
-    return kSpecBase | (r.flat_plane ? kSpecFlat : 0) | (a.atm.n_ext > 0 ? kSpecExt : 0) | (r.disp_b != 0.f ? kSpecDisp : 0) |
+    return kSpecBase | (r.flat_plane == 1 ? kSpecFlat : 0) | (r.flat_plane == 2 ? kSpecFlatTab : 0) | (a.atm.n_ext > 0 ? kSpecExt : 0) | (r.disp_b != 0.f ? kSpecDisp : 0) |
            (r.n_eff > 0 ? kSpecEff : 0) | (d.opt_enabled ? kSpecOpt : 0);
 }
 
@@ -1590,6 +1789,7 @@ cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
     if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, smem, st);
 #endif
     C8_SPEC(kSpecFlat)
+    C8_SPEC(kSpecFlatTab)
     C8_SPEC(kSpecExt)
     C8_SPEC(kSpecDisp)
     C8_SPEC(kSpecEff)
@@ -1618,6 +1818,7 @@ cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st)
 {
     const int n = a.n_h * a.n_zen;
     k_build_table<<<(n + 127) / 128, 128, 0, st>>>(a);
+    if (a.n_rho >= 2 && a.flatE && a.flatO) k_build_table_flat<<<(n + 127) / 128, 128, 0, st>>>(a);
     return cudaGetLastError();
 }
 

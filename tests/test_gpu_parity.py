@@ -765,6 +765,54 @@ def test_flat_observation_plane_far_from_the_origin():
     assert near_on["counters"]["landed"] == near_off["counters"]["landed"] and moved <= 1e-4 * near_on["counters"]["emitted"]
 
 
+_FLAT_TABLE = dict(n_h=256, n_zen=256, h_max=50000.0, zen_max_deg=80.0, n_rho=16, rho_max_m=30000.0)
+
+
+def test_flat_plane_table_nodes_and_photons_against_the_oracle(monkeypatch):
+    """Row f1 (thesis P:861, Fig. 4.10; R21): the table relative to the flat observation plane over (height,
+    zenith, polar radius, pointing angle).  Device nodes against the oracle's (0.1 mm / 0.3 ps where the 2-D nodes
+    agree to that); photons with flat_plane = 2 against the oracle, array 18 km from the origin, cfg4's near-vertical
+    tracks and tracks inclined by 60 degrees (every azimuth, so every pointing angle); the compiled variant and the
+    generic kernel agree; against the analytic step (flat_plane = 1) the positions stay within 1 mm."""
+    cfg = _off_centre(4, 2500, 18000.0, None, flat_plane=2)
+    cfg["table"] = dict(cfg["table"], **_FLAT_TABLE)
+    ctx = api.setup_context(cfg)
+    got = ctx.get_trace_table_flat()
+    want = O.table_flat_for(cfg)
+    assert got.shape == (2, 16, 256, 256, 4) and want.shape == (2, 16, 256, 256, 5)
+    zen = np.linspace(0.0, 80.0, 256)
+    for part, chans in ((0, ((0, 0, 1e-4), (1, 2, 3e-4), (2, 3, 1e-2))), (1, ((0, 0, 1e-4), (1, 2, 3e-4), (2, 3, 1e-4)))):
+        for cg, cw, tol in chans:
+            g, w = got[part, ..., cg].astype(np.float64), want[part, ..., cw].astype(np.float64)
+            ok = np.isfinite(g) & np.isfinite(w) & (zen[None, None, :] <= 70.0)
+            assert ok.mean() > 0.7 and np.abs(g - w)[ok].max() <= tol, (part, cg, np.abs(g - w)[ok].max())
+    assert (np.isfinite(got[0, ..., 0]) != np.isfinite(want[0, ..., 0])).mean() < 1e-3
+    for zen_deg, n in ((None, 2500), (60.0, 1500)):
+        c2 = _off_centre(4, n, 18000.0, zen_deg, flat_plane=2)
+        c2["table"] = dict(c2["table"], **_FLAT_TABLE)
+        ora, gpu, rep = _both(c2)
+        assert gpu["counters"]["tel_hit"] > 1e4 and gpu["counters"]["in_grid"] > 1e5 and rep["max_dpos_m"] < 0.02
+        monkeypatch.setenv("C8PH_FORCE_GENERIC", "1")
+        gen = api.run_config(c2, ctx=api.setup_context(c2))
+        monkeypatch.setenv("C8PH_FORCE_GENERIC", "0")
+        parity.compare(c2, ora, gen)
+        c1 = copy.deepcopy(c2)
+        c1["params"]["flat_plane"] = 1
+        step = O.run(c1)
+        a, b = ora["photons"], step["photons"]
+        both = (a["status"] == O.ST_LANDED) & (b["status"] == O.ST_LANDED)
+        assert both.sum() > 1e5 and np.hypot(a["x"][both] - b["x"][both], a["y"][both] - b["y"][both]).max() < 1e-3
+    # beyond rho_max the lookup is out of range: counted, not extrapolated
+    far = _off_centre(4, 400, 31000.0, None, flat_plane=2)
+    far["table"] = dict(far["table"], **_FLAT_TABLE)
+    res = api.run_config(far)
+    assert res["counters"]["table_range"] > 0.5 * (res["counters"]["emitted"] - res["counters"]["lv2"] - res["counters"]["upgoing"])
+    # flat_plane = 2 without the extra axes is a state error
+    with pytest.raises(api.C8phError) as e:
+        api.run_config(_off_centre(4, 100, 0.0, None, flat_plane=2))
+    assert e.value.code == api.E_STATE
+
+
 def test_compiled_feature_variants_and_the_generic_kernel_agree(monkeypatch):
     """The "production setting + optional features" calls run kernel variants with the features compiled in (SPEC bit
     mask); C8PH_FORCE_GENERIC=1 sends the same call through the generic variant that reads every switch at run time.
