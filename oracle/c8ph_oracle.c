@@ -104,6 +104,11 @@ typedef struct {
     int32_t opt_enabled, pad3;
     double opt_az_deg, opt_el_deg;         /* pointing direction of every telescope */
     double opt_focal_m, opt_mirror_radius_m, opt_camera_radius_m;
+    /* reading R22 (thesis sec. 6.4: "light bending at a boundary layer (e.g. lens ...)", "absorption by objects") */
+    int32_t opt_kind, opt_n_abs;           /* 0: parabolic mirror (R15); 1: plano-convex lens.  absorbing capsules (<= 8) */
+    double opt_lens_roc_m, opt_lens_thickness_m, opt_lens_index;
+    double opt_abs[8][7];                  /* capsule axis end points and radius (x0,y0,z0,x1,y1,z1,r) in the telescope
+                                              frame (right, up, axis) about the bounding-sphere centre */
 } orc_detector;
 
 enum { ORC_EMIT_CHERENKOV = 0, ORC_EMIT_FLUOR = 1 };
@@ -774,7 +779,64 @@ int orc_camera_pixel(const orc_detector *det, const double u_arr[3])
  * out: res[0..1] camera-plane coordinates, res[2..4] reflected direction (e_r, e_u, w components),
  *      res[5] path length from I to the camera along the ray (may start before I: s < 0 allowed)
  * returns 1 camera hit, 0 missed mirror / camera, -1 shadowed by the camera. */
-int orc_last_mile(const orc_detector *det, const double I[3], const double u[3], const double c[3], double res[6])
+/* Snell's law in vector form (Eq. 3.15) at a surface with unit normal N (pointing against the incoming ray or
+ * along it: the sign is taken from u.N), from index n1 into n2: u2 = (n1 u + (sqrt(n2^2 - n1^2 + (n1 u.N)^2) - n1 |u.N|) N')/n2
+ * with N' = N turned along the direction of propagation.  Returns 0 on total internal reflection (Fig. 6.6a). */
+int orc_refract(const double u[3], const double N[3], double n1, double n2, double out[3])
+{
+    double c = u[0]*N[0] + u[1]*N[1] + u[2]*N[2];
+    double sgn = c < 0.0 ? -1.0 : 1.0;                           /* N' = sgn N points along the ray */
+    double ca = fabs(c);
+    double q = n2*n2 - n1*n1 + n1*n1*ca*ca;
+    if (q < 0.0) return 0;
+    double k = sqrt(q) - n1 * ca;
+    for (int i = 0; i < 3; ++i) out[i] = (n1 * u[i] + k * sgn * N[i]) / n2;
+    return 1;
+}
+
+/* smallest distance between the segments P0 + s (P1 - P0), s in [0,1], and Q0 + t (Q1 - Q0), t in [0,1] */
+double orc_segment_distance(const double P0[3], const double P1[3], const double Q0[3], const double Q1[3])
+{
+    double d1[3], d2[3], r[3];
+    for (int k = 0; k < 3; ++k) { d1[k] = P1[k] - P0[k]; d2[k] = Q1[k] - Q0[k]; r[k] = P0[k] - Q0[k]; }
+    double a = d1[0]*d1[0] + d1[1]*d1[1] + d1[2]*d1[2], e = d2[0]*d2[0] + d2[1]*d2[1] + d2[2]*d2[2];
+    double f = d2[0]*r[0] + d2[1]*r[1] + d2[2]*r[2], cc = d1[0]*r[0] + d1[1]*r[1] + d1[2]*r[2];
+    double b = d1[0]*d2[0] + d1[1]*d2[1] + d1[2]*d2[2];
+    double sN, tN;
+    if (a <= 1e-300 && e <= 1e-300) { sN = tN = 0.0; }
+    else if (a <= 1e-300) { sN = 0.0; tN = fmin(fmax(f / e, 0.0), 1.0); }
+    else if (e <= 1e-300) { tN = 0.0; sN = fmin(fmax(-cc / a, 0.0), 1.0); }
+    else {
+        double den = a * e - b * b;
+        sN = den > 1e-300 * a * e ? fmin(fmax((b * f - cc * e) / den, 0.0), 1.0) : 0.0;
+        tN = (b * sN + f) / e;
+        if (tN < 0.0) { tN = 0.0; sN = fmin(fmax(-cc / a, 0.0), 1.0); }
+        else if (tN > 1.0) { tN = 1.0; sN = fmin(fmax((b - cc) / a, 0.0), 1.0); }
+    }
+    double dx = r[0] + sN*d1[0] - tN*d2[0], dy = r[1] + sN*d1[1] - tN*d2[1], dz = r[2] + sN*d1[2] - tN*d2[2];
+    return sqrt(dx*dx + dy*dy + dz*dz);
+}
+
+/* "absorption by objects": is the leg A -> B (telescope frame about the sphere centre) within reach of a capsule? */
+static int leg_absorbed(const orc_detector *det, const double A[3], const double B[3])
+{
+    for (int k = 0; k < det->opt_n_abs && k < 8; ++k) {
+        const double *o = det->opt_abs[k];
+        if (orc_segment_distance(A, B, o, o + 3) <= o[6]) return 1;
+    }
+    return 0;
+}
+
+/* in : I (point on the arrival ray, any), u (unit direction), c (sphere centre), r_sphere (its radius: the incoming leg
+ *      starts where the ray enters the sphere)
+ * out: res[0..1] camera-plane coordinates, res[2..4] direction at the camera (e_r, e_u, w components),
+ *      res[5] optical path length from I to the camera along the ray (may start before I: s < 0 allowed)
+ * returns 1 camera hit, 0 missed mirror / lens / camera, -1 shadowed by the camera, -2 absorbed by an object (R22),
+ *         -3 total internal reflection in the lens (R22).
+ * opt_kind 1 (R22, "light bending at a boundary layer (e.g. lens ...)"): instead of the mirror a plano-convex lens, plane
+ * face (radius R_m) at centre + (f/2) w, convex spherical face (radius of curvature R_l, apex t above the plane face)
+ * towards the sky; camera disc at centre - (f/2) w facing the lens.  Vector Snell at both faces. */
+int orc_last_mile(const orc_detector *det, const double I[3], const double u[3], const double c[3], double r_sphere, double res[6])
 {
     const double d2r = ORC_PI / 180.0;
     const double az = det->opt_az_deg * d2r, el = det->opt_el_deg * d2r;
@@ -782,15 +844,51 @@ int orc_last_mile(const orc_detector *det, const double I[3], const double u[3],
     const double w[3] = { cos(el) * cos(az), cos(el) * sin(az), sin(el) };
     const double er[3] = { -sin(az), cos(az), 0.0 };
     const double eu[3] = { w[1]*er[2] - w[2]*er[1], w[2]*er[0] - w[0]*er[2], w[0]*er[1] - w[1]*er[0] };
-    double p0[3], a, b, z0, dr, du, dw;
-    for (int k = 0; k < 3; ++k) p0[k] = I[k] - (c[k] - 0.5 * f * w[k]);       /* relative to the vertex */
-    a = p0[0]*er[0] + p0[1]*er[1] + p0[2]*er[2];
-    b = p0[0]*eu[0] + p0[1]*eu[1] + p0[2]*eu[2];
-    z0 = p0[0]*w[0] + p0[1]*w[1] + p0[2]*w[2];
+    double pc[3], g[3], dr, du, dw;
+    for (int k = 0; k < 3; ++k) pc[k] = I[k] - c[k];                           /* relative to the sphere centre */
+    g[0] = pc[0]*er[0] + pc[1]*er[1] + pc[2]*er[2];
+    g[1] = pc[0]*eu[0] + pc[1]*eu[1] + pc[2]*eu[2];
+    g[2] = pc[0]*w[0] + pc[1]*w[1] + pc[2]*w[2];
     dr = u[0]*er[0] + u[1]*er[1] + u[2]*er[2];
     du = u[0]*eu[0] + u[1]*eu[1] + u[2]*eu[2];
     dw = u[0]*w[0] + u[1]*w[1] + u[2]*w[2];
-    if (!(dw < 0.0)) return 0;                                  /* not travelling towards the mirror */
+    if (!(dw < 0.0)) return 0;                                  /* not travelling towards the mirror / lens */
+    const double d[3] = { dr, du, dw };
+    /* entry into the bounding sphere: start of the incoming leg */
+    double bq = g[0]*d[0] + g[1]*d[1] + g[2]*d[2], cq = g[0]*g[0] + g[1]*g[1] + g[2]*g[2] - r_sphere*r_sphere;
+    double s_in = -bq - sqrt(fmax(bq*bq - cq, 0.0));
+    double E[3] = { g[0] + s_in*d[0], g[1] + s_in*d[1], g[2] + s_in*d[2] };
+    if (det->opt_kind == 1) {
+        const double Rl = det->opt_lens_roc_m, th = det->opt_lens_thickness_m, nl = det->opt_lens_index;
+        const double zc = 0.5 * f + th - Rl;                    /* centre of curvature on the axis */
+        /* convex face: |g + s d - (0,0,zc)|^2 = Rl^2, the first (upper) intersection */
+        double oc[3] = { g[0], g[1], g[2] - zc };
+        double b2 = oc[0]*d[0] + oc[1]*d[1] + oc[2]*d[2], c2 = oc[0]*oc[0] + oc[1]*oc[1] + oc[2]*oc[2] - Rl*Rl;
+        double disc = b2*b2 - c2;
+        if (disc < 0.0) return 0;
+        double s1 = -b2 - sqrt(disc);
+        double P1[3] = { g[0] + s1*d[0], g[1] + s1*d[1], g[2] + s1*d[2] };
+        if (P1[0]*P1[0] + P1[1]*P1[1] > Rm*Rm || P1[2] < 0.5 * f) return 0;     /* outside the aperture / below the plane face */
+        if (leg_absorbed(det, E, P1)) return -2;
+        double N1[3] = { P1[0] / Rl, P1[1] / Rl, (P1[2] - zc) / Rl }, v[3], v2[3];
+        if (!orc_refract(d, N1, 1.0, nl, v)) return -3;
+        if (!(v[2] < 0.0)) return 0;
+        double s2 = (0.5 * f - P1[2]) / v[2];                   /* plane face z = f/2 */
+        double P2[3] = { P1[0] + s2*v[0], P1[1] + s2*v[1], 0.5 * f };
+        if (P2[0]*P2[0] + P2[1]*P2[1] > Rm*Rm) return 0;        /* leaves through the rim */
+        const double Nz[3] = { 0.0, 0.0, 1.0 };
+        if (!orc_refract(v, Nz, nl, 1.0, v2)) return -3;        /* total internal reflection at the plane face */
+        if (!(v2[2] < 0.0)) return 0;
+        double s3 = (-0.5 * f - P2[2]) / v2[2];                 /* camera plane z = -f/2 */
+        double P3[3] = { P2[0] + s3*v2[0], P2[1] + s3*v2[1], -0.5 * f };
+        if (leg_absorbed(det, P2, P3)) return -2;
+        if (P3[0]*P3[0] + P3[1]*P3[1] > Rc*Rc) return 0;
+        res[0] = P3[0]; res[1] = P3[1]; res[2] = v2[0]; res[3] = v2[1]; res[4] = v2[2];
+        res[5] = s1 + nl * s2 + s3;
+        return 1;
+    }
+    /* parabolic mirror (R15), coordinates relative to the vertex V = centre - (f/2) w */
+    double a = g[0], b = g[1], z0 = g[2] + 0.5 * f;
     /* camera disc from behind */
     double sc = (f - z0) / dw, xs = a + sc * dr, ys = b + sc * du;
     if (xs * xs + ys * ys <= Rc * Rc) return -1;
@@ -816,6 +914,10 @@ int orc_last_mile(const orc_detector *det, const double I[3], const double u[3],
     if (!(r[2] > 0.0)) return 0;
     double s2c = (f - z) / r[2];
     double xc = x + s2c * r[0], yc = y + s2c * r[1];
+    if (det->opt_n_abs > 0) {                                   /* R22: truss between the sphere entry, the mirror and the camera */
+        double M[3] = { x, y, z - 0.5 * f }, K[3] = { xc, yc, 0.5 * f };
+        if (leg_absorbed(det, E, M) || leg_absorbed(det, M, K)) return -2;
+    }
     if (xc * xc + yc * yc > Rc * Rc) return 0;
     res[0] = xc; res[1] = yc; res[2] = r[0]; res[3] = r[1]; res[4] = r[2]; res[5] = sh + s2c;
     return 1;
@@ -1211,7 +1313,7 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                              * third component keeps the record's sign convention) and the camera time */
                             const float *t = det->tel_xyzr + 4*ph.tel;
                             double c[3] = { t[0], t[1], t[2] }, res[6];
-                            if (orc_last_mile(det, Ip, ua, c, res) == 1) {
+                            if (orc_last_mile(det, Ip, ua, c, t[3], res) == 1) {
                                 ph.pix = 0;
                                 lc[ORC_CNT_CAM_HIT]++;
                                 ph.x = res[0]; ph.y = res[1];

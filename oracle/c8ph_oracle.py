@@ -69,7 +69,10 @@ class Detector(C.Structure):
                 ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_double),
                 ("opt_enabled", C.c_int32), ("pad3", C.c_int32),
                 ("opt_az_deg", C.c_double), ("opt_el_deg", C.c_double),
-                ("opt_focal_m", C.c_double), ("opt_mirror_radius_m", C.c_double), ("opt_camera_radius_m", C.c_double)]
+                ("opt_focal_m", C.c_double), ("opt_mirror_radius_m", C.c_double), ("opt_camera_radius_m", C.c_double),
+                ("opt_kind", C.c_int32), ("opt_n_abs", C.c_int32),
+                ("opt_lens_roc_m", C.c_double), ("opt_lens_thickness_m", C.c_double), ("opt_lens_index", C.c_double),
+                ("opt_abs", (C.c_double * 7) * 8)]
 
 
 class Params(C.Structure):
@@ -134,7 +137,11 @@ def lib():
                                               [C.POINTER(C.c_double), C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64,
                                                C.c_int32, C.POINTER(C.c_float)]
             L.orc_last_mile.restype = C.c_int
-            L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 4
+            L.orc_last_mile.argtypes = [C.POINTER(Detector)] + [C.POINTER(C.c_double)] * 3 + [C.c_double, C.POINTER(C.c_double)]
+            L.orc_refract.restype = C.c_int
+            L.orc_refract.argtypes = [C.POINTER(C.c_double)] * 2 + [C.c_double, C.c_double, C.POINTER(C.c_double)]
+            L.orc_segment_distance.restype = C.c_double
+            L.orc_segment_distance.argtypes = [C.POINTER(C.c_double)] * 4
             L.orc_ext_tau_vertical.restype = C.c_double
             L.orc_ext_tau_vertical.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double]
             L.orc_transmission_tabulated.restype = C.c_double
@@ -216,6 +223,16 @@ def detector_struct(det: dict, keep: _Keep) -> Detector:
     s.opt_focal_m = float(np.float32(det.get("opt_focal_m", 1.0)))
     s.opt_mirror_radius_m = float(np.float32(det.get("opt_mirror_radius_m", 0.0)))
     s.opt_camera_radius_m = float(np.float32(det.get("opt_camera_radius_m", 0.0)))
+    s.opt_kind = int(det.get("opt_kind", 0))
+    s.opt_lens_roc_m = float(np.float32(det.get("opt_lens_roc_m", 0.0)))
+    s.opt_lens_thickness_m = float(np.float32(det.get("opt_lens_thickness_m", 0.0)))
+    s.opt_lens_index = float(np.float32(det.get("opt_lens_index", 1.0)))
+    absb = np.asarray(det.get("opt_absorbers", np.zeros((0, 7))), dtype=np.float32).reshape(-1, 7)
+    s.opt_n_abs = len(absb)
+    assert len(absb) <= 8
+    for k, row in enumerate(absb):
+        for j in range(7):
+            s.opt_abs[k][j] = float(row[j])
     return s
 
 

@@ -749,10 +749,10 @@ def _optics_det(az=30.0, el=70.0, f=17.0, rm=8.5, rc=0.735):
     return det
 
 
-def _last_mile(ds, I, u, c):
+def _last_mile(ds, I, u, c, r_sphere=12.0):
     arr = lambda v: (C.c_double * len(v))(*[float(x) for x in v])
     res = (C.c_double * 6)()
-    rc = O.lib().orc_last_mile(C.byref(ds), arr(I), arr(u), arr(c), res)
+    rc = O.lib().orc_last_mile(C.byref(ds), arr(I), arr(u), arr(c), float(r_sphere), res)
     return rc, np.array(res[:])
 
 
@@ -829,6 +829,111 @@ def test_last_mile_parabolic_mirror_and_camera():
         else:
             assert code == 0
     assert checked > 50
+
+
+def test_last_mile_refracting_lens_total_internal_reflection_and_absorbers():
+    """Reading R22 (thesis sec. 6.4: "light bending at a boundary layer (e.g. lens ...)", "absorption by
+    objects"; Fig. 6.6a: total internal reflection).  Pins: vector Snell keeps n sin(angle) and the plane of incidence
+    and fails exactly beyond the critical angle; paraxial rays through the plano-convex lens meet the axis at the
+    thick-lens back focal distance R/(n-1) - t/n behind the plane face; a marginal ray of a fat lens is totally
+    reflected at the plane face exactly where an independent 2-D angle construction says so; the optical path counts
+    n inside the glass; the segment distance against brute force; a strut across the aperture of the MAGIC-like
+    telescope removes the fraction of on-axis light that follows from its two shadows (incoming and reflected beam)."""
+    from scipy.optimize import brentq as optimize_brentq
+    L = O.lib()
+    arr = lambda v: (C.c_double * len(v))(*[float(x) for x in v])
+    rng = np.random.default_rng(11)
+    # --- vector Snell
+    for _ in range(200):
+        N = rng.normal(size=3); N /= np.linalg.norm(N)
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        n1, n2 = rng.uniform(1.0, 1.8, 2)
+        out = (C.c_double * 3)()
+        ok = L.orc_refract(arr(u), arr(N), n1, n2, out)
+        si = math.sqrt(max(0.0, 1 - (u @ N) ** 2))
+        assert bool(ok) == (n1 * si <= n2)                             # total internal reflection beyond the critical angle
+        if ok:
+            v = np.array(out[:])
+            assert abs(np.linalg.norm(v) - 1) < 1e-12
+            assert n2 * math.sqrt(max(0.0, 1 - (v @ N) ** 2)) == pytest.approx(n1 * si, abs=1e-12)
+            assert abs(np.cross(u, N) @ v) < 1e-12 and (v @ N) * (u @ N) > 0           # same plane, same side
+    # --- plano-convex lens, axis vertical (el = 90, az = -90: frame (right, up) = (x, y)): plane face at z = +f/2,
+    #     camera at z = -f/2 about the centre
+    n_l, R_l, t_l = 1.5, 3.0, 0.2
+    bfd = R_l / (n_l - 1.0) - t_l / n_l                                # thick lens, curved side first
+    det = _optics_det(az=-90.0, el=90.0, f=bfd, rm=0.8, rc=0.3)
+    det.update(opt_kind=1, opt_lens_roc_m=R_l, opt_lens_thickness_m=t_l, opt_lens_index=n_l)
+    keep = O._Keep()
+    ds = O.detector_struct(det, keep)
+    c = (0.0, 0.0, 10.0)
+    for x in (1e-3, 5e-3, 0.02):
+        rc, res = _last_mile(ds, (x, 0.0, 30.0), (0, 0, -1.0), c)
+        assert rc == 1 and abs(res[0]) < 2e-3 * x + 40 * x ** 3 and abs(res[1]) < 1e-12   # paraxial focus (spherical aberration ~ x^3)
+        rcf, resf = _last_mile(O.detector_struct(dict(det, opt_focal_m=0.5 * bfd), keep), (x, 0.0, 30.0), (0, 0, -1.0), c)
+        assert rcf == 1 and resf[0] == pytest.approx(0.5 * x, rel=0.05)               # half way to the focus: half the height
+    rc, res = _last_mile(ds, (1e-3, 0.0, 30.0), (0, 0, -1.0), c)
+    sag = R_l - math.sqrt(R_l ** 2 - 1e-6)
+    assert res[5] == pytest.approx((30.0 - (10.0 + 0.5 * bfd + t_l - sag)) + n_l * (t_l - sag) + bfd, abs=1e-6)   # n inside the glass
+    # off-axis beam: the image height of a thin-lens-like system is efl * tan(field angle), efl = R/(n-1)
+    ang = 0.01
+    rc, res = _last_mile(ds, (1e-3 + 20.0 * math.tan(ang), 0.0, 30.0), (-math.sin(ang), 0, -math.cos(ang)), c)
+    assert rc == 1 and res[0] == pytest.approx(-R_l / (n_l - 1.0) * math.tan(ang), rel=2e-2)
+    # --- a fat lens (nearly a hemisphere): marginal rays meet the plane face beyond the critical angle; where that starts
+    #     follows from an independent 2-D construction with angles (entry at polar angle a1, refracted by a1 - a2)
+    n_l, R_l, t_l = 1.5, 1.0, 0.95
+    det = _optics_det(az=-90.0, el=90.0, f=1.0, rm=0.998, rc=0.9)
+    det.update(opt_kind=1, opt_lens_roc_m=R_l, opt_lens_thickness_m=t_l, opt_lens_index=n_l)
+    keep = O._Keep()
+    ds = O.detector_struct(det, keep)
+
+    def tir_2d(x):
+        a1 = math.asin(x / R_l)                                        # angle of incidence on the sphere = polar angle of the point
+        a2 = math.asin(math.sin(a1) / n_l)
+        return n_l * math.sin(a1 - a2) > 1.0                           # angle of the refracted ray against the axis
+    seen = {1: 0, -3: 0}
+    for x in np.concatenate([np.linspace(0.05, 0.98, 32), np.linspace(0.985, 0.9975, 26)]):
+        rc, res = _last_mile(ds, (x, 0.0, 30.0), (0, 0, -1.0), c, r_sphere=3.0)
+        if rc in (1, -3):
+            assert (rc == -3) == tir_2d(x), x
+            seen[rc] += 1
+    assert seen[1] > 20 and seen[-3] > 5
+    x_crit = optimize_brentq(lambda x: n_l * math.sin(math.asin(x) - math.asin(x / n_l)) - 1.0, 0.9, 0.999)
+    assert _last_mile(ds, (x_crit - 1e-6, 0.0, 30.0), (0, 0, -1.0), c, r_sphere=3.0)[0] != -3
+    assert _last_mile(ds, (x_crit + 1e-6, 0.0, 30.0), (0, 0, -1.0), c, r_sphere=3.0)[0] == -3
+    # --- segment distance against brute force
+    for _ in range(100):
+        P0, P1, Q0, Q1 = rng.uniform(-1, 1, (4, 3))
+        d = L.orc_segment_distance(arr(P0), arr(P1), arr(Q0), arr(Q1))
+        s, tt = np.meshgrid(np.linspace(0, 1, 401), np.linspace(0, 1, 401))
+        pts = (P0[None, None] + s[..., None] * (P1 - P0)) - (Q0[None, None] + tt[..., None] * (Q1 - Q0))
+        assert d <= np.linalg.norm(pts, axis=2).min() + 1e-12 and d >= np.linalg.norm(pts, axis=2).min() - 0.01
+    # --- a strut across the aperture of the MAGIC-like telescope (axis vertical), at height z_s above the sphere centre
+    f, rm, rcam, r_s, z_s = 17.0, 8.5, 0.735, 0.05, 4.0
+    det = _optics_det(az=-90.0, el=90.0, f=f, rm=rm, rc=rcam)
+    det.update(opt_absorbers=np.array([[-9.0, 0.0, z_s, 9.0, 0.0, z_s, r_s]], np.float32))
+    keep = O._Keep()
+    ds = O.detector_struct(det, keep)
+    det0 = _optics_det(az=-90.0, el=90.0, f=f, rm=rm, rc=rcam)
+    keep0 = O._Keep()
+    ds0 = O.detector_struct(det0, keep0)
+    n_hit = n_abs = n_all = 0
+    xs = np.linspace(-rm, rm, 341)
+    for x in xs:
+        for y in xs:
+            if x * x + y * y > rm * rm:
+                continue
+            rc0, _ = _last_mile(ds0, (x, y, 40.0), (0, 0, -1.0), c, r_sphere=12.0)
+            rc1, _ = _last_mile(ds, (x, y, 40.0), (0, 0, -1.0), c, r_sphere=12.0)
+            if rc0 == 1:
+                n_all += 1
+                n_abs += rc1 == -2
+                n_hit += rc1 == 1
+                # the strut runs along x at y = 0: the incoming ray is blocked if |y| <= r_s; the reflected ray from the mirror
+                # point (rho, rho^2/4f) to the focus passes the height of the strut at y (f - z_v)/(f - rho^2/4f)
+                z_v = z_s + 0.5 * f                                  # height above the vertex
+                blocked = abs(y) <= r_s or abs(y * (f - z_v) / (f - (x * x + y * y) / (4 * f))) <= r_s
+                assert (rc1 == -2) == blocked or abs(abs(y) - r_s) < 1e-9, (x, y, rc1)
+    assert n_all > 5e4 and n_hit + n_abs == n_all and 0.005 < n_abs / n_all < 0.03
 
 
 def test_last_mile_in_the_run():
