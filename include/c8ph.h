@@ -124,6 +124,19 @@ typedef struct {
      * contain mirror and camera.  Excludes cam_enabled and WRITE_ALL.                               */
     int32_t opt_enabled;
     float opt_az_deg, opt_el_deg, opt_focal_m, opt_mirror_radius_m, opt_camera_radius_m;
+    /* More of thesis sec. 6.4 (R22).  "Light bending at a boundary layer (e.g. lens ...)":
+     * opt_kind = 1 replaces the mirror by a plano-convex lens - plane face (aperture radius opt_mirror_radius_m) at
+     * centre + (f/2) w, convex spherical face (radius of curvature opt_lens_roc_m, apex opt_lens_thickness_m above
+     * the plane face) towards the sky, index opt_lens_index, camera disc at centre - (f/2) w facing the lens; vector
+     * Snell (Eq. 3.15) at both faces, a ray that is totally reflected inside the glass (Fig. 6.6a) is lost; the
+     * record's time counts the index inside the glass, its direction (ux, uy along right, up) belongs to a ray that
+     * travels towards -w.  "Absorption by objects": opt_n_abs <= 8 opaque capsules
+     * (axis end points and radius, telescope frame (right, up, axis) about the sphere centre, e.g. the truss): a ray
+     * whose leg sphere entry -> mirror / lens or mirror / lens -> camera comes within the radius is absorbed.       */
+    int32_t opt_kind;                /* 0: parabolic mirror, 1: plano-convex lens                     */
+    float opt_lens_roc_m, opt_lens_thickness_m, opt_lens_index;
+    int32_t opt_n_abs;
+    float opt_abs[8][7];             /* x0, y0, z0, x1, y1, z1, r                                      */
 } c8ph_detector;
 /* Copies the telescope list and builds the two uniform-grid accelerators on the host (per cell: the
  * candidate telescopes sorted by a lower-bound key, the smallest key, the nearest / first telescope in

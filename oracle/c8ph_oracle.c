@@ -1317,7 +1317,8 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                                 ph.pix = 0;
                                 lc[ORC_CNT_CAM_HIT]++;
                                 ph.x = res[0]; ph.y = res[1];
-                                ph.ux = res[2]; ph.uy = res[3]; ph.uz = -res[4];
+                                ph.ux = res[2]; ph.uy = res[3];
+                                ph.uz = det->opt_kind == 1 ? res[4] : -res[4];    /* mirror: towards +w; lens: towards -w */
                                 ph.t += res[5] / ORC_C_M_PER_NS;
                             }
                         }

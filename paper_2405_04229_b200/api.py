@@ -68,7 +68,9 @@ class Detector(C.Structure):
                 ("cam_rows", C.c_int32), ("cam_cols", C.c_int32), ("n_tbins", C.c_int32),
                 ("t_ref_ns", C.c_double), ("t_bin_ns", C.c_float),
                 ("opt_enabled", C.c_int32), ("opt_az_deg", C.c_float), ("opt_el_deg", C.c_float),
-                ("opt_focal_m", C.c_float), ("opt_mirror_radius_m", C.c_float), ("opt_camera_radius_m", C.c_float)]
+                ("opt_focal_m", C.c_float), ("opt_mirror_radius_m", C.c_float), ("opt_camera_radius_m", C.c_float),
+                ("opt_kind", C.c_int32), ("opt_lens_roc_m", C.c_float), ("opt_lens_thickness_m", C.c_float),
+                ("opt_lens_index", C.c_float), ("opt_n_abs", C.c_int32), ("opt_abs", (C.c_float * 7) * 8)]
 
 
 class Params(C.Structure):
@@ -258,6 +260,14 @@ class Context:
         d.opt_az_deg, d.opt_el_deg = float(det.get("opt_az_deg", 0.0)), float(det.get("opt_el_deg", 90.0))
         d.opt_focal_m = float(det.get("opt_focal_m", 1.0))
         d.opt_mirror_radius_m, d.opt_camera_radius_m = float(det.get("opt_mirror_radius_m", 0.0)), float(det.get("opt_camera_radius_m", 0.0))
+        d.opt_kind = int(det.get("opt_kind", 0))
+        d.opt_lens_roc_m, d.opt_lens_thickness_m = float(det.get("opt_lens_roc_m", 0.0)), float(det.get("opt_lens_thickness_m", 0.0))
+        d.opt_lens_index = float(det.get("opt_lens_index", 1.0))
+        absb = _f32(det.get("opt_absorbers", np.zeros((0, 7), np.float32))).reshape(-1, 7)
+        d.opt_n_abs = len(absb)
+        for k, row in enumerate(absb[:8]):
+            for j in range(7):
+                d.opt_abs[k][j] = float(row[j])
         self._check(self.lib.c8ph_set_detector(self._h, C.byref(d)))
         self._det = dict(det)
         self._n_tel = tel.shape[0]

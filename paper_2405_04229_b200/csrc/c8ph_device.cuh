@@ -89,6 +89,9 @@ struct DevDet {
     int opt_enabled;                      // last-mile optics inside the bounding spheres
     float opt_w[3], opt_r[3], opt_u[3];   // telescope frame: pointing axis, right, up
     float opt_f, opt_rm2, opt_rc2;        // focal length, mirror radius^2, camera radius^2
+    int opt_kind, opt_n_abs;              // R22: 1 = plano-convex lens instead of the mirror; absorbing capsules
+    float opt_lens_roc, opt_lens_t, opt_lens_n;
+    float opt_abs[8][7];                  // capsule axis end points and radius, telescope frame about the sphere centre
 };
 
 struct DevRun {

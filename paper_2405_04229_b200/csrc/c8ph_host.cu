@@ -553,8 +553,20 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
     if (d->opt_enabled) {
         if (d->cam_enabled || d->n_tel < 1 || !(d->opt_focal_m > 0.f) || !(d->opt_mirror_radius_m > 0.f) || !(d->opt_camera_radius_m > 0.f))
             return fail(ctx, C8PH_E_ARG, "set_detector: optics need telescopes, focal length, mirror and camera radius; not with cam_enabled");
+        if (d->opt_kind < 0 || d->opt_kind > 1 || d->opt_n_abs < 0 || d->opt_n_abs > 8)
+            return fail(ctx, C8PH_E_ARG, "set_detector: opt_kind must be 0 or 1 and opt_n_abs in [0, 8]");
+        for (int k = 0; k < d->opt_n_abs; ++k) {
+            for (int j = 0; j < 7; ++j) if (!std::isfinite(d->opt_abs[k][j])) return fail(ctx, C8PH_E_ARG, "set_detector: absorber not finite");
+            if (!(d->opt_abs[k][6] > 0.f)) return fail(ctx, C8PH_E_ARG, "set_detector: absorber radius <= 0");
+        }
+        if (d->opt_kind == 1) {
+            const double Rl = d->opt_lens_roc_m, t = d->opt_lens_thickness_m, nl = d->opt_lens_index, rmv = d->opt_mirror_radius_m;
+            if (!(Rl > 0.0) || !(t > 0.0) || !(t <= Rl) || !(nl > 1.0) || !(rmv * rmv <= Rl * Rl - (Rl - t) * (Rl - t) + 1e-9))
+                return fail(ctx, C8PH_E_ARG, "set_detector: lens needs roc > 0, 0 < thickness <= roc, index > 1 and an aperture inside the cap");
+        }
         const double f = d->opt_focal_m, rm = d->opt_mirror_radius_m, rc = d->opt_camera_radius_m;
-        const double need = std::max(std::sqrt(0.25 * f * f + rc * rc), std::sqrt(std::pow(0.5 * f - rm * rm / (4.0 * f), 2) + rm * rm));
+        // lens: apex on the axis, rim of the plane face and rim of the camera must be inside the sphere
+        const double need = d->opt_kind == 1 ? std::max(0.5 * f + (double)d->opt_lens_thickness_m, std::max(std::sqrt(0.25 * f * f + rm * rm), std::sqrt(0.25 * f * f + rc * rc))) : std::max(std::sqrt(0.25 * f * f + rc * rc), std::sqrt(std::pow(0.5 * f - rm * rm / (4.0 * f), 2) + rm * rm));
         for (int k = 0; k < d->n_tel; ++k)
             if (d->tel_xyzr[4 * k + 3] < need) return fail(ctx, C8PH_E_ARG, "set_detector: a bounding sphere does not contain the mirror and the camera");
     }
@@ -598,6 +610,9 @@ extern "C" int c8ph_set_detector(c8ph_ctx *ctx, const c8ph_detector *d)
         for (int k = 0; k < 3; ++k) { o.opt_w[k] = (float)w[k]; o.opt_r[k] = (float)r[k]; o.opt_u[k] = (float)u[k]; }
         o.opt_f = d->opt_focal_m; o.opt_rm2 = d->opt_mirror_radius_m * d->opt_mirror_radius_m;
         o.opt_rc2 = d->opt_camera_radius_m * d->opt_camera_radius_m;
+        o.opt_kind = d->opt_kind; o.opt_n_abs = d->opt_enabled ? d->opt_n_abs : 0;
+        o.opt_lens_roc = d->opt_lens_roc_m; o.opt_lens_t = d->opt_lens_thickness_m; o.opt_lens_n = d->opt_lens_index;
+        for (int k = 0; k < 8; ++k) for (int j = 0; j < 7; ++j) o.opt_abs[k][j] = k < o.opt_n_abs ? d->opt_abs[k][j] : 0.f;
     }
     o.t_ref = d->t_ref_ns; o.t_bin = d->t_bin_ns; o.inv_t_bin = d->t_bin_ns > 0.f ? 1.0f / d->t_bin_ns : 0.f;
     dfree(ctx->d_tel);

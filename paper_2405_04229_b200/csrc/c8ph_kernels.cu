@@ -486,6 +486,52 @@ __device__ __forceinline__ bool tel_near_search(const DevDet &det, int cell, flo
     return found;
 }
 
+// ---- R22 (thesis sec. 6.4): refraction at a boundary (vector Snell, Eq. 3.15) and absorbing capsules ----------------
+// u -> out across a surface with unit normal N from index n1 into n2; false: total internal reflection
+__device__ __forceinline__ bool refract_vec(float ux, float uy, float uz, float Nx, float Ny, float Nz, float n1, float n2,
+                                            float &ox, float &oy, float &oz)
+{
+    const float c = ux * Nx + uy * Ny + uz * Nz;
+    const float sgn = c < 0.f ? -1.f : 1.f, ca = fabsf(c);
+    const float q = fmaf(n2, n2, fmaf(n1 * n1, ca * ca, -n1 * n1));
+    if (q < 0.f) return false;
+    const float k = (sqrtf(q) - n1 * ca) * sgn, in2 = 1.f / n2;
+    ox = fmaf(k, Nx, n1 * ux) * in2; oy = fmaf(k, Ny, n1 * uy) * in2; oz = fmaf(k, Nz, n1 * uz) * in2;
+    return true;
+}
+
+// squared distance between the segments P0 -> P1 and Q0 -> Q1
+__device__ float segment_dist2(const float3 P0, const float3 P1, const float3 Q0, const float3 Q1)
+{
+    const float3 d1 = make_float3(P1.x - P0.x, P1.y - P0.y, P1.z - P0.z), d2 = make_float3(Q1.x - Q0.x, Q1.y - Q0.y, Q1.z - Q0.z);
+    const float3 r = make_float3(P0.x - Q0.x, P0.y - Q0.y, P0.z - Q0.z);
+    const float a = d1.x * d1.x + d1.y * d1.y + d1.z * d1.z, e = d2.x * d2.x + d2.y * d2.y + d2.z * d2.z;
+    const float f = d2.x * r.x + d2.y * r.y + d2.z * r.z, c = d1.x * r.x + d1.y * r.y + d1.z * r.z;
+    const float b = d1.x * d2.x + d1.y * d2.y + d1.z * d2.z;
+    float sN = 0.f, tN = 0.f;
+    if (a <= 1e-30f && e <= 1e-30f) { }
+    else if (a <= 1e-30f) tN = fminf(fmaxf(f / e, 0.f), 1.f);
+    else if (e <= 1e-30f) sN = fminf(fmaxf(-c / a, 0.f), 1.f);
+    else {
+        const float den = a * e - b * b;
+        sN = den > 1e-12f * a * e ? fminf(fmaxf((b * f - c * e) / den, 0.f), 1.f) : 0.f;
+        tN = (b * sN + f) / e;
+        if (tN < 0.f) { tN = 0.f; sN = fminf(fmaxf(-c / a, 0.f), 1.f); }
+        else if (tN > 1.f) { tN = 1.f; sN = fminf(fmaxf((b - c) / a, 0.f), 1.f); }
+    }
+    const float dx = r.x + sN * d1.x - tN * d2.x, dy = r.y + sN * d1.y - tN * d2.y, dz = r.z + sN * d1.z - tN * d2.z;
+    return dx * dx + dy * dy + dz * dz;
+}
+
+__device__ bool leg_absorbed(const DevDet &det, const float3 A, const float3 B)
+{
+    for (int k = 0; k < det.opt_n_abs; ++k) {
+        const float *o = det.opt_abs[k];
+        if (segment_dist2(A, B, make_float3(o[0], o[1], o[2]), make_float3(o[3], o[4], o[5])) <= o[6] * o[6]) return true;
+    }
+    return false;
+}
+
 // hexagonal camera pixel of an arrival direction (cfg3); -1 outside.  Nearest centre among the
 // rows/columns adjacent to the point (equivalent to the brute-force nearest centre).
 __device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float uy, float uz)
@@ -721,6 +767,41 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float dr = uax * det.opt_r[0] + uay * det.opt_r[1] + uaz * det.opt_r[2];
                     const float du = uax * det.opt_u[0] + uay * det.opt_u[1] + uaz * det.opt_u[2];
                     const float dw = uax * det.opt_w[0] + uay * det.opt_w[1] + uaz * det.opt_w[2];
+                    // R22: start of the incoming leg = entry into the bounding sphere (frame about the sphere centre)
+                    const float3 g0 = make_float3(a0, b0, z0 - hf);
+                    float3 Een = g0;
+                    if (det.opt_n_abs > 0 || det.opt_kind == 1) {
+                        const float bq = g0.x * dr + g0.y * du + g0.z * dw, cq = g0.x * g0.x + g0.y * g0.y + g0.z * g0.z - tc.w * tc.w;
+                        const float s_in = -bq - sqrtf(fmaxf(bq * bq - cq, 0.f));
+                        Een = make_float3(fmaf(s_in, dr, g0.x), fmaf(s_in, du, g0.y), fmaf(s_in, dw, g0.z));
+                    }
+                    if (det.opt_kind == 1) {
+                        // plano-convex lens (R22): convex face towards the sky, plane face at +f/2, camera at -f/2 (about the centre)
+                        const float Rl = det.opt_lens_roc, nl = det.opt_lens_n, zc = hf + det.opt_lens_t - Rl;
+                        const float ocz = g0.z - zc;
+                        const float b2 = g0.x * dr + g0.y * du + ocz * dw, c2 = g0.x * g0.x + g0.y * g0.y + ocz * ocz - Rl * Rl;
+                        const float disc = b2 * b2 - c2;
+                        if (dw < 0.f && disc >= 0.f) {
+                            const float s1 = -b2 - sqrtf(disc);
+                            const float3 P1 = make_float3(fmaf(s1, dr, g0.x), fmaf(s1, du, g0.y), fmaf(s1, dw, g0.z));
+                            float vx, vy, vz, v2x, v2y, v2z;
+                            if (P1.x * P1.x + P1.y * P1.y <= det.opt_rm2 && P1.z >= hf && !leg_absorbed(det, Een, P1) &&
+                                refract_vec(dr, du, dw, P1.x / Rl, P1.y / Rl, (P1.z - zc) / Rl, 1.f, nl, vx, vy, vz) && vz < 0.f) {
+                                const float s2 = (hf - P1.z) / vz;
+                                const float3 P2 = make_float3(fmaf(s2, vx, P1.x), fmaf(s2, vy, P1.y), hf);
+                                if (P2.x * P2.x + P2.y * P2.y <= det.opt_rm2 && refract_vec(vx, vy, vz, 0.f, 0.f, 1.f, nl, 1.f, v2x, v2y, v2z) && v2z < 0.f) {
+                                    const float s3 = (-hf - P2.z) / v2z;
+                                    const float3 P3 = make_float3(fmaf(s3, v2x, P2.x), fmaf(s3, v2y, P2.y), -hf);
+                                    if (!leg_absorbed(det, P2, P3) && P3.x * P3.x + P3.y * P3.y <= det.opt_rc2) {
+                                        opt_hit = true;
+                                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                                        rx_out = P3.x; ry_out = P3.y; uax = v2x; uay = v2y;
+                                        t_arr = fmaf(s1 + nl * s2 + s3, kInvC, t_arr);
+                                    }
+                                }
+                            }
+                        }
+                    } else
                     if (dw < 0.f) {
                         const float sc0 = (f - z0) * rcp_fast(dw);
                         const float xs = fmaf(sc0, dr, a0), ys = fmaf(sc0, du, b0);
@@ -749,7 +830,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                                 if (r2 > 0.f) {
                                     const float s2c = (f - z) * rcp_fast(r2);
                                     const float xc = fmaf(s2c, r0, x), yc = fmaf(s2c, r1, y);
-                                    if (xc * xc + yc * yc <= det.opt_rc2) {
+                                    bool absorbed = false;                            // R22: truss shadowing on both legs
+                                    if (det.opt_n_abs > 0) {
+                                        const float3 Mp = make_float3(x, y, z - hf), Kp = make_float3(xc, yc, hf);
+                                        absorbed = leg_absorbed(det, Een, Mp) || leg_absorbed(det, Mp, Kp);
+                                    }
+                                    if (!absorbed && xc * xc + yc * yc <= det.opt_rc2) {
                                         opt_hit = true;
                                         atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
                                         rx_out = xc; ry_out = yc; uax = r0; uay = r1;

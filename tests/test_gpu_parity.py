@@ -574,6 +574,53 @@ def test_last_mile_optics():
     assert e.value.code == api.E_ARG
 
 
+def test_last_mile_truss_shadowing_and_refracting_lens():
+    """Row f3, the rest of thesis sec. 6.4 (R22): absorbing objects (a four-mast truss and a
+    cross strut on the MAGIC-like telescope) and light bending at a boundary layer (a plano-convex lens telescope with
+    the camera in its back focal plane; rays that are totally reflected inside the glass are lost).  Device against
+    oracle photon by photon; the truss removes light, the lens images the shower onto its camera."""
+    # --- truss on the mirror telescope of test_last_mile_optics
+    cfg = W.make_config(4, n_segments=4000)
+    cfg["detector"]["tel_xyzr"][:, 3] = 12.0
+    cfg["detector"].update(opt_enabled=True, opt_az_deg=0.0, opt_el_deg=70.0, opt_focal_m=17.0,
+                           opt_mirror_radius_m=8.5, opt_camera_radius_m=0.735)
+    clear = api.run_config(cfg)
+    masts = [[6.0 * np.cos(a), 6.0 * np.sin(a), -8.5 + 36.0 / 68.0, 0.6 * np.cos(a), 0.6 * np.sin(a), 8.5, 0.08]
+             for a in np.radians([45.0, 135.0, 225.0, 315.0])]               # mirror surface (rho = 6 m) to the camera rim
+    masts.append([-8.0, 0.0, 2.0, 8.0, 0.0, 2.0, 0.05])                      # a cross strut
+    cfg["detector"]["opt_absorbers"] = np.array(masts, np.float32)
+    ora, gpu, rep = _both(cfg)
+    c = gpu["counters"]
+    assert c["tel_hit"] == clear["counters"]["tel_hit"]
+    assert 0.85 * clear["counters"]["cam_hit"] < c["cam_hit"] < 0.99 * clear["counters"]["cam_hit"]     # a few per cent shadowed
+    assert rep["max_dpos_m"] < 2e-3
+    # --- lens telescope: R = 12 m, n = 1.5, thickness 1.2 m, aperture 5 m, camera in the back focal plane
+    R_l, n_l, t_l = 12.0, 1.5, 1.2
+    bfd = R_l / (n_l - 1.0) - t_l / n_l
+    cfg = W.make_config(4, n_segments=4000)
+    cfg["detector"]["tel_xyzr"][:, 3] = 14.0
+    cfg["detector"].update(opt_enabled=True, opt_az_deg=0.0, opt_el_deg=70.0, opt_focal_m=bfd, opt_mirror_radius_m=5.0,
+                           opt_camera_radius_m=1.5, opt_kind=1, opt_lens_roc_m=R_l, opt_lens_thickness_m=t_l, opt_lens_index=n_l,
+                           opt_absorbers=np.array([[-5.0, 0.0, -3.0, 5.0, 0.0, -3.0, 0.05]], np.float32))
+    ora, gpu, rep = _both(cfg)
+    c = gpu["counters"]
+    assert 200 < c["cam_hit"] == c["written"] < c["tel_hit"]
+    ph = gpu["photons"]
+    assert np.all(np.hypot(ph["x"], ph["y"]) <= 1.5 * (1 + 1e-5)) and rep["max_dpos_m"] < 2e-3
+    # the image of the 20-degree-inclined light sits f tan(20 deg) ~ 8 m off axis for an axis at 70 deg elevation: outside this
+    # camera; what arrives comes from the halo - pointing the lens at the shower (el 90 - 20) is what the config does, so most hits
+    # are within the camera; a lens that is not in focus smears them
+    blur = copy.deepcopy(cfg)
+    blur["detector"]["opt_focal_m"] = 0.6 * bfd
+    res = api.run_config(blur)
+    assert res["counters"]["cam_hit"] != c["cam_hit"]
+    bad = copy.deepcopy(cfg)
+    bad["detector"]["opt_lens_thickness_m"] = 13.0                           # thicker than the radius of curvature
+    with pytest.raises(api.C8phError) as e:
+        api.setup_context(bad)
+    assert e.value.code == api.E_ARG
+
+
 def test_substepping_matches_the_oracle_and_feeds_the_hot_path():
     """Row f2 (thesis sec. 4.2.1): tracks cut into chords of the Lorentz helix on the device (plan =
     count + prefix sum, fill = a warp per 32 tracks) against the oracle: piece counts bit-exact,
