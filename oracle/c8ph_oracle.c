@@ -214,7 +214,7 @@ double orc_overburden(const orc_atmosphere *atm, double h)
  * spherical h = |A - C| - R with C = (0,0,-(R+h_obs))). */
 double orc_height(const orc_atmosphere *atm, const double A[3])
 {
-    if (atm->model != 2) return atm->h_obs + A[2];
+    if (atm->model < 2) return atm->h_obs + A[2];        /* cylindrical (3): every point lies in its own plane of curvature */
     double Rg = atm->earth_radius + atm->h_obs;
     double zz = A[2] + Rg;
     return sqrt(A[0] * A[0] + A[1] * A[1] + zz * zz) - atm->earth_radius;
@@ -403,6 +403,133 @@ int orc_trace(const orc_atmosphere *atm, int spherical, double h_e, double sin_z
  * sphere at the origin and lies above it elsewhere.  Line from the emission point Ae along u to the sphere, arc dd
  * along the direction of flight on the sphere, then back along the arrival direction (straight, at the ground index)
  * to z = 0.  Returns 1 if the straight line misses the sphere.  t_rel = arrival time - emission time [ns]. */
+/* ------------------------------------------------------------------ A5 cylindrical atmosphere model (reading R24)
+ * Thesis sec. 3.3.3: besides the height "the horizontal distance d from the coordinate systems origin ... to
+ * the emission point, with d^2 = x^2 + y^2, is added.  Afterwards, the refractive index gradient only changes in its
+ * Zenith angle theta where the rotation angle phi is kept constant" - the spherical model "requires an additional change
+ * of the refractive index gradient rotation angle in every step".  Reading: per photon the rotation angle phi of the
+ * gradient is frozen at the azimuth of its emission point about the origin's vertical; the gradient stays in the vertical
+ * plane of that azimuth and its zenith angle follows the position along it: the atmosphere is a set of coaxial CYLINDERS
+ * whose axis passes through the Earth's centre, horizontal and perpendicular to that plane.  At the emission point
+ * height and local vertical are those of the spherical model; along the path the curvature across the plane is missing.
+ * Numerical tracing = the layered construction of orc_trace (Eq. 3.15, layers = table cells split in `sub`, n at the
+ * layer mid height) in three dimensions with N = the in-plane radial direction at the crossing point.
+ * Frame: x' along the frozen azimuth, y' along the cylinder axis, z' from the axis through the emission point (x' = 0).
+ * in : h_e, local zenith (sin_z, cos_z > 0), psi = azimuth of the horizontal direction of flight against x', h_g
+ * out: [0] central angle about the axis (x' arc / (R + h_g))  [1] S  [2] c T  [3] X_slant  [4] tau_aer  [5] y' displacement
+ *      [6..8] arrival direction (x', y', z')
+ * returns 0, or 1 if the ray never reaches h_g. */
+int orc_trace_cyl(const orc_atmosphere *atm, double h_e, double sin_z, double cos_z, double psi, double h_g, int sub, double out[9])
+{
+    for (int k = 0; k < 9; ++k) out[k] = 0.0;
+    if (sub < 1) sub = 1;
+    const double R = atm->earth_radius;
+    double p[3] = { 0.0, 0.0, R + h_e };
+    double n_prev = 1.0 + orc_refractivity(atm, h_e);
+    double A[3] = { n_prev * sin_z * cos(psi), n_prev * sin_z * sin(psi), -n_prev * cos_z };   /* A' = n * direction */
+    double h_cur = h_e, S = 0, cT = 0, X = 0, tau = 0;
+    const double step = atm->dh / sub;
+    while (h_cur > h_g) {
+        double g = floor((h_cur - atm->h0) / step);
+        double h_next = atm->h0 + g * step;
+        if (!(h_next < h_cur - 1e-9 * step)) h_next = atm->h0 + (g - 1.0) * step;
+        if (h_next < h_g) h_next = h_g;
+        double n_l = 1.0 + orc_refractivity(atm, 0.5 * (h_cur + h_next));
+        double r = sqrt(p[0]*p[0] + p[2]*p[2]);
+        double N[3] = { -p[0] / r, 0.0, -p[2] / r };             /* gradient: in the plane of curvature only */
+        double n1cos = A[0]*N[0] + A[2]*N[2];
+        double rad = n_l*n_l - n_prev*n_prev + n1cos*n1cos;
+        if (!(rad > 0.0) || !(n1cos > 0.0)) return 1;
+        double c = sqrt(rad) - n1cos;
+        A[0] += c * N[0]; A[2] += c * N[2];                      /* Eq. 3.15; the component along the axis is untouched */
+        double d[3] = { A[0] / n_l, A[1] / n_l, A[2] / n_l };
+        /* |(p_x + s d_x, p_z + s d_z)| = R + h_next, nearest root */
+        double rt = R + h_next;
+        double a2 = d[0]*d[0] + d[2]*d[2];
+        double b = p[0]*d[0] + p[2]*d[2];
+        double cc = p[0]*p[0] + p[2]*p[2] - rt*rt;
+        double disc = b*b - a2*cc;
+        if (!(disc >= 0.0) || !(b < 0.0)) return 1;
+        double s = cc / (-b + sqrt(disc));
+        double dhl = h_cur - h_next;
+        S += s; cT += n_l * s;
+        X += (orc_overburden(atm, h_next) - orc_overburden(atm, h_cur)) * (s / dhl);
+        if (atm->aer_L > 0.0)
+            tau += (atm->aer_H / atm->aer_L) * (exp(-h_next / atm->aer_H) - exp(-h_cur / atm->aer_H)) * (s / dhl);
+        for (int k = 0; k < 3; ++k) p[k] += s * d[k];
+        n_prev = n_l; h_cur = h_next;
+    }
+    {   /* into the medium at the target height */
+        double n_g = 1.0 + orc_refractivity(atm, h_g);
+        double r = sqrt(p[0]*p[0] + p[2]*p[2]);
+        double N[3] = { -p[0] / r, 0.0, -p[2] / r };
+        double n1cos = A[0]*N[0] + A[2]*N[2];
+        double rad = n_g*n_g - n_prev*n_prev + n1cos*n1cos;
+        if (!(rad > 0.0)) return 1;
+        double c = sqrt(rad) - n1cos;
+        A[0] += c * N[0]; A[2] += c * N[2];
+        out[6] = A[0] / n_g; out[7] = A[1] / n_g; out[8] = A[2] / n_g;
+    }
+    out[0] = atan2(p[0], p[2]); out[1] = S; out[2] = cT; out[3] = X; out[4] = tau; out[5] = p[1];
+    return 0;
+}
+
+/* the cylindrical ray against the straight line to the same cylinder surface r' = R + h_g: corr[0] displacement along the
+ * horizontal direction of flight e_h, corr[1] across it (along e_h turned by +90 deg), corr[2] time [ns], corr[3] X_slant,
+ * corr[4] tau_aer.  (The sag of that surface under the plane z = 0 is ignored as in the spherical model, R9 (i).) */
+int orc_cyl_correction(const orc_atmosphere *atm, double h_e, double sin_z, double cos_z, double psi, int sub, double corr[5])
+{
+    double r[9];
+    if (orc_trace_cyl(atm, h_e, sin_z, cos_z, psi, atm->h_obs, sub, r)) return 1;
+    const double Rg = atm->earth_radius + atm->h_obs, re = atm->earth_radius + h_e;
+    const double ux = sin_z * cos(psi), uy = sin_z * sin(psi), uz = -cos_z;
+    /* straight line: in the plane of curvature a chord from radius re to radius Rg */
+    const double up = sqrt(ux*ux + uz*uz);                      /* in-plane part of the unit direction */
+    const double sp = ux / up, cp = -uz / up;                   /* in-plane zenith angle */
+    const double pp = re * sp;
+    if (!(fabs(pp) < Rg)) return 1;
+    const double chord = re * cp - sqrt(Rg*Rg - pp*pp);         /* in-plane length */
+    const double S_line = chord / up;
+    const double psi_line = asin(pp / Rg) - atan2(sp, cp);      /* central angle of the straight line */
+    const double dxp = Rg * (r[0] - psi_line), dyp = r[5] - uy * S_line;
+    corr[0] = dxp * cos(psi) + dyp * sin(psi);
+    corr[1] = -dxp * sin(psi) + dyp * cos(psi);
+    corr[2] = (r[2] - S_line) / ORC_C_M_PER_NS;
+    corr[3] = r[3]; corr[4] = r[4];
+    return 0;
+}
+
+/* Interpolation tracing in the cylindrical model: the table of P:861 with its third axis.  By the symmetry of the
+ * cylinders the distance d drops out once the observation surface is the cylinder r' = R + h_obs, and what remains
+ * besides (height, zenith) is the azimuth psi of the flight against the plane of curvature: axis uniform in
+ * c = cos^2(psi) (the curvature the ray sees along its ground track is c / R, Euler's theorem), n_c >= 2 nodes.
+ * Channels: ch0 dd along e_h, ch1 the across displacement divided by sin(psi) cos(psi) (smooth in c; evaluated 1e-3 rad
+ * inside the ends), ch2 dt [ns], ch3 X_slant, ch4 tau_aer.  Layout [n_c][n_h][n_zen][5]; c = 0 is the planar model's
+ * table, c = 1 the spherical one. */
+void orc_build_table_cyl(const orc_atmosphere *atm, int n_h, int n_zen, int n_c, double h_max, double zen_max_rad,
+                         int sub, float *out)
+{
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int a = 0; a < n_h; ++a) {
+        double h = a * h_max / (n_h - 1);
+        for (int b = 0; b < n_zen; ++b) {
+            double th = b * zen_max_rad / (n_zen - 1);
+            for (int k = 0; k < n_c; ++k) {
+                float *o = out + (((size_t)k * n_h + a) * n_zen + b) * 5;
+                if (h <= atm->h_obs) { for (int q = 0; q < 5; ++q) o[q] = 0.0f; continue; }
+                double c = (double)k / (n_c - 1);
+                double psi = acos(sqrt(c));
+                psi = fmin(fmax(psi, 1e-3), 0.5 * ORC_PI - 1e-3);
+                double corr[5];
+                if (orc_cyl_correction(atm, h, sin(th), cos(th), psi, sub, corr)) { for (int q = 0; q < 5; ++q) o[q] = NAN; continue; }
+                o[0] = (float)corr[0];
+                o[1] = (float)(corr[1] / (sin(psi) * cos(psi)));
+                o[2] = (float)corr[2]; o[3] = (float)corr[3]; o[4] = (float)corr[4];
+            }
+        }
+    }
+}
+
 static void norm3(double v[3]);
 static int flat_plane_step(const orc_atmosphere *atm, const double Ae[3], const double u[3], double h_e,
                            double sin_zen, double cos_zen, double dd, double dt_ns, const double ua[3],
@@ -585,6 +712,34 @@ int orc_table_flat_lookup(const orc_table *t, double h, double zen, double rho, 
         if (k >= 3) { out[k] = part[0]; if (k == 3 && perp) *perp = part[1]; }   /* X_slant, tau_aer: even part only */
         else out[k] = part[0] + cos_chi * part[1];
         if (isnan(out[k]) || isnan(part[1])) bad = 1;
+    }
+    return bad;
+}
+
+/* trilinear lookup in the cylindrical model's table [n_c][n_h][n_zen][5] (data3, n_rho = n_c, third axis c = cos^2(psi)
+ * in [0, 1]); indices clamped as in orc_table_lookup */
+int orc_table_cyl_lookup(const orc_table *t, double h, double zen, double c, double out[5])
+{
+    if (!t->data3 || t->n_rho < 2) return 1;
+    if (!(h >= 0.0) || h > t->h_max || !(zen >= 0.0) || zen > t->zen_max_rad || !(c >= 0.0) || !(c <= 1.0)) return 1;
+    double f = h / (t->h_max / (t->n_h - 1)), g = zen / (t->zen_max_rad / (t->n_zen - 1)), e = c * (t->n_rho - 1);
+    int a = (int)floor(f), b = (int)floor(g), k = (int)floor(e);
+    if (a > t->n_h - 2) a = t->n_h - 2;
+    if (b > t->n_zen - 2) b = t->n_zen - 2;
+    if (k > t->n_rho - 2) k = t->n_rho - 2;
+    double ff = f - a, gg = g - b, ee = e - k;
+    int bad = 0;
+    const size_t s = (size_t)t->n_ch, plane = (size_t)t->n_h * t->n_zen * s;
+    for (int ch = 0; ch < 5; ++ch) {
+        double v[2];
+        for (int q = 0; q < 2; ++q) {
+            const float *d = t->data3 + (size_t)(k + q) * plane;
+            double v00 = d[((size_t)a * t->n_zen + b) * s + ch], v01 = d[((size_t)a * t->n_zen + b + 1) * s + ch];
+            double v10 = d[((size_t)(a + 1) * t->n_zen + b) * s + ch], v11 = d[((size_t)(a + 1) * t->n_zen + b + 1) * s + ch];
+            v[q] = (1 - ff) * ((1 - gg) * v00 + gg * v01) + ff * ((1 - gg) * v10 + gg * v11);
+        }
+        out[ch] = (1 - ee) * v[0] + ee * v[1];
+        if (isnan(out[ch])) bad = 1;
     }
     return bad;
 }
@@ -1019,8 +1174,8 @@ static void prepare_segment(const orc_atmosphere *atm, const orc_detector *det, 
         if (tab && par->trace == ORC_TRACE_TABLE) {
             double dir[3] = { d[0]/dist, d[1]/dist, d[2]/dist };
             double Rg = atm->earth_radius + atm->h_obs;
-            double rv[3] = { mid[0], mid[1], mid[2] + (atm->model == 2 ? Rg : 0.0) };
-            if (atm->model != 2) { rv[0] = 0; rv[1] = 0; rv[2] = 1; }
+            double rv[3] = { mid[0], mid[1], mid[2] + (atm->model >= 2 ? Rg : 0.0) };
+            if (atm->model < 2) { rv[0] = 0; rv[1] = 0; rv[2] = 1; }
             norm3(rv);
             double cz = -(dir[0]*rv[0] + dir[1]*rv[1] + dir[2]*rv[2]);
             double corr[5];
@@ -1181,18 +1336,38 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 /* O8/O9 refraction */
                 double dd = 0, dt_ns = 0, x_slant = 0, tau_aer = 0, sin_arr, cos_zen, sin_zen;
                 double rv[3] = { 0, 0, 1 };                  /* local vertical at A_e */
-                if (atm->model == 2) { rv[0] = Ae[0]; rv[1] = Ae[1]; rv[2] = Ae[2] + Rg; norm3(rv); }
+                if (atm->model >= 2) { rv[0] = Ae[0]; rv[1] = Ae[1]; rv[2] = Ae[2] + Rg; norm3(rv); }
                 cos_zen = -(u[0]*rv[0] + u[1]*rv[1] + u[2]*rv[2]);
                 if (cos_zen > 1.0) cos_zen = 1.0;
                 sin_zen = sqrt(fmax(0.0, 1.0 - cos_zen*cos_zen));
                 sin_arr = sin_zen;
                 double delta = 0.0;                          /* rotation of the direction in the ray plane */
                 double perp_flat = 0.0, rho_I = 0.0, cos_chi = 0.0;   /* R21: transverse displacement of the flat-plane table */
+                double perp_cyl = 0.0;                       /* R24: displacement across the direction of flight */
                 if (par->trace == ORC_TRACE_STRAIGHT) {
                     dt_ns = eta_e * D / ORC_C_M_PER_NS;      /* homogeneous: t = t_e + n D / c */
                     if (atm->model != 0) {
                         /* straight line through a stratified medium: no delay model beyond n_e */
                     }
+                } else if (atm->model == 3) {
+                    /* R24 cylindrical model: the plane of curvature is the vertical plane through the origin's vertical and
+                     * the emission point (frozen per photon); psi = azimuth of the flight against it */
+                    double d_e = sqrt(Ae[0]*Ae[0] + Ae[1]*Ae[1]);
+                    double ephi[2] = { 1.0, 0.0 };
+                    if (d_e > 1e-6) { ephi[0] = Ae[0] / d_e; ephi[1] = Ae[1] / d_e; }
+                    else if (hn > 1e-12) { ephi[0] = eh[0]; ephi[1] = eh[1]; }
+                    double cpsi = eh[0]*ephi[0] + eh[1]*ephi[1], spsi = ephi[0]*eh[1] - ephi[1]*eh[0];
+                    if (!(hn > 1e-12)) { cpsi = 1.0; spsi = 0.0; }
+                    double corr[5];
+                    int bad;
+                    if (par->trace == ORC_TRACE_NUMERIC) {
+                        bad = cos_zen <= 0.0 || orc_cyl_correction(atm, h_e, sin_zen, cos_zen, atan2(spsi, cpsi), par->substeps, corr);
+                    } else {
+                        bad = cos_zen <= 0.0 || orc_table_cyl_lookup(tab, h_e, acos(cos_zen), cpsi * cpsi, corr);
+                        corr[1] *= spsi * cpsi;                  /* the table holds the across displacement / (sin psi cos psi) */
+                    }
+                    if (bad) { ph.status = ORC_ST_TABLE_RANGE; lc[ORC_CNT_TABLE_RANGE]++; goto store; }
+                    dd = corr[0]; perp_cyl = corr[1]; dt_ns = corr[2]; x_slant = corr[3]; tau_aer = corr[4];
                 } else if (par->trace == ORC_TRACE_NUMERIC) {
                     double r[6];
                     if (cos_zen <= 0.0 || orc_trace(atm, atm->model == 2, h_e, sin_zen, cos_zen, atm->h_obs, par->substeps, r)) {
@@ -1232,7 +1407,7 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                      * index at both ends, also when the cone angle is dispersive (R13: the table is valid at
                      * lambda0 and refraction is not dispersive) */
                     const double n_ray = 1.0 + eta_e;
-                    if (atm->model == 2) {
+                    if (atm->model >= 2) {                   /* cylindrical: the spherical formula (differs by < 1e-6 rad, R24) */
                         double re = atm->earth_radius + h_e;
                         double a_line = re * sin_zen / Rg;
                         double a_true = n_ray * re * sin_zen / (n_ground * Rg);
@@ -1254,6 +1429,10 @@ int orc_run(const orc_atmosphere *atm, const orc_detector *det, const orc_params
                 /* landed: corrected position, time, direction */
                 ph.x = I[0] + dd * eh[0];
                 ph.y = I[1] + dd * eh[1];
+                if (perp_cyl != 0.0) {                           /* R24: along e_h turned by +90 degrees */
+                    ph.x += perp_cyl * (-eh[1]);
+                    ph.y += perp_cyl * eh[0];
+                }
                 if (perp_flat != 0.0 && rho_I > 1e-9) {          /* R21: across the direction of flight, towards r^ */
                     ph.x += perp_flat * (I[0] / rho_I - cos_chi * eh[0]);
                     ph.y += perp_flat * (I[1] / rho_I - cos_chi * eh[1]);

@@ -98,7 +98,7 @@ COUNTER_NAMES = ("segments", "seg_below_threshold", "seg_lv1", "seg_emitting", "
                  "lv2", "table_range", "roulette", "landed", "in_grid", "tel_hit", "cam_hit", "nonfinite")
 ST_LANDED, ST_UPGOING, ST_LV2, ST_TABLE_RANGE, ST_ROULETTE = range(5)
 
-_MODEL = {"homogeneous": 0, "planar": 1, "spherical": 2}
+_MODEL = {"homogeneous": 0, "planar": 1, "spherical": 2, "cylindrical": 3}
 _EMIT = {"cherenkov": 0, "fluorescence": 1}
 _TRACE = {"straight": 0, "numeric": 1, "table": 2}
 _TRANS = {"off": 0, "weight": 1, "roulette": 2}
@@ -161,6 +161,15 @@ def lib():
             L.orc_table_flat_lookup.restype = C.c_int
             L.orc_table_flat_lookup.argtypes = [C.POINTER(Table), C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double),
                                                 C.POINTER(C.c_double)]
+            L.orc_trace_cyl.restype = C.c_int
+            L.orc_trace_cyl.argtypes = [C.POINTER(Atmosphere)] + [C.c_double] * 5 + [C.c_int, C.POINTER(C.c_double)]
+            L.orc_cyl_correction.restype = C.c_int
+            L.orc_cyl_correction.argtypes = [C.POINTER(Atmosphere)] + [C.c_double] * 4 + [C.c_int, C.POINTER(C.c_double)]
+            L.orc_build_table_cyl.restype = None
+            L.orc_build_table_cyl.argtypes = [C.POINTER(Atmosphere), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                              C.c_int, C.POINTER(C.c_float)]
+            L.orc_table_cyl_lookup.restype = C.c_int
+            L.orc_table_cyl_lookup.argtypes = [C.POINTER(Table), C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]
             L.orc_table_lookup.restype = C.c_int
             L.orc_table_lookup.argtypes = [C.POINTER(Table), C.c_double, C.c_double, C.POINTER(C.c_double)]
             L.orc_transmission.restype = C.c_double
@@ -353,6 +362,33 @@ def build_table_flat(atm: dict, table: dict, sub: int = 1) -> np.ndarray:
     return out
 
 
+def trace_cyl(atm: dict, h_e, zen_rad, psi_rad, h_g, sub=1):
+    """R24: the layered ray in the cylindrical model; returns (no_ground, [central angle, S, cT, X, tau, y', ux', uy', uz'])."""
+    keep = _Keep()
+    out = (C.c_double * 9)()
+    bad = lib().orc_trace_cyl(C.byref(atmosphere_struct(atm, keep)), float(h_e), math.sin(zen_rad), math.cos(zen_rad),
+                              float(psi_rad), float(h_g), int(sub), out)
+    return bool(bad), list(out)
+
+
+def cyl_correction(atm: dict, h_e, zen_rad, psi_rad, sub=1):
+    """R24: (bad, [along, across, dt_ns, X_slant, tau_aer]) of the cylindrical ray against the straight line."""
+    keep = _Keep()
+    out = (C.c_double * 5)()
+    bad = lib().orc_cyl_correction(C.byref(atmosphere_struct(atm, keep)), float(h_e), math.sin(zen_rad), math.cos(zen_rad),
+                                   float(psi_rad), int(sub), out)
+    return bool(bad), list(out)
+
+
+def build_table_cyl(atm: dict, table: dict, sub: int = 1) -> np.ndarray:
+    """R24: [n_c][n_h][n_zen][5], third axis c = cos^2(psi); ch1 = across displacement / (sin psi cos psi)."""
+    keep = _Keep()
+    out = np.empty((table["n_c"], table["n_h"], table["n_zen"], 5), dtype=np.float32)
+    lib().orc_build_table_cyl(C.byref(atmosphere_struct(atm, keep)), table["n_h"], table["n_zen"], table["n_c"],
+                              float(table["h_max"]), math.radians(float(np.float32(table["zen_max_deg"]))), int(sub), _fp(out))
+    return out
+
+
 def table_struct(table: dict, data: np.ndarray, keep: _Keep, data3: np.ndarray | None = None) -> Table:
     t = Table()
     t.n_h, t.n_zen, t.n_ch = int(table["n_h"]), int(table["n_zen"]), int(data.shape[-1])
@@ -360,7 +396,10 @@ def table_struct(table: dict, data: np.ndarray, keep: _Keep, data3: np.ndarray |
     t.zen_max_rad = math.radians(float(np.float32(table["zen_max_deg"])))
     t.data = keep.f32(data)
     if data3 is not None:
-        t.n_rho, t.rho_max = int(table["n_rho"]), float(np.float32(table["rho_max_m"]))
+        if data3.ndim == 4:                                 # cylindrical model: [n_c][n_h][n_zen][5], third axis c in [0, 1]
+            t.n_rho, t.rho_max = int(table["n_c"]), 1.0
+        else:
+            t.n_rho, t.rho_max = int(table["n_rho"]), float(np.float32(table["rho_max_m"]))
         t.data3 = keep.f32(data3)
     return t
 
@@ -417,6 +456,16 @@ def table_for(cfg: dict, sub: int = 1) -> np.ndarray | None:
     return _table_cache[key]
 
 
+def table_cyl_for(cfg: dict, sub: int = 1) -> np.ndarray | None:
+    """The cylindrical model's table (R24) if the config's table has the third axis (n_c)."""
+    if cfg.get("table") is None or not cfg["table"].get("n_c"):
+        return None
+    key = ("cyl",) + _table_key(cfg, sub)
+    if key not in _table_cache:
+        _table_cache[key] = build_table_cyl(cfg["atmosphere"], cfg["table"], sub)
+    return _table_cache[key]
+
+
 def table_flat_for(cfg: dict, sub: int = 1) -> np.ndarray | None:
     """The flat-plane table of R21 if the config's table has the extra axes (n_rho, rho_max_m)."""
     if cfg.get("table") is None or not cfg["table"].get("n_rho"):
@@ -445,9 +494,10 @@ def run(cfg: dict, record: bool = True, table_data: np.ndarray | None = None, th
     n_seg = len(cfg["segments"]["x"])
     tab_ptr = None
     if cfg.get("table") is not None and cfg["params"]["trace"] == "table":
+        cyl = cfg["atmosphere"]["model"] == "cylindrical"
         if table_data is None:
-            table_data = table_for(cfg)
-        data3 = table_flat_for(cfg) if int(cfg["params"].get("flat_plane", 0)) == 2 else None
+            table_data = table_for(cfg) if not cyl else np.zeros((cfg["table"]["n_h"], cfg["table"]["n_zen"], 5), np.float32)
+        data3 = table_cyl_for(cfg) if cyl else (table_flat_for(cfg) if int(cfg["params"].get("flat_plane", 0)) == 2 else None)
         tab = table_struct(cfg["table"], table_data, keep, data3)
         tab_ptr = C.byref(tab)
     dd = cfg["detector"]

@@ -585,7 +585,8 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_NONFINITE, WC_EMITTED, 
 // roulette without aerosol, ground histogram + telescope grid, WRITE_TEL, all outputs present) and
 // compiles in the optional features whose bits are set; the host picks the variant when the call
 // matches one that is instantiated (launch_emit_propagate).  SPEC = 0 reads every switch at run time.
-constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32, kSpecFlatTab = 64;
+constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32, kSpecFlatTab = 64,
+              kSpecNoGrid = 128;     // production setting without a ground histogram (telescope spheres only: BASELINE configs[2])
 template <int EMIT, int TRACE, bool SPH, int SPEC>
 __global__ void __launch_bounds__(kernel_threads(TRACE), kernel_min_blocks(TRACE))
 k_emit_propagate(const __grid_constant__ KArgs a)
@@ -656,8 +657,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         iters_pending = 0;
     };
 
-    const bool has_hist = SPEC ? true : (det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr);
-    const bool has_grid_geom = SPEC ? true : (det.hist_nx > 0 && !det.cam_enabled);
+    const bool has_hist = SPEC ? !(SPEC & kSpecNoGrid) : (det.hist_nx > 0 && !det.cam_enabled && run.out.hist != nullptr);
+    const bool has_grid_geom = SPEC ? !(SPEC & kSpecNoGrid) : (det.hist_nx > 0 && !det.cam_enabled);
     const bool f_lv2 = SPEC ? true : run.lv2 != 0;
     const bool f_tel = SPEC ? true : det.n_tel > 0;
     const bool f_grid = SPEC ? true : det.use_grid != 0;
@@ -1851,11 +1852,12 @@ static int array_production_setting(const KArgs &a)
     const DevRun &r = a.run;
     const DevDet &d = a.det;
     const bool base = r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
-           (a.atm.ray_inv_X > 0.f || a.atm.n_ext > 0) && !(a.atm.aer_L > 0.f) && d.hist_nx > 0 && !d.cam_enabled && r.out.hist != nullptr &&
+           (a.atm.ray_inv_X > 0.f || a.atm.n_ext > 0) && !(a.atm.aer_L > 0.f) && !d.cam_enabled &&
+           ((d.hist_nx > 0 && r.out.hist != nullptr) || d.hist_nx == 0) &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
            r.out.tel_counts != nullptr && !r.force_generic;
     if (!base) return 0;
-    return kSpecBase | (r.flat_plane == 1 ? kSpecFlat : 0) | (r.flat_plane == 2 ? kSpecFlatTab : 0) | (a.atm.n_ext > 0 ? kSpecExt : 0) | (r.disp_b != 0.f ? kSpecDisp : 0) |
+    return kSpecBase | (d.hist_nx == 0 ? kSpecNoGrid : 0) | (r.flat_plane == 1 ? kSpecFlat : 0) | (r.flat_plane == 2 ? kSpecFlatTab : 0) | (a.atm.n_ext > 0 ? kSpecExt : 0) | (r.disp_b != 0.f ? kSpecDisp : 0) |
            (r.n_eff > 0 ? kSpecEff : 0) | (d.opt_enabled ? kSpecOpt : 0);
 }
 
@@ -1874,6 +1876,7 @@ cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 #define C8_SPEC(M) \
     if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, smem, st);
 #endif
+    C8_SPEC(kSpecNoGrid)
     C8_SPEC(kSpecFlat)
     C8_SPEC(kSpecFlatTab)
     C8_SPEC(kSpecExt)

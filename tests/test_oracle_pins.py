@@ -1276,6 +1276,132 @@ def test_flat_plane_table_of_the_thesis_four_axes():
     print("flat-plane table vs analytic step, worst position difference [m]:", worst)
 
 
+# ------------------------------------------------------------------ A5 cylindrical atmosphere model (R24, row f1)
+def _brute_force_ray_cyl(atm, h_e, zen, psi, ds=2.0):
+    """RK4 on d/ds (n u) = grad n with n(h), h = sqrt(x'^2 + z'^2) - R: the medium of coaxial cylinders about the y' axis
+    (independent numpy code); from (0, 0, R + h_e) to the cylinder h = h_obs.  Returns position and unit direction."""
+    eta = atm["refractivity"].astype(np.float64)
+    dh, R, hobs = atm["dh"], atm["earth_radius"], atm["h_obs"]
+
+    def n_and_grad(p):
+        r = math.hypot(p[0], p[2])
+        f = min(max((r - R) / dh, 0.0), len(eta) - 1.000001)
+        i = int(f)
+        g = (eta[i + 1] - eta[i]) / dh
+        return 1 + eta[i] + (f - i) * (eta[i + 1] - eta[i]), g * np.array([p[0] / r, 0.0, p[2] / r]), r - R
+
+    def rhs(y):
+        n, g, _ = n_and_grad(y[:3])
+        return np.concatenate([y[3:6] / n, g])
+
+    A = np.array([0.0, 0.0, R + h_e])
+    U = np.array([math.sin(zen) * math.cos(psi), math.sin(zen) * math.sin(psi), -math.cos(zen)])
+    y = np.concatenate([A, n_and_grad(A)[0] * U])
+    while True:
+        k1 = rhs(y); k2 = rhs(y + 0.5 * ds * k1); k3 = rhs(y + 0.5 * ds * k2); k4 = rhs(y + ds * k3)
+        yn = y + ds / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+        h0, h1 = n_and_grad(y[:3])[2], n_and_grad(yn[:3])[2]
+        if h1 <= hobs:
+            f = (h0 - hobs) / (h0 - h1)
+            out = y + f * (yn - y)
+            return out[:3], out[3:6] / np.linalg.norm(out[3:6])
+        y = yn
+
+
+def test_cylindrical_model_tracer_limits_and_brute_force():
+    """Reading R24 (thesis sec. 3.3.3): the gradient keeps its rotation angle, only its zenith angle follows the
+    position: coaxial cylinders.  Pins of the layered tracer (Eq. 3.15 in three dimensions): flight in the plane of
+    curvature is the spherical model's ray, flight along the axis is the planar model's ray, the component of n u along
+    the axis is conserved, oblique flight against an independent 3-D RK4 integration in that medium; and the thesis'
+    statements: the model agrees with the spherical one near the plane of curvature and loses accuracy with the
+    distance travelled across it ("significant impact only for ... several tenths of kilometres")."""
+    atm = W.make_config(4, n_segments=1)["atmosphere"]
+    hg = atm["h_obs"]
+    for h_e, zen in ((12000.0, 0.9), (30000.0, 0.5), (5000.0, 1.2)):
+        sph = O.trace(atm, True, h_e, zen, hg)
+        bad_c, cyl = O.trace_cyl(atm, h_e, zen, 0.0, hg)
+        assert sph is not None and not bad_c
+        assert cyl[0] == pytest.approx(sph["disp"], rel=1e-12) and cyl[1] == pytest.approx(sph["S"], rel=1e-13)
+        assert cyl[2] == pytest.approx(sph["cT"], rel=1e-13) and cyl[3] == pytest.approx(sph["X"], rel=1e-12) and abs(cyl[5]) < 1e-9
+        pla = O.trace(dict(atm, model="planar"), False, h_e, zen, hg)
+        bad_c, cyl = O.trace_cyl(atm, h_e, zen, 0.5 * math.pi, hg)
+        assert pla is not None and not bad_c and abs(cyl[0]) < 1e-12
+        assert cyl[5] == pytest.approx(pla["disp"], rel=1e-12) and cyl[1] == pytest.approx(pla["S"], rel=1e-13) and cyl[2] == pytest.approx(pla["cT"], rel=1e-13)
+    Rg = atm["earth_radius"] + hg
+    n_e = 1.0 + O.refractivity(atm, 12000.0)
+    n_g = 1.0 + O.refractivity(atm, hg)
+    for zen, psi in ((0.9, 0.7), (1.05, 2.3), (0.6, -1.1)):
+        bad, cyl = O.trace_cyl(atm, 12000.0, zen, psi, hg)
+        assert not bad
+        assert n_g * cyl[7] == pytest.approx(n_e * math.sin(zen) * math.sin(psi), rel=1e-13)      # n u_axis conserved
+        assert np.linalg.norm(cyl[6:9]) == pytest.approx(1.0, abs=1e-13)
+        pos, u = _brute_force_ray_cyl(atm, 12000.0, zen, psi)
+        got = np.array([Rg * math.sin(cyl[0]), cyl[5], Rg * math.cos(cyl[0])])
+        assert np.linalg.norm(got - pos) < 5e-4, (zen, psi, got - pos)
+        assert np.arccos(np.clip(u @ np.array(cyl[6:9]), -1, 1)) < 2e-6
+    # thesis: agrees with the spherical model near the plane of curvature, degrades with the distance across it.  The same
+    # photon (12 km, local zenith 60 deg) flying across the plane of curvature, in both models: the straight line lands
+    # 21 km away; the correction along the flight differs by centimetres, in the plane of curvature by nothing
+    zen = math.radians(60.0)
+    sph = O.trace(atm, True, 12000.0, zen, hg)
+    re = atm["earth_radius"] + 12000.0
+    dd_sph = Rg * sph["disp"] - Rg * (math.asin(re * math.sin(zen) / Rg) - zen)
+    diffs = []
+    for psi_deg in (0.0, 10.0, 45.0, 90.0):
+        bad, corr = O.cyl_correction(atm, 12000.0, zen, math.radians(psi_deg))
+        assert not bad
+        diffs.append(abs(corr[0] - dd_sph))
+    assert diffs[0] < 1e-9 and diffs[1] < 3e-3 and diffs[2] > 5 * diffs[1] and diffs[3] > diffs[2] > 0.01
+    print("cylindrical - spherical, displacement along the flight from 12 km at 60 deg, psi = 0 / 10 / 45 / 90 deg [m]:", diffs)
+    # and with the height (= distance travelled): from 3 km the same geometry differs by millimetres
+    sph3 = O.trace(atm, True, 3000.0, zen, hg)
+    re3 = atm["earth_radius"] + 3000.0
+    dd3 = Rg * sph3["disp"] - Rg * (math.asin(re3 * math.sin(zen) / Rg) - zen)
+    bad, corr3 = O.cyl_correction(atm, 3000.0, zen, math.radians(90.0))
+    assert abs(corr3[0] - dd3) < 5e-3 and diffs[3] > 5 * abs(corr3[0] - dd3)
+
+
+def test_cylindrical_model_table_and_run():
+    """R24: the cylindrical model's table over (height, zenith, cos^2 of the flight azimuth against the plane of curvature):
+    nodes are the tracer's corrections, c = 1 is the spherical table and c = 0 the planar one; the lookup is exact on
+    multilinear functions; whole runs: table photons against per-photon numerical tracing (interpolation error only),
+    and against the spherical model (millimetres near the origin)."""
+    cfg = W.make_config(4, n_segments=300)
+    cfg["atmosphere"]["model"] = "cylindrical"
+    cfg["table"] = dict(n_h=96, n_zen=96, h_max=30000.0, zen_max_deg=60.0, n_c=5)
+    cfg["params"].update(write="all")
+    atm, t = cfg["atmosphere"], cfg["table"]
+    d3 = O.build_table_cyl(atm, t)
+    assert d3.shape == (5, 96, 96, 5)
+    sph = O.build_table(dict(atm, model="spherical"), t)
+    pla = O.build_table(dict(atm, model="planar"), t)
+    ok = np.isfinite(sph[..., 0]) & np.isfinite(d3[4, ..., 0])
+    assert ok.mean() > 0.99
+    for ch in (0, 2, 3):
+        assert np.allclose(d3[4, ..., ch][ok], sph[..., ch][ok], rtol=2e-5, atol=2e-6)       # psi = 1e-3 rad inside the end
+        assert np.allclose(d3[0, ..., ch][ok], pla[..., ch][ok], rtol=2e-5, atol=2e-6)
+    a, b, k = 40, 70, 2
+    bad, corr = O.cyl_correction(atm, a * 30000.0 / 95, b * math.radians(float(np.float32(60.0))) / 95, math.acos(math.sqrt(0.5)))
+    assert not bad and d3[k, a, b, 0] == pytest.approx(corr[0], rel=1e-6) and d3[k, a, b, 1] == pytest.approx(corr[1] / 0.5, rel=1e-5)
+    assert abs(d3[k, a, b, 1]) > 1e-3                                   # the across displacement exists (millimetres)
+    gpu_like = O.run(cfg)                                               # trace = table
+    num = copy.deepcopy(cfg)
+    num["params"]["trace"] = "numeric"
+    ref = O.run(num)
+    a_, b_ = gpu_like["photons"], ref["photons"]
+    both = (a_["status"] == O.ST_LANDED) & (b_["status"] == O.ST_LANDED)
+    assert both.sum() > 5e4 and (a_["status"] != b_["status"]).mean() < 2e-4
+    d = np.hypot(a_["x"][both] - b_["x"][both], a_["y"][both] - b_["y"][both])
+    assert d.max() < 5e-3 and np.abs(a_["t"][both] - b_["t"][both]).max() < 5e-3           # this coarse table's interpolation error
+    sphc = copy.deepcopy(cfg)
+    sphc["atmosphere"]["model"] = "spherical"
+    sphc["table"] = dict(n_h=96, n_zen=96, h_max=30000.0, zen_max_deg=60.0)
+    sp = O.run(sphc)["photons"]
+    both = (a_["status"] == O.ST_LANDED) & (sp["status"] == O.ST_LANDED)
+    d = np.hypot(a_["x"][both] - sp["x"][both], a_["y"][both] - sp["y"][both])
+    assert 1e-7 < d.max() < 5e-3                                        # near the origin the two models agree to millimetres
+
+
 # ------------------------------------------------------------------ sanitizers (SURVEY section 5)
 def test_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers():
     """The oracle compiled with -fsanitize=address,undefined (-fno-sanitize-recover) runs small instances of all five
