@@ -53,7 +53,11 @@ const char *c8ph_last_error(const c8ph_ctx *ctx);
 int c8ph_version(void);
 
 /* ---- atmosphere (thesis sec. 3.3, sec. 4.1) ------------------------------ */
-enum { C8PH_ATM_HOMOGENEOUS = 0, C8PH_ATM_PLANAR = 1, C8PH_ATM_SPHERICAL = 2 };
+/* C8PH_ATM_CYLINDRICAL (thesis sec. 3.3.3; R24): per photon the refractive-index gradient keeps the
+ * azimuth of the emission point about the origin's vertical and only its zenith angle follows the position: coaxial
+ * cylinders instead of spheres.  Heights and local verticals at the emission point are those of the spherical model;
+ * table tracing only, with a table built with n_c >= 2; no aerosol, no flat_plane.                                 */
+enum { C8PH_ATM_HOMOGENEOUS = 0, C8PH_ATM_PLANAR = 1, C8PH_ATM_SPHERICAL = 2, C8PH_ATM_CYLINDRICAL = 3 };
 typedef struct {
     uint32_t size;                   /* sizeof(c8ph_atmosphere_desc), for versioning              */
     int32_t model;                   /* C8PH_ATM_*                                                 */
@@ -90,6 +94,10 @@ typedef struct {
      * as even / odd / transverse parts).  n_rho = 0: not built.  Used by params.flat_plane = 2.                    */
     int32_t n_rho;
     float rho_max_m;
+    /* Cylindrical model (R24): third axis c = cos^2(azimuth of the flight against the plane of curvature), n_c >= 2
+     * uniform nodes in [0, 1] (c = 0: the planar model's table, c = 1: the spherical one); texels (dd, dt, X_slant,
+     * displacement across the flight / (sin psi cos psi)).  0: not built.                                          */
+    int32_t n_c;
 } c8ph_table_desc;
 /* One kernel, one thread per node: the exact layered-Snell ray (fp64) from (h_a, theta_b) to the
  * observation sphere/plane minus the straight line (asynchronous on `stream`, a cudaStream_t).   */
@@ -101,6 +109,8 @@ int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *desc, const float
 /* The flat-plane table as stored: HOST [2][n_rho][n_h][n_zen][4]; part 0 (even) = dd [m], dt [ns], X_slant, tau_aer
  * relative to the straight line to the PLANE; part 1 = odd dd, odd dt, transverse displacement P [m], 0.  Synchronous. */
 int c8ph_get_trace_table_flat(c8ph_ctx *ctx, float *host_out, int64_t n_floats);
+/* The cylindrical model's table as stored: HOST [n_c][n_h][n_zen][4].  Synchronous. */
+int c8ph_get_trace_table_cyl(c8ph_ctx *ctx, float *host_out, int64_t n_floats);
 
 /* ---- detector (thesis sec. 6.2; camera: BASELINE cfg3) ---------------------------- */
 typedef struct {

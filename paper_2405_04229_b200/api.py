@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("C8PH_LIB") or os.path.join(_HERE, "libc8ph.so")
 
 OK, E_ARG, E_STATE, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4
-ATM = {"homogeneous": 0, "planar": 1, "spherical": 2}
+ATM = {"homogeneous": 0, "planar": 1, "spherical": 2, "cylindrical": 3}
 EMIT = {"cherenkov": 0, "fluorescence": 1}
 TRACE = {"straight": 0, "numeric": 1, "table": 2}
 TRANS = {"off": 0, "weight": 1, "roulette": 2}
@@ -34,7 +34,7 @@ EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8
            "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
            "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
            "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill", "c8ph_set_line_spectrum", "c8ph_set_efficiency",
-           "c8ph_get_trace_table_flat")
+           "c8ph_get_trace_table_flat", "c8ph_get_trace_table_cyl")
 
 PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
                          ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
@@ -57,7 +57,7 @@ class AtmosphereDesc(C.Structure):
 class TableDesc(C.Structure):
     _fields_ = [("size", C.c_uint32), ("n_h", C.c_int32), ("n_zen", C.c_int32),
                 ("h_max_m", C.c_float), ("zen_max_deg", C.c_float), ("substeps", C.c_int32),
-                ("n_rho", C.c_int32), ("rho_max_m", C.c_float)]
+                ("n_rho", C.c_int32), ("rho_max_m", C.c_float), ("n_c", C.c_int32)]
 
 
 class Detector(C.Structure):
@@ -126,6 +126,7 @@ def load_library():
         L.c8ph_get_trace_table.argtypes = [C.c_void_p, _fp, C.c_int64]
         L.c8ph_set_trace_table.argtypes = [C.c_void_p, C.POINTER(TableDesc), _fp]
         L.c8ph_get_trace_table_flat.argtypes = [C.c_void_p, _fp, C.c_int64]
+        L.c8ph_get_trace_table_cyl.argtypes = [C.c_void_p, _fp, C.c_int64]
         L.c8ph_set_detector.argtypes = [C.c_void_p, C.POINTER(Detector)]
         L.c8ph_emit_propagate.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_int64, C.c_int64,
                                           C.POINTER(Params), C.c_uint64, C.POINTER(Outputs), C.c_void_p]
@@ -218,7 +219,15 @@ class Context:
         t.h_max_m, t.zen_max_deg = float(table["h_max"]), float(table["zen_max_deg"])
         t.substeps = int(table.get("substeps", 1))
         t.n_rho, t.rho_max_m = int(table.get("n_rho", 0) or 0), float(table.get("rho_max_m", 0.0) or 0.0)
+        t.n_c = int(table.get("n_c", 0) or 0)
         return t
+
+    def get_trace_table_cyl(self) -> np.ndarray:
+        """[n_c][n_h][n_zen][4] texels of the cylindrical model's table (R24)."""
+        t = self._table
+        out = np.empty((t["n_c"], t["n_h"], t["n_zen"], 4), dtype=np.float32)
+        self._check(self.lib.c8ph_get_trace_table_cyl(self._h, out.ctypes.data_as(_fp), out.size))
+        return out
 
     def get_trace_table_flat(self) -> np.ndarray:
         """[2 (even, odd)][n_rho][n_h][n_zen][4] texels of the flat-plane table (R21)."""
@@ -241,7 +250,7 @@ class Context:
         self._table = dict(table)
         data = _f32(data)
         assert data.shape == (table["n_h"], table["n_zen"], TABLE_CHANNELS)
-        self._check(self.lib.c8ph_set_trace_table(self._h, C.byref(self._table_desc(dict(table, n_rho=0))), data.ctypes.data_as(_fp)))
+        self._check(self.lib.c8ph_set_trace_table(self._h, C.byref(self._table_desc(dict(table, n_rho=0, n_c=0))), data.ctypes.data_as(_fp)))
 
     def set_detector(self, det: dict):
         d = Detector()

@@ -43,6 +43,10 @@ struct DevTable {
     int n_rho;
     float rho_max, inv_drho, e_max;
     const float4 *flatE, *flatO;
+    // cylindrical model (R24): [n_c][n_h][n_zen] texels (dd, dt, X_slant, across displacement / (sin psi cos psi))
+    int n_c;
+    float c_max;                    // (float)(n_c - 1)
+    const float4 *cyl;
 };
 
 // Uniform grid over the telescope array.  Every cell lists the telescopes that a point of the cell
@@ -157,6 +161,8 @@ struct TableBuildArgs {
     int n_rho;                      // flat-plane table (R21): nodes in rho, 0: none
     double rho_max;
     float4 *flatE, *flatO;          // [n_rho][n_h][n_zen] each
+    int n_c;                        // cylindrical model's table (R24): nodes in c = cos^2(psi), 0: none
+    float4 *cyl;                    // [n_c][n_h][n_zen]
 };
 
 struct SubstepArgs {

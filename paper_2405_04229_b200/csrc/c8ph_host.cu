@@ -33,6 +33,7 @@ struct c8ph_ctx {
     float *d_full = nullptr;
     float4 *d_hot = nullptr;
     float4 *d_flat = nullptr;          // flat-plane table (R21): E texels then O texels
+    float4 *d_cyl = nullptr;           // cylindrical model's table (R24)
     cudaArray_t tab_arr = nullptr;     // the hot texels as a 2-D array behind a texture object (DevTable::tex)
     cudaTextureObject_t tab_tex = 0;
     // detector
@@ -132,7 +133,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
     dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp);
-    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel); dfree(ctx->d_flat);
+    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel); dfree(ctx->d_flat); dfree(ctx->d_cyl);
     if (ctx->tab_tex) cudaDestroyTextureObject(ctx->tab_tex);
     if (ctx->tab_arr) cudaFreeArray(ctx->tab_arr);
     for (int k = 0; k < 2; ++k) { dfree(ctx->d_g_start[k]); dfree(ctx->d_g_items[k]); dfree(ctx->d_g_kmin[k]); }
@@ -168,7 +169,8 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
 {
     if (!ctx) return C8PH_E_ARG;
     if (!d || d->size != sizeof(c8ph_atmosphere_desc)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: bad desc/size");
-    if (d->model < C8PH_ATM_HOMOGENEOUS || d->model > C8PH_ATM_SPHERICAL) return fail(ctx, C8PH_E_ARG, "init_atmosphere: bad model");
+    if (d->model < C8PH_ATM_HOMOGENEOUS || d->model > C8PH_ATM_CYLINDRICAL) return fail(ctx, C8PH_E_ARG, "init_atmosphere: bad model");
+    if (d->model == C8PH_ATM_CYLINDRICAL && d->aer_L_m > 0.f) return fail(ctx, C8PH_E_ARG, "init_atmosphere: no aerosol in the cylindrical model");
     CU(cudaSetDevice(ctx->device));
     std::vector<float> eta, xv;
     double h0 = d->h0_m, dh = d->dh_m;
@@ -184,7 +186,7 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
         else xv.assign(d->n_nodes, 0.f);
     }
     for (float v : eta) if (!(v > -1.f) || !std::isfinite(v)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: non-finite refractivity");
-    if (d->model == C8PH_ATM_SPHERICAL && !(d->earth_radius_m > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: earth_radius");
+    if (d->model >= C8PH_ATM_SPHERICAL && !(d->earth_radius_m > 0.f)) return fail(ctx, C8PH_E_ARG, "init_atmosphere: earth_radius");
     const int n = (int)eta.size();
     const int n_pad = (n + 3) & ~3;
     std::vector<float> dxv(n_pad, 0.f), eta_p(n_pad, eta.back()), xv_p(n_pad, xv.back());
@@ -253,8 +255,10 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
     if (!ctx->have_atm) return fail(ctx, C8PH_E_STATE, "trace_table: atmosphere not initialised");
     if (t->n_rho < 0 || t->n_rho == 1 || t->n_rho > 4096 || (t->n_rho >= 2 && (!(t->rho_max_m > 0.f) || ctx->atm.model != C8PH_ATM_SPHERICAL)))
         return fail(ctx, C8PH_E_ARG, "trace_table: the flat-plane table needs n_rho >= 2, rho_max_m > 0 and the spherical model");
+    if (t->n_c < 0 || t->n_c == 1 || t->n_c > 1024 || (t->n_c >= 2 && ctx->atm.model != C8PH_ATM_CYLINDRICAL))
+        return fail(ctx, C8PH_E_ARG, "trace_table: n_c >= 2 needs the cylindrical model");
     CU(cudaSetDevice(ctx->device));
-    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_flat);
+    dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_flat); dfree(ctx->d_cyl);
     const size_t n = (size_t)t->n_h * t->n_zen;
     CU(cudaMalloc(&ctx->d_full, n * C8PH_TABLE_CHANNELS * sizeof(float)));
     CU(cudaMalloc(&ctx->d_hot, n * sizeof(float4)));
@@ -273,6 +277,11 @@ static int alloc_table(c8ph_ctx *ctx, const c8ph_table_desc *t)
         d.n_rho = t->n_rho; d.rho_max = t->rho_max_m; d.inv_drho = (float)((t->n_rho - 1) / (double)t->rho_max_m);
         d.e_max = (float)(t->n_rho - 1);
         d.flatE = ctx->d_flat; d.flatO = ctx->d_flat + (size_t)t->n_rho * n;
+    }
+    d.n_c = 0; d.c_max = 0.f; d.cyl = nullptr;
+    if (t->n_c >= 2) {
+        CU(cudaMalloc(&ctx->d_cyl, (size_t)t->n_c * n * sizeof(float4)));
+        d.n_c = t->n_c; d.c_max = (float)(t->n_c - 1); d.cyl = ctx->d_cyl;
     }
     // texture view of the hot texels: x = zenith node, y = height node, unnormalised coordinates, clamped, bilinear
     if (ctx->tab_tex) { cudaDestroyTextureObject(ctx->tab_tex); ctx->tab_tex = 0; }
@@ -317,11 +326,12 @@ extern "C" int c8ph_build_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, v
     a.full = ctx->d_full; a.hot = ctx->d_hot;
     a.n_rho = ctx->tab.n_rho; a.rho_max = ctx->tab.rho_max;
     a.flatE = const_cast<float4 *>(ctx->tab.flatE); a.flatO = const_cast<float4 *>(ctx->tab.flatO);
+    a.n_c = ctx->tab.n_c; a.cyl = ctx->d_cyl;
     cudaError_t e = launch_build_table(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "build_trace_table launch");
     rc = fill_table_texture(ctx, (cudaStream_t)stream);
     if (rc) return rc;
-    ctx->launches += ctx->tab.n_rho >= 2 ? 2 : 1;
+    ctx->launches += 1 + (ctx->tab.n_rho >= 2 ? 1 : 0) + (ctx->tab.n_c >= 2 ? 1 : 0);
     ctx->have_table = true;
     return C8PH_OK;
 }
@@ -335,6 +345,18 @@ extern "C" int c8ph_get_trace_table_flat(c8ph_ctx *ctx, float *host_out, int64_t
     CU(cudaSetDevice(ctx->device));
     CU(cudaDeviceSynchronize());
     CU(cudaMemcpy(host_out, ctx->d_flat, need * sizeof(float), cudaMemcpyDeviceToHost));
+    return C8PH_OK;
+}
+
+extern "C" int c8ph_get_trace_table_cyl(c8ph_ctx *ctx, float *host_out, int64_t n_floats)
+{
+    if (!ctx) return C8PH_E_ARG;
+    if (!ctx->have_table || ctx->tab.n_c < 2) return fail(ctx, C8PH_E_STATE, "get_trace_table_cyl: no cylindrical table");
+    const int64_t need = (int64_t)ctx->tab.n_c * ctx->tab.n_h * ctx->tab.n_zen * 4;
+    if (!host_out || n_floats < need) return fail(ctx, C8PH_E_ARG, "get_trace_table_cyl: buffer too small");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(host_out, ctx->d_cyl, need * sizeof(float), cudaMemcpyDeviceToHost));
     return C8PH_OK;
 }
 
@@ -354,7 +376,7 @@ extern "C" int c8ph_set_trace_table(c8ph_ctx *ctx, const c8ph_table_desc *t, con
 {
     if (!ctx) return C8PH_E_ARG;
     if (!host_in) return fail(ctx, C8PH_E_ARG, "set_trace_table: host_in is NULL");
-    if (t && t->size == sizeof(c8ph_table_desc) && t->n_rho != 0) return fail(ctx, C8PH_E_ARG, "set_trace_table: n_rho must be 0 (the flat-plane table is built, not injected)");
+    if (t && t->size == sizeof(c8ph_table_desc) && (t->n_rho != 0 || t->n_c != 0)) return fail(ctx, C8PH_E_ARG, "set_trace_table: n_rho and n_c must be 0 (those tables are built, not injected)");
     int rc = alloc_table(ctx, t);
     if (rc) return rc;
     const size_t n = (size_t)t->n_h * t->n_zen;
@@ -690,8 +712,12 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     if (!o->counters) return fail(ctx, C8PH_E_ARG, "emit_propagate: counters is NULL");
     if (o->photons && o->photon_capacity < 0) return fail(ctx, C8PH_E_ARG, "emit_propagate: photon_capacity");
     if (p->trace == C8PH_TRACE_TABLE && !ctx->have_table) return fail(ctx, C8PH_E_STATE, "emit_propagate: trace table not built");
-    if (p->trace == C8PH_TRACE_NUMERIC && ctx->atm.model == C8PH_ATM_SPHERICAL)
-        return fail(ctx, C8PH_E_ARG, "emit_propagate: per-photon numeric tracing is planar only; use the table in the spherical model");
+    if (p->trace == C8PH_TRACE_NUMERIC && ctx->atm.model >= C8PH_ATM_SPHERICAL)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: per-photon numeric tracing is planar only; use the table in the spherical / cylindrical model");
+    if (ctx->atm.model == C8PH_ATM_CYLINDRICAL && p->trace == C8PH_TRACE_TABLE && ctx->have_table && ctx->tab.n_c < 2)
+        return fail(ctx, C8PH_E_STATE, "emit_propagate: the cylindrical model needs a trace table built with n_c >= 2");
+    if (ctx->atm.model == C8PH_ATM_CYLINDRICAL && p->emit == C8PH_EMIT_FLUORESCENCE)
+        return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence is not available in the cylindrical model");
     if (p->trace == C8PH_TRACE_NUMERIC && p->emit == C8PH_EMIT_FLUORESCENCE) return fail(ctx, C8PH_E_ARG, "emit_propagate: fluorescence + numeric tracing");
     if (p->emit == C8PH_EMIT_CHERENKOV && !(p->lambda_min_nm > 0.f && p->lambda_max_nm > p->lambda_min_nm))
         return fail(ctx, C8PH_E_ARG, "emit_propagate: wavelength band");

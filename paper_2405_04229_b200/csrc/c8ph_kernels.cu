@@ -402,6 +402,39 @@ __device__ __forceinline__ TabVal table_lookup_flat(const DevTable &t, float h, 
     return o;
 }
 
+// R24: lookup in the cylindrical model's table: trilinear in (height, zenith, c = cos^2 psi), 8 LDG.128;
+// texel = (dd, dt, X_slant, across displacement / (sin psi cos psi))
+__device__ __forceinline__ TabVal table_lookup_cyl(const DevTable &t, float h, float thz, float c, float &ptilde)
+{
+    TabVal o;
+    o.bad = !(h <= t.h_max) || !(thz <= t.zen_max) || !(h >= 0.f) || !(c >= 0.f) || !(c <= 1.f);
+    const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
+    const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
+    const float e = fminf(fmaxf(c * t.c_max, 0.f), t.c_max);
+    const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2), ic = min((int)e, t.n_c - 2);
+    const float ff = f - (float)ia, gg = g - (float)ib, ee = e - (float)ic;
+    const unsigned plane = (unsigned)(t.n_h * t.n_zen);
+    const float4 *p = t.cyl + (unsigned)ic * plane + (unsigned)(ia * t.n_zen + ib);
+    const float w11 = ff * gg, w10 = ff - w11, w01 = gg - w11, w00 = (1.f - ff) - w01;
+    float4 lay[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const float4 *pq = p + (unsigned)q * plane;
+        const float4 v00 = __ldg(pq), v01 = __ldg(pq + 1), v10 = __ldg(pq + t.n_zen), v11 = __ldg(pq + t.n_zen + 1);
+        lay[q].x = fmaf(w11, v11.x, fmaf(w10, v10.x, fmaf(w01, v01.x, w00 * v00.x)));
+        lay[q].y = fmaf(w11, v11.y, fmaf(w10, v10.y, fmaf(w01, v01.y, w00 * v00.y)));
+        lay[q].z = fmaf(w11, v11.z, fmaf(w10, v10.z, fmaf(w01, v01.z, w00 * v00.z)));
+        lay[q].w = fmaf(w11, v11.w, fmaf(w10, v10.w, fmaf(w01, v01.w, w00 * v00.w)));
+    }
+    o.dd = fmaf(ee, lay[1].x - lay[0].x, lay[0].x);
+    o.dt = fmaf(ee, lay[1].y - lay[0].y, lay[0].y);
+    o.X = fmaf(ee, lay[1].z - lay[0].z, lay[0].z);
+    o.ta = 0.f;
+    ptilde = fmaf(ee, lay[1].w - lay[0].w, lay[0].w);
+    o.bad = o.bad || (o.dd != o.dd) || (ptilde != ptilde);
+    return o;
+}
+
 // ---- telescope search (DevGrid: sorted candidate lists with a per-cell smallest key) -----------
 // cell of (x,y), or -1 outside the grid (outside => no telescope within reach)
 __device__ __forceinline__ int grid_cell(const DevGrid &g, float x, float y)
@@ -673,6 +706,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // flat observation plane: 1 = analytic step from the sphere (R19), 2 = the thesis' table with rho and pointing axes (R21)
     const int f_flat_mode = (!SPH || TRACE == C8PH_TRACE_STRAIGHT) ? 0 : (SPEC ? ((SPEC & kSpecFlat) ? 1 : ((SPEC & kSpecFlatTab) ? 2 : 0)) : run.flat_plane);
     const bool f_flat = f_flat_mode == 1;
+    // cylindrical model (R24): generic variant only; geometry at the emission point as in the spherical model
+    const bool f_cyl = SPEC ? false : (SPH && TRACE == C8PH_TRACE_TABLE && atm.model == C8PH_ATM_CYLINDRICAL);
     const bool f_flat_tab = TRACE == C8PH_TRACE_TABLE && f_flat_mode == 2;
     const int f_write = SPEC ? (int)C8PH_WRITE_TEL : run.write;
     const bool f_cam = SPEC ? false : det.cam_enabled != 0;
@@ -1308,6 +1343,22 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         dt = eta_e * D * kInvC;                          // homogeneous: t = t_e + n D / c
                     } else if (TRACE == C8PH_TRACE_TABLE) {
                         TabVal v;
+                        if (f_cyl) {
+                            // plane of curvature = vertical plane through the origin's vertical and the emission point
+                            // (xl - D u): psi = azimuth of the flight against it
+                            const float xe = fmaf(-D, ux, xl), ye = fmaf(-D, uy, yl);
+                            const float hn2c = ux * ux + uy * uy, de2 = fmaf(xe, xe, ye * ye);
+                            const float ihc = hn2c >= 1e-24f ? rsqrt_fast(hn2c) : 0.f;
+                            const float ehx_ = ux * ihc, ehy_ = uy * ihc;
+                            float epx = ehx_, epy = ehy_;
+                            if (de2 > 1e-12f) { const float id = rsqrt_fast(de2); epx = xe * id; epy = ye * id; }
+                            float cps = ehx_ * epx + ehy_ * epy, sps = epx * ehy_ - epy * ehx_;
+                            if (ihc == 0.f) { cps = 1.f; sps = 0.f; }
+                            float ptilde;
+                            v = table_lookup_cyl(a.tab, h_e, acos01(fmaxf(cz, 0.f)), fminf(cps * cps, 1.f), ptilde);
+                            flat_perp = ptilde * sps * cps;              // across the flight: along e_h turned by +90 degrees
+                            flat_px = -ehy_; flat_py = ehx_;
+                        } else
                         if (f_flat_tab) {
                             // R21: polar radius of the straight-line point and pointing angle of the direction of flight
                             const float hn2f = ux * ux + uy * uy, rho2 = fmaf(xl, xl, yl * yl);
@@ -1411,7 +1462,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const float ih = hn2 >= 1e-18f ? rsqrt_fast(hn2) : 0.f;            // vertical photon: no correction
                     const float ehx = ux * ih, ehy = uy * ih;
                     float cx = fmaf(dd, ehx, ox), cy = fmaf(dd, ehy, oy);               // offset from the anchor
-                    if (f_flat_tab) { cx = fmaf(flat_perp, flat_px, cx); cy = fmaf(flat_perp, flat_py, cy); }
+                    if (f_flat_tab || f_cyl) { cx = fmaf(flat_perp, flat_px, cx); cy = fmaf(flat_perp, flat_py, cy); }
                     if (f_flat) {
                         // R19, flat observation plane (thesis Fig. 4.10): dd, dt and the rotation hold where
                         // the ray meets the observation sphere; the plane z = 0 lies h_I above it at the line point.
@@ -1580,7 +1631,7 @@ __device__ NodeRay trace_node(const DevAtm &atm, double h_e, double th, int subs
 {
     NodeRay o;
     o.ground = true; o.psi = o.S = o.cT = o.X = o.tau = 0.0;
-    const bool sph = atm.model == C8PH_ATM_SPHERICAL;
+    const bool sph = atm.model >= C8PH_ATM_SPHERICAL;     // the cylindrical model's 2-D table is the spherical one
     const double h_g = atm.h_obs;
     const double sz = sin(th);
     const double n_e = 1.0 + eta_lookup_d(atm, h_e);
@@ -1647,7 +1698,7 @@ __global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ Tab
     const double h_e = ia * a.h_max / (a.n_h - 1);
     const double th = ib * a.zen_max / (a.n_zen - 1);
     float out[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
-    const bool sph = atm.model == C8PH_ATM_SPHERICAL;
+    const bool sph = atm.model >= C8PH_ATM_SPHERICAL;     // the cylindrical model's 2-D table is the spherical one
     const double h_g = atm.h_obs;
     if (h_e > h_g) {
         const double sz = sin(th), cz = cos(th);
@@ -1806,6 +1857,82 @@ __global__ void __launch_bounds__(128) k_build_table_flat(const __grid_constant_
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// R24, cylindrical model (thesis sec. 3.3.3): coaxial cylinders about a horizontal axis through the Earth's centre.  The
+// gradient has no component along the axis, so kappa = n u_axis is conserved and the motion in the plane of curvature is
+// Bouguer's with the effective index n_eff = sqrt(n^2 - kappa^2): the layer loop of trace_node with n_eff in the
+// geometry, the real path s n / n_eff per in-plane chord s, and the advance along the axis kappa s / n_eff.
+// One thread per (height, zenith, c) node, psi = acos(sqrt(c)) kept 1e-3 rad inside the ends.
+__global__ void __launch_bounds__(128) k_build_table_cyl(const __grid_constant__ TableBuildArgs a)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const int plane = a.n_h * a.n_zen;
+    if (idx >= plane * a.n_c) return;
+    const int k = idx / plane, node = idx % plane;
+    const int ia = node / a.n_zen, ib = node % a.n_zen;
+    const DevAtm &atm = a.atm;
+    const double h_e = ia * a.h_max / (a.n_h - 1);
+    const double th = ib * a.zen_max / (a.n_zen - 1);
+    const float nanv = __int_as_float(0x7FC00000);
+    float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (h_e > atm.h_obs) {
+        const double c = (double)k / (a.n_c - 1);
+        double psi = acos(sqrt(c));
+        psi = fmin(fmax(psi, 1e-3), 0.5 * 3.14159265358979323846 - 1e-3);
+        const double sz = sin(th), cz = cos(th), cps = cos(psi), sps = sin(psi);
+        const double ux = sz * cps, uy = sz * sps, up = sqrt(ux * ux + cz * cz);
+        const double sin_par = ux / up, cos_par = cz / up;             // zenith angle of the in-plane motion
+        const double n_e = 1.0 + eta_lookup_d(atm, h_e);
+        const double kappa = n_e * uy;
+        const double K = n_e * up * (atm.R + h_e) * sin_par;           // n_eff r sin(theta_par)
+        const double h_g = atm.h_obs, step = (double)atm.dh / a.substeps;
+        double h_cur = h_e, psi_c = 0.0, S = 0.0, cT = 0.0, X = 0.0, yax = 0.0;
+        bool ground = true;
+        auto xv_at = [&](double h) {
+            double f = (h - (double)atm.h0) / (double)atm.dh;
+            f = fmin(fmax(f, 0.0), (double)(atm.n_nodes - 1));
+            const int kk = min((int)f, atm.n_nodes - 2);
+            const double fr = f - kk;
+            return (1.0 - fr) * (double)__ldg(atm.xv + kk) + fr * (double)__ldg(atm.xv + kk + 1);
+        };
+        double xv_cur = xv_at(h_cur);
+        while (h_cur > h_g) {
+            const double g = floor((h_cur - (double)atm.h0) / step);
+            double h_next = (double)atm.h0 + g * step;
+            if (!(h_next < h_cur - 1e-9 * step)) h_next = (double)atm.h0 + (g - 1.0) * step;
+            if (h_next < h_g) h_next = h_g;
+            const double n_l = 1.0 + eta_lookup_d(atm, 0.5 * (h_cur + h_next));
+            const double ne2 = n_l * n_l - kappa * kappa;
+            if (!(ne2 > 0.0)) { ground = false; break; }
+            const double n_eff = sqrt(ne2), p = K / n_eff;
+            const double rt = atm.R + h_cur, rb = atm.R + h_next, dhl = h_cur - h_next;
+            if (!(rb > fabs(p))) { ground = false; break; }
+            const double at = sqrt(rt * rt - p * p), ab = sqrt(rb * rb - p * p);
+            const double s_par = dhl * (rt + rb) / (at + ab);
+            const double x = p * s_par / (rt * rb);
+            psi_c += x * (1.0 + x * x * (1.0 / 6.0 + x * x * (3.0 / 40.0)));
+            const double s = s_par * n_l / n_eff;
+            yax += kappa / n_eff * s_par;
+            S += s; cT += n_l * s;
+            const double xv_next = xv_at(h_next);
+            X += (xv_next - xv_cur) * (s / dhl);
+            xv_cur = xv_next;
+            h_cur = h_next;
+        }
+        const double Rg = atm.Rg, re = atm.R + h_e, pp = re * sin_par;
+        if (ground && fabs(pp) < Rg) {
+            const double chord = re * cos_par - sqrt(Rg * Rg - pp * pp), S_line = chord / up;
+            const double psi_line = asin(pp / Rg) - atan2(sin_par, cos_par);
+            const double dxp = Rg * (psi_c - psi_line), dyp = yax - uy * S_line;
+            out = make_float4((float)(dxp * cps + dyp * sps), (float)((cT - S_line) / kC), (float)X,
+                              (float)((-dxp * sps + dyp * cps) / (sps * cps)));
+        } else {
+            out = make_float4(nanv, nanv, nanv, nanv);
+        }
+    }
+    a.cyl[idx] = out;
+}
+
 template <int EMIT, int TRACE, bool SPH, int SPEC>
 cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
 {
@@ -1851,7 +1978,8 @@ static int array_production_setting(const KArgs &a)
 {
     const DevRun &r = a.run;
     const DevDet &d = a.det;
-    const bool base = r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
+    const bool base = a.atm.model != C8PH_ATM_CYLINDRICAL &&          // the cylindrical model runs the generic variant
+           r.emit == C8PH_EMIT_CHERENKOV && r.trace == C8PH_TRACE_TABLE && r.lv2 && r.trans == C8PH_TRANS_ROULETTE &&
            (a.atm.ray_inv_X > 0.f || a.atm.n_ext > 0) && !(a.atm.aer_L > 0.f) && !d.cam_enabled &&
            ((d.hist_nx > 0 && r.out.hist != nullptr) || d.hist_nx == 0) &&
            d.n_tel > 0 && d.use_grid && !r.hit_brute && r.write == C8PH_WRITE_TEL && r.out.photons != nullptr &&
@@ -1864,7 +1992,7 @@ static int array_production_setting(const KArgs &a)
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 {
     const size_t smem = emit_smem_bytes(a);
-    const bool sph = a.atm.model == C8PH_ATM_SPHERICAL;
+    const bool sph = a.atm.model >= C8PH_ATM_SPHERICAL;
     const int spec = array_production_setting(a);
     if (spec == kSpecBase)
         return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase>(a, n_sm, smem, st)
@@ -1908,6 +2036,7 @@ cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st)
     const int n = a.n_h * a.n_zen;
     k_build_table<<<(n + 127) / 128, 128, 0, st>>>(a);
     if (a.n_rho >= 2 && a.flatE && a.flatO) k_build_table_flat<<<(n + 127) / 128, 128, 0, st>>>(a);
+    if (a.n_c >= 2 && a.cyl) k_build_table_cyl<<<(n * a.n_c + 127) / 128, 128, 0, st>>>(a);
     return cudaGetLastError();
 }
 

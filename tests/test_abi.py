@@ -45,7 +45,7 @@ def test_struct_layouts_match_the_header(tmp_path):
     """sizeof/offsetof from a C compile of the header against the ctypes mirrors."""
     fields = {
         "c8ph_atmosphere_desc": (api.AtmosphereDesc, ["size", "refractivity", "earth_radius_m", "aer_angstrom", "n_ext_lambda", "ext_tau_v"]),
-        "c8ph_table_desc": (api.TableDesc, ["size", "h_max_m", "substeps", "n_rho", "rho_max_m"]),
+        "c8ph_table_desc": (api.TableDesc, ["size", "h_max_m", "substeps", "n_rho", "rho_max_m", "n_c"]),
         "c8ph_detector": (api.Detector, ["size", "tel_xyzr", "cam_enabled", "t_ref_ns", "t_bin_ns", "opt_enabled", "opt_camera_radius_m", "opt_kind", "opt_lens_index", "opt_n_abs", "opt_abs"]),
         "c8ph_params": (api.Params, ["size", "write", "bunch_weight", "aim_factor", "disp_lambda0_nm", "use_efficiency", "flat_plane"]),
         "c8ph_segments": (api.Segments, ["size", "x", "edep", "id"]),

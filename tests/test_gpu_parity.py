@@ -860,6 +860,45 @@ def test_flat_plane_table_nodes_and_photons_against_the_oracle(monkeypatch):
     assert e.value.code == api.E_STATE
 
 
+def test_cylindrical_atmosphere_model_nodes_and_photons_against_the_oracle():
+    """Row f1 (thesis sec. 3.3.3; R24): the cylindrical model.  The device builds its table by Bouguer's
+    invariant in the plane of curvature with the effective index sqrt(n^2 - kappa^2); the oracle by stepping Eq. 3.15 in
+    three dimensions: node by node 0.1 mm / 0.3 ps (also the displacement across the flight, which the spherical model
+    does not have).  Photons: cfg4's array 8 km from the origin, tracks inclined by 50 degrees at every azimuth (so every
+    angle against the plane of curvature), device against oracle; and against the spherical model the same photons
+    differ by millimetres to centimetres, as the thesis says of instrumented areas of this size."""
+    tab = dict(n_h=192, n_zen=192, h_max=40000.0, zen_max_deg=75.0, n_c=5)
+    cfg = _off_centre(4, 1500, 8000.0, 50.0)
+    cfg["atmosphere"]["model"] = "cylindrical"
+    cfg["table"] = dict(tab)
+    ctx = api.setup_context(cfg)
+    got = ctx.get_trace_table_cyl()
+    want = O.table_cyl_for(cfg)
+    assert got.shape == (5, 192, 192, 4) and want.shape == (5, 192, 192, 5)
+    zen = np.linspace(0.0, 75.0, 192)
+    for cg, cw, tol in ((0, 0, 1e-4), (1, 2, 3e-4), (2, 3, 1e-2), (3, 1, 2e-4)):
+        g, w = got[..., cg].astype(np.float64), want[..., cw].astype(np.float64)
+        ok = np.isfinite(g) & np.isfinite(w) & (zen[None, None, :] <= 70.0)
+        assert ok.mean() > 0.85 and np.abs(g - w)[ok].max() <= tol, (cg, np.abs(g - w)[ok].max())
+    assert np.abs(got[2, 100, 150, 3]) > 1e-3                          # the across displacement is there (millimetres)
+    ora, gpu, rep = _both(cfg, ctx=ctx)
+    assert gpu["counters"]["tel_hit"] > 1e4 and gpu["counters"]["in_grid"] > 1e5 and rep["max_dpos_m"] < 5e-3
+    sph = copy.deepcopy(cfg)
+    sph["atmosphere"]["model"] = "spherical"
+    sph["table"] = {k: v for k, v in tab.items() if k != "n_c"}
+    so = O.run(sph)
+    a, b = ora["photons"], so["photons"]
+    both = (a["status"] == O.ST_LANDED) & (b["status"] == O.ST_LANDED)
+    d = np.hypot(a["x"][both] - b["x"][both], a["y"][both] - b["y"][both])
+    assert both.sum() > 1e5 and 1e-3 < d.max() < 0.2 and np.median(d) > 1e-4
+    # state errors: the model needs its table, and has no numeric tracing, aerosol or fluorescence
+    bad = copy.deepcopy(cfg)
+    bad["table"] = {k: v for k, v in tab.items() if k != "n_c"}
+    with pytest.raises(api.C8phError) as e:
+        api.run_config(bad)
+    assert e.value.code == api.E_STATE
+
+
 def test_compiled_feature_variants_and_the_generic_kernel_agree(monkeypatch):
     """The "production setting + optional features" calls run kernel variants with the features compiled in (SPEC bit
     mask); C8PH_FORCE_GENERIC=1 sends the same call through the generic variant that reads every switch at run time.
