@@ -602,14 +602,25 @@ __device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float u
 
 // a9 for a segment without a valid axis anchor (P_z >= -0.05: near-horizontal or up-going particle):
 // plain Eq. 3.3 from the emission point.  Rare; kept out of line so the common path does not pay.
+#ifndef C8PH_LINE_BY_VALUE
+#define C8PH_LINE_BY_VALUE 1    // 1: the out-of-line general straight line returns its point in registers (no local-memory out-parameters)
+#endif
+#if C8PH_LINE_BY_VALUE
+__device__ __noinline__ float2 line_general(const SegCold *sc, float s, float D, float Px, float Py, float ux, float uy)
+{
+    return make_float2(fmaf(D, ux, fmaf(s, Px, sc->Ax)), fmaf(D, uy, fmaf(s, Py, sc->Ay)));
+}
+#else
 __device__ __noinline__ void line_general(const SegCold *sc, float s, float D, float Px, float Py, float ux, float uy,
                                           float &ox, float &oy)
 {
     ox = fmaf(D, ux, fmaf(s, Px, sc->Ax));
     oy = fmaf(D, uy, fmaf(s, Py, sc->Ay));
 }
+#endif
 
-// per-warp event counters kept in shared memory (u64), flushed to the global counters at the end
+// event counters of the CTA kept in shared memory (u64, shared-memory atomics once per segment group / counter flush),
+// flushed to the global counters at the end
 enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_NONFINITE, WC_EMITTED, WC_UP, WC_LV2, WC_TR, WC_ROUL, WC_GRID, WC_TEL,
        WC_CAM, WC_WRITTEN, WC_OVERFLOW, WC_N };
 
@@ -627,7 +638,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     constexpr int kWarps = kernel_threads(TRACE) / 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
-    __shared__ unsigned long long s_cnt[kWarps][WC_N];
+    __shared__ unsigned long long s_cnt[WC_N];               // event counters of the CTA (shared-memory atomics, rare)
 
     const HotConst &hc = a.hc;
     const DevAtm &atm = a.atm;
@@ -652,7 +663,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
     SegSlot *g_slot = static_cast<SegSlot *>(run.slots) + ((size_t)blockIdx.x * kWarps + warp) * 32;
 
-    if (lane < WC_N) s_cnt[warp][lane] = 0ull;
+    if (threadIdx.x < WC_N) s_cnt[threadIdx.x] = 0ull;
+    __syncthreads();
 #if !C8PH_QUEUE_CONVERGED
     if (lane == 0) s_qn[warp] = 0;
 #endif
@@ -683,8 +695,8 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         const uint32_t v2 = __reduce_add_sync(FULL, pkB & 0xFFFFu), v3 = __reduce_add_sync(FULL, pkB >> 16);
         const uint32_t v4 = __reduce_add_sync(FULL, pkC & 0xFFFFu), v5 = __reduce_add_sync(FULL, pkC >> 16);
         if (lane == 0) {
-            s_cnt[warp][WC_UP] += v0; s_cnt[warp][WC_LV2] += v1; s_cnt[warp][WC_TR] += v2;
-            s_cnt[warp][WC_ROUL] += v3; s_cnt[warp][WC_GRID] += v4; s_cnt[warp][WC_TEL] += v5;
+            auto bump = [&](int idx, uint32_t v) { if (v) atomicAdd(&s_cnt[idx], (unsigned long long)v); };
+            bump(WC_UP, v0); bump(WC_LV2, v1); bump(WC_TR, v2); bump(WC_ROUL, v3); bump(WC_GRID, v4); bump(WC_TEL, v5);
         }
         pkA = pkB = pkC = 0;
         iters_pending = 0;
@@ -830,7 +842,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                                     const float3 P3 = make_float3(fmaf(s3, v2x, P2.x), fmaf(s3, v2y, P2.y), -hf);
                                     if (!leg_absorbed(det, P2, P3) && P3.x * P3.x + P3.y * P3.y <= det.opt_rc2) {
                                         opt_hit = true;
-                                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                                        atomicAdd(&s_cnt[WC_CAM], 1ull);
                                         rx_out = P3.x; ry_out = P3.y; uax = v2x; uay = v2y;
                                         t_arr = fmaf(s1 + nl * s2 + s3, kInvC, t_arr);
                                     }
@@ -873,7 +885,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                                     }
                                     if (!absorbed && xc * xc + yc * yc <= det.opt_rc2) {
                                         opt_hit = true;
-                                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                                        atomicAdd(&s_cnt[WC_CAM], 1ull);
                                         rx_out = xc; ry_out = yc; uax = r0; uay = r1;
                                         t_arr = fmaf(sh + s2c, kInvC, t_arr);
                                     }
@@ -886,7 +898,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const int pix = camera_pixel(det, uax, uay, uaz);
                     const float tb = floorf(t_arr * det.inv_t_bin);
                     if (pix >= 0 && tb >= 0.f && tb < (float)det.n_tbins) {
-                        atomicAdd(&s_cnt[warp][WC_CAM], 1ull);
+                        atomicAdd(&s_cnt[WC_CAM], 1ull);
                         if (run.out.hist) atomicAdd(run.out.hist + (size_t)pix * det.n_tbins + (int)tb, wgt);
                     }
                 }
@@ -911,7 +923,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                                                    ((jslot >> 5) << 14) | (tel >= 0 ? (uint32_t)tel : C8PH_TEL_NONE)));
                         if (run.out.photon_weight) __stcs(run.out.photon_weight + idx, wgt);
                     } else {
-                        atomicAdd(&s_cnt[warp][WC_OVERFLOW], 1ull);
+                        atomicAdd(&s_cnt[WC_OVERFLOW], 1ull);
                     }
                 }
             }
@@ -1160,10 +1172,9 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             const unsigned me_ = __ballot_sync(FULL, myN > 0), mnf = __ballot_sync(FULL, nonfinite);
             const uint32_t nsum = __reduce_add_sync(FULL, (uint32_t)myN);
             if (lane == 0) {
-                s_cnt[warp][WC_BELOW] += __popc(mb); s_cnt[warp][WC_LV1] += __popc(ml);
-                s_cnt[warp][WC_CLIPPED] += __popc(mcl); s_cnt[warp][WC_EMITTING] += __popc(me_);
-                s_cnt[warp][WC_NONFINITE] += __popc(mnf);
-                s_cnt[warp][WC_EMITTED] += nsum;
+                auto bump = [&](int idx, unsigned v) { if (v) atomicAdd(&s_cnt[idx], (unsigned long long)v); };
+                bump(WC_BELOW, __popc(mb)); bump(WC_LV1, __popc(ml)); bump(WC_CLIPPED, __popc(mcl));
+                bump(WC_EMITTING, __popc(me_)); bump(WC_NONFINITE, __popc(mnf)); bump(WC_EMITTED, nsum);
             }
         }
         unsigned emask = __ballot_sync(FULL, myN > 0);
@@ -1297,7 +1308,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                         oy = zq * (wy * sg.Pz - sg.Py * wz);
                     } else {
                         if (!(Z > 0.f)) { pkA += 1u; break; }           // emitted at or below the observation level (R7: t* > 0)
+#if C8PH_LINE_BY_VALUE
+                        const float2 o2 = line_general(sc, s, D, sg.Px, sg.Py, ux, uy);
+                        ox = o2.x; oy = o2.y;
+#else
                         line_general(sc, s, D, sg.Px, sg.Py, ux, uy, ox, oy);
+#endif
                     }
                     const float xl = sg.Gx + ox, yl = sg.Gy + oy;
                     // a10: LV2/LV3 on the straight-line point, before the correction: keep iff
@@ -1594,13 +1610,13 @@ k_emit_propagate(const __grid_constant__ KArgs a)
         drain(true);                                                  // slots are rewritten by the next group
     }
     flush_counts();
-    __syncwarp();
+    __syncthreads();
 
-    // ---- counters: one global atomic per warp and non-zero counter
-    if (run.out.counters && lane == 0) {
-        const unsigned long long *c = s_cnt[warp];
+    // ---- counters: one global atomic per CTA and non-zero counter
+    if (run.out.counters && threadIdx.x == 0) {
+        const unsigned long long *c = s_cnt;
         auto add = [&](int idx, unsigned long long v) { if (v) atomicAdd(&cntp[idx], v); };
-        if (blockIdx.x == 0 && warp == 0) add(C8PH_CNT_SEGMENTS, (unsigned long long)run.n_seg);
+        if (blockIdx.x == 0) add(C8PH_CNT_SEGMENTS, (unsigned long long)run.n_seg);
         add(C8PH_CNT_SEG_BELOW_THRESHOLD, c[WC_BELOW]);
         add(C8PH_CNT_SEG_LV1, c[WC_LV1]);
         add(C8PH_CNT_SEG_EMITTING, c[WC_EMITTING]);
