@@ -24,6 +24,11 @@ struct DevAtm {
     float aer_L, aer_H, aer_lambda, aer_angstrom;
     const float *aexp;      // DEVICE [n_pad] aerosol column A(h_k) = (H/L) exp(-h_k/H) at the nodes (zeros without aerosol)
     float aer_HL, aer_invH, aer_Ag;   // H/L, 1/H, A(h_obs)
+    // planar layered sum in closed form: mom[q * n_pad + k] = sum over the layers between the observation level and
+    // node k of thickness * nu_l^(q+1) (q = 0..3) and of dX_v * n_l * nu_l^(q-4) (q = 4..7), nu_l = n_l^2 - 1 at the
+    // layer's mid height (c8ph_init_atmosphere)
+    const float *mom;
+    float nu_span;                    // max nu - min nu over the table: bounds the expansion parameter
     int n_ext;              // tabulated extinction: wavelength nodes (0: off)
     float ext_l0, ext_inv_dl;
     const float *ext;       // DEVICE [n_ext][n_nodes] vertical optical depth obs level -> node

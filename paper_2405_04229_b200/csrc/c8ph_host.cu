@@ -25,7 +25,7 @@ struct c8ph_ctx {
     bool force_brute = false;          // C8PH_FORCE_BRUTE=1: search all telescopes (validation of the grids)
     bool force_generic = false;        // C8PH_FORCE_GENERIC=1: never pick the production-setting kernel variant
     double eta_span = 0.0;             // max |n(h) - n(h_obs)| over the table
-    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr, *d_aexp = nullptr;
+    float *d_eta = nullptr, *d_xv = nullptr, *d_dxv = nullptr, *d_ext = nullptr, *d_aexp = nullptr, *d_mom = nullptr;
     // table
     bool have_table = false;
     DevTable tab{};
@@ -132,7 +132,7 @@ extern "C" int c8ph_destroy(c8ph_ctx *ctx)
 {
     if (!ctx) return C8PH_E_ARG;
     cudaSetDevice(ctx->device);
-    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp);
+    dfree(ctx->d_eta); dfree(ctx->d_xv); dfree(ctx->d_dxv); dfree(ctx->d_ext); dfree(ctx->d_aexp); dfree(ctx->d_mom);
     dfree(ctx->d_full); dfree(ctx->d_hot); dfree(ctx->d_tel); dfree(ctx->d_flat); dfree(ctx->d_cyl);
     if (ctx->tab_tex) cudaDestroyTextureObject(ctx->tab_tex);
     if (ctx->tab_arr) cudaFreeArray(ctx->tab_arr);
@@ -228,6 +228,37 @@ extern "C" int c8ph_init_atmosphere(c8ph_ctx *ctx, const c8ph_atmosphere_desc *d
         a.aexp = ctx->d_aexp;
     }
     a.xv_g = (float)lerp_table(xv, h0, dh, d->h_obs_m);
+    {
+        // The planar layered sum in closed form ("layered sum"): with nu_l = n_l^2 - 1 at the layer's
+        // mid height, every term of the sum is a power series in (nu_l - nu_e) / (n_e cos z)^2, so the photon needs only
+        // the sums of thickness * nu_l^p (p = 1..4) and of dX_v * n_l * nu_l^p (p = 0..3) over the layers between the
+        // observation level and its emission cell.  mom[q][k] holds them for the layers from the observation level up to
+        // node k, the same layers, mid-height values and float inputs the per-layer loop uses, accumulated in fp64.
+        const float fgf = std::fmin(std::fmax(((float)a.h_obs - a.h0) * a.inv_dh, 0.f), (float)(n - 1));
+        const int kg = std::min((int)fgf, n - 2);
+        const double frg = (double)(fgf - (float)kg);
+        std::vector<float> mom(8 * (size_t)n_pad, 0.f);
+        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        double nu_lo = 1e300, nu_hi = -1e300;
+        for (int k = 0; k < n; ++k) { const double v = (double)eta[k] * (2.0 + (double)eta[k]); nu_lo = std::min(nu_lo, v); nu_hi = std::max(nu_hi, v); }
+        auto add_layer = [&](double eta_l, double thick, double dxv_l) {
+            const double nl = 1.0 + eta_l, nu = eta_l * (2.0 + eta_l);
+            double pw = nu;
+            for (int q = 0; q < 4; ++q) { acc[q] += thick * pw; pw *= nu; }
+            pw = 1.0;
+            for (int q = 4; q < 8; ++q) { acc[q] += dxv_l * nl * pw; pw *= nu; }
+        };
+        for (int k = kg + 1; k < n; ++k) {
+            if (k == kg + 1) add_layer((double)eta[kg] + 0.5 * (1.0 + frg) * ((double)eta[kg + 1] - (double)eta[kg]), (1.0 - frg) * (double)a.dh, (1.0 - frg) * (double)dxv[kg]);
+            else add_layer(0.5 * ((double)eta[k - 1] + (double)eta[k]), (double)a.dh, (double)dxv[k - 1]);
+            for (int q = 0; q < 8; ++q) mom[(size_t)q * n_pad + k] = (float)acc[q];
+        }
+        dfree(ctx->d_mom);
+        CU(cudaMalloc(&ctx->d_mom, mom.size() * sizeof(float)));
+        CU(cudaMemcpy(ctx->d_mom, mom.data(), mom.size() * sizeof(float), cudaMemcpyHostToDevice));
+        a.mom = ctx->d_mom;
+        a.nu_span = (float)(nu_hi - nu_lo);
+    }
     a.n_ext = 0; a.ext = nullptr; a.ext_l0 = 0.f; a.ext_inv_dl = 0.f;
     dfree(ctx->d_ext);
     if (d->n_ext_lambda > 0) {

@@ -600,6 +600,14 @@ __device__ __forceinline__ int camera_pixel(const DevDet &det, float ux, float u
     return best;
 }
 
+// 1: the planar layered Snell sum (TRACE_NUMERIC) in closed form from per-node layer moments where its series
+//    converges to fp32 accuracy (no aerosol, nu_span / (n_e cos z)^2 < kLayerSeriesMax), the per-layer loop elsewhere;
+//    0: always the loop
+#ifndef C8PH_LAYER_MOMENTS
+#define C8PH_LAYER_MOMENTS 1
+#endif
+constexpr float kLayerSeriesMax = 0.02f;
+
 // a9 for a segment without a valid axis anchor (P_z >= -0.05: near-horizontal or up-going particle):
 // plain Eq. 3.3 from the emission point.  Rare; kept out of line so the common path does not pay.
 #ifndef C8PH_LINE_BY_VALUE
@@ -1431,6 +1439,40 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                                 layer(aer, fmaf(0.5f * (1.f + frg), s_eta[kg + 1] - s_eta[kg], s_eta[kg]), (1.f - frg) * atm.dh, (1.f - frg) * s_dxv[kg], Ag - A(kg + 1));
                             }
                         };
+                        const float re2 = r_e * r_e;
+                        if (C8PH_LAYER_MOMENTS && !aer_staged && ke > kg && ok && atm.nu_span * re2 < kLayerSeriesMax) {
+                            // The same sum in closed form.  With nu = n^2 - 1: n_l^2 - K^2 = (1 + x_l) / r_e^2,
+                            // x_l = (nu_l - nu_e) r_e^2, so r_l = r_e (1 + x_l)^(-1/2) and every term of the three sums
+                            // is a power series in x_l (|x_l| < 0.02 here: the p = 5 term is below 1e-9 of the first).
+                            // sum thickness x_l^p follows from the binomial expansion of (nu_l - nu_e)^p and the layer
+                            // moments mom[] (c8ph_init_atmosphere) up to the node below the emission cell, plus the
+                            // partial layer of the emission cell itself.
+                            const float eta_p = fmaf(0.5f * fre, s_eta[ke + 1] - s_eta[ke], s_eta[ke]);
+                            const float nu_p = eta_p * (2.f + eta_p), th_p = fre * atm.dh, g_p = fre * s_dxv[ke] * (1.f + eta_p);
+                            const float *mk = atm.mom + ke;
+                            const int np = atm.n_pad;
+                            const float nu_p2 = nu_p * nu_p;
+                            const float M1 = fmaf(th_p, nu_p, __ldg(mk)), M2 = fmaf(th_p, nu_p2, __ldg(mk + np));
+                            const float M3 = fmaf(th_p * nu_p, nu_p2, __ldg(mk + 2 * np)), M4 = fmaf(th_p * nu_p2, nu_p2, __ldg(mk + 3 * np));
+                            const float G0 = __ldg(mk + 4 * np) + g_p, G1 = fmaf(g_p, nu_p, __ldg(mk + 5 * np)), G2 = fmaf(g_p, nu_p2, __ldg(mk + 6 * np));
+                            const float G3 = fmaf(g_p * nu_p, nu_p2, __ldg(mk + 7 * np));
+                            const float Hh = (fe - fg) * atm.dh;                     // sum of the layer thicknesses
+                            const float d = -eta_e * (2.f + eta_e);                  // -nu_e
+                            // S_p = sum thickness x_l^p
+                            const float S1 = re2 * fmaf(d, Hh, M1);
+                            const float S2 = re2 * re2 * fmaf(d, fmaf(d, Hh, 2.f * M1), M2);
+                            const float S3 = re2 * re2 * re2 * fmaf(d, fmaf(d, fmaf(d, Hh, 3.f * M1), 3.f * M2), M3);
+                            const float S4 = (re2 * re2) * (re2 * re2) * fmaf(d, fmaf(d, fmaf(d, fmaf(d, Hh, 4.f * M1), 6.f * M2), 4.f * M3), M4);
+                            const float Am = fmaf(0.2734375f, S4, fmaf(-0.3125f, S3, fmaf(0.375f, S2, -0.5f * S1)));       // sum thickness ((1+x)^(-1/2) - 1)
+                            const float Ap = fmaf(-0.0390625f, S4, fmaf(0.0625f, S3, fmaf(-0.125f, S2, 0.5f * S1)));      // sum thickness ((1+x)^(+1/2) - 1)
+                            aX = K * r_e * Am;
+                            // sum thickness (n_l^2 r_l - n_e r_e), n_l^2 r_l = (1+x)^(1/2) / r_e + K^2 r_e (1+x)^(-1/2)
+                            aT = fmaf(Hh * r_e * n_e, eta_e, fmaf(Ap, n_e * cz, K * K * r_e * Am));
+                            // sum dX_v n_l r_l
+                            const float T1 = re2 * fmaf(d, G0, G1), T2 = re2 * re2 * fmaf(d, fmaf(d, G0, 2.f * G1), G2);
+                            const float T3 = re2 * re2 * re2 * fmaf(d, fmaf(d, fmaf(d, G0, 3.f * G1), 3.f * G2), G3);
+                            aS = r_e * fmaf(-0.3125f, T3, fmaf(0.375f, T2, fmaf(-0.5f, T1, G0)));
+                        } else
                         if (aer_staged) walk(std::true_type{}); else walk(std::false_type{});
                         if (!ok) { pkB += 1u; break; }
                         dd = aX; dt = aT * kInvC; Xs = aS; ta = aA;

@@ -49,6 +49,28 @@ def test_cfg1_planar_numeric_weight():
     assert abs(rep["hist_total"][0] - rep["hist_total"][1]) / rep["hist_total"][0] < 1e-5
 
 
+@pytest.mark.parametrize("zenith_deg", [0.0, 40.0, 64.0, 72.0])
+def test_planar_layered_sum_inclined(zenith_deg):
+    """Eq. 3.15 per photon at inclined incidence, photon by photon against the oracle's layer loop.  The device sums the
+    layers in closed form (layer moments) where (nu_max - nu_min) / (n_e cos z)^2 < 0.02 and layer by
+    layer beyond.  With six times the refractivity of air (so that the switch sits at 65 degrees, where the landing
+    point is still well conditioned in fp32) 0 / 40 degrees are all closed form, 64 mixes the two inside one warp
+    (Cherenkov cone, segment tilts of 2 degrees), 72 is all loop."""
+    cfg = W.make_config(1, n_segments=600)
+    atm = cfg["atmosphere"]
+    atm["refractivity"] = (6.0 * atm["refractivity"].astype(np.float64)).astype(np.float32)
+    rng = np.random.default_rng(11)
+    cfg["segments"] = W._shower_segments(rng, 600, atm, zenith_deg, 25.0, 330.0, 70.0, 80.0, 2.0, 5.0, 5.0, 2.0, 5.0)
+    W._grid(cfg["detector"], 400, 2.5 / math.cos(math.radians(zenith_deg)) ** 2)
+    # clock zero = the shower front at the core (arrival times of ~1e6 ns have an fp32 spacing of 0.125 ns in the record)
+    s = cfg["segments"]
+    front = s["t0"].astype(np.float64) + (s["z"].astype(np.float64) - atm["h_obs"]) / math.cos(math.radians(zenith_deg)) / 0.299792458
+    s["t0"] = (s["t0"].astype(np.float64) - np.median(front)).astype(np.float32)
+    ora, gpu, rep = _both(cfg)
+    assert gpu["counters"]["landed"] > 1e4
+    assert abs(rep["hist_total"][0] - rep["hist_total"][1]) / rep["hist_total"][0] < 1e-5
+
+
 def test_cfg2_spherical_table_filters_roulette():
     cfg = W.make_config(2, n_segments=20000)
     ora, gpu, rep = _both(cfg)
