@@ -168,7 +168,7 @@ constexpr int kFillThreads = 128;
 enum { TF_AX, TF_AY, TF_AZ, TF_VX, TF_VY, TF_VZ, TF_R1X, TF_R1Y, TF_R1Z, TF_R2X, TF_R2Y, TF_R2Z, TF_UX, TF_UY, TF_UZ,
        TF_HK, TF_D, TF_SD, TF_CD, TF_Q, TF_T0, TF_IBC, TF_N };
 
-__global__ void __launch_bounds__(kFillThreads) k_substep_fill(const __grid_constant__ SubstepArgs a)
+__global__ void __launch_bounds__(kFillThreads, 6) k_substep_fill(const __grid_constant__ SubstepArgs a)
 {
     __shared__ double s_trk[kFillThreads / 32][TF_N][32];
     __shared__ float s_trkf[kFillThreads / 32][3][32];                 // chord length, beta, charge
@@ -255,12 +255,17 @@ __global__ void __launch_bounds__(kFillThreads) k_substep_fill(const __grid_cons
 // multiplies theta_0, so a piece's direction moves by < 1e-8 rad; stiffer kicks (0.35 rad for a 10 MeV electron over
 // 25 m of air at sea level) take the fp64 functions.  theta_0 itself is fp32 arithmetic on fp64-derived inputs.
 //
-// The lanes of a warp walk in lock step, so a warp costs its longest track: a CTA takes 1024 consecutive tracks,
+// The lanes of a warp walk in lock step, so a warp costs its longest track: a CTA takes 512 consecutive tracks,
 // orders them by piece count in shared memory (counting sort, 63 and more pieces in one class; the order inside a
 // class is arbitrary and does not matter: every piece has its own place in the output) and hands each warp 32 tracks
-// that are neighbours in that order.  Measured on 1e7 tracks with a log-uniform momentum spectrum: 11.6 -> 21.5 active
-// lanes per warp instruction.
-constexpr int kMsThreads = 128, kMsChunk = 1024, kMsBins = 64;
+// that are neighbours in that order.  Measured on 1e7 tracks with a log-uniform momentum spectrum: 11.6 -> 20.4 active
+// lanes per warp instruction.  The chunk size trades balance against the output footprint in flight: a track's run is
+// ~40 B per array, so most 32-byte sectors are completed by a neighbouring track that another warp walks later, and
+// sectors evicted from L2 half written cost a DRAM read-modify-write (chunks of 256 / 512 / 1024 tracks: 11.1 / 14.3 /
+// 18.7 GB of DRAM traffic for 4.7 GB of input + output, 7.7 / 6.9 / 8.0 ms; staging a 256-track chunk's whole output
+// in shared memory and writing it as one range brings the traffic to 5.0 GB but costs a CTA-wide barrier per chunk
+// behind its longest track: 10.9 ms).
+constexpr int kMsThreads = 128, kMsChunk = 512, kMsBins = 64;
 
 // the whole warp calls this; lanes without a track pass valid = false.  Pieces are staged in the warp's shared-memory
 // tile (10 fields x 32 tracks x 8 pieces, row pitch 9 floats: conflict-free for lane = track and for the flush) and
