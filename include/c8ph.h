@@ -307,6 +307,24 @@ int c8ph_substep_fill(c8ph_ctx *ctx, const c8ph_segments *tracks, const float *p
                       const c8ph_substep_desc *desc, const int64_t *offsets,
                       const c8ph_segments_out *out, void *stream);
 
+/* ---- allocation-free planning (for callers that cannot call cudaMalloc: CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  Same operation, arguments and result as c8ph_substep_plan (the piece count
+ * needs no atmosphere), but without a context (c8ph_create allocates) and for at most
+ * C8PH_SUBSTEP_STATIC_MAX_TRACKS tracks per call: the scan scratch is a static device array of that size / 1024 x 8 B
+ * = 32 KB inside the library, held by every GPU that loads it until the process exits.  The call runs on the CURRENT
+ * device, asynchronously on `stream`, and calls no cudaMalloc / cudaFree or allocating library routine (its first
+ * call on a device resolves the array's address with cudaGetSymbolAddress: make that call outside a capture).
+ * All calls on a device share the scratch and it keeps the last call's contents (every element a call reads it has
+ * written before): calls that overlap on the GPU - different streams without ordering - race; order them.
+ * tracks / p_GeV / offsets / desc->clipped: DEVICE pointers of the current device, caller-owned.
+ * Errors: C8PH_E_ARG for NULL / inconsistent arguments and for n_tracks > C8PH_SUBSTEP_STATIC_MAX_TRACKS (nothing
+ * is launched; split the call or use c8ph_substep_plan), C8PH_E_CUDA for a failed runtime call; the text is in
+ * c8ph_substep_plan_static_error() (per host thread).                                                      */
+#define C8PH_SUBSTEP_STATIC_MAX_TRACKS 4194304
+int c8ph_substep_plan_static(const c8ph_segments *tracks, const float *p_GeV, int64_t n_tracks,
+                             const c8ph_substep_desc *desc, int64_t *offsets, void *stream);
+const char *c8ph_substep_plan_static_error(void);
+
 /* Device time of the last c8ph_emit_propagate kernel of this context in ms (CUDA events on the
  * launch stream; synchronises on the end event).  Returns < 0 if nothing was launched.          */
 float c8ph_last_kernel_ms(c8ph_ctx *ctx);

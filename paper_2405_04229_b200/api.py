@@ -34,7 +34,8 @@ EXPORTS = ("c8ph_create", "c8ph_destroy", "c8ph_last_error", "c8ph_version", "c8
            "c8ph_build_trace_table", "c8ph_get_trace_table", "c8ph_set_trace_table", "c8ph_set_detector",
            "c8ph_emit_propagate", "c8ph_emit_propagate_host", "c8ph_last_kernel_ms", "c8ph_launch_count",
            "c8ph_counter_name", "c8ph_substep_plan", "c8ph_substep_fill", "c8ph_set_line_spectrum", "c8ph_set_efficiency",
-           "c8ph_get_trace_table_flat", "c8ph_get_trace_table_cyl")
+           "c8ph_get_trace_table_flat", "c8ph_get_trace_table_cyl", "c8ph_substep_plan_static", "c8ph_substep_plan_static_error")
+SUBSTEP_STATIC_MAX_TRACKS = 4194304      # C8PH_SUBSTEP_STATIC_MAX_TRACKS
 
 PHOTON_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("ux", "<f4"), ("uy", "<f4"), ("t_ns", "<f4"),
                          ("lambda_nm", "<f4"), ("seg", "<u4"), ("j_tel", "<u4")])
@@ -140,6 +141,8 @@ def load_library():
                                         C.c_void_p, C.c_void_p]
         L.c8ph_substep_fill.argtypes = [C.c_void_p, C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(SubstepDesc),
                                         C.c_void_p, C.POINTER(SegmentsOut), C.c_void_p]
+        L.c8ph_substep_plan_static.argtypes = [C.POINTER(Segments), C.c_void_p, C.c_int64, C.POINTER(SubstepDesc), C.c_void_p, C.c_void_p]
+        L.c8ph_substep_plan_static_error.restype = C.c_char_p
         L.c8ph_set_line_spectrum.argtypes = [C.c_void_p, C.c_int32, _fp, _fp]
         L.c8ph_set_efficiency.argtypes = [C.c_void_p, C.c_int32, C.c_float, C.c_float, _fp]
         L.c8ph_counter_name.argtypes = [C.c_int]
@@ -481,6 +484,33 @@ def _dev_ptr(t, dtype, min_elems):
         assert str(t.dtype) == "torch." + dtype, (t.dtype, dtype)
         assert t.numel() >= min_elems, (t.numel(), min_elems)
     return t.data_ptr()
+
+
+def substep_plan_static(trk_dev: dict, n_tracks: int, B_tesla, tol_m: float, offsets, max_sub: int = 4096, stream=None,
+                        ms_max_step_m=None, clipped=None) -> None:
+    """c8ph_substep_plan_static: the piece-count scan without a context and without any allocation (scratch = a
+    static device array inside the library, at most SUBSTEP_STATIC_MAX_TRACKS tracks).  trk_dev as in
+    Context.substep_tracks; offsets: caller's int64[n_tracks + 1] CUDA tensor (written); clipped: optional int64[1]
+    CUDA tensor (incremented).  Runs on the current device and stream; argument marshalling only."""
+    lib = load_library()
+    need = n_tracks if n_tracks <= SUBSTEP_STATIC_MAX_TRACKS else 0     # beyond the limit the library refuses: no size check here
+    t = Segments()
+    t.size = C.sizeof(Segments)
+    for k in SEG_FIELDS:
+        v = trk_dev.get(k)
+        setattr(t, k, _dev_ptr(v, "float32", need) if (v is not None and k != "edep") else None)
+    d = SubstepDesc()
+    d.size = C.sizeof(SubstepDesc)
+    d.B_tesla = (C.c_float * 3)(*[float(b) for b in B_tesla])
+    d.tol_m, d.max_sub = float(tol_m), int(max_sub)
+    d.ms_enabled = 0 if ms_max_step_m is None else 1
+    d.ms_max_step_m = 0.0 if ms_max_step_m is None else float(ms_max_step_m)
+    d.ms_X0_gcm2, d.seed, d.track_id_base = 36.62, 1, 0
+    d.clipped = clipped.data_ptr() if clipped is not None else None
+    rc = lib.c8ph_substep_plan_static(C.byref(t), _dev_ptr(trk_dev.get("p_GeV"), "float32", need), int(n_tracks), C.byref(d),
+                                      _dev_ptr(offsets, "int64", need + 1), _stream_ptr(stream))
+    if rc:
+        raise C8phError(rc, lib.c8ph_substep_plan_static_error().decode())
 
 
 # ---- convenience: run a whole workload dict on the device -----------------------------------------

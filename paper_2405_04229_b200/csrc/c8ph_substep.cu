@@ -4,6 +4,8 @@
 // must reproduce km-scale positions to well below the 15 cm resolution the thesis quotes.
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <cstdio>
+#include <cmath>
 #include "c8ph_device.cuh"
 #include "c8ph_philox.cuh"
 
@@ -482,3 +484,77 @@ cudaError_t launch_substep_fill(const SubstepArgs &a, int n_sm, cudaStream_t st)
 }
 
 }  // namespace c8ph
+
+// ------------------------------------------------------------------------------------------------------------------
+// c8ph_substep_plan_static: the planning step for callers that must not allocate (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  No context (c8ph_create allocates): the scan scratch - one
+// block total per 1024 tracks - is the file-scope device array below, C8PH_SUBSTEP_STATIC_MAX_TRACKS / 1024 x 8 B =
+// 32 KB that every GPU loading the library holds until exit.  In host code `g_static_bsums` is a host-side stand-in,
+// not a device address: the address the kernels get comes from cudaGetSymbolAddress, resolved once per device with
+// that device current.  All calls on a device share the array: two calls that overlap on the GPU (different streams,
+// no ordering) race on it.  Nothing in it has to start at zero: k_substep_count writes every block total a call reads
+// before k_substep_scan_blocks reads it, so the contents the previous call left behind are never seen.
+static __device__ __align__(256) long long g_static_bsums[C8PH_SUBSTEP_STATIC_MAX_TRACKS / 1024];
+static_assert(c8ph::kScanThreads == 1024, "the static scratch is sized for 1024-track scan blocks");
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+long long *g_static_ptr[kStaticMaxDevices];          // device address of g_static_bsums, per device (0: not resolved yet)
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char *msg, cudaError_t e = cudaSuccess)
+{
+    if (e != cudaSuccess) snprintf(g_static_err, sizeof g_static_err, "%s: %s", msg, cudaGetErrorString(e));
+    else snprintf(g_static_err, sizeof g_static_err, "%s", msg);
+    return code;
+}
+}  // namespace
+
+extern "C" const char *c8ph_substep_plan_static_error(void) { return g_static_err; }
+
+extern "C" int c8ph_substep_plan_static(const c8ph_segments *t, const float *p_GeV, int64_t n, const c8ph_substep_desc *d,
+                                        int64_t *offsets, void *stream)
+{
+    if (!t || t->size != sizeof(c8ph_segments) || !d || d->size != sizeof(c8ph_substep_desc))
+        return static_fail(C8PH_E_ARG, "substep_plan_static: NULL struct or size mismatch");
+    if (n < 0) return static_fail(C8PH_E_ARG, "substep_plan_static: n_tracks < 0");
+    if (n > (int64_t)C8PH_SUBSTEP_STATIC_MAX_TRACKS) {
+        snprintf(g_static_err, sizeof g_static_err,
+                 "substep_plan_static: n_tracks = %lld exceeds C8PH_SUBSTEP_STATIC_MAX_TRACKS = %lld (split the call, or use "
+                 "c8ph_substep_plan with a context)", (long long)n, (long long)C8PH_SUBSTEP_STATIC_MAX_TRACKS);
+        return C8PH_E_ARG;
+    }
+    if (!offsets) return static_fail(C8PH_E_ARG, "substep_plan_static: offsets is NULL");
+    if (n > 0 && (!t->x || !t->y || !t->z || !t->dx || !t->dy || !t->dz || !t->len || !t->beta || !t->t0 || !t->charge || !p_GeV))
+        return static_fail(C8PH_E_ARG, "substep_plan_static: NULL track array");
+    if (!(d->tol_m > 0.f) || d->max_sub < 1 || d->max_sub > (1 << 20))
+        return static_fail(C8PH_E_ARG, "substep_plan_static: tol_m > 0 and 1 <= max_sub <= 2^20 required");
+    if (d->ms_enabled && !(d->ms_max_step_m >= 0.f)) return static_fail(C8PH_E_ARG, "substep_plan_static: ms_max_step_m >= 0 required");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if (n == 0) {
+        if ((e = cudaMemsetAsync(offsets, 0, sizeof(int64_t), st)) != cudaSuccess) return static_fail(C8PH_E_CUDA, "substep_plan_static: memset", e);
+        return C8PH_OK;
+    }
+    // set-up, once per device, with that device current: the device address of the scratch array
+    int dev = -1;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return static_fail(C8PH_E_CUDA, "substep_plan_static: cudaGetDevice", e);
+    if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(C8PH_E_ARG, "substep_plan_static: device ordinal out of range");
+    long long *scratch = __atomic_load_n(&g_static_ptr[dev], __ATOMIC_ACQUIRE);
+    if (!scratch) {
+        if ((e = cudaGetSymbolAddress((void **)&scratch, g_static_bsums)) != cudaSuccess || !scratch)
+            return static_fail(C8PH_E_CUDA, "substep_plan_static: cudaGetSymbolAddress", e);
+        __atomic_store_n(&g_static_ptr[dev], scratch, __ATOMIC_RELEASE);      // every thread resolves the same address
+    }
+    c8ph::SubstepArgs a{};
+    a.trk = *t; a.p_GeV = p_GeV; a.n = n;
+    for (int k = 0; k < 3; ++k) a.B[k] = d->B_tesla[k];
+    a.Bn = sqrt(a.B[0] * a.B[0] + a.B[1] * a.B[1] + a.B[2] * a.B[2]);
+    a.tol = d->tol_m; a.max_sub = d->max_sub;
+    a.ms_enabled = d->ms_enabled ? 1 : 0; a.ms_max_step = d->ms_max_step_m; a.ms_X0 = d->ms_X0_gcm2;
+    a.id_base = d->track_id_base;
+    a.clipped = reinterpret_cast<unsigned long long *>(d->clipped);
+    a.offsets = reinterpret_cast<long long *>(offsets);
+    if ((e = c8ph::launch_substep_plan(a, scratch, st)) != cudaSuccess) return static_fail(C8PH_E_CUDA, "substep_plan_static: launch", e);
+    return C8PH_OK;
+}
