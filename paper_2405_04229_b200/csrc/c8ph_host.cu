@@ -472,10 +472,16 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
     }
     cs = std::max(cs, ext / 1536.0);
     if (!(cs > 0.0)) cs = 1.0;
+    // fp32 rounding of (x - x0) * inv_cs on the device: a few ulp of the largest coordinate
+    const double pad = 1e-3 * cs + 8.0 * (coord_max + ext + 8.0 * cs) * 1.2e-7 + 1e-4;
+    if (mode == 0) {
+        // hit grid: a ring of cells no telescope reaches around the footprint, so that the device may CLAMP the cell
+        // coordinates of a point outside the grid instead of testing them (the ring cells are empty: checked below)
+        const double ring = (1.0 + std::ceil(2.0 * pad / cs)) * cs;
+        x0 -= ring; y0 -= ring; x1 += ring; y1 += ring;
+    }
     const int nx = std::max(1, (int)std::ceil((x1 - x0) / cs)), ny = std::max(1, (int)std::ceil((y1 - y0) / cs));
     const size_t ncell = (size_t)nx * ny;
-    // fp32 rounding of (x - x0) * inv_cs on the device: a few ulp of the largest coordinate
-    const double pad = 1e-3 * cs + 8.0 * (coord_max + ext) * 1.2e-7 + 1e-4;
     struct Entry { uint32_t cell; float key; int k; };
     std::vector<Entry> ent;
     std::vector<float> near_d(mode == 1 ? ncell : 0, INFINITY);      // LV2: least dist(cell centre, centre_k) - r_k so far
@@ -519,6 +525,14 @@ static int build_grid(c8ph_ctx *ctx, int which, const std::vector<float> &tel, i
         memcpy(&kb, &ent[i].k, sizeof kb);
         items[i] = make_float2(ent[i].key, kb);
         if (ent[i].key < kmin[ent[i].cell]) kmin[ent[i].cell] = ent[i].key;
+    }
+    if (mode == 0 && n > 0) {
+        bool ring_empty = nx >= 3 && ny >= 3;
+        for (int ix = 0; ix < nx && ring_empty; ++ix)
+            ring_empty = start[(size_t)ix + 1] == start[(size_t)ix] && start[(size_t)(ny - 1) * nx + ix + 1] == start[(size_t)(ny - 1) * nx + ix];
+        for (int iy = 0; iy < ny && ring_empty; ++iy)
+            ring_empty = start[(size_t)iy * nx + 1] == start[(size_t)iy * nx] && start[(size_t)iy * nx + nx] == start[(size_t)iy * nx + nx - 1];
+        if (!ring_empty) return fail(ctx, C8PH_E_STATE, "set_detector: internal error, the border ring of the hit grid is not empty");
     }
     dfree(ctx->d_g_start[which]); dfree(ctx->d_g_items[which]); dfree(ctx->d_g_kmin[which]);
     CU(cudaMalloc(&ctx->d_g_start[which], start.size() * sizeof(int)));

@@ -51,6 +51,12 @@
 #ifndef C8PH_ETA_SEGFIT
 #define C8PH_ETA_SEGFIT 0       // 1: n(h_e) along a segment from a per-segment quadratic in s, fitted in fp64 and checked against the
 #endif                          //    piecewise-linear table (Listing 4.1) to 4e-7 relative; segments that fail it read the table per photon
+#ifndef C8PH_TABLE_EXIT
+#define C8PH_TABLE_EXIT 1       // 1: the table lookup leaves before its loads when (h, zenith) is out of range, instead of clamping the node coordinates
+#endif
+#ifndef C8PH_HIT_RING
+#define C8PH_HIT_RING 1         // 1: a point outside the hit grid is clamped into the grid's ring of empty border cells instead of being tested
+#endif
 #ifndef C8PH_SLOT_PREFETCH
 #define C8PH_SLOT_PREFETCH 1    // 1: the next emitting segment's slot (two 128 B lines) is prefetched into L1 while the current one runs
 #endif
@@ -344,8 +350,15 @@ __device__ __forceinline__ TabVal table_lookup(const DevTable &t, float h, float
         return o;
     }
 #endif
+#if C8PH_TABLE_EXIT
+    // out of range (or NaN): the photon is dropped, nothing is read; inside the range 0 <= h <= h_max and
+    // 0 <= thz <= zen_max bound the node coordinates, so only the top node needs the integer clamp
+    if (o.bad) { o.dd = o.dt = o.X = o.ta = 0.f; return o; }
+    const float f = h * t.inv_dh, g = thz * t.inv_dz;
+#else
     const float f = fminf(fmaxf(h * t.inv_dh, 0.f), t.f_max);
     const float g = fminf(fmaxf(thz * t.inv_dz, 0.f), t.g_max);
+#endif
     const int ia = min((int)f, t.n_h - 2), ib = min((int)g, t.n_zen - 2);
     const float ff = f - (float)ia, gg = g - (float)ib;
     const float4 *p = t.hot + (unsigned)(ia * t.n_zen + ib);
@@ -1556,10 +1569,19 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     if (f_tel) {
                         const bool brute = f_hit_brute || !f_grid || -uz < hc.grid_min_cos;
                         if (f_grid) {
+#if C8PH_HIT_RING
+                            // the grid has a border ring of empty cells (c8ph_set_detector): a point outside it is
+                            // clamped into the ring (negative coordinates wrap to large unsigned values) and finds "empty"
+                            const unsigned gx = min((unsigned)__float2int_rd((xg - hc.hit_x0) * hc.hit_inv_cs), (unsigned)(hc.hit_nx - 1));
+                            const unsigned gy = min((unsigned)__float2int_rd((yg - hc.hit_y0) * hc.hit_inv_cs), (unsigned)(hc.hit_ny - 1));
+                            cell = (int)(gy * (unsigned)hc.hit_nx + gx);
+                            kmin = (float)__ldg(hc.hit_kq + cell);
+#else
                             const int gx = __float2int_rd((xg - hc.hit_x0) * hc.hit_inv_cs), gy = __float2int_rd((yg - hc.hit_y0) * hc.hit_inv_cs);
                             cell = ((unsigned)gx < (unsigned)hc.hit_nx && (unsigned)gy < (unsigned)hc.hit_ny) ? gy * hc.hit_nx + gx : -1;
                             kmin = (float)__ldg(hc.hit_kq + max(cell, 0));  // cell -1 (outside): never a candidate
                             if (cell < 0) kmin = 255.f;
+#endif
                         }
                         if (brute) cell = -2;
                     }
