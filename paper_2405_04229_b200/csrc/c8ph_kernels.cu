@@ -94,7 +94,17 @@ namespace {
 #define C8PH_MIN_BLOCKS 1
 #endif
 constexpr int kMaxWarpsPerSM = 64;                             // hardware limit; the segment-slot scratch is sized for it
-__host__ __device__ constexpr int kernel_threads(int trace) { return trace == C8PH_TRACE_NUMERIC ? 256 : C8PH_THREADS; }
+#ifndef C8PH_THREADS_WIDE
+#define C8PH_THREADS_WIDE 640   // variants that spill at 80 registers: 20 warps at 96 registers (5 x 128 threads; 672 / 704 are rounded up to 768 by ptxas)
+#endif
+// Cherenkov variants with every switch at run time (SPEC = 0) and the 16-texel flat-plane table variant run 640 threads:
+// 15.8 -> 14.1 ms and 16.1 -> 13.4 ms on 2e6 cfg4 segments; every other compiled variant and fluorescence are faster at 768
+// (profiles/r2_extras.md)
+__host__ __device__ constexpr int kernel_threads(int emit, int trace, int spec)
+{
+    return trace == C8PH_TRACE_NUMERIC ? 256
+         : ((spec == 0 && emit == C8PH_EMIT_CHERENKOV) || (spec & 64) != 0) ? C8PH_THREADS_WIDE : C8PH_THREADS;
+}
 __host__ __device__ constexpr int kernel_min_blocks(int trace) { return trace == C8PH_TRACE_NUMERIC ? 2 : C8PH_MIN_BLOCKS; }
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
 constexpr double kC = 0.299792458;               // m / ns
@@ -653,10 +663,11 @@ enum { WC_BELOW = 0, WC_LV1, WC_EMITTING, WC_CLIPPED, WC_NONFINITE, WC_EMITTED, 
 constexpr int kSpecBase = 1, kSpecFlat = 2, kSpecExt = 4, kSpecDisp = 8, kSpecEff = 16, kSpecOpt = 32, kSpecFlatTab = 64,
               kSpecNoGrid = 128;     // production setting without a ground histogram (telescope spheres only: BASELINE configs[2])
 template <int EMIT, int TRACE, bool SPH, int SPEC>
-__global__ void __launch_bounds__(kernel_threads(TRACE), kernel_min_blocks(TRACE))
+__global__ void __launch_bounds__(kernel_threads(EMIT, TRACE, SPEC), kernel_min_blocks(TRACE))
 k_emit_propagate(const __grid_constant__ KArgs a)
 {
-    constexpr int kWarps = kernel_threads(TRACE) / 32;
+    static_assert(kSpecFlatTab == 64, "kernel_threads() names the flat-plane-table bit by value");
+    constexpr int kWarps = kernel_threads(EMIT, TRACE, SPEC) / 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
     __shared__ unsigned long long s_cnt[WC_N];               // event counters of the CTA (shared-memory atomics, rare)
@@ -2013,10 +2024,19 @@ __global__ void __launch_bounds__(128) k_build_table_cyl(const __grid_constant__
     a.cyl[idx] = out;
 }
 
+// dynamic shared memory of a variant with `threads` threads: [staged n(h) tables] + one candidate queue per warp
+size_t smem_for(const KArgs &a, int threads)
+{
+    size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
+    if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
+    return tables + (size_t)(threads / 32) * kQueue * Q_WORDS * sizeof(float);
+}
+
 template <int EMIT, int TRACE, bool SPH, int SPEC>
-cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
+cudaError_t launch_one(const KArgs &a, int n_sm, cudaStream_t st)
 {
     auto kern = k_emit_propagate<EMIT, TRACE, SPH, SPEC>;
+    const size_t smem = smem_for(a, kernel_threads(EMIT, TRACE, SPEC));
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     {
@@ -2024,7 +2044,7 @@ cudaError_t launch_one(const KArgs &a, int n_sm, size_t smem, cudaStream_t st)
         if (cv) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv));
     }
     int per_sm = 0;
-    constexpr int kThreads = kernel_threads(TRACE), kWarps = kThreads / 32;
+    constexpr int kThreads = kernel_threads(EMIT, TRACE, SPEC), kWarps = kThreads / 32;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
@@ -2045,11 +2065,9 @@ size_t segment_slot_bytes(int n_sm)
     return (size_t)n_sm * kMaxWarpsPerSM * 32 * sizeof(SegSlot);
 }
 
-size_t emit_smem_bytes(const KArgs &a)
+size_t emit_smem_bytes(const KArgs &a)               // upper bound over the variants of this (emit, trace): host-side validation
 {
-    size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
-    if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
-    return tables + (size_t)(kernel_threads(a.run.trace) / 32) * kQueue * Q_WORDS * sizeof(float);
+    return smem_for(a, std::max(kernel_threads(a.run.emit, a.run.trace, 0), kernel_threads(a.run.emit, a.run.trace, kSpecBase)));
 }
 
 // SPEC mask of the call: 0 unless it matches the switches the SPEC != 0 variants are compiled for,
@@ -2071,18 +2089,17 @@ static int array_production_setting(const KArgs &a)
 
 cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 {
-    const size_t smem = emit_smem_bytes(a);
     const bool sph = a.atm.model >= C8PH_ATM_SPHERICAL;
     const int spec = array_production_setting(a);
     if (spec == kSpecBase)
-        return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase>(a, n_sm, smem, st)
-                   : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, kSpecBase>(a, n_sm, smem, st);
+        return sph ? launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase>(a, n_sm, st)
+                   : launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, false, kSpecBase>(a, n_sm, st);
     // production setting + optional features (spherical model): the combinations that are compiled
 #if C8PH_PROD_ONLY
 #define C8_SPEC(M)
 #else
 #define C8_SPEC(M) \
-    if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, smem, st);
+    if (sph && spec == (kSpecBase | (M))) return launch_one<C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE, true, kSpecBase | (M)>(a, n_sm, st);
 #endif
     C8_SPEC(kSpecNoGrid)
     C8_SPEC(kSpecFlat)
@@ -2101,7 +2118,7 @@ cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st)
 #undef C8_SPEC
 #define C8_CASE(E, T)                                                             \
     if (a.run.emit == E && a.run.trace == T)                                      \
-        return sph ? launch_one<E, T, true, 0>(a, n_sm, smem, st) : launch_one<E, T, false, 0>(a, n_sm, smem, st);
+        return sph ? launch_one<E, T, true, 0>(a, n_sm, st) : launch_one<E, T, false, 0>(a, n_sm, st);
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_STRAIGHT)
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_NUMERIC)
     C8_CASE(C8PH_EMIT_CHERENKOV, C8PH_TRACE_TABLE)
