@@ -100,10 +100,23 @@ constexpr int kMaxWarpsPerSM = 64;                             // hardware limit
 // Cherenkov variants with every switch at run time (SPEC = 0) and the 16-texel flat-plane table variant run 640 threads:
 // 15.8 -> 14.1 ms and 16.1 -> 13.4 ms on 2e6 cfg4 segments; every other compiled variant and fluorescence are faster at 768
 // (profiles/r2_extras.md)
+#ifndef C8PH_THREADS_DENSE
+#define C8PH_THREADS_DENSE 896  // 28 warps at 72 registers: the production variants without optional per-photon features
+#endif
+#ifndef C8PH_QUEUE_COMPACT
+#define C8PH_QUEUE_COMPACT 1    // 1: 56-byte queue entries in the SPEC != 0 variants (needs the default queue knobs)
+#endif
+__host__ __device__ constexpr bool queue_compact(int spec)
+{
+    return C8PH_QUEUE_COMPACT && C8PH_QUEUE_LANE_ATOMS && C8PH_QUEUE_VOTE && !C8PH_QUEUE_CONVERGED && spec != 0;
+}
+__host__ __device__ constexpr int queue_words(int spec) { return queue_compact(spec) ? 14 : 16; }
 __host__ __device__ constexpr int kernel_threads(int emit, int trace, int spec)
 {
+    // spec 1 / 17 / 129: base, + efficiency, without ground grid
     return trace == C8PH_TRACE_NUMERIC ? 256
-         : ((spec == 0 && emit == C8PH_EMIT_CHERENKOV) || (spec & 64) != 0) ? C8PH_THREADS_WIDE : C8PH_THREADS;
+         : ((spec == 0 && emit == C8PH_EMIT_CHERENKOV) || (spec & 64) != 0) ? C8PH_THREADS_WIDE
+         : (queue_compact(spec) && (spec == 1 || spec == 17 || spec == 129)) ? C8PH_THREADS_DENSE : C8PH_THREADS;
 }
 __host__ __device__ constexpr int kernel_min_blocks(int trace) { return trace == C8PH_TRACE_NUMERIC ? 2 : C8PH_MIN_BLOCKS; }
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
@@ -190,6 +203,11 @@ static_assert(sizeof(SegHot) == 112 && sizeof(SegCold) == 64 && sizeof(SegSlot) 
 // entry = 4 x float4: (x, y, ux, uy) (uz, s, q w_z, dt) (1/lambda, weight, eta_e, h_e) (dd, cos zenith, cell, j<<5|slot)
 constexpr int Q_WORDS = 16;
 constexpr int kQueue = 64;                       // ring entries per warp (a drain leaves < 32)
+// compact entry of the production variants (56 B, three float4 planes + one float2 plane per warp): the weight is the
+// bunch weight (roulette mode) and h_e is recomputed from s and the segment slot in finish(), bit for bit:
+// (x, y, ux, uy) (uz, s, q w_z, dt) (1/lambda, eta_e, dd, cos zenith) (cell, j<<5|slot)
+// 28 queues of 3.5 KB = 98 KB fit the 100 KB carve-out that 24 queues of 4 KB fill: 28 warps per SM with the same L1
+constexpr int Q_WORDS_COMPACT = 14;
 
 template <typename T>
 __device__ __forceinline__ void copy16(T *dst, const T *src)
@@ -688,7 +706,12 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     float *s_aexp = s_dxv + (STAGED ? atm.n_pad : 0);       // aerosol column A(h_k) = (H/L) exp(-h_k/H), staged only with aerosol
     const bool aer_staged = STAGED && atm.aer_L > 0.f;
     float *s_end = s_aexp + (aer_staged ? atm.n_pad : 0);
-    float4 *s_q = reinterpret_cast<float4 *>(s_end) + warp * (kQueue * 4);   // s_q[slot * 4 + part]
+    constexpr bool QC = queue_compact(SPEC);
+    constexpr int QW = queue_words(SPEC);
+    static_assert(QW == (QC ? Q_WORDS_COMPACT : Q_WORDS), "queue entry size");
+    // 16-word entries: s_q[slot * 4 + part]; compact: planes s_q[part * kQueue + slot] (part 0..2) and s_q3[slot]
+    float4 *s_q = reinterpret_cast<float4 *>(reinterpret_cast<unsigned char *>(s_end) + (size_t)warp * (kQueue * QW * 4));
+    float2 *s_q3 = reinterpret_cast<float2 *>(s_q + 3 * kQueue);
 #if !C8PH_QUEUE_CONVERGED
     __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
 #endif
@@ -790,9 +813,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // ballot-compacted record store.  Called warp-converged; `act` marks the lanes that carry a photon.
     auto finish = [&](bool act, float4 q0, float4 q1, float4 q2, float4 q3) {
         const float ux = q0.z, uy = q0.w, uz = q1.x, s = q1.y, qw = q1.z, dt = q1.w;
-        const float lam_inv = q2.x, wgt = q2.y, eta_e = q2.z, h_e = q2.w, dd = q3.x, cz = q3.y;
+        const float lam_inv = q2.x, wgt = q2.y, eta_e = q2.z, dd = q3.x, cz = q3.y;
         int cell = __float_as_int(q3.z);
         const uint32_t jslot = __float_as_uint(q3.w);
+        float h_e = q2.w;
+        if (QC) {                                             // compact entry: the emission height from s, as the photon loop formed it
+            const SegHot *shq = &(g_slot + (jslot & 31u))->h;
+            h_e = fmaf(s, fmaf(s, shq->k2, shq->cA), shq->hA);
+        }
         int tel = -1;
         float uax = ux, uay = uy, uaz = uz, t_arr = 0.f;
         float rx_out = 0.f, ry_out = 0.f;                     // record position (ground plane, or camera plane with optics)
@@ -972,9 +1000,16 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #endif
         while (n >= 32 || (all && n > 0)) {
             const int take = n < 32 ? n : 32;
-            const float4 *e = s_q + ((q_head + lane) & (kQueue - 1)) * 4;
             const bool act = lane < take;
-            finish(act, e[0], e[1], e[2], e[3]);
+            if (QC) {
+                const int qi = (q_head + lane) & (kQueue - 1);
+                const float4 p0 = s_q[qi], p1 = s_q[kQueue + qi], p2 = s_q[2 * kQueue + qi];
+                const float2 p3 = s_q3[qi];
+                finish(act, p0, p1, make_float4(p2.x, hc.w, p2.y, 0.f), make_float4(p2.z, p2.w, p3.x, p3.y));
+            } else {
+                const float4 *e = s_q + ((q_head + lane) & (kQueue - 1)) * 4;
+                finish(act, e[0], e[1], e[2], e[3]);
+            }
             q_head = (q_head + take) & (kQueue - 1);
             n -= take;
             __syncwarp();
@@ -1641,6 +1676,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #if C8PH_QUEUE_VOTE
                     qfull = qb >= 31;
 #endif
+                    if (QC) {
+                        const int qi = (q_head + qb) & (kQueue - 1);
+                        s_q[qi] = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
+                        s_q[kQueue + qi] = make_float4(uz, s, q * wz, dt);
+                        s_q[2 * kQueue + qi] = make_float4(lam_inv, eta_e, dd, cz);
+                        s_q3[qi] = make_float2(__int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+                        break;
+                    }
                     float4 *e = s_q + ((q_head + qb) & (kQueue - 1)) * 4;
 #else
                     const unsigned am = __activemask();
@@ -2025,18 +2068,18 @@ __global__ void __launch_bounds__(128) k_build_table_cyl(const __grid_constant__
 }
 
 // dynamic shared memory of a variant with `threads` threads: [staged n(h) tables] + one candidate queue per warp
-size_t smem_for(const KArgs &a, int threads)
+size_t smem_for(const KArgs &a, int threads, int q_words)
 {
     size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
     if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
-    return tables + (size_t)(threads / 32) * kQueue * Q_WORDS * sizeof(float);
+    return tables + (size_t)(threads / 32) * kQueue * q_words * sizeof(float);
 }
 
 template <int EMIT, int TRACE, bool SPH, int SPEC>
 cudaError_t launch_one(const KArgs &a, int n_sm, cudaStream_t st)
 {
     auto kern = k_emit_propagate<EMIT, TRACE, SPH, SPEC>;
-    const size_t smem = smem_for(a, kernel_threads(EMIT, TRACE, SPEC));
+    const size_t smem = smem_for(a, kernel_threads(EMIT, TRACE, SPEC), queue_words(SPEC));
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     {
@@ -2067,7 +2110,8 @@ size_t segment_slot_bytes(int n_sm)
 
 size_t emit_smem_bytes(const KArgs &a)               // upper bound over the variants of this (emit, trace): host-side validation
 {
-    return smem_for(a, std::max(kernel_threads(a.run.emit, a.run.trace, 0), kernel_threads(a.run.emit, a.run.trace, kSpecBase)));
+    return std::max(smem_for(a, kernel_threads(a.run.emit, a.run.trace, 0), queue_words(0)),
+                    smem_for(a, kernel_threads(a.run.emit, a.run.trace, kSpecBase), queue_words(kSpecBase)));
 }
 
 // SPEC mask of the call: 0 unless it matches the switches the SPEC != 0 variants are compiled for,
