@@ -101,7 +101,7 @@ constexpr int kMaxWarpsPerSM = 64;                             // hardware limit
 // 15.8 -> 14.1 ms and 16.1 -> 13.4 ms on 2e6 cfg4 segments; every other compiled variant and fluorescence are faster at 768
 // (profiles/r2_extras.md)
 #ifndef C8PH_THREADS_DENSE
-#define C8PH_THREADS_DENSE 896  // 28 warps at 72 registers: the production variants without optional per-photon features
+#define C8PH_THREADS_DENSE 896  // 28 warps at 72 registers: the compiled variants with 56-byte queue entries
 #endif
 #ifndef C8PH_QUEUE_COMPACT
 #define C8PH_QUEUE_COMPACT 1    // 1: 56-byte queue entries in the SPEC != 0 variants (needs the default queue knobs)
@@ -113,10 +113,11 @@ __host__ __device__ constexpr bool queue_compact(int spec)
 __host__ __device__ constexpr int queue_words(int spec) { return queue_compact(spec) ? 14 : 16; }
 __host__ __device__ constexpr int kernel_threads(int emit, int trace, int spec)
 {
-    // spec 1 / 17 / 129: base, + efficiency, without ground grid
+    // 896 threads: the compiled variants without the analytic flat-plane step (bit 2) and the optics (bit 32), which
+    // gain nothing from it (profiles/r2_extras.md)
     return trace == C8PH_TRACE_NUMERIC ? 256
          : ((spec == 0 && emit == C8PH_EMIT_CHERENKOV) || (spec & 64) != 0) ? C8PH_THREADS_WIDE
-         : (queue_compact(spec) && (spec == 1 || spec == 17 || spec == 129)) ? C8PH_THREADS_DENSE : C8PH_THREADS;
+         : (queue_compact(spec) && (spec & (2 | 32)) == 0) ? C8PH_THREADS_DENSE : C8PH_THREADS;
 }
 __host__ __device__ constexpr int kernel_min_blocks(int trace) { return trace == C8PH_TRACE_NUMERIC ? 2 : C8PH_MIN_BLOCKS; }
 constexpr float kInvC = 1.0f / 0.299792458f;     // ns per metre
@@ -684,7 +685,7 @@ template <int EMIT, int TRACE, bool SPH, int SPEC>
 __global__ void __launch_bounds__(kernel_threads(EMIT, TRACE, SPEC), kernel_min_blocks(TRACE))
 k_emit_propagate(const __grid_constant__ KArgs a)
 {
-    static_assert(kSpecFlatTab == 64, "kernel_threads() names the flat-plane-table bit by value");
+    static_assert(kSpecFlat == 2 && kSpecOpt == 32 && kSpecFlatTab == 64, "kernel_threads() names the feature bits by value");
     constexpr int kWarps = kernel_threads(EMIT, TRACE, SPEC) / 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
