@@ -58,7 +58,7 @@
 #define C8PH_HIT_RING 1         // 1: a point outside the hit grid is clamped into the grid's ring of empty border cells instead of being tested
 #endif
 #ifndef C8PH_SLOT_PREFETCH
-#define C8PH_SLOT_PREFETCH 1    // 1: the next emitting segment's slot (two 128 B lines) is prefetched into L1 while the current one runs
+#define C8PH_SLOT_PREFETCH 0    // 1: the next emitting segment's slot (two 128 B lines) is prefetched into L1 while the current one runs (measured: +0.3 % time)
 #endif
 #ifndef C8PH_HIT_PREFETCH
 #define C8PH_HIT_PREFETCH 0     // 1: a lane that queues a telescope candidate prefetches the hit cell's first-telescope record (finish() reads it)
@@ -83,10 +83,11 @@ namespace c8ph {
 
 namespace {
 
-// Launch shape.  Table / straight tracing: ONE CTA of 768 threads per SM (24 warps at 80 registers): the per-warp candidate
-// queues (4 KB each) plus one CTA's static and reserved shared memory then fit the 100 KB carve-out, which leaves
-// 156 KB of L1 instead of 124 KB with three CTAs of 256 threads (measured: profiles/r2_ab.md).  The layered-sum variant
-// stages 80-120 KB of tables per CTA and runs two CTAs of 256 threads.
+// Launch shape.  Table / straight tracing: ONE CTA per SM whose per-warp candidate queues plus static and reserved shared
+// memory fit the 100 KB carve-out, which leaves 156 KB of L1 (124 KB with three CTAs of 256 threads: +4 % time; measured
+// in profiles/r2_ab.md): 768 threads (24 warps at 80 registers, 4 KB queues) by default, 896 / 640 threads for the
+// variants kernel_threads() names.  The layered-sum variant stages 80-120 KB of tables per CTA and runs two CTAs of 256
+// threads.
 #ifndef C8PH_THREADS
 #define C8PH_THREADS 768
 #endif
