@@ -711,11 +711,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     constexpr bool QC = queue_compact(SPEC);
     constexpr int QW = queue_words(SPEC);
     static_assert(QW == (QC ? Q_WORDS_COMPACT : Q_WORDS), "queue entry size");
+    static_assert(kQueue == 64, "the push's plane offsets (16 + 1024 k, 3088) are written for 64 entries");
     // 16-word entries: s_q[slot * 4 + part]; compact: planes s_q[part * kQueue + slot] (part 0..2) and s_q3[slot]
-    float4 *s_q = reinterpret_cast<float4 *>(reinterpret_cast<unsigned char *>(s_end) + (size_t)warp * (kQueue * QW * 4));
+    // compact layout: the warp's fill count sits in the 16 bytes in front of its planes, so that the push forms every
+    // address from the one register that holds the count's shared-memory address (kQueueHead bytes per warp)
+    constexpr int kQueueHead = QC ? 16 : 0;
+    unsigned char *s_qblock = reinterpret_cast<unsigned char *>(s_end) + (size_t)warp * (kQueue * QW * 4 + kQueueHead);
+    float4 *s_q = reinterpret_cast<float4 *>(s_qblock + kQueueHead);
     float2 *s_q3 = reinterpret_cast<float2 *>(s_q + 3 * kQueue);
 #if !C8PH_QUEUE_CONVERGED
-    __shared__ int s_qn[kWarps];                              // entries waiting in the warp's queue
+    __shared__ int s_qn_static[QC ? 1 : kWarps];              // entries waiting in the warp's queue (16-word layout)
+    int *const s_qn_w = QC ? reinterpret_cast<int *>(s_qblock) : &s_qn_static[warp];
+    const uint32_t qn_addr = smem_u32(s_qn_w);
 #endif
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
     SegSlot *g_slot = static_cast<SegSlot *>(run.slots) + ((size_t)blockIdx.x * kWarps + warp) * 32;
@@ -723,7 +730,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     if (threadIdx.x < WC_N) s_cnt[threadIdx.x] = 0ull;
     __syncthreads();
 #if !C8PH_QUEUE_CONVERGED
-    if (lane == 0) s_qn[warp] = 0;
+    if (lane == 0) *s_qn_w = 0;
 #endif
     // ---- layered-sum variant: stage the atmosphere tables with one TMA bulk copy per array
     if (STAGE_ETA) {
@@ -998,7 +1005,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #if C8PH_QUEUE_CONVERGED
         int n = q_n;
 #else
-        int n = s_qn[warp];
+        int n = *s_qn_w;
 #endif
         while (n >= 32 || (all && n > 0)) {
             const int take = n < 32 ? n : 32;
@@ -1018,7 +1025,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #if C8PH_QUEUE_CONVERGED
             q_n = n;
 #else
-            if (lane == 0) s_qn[warp] = n;
+            if (lane == 0) *s_qn_w = n;
             __syncwarp();
 #endif
         }
@@ -1265,8 +1272,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             const int n_iter = (sg.N + 31) >> 5;
             if (iters_pending + n_iter > 60000) flush_counts();
             iters_pending += n_iter;
-            for (int it = 0; it < n_iter; ++it) {
-                const int j = it * 32 + lane;
+            // the loop variable is the queue entry's last word, js = j << 5 | slot of the segment (j = 32 it + lane): the photon
+            // index is one shift away and neither the lane index nor the slot number needs a register of its own
+            for (uint32_t js = ((uint32_t)lane << 5) | (uint32_t)src; js < ((uint32_t)n_iter << 10); js += 1024u) {
+                const int j = (int)(js >> 5);
 #if C8PH_QUEUE_VOTE && C8PH_QUEUE_LANE_ATOMS && !C8PH_QUEUE_CONVERGED
                 bool qfull = false;
 #endif
@@ -1275,7 +1284,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                 float4 qe0, qe1, qe2, qe3;                            // defined where qpush is set
 #endif
                 // one photon per lane; every cut leaves through the same exit (one reconvergence point)
-                if (j < sg.N) do {
+                if (js < ((uint32_t)sg.N << 5)) do {                  // j < N
                     const uint4 rn = philox4x32_10((uint32_t)j, sg.id_lo, sg.id_hi, 0u, hc.key);
                     const float u1 = u01(rn.y), u2 = u01(rn.z);
                     // a6: emission point on the track, its height and n(h_e) (Listing 4.1)
@@ -1661,7 +1670,7 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     qe0 = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
                     qe1 = make_float4(uz, s, q * wz, dt);
                     qe2 = make_float4(lam_inv, wgt, eta_e, h_e);
-                    qe3 = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+                    qe3 = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(js));
                     qpush = true;
 #else
                     // slots are handed out per group of lanes
@@ -1674,16 +1683,18 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #endif
 #if C8PH_QUEUE_LANE_ATOMS
                     int qb;                                              // inline asm: no compiler-generated warp aggregation
-                    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])) : "memory");
+                    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(qb) : "r"(qn_addr) : "memory");
 #if C8PH_QUEUE_VOTE
                     qfull = qb >= 31;
 #endif
                     if (QC) {
-                        const int qi = (q_head + qb) & (kQueue - 1);
-                        s_q[qi] = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
-                        s_q[kQueue + qi] = make_float4(uz, s, q * wz, dt);
-                        s_q[2 * kQueue + qi] = make_float4(lam_inv, eta_e, dd, cz);
-                        s_q3[qi] = make_float2(__int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+                        const uint32_t qi = (uint32_t)(q_head + qb) & (uint32_t)(kQueue - 1);
+                        const uint32_t a4 = qn_addr + qi * 16u, a2 = qn_addr + qi * 8u;     // + 16: past the fill count
+                        const float e0x = f_opt ? cx : xg, e0y = f_opt ? cy : yg;
+                        asm volatile("st.shared.v4.f32 [%0+16], {%1, %2, %3, %4};" ::"r"(a4), "f"(e0x), "f"(e0y), "f"(ux), "f"(uy) : "memory");
+                        asm volatile("st.shared.v4.f32 [%0+1040], {%1, %2, %3, %4};" ::"r"(a4), "f"(uz), "f"(s), "f"(q * wz), "f"(dt) : "memory");
+                        asm volatile("st.shared.v4.f32 [%0+2064], {%1, %2, %3, %4};" ::"r"(a4), "f"(lam_inv), "f"(eta_e), "f"(dd), "f"(cz) : "memory");
+                        asm volatile("st.shared.v2.b32 [%0+3088], {%1, %2};" ::"r"(a2), "r"(cell), "r"(js) : "memory");
                         break;
                     }
                     float4 *e = s_q + ((q_head + qb) & (kQueue - 1)) * 4;
@@ -1692,14 +1703,14 @@ k_emit_propagate(const __grid_constant__ KArgs a)
                     const int leader = __ffs(am) - 1;
                     int qb = 0;
                     if (lane == leader)                                  // plain ATOMS: the group is already aggregated
-                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(qb) : "r"(smem_u32(&s_qn[warp])), "r"(__popc(am)) : "memory");
+                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(qb) : "r"(qn_addr), "r"(__popc(am)) : "memory");
                     qb = __shfl_sync(am, qb, leader);
                     float4 *e = s_q + ((q_head + qb + __popc(am & ((1u << lane) - 1u))) & (kQueue - 1)) * 4;
 #endif
                     e[0] = f_opt ? make_float4(cx, cy, ux, uy) : make_float4(xg, yg, ux, uy);
                     e[1] = make_float4(uz, s, q * wz, dt);
                     e[2] = make_float4(lam_inv, wgt, eta_e, h_e);
-                    e[3] = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(((uint32_t)j << 5) | (uint32_t)src));
+                    e[3] = make_float4(dd, cz, __int_as_float(cell), __uint_as_float(js));
 #endif
                 } while (false);
 #if C8PH_QUEUE_CONVERGED
@@ -2074,7 +2085,7 @@ size_t smem_for(const KArgs &a, int threads, int q_words)
 {
     size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
     if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
-    return tables + (size_t)(threads / 32) * kQueue * q_words * sizeof(float);
+    return tables + (size_t)(threads / 32) * ((size_t)kQueue * q_words * sizeof(float) + (q_words == Q_WORDS_COMPACT ? 16u : 0u));
 }
 
 template <int EMIT, int TRACE, bool SPH, int SPEC>
