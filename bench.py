@@ -50,20 +50,20 @@ I_ALG_SURVEY_PER_PHOTON = 250.0
 # page profiles/r2_cfg4_source.csv.gz (tests/test_roofline_audit.py checks these numbers against it).  Not counted: the
 # loop slot, the queue push, LV2 list walks, candidates that miss, partly filled drains, idle lanes.
 I_ALG_OWN = {
-    "segment": 1114.6,    # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor, slot store (per segment)
-    "emitted": 214.0,     # a5-a12: Philox4x32-10, uniforms, emission point, n(h), cone, sincos, straight line, LV2 box, zenith,
+    "segment": 1127.2,    # a1-a4: SoA ingest, fp64 yield / LV1 / Rodrigues / anchor, slot store (per segment)
+    "emitted": 215.0,     # a5-a12: Philox4x32-10, uniforms, emission point, n(h), cone, sincos, straight line, LV2 box, zenith,
                           #         acos, bilinear float4 lookup, transmission, roulette
     "landed": 50.0,       # a15 + a14 pre-test: corrected position, telescope-grid cell + smallest key, bin index
     "in_grid": 6.0,       # a15: bin address + RED.ADD.F32
-    "tel_hit": 156.0,     # a13/a14/a16: finish() (time, arrival direction, sphere search, record), once per hit
+    "tel_hit": 160.0,     # a13/a14/a16: finish() (time, arrival direction, sphere search, record), once per hit
 }
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_emit_propagate launch on the N=1 workload, from the
 # ncu --set full capture summarised in profiles/r2_cfg4_final.md.  Reported as `roofline.traffic` only when the run is
 # that workload (cfg4, 1e7 segments); otherwise null.
-NCU_TRAFFIC_BYTES_CFG4 = 0.680863744e9 + 5.121840e9
-NCU_ISSUE_SLOTS_BUSY_CFG4 = 0.7121                 # smsp issue slots busy of the same capture
+NCU_TRAFFIC_BYTES_CFG4 = 0.721679872e9 + 5.245904e9
+NCU_ISSUE_SLOTS_BUSY_CFG4 = 0.7553                 # smsp issue slots busy of the same capture
 
 
 def _stage_population(cnt: dict) -> dict:
