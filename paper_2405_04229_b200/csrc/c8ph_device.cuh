@@ -132,6 +132,7 @@ struct DevRun {
     c8ph_outputs out;               // DEVICE pointers
     unsigned long long *cursor;     // DEVICE work cursor (segments)
     void *slots;                    // DEVICE scratch: 32 prepared-segment slots per resident warp
+    void *qring;                    // DEVICE scratch: candidate queues of the resident warps when they live in global memory (C8PH_QUEUE_GLOBAL)
     int segs_per_grab;              // segments one warp prepares per grab (1..32)
 };
 
@@ -192,6 +193,7 @@ cudaError_t launch_emit_propagate(const KArgs &a, int n_sm, cudaStream_t st);
 cudaError_t launch_build_table(const TableBuildArgs &a, cudaStream_t st);
 size_t emit_smem_bytes(const KArgs &a);
 size_t segment_slot_bytes(int n_sm);
+size_t queue_ring_bytes(int n_sm);
 cudaError_t launch_substep_plan(const SubstepArgs &a, long long *block_sums, cudaStream_t st);
 cudaError_t launch_substep_fill(const SubstepArgs &a, int n_sm, cudaStream_t st);
 size_t substep_scratch_elems(long long n);

@@ -116,7 +116,7 @@ extern "C" int c8ph_create(c8ph_ctx **out, int cuda_device)
     if ((e = cudaSetDevice(cuda_device)) != cudaSuccess ||
         (e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_cursor, sizeof(unsigned long long))) != cudaSuccess ||
-        (e = cudaMalloc(&ctx->d_slots, segment_slot_bytes(ctx->n_sm))) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_slots, segment_slot_bytes(ctx->n_sm) + queue_ring_bytes(ctx->n_sm))) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_bsums, kSubstepBlockSums * sizeof(long long))) != cudaSuccess ||
         (e = cudaEventCreate(&ctx->ev0)) != cudaSuccess || (e = cudaEventCreate(&ctx->ev1)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&ctx->ev_done, cudaEventDisableTiming)) != cudaSuccess) {
@@ -835,6 +835,7 @@ static int make_args(c8ph_ctx *ctx, const c8ph_segments *s, int64_t n_seg, int64
     r.seg = *s; r.out = *o;
     r.cursor = ctx->d_cursor;
     r.slots = ctx->d_slots;
+    r.qring = static_cast<unsigned char *>(ctx->d_slots) + segment_slot_bytes(ctx->n_sm);
     const long long warps = (long long)ctx->n_sm * 2 * 8;
     long long g = n_seg / (warps * 4);
     r.segs_per_grab = (int)std::min<long long>(32, std::max<long long>(1, g));

@@ -104,6 +104,9 @@ constexpr int kMaxWarpsPerSM = 64;                             // hardware limit
 #ifndef C8PH_THREADS_DENSE
 #define C8PH_THREADS_DENSE 896  // 28 warps at 72 registers: the compiled variants with 56-byte queue entries
 #endif
+#ifndef C8PH_QUEUE_GLOBAL
+#define C8PH_QUEUE_GLOBAL 0     // 1: the compact candidate queues live in global memory (L2, st/ld .cg) instead of shared memory: no carve-out
+#endif
 #ifndef C8PH_QUEUE_COMPACT
 #define C8PH_QUEUE_COMPACT 1    // 1: 56-byte queue entries in the SPEC != 0 variants (needs the default queue knobs)
 #endif
@@ -716,12 +719,16 @@ k_emit_propagate(const __grid_constant__ KArgs a)
     // compact layout: the warp's fill count sits in the 16 bytes in front of its planes, so that the push forms every
     // address from the one register that holds the count's shared-memory address (kQueueHead bytes per warp)
     constexpr int kQueueHead = QC ? 16 : 0;
-    unsigned char *s_qblock = reinterpret_cast<unsigned char *>(s_end) + (size_t)warp * (kQueue * QW * 4 + kQueueHead);
+    constexpr bool QG = QC && C8PH_QUEUE_GLOBAL;
+    constexpr uint32_t kQBlock = kQueue * QW * 4 + kQueueHead;      // bytes per warp
+    unsigned char *const q_cta = QG ? static_cast<unsigned char *>(run.qring) + (size_t)blockIdx.x * (kWarps * kQBlock)
+                                    : reinterpret_cast<unsigned char *>(s_end);
+    unsigned char *s_qblock = q_cta + (size_t)warp * kQBlock;
     float4 *s_q = reinterpret_cast<float4 *>(s_qblock + kQueueHead);
     float2 *s_q3 = reinterpret_cast<float2 *>(s_q + 3 * kQueue);
 #if !C8PH_QUEUE_CONVERGED
-    __shared__ int s_qn_static[QC ? 1 : kWarps];              // entries waiting in the warp's queue (16-word layout)
-    int *const s_qn_w = QC ? reinterpret_cast<int *>(s_qblock) : &s_qn_static[warp];
+    __shared__ int s_qn_static[(QC && !QG) ? 1 : kWarps];     // entries waiting in the warp's queue (16-word layout, global queues)
+    int *const s_qn_w = (QC && !QG) ? reinterpret_cast<int *>(s_qblock) : &s_qn_static[warp];
     const uint32_t qn_addr = smem_u32(s_qn_w);
 #endif
     // segment slots of this warp: global scratch owned by the context (L2-resident, re-read through L1)
@@ -1012,8 +1019,10 @@ k_emit_propagate(const __grid_constant__ KArgs a)
             const bool act = lane < take;
             if (QC) {
                 const int qi = (q_head + lane) & (kQueue - 1);
-                const float4 p0 = s_q[qi], p1 = s_q[kQueue + qi], p2 = s_q[2 * kQueue + qi];
-                const float2 p3 = s_q3[qi];
+                float4 p0, p1, p2;
+                float2 p3;
+                if (QG) { p0 = __ldcg(s_q + qi); p1 = __ldcg(s_q + kQueue + qi); p2 = __ldcg(s_q + 2 * kQueue + qi); p3 = __ldcg(s_q3 + qi); }
+                else { p0 = s_q[qi]; p1 = s_q[kQueue + qi]; p2 = s_q[2 * kQueue + qi]; p3 = s_q3[qi]; }
                 finish(act, p0, p1, make_float4(p2.x, hc.w, p2.y, 0.f), make_float4(p2.z, p2.w, p3.x, p3.y));
             } else {
                 const float4 *e = s_q + ((q_head + lane) & (kQueue - 1)) * 4;
@@ -1689,6 +1698,17 @@ k_emit_propagate(const __grid_constant__ KArgs a)
 #endif
                     if (QC) {
                         const uint32_t qi = (uint32_t)(q_head + qb) & (uint32_t)(kQueue - 1);
+                        if (QG) {
+                            // the warp's block from the count's address: (qn_addr - &s_qn_static[0]) / 4 = warp
+                            const uint32_t woff = (qn_addr - smem_u32(&s_qn_static[0])) * (kQBlock / 4u);
+                            unsigned char *g4 = q_cta + (woff + qi * 16u), *g2 = q_cta + (woff + qi * 8u);
+                            const float e0x = f_opt ? cx : xg, e0y = f_opt ? cy : yg;
+                            asm volatile("st.global.cg.v4.f32 [%0+16], {%1, %2, %3, %4};" ::"l"(g4), "f"(e0x), "f"(e0y), "f"(ux), "f"(uy) : "memory");
+                            asm volatile("st.global.cg.v4.f32 [%0+1040], {%1, %2, %3, %4};" ::"l"(g4), "f"(uz), "f"(s), "f"(q * wz), "f"(dt) : "memory");
+                            asm volatile("st.global.cg.v4.f32 [%0+2064], {%1, %2, %3, %4};" ::"l"(g4), "f"(lam_inv), "f"(eta_e), "f"(dd), "f"(cz) : "memory");
+                            asm volatile("st.global.cg.v2.b32 [%0+3088], {%1, %2};" ::"l"(g2), "r"(cell), "r"(js) : "memory");
+                            break;
+                        }
                         const uint32_t a4 = qn_addr + qi * 16u, a2 = qn_addr + qi * 8u;     // + 16: past the fill count
                         const float e0x = f_opt ? cx : xg, e0y = f_opt ? cy : yg;
                         asm volatile("st.shared.v4.f32 [%0+16], {%1, %2, %3, %4};" ::"r"(a4), "f"(e0x), "f"(e0y), "f"(ux), "f"(uy) : "memory");
@@ -2085,6 +2105,7 @@ size_t smem_for(const KArgs &a, int threads, int q_words)
 {
     size_t tables = a.run.trace == C8PH_TRACE_NUMERIC ? (size_t)a.atm.n_pad * 4u * (a.atm.aer_L > 0.f ? 3u : 2u) : 0u;
     if (C8PH_ETA_STAGED && a.run.trace == C8PH_TRACE_TABLE) tables = (size_t)a.atm.n_pad * 4u;
+    if (C8PH_QUEUE_GLOBAL && q_words == Q_WORDS_COMPACT) return tables;
     return tables + (size_t)(threads / 32) * ((size_t)kQueue * q_words * sizeof(float) + (q_words == Q_WORDS_COMPACT ? 16u : 0u));
 }
 
@@ -2115,6 +2136,11 @@ cudaError_t launch_one(const KArgs &a, int n_sm, cudaStream_t st)
 }
 
 }  // namespace
+
+size_t queue_ring_bytes(int n_sm)
+{
+    return C8PH_QUEUE_GLOBAL ? (size_t)n_sm * kMaxWarpsPerSM * (kQueue * Q_WORDS_COMPACT * 4 + 16) : 0;
+}
 
 size_t segment_slot_bytes(int n_sm)
 {
